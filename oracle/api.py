@@ -1,0 +1,200 @@
+"""ctypes loader and numpy marshalling for the CPU oracle (oracle/fcg_oracle.c).
+
+TEST INFRASTRUCTURE ONLY.  Importable from tests/, __graft_entry__.smoke() and the cpu_baseline /
+``--impl reference`` legs of bench.py -- never from the product package.  This module holds no
+arithmetic of the method: every number comes out of fcg_oracle.c.  It imports nothing from
+paper_1305_3625_b200.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+import threading
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = [os.path.join(_HERE, "fcg_oracle.c"), os.path.join(_HERE, "fcg_oracle_impl.h")]
+_LIB_PATH = os.path.join(_HERE, "libfcg_oracle.so")
+_lock = threading.Lock()
+_lib = None
+
+OK, NOT_CONVERGED, BREAKDOWN, NO_CANDIDATE = 0, 1, -4, -6
+
+
+def build(force: bool = False) -> str:
+    """Compile fcg_oracle.c with gcc (-O2, OpenMP, no FMA contraction) next to its source."""
+    newest = max(os.path.getmtime(p) for p in _SRC)
+    if force or not os.path.exists(_LIB_PATH) or os.path.getmtime(_LIB_PATH) < newest:
+        tmp = _LIB_PATH + f".tmp{os.getpid()}"
+        cmd = ["gcc", "-O2", "-fopenmp", "-ffp-contract=off", "-fPIC", "-shared", "-Wall",
+               _SRC[0], "-o", tmp, "-lm"]
+        subprocess.run(cmd, check=True, cwd=_HERE)
+        os.replace(tmp, _LIB_PATH)
+    return _LIB_PATH
+
+
+def lib() -> C.CDLL:
+    global _lib
+    with _lock:
+        if _lib is None:
+            _lib = C.CDLL(build())
+            _declare(_lib)
+    return _lib
+
+
+_vp, _i, _d, _ll = C.c_void_p, C.c_int, C.c_double, C.c_longlong
+
+
+def _declare(L: C.CDLL) -> None:
+    L.oracle_spectrum.argtypes = [_i, _vp]
+    L.oracle_spectrum.restype = None
+    L.oracle_dft2_brute.argtypes = [_i, _vp, _vp]
+    L.oracle_dft2_brute.restype = None
+    L.oracle_idft2_brute.argtypes = [_i, _vp, _vp]
+    L.oracle_idft2_brute.restype = None
+    L.oracle_conv_direct.argtypes = [_i, _vp, _vp, _vp]
+    L.oracle_conv_direct.restype = None
+    L.oracle_num_threads.restype = _i
+    L.oracle_set_num_threads.argtypes = [_i]
+    for suf in ("_f64", "_f32"):
+        f = getattr(L, "oracle_fft2" + suf)
+        f.argtypes = [_i, _vp, _i]; f.restype = _i
+        f = getattr(L, "oracle_apply" + suf)
+        f.argtypes = [_i, _vp, _vp, _vp, _vp]; f.restype = _i
+        f = getattr(L, "oracle_cg" + suf)
+        f.argtypes = [_i, _vp, _vp, _vp, _vp, _d, _i, C.POINTER(_i), C.POINTER(_d), _vp, _vp, _vp]
+        f.restype = _i
+        f = getattr(L, "oracle_break_step" + suf)
+        f.argtypes = [_ll, _vp, _vp, _vp, C.POINTER(_ll), C.POINTER(_d), C.POINTER(_d)]
+        f.restype = _i
+        f = getattr(L, "oracle_fracture" + suf)
+        f.argtypes = [_i, _vp, _vp, _vp, _vp, _vp, _i, _d, _i, _vp, _vp, _vp]
+        f.restype = _i
+
+
+def _suf(dtype) -> str:
+    dt = np.dtype(dtype)
+    if dt == np.float64:
+        return "_f64"
+    if dt == np.float32:
+        return "_f32"
+    raise TypeError(f"oracle supports float32/float64, got {dt}")
+
+
+def _arr(a, dtype, shape=None) -> np.ndarray:
+    a = np.ascontiguousarray(a, dtype=dtype)
+    if shape is not None and a.shape != shape:
+        raise ValueError(f"expected shape {shape}, got {a.shape}")
+    return a
+
+
+def _p(a: np.ndarray | None):
+    return None if a is None else a.ctypes.data_as(C.c_void_p)
+
+
+def num_threads() -> int:
+    return int(lib().oracle_num_threads())
+
+
+def set_num_threads(n: int) -> None:
+    lib().oracle_set_num_threads(int(n))
+
+
+def spectrum(L: int) -> np.ndarray:
+    s = np.empty((L, L), np.float64)
+    lib().oracle_spectrum(L, _p(s))
+    return s
+
+
+def dft2_brute(x: np.ndarray) -> np.ndarray:
+    L = x.shape[0]
+    x = _arr(x, np.float64, (L, L))
+    X = np.empty((L, L), np.complex128)
+    lib().oracle_dft2_brute(L, _p(x), _p(X))
+    return X
+
+
+def idft2_brute(X: np.ndarray) -> np.ndarray:
+    L = X.shape[0]
+    X = _arr(X, np.complex128, (L, L))
+    x = np.empty((L, L), np.complex128)
+    lib().oracle_idft2_brute(L, _p(X), _p(x))
+    return x
+
+
+def conv_direct(c: np.ndarray, x: np.ndarray) -> np.ndarray:
+    L = x.shape[0]
+    c = _arr(c, np.float64, (L, L)); x = _arr(x, np.float64, (L, L))
+    y = np.empty((L, L), np.float64)
+    lib().oracle_conv_direct(L, _p(c), _p(x), _p(y))
+    return y
+
+
+def fft2(x: np.ndarray, inverse: bool = False) -> np.ndarray:
+    """2D DFT of a complex (or real) L x L array in the precision of x (complex64/complex128)."""
+    x = np.asarray(x)
+    L = x.shape[0]
+    cdt = np.complex64 if x.dtype in (np.float32, np.complex64) else np.complex128
+    rdt = np.float32 if cdt == np.complex64 else np.float64
+    buf = np.array(x, dtype=cdt, order="C", copy=True).reshape(L, L)
+    st = getattr(lib(), "oracle_fft2" + _suf(rdt))(L, _p(buf), 1 if inverse else 0)
+    if st != 0:
+        raise ValueError("oracle_fft2: L must be a power of two")
+    return buf
+
+
+def apply(s, k, x) -> np.ndarray:
+    """y = k o x + F^-1(s o F x) in the dtype of x."""
+    x = np.asarray(x); dt = x.dtype; L = x.shape[0]
+    s = _arr(s, dt, (L, L)); k = _arr(k, dt, (L, L)); x = _arr(x, dt, (L, L))
+    y = np.empty((L, L), dt)
+    st = getattr(lib(), "oracle_apply" + _suf(dt))(L, _p(s), _p(k), _p(x), _p(y))
+    if st != 0:
+        raise ValueError("oracle_apply: bad argument")
+    return y
+
+
+def cg(s, k, f, u0, tol: float, maxit: int, history: bool = False, directions: bool = False):
+    """Returns dict(u, iters, relres, status[, hist][, P, R]); dtype taken from f."""
+    f = np.asarray(f); dt = f.dtype; L = f.shape[0]; N = L * L
+    s = _arr(s, dt, (L, L)); k = _arr(k, dt, (L, L)); f = _arr(f, dt, (L, L))
+    u = np.array(u0, dtype=dt, order="C", copy=True).reshape(L, L)
+    hist = np.full(maxit + 1, np.nan, np.float64) if history else None
+    P = np.zeros((maxit, N), dt) if directions else None
+    R = np.zeros((maxit, N), dt) if directions else None
+    it = C.c_int(0); rr = C.c_double(0.0)
+    st = getattr(lib(), "oracle_cg" + _suf(dt))(L, _p(s), _p(k), _p(f), _p(u), float(tol), int(maxit),
+                                                 C.byref(it), C.byref(rr), _p(hist), _p(P), _p(R))
+    out = dict(u=u, iters=int(it.value), relres=float(rr.value), status=int(st))
+    if history:
+        out["hist"] = hist[: it.value + 1]
+    if directions:
+        out["P"] = P[: it.value]; out["R"] = R[: it.value]
+    return out
+
+
+def break_step(k: np.ndarray, u, t):
+    """In-place on k (must be a C-contiguous float array). Returns (index, ratio, second, status)."""
+    dt = k.dtype
+    if not k.flags.c_contiguous:
+        raise ValueError("k must be C-contiguous (modified in place)")
+    u = _arr(u, dt); t = _arr(t, dt)
+    idx = C.c_longlong(-1); ratio = C.c_double(0.0); second = C.c_double(0.0)
+    st = getattr(lib(), "oracle_break_step" + _suf(dt))(k.size, _p(k), _p(u), _p(t),
+                                                         C.byref(idx), C.byref(ratio), C.byref(second))
+    return int(idx.value), float(ratio.value), float(second.value), int(st)
+
+
+def fracture(s, k, f, u, t, nsteps: int, tol: float, maxit: int):
+    """In-place on k and u. Returns dict(index[nsteps], iters[nsteps], gap[nsteps], steps)."""
+    dt = k.dtype; L = k.shape[0]
+    s = _arr(s, dt, (L, L)); f = _arr(f, dt, (L, L)); t = _arr(t, dt, (L, L))
+    if not (k.flags.c_contiguous and u.flags.c_contiguous and u.dtype == dt):
+        raise ValueError("k, u must be C-contiguous arrays of one dtype (modified in place)")
+    index = np.full(nsteps, -1, np.int64); iters = np.zeros(nsteps, np.int32)
+    gap = np.full(nsteps, np.nan, np.float64)
+    done = getattr(lib(), "oracle_fracture" + _suf(dt))(L, _p(s), _p(k), _p(f), _p(u), _p(t), int(nsteps),
+                                                        float(tol), int(maxit), _p(index), _p(iters), _p(gap))
+    return dict(index=index, iters=iters, gap=gap, steps=int(done))

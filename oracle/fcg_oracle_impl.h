@@ -1,0 +1,236 @@
+/*
+ * oracle/fcg_oracle_impl.h -- precision-generic body of the CPU oracle.
+ *
+ * TEST INFRASTRUCTURE ONLY.  Included twice by fcg_oracle.c, once with REAL=double (SUF=_f64)
+ * and once with REAL=float (SUF=_f32).  Shares no code with the CUDA path.
+ *
+ * Everything here is the plain definition or the paper's algorithm written out in the paper's
+ * order (PAPER.md = /root/reference/PAPER.md):
+ *   - Listing 4: cpyComplex -> forward 2D FFT -> elementMult with the static
+ *     spectrum -> inverse 2D FFT -> cpyReal; normalisation afterwards (Listing 3).
+ *   - Listing 2: un-preconditioned conjugate gradient.
+ *   - break rule: BASELINE.json configs[3] (the paper only says "bonds break").
+ *
+ * Precision reading S12: vectors, spectrum, twiddles and FFT arithmetic in
+ * REAL; dot-product accumulators and the CG scalars alpha, beta, rho in double for both REAL types.
+ */
+
+typedef struct { REAL re, im; } CPLX;
+
+/* ---- textbook iterative radix-2 complex FFT (bit reversal + log2 n butterfly stages) ------------
+ * X[k] = sum_j x[j] exp(sign * 2 pi i j k / n); sign = -1 forward, +1 inverse (unnormalised).
+ * tw[j] = exp(sign * 2 pi i j / n) for j < n/2, each evaluated with fp64 cos/sin of its own angle
+ * (no recurrence) and then rounded to REAL. */
+static void FN(make_twiddles)(CPLX* tw, int n, int sign)
+{
+    for (int j = 0; j < n / 2; ++j) {
+        double ang = (double)sign * 2.0 * M_PI * (double)j / (double)n;
+        tw[j].re = (REAL)cos(ang);
+        tw[j].im = (REAL)sin(ang);
+    }
+}
+
+static void FN(fft1d)(CPLX* x, int n, const CPLX* tw)
+{
+    /* bit-reversal permutation */
+    for (int i = 1, j = 0; i < n; ++i) {
+        int bit = n >> 1;
+        for (; j & bit; bit >>= 1) j ^= bit;
+        j ^= bit;
+        if (i < j) { CPLX t = x[i]; x[i] = x[j]; x[j] = t; }
+    }
+    /* butterfly stages, len = 2, 4, ..., n */
+    for (int len = 2; len <= n; len <<= 1) {
+        int half = len >> 1, step = n / len;
+        for (int base = 0; base < n; base += len) {
+            for (int j = 0; j < half; ++j) {
+                CPLX w = tw[j * step];
+                CPLX a = x[base + j], b = x[base + j + half];
+                CPLX wb;
+                wb.re = w.re * b.re - w.im * b.im;
+                wb.im = w.re * b.im + w.im * b.re;
+                x[base + j].re = a.re + wb.re;        x[base + j].im = a.im + wb.im;
+                x[base + j + half].re = a.re - wb.re; x[base + j + half].im = a.im - wb.im;
+            }
+        }
+    }
+}
+
+/* 2D transform of an L x L row-major complex array, in place: all rows, then all columns. */
+static void FN(fft2d)(CPLX* buf, int L, int sign)
+{
+    CPLX* tw = (CPLX*)malloc(sizeof(CPLX) * (size_t)(L / 2 + 1));
+    FN(make_twiddles)(tw, L, sign);
+#pragma omp parallel
+    {
+        CPLX* col = (CPLX*)malloc(sizeof(CPLX) * (size_t)L);
+#pragma omp for schedule(static)
+        for (int a = 0; a < L; ++a) FN(fft1d)(buf + (size_t)a * L, L, tw);
+#pragma omp for schedule(static)
+        for (int b = 0; b < L; ++b) {
+            for (int a = 0; a < L; ++a) col[a] = buf[(size_t)a * L + b];
+            FN(fft1d)(col, L, tw);
+            for (int a = 0; a < L; ++a) buf[(size_t)a * L + b] = col[a];
+        }
+        free(col);
+    }
+    free(tw);
+}
+
+/* Public: forward (sign=-1) or inverse (sign=+1, includes the 1/L^2 factor) 2D DFT of an
+ * interleaved complex L x L array, in place.  Definition: SURVEY.md 8(c) "DFT". */
+int FN(oracle_fft2)(int L, REAL* buf_interleaved, int inverse)
+{
+    if (L < 1 || (L & (L - 1))) return -1;
+    CPLX* buf = (CPLX*)buf_interleaved;
+    FN(fft2d)(buf, L, inverse ? +1 : -1);
+    if (inverse) {
+        REAL scale = (REAL)(1.0 / ((double)L * (double)L)); /* power of two: exact */
+        size_t N = (size_t)L * L;
+        for (size_t i = 0; i < N; ++i) { buf[i].re *= scale; buf[i].im *= scale; }
+    }
+    return 0;
+}
+
+/* c = C x = F^-1 ( s o F x ), the route of Listing 4. work: N complex. */
+static void FN(convolve)(int L, const REAL* s, const REAL* x, REAL* c, CPLX* work)
+{
+    size_t N = (size_t)L * L;
+    REAL scale = (REAL)(1.0 / ((double)L * (double)L));
+    for (size_t i = 0; i < N; ++i) { work[i].re = x[i]; work[i].im = (REAL)0; }   /* cpyComplex */
+    FN(fft2d)(work, L, -1);                                                        /* cufft2D fwd */
+    for (size_t i = 0; i < N; ++i) { work[i].re *= s[i]; work[i].im *= s[i]; }     /* elementMult */
+    FN(fft2d)(work, L, +1);                                                        /* cufft2D inv */
+    for (size_t i = 0; i < N; ++i) c[i] = work[i].re * scale;                      /* cpyReal + normalise */
+}
+
+/* y = A x = k o x + C x   ("one element-by-element multiplication and a call to CUBLAS later",
+ * PAPER.md:151; operator of BASELINE.json configs[0]). */
+static void FN(apply)(int L, const REAL* s, const REAL* k, const REAL* x, REAL* y, CPLX* work)
+{
+    size_t N = (size_t)L * L;
+    FN(convolve)(L, s, x, y, work);
+    for (size_t i = 0; i < N; ++i) y[i] = k[i] * x[i] + y[i];
+}
+
+int FN(oracle_apply)(int L, const REAL* s, const REAL* k, const REAL* x, REAL* y)
+{
+    if (L < 1 || (L & (L - 1))) return -1;
+    CPLX* work = (CPLX*)malloc(sizeof(CPLX) * (size_t)L * L);
+    FN(apply)(L, s, k, x, y, work);
+    free(work);
+    return 0;
+}
+
+/* dot product with a double accumulator, plain left-to-right sum (reading S12). */
+static double FN(dot)(size_t N, const REAL* a, const REAL* b)
+{
+    double acc = 0.0;
+    for (size_t i = 0; i < N; ++i) acc += (double)a[i] * (double)b[i];
+    return acc;
+}
+
+/* Conjugate gradient, Listing 2 in Hestenes-Stiefel form, step by step as in
+ * SURVEY.md 8(c).  Stopping rule (readings S3, S11, S15): first iteration at which the recurrence
+ * residual satisfies sqrt(r.r) <= tol * sqrt(f.f).
+ *   u        in: initial guess, out: solution
+ *   iters    number of operator applications inside the loop (reading S14)
+ *   relres   sqrt(rho)/||f|| at exit
+ *   hist     optional, capacity maxit+1: relative residual after 0,1,2,... iterations
+ *   Phist/Rhist optional, capacity maxit*N each: search direction p_i and residual r_i (before the
+ *            update of iteration i) -- used only by the CG-invariant pins on tiny grids
+ * returns 0 converged, 1 maxit reached, -4 breakdown (p.Ap <= 0 or not finite), -1 bad argument. */
+int FN(oracle_cg)(int L, const REAL* s, const REAL* k, const REAL* f, REAL* u, double tol, int maxit,
+                  int* iters, double* relres, double* hist, REAL* Phist, REAL* Rhist)
+{
+    if (L < 1 || (L & (L - 1)) || maxit < 0 || !(tol >= 0.0)) return -1;
+    size_t N = (size_t)L * L;
+    int status = 1, it = 0;
+    double fn = sqrt(FN(dot)(N, f, f));
+    if (fn == 0.0) {
+        for (size_t i = 0; i < N; ++i) u[i] = (REAL)0;
+        *iters = 0; *relres = 0.0; if (hist) hist[0] = 0.0;
+        return 0;
+    }
+    REAL* r = (REAL*)malloc(sizeof(REAL) * N);
+    REAL* p = (REAL*)malloc(sizeof(REAL) * N);
+    REAL* q = (REAL*)malloc(sizeof(REAL) * N);
+    CPLX* work = (CPLX*)malloc(sizeof(CPLX) * N);
+
+    FN(apply)(L, s, k, u, q, work);                              /* set up initial values */
+    for (size_t i = 0; i < N; ++i) { r[i] = f[i] - q[i]; p[i] = r[i]; }
+    double rho = FN(dot)(N, r, r);
+    if (hist) hist[0] = sqrt(rho) / fn;
+    if (sqrt(rho) <= tol * fn) { status = 0; goto done; }
+
+    while (it < maxit) {
+        if (Phist) memcpy(Phist + (size_t)it * N, p, sizeof(REAL) * N);
+        if (Rhist) memcpy(Rhist + (size_t)it * N, r, sizeof(REAL) * N);
+        FN(apply)(L, s, k, p, q, work);                          /* calculate A*x */
+        double pq = FN(dot)(N, p, q);                            /* search length (dot product) */
+        if (!(pq > 0.0) || !isfinite(pq)) { status = -4; goto done; }
+        double alpha = rho / pq;
+        REAL al = (REAL)alpha;
+        for (size_t i = 0; i < N; ++i) u[i] = u[i] + al * p[i];  /* new x */
+        for (size_t i = 0; i < N; ++i) r[i] = r[i] - al * q[i];  /* residue */
+        double rho_new = FN(dot)(N, r, r);                       /* residue length */
+        ++it;
+        if (hist) hist[it] = sqrt(rho_new) / fn;
+        if (sqrt(rho_new) <= tol * fn) { rho = rho_new; status = 0; break; }   /* check convergence */
+        double beta = rho_new / rho;                             /* update calculation variables */
+        REAL be = (REAL)beta;
+        for (size_t i = 0; i < N; ++i) p[i] = r[i] + be * p[i];
+        rho = rho_new;
+    }
+done:
+    *iters = it;
+    *relres = sqrt(rho) / fn;
+    free(r); free(p); free(q); free(work);
+    return status;
+}
+
+/* Break step (BASELINE.json configs[3]; readings S5, S13): over candidates {i : k_i > 0}
+ * ratio_i = (k_i * u_i) / t_i  -- one IEEE multiply and one IEEE divide in double -- pick the
+ * maximum, ties -> lowest i, NaN skipped; set k_i = 0.  second = runner-up ratio (for the top-2
+ * gap of reading S17), -inf if none.  returns 0, or -6 when there is no candidate (index = -1). */
+int FN(oracle_break_step)(long long N, REAL* k, const REAL* u, const REAL* t,
+                          long long* index, double* ratio, double* second)
+{
+    long long best = -1;
+    double rbest = 0.0, rsecond = -INFINITY;
+    for (long long i = 0; i < N; ++i) {
+        if (!(k[i] > (REAL)0)) continue;
+        double load = (double)k[i] * (double)u[i];
+        double rt = load / (double)t[i];
+        if (rt != rt) continue;
+        if (best < 0) { best = i; rbest = rt; }
+        else if (rt > rbest) { rsecond = rbest; rbest = rt; best = i; }
+        else if (rt > rsecond) rsecond = rt;
+    }
+    *index = best; *ratio = rbest; if (second) *second = rsecond;
+    if (best < 0) return -6;
+    k[best] = (REAL)0;
+    return 0;
+}
+
+/* Quasi-static loop (BASELINE.json configs[3]; reading S11: warm start from previous u).
+ * For each step: solve A u = f by CG from the current u, then break one site.
+ * out_index[nsteps], out_iters[nsteps], out_gap[nsteps] (relative top-2 gap, may be NULL).
+ * returns the number of completed steps (== nsteps on success), or a negative CG status. */
+int FN(oracle_fracture)(int L, const REAL* s, REAL* k, const REAL* f, REAL* u, const REAL* t,
+                        int nsteps, double tol, int maxit,
+                        long long* out_index, int* out_iters, double* out_gap)
+{
+    long long N = (long long)L * L;
+    for (int step = 0; step < nsteps; ++step) {
+        int it; double rr;
+        int st = FN(oracle_cg)(L, s, k, f, u, tol, maxit, &it, &rr, NULL, NULL, NULL);
+        if (st < 0) return st;
+        long long idx; double ratio, second;
+        int bs = FN(oracle_break_step)(N, k, u, t, &idx, &ratio, &second);
+        if (bs < 0) return step;
+        out_index[step] = idx; out_iters[step] = it;
+        if (out_gap) out_gap[step] = (ratio - second) / fabs(ratio);
+    }
+    return nsteps;
+}
