@@ -1,0 +1,136 @@
+/*
+ * fcg.h -- C ABI of libfcg: FFT-accelerated conjugate gradient for the lattice fracture model of
+ * arXiv 1305.3625 (Gjerden), hand-written CUDA for NVIDIA B200 (sm_100a).  No cuFFT, no cuBLAS,
+ * no CPU fallback.
+ *
+ * Citations: "PAPER.md:<line>" = /root/reference/PAPER.md; "configs[i]" / "north_star" =
+ * BASELINE.json; "S<n>" = reading n in SURVEY.md section 8(c) / DESIGN.md.
+ *
+ * The problem (north_star, Listings 2 and 4):
+ *     solve  A u = f,   A = diag(k) + C,   C x = F^-1 ( s o F x )
+ * on a periodic L x L lattice.  F is the 2D DFT
+ *     X[m,n] = sum_{a,b} x[a,b] exp(-2 pi i (m a + n b) / L),
+ * s is a real spectrum (row-major [m][n]); C x is real because only the even part
+ * (s[m,n] + s[-m,-n])/2 of s survives the final "take the real part" step (cpyReal).
+ *
+ * Conventions for every call
+ *   - Site index i = a*L + b (row a, column b fastest).  N = L*L.
+ *   - Every array argument is a DEVICE pointer to contiguous memory of the handle's dtype
+ *     (float for FCG_F32, double for FCG_F64), 16-byte aligned, owned by the caller (e.g. a
+ *     torch tensor).  The library never frees or keeps a caller pointer after the call returns.
+ *     Exceptions are spelled out: names ending in _host are HOST pointers.
+ *   - All work is enqueued on the stream given to fcg_create.  Calls that fill host out-params
+ *     (fcg_solve, fcg_break_step) end with one small device-to-host copy and one stream
+ *     synchronisation ("reporting back only a few values to the CPU each time the solver has
+ *     completed").  Nothing inside the CG loop synchronises with the host.
+ *   - Return value: fcg_status.  >= 0 means the outputs are valid.  On error the outputs are
+ *     unspecified unless stated; fcg_last_error() gives a message.  A handle is not thread-safe.
+ *   - L must be a power of two, 16 <= L <= 8192 (S8); otherwise FCG_UNSUPPORTED.
+ */
+#ifndef FCG_H
+#define FCG_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct fcg_handle_s* fcg_handle;
+
+typedef enum { FCG_F32 = 0, FCG_F64 = 1 } fcg_dtype;
+
+typedef enum {
+    FCG_OK            =  0,
+    FCG_NOT_CONVERGED =  1,  /* maxit reached; u, iters, rel_residual are valid (S16) */
+    FCG_INVALID_ARG   = -1,
+    FCG_UNSUPPORTED   = -2,
+    FCG_CUDA_ERROR    = -3,
+    FCG_BREAKDOWN     = -4,  /* p.Ap <= 0 or not finite; u holds the last iterate before the breakdown */
+    FCG_NO_SPECTRUM   = -5,  /* fcg_set_spectrum has not been called */
+    FCG_NO_CANDIDATE  = -6   /* fcg_break_step: no site with k > 0 (and a non-NaN ratio); index = -1 */
+} fcg_status;
+
+/* Options for fcg_set_option. */
+typedef enum {
+    FCG_OPT_LOOP_MODE    = 0, /* 0 (default): whole solve = one CUDA graph with a device-side WHILE node;
+                                 1: kernels enqueued directly, in chunks of FCG_OPT_CHUNK iterations that
+                                    exit early on the device flag, host polls once per chunk */
+    FCG_OPT_CHUNK        = 1, /* iterations per chunk in loop mode 1 (default 16) */
+    FCG_OPT_ROW_VARIANT  = 2  /* -1 (default): tuned rows-per-CTA of the row passes; 0,1,..: force variant */
+} fcg_option;
+
+/* Bytes of device workspace a handle of this size needs (0 if the size is unsupported). */
+size_t fcg_workspace_bytes(int L, fcg_dtype dt);
+
+/* Lifecycle (allocate -> plan -> execute -> destroy of Listing 3, without cuFFT).
+ *   workspace    device memory of at least fcg_workspace_bytes(), 256-byte aligned, caller-owned and kept
+ *                alive until fcg_destroy; or NULL: the library allocates and frees its own.
+ *   cuda_stream  a cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream); NULL = default stream.
+ * Builds twiddle tables and launch plans; may synchronise the stream. */
+int fcg_create(int L, fcg_dtype dt, void* workspace, void* cuda_stream, fcg_handle* out);
+int fcg_destroy(fcg_handle h);
+int fcg_set_option(fcg_handle h, int option, int value);
+
+/* Static spectrum ("the FFT of G is static and performed during initialization").
+ *   s  device, L x L reals, row-major [m][n].  Copied into an internal layout (even part, scaled by
+ *      1/L^2 -- exact for power-of-two L, S6 -- permuted to the transform's digit-reversed order);
+ *      the caller's array is not referenced afterwards. */
+int fcg_set_spectrum(fcg_handle h, const void* s);
+
+/* y = A x = k o x + C x  (Listing 4 + "one element-by-element multiplication and a call to CUBLAS",
+ * PAPER.md:141-151).  k, x read-only; y written; y must not alias k or x.  Asynchronous. */
+int fcg_apply(fcg_handle h, const void* k, const void* x, void* y);
+
+/* Conjugate gradient, Listing 2, un-preconditioned.
+ *   k, f          read-only, N reals each
+ *   u             in: initial guess (warm start, configs[3]); out: solution
+ *   tol, maxit    stop at the FIRST iteration with ||r||_2 <= tol * ||f||_2, r the recurrence residual
+ *                 (S3, S11, S15), or after maxit iterations (status FCG_NOT_CONVERGED)
+ *   iters_host    number of operator applications inside the loop (S14)
+ *   rel_residual_host   ||r||_2 / ||f||_2 at exit
+ * Dot products are accumulated in double and the scalars alpha, beta, rho are double for both dtypes
+ * (S12); partial sums are combined in a fixed order, so repeated runs are bit-identical.
+ * f == 0 gives u = 0, 0 iterations.  Blocks until the solve has finished. */
+int fcg_solve(fcg_handle h, const void* k, const void* f, void* u, double tol, int maxit,
+              int* iters_host, double* rel_residual_host);
+
+/* Same solve with HOST arrays (N reals each): copies k, f, u to library-owned device buffers, solves,
+ * copies u back.  This is the end-to-end entry point timed by bench.py ("e2e"). */
+int fcg_solve_host(fcg_handle h, const void* k_host, const void* f_host, void* u_host, double tol,
+                   int maxit, int* iters_host, double* rel_residual_host);
+
+/* Stand-alone transforms (north_star "fcg_fft_fwd/inv").
+ *   x  L x L reals;  X  L x (L/2+1) interleaved complex, row-major [m][n], n = 0..L/2
+ *   fwd: X = F x (half spectrum; the rest follows from X[-m,-n] = conj X[m,n])
+ *   inv: x = F^-1 X including 1/L^2, so inv(fwd(x)) == x.  X must be the spectrum of a real field
+ *        (S18); only n = 0..L/2 is read.
+ * x and X must not overlap.  Asynchronous. */
+int fcg_fft_fwd(fcg_handle h, const void* x, void* X);
+int fcg_fft_inv(fcg_handle h, const void* X, void* x);
+
+/* Break step of the quasi-static loop (rule of configs[3], S5, S13):
+ * over candidates {i : k_i > 0}: ratio_i = (k_i * u_i) / t_i, one IEEE multiply and one IEEE divide in
+ * double; pick the maximum, ties -> lowest i, NaN skipped; set k_i = 0.
+ *   k  in/out;  u, t read-only;  index_host = i (or -1);  ratio_host = the winning ratio.
+ * Blocks until done. */
+int fcg_break_step(fcg_handle h, void* k, const void* u, const void* t,
+                   long long* index_host, double* ratio_host);
+
+/* Quasi-static loop (configs[3]): nsteps times { fcg_solve warm-started from the current u;
+ * fcg_break_step }.  index_host[nsteps], iters_host[nsteps] are HOST arrays.  Stops early (returning the
+ * status) on a negative status; steps_done_host receives the number of completed steps. */
+int fcg_fracture(fcg_handle h, void* k, const void* f, void* u, const void* t, int nsteps, double tol,
+                 int maxit, long long* index_host, int* iters_host, int* steps_done_host);
+
+/* Number of this library's kernel launches enqueued by the last fcg_solve / fcg_solve_host /
+ * fcg_fracture call on this handle (graph kernel nodes counted once per execution). */
+long long fcg_last_launch_count(fcg_handle h);
+
+const char* fcg_last_error(fcg_handle h);
+const char* fcg_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FCG_H */

@@ -1,0 +1,198 @@
+"""Thin ctypes binding of libfcg.so -- same names as the C calls of include/fcg.h, argument marshalling only.
+
+Every step of the hot path runs in the library's CUDA kernels; torch is used for device memory and
+streams.  There is no CPU fallback: loading fails loudly when libfcg.so is missing, and fcg_create
+fails when there is no CUDA device.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libfcg.so")
+
+FCG_F32, FCG_F64 = 0, 1
+FCG_OK, FCG_NOT_CONVERGED = 0, 1
+FCG_INVALID_ARG, FCG_UNSUPPORTED, FCG_CUDA_ERROR, FCG_BREAKDOWN, FCG_NO_SPECTRUM, FCG_NO_CANDIDATE = -1, -2, -3, -4, -5, -6
+FCG_OPT_LOOP_MODE, FCG_OPT_CHUNK, FCG_OPT_ROW_VARIANT = 0, 1, 2
+
+EXPORTS = ["fcg_workspace_bytes", "fcg_create", "fcg_destroy", "fcg_set_option", "fcg_set_spectrum", "fcg_apply",
+           "fcg_solve", "fcg_solve_host", "fcg_fft_fwd", "fcg_fft_inv", "fcg_break_step", "fcg_fracture",
+           "fcg_last_launch_count", "fcg_last_error", "fcg_version"]
+
+_lib = None
+
+
+class FcgError(RuntimeError):
+    def __init__(self, status: int, msg: str):
+        super().__init__(f"fcg status {status}: {msg}")
+        self.status = status
+
+
+def lib() -> C.CDLL:
+    """Load libfcg.so (built in-tree by paper_1305_3625_b200.build). Raises if it is missing."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise FileNotFoundError(f"{LIB_PATH} not found: run `python -m paper_1305_3625_b200.build` (there is no CPU fallback)")
+        L = C.CDLL(LIB_PATH)
+        vp, i, d, ll = C.c_void_p, C.c_int, C.c_double, C.c_longlong
+        L.fcg_workspace_bytes.argtypes = [i, i]; L.fcg_workspace_bytes.restype = C.c_size_t
+        L.fcg_create.argtypes = [i, i, vp, vp, C.POINTER(vp)]; L.fcg_create.restype = i
+        L.fcg_destroy.argtypes = [vp]; L.fcg_destroy.restype = i
+        L.fcg_set_option.argtypes = [vp, i, i]; L.fcg_set_option.restype = i
+        L.fcg_set_spectrum.argtypes = [vp, vp]; L.fcg_set_spectrum.restype = i
+        L.fcg_apply.argtypes = [vp, vp, vp, vp]; L.fcg_apply.restype = i
+        L.fcg_solve.argtypes = [vp, vp, vp, vp, d, i, C.POINTER(i), C.POINTER(d)]; L.fcg_solve.restype = i
+        L.fcg_solve_host.argtypes = [vp, vp, vp, vp, d, i, C.POINTER(i), C.POINTER(d)]; L.fcg_solve_host.restype = i
+        L.fcg_fft_fwd.argtypes = [vp, vp, vp]; L.fcg_fft_fwd.restype = i
+        L.fcg_fft_inv.argtypes = [vp, vp, vp]; L.fcg_fft_inv.restype = i
+        L.fcg_break_step.argtypes = [vp, vp, vp, vp, C.POINTER(ll), C.POINTER(d)]; L.fcg_break_step.restype = i
+        L.fcg_fracture.argtypes = [vp, vp, vp, vp, vp, i, d, i, vp, vp, C.POINTER(i)]; L.fcg_fracture.restype = i
+        L.fcg_last_launch_count.argtypes = [vp]; L.fcg_last_launch_count.restype = ll
+        L.fcg_last_error.argtypes = [vp]; L.fcg_last_error.restype = C.c_char_p
+        L.fcg_version.argtypes = []; L.fcg_version.restype = C.c_char_p
+        _lib = L
+    return _lib
+
+
+def _dt(dtype) -> int:
+    if dtype == torch.float64:
+        return FCG_F64
+    if dtype == torch.float32:
+        return FCG_F32
+    raise TypeError(f"fcg supports torch.float32/float64, got {dtype}")
+
+
+class Fcg:
+    """One handle = one lattice size and dtype on the current CUDA device and stream (fcg_create)."""
+
+    def __init__(self, L: int, dtype=torch.float64, device="cuda", stream: torch.cuda.Stream | None = None,
+                 own_workspace: bool = False):
+        self.L, self.N, self.dtype = L, L * L, dtype
+        self.device = torch.device(device)
+        self._lib = lib()
+        self._h = C.c_void_p()
+        with torch.cuda.device(self.device):
+            self.stream = stream or torch.cuda.current_stream(self.device)
+            nbytes = self._lib.fcg_workspace_bytes(L, _dt(dtype))
+            if nbytes == 0:
+                raise FcgError(FCG_UNSUPPORTED, f"L={L} unsupported (power of two, 16..8192)")
+            self._ws = None if own_workspace else torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+            ws_ptr = None if own_workspace else self._ws.data_ptr()
+            st = self._lib.fcg_create(L, _dt(dtype), ws_ptr, self.stream.cuda_stream, C.byref(self._h))
+        if st != FCG_OK:
+            self._h = C.c_void_p()
+            raise FcgError(st, "fcg_create failed (no CUDA device, or unsupported size)")
+
+    # -- helpers -------------------------------------------------------------------------------
+    def _chk(self, t: torch.Tensor, numel: int | None = None, dtype=None) -> int:
+        dtype = dtype or self.dtype
+        if not (t.is_cuda and t.is_contiguous() and t.dtype == dtype):
+            raise ValueError(f"expected contiguous CUDA tensor of {dtype}")
+        if numel is not None and t.numel() != numel:
+            raise ValueError(f"expected {numel} elements, got {t.numel()}")
+        return t.data_ptr()
+
+    def _raise(self, st: int):
+        raise FcgError(st, self._lib.fcg_last_error(self._h).decode())
+
+    def last_error(self) -> str:
+        return self._lib.fcg_last_error(self._h).decode()
+
+    def close(self):
+        if self._h:
+            self._lib.fcg_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # -- the C calls -----------------------------------------------------------------------------
+    def fcg_set_option(self, option: int, value: int):
+        st = self._lib.fcg_set_option(self._h, option, value)
+        if st != FCG_OK:
+            self._raise(st)
+
+    def fcg_set_spectrum(self, s: torch.Tensor):
+        st = self._lib.fcg_set_spectrum(self._h, self._chk(s, self.N))
+        if st != FCG_OK:
+            self._raise(st)
+
+    def fcg_apply(self, k: torch.Tensor, x: torch.Tensor, y: torch.Tensor | None = None) -> torch.Tensor:
+        y = torch.empty_like(x) if y is None else y
+        st = self._lib.fcg_apply(self._h, self._chk(k, self.N), self._chk(x, self.N), self._chk(y, self.N))
+        if st != FCG_OK:
+            self._raise(st)
+        return y
+
+    def fcg_solve(self, k: torch.Tensor, f: torch.Tensor, u: torch.Tensor, tol: float, maxit: int):
+        """In place on u. Returns (iters, rel_residual, status); raises on error statuses other than BREAKDOWN."""
+        it = C.c_int(0); rr = C.c_double(0.0)
+        st = self._lib.fcg_solve(self._h, self._chk(k, self.N), self._chk(f, self.N), self._chk(u, self.N),
+                                 float(tol), int(maxit), C.byref(it), C.byref(rr))
+        if st < 0 and st != FCG_BREAKDOWN:
+            self._raise(st)
+        return int(it.value), float(rr.value), int(st)
+
+    def fcg_solve_host(self, k: torch.Tensor, f: torch.Tensor, u: torch.Tensor, tol: float, maxit: int):
+        """Same with HOST tensors (pinned for full copy speed); u updated in place."""
+        for t in (k, f, u):
+            if t.is_cuda or not t.is_contiguous() or t.dtype != self.dtype or t.numel() != self.N:
+                raise ValueError("expected contiguous host tensors of the handle's dtype and size")
+        it = C.c_int(0); rr = C.c_double(0.0)
+        st = self._lib.fcg_solve_host(self._h, k.data_ptr(), f.data_ptr(), u.data_ptr(), float(tol), int(maxit),
+                                      C.byref(it), C.byref(rr))
+        if st < 0 and st != FCG_BREAKDOWN:
+            self._raise(st)
+        return int(it.value), float(rr.value), int(st)
+
+    def fcg_fft_fwd(self, x: torch.Tensor, X: torch.Tensor | None = None) -> torch.Tensor:
+        cdt = torch.complex128 if self.dtype == torch.float64 else torch.complex64
+        X = torch.empty((self.L, self.L // 2 + 1), dtype=cdt, device=x.device) if X is None else X
+        st = self._lib.fcg_fft_fwd(self._h, self._chk(x, self.N), self._chk(X, self.L * (self.L // 2 + 1), cdt))
+        if st != FCG_OK:
+            self._raise(st)
+        return X
+
+    def fcg_fft_inv(self, X: torch.Tensor, x: torch.Tensor | None = None) -> torch.Tensor:
+        cdt = torch.complex128 if self.dtype == torch.float64 else torch.complex64
+        x = torch.empty((self.L, self.L), dtype=self.dtype, device=X.device) if x is None else x
+        st = self._lib.fcg_fft_inv(self._h, self._chk(X, self.L * (self.L // 2 + 1), cdt), self._chk(x, self.N))
+        if st != FCG_OK:
+            self._raise(st)
+        return x
+
+    def fcg_break_step(self, k: torch.Tensor, u: torch.Tensor, t: torch.Tensor):
+        """In place on k. Returns (index, ratio, status)."""
+        idx = C.c_longlong(-1); ratio = C.c_double(0.0)
+        st = self._lib.fcg_break_step(self._h, self._chk(k, self.N), self._chk(u, self.N), self._chk(t, self.N),
+                                      C.byref(idx), C.byref(ratio))
+        if st < 0 and st != FCG_NO_CANDIDATE:
+            self._raise(st)
+        return int(idx.value), float(ratio.value), int(st)
+
+    def fcg_fracture(self, k: torch.Tensor, f: torch.Tensor, u: torch.Tensor, t: torch.Tensor, nsteps: int,
+                     tol: float, maxit: int):
+        """In place on k and u. Returns (index[int64 numpy], iters[int32 numpy], steps_done, status)."""
+        import numpy as np
+        index = np.full(nsteps, -1, np.int64); iters = np.zeros(nsteps, np.int32); done = C.c_int(0)
+        st = self._lib.fcg_fracture(self._h, self._chk(k, self.N), self._chk(f, self.N), self._chk(u, self.N),
+                                    self._chk(t, self.N), int(nsteps), float(tol), int(maxit),
+                                    index.ctypes.data_as(C.c_void_p), iters.ctypes.data_as(C.c_void_p), C.byref(done))
+        if st < 0 and st not in (FCG_BREAKDOWN, FCG_NO_CANDIDATE):
+            self._raise(st)
+        return index, iters, int(done.value), int(st)
+
+    def fcg_last_launch_count(self) -> int:
+        return int(self._lib.fcg_last_launch_count(self._h))
+
+
+def fcg_version() -> str:
+    return lib().fcg_version().decode()

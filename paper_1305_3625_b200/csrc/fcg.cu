@@ -1,0 +1,480 @@
+// fcg.cu -- the C ABI of include/fcg.h: handle, workspace, launch sequences, CUDA-graph construction.
+// Kernels live in fcg_kernels.cuh / fcg_passes.cuh; the transform passes are instantiated per lattice
+// size in fcg_inst.cu.  No cuFFT, no cuBLAS, no host arithmetic on the data path.
+#define FCG_MAIN_TU
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "../../include/fcg.h"
+#include "fcg_kernels.cuh"
+#include "fcg_plans.cuh"
+
+using namespace fcg;
+
+namespace {
+
+constexpr int VEC_BLOCKS_MAX = 148 * 4;
+constexpr size_t ALIGN = 256;
+size_t align_up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
+
+const PassTable* get_table(int L, int dtype) {
+    switch (L) {
+        case 16: return fcg_pass_table_16(dtype);
+        case 32: return fcg_pass_table_32(dtype);
+        case 64: return fcg_pass_table_64(dtype);
+        case 128: return fcg_pass_table_128(dtype);
+        case 256: return fcg_pass_table_256(dtype);
+        case 512: return fcg_pass_table_512(dtype);
+        case 1024: return fcg_pass_table_1024(dtype);
+        case 2048: return fcg_pass_table_2048(dtype);
+        case 4096: return fcg_pass_table_4096(dtype);
+        case 8192: return fcg_pass_table_8192(dtype);
+    }
+    return nullptr;
+}
+
+struct Layout {            // byte offsets into the workspace
+    size_t Tb, shat, r, p, q, tw, partial_row, partial_vec, brk_r, brk_i, scalars, brk_out, brk_ticket, total;
+};
+Layout make_layout(int L, size_t w) {
+    const size_t N = (size_t)L * L;
+    Layout o{}; size_t off = 0;
+    auto take = [&](size_t bytes) { size_t at = off; off = align_up(off + bytes); return at; };
+    o.Tb = take(N * w);                                   // (L/2) x L complex
+    o.shat = take(((size_t)L / 2 + 1) * L * w);
+    o.r = take(N * w); o.p = take(N * w); o.q = take(N * w);
+    o.tw = take((size_t)L * 2 * w);
+    o.partial_row = take((size_t)L * 2 * sizeof(double));
+    o.partial_vec = take(VEC_BLOCKS_MAX * sizeof(double));
+    o.brk_r = take(VEC_BLOCKS_MAX * sizeof(double));
+    o.brk_i = take(VEC_BLOCKS_MAX * sizeof(long long));
+    o.scalars = take(sizeof(Scalars));
+    o.brk_out = take(sizeof(BreakResult));
+    o.brk_ticket = take(sizeof(unsigned int));
+    o.total = off;
+    return o;
+}
+
+struct GraphEntry {
+    const void *k, *f; void* u; double tol; int maxit, var;
+    cudaGraph_t graph; cudaGraphExec_t exec; unsigned long long stamp;
+};
+
+}  // namespace
+
+struct fcg_handle_s {
+    int L = 0, dtype = 0; size_t w = 0, N = 0;
+    const PassTable* tab = nullptr;
+    cudaStream_t stream = nullptr, cap_stream = nullptr;
+    char* ws = nullptr; bool own_ws = false;
+    Layout lay{};
+    bool have_spectrum = false;
+    int loop_mode = 0, chunk = 16, row_var_opt = -1;
+    Scalars* h_sc = nullptr;            // pinned
+    BreakResult* h_brk = nullptr;       // pinned
+    void *hk = nullptr, *hf = nullptr, *hu = nullptr;   // device staging of fcg_solve_host
+    std::vector<GraphEntry> graphs; unsigned long long stamp = 0;
+    long long launches = 0;
+    std::string err;
+
+    template <typename U> U* at(size_t off) const { return reinterpret_cast<U*>(ws + off); }
+    Scalars* sc() const { return at<Scalars>(lay.scalars); }
+    int vec_blocks() const {
+        size_t nvec = N / (dtype == FCG_F64 ? 2 : 4);
+        size_t b = (nvec + 255) / 256;
+        return (int)(b < (size_t)VEC_BLOCKS_MAX ? b : (size_t)VEC_BLOCKS_MAX);
+    }
+    int row_var() const {
+        if (row_var_opt >= 0 && row_var_opt < FCG_NROWVAR && tab->row_valid[row_var_opt]) return row_var_opt;
+        int best = 0;
+        for (int v = 0; v < FCG_NROWVAR; ++v)
+            if (tab->row_valid[v] && tab->row_smem[v] <= 72 * 1024 && L / (2 * tab->row_F[v]) >= 256) best = v;
+        return best;
+    }
+};
+
+namespace {
+
+#define FCG_CK(h, expr)                                                                          \
+    do {                                                                                         \
+        cudaError_t e_ = (expr);                                                                 \
+        if (e_ != cudaSuccess) {                                                                 \
+            (h)->err = std::string(#expr) + ": " + cudaGetErrorString(e_);                       \
+            return FCG_CUDA_ERROR;                                                               \
+        }                                                                                        \
+    } while (0)
+
+int fail(fcg_handle h, int code, const char* msg) { if (h) h->err = msg; return code; }
+
+// ---- launch sequences (typed) ---------------------------------------------------------------
+template <typename T> struct Seq {
+    fcg_handle h; cudaStream_t st;
+    cx<T>* Tb() const { return h->at<cx<T>>(h->lay.Tb); }
+    const cx<T>* tw() const { return h->at<cx<T>>(h->lay.tw); }
+    const T* shat() const { return h->at<T>(h->lay.shat); }
+    T* r() const { return h->at<T>(h->lay.r); }
+    T* p() const { return h->at<T>(h->lay.p); }
+    T* q() const { return h->at<T>(h->lay.q); }
+
+    cudaError_t row_fwd(int mode, const T* x, T* u) const {
+        RowFwdArgs<T> A{}; A.mode = mode; A.x = x; A.u = u; A.p = p(); A.r = r(); A.Tb = Tb(); A.tw = tw(); A.sc = h->sc();
+        ++h->launches; return h->tab->row_fwd(h->row_var(), &A, st);
+    }
+    cudaError_t col(int mode, bool cg) const {
+        ColArgs<T> A{}; A.mode = mode; A.Tb = Tb(); A.shat = shat(); A.tw = tw(); A.sc = cg ? h->sc() : nullptr;
+        ++h->launches; return h->tab->col(&A, st);
+    }
+    cudaError_t row_inv(int mode, const T* k, const T* v, const T* f, T* out, T* out2) const {
+        RowInvArgs<T> A{}; A.mode = mode; A.Tb = Tb(); A.tw = tw(); A.k = k; A.v = v; A.f = f; A.out = out; A.out2 = out2;
+        A.scale = (T)(1.0 / ((double)h->L * (double)h->L));
+        A.partial = h->at<double>(h->lay.partial_row); A.sc = h->sc();
+        ++h->launches; return h->tab->row_inv(h->row_var(), &A, st);
+    }
+    // set up initial values: r = f - A u, p = 0 (first direction p = r + 0*p), rho, ||f||^2
+    cudaError_t init(const T* k, const T* f, T* u, double tol, int maxit, bool use_cond, unsigned long long cond) const {
+        SetupArgs sa{tol, maxit, use_cond ? 1 : 0, cond};
+        cg_setup_kernel<<<1, 32, 0, st>>>(h->sc(), sa); ++h->launches;
+        cudaError_t e;
+        if ((e = cudaGetLastError()) != cudaSuccess) return e;
+        if ((e = row_fwd(ROWF_PLAIN, u, nullptr)) != cudaSuccess) return e;
+        if ((e = col(COL_CONV, false)) != cudaSuccess) return e;
+        return row_inv(ROWI_RESID, k, u, f, r(), p());
+    }
+    // one pass of Listing 2
+    cudaError_t iteration(const T* k, T* u) const {
+        cudaError_t e;
+        if ((e = row_fwd(ROWF_CG, nullptr, u)) != cudaSuccess) return e;            // new x (lagged), new p, row transform
+        if ((e = col(COL_CONV, true)) != cudaSuccess) return e;                     // column transform * spectrum * inverse
+        if ((e = row_inv(ROWI_CG, k, p(), nullptr, q(), nullptr)) != cudaSuccess) return e;   // q = A p, p.q, alpha
+        const size_t nvec = h->N / Vec<T>::W;
+        cg_update_r_kernel<T><<<h->vec_blocks(), 256, 0, st>>>(r(), q(), nvec, h->at<double>(h->lay.partial_vec), h->sc());
+        ++h->launches;
+        return cudaGetLastError();                                                  // r, r.r, beta, convergence
+    }
+    cudaError_t finish(T* u) const {
+        const size_t nvec = h->N / Vec<T>::W;
+        cg_finish_kernel<T><<<h->vec_blocks(), 256, 0, st>>>(u, p(), nvec, h->sc()); ++h->launches;
+        cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess) return e;
+        return cudaMemcpyAsync(h->h_sc, h->sc(), sizeof(Scalars), cudaMemcpyDeviceToHost, st);
+    }
+};
+
+void drop_graph(GraphEntry& g) {
+    if (g.exec) cudaGraphExecDestroy(g.exec);
+    if (g.graph) cudaGraphDestroy(g.graph);
+    g.exec = nullptr; g.graph = nullptr;
+}
+
+// Whole solve as one graph:  init  ->  WHILE(cond){ iteration }  ->  finish + D2H of the scalars.
+// cond is written on the device by the residual / r-update kernels (cudaGraphSetConditional).
+template <typename T>
+cudaError_t build_graph(fcg_handle h, GraphEntry& ge) {
+    cudaError_t e;
+    cudaStream_t cs = h->cap_stream;
+    Seq<T> s{h, cs};
+    const long long saved = h->launches;
+    ge.graph = nullptr; ge.exec = nullptr;
+    if ((e = cudaGraphCreate(&ge.graph, 0)) != cudaSuccess) return e;
+    cudaGraphConditionalHandle cond;
+    if ((e = cudaGraphConditionalHandleCreate(&cond, ge.graph, 0, cudaGraphCondAssignDefault)) != cudaSuccess) return e;
+
+    if ((e = cudaStreamBeginCaptureToGraph(cs, ge.graph, nullptr, nullptr, 0, cudaStreamCaptureModeRelaxed)) != cudaSuccess) return e;
+    e = s.init((const T*)ge.k, (const T*)ge.f, (T*)ge.u, ge.tol, ge.maxit, true, (unsigned long long)cond);
+    cudaStreamCaptureStatus cst; const cudaGraphNode_t* deps = nullptr; size_t ndeps = 0;
+    cudaError_t e2 = cudaStreamGetCaptureInfo(cs, &cst, nullptr, nullptr, &deps, &ndeps);
+    std::vector<cudaGraphNode_t> dep(deps, deps + (e2 == cudaSuccess ? ndeps : 0));
+    cudaGraph_t tmp;
+    cudaError_t e3 = cudaStreamEndCapture(cs, &tmp);
+    if (e != cudaSuccess) return e;
+    if (e2 != cudaSuccess) return e2;
+    if (e3 != cudaSuccess) return e3;
+
+    cudaGraphNodeParams np{};
+    np.type = cudaGraphNodeTypeConditional;
+    np.conditional.handle = cond;
+    np.conditional.type = cudaGraphCondTypeWhile;
+    np.conditional.size = 1;
+    cudaGraphNode_t wnode;
+    if ((e = cudaGraphAddNode(&wnode, ge.graph, dep.data(), dep.size(), &np)) != cudaSuccess) return e;
+    cudaGraph_t body = np.conditional.phGraph_out[0];
+
+    if ((e = cudaStreamBeginCaptureToGraph(cs, body, nullptr, nullptr, 0, cudaStreamCaptureModeRelaxed)) != cudaSuccess) return e;
+    e = s.iteration((const T*)ge.k, (T*)ge.u);
+    e3 = cudaStreamEndCapture(cs, &tmp);
+    if (e != cudaSuccess) return e;
+    if (e3 != cudaSuccess) return e3;
+
+    if ((e = cudaStreamBeginCaptureToGraph(cs, ge.graph, &wnode, nullptr, 1, cudaStreamCaptureModeRelaxed)) != cudaSuccess) return e;
+    e = s.finish((T*)ge.u);
+    e3 = cudaStreamEndCapture(cs, &tmp);
+    if (e != cudaSuccess) return e;
+    if (e3 != cudaSuccess) return e3;
+
+    h->launches = saved;
+    return cudaGraphInstantiate(&ge.exec, ge.graph, 0);
+}
+
+template <typename T>
+int solve_impl(fcg_handle h, const void* k, const void* f, void* u, double tol, int maxit, int* iters, double* relres) {
+    h->launches = 0;
+    if (h->loop_mode == 0) {
+        const int var = h->row_var();
+        GraphEntry* hit = nullptr;
+        for (auto& g : h->graphs)
+            if (g.k == k && g.f == f && g.u == u && g.tol == tol && g.maxit == maxit && g.var == var) { hit = &g; break; }
+        if (!hit) {
+            if (h->graphs.size() >= 8) {
+                size_t lru = 0;
+                for (size_t i = 1; i < h->graphs.size(); ++i) if (h->graphs[i].stamp < h->graphs[lru].stamp) lru = i;
+                drop_graph(h->graphs[lru]); h->graphs.erase(h->graphs.begin() + lru);
+            }
+            GraphEntry ge{k, f, u, tol, maxit, var, nullptr, nullptr, 0};
+            cudaError_t e = build_graph<T>(h, ge);
+            if (e != cudaSuccess) {
+                // conditional graph nodes unavailable: fall back to direct launches for the rest of this handle's life
+                h->err = std::string("graph construction failed (") + cudaGetErrorString(e) + "); using loop mode 1";
+                cudaStreamCaptureStatus cst;
+                if (cudaStreamIsCapturing(h->cap_stream, &cst) == cudaSuccess && cst != cudaStreamCaptureStatusNone) {
+                    cudaGraph_t junk = nullptr; cudaStreamEndCapture(h->cap_stream, &junk);
+                }
+                drop_graph(ge); cudaGetLastError();
+                h->loop_mode = 1;
+            } else {
+                h->graphs.push_back(ge); hit = &h->graphs.back();
+            }
+        }
+        if (hit) {
+            hit->stamp = ++h->stamp;
+            FCG_CK(h, cudaGraphLaunch(hit->exec, h->stream));
+            FCG_CK(h, cudaStreamSynchronize(h->stream));
+            h->launches = 5 + 4LL * h->h_sc->it;
+        }
+    }
+    if (h->loop_mode != 0) {
+        Seq<T> s{h, h->stream};
+        FCG_CK(h, s.init((const T*)k, (const T*)f, (T*)u, tol, maxit, false, 0ULL));
+        FCG_CK(h, cudaMemcpyAsync(h->h_sc, h->sc(), sizeof(Scalars), cudaMemcpyDeviceToHost, h->stream));
+        FCG_CK(h, cudaStreamSynchronize(h->stream));
+        while (!h->h_sc->done) {
+            for (int c = 0; c < h->chunk; ++c) FCG_CK(h, s.iteration((const T*)k, (T*)u));
+            FCG_CK(h, cudaMemcpyAsync(h->h_sc, h->sc(), sizeof(Scalars), cudaMemcpyDeviceToHost, h->stream));
+            FCG_CK(h, cudaStreamSynchronize(h->stream));
+        }
+        FCG_CK(h, s.finish((T*)u));
+        FCG_CK(h, cudaStreamSynchronize(h->stream));
+    }
+    if (iters) *iters = h->h_sc->it;
+    if (relres) *relres = h->h_sc->relres;
+    return h->h_sc->status;
+}
+
+template <typename T>
+int break_impl(fcg_handle h, void* k, const void* u, const void* t, long long* index, double* ratio) {
+    break_argmax_kernel<T><<<h->vec_blocks(), 256, 0, h->stream>>>(
+        (T*)k, (const T*)u, (const T*)t, (long long)h->N, h->at<double>(h->lay.brk_r), h->at<long long>(h->lay.brk_i),
+        h->at<unsigned int>(h->lay.brk_ticket), h->at<BreakResult>(h->lay.brk_out));
+    ++h->launches;
+    FCG_CK(h, cudaGetLastError());
+    FCG_CK(h, cudaMemcpyAsync(h->h_brk, h->at<BreakResult>(h->lay.brk_out), sizeof(BreakResult), cudaMemcpyDeviceToHost, h->stream));
+    FCG_CK(h, cudaStreamSynchronize(h->stream));
+    if (index) *index = h->h_brk->index;
+    if (ratio) *ratio = h->h_brk->ratio;
+    return h->h_brk->status;
+}
+
+template <typename T>
+int fft_impl(fcg_handle h, const void* in, void* out, bool inverse) {
+    Seq<T> s{h, h->stream};
+    const int L = h->L;
+    dim3 blk(32, 8), grd((L / 2 + 31) / 32, (L + 31) / 32);
+    if (!inverse) {
+        FCG_CK(h, s.row_fwd(ROWF_PLAIN, (const T*)in, nullptr));
+        FCG_CK(h, s.col(COL_FWD, false));
+        halfspec_export_kernel<T><<<grd, blk, 0, h->stream>>>(s.Tb(), (cx<T>*)out, L);
+        FCG_CK(h, cudaGetLastError());
+    } else {
+        halfspec_import_kernel<T><<<grd, blk, 0, h->stream>>>((const cx<T>*)in, s.Tb(), L);
+        FCG_CK(h, cudaGetLastError());
+        FCG_CK(h, s.col(COL_INV, false));
+        FCG_CK(h, s.row_inv(ROWI_PLAIN, nullptr, nullptr, nullptr, (T*)out, nullptr));
+    }
+    return FCG_OK;
+}
+
+template <typename T>
+int apply_impl(fcg_handle h, const void* k, const void* x, void* y) {
+    Seq<T> s{h, h->stream};
+    FCG_CK(h, s.row_fwd(ROWF_PLAIN, (const T*)x, nullptr));
+    FCG_CK(h, s.col(COL_CONV, false));
+    FCG_CK(h, s.row_inv(ROWI_APPLY, (const T*)k, (const T*)x, nullptr, (T*)y, nullptr));
+    return FCG_OK;
+}
+
+template <typename T>
+int twiddle_init(fcg_handle h) {
+    std::vector<cx<T>> tw(h->L);
+    for (int j = 0; j < h->L; ++j) {
+        const double ang = 2.0 * M_PI * (double)j / (double)h->L;
+        tw[j].x = (T)std::cos(ang); tw[j].y = (T)(-std::sin(ang));
+    }
+    FCG_CK(h, cudaMemcpyAsync(h->at<void>(h->lay.tw), tw.data(), tw.size() * sizeof(cx<T>), cudaMemcpyHostToDevice, h->stream));
+    FCG_CK(h, cudaStreamSynchronize(h->stream));
+    return FCG_OK;
+}
+
+bool supported(int L) { return L >= 16 && L <= 8192 && (L & (L - 1)) == 0; }
+
+}  // namespace
+
+// ================================================================================== C ABI
+extern "C" {
+
+const char* fcg_version(void) { return "fcg 0.1 (sm_100a)"; }
+
+size_t fcg_workspace_bytes(int L, fcg_dtype dt) {
+    if (!supported(L) || (dt != FCG_F32 && dt != FCG_F64)) return 0;
+    return make_layout(L, dt == FCG_F64 ? 8 : 4).total;
+}
+
+int fcg_create(int L, fcg_dtype dt, void* workspace, void* cuda_stream, fcg_handle* out) {
+    if (!out) return FCG_INVALID_ARG;
+    *out = nullptr;
+    if (dt != FCG_F32 && dt != FCG_F64) return FCG_INVALID_ARG;
+    if (!supported(L)) return FCG_UNSUPPORTED;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) { cudaGetLastError(); return FCG_CUDA_ERROR; }
+    fcg_handle h = new fcg_handle_s();
+    h->L = L; h->dtype = dt; h->w = dt == FCG_F64 ? 8 : 4; h->N = (size_t)L * L;
+    h->tab = get_table(L, dt);
+    h->stream = (cudaStream_t)cuda_stream;
+    h->lay = make_layout(L, h->w);
+    auto bail = [&](int code) { fcg_destroy(h); return code; };
+    if (workspace) { h->ws = (char*)workspace; }
+    else {
+        if (cudaMalloc((void**)&h->ws, h->lay.total) != cudaSuccess) { cudaGetLastError(); return bail(FCG_CUDA_ERROR); }
+        h->own_ws = true;
+    }
+    if (cudaMallocHost((void**)&h->h_sc, sizeof(Scalars)) != cudaSuccess) return bail(FCG_CUDA_ERROR);
+    if (cudaMallocHost((void**)&h->h_brk, sizeof(BreakResult)) != cudaSuccess) return bail(FCG_CUDA_ERROR);
+    std::memset(h->h_sc, 0, sizeof(Scalars));
+    if (cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking) != cudaSuccess) return bail(FCG_CUDA_ERROR);
+    if (h->tab->init() != cudaSuccess) return bail(FCG_CUDA_ERROR);
+    if (cudaMemsetAsync(h->ws + h->lay.scalars, 0, h->lay.total - h->lay.scalars, h->stream) != cudaSuccess) return bail(FCG_CUDA_ERROR);
+    int st = dt == FCG_F64 ? twiddle_init<double>(h) : twiddle_init<float>(h);
+    if (st != FCG_OK) return bail(st);
+    *out = h;
+    return FCG_OK;
+}
+
+int fcg_destroy(fcg_handle h) {
+    if (!h) return FCG_INVALID_ARG;
+    if (h->stream || h->ws) cudaStreamSynchronize(h->stream);
+    for (auto& g : h->graphs) drop_graph(g);
+    if (h->cap_stream) cudaStreamDestroy(h->cap_stream);
+    if (h->own_ws && h->ws) cudaFree(h->ws);
+    if (h->h_sc) cudaFreeHost(h->h_sc);
+    if (h->h_brk) cudaFreeHost(h->h_brk);
+    if (h->hk) cudaFree(h->hk);
+    if (h->hf) cudaFree(h->hf);
+    if (h->hu) cudaFree(h->hu);
+    cudaGetLastError();
+    delete h;
+    return FCG_OK;
+}
+
+int fcg_set_option(fcg_handle h, int option, int value) {
+    if (!h) return FCG_INVALID_ARG;
+    switch (option) {
+        case FCG_OPT_LOOP_MODE: if (value != 0 && value != 1) return fail(h, FCG_INVALID_ARG, "loop mode must be 0 or 1"); h->loop_mode = value; return FCG_OK;
+        case FCG_OPT_CHUNK: if (value < 1) return fail(h, FCG_INVALID_ARG, "chunk must be >= 1"); h->chunk = value; return FCG_OK;
+        case FCG_OPT_ROW_VARIANT:
+            if (value >= FCG_NROWVAR || (value >= 0 && !h->tab->row_valid[value])) return fail(h, FCG_INVALID_ARG, "row variant not available for this size");
+            h->row_var_opt = value; return FCG_OK;
+    }
+    return fail(h, FCG_INVALID_ARG, "unknown option");
+}
+
+int fcg_set_spectrum(fcg_handle h, const void* s) {
+    if (!h || !s) return fail(h, FCG_INVALID_ARG, "null argument");
+    FCG_CK(h, h->tab->spectrum_prep(s, h->at<void>(h->lay.shat), h->stream));
+    FCG_CK(h, cudaStreamSynchronize(h->stream));      // the caller's array is not referenced after return
+    h->have_spectrum = true;
+    return FCG_OK;
+}
+
+int fcg_apply(fcg_handle h, const void* k, const void* x, void* y) {
+    if (!h || !k || !x || !y) return fail(h, FCG_INVALID_ARG, "null argument");
+    if (y == k || y == x) return fail(h, FCG_INVALID_ARG, "y must not alias k or x");
+    if (!h->have_spectrum) return fail(h, FCG_NO_SPECTRUM, "fcg_set_spectrum has not been called");
+    return h->dtype == FCG_F64 ? apply_impl<double>(h, k, x, y) : apply_impl<float>(h, k, x, y);
+}
+
+int fcg_solve(fcg_handle h, const void* k, const void* f, void* u, double tol, int maxit, int* iters_host, double* rel_residual_host) {
+    if (!h || !k || !f || !u) return fail(h, FCG_INVALID_ARG, "null argument");
+    if (!(tol >= 0.0) || maxit < 0) return fail(h, FCG_INVALID_ARG, "tol must be >= 0 and maxit >= 0");
+    if (!h->have_spectrum) return fail(h, FCG_NO_SPECTRUM, "fcg_set_spectrum has not been called");
+    return h->dtype == FCG_F64 ? solve_impl<double>(h, k, f, u, tol, maxit, iters_host, rel_residual_host)
+                               : solve_impl<float>(h, k, f, u, tol, maxit, iters_host, rel_residual_host);
+}
+
+int fcg_solve_host(fcg_handle h, const void* k_host, const void* f_host, void* u_host, double tol, int maxit,
+                   int* iters_host, double* rel_residual_host) {
+    if (!h || !k_host || !f_host || !u_host) return fail(h, FCG_INVALID_ARG, "null argument");
+    const size_t bytes = h->N * h->w;
+    if (!h->hk) { FCG_CK(h, cudaMalloc(&h->hk, bytes)); FCG_CK(h, cudaMalloc(&h->hf, bytes)); FCG_CK(h, cudaMalloc(&h->hu, bytes)); }
+    FCG_CK(h, cudaMemcpyAsync(h->hk, k_host, bytes, cudaMemcpyHostToDevice, h->stream));
+    FCG_CK(h, cudaMemcpyAsync(h->hf, f_host, bytes, cudaMemcpyHostToDevice, h->stream));
+    FCG_CK(h, cudaMemcpyAsync(h->hu, u_host, bytes, cudaMemcpyHostToDevice, h->stream));
+    int st = fcg_solve(h, h->hk, h->hf, h->hu, tol, maxit, iters_host, rel_residual_host);
+    if (st < 0 && st != FCG_BREAKDOWN) return st;
+    FCG_CK(h, cudaMemcpyAsync(u_host, h->hu, bytes, cudaMemcpyDeviceToHost, h->stream));
+    FCG_CK(h, cudaStreamSynchronize(h->stream));
+    return st;
+}
+
+int fcg_fft_fwd(fcg_handle h, const void* x, void* X) {
+    if (!h || !x || !X) return fail(h, FCG_INVALID_ARG, "null argument");
+    return h->dtype == FCG_F64 ? fft_impl<double>(h, x, X, false) : fft_impl<float>(h, x, X, false);
+}
+
+int fcg_fft_inv(fcg_handle h, const void* X, void* x) {
+    if (!h || !x || !X) return fail(h, FCG_INVALID_ARG, "null argument");
+    return h->dtype == FCG_F64 ? fft_impl<double>(h, X, x, true) : fft_impl<float>(h, X, x, true);
+}
+
+int fcg_break_step(fcg_handle h, void* k, const void* u, const void* t, long long* index_host, double* ratio_host) {
+    if (!h || !k || !u || !t) return fail(h, FCG_INVALID_ARG, "null argument");
+    h->launches = 0;
+    return h->dtype == FCG_F64 ? break_impl<double>(h, k, u, t, index_host, ratio_host)
+                               : break_impl<float>(h, k, u, t, index_host, ratio_host);
+}
+
+int fcg_fracture(fcg_handle h, void* k, const void* f, void* u, const void* t, int nsteps, double tol, int maxit,
+                 long long* index_host, int* iters_host, int* steps_done_host) {
+    if (!h || !k || !f || !u || !t || nsteps < 0 || !index_host || !iters_host) return fail(h, FCG_INVALID_ARG, "bad argument");
+    long long total = 0; int done = 0, st = FCG_OK;
+    for (int step = 0; step < nsteps; ++step) {
+        int it = 0; double rr = 0.0;
+        st = fcg_solve(h, k, f, u, tol, maxit, &it, &rr);
+        total += h->launches;
+        if (st < 0) break;
+        long long idx = -1; double ratio = 0.0;
+        st = fcg_break_step(h, k, u, t, &idx, &ratio);
+        total += h->launches;
+        if (st < 0) break;
+        index_host[step] = idx; iters_host[step] = it; ++done; st = FCG_OK;
+    }
+    if (steps_done_host) *steps_done_host = done;
+    h->launches = total;
+    return st;
+}
+
+long long fcg_last_launch_count(fcg_handle h) { return h ? h->launches : -1; }
+
+const char* fcg_last_error(fcg_handle h) { return h ? h->err.c_str() : "null handle"; }
+
+}  // extern "C"

@@ -1,0 +1,86 @@
+// fcg_engine.cuh -- one transform stage as seen by one thread, with pluggable element load/store.
+//
+// A stage of plan P (fcg_math.cuh) consists of N/R independent radix-R butterflies.  A transform is
+// worked on by P::NT = N/RMAX threads; thread `lt` owns butterflies g = lt + i*NT.  Consecutive
+// threads own consecutive elements, so both the shared-memory accesses (after Swz) and the global
+// accesses of the first/last stage are contiguous across a warp.
+//
+// ld(e) returns logical element e of the transform, st(e, v) stores it.  "Logical" means the plain
+// in-place index; the caller maps it to swizzled shared memory or to global memory.
+#pragma once
+#include "fcg_math.cuh"
+
+namespace fcg {
+
+// tw[j] = exp(-2 pi i j / N), j = 0..N-1 (forward sign); the inverse uses the conjugate.
+template <typename P, int s, int DIR, typename T, typename LD, typename ST>
+FCG_HD void run_stage(int lt, const cx<T>* __restrict__ tw, LD ld, ST st)
+{
+    constexpr int R = P::radix(s);
+    constexpr int M = P::mlen(s);          // sub-block length
+    constexpr int Q = M / R;               // element stride inside a butterfly
+    constexpr int NB = P::N / R;           // butterflies in this stage
+    constexpr int PER = NB / P::NT;        // butterflies per thread
+    constexpr int PRE = P::prefix(s);      // w_M^{j u} = tw[j u PRE]
+    static_assert(PER >= 1, "plan: NT too large for this radix");
+#pragma unroll
+    for (int i = 0; i < PER; ++i) {
+        const int g = lt + i * P::NT;
+        const int blk = g / Q, j = g % Q;
+        const int base = blk * M + j;
+        cx<T> a[R];
+#pragma unroll
+        for (int t = 0; t < R; ++t) a[t] = ld(base + t * Q);
+        if (DIR < 0) {
+            dftR<R, -1>(a);
+            if (Q > 1) {
+#pragma unroll
+                for (int u = 1; u < R; ++u) a[u] = cmulw(a[u], tw[j * u * PRE]);
+            }
+        } else {
+            if (Q > 1) {
+#pragma unroll
+                for (int u = 1; u < R; ++u) a[u] = cmulwc(a[u], tw[j * u * PRE]);
+            }
+            dftR<R, +1>(a);
+        }
+#pragma unroll
+        for (int t = 0; t < R; ++t) st(base + t * Q, a[t]);
+    }
+}
+
+// Last forward stage, a pointwise real multiply, and the first inverse stage, all in registers:
+//   a <- DFT_R(a);  a[u] *= mul(e_u);  a <- DFT_R^H(a)
+// (the last stage has Q = 1, so no twiddles are involved).  mul(e) returns the real factor for position e.
+template <typename P, typename T, typename LD, typename ST, typename MUL>
+FCG_HD void run_middle(int lt, LD ld, ST st, MUL mul)
+{
+    constexpr int R = P::RLAST;
+    constexpr int NB = P::N / R;
+    constexpr int PER = NB / P::NT;
+#pragma unroll
+    for (int i = 0; i < PER; ++i) {
+        const int base = (lt + i * P::NT) * R;
+        cx<T> a[R];
+#pragma unroll
+        for (int t = 0; t < R; ++t) a[t] = ld(base + t);
+        dftR<R, -1>(a);
+#pragma unroll
+        for (int u = 0; u < R; ++u) { const T sv = mul(base + u); a[u].x *= sv; a[u].y *= sv; }
+        dftR<R, +1>(a);
+#pragma unroll
+        for (int t = 0; t < R; ++t) st(base + t, a[t]);
+    }
+}
+
+// Compile-time loops over the middle stages (everything between the first and the last stage lives in
+// shared memory and needs a barrier after each stage; `sync()` is __syncthreads on the device and a
+// no-op in the host harness, which runs whole phases thread by thread instead).
+template <typename T, typename P> struct SmemIO {
+    using S = Swz<T, P::RLAST>;
+    cx<T>* sm;
+    FCG_HD cx<T> ld(int e) const { return sm[S::at(e)]; }
+    FCG_HD void st(int e, cx<T> v) const { sm[S::at(e)] = v; }
+};
+
+}  // namespace fcg

@@ -1,0 +1,102 @@
+// fcg_inst.cu -- instantiates the transform passes for one lattice size.  Compiled once per supported L
+// with -DFCG_INST_L=<L> (paper_1305_3625_b200/build.py) so the sizes build in parallel.
+#include "fcg_kernels.cuh"
+#include "fcg_plans.cuh"
+
+#ifndef FCG_INST_L
+#error "compile with -DFCG_INST_L=<L>"
+#endif
+
+namespace fcg {
+namespace {
+
+template <typename T> struct Inst {
+    using P = typename PlanFor<T, FCG_INST_L>::type;
+    using RS = RowShape<T, P>;
+    using CS = ColShape<T, P>;
+    static constexpr int L = FCG_INST_L;
+
+    template <int V> static cudaError_t init_row() {
+        if constexpr (RS::valid(V)) {
+            cudaError_t e = cudaFuncSetAttribute(row_fwd_kernel<T, P, RS::F(V)>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RS::smem(V));
+            if (e != cudaSuccess) return e;
+            return cudaFuncSetAttribute(row_inv_kernel<T, P, RS::F(V)>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RS::smem(V));
+        }
+        return cudaSuccess;
+    }
+    static cudaError_t init() {
+        cudaError_t e;
+        if ((e = init_row<0>()) != cudaSuccess) return e;
+        if ((e = init_row<1>()) != cudaSuccess) return e;
+        if ((e = init_row<2>()) != cudaSuccess) return e;
+        if ((e = init_row<3>()) != cudaSuccess) return e;
+        return cudaFuncSetAttribute(col_kernel<T, P, CS::COLS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)CS::smem);
+    }
+
+    template <int V> static cudaError_t row_fwd_v(const RowFwdArgs<T>& A, cudaStream_t st) {
+        if constexpr (RS::valid(V)) {
+            row_fwd_kernel<T, P, RS::F(V)><<<L / (2 * RS::F(V)), RS::F(V) * P::NT, RS::smem(V), st>>>(A);
+            return cudaGetLastError();
+        }
+        return cudaErrorInvalidValue;
+    }
+    static cudaError_t row_fwd(int var, const void* args, cudaStream_t st) {
+        const RowFwdArgs<T>& A = *static_cast<const RowFwdArgs<T>*>(args);
+        switch (var) {
+            case 0: return row_fwd_v<0>(A, st);
+            case 1: return row_fwd_v<1>(A, st);
+            case 2: return row_fwd_v<2>(A, st);
+            case 3: return row_fwd_v<3>(A, st);
+        }
+        return cudaErrorInvalidValue;
+    }
+    template <int V> static cudaError_t row_inv_v(const RowInvArgs<T>& A, cudaStream_t st) {
+        if constexpr (RS::valid(V)) {
+            row_inv_kernel<T, P, RS::F(V)><<<L / (2 * RS::F(V)), RS::F(V) * P::NT, RS::smem(V), st>>>(A);
+            return cudaGetLastError();
+        }
+        return cudaErrorInvalidValue;
+    }
+    static cudaError_t row_inv(int var, const void* args, cudaStream_t st) {
+        const RowInvArgs<T>& A = *static_cast<const RowInvArgs<T>*>(args);
+        switch (var) {
+            case 0: return row_inv_v<0>(A, st);
+            case 1: return row_inv_v<1>(A, st);
+            case 2: return row_inv_v<2>(A, st);
+            case 3: return row_inv_v<3>(A, st);
+        }
+        return cudaErrorInvalidValue;
+    }
+    static cudaError_t col(const void* args, cudaStream_t st) {
+        const ColArgs<T>& A = *static_cast<const ColArgs<T>*>(args);
+        col_kernel<T, P, CS::COLS><<<(L / 2) / CS::COLS, CS::COLS * P::NT, CS::smem, st>>>(A);
+        return cudaGetLastError();
+    }
+    static cudaError_t spectrum_prep(const void* s, void* shat, cudaStream_t st) {
+        spectrum_prep_kernel<T, P><<<148 * 2, 256, 0, st>>>(static_cast<const T*>(s), static_cast<T*>(shat));
+        return cudaGetLastError();
+    }
+    static PassTable make(int dtype) {
+        PassTable t{};
+        t.L = L; t.dtype = dtype;
+        for (int v = 0; v < FCG_NROWVAR; ++v) {
+            t.row_valid[v] = RS::valid(v); t.row_F[v] = RS::F(v);
+            t.row_threads[v] = RS::F(v) * P::NT; t.row_smem[v] = RS::smem(v);
+        }
+        t.cols = CS::COLS; t.col_threads = CS::COLS * P::NT; t.col_smem = CS::smem;
+        t.init = &init; t.row_fwd = &row_fwd; t.col = &col; t.row_inv = &row_inv; t.spectrum_prep = &spectrum_prep;
+        return t;
+    }
+};
+
+}  // namespace
+
+#define FCG_CAT2(a, b) a##b
+#define FCG_CAT(a, b) FCG_CAT2(a, b)
+const PassTable* FCG_CAT(fcg_pass_table_, FCG_INST_L)(int dtype) {
+    static const PassTable t32 = Inst<float>::make(0);
+    static const PassTable t64 = Inst<double>::make(1);
+    return dtype == 0 ? &t32 : &t64;
+}
+
+}  // namespace fcg

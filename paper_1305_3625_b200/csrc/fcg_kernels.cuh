@@ -1,0 +1,328 @@
+// fcg_kernels.cuh -- __global__ entry points of libfcg.
+//   transform passes (templated on plan): row_fwd_kernel, col_kernel, row_inv_kernel, spectrum_prep_kernel
+//   BLAS-1 of Listing 2 with device-side reductions and convergence test:
+//       cg_setup_kernel, cg_update_r_kernel, cg_finish_kernel
+//   break step (BASELINE.json configs[3]): break_argmax_kernel
+//   public half-spectrum layout helpers: halfspec_export/import kernels
+#pragma once
+#include <cuda_runtime.h>
+#include "fcg_passes.cuh"
+
+namespace fcg {
+
+constexpr int ST_OK = 0, ST_NOT_CONVERGED = 1, ST_BREAKDOWN = -4;
+
+struct DevRunner {
+    template <typename Fn> FCG_HD void operator()(Fn&& f) {
+#ifdef __CUDA_ARCH__
+        f((int)threadIdx.x);
+        __syncthreads();
+#else
+        (void)f;
+#endif
+    }
+};
+
+#ifdef __CUDACC__
+__device__ __forceinline__ void set_cond(const Scalars* sc, bool go) {
+    if (sc->use_cond) cudaGraphSetConditional((cudaGraphConditionalHandle)sc->cond, go ? 1u : 0u);
+}
+
+// Sum of one double per thread over the CTA, fixed tree (bit-reproducible). Result valid in thread 0.
+template <int NV>
+__device__ __forceinline__ void block_sum(double (&v)[NV], double* red /* [NV][32] shared */) {
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
+#pragma unroll
+    for (int q = 0; q < NV; ++q) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v[q] += __shfl_down_sync(0xffffffffu, v[q], o);
+        if (lane == 0) red[q * 32 + w] = v[q];
+    }
+    __syncthreads();
+    if (w == 0) {
+#pragma unroll
+        for (int q = 0; q < NV; ++q) {
+            double x = lane < nw ? red[q * 32 + lane] : 0.0;
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) x += __shfl_down_sync(0xffffffffu, x, o);
+            v[q] = x;
+        }
+    }
+}
+
+// Publish this CTA's partial sums; the last CTA to arrive adds all partials in a fixed order and
+// returns true in every one of its threads with the totals in tot[] (valid in thread 0).
+template <int NV>
+__device__ __forceinline__ bool grid_sum_last(double (&v)[NV], double* partial, unsigned int* ticket,
+                                              double* red, double (&tot)[NV]) {
+    __shared__ int is_last;
+    block_sum<NV>(v, red);
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int q = 0; q < NV; ++q) partial[(size_t)blockIdx.x * NV + q] = v[q];
+        __threadfence();
+        const unsigned int t = atomicAdd(ticket, 1u);
+        is_last = (t == gridDim.x - 1);
+    }
+    __syncthreads();
+    if (!is_last) return false;
+    __threadfence();
+#pragma unroll
+    for (int q = 0; q < NV; ++q) tot[q] = 0.0;
+    for (unsigned int b = threadIdx.x; b < gridDim.x; b += blockDim.x)
+#pragma unroll
+        for (int q = 0; q < NV; ++q) tot[q] += __ldcg(partial + (size_t)b * NV + q);
+    __syncthreads();
+    block_sum<NV>(tot, red);
+    if (threadIdx.x == 0) *ticket = 0u;
+    return true;
+}
+
+// ------------------------------------------------------------------------------- transform passes
+template <typename T, typename P, int F>
+__global__ void __launch_bounds__(F * P::NT) row_fwd_kernel(const RowFwdArgs<T> A) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    if (A.mode == ROWF_CG && A.sc->done) return;
+    DevRunner run;
+    row_fwd_body<T, P, F>(A, (int)blockIdx.x, reinterpret_cast<cx<T>*>(smem_raw), run);
+}
+
+template <typename T, typename P, int COLS>
+__global__ void __launch_bounds__(COLS * P::NT) col_kernel(const ColArgs<T> A) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    if (A.sc && A.sc->done) return;
+    DevRunner run;
+    col_body<T, P, COLS>(A, (int)blockIdx.x, reinterpret_cast<cx<T>*>(smem_raw), run);
+}
+
+template <typename T, typename P, int F>
+__global__ void __launch_bounds__(F * P::NT) row_inv_kernel(const RowInvArgs<T> A) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    __shared__ double red[2 * 32];
+    if (A.mode == ROWI_CG && A.sc->done) return;
+    DevRunner run;
+    double acc[2] = {0.0, 0.0};
+    row_inv_body<T, P, F>(A, (int)blockIdx.x, reinterpret_cast<cx<T>*>(smem_raw), run, acc);
+    if (A.mode != ROWI_CG && A.mode != ROWI_RESID) return;
+    double tot[2];
+    if (!grid_sum_last<2>(acc, A.partial, &A.sc->ticket[0], red, tot)) return;
+    if (threadIdx.x != 0) return;
+    Scalars* sc = A.sc;
+    if (A.mode == ROWI_CG) {
+        const double pq = tot[0];
+        sc->pq = pq;
+        if (!(pq > 0.0) || !isfinite(pq)) { sc->status = ST_BREAKDOWN; sc->done = 1; sc->alpha = 0.0; }
+        else sc->alpha = sc->rho / pq;                                   // search length
+    } else {                                                             // set up initial values
+        const double rho = tot[0], fn2 = tot[1];
+        sc->rho = rho; sc->fn2 = fn2; sc->it = 0; sc->alpha = 0.0; sc->beta = 0.0;
+        if (fn2 == 0.0) { sc->zero_u = 1; sc->done = 1; sc->status = ST_OK; sc->rho = 0.0; sc->relres = 0.0; }
+        else {
+            sc->relres = sqrt(rho) / sqrt(fn2);
+            if (sqrt(rho) <= sc->tol * sqrt(fn2)) { sc->done = 1; sc->status = ST_OK; }
+            else if (sc->maxit <= 0) { sc->done = 1; sc->status = ST_NOT_CONVERGED; }
+        }
+        set_cond(sc, !sc->done);
+    }
+}
+
+template <typename T, typename P>
+__global__ void spectrum_prep_kernel(const T* __restrict__ s, T* __restrict__ shat) {
+    constexpr int L = P::N;
+    for (int idx = blockIdx.x * blockDim.x + threadIdx.x; idx < L * (L / 2); idx += gridDim.x * blockDim.x)
+        spectrum_prep_one<T, P>(idx, s, shat);
+}
+
+// ------------------------------------------------------------------------------- CG vector kernels
+struct SetupArgs { double tol; int maxit; int use_cond; unsigned long long cond; };
+
+#ifdef FCG_MAIN_TU   // non-template kernel: defined in fcg.cu only
+__global__ void cg_setup_kernel(Scalars* sc, SetupArgs a) {
+    if (threadIdx.x == 0 && blockIdx.x == 0) {
+        sc->rho = 0; sc->pq = 0; sc->alpha = 0; sc->beta = 0; sc->fn2 = 0; sc->relres = 0;
+        sc->tol = a.tol; sc->maxit = a.maxit; sc->it = 0; sc->done = 0; sc->status = 0; sc->zero_u = 0;
+        sc->use_cond = a.use_cond; sc->cond = a.cond;
+        sc->ticket[0] = sc->ticket[1] = sc->ticket[2] = sc->ticket[3] = 0u;
+    }
+}
+#endif
+
+template <typename T> struct Vec;
+template <> struct Vec<double> { using type = double2; static constexpr int W = 2; };
+template <> struct Vec<float> { using type = float4; static constexpr int W = 4; };
+
+__device__ __forceinline__ void axpy_sq(double2& r, const double2 q, double a, double& acc) {
+    r.x = r.x - a * q.x; r.y = r.y - a * q.y;
+    acc += r.x * r.x; acc += r.y * r.y;
+}
+__device__ __forceinline__ void axpy_sq(float4& r, const float4 q, float a, double& acc) {
+    r.x = r.x - a * q.x; r.y = r.y - a * q.y; r.z = r.z - a * q.z; r.w = r.w - a * q.w;
+    acc += (double)r.x * (double)r.x; acc += (double)r.y * (double)r.y;
+    acc += (double)r.z * (double)r.z; acc += (double)r.w * (double)r.w;
+}
+
+// residue, residue length (97), update calculation variables (98: beta), check convergence (99)
+template <typename T>
+__global__ void __launch_bounds__(256) cg_update_r_kernel(T* __restrict__ r, const T* __restrict__ q, size_t nvec,
+                                                           double* partial, Scalars* sc) {
+    __shared__ double red[32];
+    using V = typename Vec<T>::type;
+    if (sc->done) {      // breakdown in this iteration, or (loop mode 1) already finished
+        if (blockIdx.x == 0 && threadIdx.x == 0) set_cond(sc, false);
+        return;
+    }
+    const T a = (T)sc->alpha;
+    double acc[1] = {0.0};
+    V* rv = reinterpret_cast<V*>(r);
+    const V* qv = reinterpret_cast<const V*>(q);
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < nvec; i += (size_t)gridDim.x * blockDim.x) {
+        V x = rv[i];
+        axpy_sq(x, __ldg(qv + i), a, acc[0]);
+        rv[i] = x;
+    }
+    double tot[1];
+    if (!grid_sum_last<1>(acc, partial, &sc->ticket[1], red, tot)) return;
+    if (threadIdx.x != 0) return;
+    const double rho_new = tot[0], fn2 = sc->fn2;
+    const int it = sc->it + 1;
+    sc->it = it;
+    if (sqrt(rho_new) <= sc->tol * sqrt(fn2)) { sc->done = 1; sc->status = ST_OK; }
+    else if (it >= sc->maxit) { sc->done = 1; sc->status = ST_NOT_CONVERGED; }
+    else sc->beta = rho_new / sc->rho;
+    sc->rho = rho_new;
+    sc->relres = sqrt(rho_new) / sqrt(fn2);
+    set_cond(sc, !sc->done);
+}
+
+// last lagged "new x" after the loop has ended; u = 0 when f = 0
+template <typename T>
+__global__ void __launch_bounds__(256) cg_finish_kernel(T* __restrict__ u, const T* __restrict__ p, size_t nvec, const Scalars* sc) {
+    using V = typename Vec<T>::type;
+    const int zero = sc->zero_u;
+    const T a = (T)sc->alpha;
+    if (!zero && a == (T)0) return;
+    V* uv = reinterpret_cast<V*>(u);
+    const V* pv = reinterpret_cast<const V*>(p);
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < nvec; i += (size_t)gridDim.x * blockDim.x) {
+        V x = uv[i];
+        T* xs = reinterpret_cast<T*>(&x);
+        if (zero) {
+#pragma unroll
+            for (int c = 0; c < Vec<T>::W; ++c) xs[c] = (T)0;
+        } else {
+            const V pp = __ldg(pv + i);
+            const T* ps = reinterpret_cast<const T*>(&pp);
+#pragma unroll
+            for (int c = 0; c < Vec<T>::W; ++c) xs[c] = xs[c] + a * ps[c];
+        }
+        uv[i] = x;
+    }
+}
+
+// ------------------------------------------------------------------------------- break step
+struct BreakResult { long long index; double ratio; int status; int pad; };
+
+__device__ __forceinline__ bool better(double ra, long long ia, double rb, long long ib) {
+    if (ia < 0) return false;
+    if (ib < 0) return true;
+    return ra > rb || (ra == rb && ia < ib);
+}
+
+template <typename T>
+__global__ void __launch_bounds__(256) break_argmax_kernel(T* __restrict__ k, const T* __restrict__ u, const T* __restrict__ t,
+                                                            long long n, double* pr, long long* pi, unsigned int* ticket,
+                                                            BreakResult* out) {
+    __shared__ double sr[32];
+    __shared__ long long si[32];
+    __shared__ int is_last;
+    double br = 0.0; long long bi = -1;
+    auto consider = [&](double r, long long i) { if (better(r, i, br, bi)) { br = r; bi = i; } };
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+        const T ki = k[i];
+        if (!(ki > (T)0)) continue;
+        const double load = (double)ki * (double)u[i];      // l_i = k_i u_i   (one IEEE multiply)
+        const double rt = load / (double)t[i];              // l_i / t_i       (one IEEE divide)
+        if (rt != rt) continue;
+        consider(rt, i);
+    }
+    auto warp_red = [&]() {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            const double r2 = __shfl_down_sync(0xffffffffu, br, o);
+            const long long i2 = __shfl_down_sync(0xffffffffu, bi, o);
+            consider(r2, i2);
+        }
+    };
+    auto block_red = [&]() {
+        const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+        warp_red();
+        if (lane == 0) { sr[w] = br; si[w] = bi; }
+        __syncthreads();
+        if (w == 0) {
+            br = lane < (int)(blockDim.x >> 5) ? sr[lane] : 0.0;
+            bi = lane < (int)(blockDim.x >> 5) ? si[lane] : -1;
+            warp_red();
+        }
+    };
+    block_red();
+    if (threadIdx.x == 0) {
+        pr[blockIdx.x] = br; pi[blockIdx.x] = bi;
+        __threadfence();
+        is_last = (atomicAdd(ticket, 1u) == gridDim.x - 1);
+    }
+    __syncthreads();
+    if (!is_last) return;
+    __threadfence();
+    br = 0.0; bi = -1;
+    for (unsigned int b = threadIdx.x; b < gridDim.x; b += blockDim.x) consider(__ldcg(pr + b), __ldcg(pi + b));
+    __syncthreads();
+    block_red();
+    if (threadIdx.x == 0) {
+        *ticket = 0u;
+        out->index = bi; out->ratio = br; out->status = bi < 0 ? -6 : 0;
+        if (bi >= 0) k[bi] = (T)0;
+    }
+}
+
+// ------------------------------------------------------------------------------- public half-spectrum layout
+// T2[n][m] (n < L/2, natural m; row 0 = W = Y0 + i YN) <-> X[m][n], n = 0..L/2, row length L/2+1.
+template <typename T>
+__global__ void halfspec_export_kernel(const cx<T>* __restrict__ T2, cx<T>* __restrict__ X, int L) {
+    __shared__ cx<T> tile[32][33];
+    const int n0 = blockIdx.x * 32, m0 = blockIdx.y * 32, W = L / 2 + 1;
+    for (int j = threadIdx.y; j < 32; j += blockDim.y)
+        if (n0 + j < L / 2 && m0 + (int)threadIdx.x < L) tile[j][threadIdx.x] = T2[(size_t)(n0 + j) * L + m0 + threadIdx.x];
+    __syncthreads();
+    for (int j = threadIdx.y; j < 32; j += blockDim.y) {
+        const int m = m0 + j, n = n0 + threadIdx.x;
+        if (n > 0 && n < L / 2 && m < L) X[(size_t)m * W + n] = tile[threadIdx.x][j];
+    }
+    if (blockIdx.x == 0 && threadIdx.y == 0 && m0 + (int)threadIdx.x < L) {        // unpack the n = 0 and n = L/2 columns
+        const int m = m0 + threadIdx.x, mm = (L - m) % L;
+        const cx<T> a = T2[m], b = T2[mm];
+        const T h = (T)0.5;
+        X[(size_t)m * W] = mk<T>((a.x + b.x) * h, (a.y - b.y) * h);
+        X[(size_t)m * W + L / 2] = mk<T>((a.y + b.y) * h, (b.x - a.x) * h);
+    }
+}
+
+template <typename T>
+__global__ void halfspec_import_kernel(const cx<T>* __restrict__ X, cx<T>* __restrict__ T2, int L) {
+    __shared__ cx<T> tile[32][33];
+    const int n0 = blockIdx.x * 32, m0 = blockIdx.y * 32, W = L / 2 + 1;
+    for (int j = threadIdx.y; j < 32; j += blockDim.y)
+        if (m0 + j < L && n0 + (int)threadIdx.x < L / 2) tile[j][threadIdx.x] = X[(size_t)(m0 + j) * W + n0 + threadIdx.x];
+    __syncthreads();
+    for (int j = threadIdx.y; j < 32; j += blockDim.y) {
+        const int n = n0 + j, m = m0 + threadIdx.x;
+        if (n > 0 && n < L / 2 && m < L) T2[(size_t)n * L + m] = tile[threadIdx.x][j];
+    }
+    if (blockIdx.x == 0 && threadIdx.y == 0 && m0 + (int)threadIdx.x < L) {
+        const int m = m0 + threadIdx.x;
+        const cx<T> x0 = X[(size_t)m * W], xN = X[(size_t)m * W + L / 2];
+        T2[m] = mk<T>(x0.x - xN.y, x0.y + xN.x);
+    }
+}
+#endif  // __CUDACC__
+
+}  // namespace fcg

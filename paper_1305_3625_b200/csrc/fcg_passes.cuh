@@ -1,0 +1,304 @@
+// fcg_passes.cuh -- the three transform passes of one operator application  q = k o p + C p
+// (Listing 4), each fused with its neighbouring vector work of Listing 2
+// (PAPER.md:88-100).  Data layout and byte counts: DESIGN.md sections 3-4.
+//
+//   row_fwd  (P1): [u += alpha p; p = r + beta p;]  T[n][a] = sum_b p[a,b] w^{n b},  n < L/2
+//   col_conv (P2): T[n][.] <- F_col^H ( shat[n][.] o F_col T[n][.] )               (in place)
+//   row_inv  (P3): c = F_row^H T;  q = k o p + c  [+ partial p.q]  (or residual / apply / plain)
+//
+// Two real rows are transformed by one complex FFT (z = x_even + i x_odd) and separated with
+// X_even[n] = (Z[n] + conj Z[L-n])/2, X_odd[n] = (Z[n] - conj Z[L-n])/(2i).  Row n = 0 of T packs the
+// two purely real columns n = 0 and n = L/2 as T[0][a] = X_a[0] + i X_a[L/2], so T is exactly
+// L/2 x L complex.  T is stored transposed (n-major) so that the column pass streams contiguous
+// columns; the transposition happens in the row passes through shared memory, with 2F*sizeof(complex)
+// contiguous bytes per n.
+//
+// Every body is written against a Runner: run(f) executes f(tid) for each thread of the CTA followed
+// by a CTA barrier.  On the device that is one call + __syncthreads(); the host harness
+// (tests/emul) loops over tid instead, which lets the index algebra be checked without a GPU.
+#pragma once
+#include <type_traits>
+#include "fcg_engine.cuh"
+
+namespace fcg {
+
+// Device-resident CG state (one per handle).  All scalars are double for both dtypes (reading S12).
+struct Scalars {
+    double rho, pq, alpha, beta, fn2, tol, relres;
+    int it, maxit, done, status, zero_u, use_cond;
+    unsigned int ticket[4];
+    unsigned long long cond;       // cudaGraphConditionalHandle of the WHILE node (loop mode 0)
+};
+
+enum { ROWF_PLAIN = 0, ROWF_CG = 1 };
+enum { ROWI_PLAIN = 0, ROWI_CG = 1, ROWI_RESID = 2, ROWI_APPLY = 3 };
+enum { COL_CONV = 0, COL_FWD = 1, COL_INV = 2 };
+
+template <typename T> struct RowFwdArgs {
+    int mode;
+    const T* x;            // PLAIN: input field
+    T* u; T* p; const T* r;        // CG: vectors updated in place / read
+    cx<T>* Tb;             // [L/2][L] transposed half spectrum
+    const cx<T>* tw;       // exp(-2 pi i j / L)
+    const Scalars* sc;
+};
+
+template <typename T> struct ColArgs {
+    int mode;
+    cx<T>* Tb;             // in place
+    const T* shat;         // [(L/2)+1][L], digit-reversed along m, pre-scaled by 1/L^2
+    const cx<T>* tw;
+    const Scalars* sc;
+};
+
+template <typename T> struct RowInvArgs {
+    int mode;
+    const cx<T>* Tb;
+    const cx<T>* tw;
+    const T* k; const T* v; const T* f;   // CG: v = p;  RESID: v = u, f;  APPLY: v = x
+    T* out; T* out2;                      // CG: q;  RESID: r, p(:=0);  APPLY: y;  PLAIN: x
+    T scale;                              // PLAIN: 1/L^2
+    double* partial;                      // [gridDim.x][2]
+    Scalars* sc;
+};
+
+template <int A, int B, typename F> FCG_HD void static_for_up(F&& f) {
+    if constexpr (A <= B) { f(std::integral_constant<int, A>{}); static_for_up<A + 1, B>(f); }
+}
+template <int A, int B, typename F> FCG_HD void static_for_down(F&& f) {
+    if constexpr (A >= B) { f(std::integral_constant<int, A>{}); static_for_down<A - 1, B>(f); }
+}
+
+// Region stride of one packed transform in shared memory (elements).  The +2 skew puts the F regions of a
+// row-pass CTA on different banks when F lanes read the same position of F different transforms.
+template <typename P> constexpr int region_stride() { return P::N + 2; }
+
+// shat[n][pos(m)] from the caller's s[m][n]: even part, 1/L^2, digit-reversed along m; row 0 and row L/2
+// hold (s0 + sN)/2 and (s0 - sN)/2 for the packed n = 0 / n = L/2 column (col_body).  idx = m*(L/2) + n.
+template <typename T, typename P>
+FCG_HD void spectrum_prep_one(int idx, const T* __restrict__ s, T* __restrict__ shat) {
+    constexpr int L = P::N;
+    const T scale = (T)(1.0 / ((double)L * (double)L));
+    const T h = (T)0.5;
+    const int m = idx / (L / 2), n = idx % (L / 2);
+    const int mm = (L - m) % L;
+    const int e = P::pos_of(m);
+    if (n > 0) {
+        const T ev = (s[(size_t)m * L + n] + s[(size_t)mm * L + (L - n)]) * h;
+        shat[(size_t)n * L + e] = ev * scale;
+    } else {
+        const T s0 = (s[(size_t)m * L] + s[(size_t)mm * L]) * h * scale;
+        const T sN = (s[(size_t)m * L + L / 2] + s[(size_t)mm * L + L / 2]) * h * scale;
+        shat[e] = (s0 + sN) * h;
+        shat[(size_t)(L / 2) * L + e] = (s0 - sN) * h;
+    }
+}
+
+// --------------------------------------------------------------------------------------------- P1
+template <typename T, typename P, int F, typename Runner>
+FCG_HD void row_fwd_body(const RowFwdArgs<T>& A, int block, cx<T>* smem, Runner& run)
+{
+    constexpr int L = P::N, S = P::S, NT = P::NT;
+    const int a0 = block * 2 * F;
+    T alpha = (T)0, beta = (T)0;
+    if (A.mode == ROWF_CG) { alpha = (T)A.sc->alpha; beta = (T)A.sc->beta; }
+
+    // stage 1: global -> (vector update) -> butterfly -> shared
+    run([&](int tid) {
+        const int f = tid / NT, lt = tid % NT;
+        SmemIO<T, P> io{smem + f * region_stride<P>()};
+        const size_t row0 = (size_t)(a0 + 2 * f) * L, row1 = row0 + L;
+        auto ld = [&](int e) -> cx<T> {
+            if (A.mode == ROWF_CG) {
+                T p0 = A.p[row0 + e], p1 = A.p[row1 + e];
+                const T r0 = A.r[row0 + e], r1 = A.r[row1 + e];
+                T u0 = A.u[row0 + e], u1 = A.u[row1 + e];
+                u0 = u0 + alpha * p0; u1 = u1 + alpha * p1;       // new x, lagged one pass
+                p0 = r0 + beta * p0;  p1 = r1 + beta * p1;        // new direction
+                A.u[row0 + e] = u0; A.u[row1 + e] = u1;
+                A.p[row0 + e] = p0; A.p[row1 + e] = p1;
+                return mk<T>(p0, p1);
+            }
+            return mk<T>(A.x[row0 + e], A.x[row1 + e]);
+        };
+        run_stage<P, 1, -1, T>(lt, A.tw, ld, [&](int e, cx<T> v) { io.st(e, v); });
+    });
+    // stages 2..S in shared memory
+    static_for_up<2, S>([&](auto s) {
+        run([&](int tid) {
+            const int f = tid / NT, lt = tid % NT;
+            SmemIO<T, P> io{smem + f * region_stride<P>()};
+            run_stage<P, decltype(s)::value, -1, T>(lt, A.tw, [&](int e) { return io.ld(e); },
+                                                    [&](int e, cx<T> v) { io.st(e, v); });
+        });
+    });
+    // separate the two rows of each packed transform and store transposed: lanes run over f first, so a
+    // warp writes 2F consecutive complex numbers per n
+    run([&](int tid) {
+        constexpr int ITEMS = F * (L / 2), NTH = F * NT;
+        const T h = (T)0.5;
+#pragma unroll 4
+        for (int item = tid; item < ITEMS; item += NTH) {
+            const int f = item % F, n = item / F;
+            SmemIO<T, P> io{smem + f * region_stride<P>()};
+            cx<T> X0, X1;
+            if (n == 0) {
+                const cx<T> Z0 = io.ld(P::pos_of(0)), ZN = io.ld(P::pos_of(L / 2));
+                X0 = mk<T>(Z0.x, ZN.x); X1 = mk<T>(Z0.y, ZN.y);
+            } else {
+                const cx<T> Za = io.ld(P::pos_of(n)), Zb = io.ld(P::pos_of(L - n));
+                X0 = mk<T>((Za.x + Zb.x) * h, (Za.y - Zb.y) * h);
+                X1 = mk<T>((Za.y + Zb.y) * h, (Zb.x - Za.x) * h);
+            }
+            cx<T>* dst = A.Tb + (size_t)n * L + a0 + 2 * f;
+            dst[0] = X0; dst[1] = X1;
+        }
+    });
+}
+
+// --------------------------------------------------------------------------------------------- P2
+// COLS columns per CTA, column n = block*COLS + c, region c of shared memory.
+template <typename T, typename P, int COLS, typename Runner>
+FCG_HD void col_body(const ColArgs<T>& A, int block, cx<T>* smem, Runner& run)
+{
+    constexpr int L = P::N, S = P::S, NT = P::NT;
+    const int n0 = block * COLS;
+    const bool special = (A.mode == COL_CONV) && (n0 == 0);    // this CTA holds the packed n=0 / n=L/2 column
+    auto region = [&](int tid) { return SmemIO<T, P>{smem + (tid / NT) * region_stride<P>()}; };
+    auto column = [&](int tid) { return A.Tb + (size_t)(n0 + tid / NT) * L; };
+
+    auto fwd_stage = [&](auto s) {           // stage s forward: loads global iff s == 1, stores shared
+        run([&](int tid) {
+            auto io = region(tid); cx<T>* col = column(tid);
+            constexpr int sv = decltype(s)::value;
+            if constexpr (sv == 1)
+                run_stage<P, 1, -1, T>(tid % NT, A.tw, [&](int e) { return col[e]; }, [&](int e, cx<T> v) { io.st(e, v); });
+            else
+                run_stage<P, sv, -1, T>(tid % NT, A.tw, [&](int e) { return io.ld(e); }, [&](int e, cx<T> v) { io.st(e, v); });
+        });
+    };
+    auto inv_stage = [&](auto s) {           // stage s inverse: loads shared, stores global iff s == 1
+        run([&](int tid) {
+            auto io = region(tid); cx<T>* col = column(tid);
+            constexpr int sv = decltype(s)::value;
+            if constexpr (sv == 1)
+                run_stage<P, 1, +1, T>(tid % NT, A.tw, [&](int e) { return io.ld(e); }, [&](int e, cx<T> v) { col[e] = v; });
+            else
+                run_stage<P, sv, +1, T>(tid % NT, A.tw, [&](int e) { return io.ld(e); }, [&](int e, cx<T> v) { io.st(e, v); });
+        });
+    };
+
+    if (A.mode == COL_CONV && !special) {
+        static_for_up<1, S - 1>(fwd_stage);
+        run([&](int tid) {                   // last forward stage * shat * first inverse stage, in registers
+            auto io = region(tid); cx<T>* col = column(tid);
+            const T* sh = A.shat + (size_t)(n0 + tid / NT) * L;
+            if constexpr (S == 1)
+                run_middle<P, T>(tid % NT, [&](int e) { return col[e]; }, [&](int e, cx<T> v) { col[e] = v; },
+                                 [&](int e) { return sh[e]; });
+            else
+                run_middle<P, T>(tid % NT, [&](int e) { return io.ld(e); }, [&](int e, cx<T> v) { io.st(e, v); },
+                                 [&](int e) { return sh[e]; });
+        });
+        static_for_down<S - 1, 1>(inv_stage);
+        return;
+    }
+    if (A.mode == COL_CONV) {                // special CTA: column 0 needs W[m] and W[-m] together
+        static_for_up<1, S>(fwd_stage);
+        run([&](int tid) {
+            auto io = region(tid);
+            const int c = tid / NT, lt = tid % NT;
+            const T* sh = A.shat + (size_t)(n0 + c) * L;
+            if (c == 0) {
+                // packed column: W = Y0 + i YN.  W'[m] = sp[m] W[m] + sm[m] conj W[-m],
+                // sp = (s0 + sN)/2 (row 0 of shat), sm = (s0 - sN)/2 (row L/2 of shat); pairs (m, L-m), m <= L/2
+                const T* sm_ = A.shat + (size_t)(L / 2) * L;
+                for (int m = lt; m <= L / 2; m += NT) {
+                    const int e = P::pos_of(m), e2 = P::pos_of((L - m) % L);
+                    const cx<T> Wa = io.ld(e), Wb = io.ld(e2);
+                    cx<T> va, vb;
+                    va.x = sh[e] * Wa.x + sm_[e] * Wb.x;   va.y = sh[e] * Wa.y - sm_[e] * Wb.y;
+                    vb.x = sh[e2] * Wb.x + sm_[e2] * Wa.x; vb.y = sh[e2] * Wb.y - sm_[e2] * Wa.y;
+                    io.st(e, va);
+                    if (e2 != e) io.st(e2, vb);
+                }
+            } else {
+                for (int e = lt; e < L; e += NT) { cx<T> w = io.ld(e); w.x *= sh[e]; w.y *= sh[e]; io.st(e, w); }
+            }
+        });
+        static_for_down<S, 1>(inv_stage);
+        return;
+    }
+    if (A.mode == COL_FWD) {                 // public transform: forward only, natural m order out (in place)
+        static_for_up<1, S>(fwd_stage);
+        run([&](int tid) {
+            auto io = region(tid); cx<T>* col = column(tid);
+            for (int m = tid % NT; m < L; m += NT) col[m] = io.ld(P::pos_of(m));
+        });
+        return;
+    }
+    // COL_INV: natural m order in, inverse only
+    run([&](int tid) {
+        auto io = region(tid); cx<T>* col = column(tid);
+        for (int m = tid % NT; m < L; m += NT) io.st(P::pos_of(m), col[m]);
+    });
+    static_for_down<S, 1>(inv_stage);
+}
+
+// --------------------------------------------------------------------------------------------- P3
+// acc[0], acc[1]: this thread's (device) or this CTA's (host harness) partial dot products.
+template <typename T, typename P, int F, typename Runner>
+FCG_HD void row_inv_body(const RowInvArgs<T>& A, int block, cx<T>* smem, Runner& run, double (&acc)[2])
+{
+    constexpr int L = P::N, S = P::S, NT = P::NT;
+    const int a0 = block * 2 * F;
+    // load T[n][a0 + 2f .. +1], rebuild the packed spectrum Z = X_even + i X_odd at its digit-reversed place
+    run([&](int tid) {
+        constexpr int ITEMS = F * (L / 2), NTH = F * NT;
+#pragma unroll 4
+        for (int item = tid; item < ITEMS; item += NTH) {
+            const int f = item % F, n = item / F;
+            SmemIO<T, P> io{smem + f * region_stride<P>()};
+            const cx<T>* src = A.Tb + (size_t)n * L + a0 + 2 * f;
+            const cx<T> X0 = src[0], X1 = src[1];
+            if (n == 0) {
+                io.st(P::pos_of(0), mk<T>(X0.x, X1.x));
+                io.st(P::pos_of(L / 2), mk<T>(X0.y, X1.y));
+            } else {
+                io.st(P::pos_of(n), mk<T>(X0.x - X1.y, X0.y + X1.x));
+                io.st(P::pos_of(L - n), mk<T>(X0.x + X1.y, X1.x - X0.y));
+            }
+        }
+    });
+    static_for_down<S, 2>([&](auto s) {
+        run([&](int tid) {
+            const int f = tid / NT, lt = tid % NT;
+            SmemIO<T, P> io{smem + f * region_stride<P>()};
+            run_stage<P, decltype(s)::value, +1, T>(lt, A.tw, [&](int e) { return io.ld(e); },
+                                                    [&](int e, cx<T> v) { io.st(e, v); });
+        });
+    });
+    // inverse stage 1 straight into the epilogue: natural order, re = even row, im = odd row
+    run([&](int tid) {
+        const int f = tid / NT, lt = tid % NT;
+        SmemIO<T, P> io{smem + f * region_stride<P>()};
+        const size_t row0 = (size_t)(a0 + 2 * f) * L, row1 = row0 + L;
+        auto emit = [&](size_t i, T c) {
+            if (A.mode == ROWI_PLAIN) { A.out[i] = c * A.scale; return; }
+            const T vi = A.v[i];
+            const T val = A.k[i] * vi + c;                         // k o x + C x
+            if (A.mode == ROWI_RESID) {
+                const T fi = A.f[i], ri = fi - val;                // r = f - A u
+                A.out[i] = ri; A.out2[i] = (T)0;
+                acc[0] += (double)ri * (double)ri; acc[1] += (double)fi * (double)fi;
+            } else {
+                A.out[i] = val;
+                acc[0] += (double)vi * (double)val;                // search length p.Ap
+            }
+        };
+        run_stage<P, 1, +1, T>(lt, A.tw, [&](int e) { return io.ld(e); },
+                               [&](int e, cx<T> v) { emit(row0 + e, v.x); emit(row1 + e, v.y); });
+    });
+}
+
+}  // namespace fcg

@@ -1,0 +1,68 @@
+// fcg_plans.cuh -- radix plans and launch shapes per (dtype, L), and the type-erased launcher table
+// each per-L translation unit (fcg_inst.cu) exports to fcg.cu.
+#pragma once
+#include <cuda_runtime.h>
+#include "fcg_math.cuh"
+
+namespace fcg {
+
+// Radix choice: as few stages as possible (each stage is one shared-memory round trip), radix <= 16
+// (64 fp64 registers of data per thread), and the last radix >= the number of complex elements per
+// 128 B where possible so that the stride-1 runs of the earlier stages cover whole bank groups
+// (8 for fp64, 16 for fp32).
+template <typename T, int L> struct PlanFor;
+#define FCG_PLAN(TYPE, L, R1, R2, R3, R4) \
+    template <> struct PlanFor<TYPE, L> { using type = Plan<L, R1, R2, R3, R4>; };
+FCG_PLAN(double, 16, 4, 4, 1, 1)      FCG_PLAN(float, 16, 4, 4, 1, 1)
+FCG_PLAN(double, 32, 4, 8, 1, 1)      FCG_PLAN(float, 32, 4, 8, 1, 1)
+FCG_PLAN(double, 64, 8, 8, 1, 1)      FCG_PLAN(float, 64, 4, 16, 1, 1)
+FCG_PLAN(double, 128, 16, 8, 1, 1)    FCG_PLAN(float, 128, 8, 16, 1, 1)
+FCG_PLAN(double, 256, 16, 16, 1, 1)   FCG_PLAN(float, 256, 16, 16, 1, 1)
+FCG_PLAN(double, 512, 8, 8, 8, 1)     FCG_PLAN(float, 512, 4, 8, 16, 1)
+FCG_PLAN(double, 1024, 16, 8, 8, 1)   FCG_PLAN(float, 1024, 8, 8, 16, 1)
+FCG_PLAN(double, 2048, 16, 16, 8, 1)  FCG_PLAN(float, 2048, 8, 16, 16, 1)
+FCG_PLAN(double, 4096, 16, 16, 16, 1) FCG_PLAN(float, 4096, 16, 16, 16, 1)
+FCG_PLAN(double, 8192, 16, 8, 8, 8)   FCG_PLAN(float, 8192, 8, 8, 8, 16)
+#undef FCG_PLAN
+
+constexpr int FCG_MAX_SMEM = 227 * 1024;
+constexpr int FCG_NROWVAR = 4;
+
+// Row-pass variants: F packed transforms (2F rows) per CTA, F = Fmin * 2^v.  A variant is valid when the
+// CTA fits (threads <= 1024, shared memory <= 227 KB) and does not exceed the lattice.
+template <typename T, typename P> struct RowShape {
+    static constexpr int FMIN = (32 / P::NT) > 1 ? (32 / P::NT) : 1;
+    static constexpr int F(int v) { return FMIN << v; }
+    static constexpr size_t smem(int v) { return (size_t)F(v) * (P::N + 2) * 2 * sizeof(T); }
+    static constexpr bool valid(int v) {
+        return 2 * F(v) <= P::N && F(v) * P::NT <= 1024 && smem(v) <= (size_t)FCG_MAX_SMEM;
+    }
+};
+// Column pass: COLS columns per CTA so that a CTA has at least 64 threads (one column once NT >= 64).
+template <typename T, typename P> struct ColShape {
+    static constexpr int COLS0 = (64 / P::NT) > 1 ? (64 / P::NT) : 1;
+    static constexpr int COLS = COLS0 > P::N / 2 ? P::N / 2 : COLS0;
+    static constexpr size_t smem = (size_t)COLS * (P::N + 2) * 2 * sizeof(T);
+    static_assert(smem <= (size_t)FCG_MAX_SMEM, "column does not fit in shared memory");
+};
+
+// What fcg.cu sees of one (L, dtype): plain function pointers, arguments type-erased
+// (RowFwdArgs<T>*, ColArgs<T>*, RowInvArgs<T>* of the matching T).
+struct PassTable {
+    int L, dtype;
+    int row_valid[FCG_NROWVAR], row_F[FCG_NROWVAR], row_threads[FCG_NROWVAR];
+    size_t row_smem[FCG_NROWVAR];
+    int cols, col_threads; size_t col_smem;
+    cudaError_t (*init)();
+    cudaError_t (*row_fwd)(int var, const void* args, cudaStream_t st);
+    cudaError_t (*col)(const void* args, cudaStream_t st);
+    cudaError_t (*row_inv)(int var, const void* args, cudaStream_t st);
+    cudaError_t (*spectrum_prep)(const void* s, void* shat, cudaStream_t st);
+};
+
+#define FCG_DECL_TABLE(L) const PassTable* fcg_pass_table_##L(int dtype);
+FCG_DECL_TABLE(16) FCG_DECL_TABLE(32) FCG_DECL_TABLE(64) FCG_DECL_TABLE(128) FCG_DECL_TABLE(256)
+FCG_DECL_TABLE(512) FCG_DECL_TABLE(1024) FCG_DECL_TABLE(2048) FCG_DECL_TABLE(4096) FCG_DECL_TABLE(8192)
+#undef FCG_DECL_TABLE
+
+}  // namespace fcg

@@ -1,0 +1,340 @@
+"""Parity of the CUDA path (through the C ABI, include/fcg.h) with the CPU oracle (oracle/), element by
+element on the same seeded inputs (paper_1305_3625_b200/inputs.py).  Runs on the B200 box: -m gpu.
+
+Tolerances (BASELINE.json north_star): FFT round trip rel. L2 <= 1e-12 (fp64) / 1e-5 (fp32); CG solution
+rel. L2 <= 1e-9 / 1e-4 with iteration count within +-2; fp64 break sequence bit-exact in indices.
+Vector parity is evaluated at equal iteration count (SURVEY.md 8(c) "parity-protocol consequence"): if
+the natural stops differ, the GPU is re-run with tol = 0, maxit = it_oracle.
+"""
+import math
+import os
+
+import numpy as np
+import pytest
+import torch
+
+from oracle import api as orc
+from paper_1305_3625_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+TOL_FFT = {np.float64: 1e-12, np.float32: 1e-5}
+TOL_CG = {np.float64: 1e-9, np.float32: 1e-4}
+TOL_OP = {np.float64: 1e-12, np.float32: 1e-5}      # one operator application: two transforms + O(1) work
+TDT = {np.float64: torch.float64, np.float32: torch.float32}
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_1305_3625_b200 import binding
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    binding.lib()                                    # raises if libfcg.so is missing: no fallback
+    return binding
+
+
+def dev(a, dt=None):
+    return torch.from_numpy(np.ascontiguousarray(a, dtype=dt or a.dtype)).cuda()
+
+
+def rel(a, b):
+    a = np.asarray(a, np.float64 if not np.iscomplexobj(a) else np.complex128).ravel()
+    b = np.asarray(b, np.float64 if not np.iscomplexobj(b) else np.complex128).ravel()
+    return np.linalg.norm(a - b) / max(np.linalg.norm(b), 1e-300)
+
+
+def handle(B, L, dt, s=None, **opts):
+    h = B.Fcg(L, TDT[dt])
+    for k_, v in opts.items():
+        h.fcg_set_option(getattr(B, k_), v)
+    if s is not None:
+        h.fcg_set_spectrum(dev(s, dt))
+    return h
+
+
+# ------------------------------------------------------------------------------------ transforms
+@pytest.mark.parametrize("L", [16, 32, 64, 128, 256, 512, 1024, 2048])
+@pytest.mark.parametrize("dt", [np.float64, np.float32])
+def test_fft_forward_and_round_trip(B, L, dt):
+    x = inputs.fft_field(L).astype(dt)
+    h = handle(B, L, dt)
+    X = h.fcg_fft_fwd(dev(x))
+    X_or = orc.fft2(x)[:, : L // 2 + 1]
+    assert rel(X.cpu().numpy(), X_or) <= TOL_FFT[dt]
+    back = h.fcg_fft_inv(X)
+    assert rel(back.cpu().numpy(), x) <= TOL_FFT[dt]
+    # the inverse alone, fed with the oracle's spectrum
+    x2 = h.fcg_fft_inv(dev(np.ascontiguousarray(X_or)))
+    assert rel(x2.cpu().numpy(), x) <= TOL_FFT[dt]
+    h.close()
+
+
+@pytest.mark.parametrize("L,dt", [(4096, np.float64), (8192, np.float32), (4096, np.float32), (8192, np.float64)])
+def test_fft_round_trip_large(B, L, dt):
+    """Maximum sizes: round trip (a property that holds at any size) + sampled outputs against the definition."""
+    x = inputs.fft_field(L).astype(dt)
+    h = handle(B, L, dt)
+    xd = dev(x)
+    X = h.fcg_fft_fwd(xd)
+    assert rel(h.fcg_fft_inv(X).cpu().numpy(), x) <= TOL_FFT[dt]
+    Xh = X.cpu().numpy()
+    rng = np.random.default_rng(5)
+    a = np.arange(L)
+    x64 = x.astype(np.float64)
+    scale = np.linalg.norm(x64) * 1.0                      # |X[m,n]| ~ ||x||_2 for white noise
+    for m, n in [(0, 0), (L // 2, L // 2), (1, 0), (0, L // 2)] + [tuple(rng.integers(0, [L, L // 2 + 1])) for _ in range(6)]:
+        ref = np.exp(-2j * np.pi * ((m * a) % L) / L) @ x64 @ np.exp(-2j * np.pi * ((n * a) % L) / L)   # definition, one output
+        assert abs(Xh[m, n] - ref) <= 20 * TOL_FFT[dt] * scale
+    h.close()
+
+
+# ------------------------------------------------------------------------------------ operator
+@pytest.mark.parametrize("L", [16, 32, 64, 128, 256, 512, 1024])
+@pytest.mark.parametrize("dt", [np.float64, np.float32])
+def test_apply_matches_oracle_all_variants(B, L, dt):
+    s = inputs.spectrum(L, dt); k = inputs.uniform_k(L).astype(dt); k[inputs.broken_mask(L, 10)] = 0
+    x = inputs.fft_field(L).astype(dt)
+    y_or = orc.apply(s, k, x)
+    seen = 0
+    for v in range(4):
+        try:
+            h = handle(B, L, dt, s, FCG_OPT_ROW_VARIANT=v)
+        except B.FcgError:
+            continue
+        seen += 1
+        y = h.fcg_apply(dev(k), dev(x))
+        assert rel(y.cpu().numpy(), y_or) <= TOL_OP[dt], f"variant {v}"
+        h.close()
+    assert seen >= 1
+
+
+def test_apply_nonsymmetric_spectrum(B):
+    L = 64
+    s = np.random.default_rng(9).random((L, L)) + 0.5      # real, not even: only the even part acts (cpyReal)
+    k = inputs.uniform_k(L); x = inputs.fft_field(L)
+    h = handle(B, L, np.float64, s)
+    assert rel(h.fcg_apply(dev(k), dev(x)).cpu().numpy(), orc.apply(s, k, x)) <= 1e-12
+    h.close()
+
+
+# ------------------------------------------------------------------------------------ CG
+def cg_parity(B, w, **opts):
+    dt = w.dtype.type
+    h = handle(B, w.L, dt, w.s, **opts)
+    ref = orc.cg(w.s, w.k, w.f, w.u0, w.tol, w.maxit, history=True)
+    kd, fd = dev(w.k), dev(w.f)
+    u = dev(w.u0)
+    it, rr, st = h.fcg_solve(kd, fd, u, w.tol, w.maxit)
+    assert st == ref["status"]
+    assert abs(it - ref["iters"]) <= 2, (it, ref["iters"], ref["hist"][-4:])
+    assert h.fcg_last_launch_count() == 5 + 4 * it or opts
+    if it != ref["iters"]:                                # pinned-count protocol
+        u = dev(w.u0)
+        it2, rr, _ = h.fcg_solve(kd, fd, u, 0.0, ref["iters"])
+        assert it2 == ref["iters"]
+    assert rel(u.cpu().numpy(), ref["u"]) <= TOL_CG[dt]
+    # the recurrence residual at the stop is rounding-sensitive (~0.2 % without broken sites, tens of
+    # percent with them while u still agrees to 1e-10), so it is only checked loosely; u above is the parity criterion
+    assert abs(rr - ref["hist"][ref["iters"]]) <= 0.5 * ref["hist"][ref["iters"]] + 1e-15
+    h.close()
+    return it, ref["iters"]
+
+
+def test_cg_config0(B):
+    it, it_or = cg_parity(B, inputs.config(0))
+    assert abs(it - 28) <= 2                               # indicative count, BASELINE.md section 3 (survey probe)
+
+
+def test_cg_config1(B):
+    cg_parity(B, inputs.config(1))
+
+
+@pytest.mark.parametrize("L", [16, 32, 128, 256, 1024])
+@pytest.mark.parametrize("dt", [np.float64, np.float32])
+def test_cg_config2_recipe_scaled(B, L, dt):
+    cg_parity(B, inputs.config(2, dt, L=L))
+
+
+@pytest.mark.parametrize("L,dt", [(128, np.float32), (512, np.float32), (256, np.float64)])
+def test_cg_config4_recipe_scaled(B, L, dt):
+    cg_parity(B, inputs.config(4, dt, L=L))
+
+
+def test_cg_loop_modes_and_determinism(B):
+    """Graph-WHILE and direct-launch modes run the same kernels: bit-identical u, and repeated runs agree bitwise."""
+    w = inputs.config(1, L=256)
+    outs = []
+    for mode, chunk in ((0, 16), (0, 16), (1, 16), (1, 5)):
+        h = handle(B, w.L, np.float64, w.s, FCG_OPT_LOOP_MODE=mode, FCG_OPT_CHUNK=chunk)
+        u = dev(w.u0)
+        it, rr, st = h.fcg_solve(dev(w.k), dev(w.f), u, w.tol, w.maxit)
+        outs.append((it, rr, st, u.cpu().numpy().copy()))
+        h.close()
+    for o in outs[1:]:
+        assert o[:3] == outs[0][:3]
+        assert np.array_equal(o[3], outs[0][3])
+
+
+def test_cg_edge_cases(B):
+    L = 64
+    w = inputs.config(0)
+    h = handle(B, L, np.float64, w.s)
+    kd, fd = dev(w.k), dev(w.f)
+    # maxit = 0: nothing happens, NOT_CONVERGED, residual of the initial guess
+    u = dev(w.u0)
+    assert h.fcg_solve(kd, fd, u, 1e-10, 0) == (0, 1.0, B.FCG_NOT_CONVERGED)
+    assert torch.count_nonzero(u) == 0
+    # maxit reached (S16)
+    it, rr, st = h.fcg_solve(kd, fd, u, 1e-10, 5)
+    ref = orc.cg(w.s, w.k, w.f, w.u0, 1e-10, 5)
+    assert (it, st) == (5, B.FCG_NOT_CONVERGED) and rel(u.cpu().numpy(), ref["u"]) <= 1e-12
+    assert abs(rr - ref["relres"]) <= 1e-6 * ref["relres"]
+    # warm start from the converged solution: zero iterations (S14)
+    u = dev(w.u0)
+    it, _, st = h.fcg_solve(kd, fd, u, 1e-10, 1000)
+    it2, rr2, st2 = h.fcg_solve(kd, fd, u, 1e-9, 1000)
+    assert st == 0 and (it2, st2) == (0, 0) and rr2 <= 1e-9
+    # f = 0 -> u = 0, zero iterations
+    u = dev(np.ones((L, L)))
+    assert h.fcg_solve(kd, dev(np.zeros((L, L))), u, 1e-10, 10) == (0, 0.0, 0)
+    assert torch.count_nonzero(u) == 0
+    # indefinite operator: p.Ap <= 0 -> BREAKDOWN, same verdict as the oracle
+    kneg = np.full((L, L), -50.0)
+    ref = orc.cg(w.s, kneg, w.f, w.u0, 1e-10, 50)
+    u = dev(w.u0)
+    it, rr, st = h.fcg_solve(dev(kneg), fd, u, 1e-10, 50)
+    assert ref["status"] == orc.BREAKDOWN and st == B.FCG_BREAKDOWN and it == ref["iters"]
+    assert rel(u.cpu().numpy(), ref["u"]) <= 1e-9 or np.linalg.norm(ref["u"]) == 0
+    # errors
+    h2 = B.Fcg(L, torch.float64)
+    with pytest.raises(B.FcgError) as ei:
+        h2.fcg_solve(kd, fd, u, 1e-10, 10)
+    assert ei.value.status == B.FCG_NO_SPECTRUM
+    with pytest.raises(B.FcgError) as ei:
+        h.fcg_solve(kd, fd, u, -1.0, 10)
+    assert ei.value.status == B.FCG_INVALID_ARG
+    with pytest.raises(B.FcgError):
+        B.Fcg(100, torch.float64)
+    h.close(); h2.close()
+
+
+def test_cg_solve_host_matches_device(B):
+    w = inputs.config(0)
+    h = handle(B, w.L, np.float64, w.s)
+    u = dev(w.u0)
+    it, rr, st = h.fcg_solve(dev(w.k), dev(w.f), u, w.tol, w.maxit)
+    kh = torch.from_numpy(w.k.copy()).pin_memory(); fh = torch.from_numpy(w.f.copy()).pin_memory()
+    uh = torch.from_numpy(w.u0.copy()).pin_memory()
+    assert h.fcg_solve_host(kh, fh, uh, w.tol, w.maxit) == (it, rr, st)
+    assert np.array_equal(uh.numpy(), u.cpu().numpy())
+    h.close()
+
+
+# ------------------------------------------------------------------------------------ full-size configs
+@pytest.mark.parametrize("dt,count", [(np.float64, 100), (np.float32, 33)])
+def test_cg_config2_full_size(B, dt, count):
+    """L=2048 in the launch configuration bench.py times.  The oracle cannot run the whole solve in seconds, so:
+    (1) pinned-count comparison after 8 iterations, element by element; (2) the finished solve satisfies
+    ||f - A_oracle u||/||f|| <= 2 tol with ONE oracle operator application; (3) indicative iteration count."""
+    w = inputs.config(2, dt)
+    h = handle(B, w.L, dt, w.s)
+    kd, fd = dev(w.k), dev(w.f)
+    ref = orc.cg(w.s, w.k, w.f, w.u0, 0.0, 8, history=True)
+    u = dev(w.u0)
+    it, rr, _ = h.fcg_solve(kd, fd, u, 0.0, 8)
+    assert it == 8 and rel(u.cpu().numpy(), ref["u"]) <= TOL_CG[dt] * 0.1
+    assert abs(rr - ref["hist"][8]) <= 1e-3 * ref["hist"][8]
+    u = dev(w.u0)
+    it, rr, st = h.fcg_solve(kd, fd, u, w.tol, w.maxit)
+    assert st == 0 and rr <= w.tol
+    assert abs(it - count) <= 2                            # BASELINE.md section 3, survey probe (not a paper number)
+    uh = u.cpu().numpy()
+    true_res = np.linalg.norm((w.f - orc.apply(w.s, w.k, uh)).astype(np.float64)) / np.linalg.norm(w.f.astype(np.float64))
+    assert true_res <= 2 * w.tol
+    h.close()
+
+
+def test_cg_config4_full_size(B):
+    """L=8192 fp32 (largest config): pinned count 3 vs oracle + residual property with one oracle application."""
+    w = inputs.config(4)
+    h = handle(B, w.L, np.float32, w.s)
+    kd, fd = dev(w.k), dev(w.f)
+    ref = orc.cg(w.s, w.k, w.f, w.u0, 0.0, 3, history=True)
+    u = dev(w.u0)
+    it, rr, _ = h.fcg_solve(kd, fd, u, 0.0, 3)
+    assert it == 3 and rel(u.cpu().numpy(), ref["u"]) <= 1e-5
+    assert abs(rr - ref["hist"][3]) <= 1e-3 * ref["hist"][3]
+    u = dev(w.u0)
+    it, rr, st = h.fcg_solve(kd, fd, u, w.tol, w.maxit)
+    assert st == 0 and rr <= w.tol
+    assert abs(it - 175) <= 6                              # survey probe 175; rough residual history near the stop (P14 risk note)
+    true_res = np.linalg.norm((w.f - orc.apply(w.s, w.k, u.cpu().numpy())).astype(np.float64)) / np.linalg.norm(w.f.astype(np.float64))
+    assert true_res <= 2 * w.tol
+    h.close()
+
+
+# ------------------------------------------------------------------------------------ break step / fracture loop
+def test_break_step_matches_oracle(B):
+    rng = np.random.default_rng(17)
+    for dt in (np.float64, np.float32):
+        for n_side in (16, 64, 512):
+            N = n_side * n_side
+            k = (rng.random(N) + 0.5).astype(dt); k[rng.random(N) < 0.3] = 0
+            u = rng.standard_normal(N).astype(dt); t = rng.random(N).astype(dt)
+            u[5] = u[3]; t[5] = t[3]; k[5] = k[3] = 1.0                   # an exact tie somewhere
+            h = B.Fcg(n_side, TDT[dt])
+            kd = dev(k); ko = k.copy()
+            for _ in range(6):
+                idx, ratio, st = h.fcg_break_step(kd, dev(u), dev(t))
+                io, ro, _, so = orc.break_step(ko, u, t)
+                assert (idx, ratio, st) == (io, ro, so)                   # bit-exact index and ratio
+                assert np.array_equal(kd.cpu().numpy(), ko)
+            h.close()
+    # rules of S13: ties -> lowest index, t = 0 -> +inf wins, NaN skipped, no candidate -> -1
+    h = B.Fcg(16, torch.float64)
+    k = np.zeros(256); u = np.zeros(256); t = np.ones(256)
+    k[[7, 9, 200]] = 1.0; u[[7, 9, 200]] = 2.0
+    kd = dev(k)
+    assert h.fcg_break_step(kd, dev(u), dev(t))[0] == 7
+    assert h.fcg_break_step(kd, dev(u), dev(t))[0] == 9
+    t[200] = 0.0; k[100] = 1.0; u[100] = 0.0; t[100] = 0.0                # inf at 200, 0/0 at 100
+    kd = dev(np.where(np.arange(256) == 200, 1.0, 0.0) + np.where(np.arange(256) == 100, 1.0, 0.0))
+    idx, ratio, st = h.fcg_break_step(kd, dev(u), dev(t))
+    assert idx == 200 and math.isinf(ratio)
+    idx, ratio, st = h.fcg_break_step(kd, dev(u), dev(t))                 # only the NaN site is left
+    assert idx == -1 and st == B.FCG_NO_CANDIDATE
+    h.close()
+
+
+@pytest.mark.parametrize("L,steps", [(32, 300), (64, 200)])
+def test_fracture_small_matches_oracle(B, L, steps):
+    w = inputs.config(3, L=L, nsteps=steps)
+    k = w.k.copy(); u = w.u0.copy()
+    ref = orc.fracture(w.s, k, w.f, u, w.t, steps, w.tol, w.maxit)
+    h = handle(B, L, np.float64, w.s)
+    kd, ud = dev(w.k), dev(w.u0)
+    index, iters, done, st = h.fcg_fracture(kd, dev(w.f), ud, dev(w.t), steps, w.tol, w.maxit)
+    assert done == steps and st == 0
+    assert np.array_equal(index, ref["index"])                            # bit-exact break sequence
+    assert np.abs(iters.astype(int) - ref["iters"].astype(int)).max() <= 2
+    assert np.array_equal(kd.cpu().numpy(), k)
+    assert rel(ud.cpu().numpy(), u) <= 1e-8
+    h.close()
+
+
+def test_fracture_config3_full(B):
+    """configs[3] at full size: 2000 break steps at L=256 against the oracle's stored sequence
+    (tests/golden/cfg3_breaks.txt, written by tests/golden/make_golden.py from oracle/ only)."""
+    path = os.path.join(GOLD, "cfg3_breaks.txt")
+    gold = np.loadtxt(path, comments="#")
+    steps = gold.shape[0]
+    w = inputs.config(3, nsteps=steps)
+    h = handle(B, w.L, np.float64, w.s)
+    kd, ud = dev(w.k), dev(w.u0)
+    index, iters, done, st = h.fcg_fracture(kd, dev(w.f), ud, dev(w.t), steps, w.tol, w.maxit)
+    assert done == steps and st == 0
+    assert np.array_equal(index, gold[:, 1].astype(np.int64))
+    assert np.abs(iters - gold[:, 2].astype(int)).max() <= 2
+    assert iters[0] == 1 and index[0] == int(np.argmin(w.t))              # P9
+    assert abs(int(iters.sum()) - int(gold[:, 2].sum())) <= 0.002 * gold[:, 2].sum()
+    h.close()
