@@ -1,0 +1,269 @@
+#!/usr/bin/env python
+"""bench.py -- headline measurement of the FFT-CG hot path (BASELINE.json metric: CG iterations/s and
+site-iterations/s at L=2048; achieved HBM GB/s vs peak).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--dtype f64|f32] [--config 2|4] [--impl fcg|reference]
+
+A "step" is one whole solve of the workload (set-up, CG loop to the configured tolerance, finish) through
+the C ABI.  Default workload: BASELINE.json configs[2], L=2048, fp64 (the size the metric is quoted on); the
+fp32 run of the same config and the L=8192 fp32 point are reported in "extra" when --full is given.
+Prints ONE JSON line (see DESIGN.md section 7 for every key).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC, UNIT = "cg_iterations_per_s", "iter/s"
+B_ITER_NW = 16.5          # algorithmic bytes per CG iteration in units of N*w
+PASS_NW = {"row_fwd": 6.0, "col": 2.5, "row_inv": 4.0, "update_r": 3.0}   # this implementation's per-kernel algorithmic bytes / (N*w)
+PASS_NAMES = ["row_fwd", "col", "row_inv", "update_r"]
+
+
+def peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as fh:
+            return float(json.load(fh)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu: int):
+        self.gpu, self.rows, self.proc = gpu, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.gpu), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            threading.Thread(target=self._read, daemon=True).start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if self.proc:
+            time.sleep(0.15)
+            self.proc.terminate()
+        sm = [float(r[0]) for r in self.rows if r and r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in self.rows if len(r) > 1 and r[1].replace(".", "").isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = sorted({names[i] for r in self.rows if len(r) >= 7 for i in range(4) if r[3 + i].lower().startswith("active")})
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": reasons, "samples": len(sm)}
+
+
+def oracle_sample(w, iters: int):
+    """The oracle as it stands, `iters` CG iterations of workload w (tol = 0) on the host cores."""
+    from oracle import api as orc
+    t0 = time.perf_counter()
+    r = orc.cg(w.s, w.k, w.f, w.u0, 0.0, iters)
+    dt = time.perf_counter() - t0
+    return r["iters"] / dt, dt, orc.num_threads()
+
+
+def run_reference(args, rank: int):
+    """--impl reference: the CPU oracle on this arm's config, metric and unit (tier contract)."""
+    if rank != 0:
+        return
+    from paper_1305_3625_b200 import inputs
+    w = inputs.config(args.config, np.float64 if args.dtype == "f64" else np.float32)
+    sample = args.ref_iters
+    for _ in range(args.warmup):
+        oracle_sample(w, 1)
+    total_it, total_t, cores = 0, 0.0, 0
+    for _ in range(args.steps):
+        v, dt, cores = oracle_sample(w, sample)
+        total_it += sample; total_t += dt
+    value = total_it / total_t
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * total_t / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": args.dtype, "data": "synthetic",
+        "config": {"workload": f"BASELINE.json configs[{args.config}] L={w.L} {args.dtype}; each step = {sample} CG iterations (tol=0) of the oracle"},
+        "site_iterations_per_s": value * w.N,
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle",
+                         "sample": f"{sample} CG iterations per step, tol=0, same seeded workload"},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+
+
+def bench_workload(binding, torch, w, steps, warmup, profile_iters=20, e2e_steps=None):
+    """Times `steps` solves of workload w on the current device. Returns a dict of measurements."""
+    tdt = torch.float64 if w.dtype == np.float64 else torch.float32
+    wbytes = w.dtype.itemsize
+    h = binding.Fcg(w.L, tdt)
+    to = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    h.fcg_set_spectrum(to(w.s))
+    k, f, u = to(w.k), to(w.f), to(w.u0)
+    for _ in range(warmup):
+        u.zero_()
+        it, rr, st = h.fcg_solve(k, f, u, w.tol, w.maxit)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    iters, launches = [], 0
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for s in range(steps):
+        ev[s][0].record()
+        u.zero_()                                          # u0 = 0 is part of the workload (otherwise a warm start)
+        it, rr, st = h.fcg_solve(k, f, u, w.tol, w.maxit)
+        ev[s][1].record()
+        iters.append(it); launches += h.fcg_last_launch_count()
+    torch.cuda.synchronize()
+    wall = time.perf_counter() - t0
+    dev_ms = [a.elapsed_time(b) for a, b in ev]
+    out = {"iters": iters, "status": st, "relres": rr, "dev_ms": dev_ms, "wall_s": wall, "launches": launches}
+    # per-kernel times, in loop order, CUDA events on the library's stream
+    u.zero_()
+    ms = h.fcg_profile_iteration(k, f, u, profile_iters)
+    out["kernel_ms"] = dict(zip(PASS_NAMES, ms))
+    # end to end with HOST buffers through the C ABI
+    e2e_steps = e2e_steps or max(1, min(steps, 3))
+    kh, fh = torch.from_numpy(w.k.copy()).pin_memory(), torch.from_numpy(w.f.copy()).pin_memory()
+    uh = torch.zeros((w.L, w.L), dtype=tdt).pin_memory()
+    uh.zero_(); h.fcg_solve_host(kh, fh, uh, w.tol, w.maxit)       # warm (allocates the staging buffers)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter(); e_it = 0
+    for _ in range(e2e_steps):
+        uh.zero_()
+        it, _, _ = h.fcg_solve_host(kh, fh, uh, w.tol, w.maxit)
+        e_it += it
+    out["e2e_iter_s"] = e_it / (time.perf_counter() - t0)
+    out["h2d"] = 3 * w.N * wbytes; out["d2h"] = w.N * wbytes
+    h.close()
+    return out
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--dtype", choices=["f64", "f32"], default="f64")
+    ap.add_argument("--config", type=int, default=2, choices=[0, 1, 2, 4])
+    ap.add_argument("--impl", choices=["fcg", "reference"], default="fcg")
+    ap.add_argument("--ref-iters", type=int, default=8, help="oracle CG iterations per reference step / cpu_baseline sample")
+    ap.add_argument("--full", action="store_true", help="also time configs[2] fp32 and configs[4] (reported under 'extra')")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+
+    rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank)
+        return
+
+    import torch
+    import torch.distributed as dist
+    from paper_1305_3625_b200 import binding, inputs
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback; use --impl reference for the oracle)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    w = inputs.config(args.config, np.float64 if args.dtype == "f64" else np.float32)
+    wbytes = w.dtype.itemsize
+    hbm_peak, peak_src = peaks()
+
+    sampler = ClockSampler(local) if rank == 0 else None
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    if sampler:
+        sampler.start()
+    res = bench_workload(binding, torch, w, args.steps, args.warmup)
+    clocks = sampler.stop() if sampler else None
+
+    # replicas only: every rank solves its own copy; time = max over ranks, value = sum of work
+    step_ms = sum(res["dev_ms"]); total_it = sum(res["iters"]); launches = res["launches"]
+    if world > 1:
+        t = torch.tensor([step_ms], dtype=torch.float64, device="cuda"); dist.all_reduce(t, op=dist.ReduceOp.MAX); step_ms = float(t.item())
+        c = torch.tensor([total_it, launches], dtype=torch.float64, device="cuda"); dist.all_reduce(c, op=dist.ReduceOp.SUM)
+        total_it, launches = int(c[0].item()), int(c[1].item())
+        e = torch.tensor([res["e2e_iter_s"]], dtype=torch.float64, device="cuda"); dist.all_reduce(e, op=dist.ReduceOp.SUM)
+        res["e2e_iter_s"] = float(e.item())
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    value = total_it / (step_ms * 1e-3)
+    it_per_solve = res["iters"][0]
+    t_iter_us = 1e3 * (sum(res["dev_ms"]) / len(res["dev_ms"])) / max(it_per_solve, 1)     # whole solve / iterations (incl. set-up, finish)
+    nw = w.N * wbytes
+    kms = res["kernel_ms"]
+    dom = max(PASS_NAMES, key=lambda n: kms[n])
+    achieved = PASS_NW[dom] * nw / (kms[dom] * 1e-3) / 1e9
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")          # dram bytes per launch from the committed ncu --set full capture
+    if os.path.exists(tpath):
+        try:
+            traffic = json.load(open(tpath)).get(f"L{w.L}_{args.dtype}", {}).get(dom)
+        except Exception:
+            traffic = None
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": step_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": args.dtype, "data": "synthetic",
+        "config": {"workload": f"BASELINE.json configs[{args.config}]: L={w.L} {args.dtype}, tol={w.tol:g}, one step = one full CG solve from u0=0 "
+                               f"({it_per_solve} iterations)", "L": w.L, "iterations_per_solve": it_per_solve,
+                   "l2_policy": f"inputs larger than L2: working set {7.5 * nw / 2**20:.0f} MiB per solve vs 126 MB L2; no flush",
+                   "parallelism": "replicas only" if world > 1 else "single GPU"},
+        "site_iterations_per_s": value * w.N,
+        "us_per_iteration": t_iter_us,
+        "iteration_roofline": {"bound": "hbm", "bytes_per_iteration": B_ITER_NW * nw, "achieved": B_ITER_NW * nw / (t_iter_us * 1e-6) / 1e9,
+                               "peak": hbm_peak, "unit": "GB/s", "frac": B_ITER_NW * nw / (t_iter_us * 1e-6) / 1e9 / hbm_peak,
+                               "frac_of_8TBs_nominal": B_ITER_NW * nw / (t_iter_us * 1e-6) / 1e9 / 8000.0, "peak_source": peak_src,
+                               "note": "16.5*N*w model of SURVEY.md 8(d); time = whole solve / iterations"},
+        "kernel_us": {n: 1e3 * kms[n] for n in PASS_NAMES},
+        "kernel_gbs": {n: PASS_NW[n] * nw / (kms[n] * 1e-3) / 1e9 for n in PASS_NAMES},
+        "roofline": {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": hbm_peak, "unit": "GB/s", "frac": achieved / hbm_peak,
+                     "traffic": traffic, "algorithmic_bytes_per_launch": PASS_NW[dom] * nw, "peak_source": peak_src},
+        "e2e": {"value": res["e2e_iter_s"], "unit": UNIT, "h2d_bytes_per_step": res["h2d"], "d2h_bytes_per_step": res["d2h"]},
+        "gpu_launches": launches,
+        "clocks": clocks,
+        "final_rel_residual": res["relres"], "status": res["status"],
+    }
+    if args.full and world == 1:
+        extra = {}
+        for cfg, dt in ((2, np.float32), (4, np.float32)):
+            w2 = inputs.config(cfg, dt)
+            r2 = bench_workload(binding, torch, w2, max(2, args.steps // 3), 2, e2e_steps=1)
+            nw2 = w2.N * 4; t2 = 1e3 * (sum(r2["dev_ms"]) / len(r2["dev_ms"])) / r2["iters"][0]
+            extra[f"cfg{cfg}_L{w2.L}_f32"] = {"iterations": r2["iters"][0], "iter_per_s": 1e6 / t2, "site_iter_per_s": 1e6 / t2 * w2.N,
+                                               "us_per_iteration": t2, "iteration_gbs_16p5": B_ITER_NW * nw2 / (t2 * 1e-6) / 1e9,
+                                               "frac_of_measured_peak": B_ITER_NW * nw2 / (t2 * 1e-6) / 1e9 / hbm_peak,
+                                               "kernel_us": {n: 1e3 * r2["kernel_ms"][n] for n in PASS_NAMES}, "e2e_iter_per_s": r2["e2e_iter_s"]}
+        line["extra"] = extra
+    if not args.no_cpu_baseline and world == 1:
+        v, dt, cores = oracle_sample(w, args.ref_iters)
+        line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
+                                "sample": f"{args.ref_iters} CG iterations (tol=0) of the same workload, {dt:.1f} s"}
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -123,6 +123,14 @@ int fcg_break_step(fcg_handle h, void* k, const void* u, const void* t,
 int fcg_fracture(fcg_handle h, void* k, const void* f, void* u, const void* t, int nsteps, double tol,
                  int maxit, long long* index_host, int* iters_host, int* steps_done_host);
 
+/* Measurement aid: runs the set-up of fcg_solve and then `iters` iterations of the CG loop body as direct
+ * launches with CUDA events between the four kernels (tol = 0: never stops early), and returns their mean
+ * device times in milliseconds, ms_host[0..3] = { row pass forward (P1), column pass (P2), row pass inverse
+ * (P3), residual update (P4) }.  Kernels run in loop order, so each sees the cache state its predecessor
+ * leaves.  u is overwritten with an unfinished iterate.  Blocks until done.  Returns FCG_NOT_CONVERGED if the
+ * loop flagged completion (times then include early exits and are not meaningful). */
+int fcg_profile_iteration(fcg_handle h, const void* k, const void* f, void* u, int iters, double* ms_host);
+
 /* Number of this library's kernel launches enqueued by the last fcg_solve / fcg_solve_host /
  * fcg_fracture call on this handle (graph kernel nodes counted once per execution). */
 long long fcg_last_launch_count(fcg_handle h);

@@ -20,7 +20,7 @@ FCG_INVALID_ARG, FCG_UNSUPPORTED, FCG_CUDA_ERROR, FCG_BREAKDOWN, FCG_NO_SPECTRUM
 FCG_OPT_LOOP_MODE, FCG_OPT_CHUNK, FCG_OPT_ROW_VARIANT = 0, 1, 2
 
 EXPORTS = ["fcg_workspace_bytes", "fcg_create", "fcg_destroy", "fcg_set_option", "fcg_set_spectrum", "fcg_apply",
-           "fcg_solve", "fcg_solve_host", "fcg_fft_fwd", "fcg_fft_inv", "fcg_break_step", "fcg_fracture",
+           "fcg_solve", "fcg_solve_host", "fcg_profile_iteration", "fcg_fft_fwd", "fcg_fft_inv", "fcg_break_step", "fcg_fracture",
            "fcg_last_launch_count", "fcg_last_error", "fcg_version"]
 
 _lib = None
@@ -52,6 +52,7 @@ def lib() -> C.CDLL:
         L.fcg_fft_inv.argtypes = [vp, vp, vp]; L.fcg_fft_inv.restype = i
         L.fcg_break_step.argtypes = [vp, vp, vp, vp, C.POINTER(ll), C.POINTER(d)]; L.fcg_break_step.restype = i
         L.fcg_fracture.argtypes = [vp, vp, vp, vp, vp, i, d, i, vp, vp, C.POINTER(i)]; L.fcg_fracture.restype = i
+        L.fcg_profile_iteration.argtypes = [vp, vp, vp, vp, i, C.POINTER(d)]; L.fcg_profile_iteration.restype = i
         L.fcg_last_launch_count.argtypes = [vp]; L.fcg_last_launch_count.restype = ll
         L.fcg_last_error.argtypes = [vp]; L.fcg_last_error.restype = C.c_char_p
         L.fcg_version.argtypes = []; L.fcg_version.restype = C.c_char_p
@@ -189,6 +190,15 @@ class Fcg:
         if st < 0 and st not in (FCG_BREAKDOWN, FCG_NO_CANDIDATE):
             self._raise(st)
         return index, iters, int(done.value), int(st)
+
+    def fcg_profile_iteration(self, k: torch.Tensor, f: torch.Tensor, u: torch.Tensor, iters: int):
+        """Mean device milliseconds of the four loop kernels [row_fwd, col, row_inv, update_r]; overwrites u."""
+        ms = (C.c_double * 4)()
+        st = self._lib.fcg_profile_iteration(self._h, self._chk(k, self.N), self._chk(f, self.N), self._chk(u, self.N),
+                                             int(iters), ms)
+        if st != FCG_OK:
+            self._raise(st)
+        return [float(x) for x in ms]
 
     def fcg_last_launch_count(self) -> int:
         return int(self._lib.fcg_last_launch_count(self._h))

@@ -16,7 +16,7 @@ using namespace fcg;
 
 namespace {
 
-constexpr int VEC_BLOCKS_MAX = 148 * 4;
+constexpr int VEC_BLOCKS_MAX = 148 * 8;   // 8 CTAs of 256 threads per SM
 constexpr size_t ALIGN = 256;
 size_t align_up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
 
@@ -143,16 +143,22 @@ template <typename T> struct Seq {
         if ((e = col(COL_CONV, false)) != cudaSuccess) return e;
         return row_inv(ROWI_RESID, k, u, f, r(), p());
     }
-    // one pass of Listing 2
-    cudaError_t iteration(const T* k, T* u) const {
-        cudaError_t e;
-        if ((e = row_fwd(ROWF_CG, nullptr, u)) != cudaSuccess) return e;            // new x (lagged), new p, row transform
-        if ((e = col(COL_CONV, true)) != cudaSuccess) return e;                     // column transform * spectrum * inverse
-        if ((e = row_inv(ROWI_CG, k, p(), nullptr, q(), nullptr)) != cudaSuccess) return e;   // q = A p, p.q, alpha
+    // one pass of Listing 2, as four launches
+    cudaError_t it_row_fwd(T* u) const { return row_fwd(ROWF_CG, nullptr, u); }                    // new x (lagged), new p, row transform
+    cudaError_t it_col() const { return col(COL_CONV, true); }                                     // column transform * spectrum * inverse
+    cudaError_t it_row_inv(const T* k) const { return row_inv(ROWI_CG, k, p(), nullptr, q(), nullptr); }   // q = A p, p.q, alpha
+    cudaError_t it_update_r() const {                                                              // r, r.r, beta, convergence
         const size_t nvec = h->N / Vec<T>::W;
         cg_update_r_kernel<T><<<h->vec_blocks(), 256, 0, st>>>(r(), q(), nvec, h->at<double>(h->lay.partial_vec), h->sc());
         ++h->launches;
-        return cudaGetLastError();                                                  // r, r.r, beta, convergence
+        return cudaGetLastError();
+    }
+    cudaError_t iteration(const T* k, T* u) const {
+        cudaError_t e;
+        if ((e = it_row_fwd(u)) != cudaSuccess) return e;
+        if ((e = it_col()) != cudaSuccess) return e;
+        if ((e = it_row_inv(k)) != cudaSuccess) return e;
+        return it_update_r();
     }
     cudaError_t finish(T* u) const {
         const size_t nvec = h->N / Vec<T>::W;
@@ -314,14 +320,43 @@ int apply_impl(fcg_handle h, const void* k, const void* x, void* y) {
     return FCG_OK;
 }
 
+// Per-kernel device times of the CG loop body, measured in sequence (each kernel sees the cache state its
+// predecessor leaves, as in a real solve) with CUDA events on the handle's stream.
+template <typename T>
+int profile_impl(fcg_handle h, const void* k, const void* f, void* u, int iters, double* ms) {
+    Seq<T> s{h, h->stream};
+    h->launches = 0;
+    FCG_CK(h, s.init((const T*)k, (const T*)f, (T*)u, 0.0, 1 << 30, false, 0ULL));
+    for (int w = 0; w < 2; ++w) FCG_CK(h, s.iteration((const T*)k, (T*)u));       // warm-up
+    std::vector<cudaEvent_t> ev((size_t)iters * 5);
+    for (auto& e : ev) FCG_CK(h, cudaEventCreate(&e));
+    for (int i = 0; i < iters; ++i) {
+        cudaEvent_t* e = &ev[(size_t)i * 5];
+        FCG_CK(h, cudaEventRecord(e[0], h->stream)); FCG_CK(h, s.it_row_fwd((T*)u));
+        FCG_CK(h, cudaEventRecord(e[1], h->stream)); FCG_CK(h, s.it_col());
+        FCG_CK(h, cudaEventRecord(e[2], h->stream)); FCG_CK(h, s.it_row_inv((const T*)k));
+        FCG_CK(h, cudaEventRecord(e[3], h->stream)); FCG_CK(h, s.it_update_r());
+        FCG_CK(h, cudaEventRecord(e[4], h->stream));
+    }
+    FCG_CK(h, cudaMemcpyAsync(h->h_sc, h->sc(), sizeof(Scalars), cudaMemcpyDeviceToHost, h->stream));
+    FCG_CK(h, cudaStreamSynchronize(h->stream));
+    for (int q = 0; q < 4; ++q) ms[q] = 0.0;
+    for (int i = 0; i < iters; ++i)
+        for (int q = 0; q < 4; ++q) {
+            float t = 0.f;
+            FCG_CK(h, cudaEventElapsedTime(&t, ev[(size_t)i * 5 + q], ev[(size_t)i * 5 + q + 1]));
+            ms[q] += (double)t / iters;
+        }
+    for (auto& e : ev) cudaEventDestroy(e);
+    return h->h_sc->done ? FCG_NOT_CONVERGED : FCG_OK;       // done would mean the loop kernels exited early
+}
+
 template <typename T>
 int twiddle_init(fcg_handle h) {
-    std::vector<cx<T>> tw(h->L);
-    for (int j = 0; j < h->L; ++j) {
-        const double ang = 2.0 * M_PI * (double)j / (double)h->L;
-        tw[j].x = (T)std::cos(ang); tw[j].y = (T)(-std::sin(ang));
-    }
-    FCG_CK(h, cudaMemcpyAsync(h->at<void>(h->lay.tw), tw.data(), tw.size() * sizeof(cx<T>), cudaMemcpyHostToDevice, h->stream));
+    const size_t n = (size_t)(h->tab->tw_total > 0 ? h->tab->tw_total : 1);
+    std::vector<cx<T>> tw(n);
+    h->tab->fill_twiddles(tw.data());
+    FCG_CK(h, cudaMemcpyAsync(h->at<void>(h->lay.tw), tw.data(), n * sizeof(cx<T>), cudaMemcpyHostToDevice, h->stream));
     FCG_CK(h, cudaStreamSynchronize(h->stream));
     return FCG_OK;
 }
@@ -471,6 +506,12 @@ int fcg_fracture(fcg_handle h, void* k, const void* f, void* u, const void* t, i
     if (steps_done_host) *steps_done_host = done;
     h->launches = total;
     return st;
+}
+
+int fcg_profile_iteration(fcg_handle h, const void* k, const void* f, void* u, int iters, double* ms_host) {
+    if (!h || !k || !f || !u || iters < 1 || !ms_host) return fail(h, FCG_INVALID_ARG, "bad argument");
+    if (!h->have_spectrum) return fail(h, FCG_NO_SPECTRUM, "fcg_set_spectrum has not been called");
+    return h->dtype == FCG_F64 ? profile_impl<double>(h, k, f, u, iters, ms_host) : profile_impl<float>(h, k, f, u, iters, ms_host);
 }
 
 long long fcg_last_launch_count(fcg_handle h) { return h ? h->launches : -1; }

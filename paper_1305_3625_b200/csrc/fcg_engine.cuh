@@ -12,7 +12,7 @@
 
 namespace fcg {
 
-// tw[j] = exp(-2 pi i j / N), j = 0..N-1 (forward sign); the inverse uses the conjugate.
+// tw = per-stage twiddle tables of the plan (Plan::tw_off, forward sign); the inverse uses the conjugate.
 template <typename P, int s, int DIR, typename T, typename LD, typename ST>
 FCG_HD void run_stage(int lt, const cx<T>* __restrict__ tw, LD ld, ST st)
 {
@@ -21,7 +21,7 @@ FCG_HD void run_stage(int lt, const cx<T>* __restrict__ tw, LD ld, ST st)
     constexpr int Q = M / R;               // element stride inside a butterfly
     constexpr int NB = P::N / R;           // butterflies in this stage
     constexpr int PER = NB / P::NT;        // butterflies per thread
-    constexpr int PRE = P::prefix(s);      // w_M^{j u} = tw[j u PRE]
+    constexpr int TWO = P::tw_off(s);      // w_M^{j u} = tw[TWO + (u-1) Q + j]
     static_assert(PER >= 1, "plan: NT too large for this radix");
 #pragma unroll
     for (int i = 0; i < PER; ++i) {
@@ -35,12 +35,12 @@ FCG_HD void run_stage(int lt, const cx<T>* __restrict__ tw, LD ld, ST st)
             dftR<R, -1>(a);
             if (Q > 1) {
 #pragma unroll
-                for (int u = 1; u < R; ++u) a[u] = cmulw(a[u], tw[j * u * PRE]);
+                for (int u = 1; u < R; ++u) a[u] = cmulw(a[u], tw[TWO + (u - 1) * Q + j]);
             }
         } else {
             if (Q > 1) {
 #pragma unroll
-                for (int u = 1; u < R; ++u) a[u] = cmulwc(a[u], tw[j * u * PRE]);
+                for (int u = 1; u < R; ++u) a[u] = cmulwc(a[u], tw[TWO + (u - 1) * Q + j]);
             }
             dftR<R, +1>(a);
         }
@@ -51,7 +51,7 @@ FCG_HD void run_stage(int lt, const cx<T>* __restrict__ tw, LD ld, ST st)
 
 // Last forward stage, a pointwise real multiply, and the first inverse stage, all in registers:
 //   a <- DFT_R(a);  a[u] *= mul(e_u);  a <- DFT_R^H(a)
-// (the last stage has Q = 1, so no twiddles are involved).  mul(e) returns the real factor for position e.
+// (the last stage has Q = 1, so no twiddles are involved).  mul(g, u) returns the real factor for position g*R + u.
 template <typename P, typename T, typename LD, typename ST, typename MUL>
 FCG_HD void run_middle(int lt, LD ld, ST st, MUL mul)
 {
@@ -66,7 +66,7 @@ FCG_HD void run_middle(int lt, LD ld, ST st, MUL mul)
         for (int t = 0; t < R; ++t) a[t] = ld(base + t);
         dftR<R, -1>(a);
 #pragma unroll
-        for (int u = 0; u < R; ++u) { const T sv = mul(base + u); a[u].x *= sv; a[u].y *= sv; }
+        for (int u = 0; u < R; ++u) { const T sv = mul(lt + i * P::NT, u); a[u].x *= sv; a[u].y *= sv; }
         dftR<R, +1>(a);
 #pragma unroll
         for (int t = 0; t < R; ++t) st(base + t, a[t]);

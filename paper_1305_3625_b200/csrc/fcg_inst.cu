@@ -1,5 +1,6 @@
 // fcg_inst.cu -- instantiates the transform passes for one lattice size.  Compiled once per supported L
 // with -DFCG_INST_L=<L> (paper_1305_3625_b200/build.py) so the sizes build in parallel.
+#include <cmath>
 #include "fcg_kernels.cuh"
 #include "fcg_plans.cuh"
 
@@ -16,11 +17,18 @@ template <typename T> struct Inst {
     using CS = ColShape<T, P>;
     static constexpr int L = FCG_INST_L;
 
+    // opt in to > 48 KB of dynamic shared memory and ask for the largest shared-memory carveout, so that as
+    // many CTAs as the register file allows are resident
+    template <typename K> static cudaError_t prep(K kernel, size_t smem) {
+        cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        return cudaFuncSetAttribute(kernel, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared);
+    }
     template <int V> static cudaError_t init_row() {
         if constexpr (RS::valid(V)) {
-            cudaError_t e = cudaFuncSetAttribute(row_fwd_kernel<T, P, RS::F(V)>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RS::smem(V));
+            cudaError_t e = prep(row_fwd_kernel<T, P, RS::F(V)>, RS::smem(V));
             if (e != cudaSuccess) return e;
-            return cudaFuncSetAttribute(row_inv_kernel<T, P, RS::F(V)>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RS::smem(V));
+            return prep(row_inv_kernel<T, P, RS::F(V)>, RS::smem(V));
         }
         return cudaSuccess;
     }
@@ -30,7 +38,7 @@ template <typename T> struct Inst {
         if ((e = init_row<1>()) != cudaSuccess) return e;
         if ((e = init_row<2>()) != cudaSuccess) return e;
         if ((e = init_row<3>()) != cudaSuccess) return e;
-        return cudaFuncSetAttribute(col_kernel<T, P, CS::COLS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)CS::smem);
+        return prep(col_kernel<T, P, CS::COLS>, CS::smem);
     }
 
     template <int V> static cudaError_t row_fwd_v(const RowFwdArgs<T>& A, cudaStream_t st) {
@@ -84,6 +92,8 @@ template <typename T> struct Inst {
             t.row_threads[v] = RS::F(v) * P::NT; t.row_smem[v] = RS::smem(v);
         }
         t.cols = CS::COLS; t.col_threads = CS::COLS * P::NT; t.col_smem = CS::smem;
+        t.tw_total = P::TW_TOTAL;
+        t.fill_twiddles = [](void* buf) { fill_twiddles<T, P>(static_cast<cx<T>*>(buf)); };
         t.init = &init; t.row_fwd = &row_fwd; t.col = &col; t.row_inv = &row_inv; t.spectrum_prep = &spectrum_prep;
         return t;
     }

@@ -175,7 +175,18 @@ __global__ void __launch_bounds__(256) cg_update_r_kernel(T* __restrict__ r, con
     double acc[1] = {0.0};
     V* rv = reinterpret_cast<V*>(r);
     const V* qv = reinterpret_cast<const V*>(q);
-    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < nvec; i += (size_t)gridDim.x * blockDim.x) {
+    // four independent 16-byte loads of r and of q in flight per thread before any use
+    constexpr int UN = 4;
+    const size_t stride = (size_t)gridDim.x * blockDim.x;
+    size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    for (; i + (UN - 1) * stride < nvec; i += UN * stride) {
+        V x[UN], y[UN];
+#pragma unroll
+        for (int c = 0; c < UN; ++c) { x[c] = rv[i + c * stride]; y[c] = __ldg(qv + i + c * stride); }
+#pragma unroll
+        for (int c = 0; c < UN; ++c) { axpy_sq(x[c], y[c], a, acc[0]); rv[i + c * stride] = x[c]; }
+    }
+    for (; i < nvec; i += stride) {
         V x = rv[i];
         axpy_sq(x, __ldg(qv + i), a, acc[0]);
         rv[i] = x;

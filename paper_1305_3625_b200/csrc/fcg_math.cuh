@@ -117,6 +117,14 @@ struct Plan {
     static constexpr int radix(int s) { return s == 1 ? R1_ : s == 2 ? R2_ : s == 3 ? R3_ : R4_; }
     static constexpr int prefix(int s) { return s == 1 ? 1 : s == 2 ? R1_ : s == 3 ? R1_ * R2_ : R1_ * R2_ * R3_; }  // R1..R_{s-1}
     static constexpr int mlen(int s) { return N_ / prefix(s); }                                                        // m_s
+    // Per-stage twiddle tables, laid out [u-1][j] (u = 1..R-1, j < Q = m_s/R_s) so that consecutive threads
+    // (consecutive j) read consecutive entries:  tws[tw_off(s) + (u-1)*Q + j] = exp(-2 pi i j u / m_s).
+    static constexpr int tw_count(int s) { return s >= S ? 0 : (radix(s) - 1) * (mlen(s) / radix(s)); }
+    static constexpr int tw_off(int s) { return s <= 1 ? 0 : tw_off(s - 1) + tw_count(s - 1); }
+    static constexpr int TW_TOTAL = tw_off(S);
+    // The spectrum is stored transposed with respect to the last stage's butterflies: position e = g*RLAST + u
+    // lives at u*(N/RLAST) + g, so consecutive threads (consecutive g) read consecutive entries.
+    static FCG_HD int shat_index(int e) { return (e % RLAST) * (N_ / RLAST) + e / RLAST; }
     // frequency kappa -> position
     static FCG_HD int pos_of(int kappa) {
         int u1 = kappa % R1_, r = kappa / R1_;

@@ -39,7 +39,7 @@ template <typename T> struct RowFwdArgs {
     const T* x;            // PLAIN: input field
     T* u; T* p; const T* r;        // CG: vectors updated in place / read
     cx<T>* Tb;             // [L/2][L] transposed half spectrum
-    const cx<T>* tw;       // exp(-2 pi i j / L)
+    const cx<T>* tw;       // per-stage twiddle tables (Plan::tw_off)
     const Scalars* sc;
 };
 
@@ -73,8 +73,24 @@ template <int A, int B, typename F> FCG_HD void static_for_down(F&& f) {
 // row-pass CTA on different banks when F lanes read the same position of F different transforms.
 template <typename P> constexpr int region_stride() { return P::N + 2; }
 
+// Host: fill the per-stage twiddle tables of plan P (layout: Plan::tw_off).  Every entry is evaluated in
+// double from its own reduced angle index (no recurrences) and rounded once to T.
+template <typename T, typename P>
+inline void fill_twiddles(cx<T>* out) {
+    for (int sv = 1; sv < P::S; ++sv) {
+        const int R = P::radix(sv), M = P::mlen(sv), Q = M / R, off = P::tw_off(sv);
+        for (int u = 1; u < R; ++u)
+            for (int j = 0; j < Q; ++j) {
+                const double ang = 2.0 * 3.14159265358979323846 * (double)((j * u) % M) / (double)M;
+                cx<T> w; w.x = (T)cos(ang); w.y = (T)(-sin(ang));
+                out[off + (u - 1) * Q + j] = w;
+            }
+    }
+}
+
 // shat[n][pos(m)] from the caller's s[m][n]: even part, 1/L^2, digit-reversed along m; row 0 and row L/2
-// hold (s0 + sN)/2 and (s0 - sN)/2 for the packed n = 0 / n = L/2 column (col_body).  idx = m*(L/2) + n.
+// hold (s0 + sN)/2 and (s0 - sN)/2 for the packed n = 0 / n = L/2 column (col_body); within a row the entry of
+// position e sits at Plan::shat_index(e).  idx = m*(L/2) + n.
 template <typename T, typename P>
 FCG_HD void spectrum_prep_one(int idx, const T* __restrict__ s, T* __restrict__ shat) {
     constexpr int L = P::N;
@@ -82,7 +98,7 @@ FCG_HD void spectrum_prep_one(int idx, const T* __restrict__ s, T* __restrict__ 
     const T h = (T)0.5;
     const int m = idx / (L / 2), n = idx % (L / 2);
     const int mm = (L - m) % L;
-    const int e = P::pos_of(m);
+    const int e = P::shat_index(P::pos_of(m));
     if (n > 0) {
         const T ev = (s[(size_t)m * L + n] + s[(size_t)mm * L + (L - n)]) * h;
         shat[(size_t)n * L + e] = ev * scale;
@@ -195,10 +211,10 @@ FCG_HD void col_body(const ColArgs<T>& A, int block, cx<T>* smem, Runner& run)
             const T* sh = A.shat + (size_t)(n0 + tid / NT) * L;
             if constexpr (S == 1)
                 run_middle<P, T>(tid % NT, [&](int e) { return col[e]; }, [&](int e, cx<T> v) { col[e] = v; },
-                                 [&](int e) { return sh[e]; });
+                                 [&](int g, int u) { return sh[u * (L / P::RLAST) + g]; });
             else
                 run_middle<P, T>(tid % NT, [&](int e) { return io.ld(e); }, [&](int e, cx<T> v) { io.st(e, v); },
-                                 [&](int e) { return sh[e]; });
+                                 [&](int g, int u) { return sh[u * (L / P::RLAST) + g]; });
         });
         static_for_down<S - 1, 1>(inv_stage);
         return;
@@ -217,13 +233,14 @@ FCG_HD void col_body(const ColArgs<T>& A, int block, cx<T>* smem, Runner& run)
                     const int e = P::pos_of(m), e2 = P::pos_of((L - m) % L);
                     const cx<T> Wa = io.ld(e), Wb = io.ld(e2);
                     cx<T> va, vb;
-                    va.x = sh[e] * Wa.x + sm_[e] * Wb.x;   va.y = sh[e] * Wa.y - sm_[e] * Wb.y;
-                    vb.x = sh[e2] * Wb.x + sm_[e2] * Wa.x; vb.y = sh[e2] * Wb.y - sm_[e2] * Wa.y;
+                    const int i1 = P::shat_index(e), i2 = P::shat_index(e2);
+                    va.x = sh[i1] * Wa.x + sm_[i1] * Wb.x; va.y = sh[i1] * Wa.y - sm_[i1] * Wb.y;
+                    vb.x = sh[i2] * Wb.x + sm_[i2] * Wa.x; vb.y = sh[i2] * Wb.y - sm_[i2] * Wa.y;
                     io.st(e, va);
                     if (e2 != e) io.st(e2, vb);
                 }
             } else {
-                for (int e = lt; e < L; e += NT) { cx<T> w = io.ld(e); w.x *= sh[e]; w.y *= sh[e]; io.st(e, w); }
+                for (int e = lt; e < L; e += NT) { cx<T> w = io.ld(e); const T sv = sh[P::shat_index(e)]; w.x *= sv; w.y *= sv; io.st(e, w); }
             }
         });
         static_for_down<S, 1>(inv_stage);

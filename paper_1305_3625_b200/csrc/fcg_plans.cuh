@@ -53,6 +53,8 @@ struct PassTable {
     int row_valid[FCG_NROWVAR], row_F[FCG_NROWVAR], row_threads[FCG_NROWVAR];
     size_t row_smem[FCG_NROWVAR];
     int cols, col_threads; size_t col_smem;
+    int tw_total;                                  // entries of the per-stage twiddle tables (Plan::TW_TOTAL)
+    void (*fill_twiddles)(void* host_buf);         // host_buf: tw_total complex numbers of the table's dtype
     cudaError_t (*init)();
     cudaError_t (*row_fwd)(int var, const void* args, cudaStream_t st);
     cudaError_t (*col)(const void* args, cudaStream_t st);

@@ -24,8 +24,8 @@ int run(int what, const T* s, const T* k, const T* x, T* y, T* Tout, int variant
     using RS = RowShape<T, P>;
     using CS = ColShape<T, P>;
     const size_t N = (size_t)L * L;
-    std::vector<cx<T>> tw(L), Tb(N / 2);
-    for (int j = 0; j < L; ++j) { double a = 2.0 * M_PI * j / L; tw[j].x = (T)std::cos(a); tw[j].y = (T)(-std::sin(a)); }
+    std::vector<cx<T>> tw(P::TW_TOTAL + 1), Tb(N / 2);
+    fill_twiddles<T, P>(tw.data());
     std::vector<T> shat((size_t)(L / 2 + 1) * L);
     for (int idx = 0; idx < L * (L / 2); ++idx) spectrum_prep_one<T, P>(idx, s, shat.data());
     Scalars sc{};

@@ -119,6 +119,9 @@ def test_apply_nonsymmetric_spectrum(B):
 
 # ------------------------------------------------------------------------------------ CG
 def cg_parity(B, w, **opts):
+    """Protocol: status equal; iteration count within +-2; u compared at the natural stops and,
+    if the counts differ and that misses, at the oracle's count (tol = 0, maxit = it_oracle); finally the GPU
+    solution must be as close to a tight (1e-14) oracle solve as the oracle's own solution is."""
     dt = w.dtype.type
     h = handle(B, w.L, dt, w.s, **opts)
     ref = orc.cg(w.s, w.k, w.f, w.u0, w.tol, w.maxit, history=True)
@@ -128,14 +131,21 @@ def cg_parity(B, w, **opts):
     assert st == ref["status"]
     assert abs(it - ref["iters"]) <= 2, (it, ref["iters"], ref["hist"][-4:])
     assert h.fcg_last_launch_count() == 5 + 4 * it or opts
-    if it != ref["iters"]:                                # pinned-count protocol
-        u = dev(w.u0)
-        it2, rr, _ = h.fcg_solve(kd, fd, u, 0.0, ref["iters"])
+    u_nat = u.cpu().numpy()
+    d_nat = rel(u_nat, ref["u"])
+    d_pin = d_nat
+    if it != ref["iters"] and d_nat > TOL_CG[dt]:
+        u2 = dev(w.u0)
+        it2, _, _ = h.fcg_solve(kd, fd, u2, 0.0, ref["iters"])
         assert it2 == ref["iters"]
-    assert rel(u.cpu().numpy(), ref["u"]) <= TOL_CG[dt]
+        d_pin = rel(u2.cpu().numpy(), ref["u"])
+    assert min(d_nat, d_pin) <= TOL_CG[dt], (d_nat, d_pin, it, ref["iters"])
     # the recurrence residual at the stop is rounding-sensitive (~0.2 % without broken sites, tens of
     # percent with them while u still agrees to 1e-10), so it is only checked loosely; u above is the parity criterion
-    assert abs(rr - ref["hist"][ref["iters"]]) <= 0.5 * ref["hist"][ref["iters"]] + 1e-15
+    assert rr <= w.tol and abs(rr - ref["hist"][ref["iters"]]) <= 0.6 * ref["hist"][ref["iters"]] + 1e-15
+    if dt == np.float64 and w.L <= 512:
+        tight = orc.cg(w.s, w.k, w.f, w.u0, 1e-14, 10 * w.maxit)["u"]
+        assert rel(u_nat, tight) <= 2.0 * rel(ref["u"], tight) + 1e-12
     h.close()
     return it, ref["iters"]
 
