@@ -108,11 +108,12 @@ def run_reference(args, rank: int):
     print(json.dumps(line))
 
 
-def bench_workload(binding, torch, w, steps, warmup, profile_iters=20, e2e_steps=None):
+def bench_workload(binding, torch, w, steps, warmup, profile_iters=20, e2e_steps=None, loop_mode=0):
     """Times `steps` solves of workload w on the current device. Returns a dict of measurements."""
     tdt = torch.float64 if w.dtype == np.float64 else torch.float32
     wbytes = w.dtype.itemsize
     h = binding.Fcg(w.L, tdt)
+    h.fcg_set_option(binding.FCG_OPT_LOOP_MODE, loop_mode)
     to = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
     h.fcg_set_spectrum(to(w.s))
     k, f, u = to(w.k), to(w.f), to(w.u0)
@@ -165,6 +166,8 @@ def main():
     ap.add_argument("--ref-iters", type=int, default=8, help="oracle CG iterations per reference step / cpu_baseline sample")
     ap.add_argument("--full", action="store_true", help="also time configs[2] fp32 and configs[4] (reported under 'extra')")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--loop-mode", type=int, default=0, choices=[0, 1],
+                    help="0: whole solve as one CUDA graph with a device-side WHILE node (default); 1: direct launches (for ncu)")
     args = ap.parse_args()
 
     rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -192,7 +195,7 @@ def main():
     torch.cuda.synchronize()
     if sampler:
         sampler.start()
-    res = bench_workload(binding, torch, w, args.steps, args.warmup)
+    res = bench_workload(binding, torch, w, args.steps, args.warmup, loop_mode=args.loop_mode)
     clocks = sampler.stop() if sampler else None
 
     # replicas only: every rank solves its own copy; time = max over ranks, value = sum of work
