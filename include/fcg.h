@@ -57,7 +57,9 @@ typedef enum {
                                  1: kernels enqueued directly, in chunks of FCG_OPT_CHUNK iterations that
                                     exit early on the device flag, host polls once per chunk */
     FCG_OPT_CHUNK        = 1, /* iterations per chunk in loop mode 1 (default 16) */
-    FCG_OPT_ROW_VARIANT  = 2  /* -1 (default): tuned rows-per-CTA of the row passes; 0,1,..: force variant */
+    FCG_OPT_ROW_VARIANT  = 2, /* -1 (default): tuned rows-per-CTA of the classic row passes; 0,1,..: force variant */
+    FCG_OPT_ENGINE       = 3  /* 0 (default): pipelined TMA passes where the lattice is large enough (L >= 512), classic
+                                 passes otherwise; 1: classic passes only (synchronous loads; kept for A/B measurements) */
 } fcg_option;
 
 /* Bytes of device workspace a handle of this size needs (0 if the size is unsupported). */

@@ -8,6 +8,8 @@
 #include <string>
 #include <vector>
 
+#include <cuda.h>
+
 #include "../../include/fcg.h"
 #include "fcg_kernels.cuh"
 #include "fcg_plans.cuh"
@@ -72,7 +74,10 @@ struct fcg_handle_s {
     char* ws = nullptr; bool own_ws = false;
     Layout lay{};
     bool have_spectrum = false;
-    int loop_mode = 0, chunk = 16, row_var_opt = -1;
+    int loop_mode = 0, chunk = 16, row_var_opt = -1, engine_opt = 0;
+    alignas(64) CUtensorMap tmap;       // T as a 2D tensor [L/2][2L reals], box = 2 complex x v2_tbox frequencies (row_inv2)
+    bool have_tmap = false;
+    bool v2() const { return engine_opt == 0 && tab->v2 && have_tmap; }
     Scalars* h_sc = nullptr;            // pinned
     BreakResult* h_brk = nullptr;       // pinned
     void *hk = nullptr, *hf = nullptr, *hu = nullptr;   // device staging of fcg_solve_host
@@ -121,17 +126,20 @@ template <typename T> struct Seq {
 
     cudaError_t row_fwd(int mode, const T* x, T* u) const {
         RowFwdArgs<T> A{}; A.mode = mode; A.x = x; A.u = u; A.p = p(); A.r = r(); A.Tb = Tb(); A.tw = tw(); A.sc = h->sc();
-        ++h->launches; return h->tab->row_fwd(h->row_var(), &A, st);
+        ++h->launches;
+        return h->v2() ? h->tab->row_fwd2(&A, st) : h->tab->row_fwd(h->row_var(), &A, st);
     }
     cudaError_t col(int mode, bool cg) const {
         ColArgs<T> A{}; A.mode = mode; A.Tb = Tb(); A.shat = shat(); A.tw = tw(); A.sc = cg ? h->sc() : nullptr;
-        ++h->launches; return h->tab->col(&A, st);
+        ++h->launches;
+        return (h->v2() && mode == COL_CONV) ? h->tab->col2(&A, st) : h->tab->col(&A, st);
     }
     cudaError_t row_inv(int mode, const T* k, const T* v, const T* f, T* out, T* out2) const {
         RowInvArgs<T> A{}; A.mode = mode; A.Tb = Tb(); A.tw = tw(); A.k = k; A.v = v; A.f = f; A.out = out; A.out2 = out2;
         A.scale = (T)(1.0 / ((double)h->L * (double)h->L));
         A.partial = h->at<double>(h->lay.partial_row); A.sc = h->sc();
-        ++h->launches; return h->tab->row_inv(h->row_var(), &A, st);
+        ++h->launches;
+        return h->v2() ? h->tab->row_inv2(&A, &h->tmap, st) : h->tab->row_inv(h->row_var(), &A, st);
     }
     // set up initial values: r = f - A u, p = 0 (first direction p = r + 0*p), rho, ||f||^2
     cudaError_t init(const T* k, const T* f, T* u, double tol, int maxit, bool use_cond, unsigned long long cond) const {
@@ -228,7 +236,7 @@ template <typename T>
 int solve_impl(fcg_handle h, const void* k, const void* f, void* u, double tol, int maxit, int* iters, double* relres) {
     h->launches = 0;
     if (h->loop_mode == 0) {
-        const int var = h->row_var();
+        const int var = h->v2() ? 100 : h->row_var();
         GraphEntry* hit = nullptr;
         for (auto& g : h->graphs)
             if (g.k == k && g.f == f && g.u == u && g.tol == tol && g.maxit == maxit && g.var == var) { hit = &g; break; }
@@ -363,6 +371,32 @@ int twiddle_init(fcg_handle h) {
 
 bool supported(int L) { return L >= 16 && L <= 8192 && (L & (L - 1)) == 0; }
 
+// CUtensorMap of T for the tile loads of row_inv2 (driver entry point fetched through the runtime: no -lcuda)
+int tensor_map_init(fcg_handle h) {
+    typedef CUresult (*EncodeTiled)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                    const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                    CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn ||
+        qres != cudaDriverEntryPointSuccess) {
+        cudaGetLastError();
+        h->err = "cuTensorMapEncodeTiled unavailable; using the classic passes";
+        return FCG_OK;
+    }
+    const cuuint64_t gdim[2] = {(cuuint64_t)2 * h->L, (cuuint64_t)h->L / 2};
+    const cuuint64_t gstride[1] = {(cuuint64_t)2 * h->L * h->w};
+    const cuuint32_t box[2] = {4u, (cuuint32_t)h->tab->v2_tbox};
+    const cuuint32_t estr[2] = {1u, 1u};
+    CUresult r = reinterpret_cast<EncodeTiled>(fn)(&h->tmap, h->dtype == FCG_F64 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32,
+                                                   2, h->ws + h->lay.Tb, gdim, gstride, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                                                   CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                                                   CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) { h->err = "cuTensorMapEncodeTiled failed (code " + std::to_string((int)r) + ")"; return FCG_CUDA_ERROR; }
+    h->have_tmap = true;
+    return FCG_OK;
+}
+
 }  // namespace
 
 // ================================================================================== C ABI
@@ -401,6 +435,7 @@ int fcg_create(int L, fcg_dtype dt, void* workspace, void* cuda_stream, fcg_hand
     if (cudaMemsetAsync(h->ws + h->lay.scalars, 0, h->lay.total - h->lay.scalars, h->stream) != cudaSuccess) return bail(FCG_CUDA_ERROR);
     int st = dt == FCG_F64 ? twiddle_init<double>(h) : twiddle_init<float>(h);
     if (st != FCG_OK) return bail(st);
+    if (h->tab->v2 && (st = tensor_map_init(h)) != FCG_OK) return bail(st);
     *out = h;
     return FCG_OK;
 }
@@ -429,6 +464,7 @@ int fcg_set_option(fcg_handle h, int option, int value) {
         case FCG_OPT_ROW_VARIANT:
             if (value >= FCG_NROWVAR || (value >= 0 && !h->tab->row_valid[value])) return fail(h, FCG_INVALID_ARG, "row variant not available for this size");
             h->row_var_opt = value; return FCG_OK;
+        case FCG_OPT_ENGINE: if (value != 0 && value != 1) return fail(h, FCG_INVALID_ARG, "engine must be 0 or 1"); h->engine_opt = value; return FCG_OK;
     }
     return fail(h, FCG_INVALID_ARG, "unknown option");
 }

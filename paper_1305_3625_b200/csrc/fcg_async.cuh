@@ -1,0 +1,426 @@
+// fcg_async.cuh -- the three transform passes of one operator application (Listing 4) with their
+// fused vector work (Listing 2), written for sm_100a's asynchronous copy engine:
+//
+//   * one CTA per transform (P::NT threads), several CTAs resident per SM, so that one CTA's copies are in flight
+//     while its neighbours run butterflies;
+//   * every global read arrives through TMA (cp.async.bulk / cp.async.bulk.tensor) into shared memory and signals
+//     an mbarrier: no register staging, no load latency on the instruction stream, depth bounded by shared memory;
+//   * vectors that are read strip-wise (p, r, u in P1; k, p in P3) stream through a small ring of shared-memory
+//     slots that lives inside the transform's own work buffer while that buffer is idle;
+//   * the column pass runs in place in shared memory and leaves through one bulk store;
+//   * twiddles: one base twiddle per butterfly in registers + powers (fcg_engine.cuh), no table traffic.
+//
+// Every hand-over between the threads' own (generic-proxy) accesses to a shared-memory slot and a TMA (async-proxy)
+// access to the same slot goes through an mbarrier: "full" barriers carry the copy's byte count, "empty" / "ready"
+// barriers collect one arrival per warp.  A CTA barrier (bar.sync) is NOT used for that: it only orders the generic
+// proxy.  A consumer releases a slot with fence.proxy.async + arrive (tma::mbar_warp_release): without the fence a
+// still-queued ld.shared can be overtaken by the refill (measured, see fcg_tma.cuh).  bar.sync is used between
+// butterfly stages only.
+//
+// Same mathematics, data layout (T[n][a], packed n=0/L/2 column, digit-reversed spectrum) and modes as
+// fcg_passes.cuh, which remains the path for small lattices (NT < 64) and the host-replayable statement of the
+// index algebra.  Byte counts per launch: DESIGN.md section 4.
+#pragma once
+#include <cuda.h>
+#include "fcg_kernels.cuh"
+#include "fcg_plans.cuh"
+#include "fcg_tma.cuh"
+
+namespace fcg {
+
+template <typename T, typename P> struct AsyncShape {
+    static constexpr int L = P::N, NT = P::NT, R1 = P::radix(1), Q1 = L / R1, PER1 = Q1 / NT;
+    static constexpr bool valid = NT >= 64 && L >= 512;
+    static constexpr size_t WBYTES = (size_t)L * 2 * sizeof(T);              // one complex transform
+    static constexpr uint32_t PIECE = (uint32_t)(Q1 * sizeof(T));            // one stage-1 strip of one real row
+    static constexpr int MAXSLOT = 8;
+    // P3: ring beside the work buffer; first holds two tiles of T (TSUB frequencies each), then strips of k, p (, f)
+    static constexpr size_t RB = WBYTES > 32768 ? 32768 : WBYTES;
+    static constexpr int TSUB = (int)(RB / 2 / (2 * 2 * sizeof(T)));
+    static constexpr int TBOX = TSUB < 256 ? TSUB : 256;                     // frequencies per tensor-map box
+    static constexpr int NSUB = (L / 2) / TSUB;
+    static constexpr size_t fwd_smem = WBYTES + 128;                          // + 128: the kernels align the dynamic base themselves
+    static constexpr size_t col_smem = WBYTES + (size_t)L * sizeof(T) + 128;
+    static constexpr size_t inv_smem = WBYTES + RB + 128;
+    static constexpr int thread_cap = sizeof(T) == 8 ? 512 : 1024;           // 128 / 64 registers per thread
+    static constexpr int ctas(size_t smem) {
+        const int by_smem = (int)((size_t)FCG_MAX_SMEM / (smem + 1024));
+        const int by_thr = thread_cap / NT > 1 ? thread_cap / NT : 1;
+        return by_smem < 1 ? 1 : (by_smem < by_thr ? by_smem : by_thr);
+    }
+    static_assert(!valid || (WBYTES >= 6 * (size_t)PIECE && RB >= 6 * (size_t)PIECE), "ring too small for one strip");
+    static_assert(!valid || (TSUB % TBOX == 0 && (L / 2) % TSUB == 0 && NSUB >= 2 && NSUB % 2 == 0 && NT % 32 == 0), "tile shape");
+};
+
+#ifdef __CUDACC__
+
+// TMA tensor tiles want a 128-byte aligned destination; the dynamic shared-memory base only promises 16
+__device__ __forceinline__ unsigned char* align128(unsigned char* p) { return p + ((128u - (tma::smem_u32(p) & 127u)) & 127u); }
+
+template <typename T> __device__ __forceinline__ void store_pair(cx<T>* dst, cx<T> a, cx<T> b);
+template <> __device__ __forceinline__ void store_pair<double>(double2* dst, double2 a, double2 b) { dst[0] = a; dst[1] = b; }
+template <> __device__ __forceinline__ void store_pair<float>(float2* dst, float2 a, float2 b) {
+    *reinterpret_cast<float4*>(dst) = make_float4(a.x, a.y, b.x, b.y);
+}
+
+template <typename P> constexpr int per_max() {
+    int m = 1;
+    for (int s = 1; s <= P::S; ++s) { const int per = (P::N / P::radix(s)) / P::NT; if (per > m) m = per; }
+    return m;
+}
+
+// --------------------------------------------------------------------------------------------- P1
+//   [u += alpha p;  p = r + beta p;]   T[n][a0], T[n][a0+1] = row transforms of rows a0, a0+1 of p (or x)
+template <typename T, typename P, int CTAS>
+__global__ void __launch_bounds__(P::NT, CTAS) row_fwd2_kernel(const RowFwdArgs<T> A)
+{
+    using AS = AsyncShape<T, P>;
+    constexpr int L = P::N, S = P::S, NT = P::NT, R1 = AS::R1, Q1 = AS::Q1, PER1 = AS::PER1, PM = per_max<P>();
+    constexpr uint32_t PIECE = AS::PIECE;
+    extern __shared__ unsigned char smem_dyn[];
+    unsigned char* const smem_raw = align128(smem_dyn);
+    __shared__ __align__(8) uint64_t full[AS::MAXSLOT];
+    __shared__ __align__(8) uint64_t empty[AS::MAXSLOT];
+    cx<T>* W = reinterpret_cast<cx<T>*>(smem_raw);
+    SmemIO<T, P> io{W};
+    const int lt = threadIdx.x, lane = lt & 31, warp = lt >> 5;
+    const int a0 = 2 * (int)blockIdx.x;
+    const size_t row0 = (size_t)a0 * L;
+    const bool cg = A.mode == ROWF_CG;
+    const int nv = cg ? 6 : 2;
+    int nslot = (int)(AS::WBYTES / (nv * PIECE));
+    nslot = nslot > AS::MAXSLOT ? AS::MAXSLOT : nslot;
+    nslot = nslot > R1 ? R1 : nslot;
+
+    // strip t of the two rows: elements [t Q1, (t+1) Q1) of p0 p1 r0 r1 u0 u1 (or x0 x1); called by all of warp 0
+    auto issue = [&](int t) {
+        const int slot = t % nslot;
+        if (lane == 0) tma::mbar_expect_tx(&full[slot], nv * PIECE);
+        __syncwarp();
+        if (lane < nv) {
+            const T* src = cg ? (lane < 2 ? A.p : lane < 4 ? A.r : A.u) : A.x;
+            src += row0 + (size_t)(lane & 1) * L + (size_t)t * Q1;
+            tma::bulk_g2s(smem_raw + (size_t)slot * nv * PIECE + (size_t)lane * PIECE, src, PIECE, &full[slot]);
+        }
+    };
+    if (lt == 0) {
+        for (int i = 0; i < AS::MAXSLOT; ++i) { tma::mbar_init(&full[i], 1); tma::mbar_init(&empty[i], NT / 32); }
+        tma::fence_mbar_init();
+    }
+    __syncthreads();
+    if (warp == 0)
+        for (int t = 0; t < nslot; ++t) issue(t);
+
+    T alpha = (T)0, beta = (T)0;
+    bool done = false;
+    if (cg) { done = A.sc->done != 0; alpha = (T)A.sc->alpha; beta = (T)A.sc->beta; }
+    cx<T> wb[S + 1][PM];
+    static_for_up<1, S - 1>([&](auto s) { base_tw<P, decltype(s)::value, T>(lt, A.tw, wb[decltype(s)::value]); });
+
+    if (done) {      // converged: nothing may change; drain the copies already issued and leave
+        for (int t = 0; t < nslot; ++t) tma::mbar_wait(&full[t], 0);
+        return;
+    }
+
+    // phase A: strips stream through the ring; vector update on the fly; z = p_even + i p_odd
+    cx<T> z[PER1][R1];
+#pragma unroll
+    for (int t = 0; t < R1; ++t) {
+        const int slot = t % nslot;
+        tma::mbar_wait(&full[slot], (uint32_t)((t / nslot) & 1));
+        const T* sl = reinterpret_cast<const T*>(smem_raw + (size_t)slot * nv * PIECE);
+#pragma unroll
+        for (int i = 0; i < PER1; ++i) {
+            const int j = lt + i * NT;
+            if (cg) {
+                T p0 = sl[j], p1 = sl[Q1 + j];
+                const T r0 = sl[2 * Q1 + j], r1 = sl[3 * Q1 + j];
+                T u0 = sl[4 * Q1 + j], u1 = sl[5 * Q1 + j];
+                u0 = u0 + alpha * p0; u1 = u1 + alpha * p1;       // new x, lagged one pass
+                p0 = r0 + beta * p0;  p1 = r1 + beta * p1;        // new direction
+                const size_t i0 = row0 + (size_t)t * Q1 + j;
+                A.u[i0] = u0; A.u[i0 + L] = u1;
+                A.p[i0] = p0; A.p[i0 + L] = p1;
+                z[i][t] = mk<T>(p0, p1);
+            } else {
+                z[i][t] = mk<T>(sl[j], sl[Q1 + j]);
+            }
+        }
+        if (t + nslot < R1) {
+            tma::mbar_warp_release(&empty[slot]);                  // this warp has read the slot
+            if (warp == 0) {
+                tma::mbar_wait(&empty[slot], (uint32_t)((t / nslot) & 1));     // ... and so has every other warp
+                issue(t + nslot);
+            }
+        }
+    }
+    __syncthreads();                                              // ring (inside W) fully consumed
+    stage_math<P, 1, -1, T>(z, wb[1]);
+    stage_st<P, 1, T>(lt, [&](int e, cx<T> v) { io.st(e, v); }, z);
+    __syncthreads();
+    static_for_up<2, S>([&](auto s) {
+        constexpr int sv = decltype(s)::value;
+        cx<T> a[St<P, sv>::PER][St<P, sv>::R];
+        stage_ld<P, sv, T>(lt, [&](int e) { return io.ld(e); }, a);
+        stage_math<P, sv, -1, T>(a, wb[sv]);
+        stage_st<P, sv, T>(lt, [&](int e, cx<T> v) { io.st(e, v); }, a);
+        __syncthreads();
+    });
+    // separate the two rows and store transposed: T[n][a0] = X_even[n], T[n][a0+1] = X_odd[n]
+    const T h = (T)0.5;
+#pragma unroll 4
+    for (int n = lt; n < L / 2; n += NT) {
+        cx<T> X0, X1;
+        if (n == 0) {
+            const cx<T> Z0 = io.ld(P::pos_of(0)), ZN = io.ld(P::pos_of(L / 2));
+            X0 = mk<T>(Z0.x, ZN.x); X1 = mk<T>(Z0.y, ZN.y);
+        } else {
+            const cx<T> Za = io.ld(P::pos_of(n)), Zb = io.ld(P::pos_of(L - n));
+            X0 = mk<T>((Za.x + Zb.x) * h, (Za.y - Zb.y) * h);
+            X1 = mk<T>((Za.y + Zb.y) * h, (Zb.x - Za.x) * h);
+        }
+        store_pair<T>(A.Tb + (size_t)n * L + a0, X0, X1);
+    }
+}
+
+// --------------------------------------------------------------------------------------------- P2
+//   column n of T, in place:  T[n][.] <- F^H ( shat[n][.] o F T[n][.] )
+template <typename T, typename P, int CTAS>
+__global__ void __launch_bounds__(P::NT, CTAS) col2_kernel(const ColArgs<T> A)
+{
+    using AS = AsyncShape<T, P>;
+    constexpr int L = P::N, S = P::S, NT = P::NT, PM = per_max<P>();
+    extern __shared__ unsigned char smem_dyn[];
+    unsigned char* const smem_raw = align128(smem_dyn);
+    __shared__ __align__(8) uint64_t bar, ready;
+    cx<T>* W = reinterpret_cast<cx<T>*>(smem_raw);
+    T* sh = reinterpret_cast<T*>(smem_raw + AS::WBYTES);
+    SmemIO<T, P> io{W};
+    const int lt = threadIdx.x, n = (int)blockIdx.x;
+    cx<T>* col = A.Tb + (size_t)n * L;
+    if (lt == 0) {
+        tma::mbar_init(&bar, 1);
+        tma::mbar_init(&ready, NT / 32);
+        tma::fence_mbar_init();
+        tma::mbar_expect_tx(&bar, (uint32_t)(AS::WBYTES + (n ? L * sizeof(T) : 0)));
+        tma::bulk_g2s(W, col, (uint32_t)AS::WBYTES, &bar);
+        if (n) tma::bulk_g2s(sh, A.shat + (size_t)n * L, (uint32_t)(L * sizeof(T)), &bar);
+    }
+    __syncthreads();
+    const bool done = A.sc && A.sc->done;
+    cx<T> wb[S + 1][PM];
+    static_for_up<1, S - 1>([&](auto s) { base_tw<P, decltype(s)::value, T>(lt, A.tw, wb[decltype(s)::value]); });
+    tma::mbar_wait(&bar, 0);
+    if (done) return;
+
+    auto ld_sw = [&](int e) { return io.ld(e); };
+    auto st_sw = [&](int e, cx<T> v) { io.st(e, v); };
+    auto fwd_smem_stage = [&](auto s) {
+        constexpr int sv = decltype(s)::value;
+        cx<T> a[St<P, sv>::PER][St<P, sv>::R];
+        stage_ld<P, sv, T>(lt, ld_sw, a);
+        stage_math<P, sv, -1, T>(a, wb[sv]);
+        stage_st<P, sv, T>(lt, st_sw, a);
+        __syncthreads();
+    };
+    auto inv_smem_stage = [&](auto s) {
+        constexpr int sv = decltype(s)::value;
+        cx<T> a[St<P, sv>::PER][St<P, sv>::R];
+        stage_ld<P, sv, T>(lt, ld_sw, a);
+        stage_math<P, sv, +1, T>(a, wb[sv]);
+        stage_st<P, sv, T>(lt, st_sw, a);
+        __syncthreads();
+    };
+    {   // forward stage 1: the column arrived in natural (linear) order; it leaves the stage swizzled
+        cx<T> a[St<P, 1>::PER][St<P, 1>::R];
+        stage_ld<P, 1, T>(lt, [&](int e) { return W[e]; }, a);
+        __syncthreads();
+        stage_math<P, 1, -1, T>(a, wb[1]);
+        stage_st<P, 1, T>(lt, st_sw, a);
+        __syncthreads();
+    }
+    if (n != 0) {
+        static_for_up<2, S - 1>(fwd_smem_stage);
+        // last forward stage * shat * first inverse stage, in registers
+        run_middle<P, T>(lt, ld_sw, st_sw, [&](int g, int u) { return sh[u * (L / P::RLAST) + g]; });
+        __syncthreads();
+        static_for_down<S - 1, 2>(inv_smem_stage);
+    } else {
+        // packed column: W = Y0 + i YN.  W'[m] = sp[m] W[m] + sm[m] conj W[-m], sp = (s0+sN)/2 (row 0 of shat),
+        // sm = (s0-sN)/2 (row L/2 of shat); pairs (m, L-m), m <= L/2
+        static_for_up<2, S>(fwd_smem_stage);
+        const T* sp_ = A.shat;
+        const T* sm_ = A.shat + (size_t)(L / 2) * L;
+        for (int m = lt; m <= L / 2; m += NT) {
+            const int e = P::pos_of(m), e2 = P::pos_of((L - m) % L);
+            const cx<T> Wa = io.ld(e), Wb = io.ld(e2);
+            cx<T> va, vb;
+            const int i1 = P::shat_index(e), i2 = P::shat_index(e2);
+            va.x = sp_[i1] * Wa.x + sm_[i1] * Wb.x; va.y = sp_[i1] * Wa.y - sm_[i1] * Wb.y;
+            vb.x = sp_[i2] * Wb.x + sm_[i2] * Wa.x; vb.y = sp_[i2] * Wb.y - sm_[i2] * Wa.y;
+            io.st(e, va);
+            if (e2 != e) io.st(e2, vb);
+        }
+        __syncthreads();
+        static_for_down<S, 2>(inv_smem_stage);
+    }
+    {   // inverse stage 1: swizzled in, natural order out, ready for the bulk store
+        cx<T> a[St<P, 1>::PER][St<P, 1>::R];
+        stage_ld<P, 1, T>(lt, ld_sw, a);
+        stage_math<P, 1, +1, T>(a, wb[1]);
+        __syncthreads();
+        stage_st<P, 1, T>(lt, [&](int e, cx<T> v) { W[e] = v; }, a);
+    }
+    tma::fence_proxy_async();                 // my writes -> visible to the async proxy
+    tma::mbar_warp_arrive(&ready);
+    if (lt == 0) {
+        tma::mbar_wait(&ready, 0);            // every warp's part of the column is in place
+        tma::bulk_s2g(col, W, (uint32_t)AS::WBYTES);
+        tma::bulk_commit();
+        tma::bulk_wait_read0();          // shared memory must outlive the store's read
+    }
+}
+
+// --------------------------------------------------------------------------------------------- P3
+//   c = F_row^H T (rows a0, a0+1);  q = k o p + c  [+ partial p.q]   (or residual / apply / plain)
+template <typename T, typename P, int CTAS>
+__global__ void __launch_bounds__(P::NT, CTAS) row_inv2_kernel(const RowInvArgs<T> A, const __grid_constant__ CUtensorMap tmap)
+{
+    using AS = AsyncShape<T, P>;
+    constexpr int L = P::N, S = P::S, NT = P::NT, R1 = AS::R1, Q1 = AS::Q1, PER1 = AS::PER1, PM = per_max<P>();
+    constexpr uint32_t PIECE = AS::PIECE;
+    constexpr int TSUB = AS::TSUB, NSUB = AS::NSUB, TBOX = AS::TBOX;
+    constexpr uint32_t TBYTES = (uint32_t)(TSUB * 2 * sizeof(cx<T>));
+    extern __shared__ unsigned char smem_dyn[];
+    unsigned char* const smem_raw = align128(smem_dyn);
+    __shared__ __align__(8) uint64_t tfull[2], tempty[2];
+    __shared__ __align__(8) uint64_t kfull[AS::MAXSLOT], kempty[AS::MAXSLOT];
+    __shared__ double red[2 * 32];
+    cx<T>* W = reinterpret_cast<cx<T>*>(smem_raw);
+    unsigned char* ring = smem_raw + AS::WBYTES;
+    SmemIO<T, P> io{W};
+    const int lt = threadIdx.x, lane = lt & 31, warp = lt >> 5;
+    const int a0 = 2 * (int)blockIdx.x;
+    const size_t row0 = (size_t)a0 * L;
+    const int mode = A.mode;
+    const int nv = mode == ROWI_PLAIN ? 0 : (mode == ROWI_RESID ? 6 : 4);
+    int nks = nv ? (int)(AS::RB / (nv * PIECE)) : 1;
+    nks = nks > AS::MAXSLOT ? AS::MAXSLOT : nks;
+    nks = nks > R1 ? R1 : nks;
+
+    auto issue_T = [&](int sub) {        // thread 0: TSUB frequencies x (a0, a0+1) of T, as TSUB/TBOX boxes
+        const int slot = sub & 1;
+        tma::mbar_expect_tx(&tfull[slot], TBYTES);
+#pragma unroll
+        for (int b = 0; b < TSUB / TBOX; ++b)
+            tma::tensor_g2s_2d(ring + (size_t)slot * TBYTES + (size_t)b * TBOX * 2 * sizeof(cx<T>), &tmap, 2 * a0, sub * TSUB + b * TBOX,
+                               &tfull[slot]);
+    };
+    auto issue_K = [&](int t) {          // all of warp 0: strip t of k0 k1 v0 v1 (f0 f1)
+        const int slot = t % nks;
+        if (lane == 0) tma::mbar_expect_tx(&kfull[slot], nv * PIECE);
+        __syncwarp();
+        if (lane < nv) {
+            const T* src = lane < 2 ? A.k : lane < 4 ? A.v : A.f;
+            src += row0 + (size_t)(lane & 1) * L + (size_t)t * Q1;
+            tma::bulk_g2s(ring + (size_t)slot * nv * PIECE + (size_t)lane * PIECE, src, PIECE, &kfull[slot]);
+        }
+    };
+    if (lt == 0) {
+        tma::prefetch_tmap(&tmap);
+        tma::mbar_init(&tfull[0], 1); tma::mbar_init(&tfull[1], 1);
+        tma::mbar_init(&tempty[0], NT / 32); tma::mbar_init(&tempty[1], NT / 32);
+        for (int i = 0; i < AS::MAXSLOT; ++i) { tma::mbar_init(&kfull[i], 1); tma::mbar_init(&kempty[i], NT / 32); }
+        tma::fence_mbar_init();
+        issue_T(0); issue_T(1);
+    }
+    __syncthreads();
+    const bool done = mode == ROWI_CG && A.sc->done;
+    cx<T> wb[S + 1][PM];
+    static_for_up<1, S - 1>([&](auto s) { base_tw<P, decltype(s)::value, T>(lt, A.tw, wb[decltype(s)::value]); });
+    if (done) { tma::mbar_wait(&tfull[0], 0); tma::mbar_wait(&tfull[1], 0); return; }
+
+    // rebuild the packed spectrum Z = X_even + i X_odd at its digit-reversed place, tile by tile
+    for (int sub = 0; sub < NSUB; ++sub) {
+        tma::mbar_wait(&tfull[sub & 1], (uint32_t)((sub >> 1) & 1));
+        const cx<T>* Ts = reinterpret_cast<const cx<T>*>(ring + (size_t)(sub & 1) * TBYTES);
+#pragma unroll 4
+        for (int nl = lt; nl < TSUB; nl += NT) {
+            const int n = sub * TSUB + nl;
+            const cx<T> X0 = Ts[2 * nl], X1 = Ts[2 * nl + 1];
+            if (n == 0) {
+                io.st(P::pos_of(0), mk<T>(X0.x, X1.x));
+                io.st(P::pos_of(L / 2), mk<T>(X0.y, X1.y));
+            } else {
+                io.st(P::pos_of(n), mk<T>(X0.x - X1.y, X0.y + X1.x));
+                io.st(P::pos_of(L - n), mk<T>(X0.x + X1.y, X1.x - X0.y));
+            }
+        }
+        tma::mbar_warp_release(&tempty[sub & 1]);                  // this warp has read the tile
+        if (lt == 0 && sub + 2 < NSUB) {
+            tma::mbar_wait(&tempty[sub & 1], (uint32_t)((sub >> 1) & 1));
+            issue_T(sub + 2);
+        }
+    }
+    __syncthreads();                                              // Z complete in W
+    // once every warp is done with the tiles the ring is free: start streaming the strips of k, p (, f) for the epilogue
+    if (warp == 0 && nv) {
+        constexpr uint32_t fin = (uint32_t)((NSUB / 2 - 1) & 1);
+        tma::mbar_wait(&tempty[0], fin); tma::mbar_wait(&tempty[1], fin);
+        for (int t = 0; t < nks; ++t) issue_K(t);
+    }
+
+    static_for_down<S, 2>([&](auto s) {
+        constexpr int sv = decltype(s)::value;
+        cx<T> a[St<P, sv>::PER][St<P, sv>::R];
+        stage_ld<P, sv, T>(lt, [&](int e) { return io.ld(e); }, a);
+        stage_math<P, sv, +1, T>(a, wb[sv]);
+        stage_st<P, sv, T>(lt, [&](int e, cx<T> v) { io.st(e, v); }, a);
+        __syncthreads();
+    });
+    // inverse stage 1 straight into the epilogue: natural order, re = even row, im = odd row
+    cx<T> c[PER1][R1];
+    stage_ld<P, 1, T>(lt, [&](int e) { return io.ld(e); }, c);
+    stage_math<P, 1, +1, T>(c, wb[1]);
+    double acc[2] = {0.0, 0.0};
+#pragma unroll
+    for (int t = 0; t < R1; ++t) {
+        const T* sl = nullptr;
+        if (nv) {
+            const int slot = t % nks;
+            tma::mbar_wait(&kfull[slot], (uint32_t)((t / nks) & 1));
+            sl = reinterpret_cast<const T*>(ring + (size_t)slot * nv * PIECE);
+        }
+#pragma unroll
+        for (int i = 0; i < PER1; ++i) {
+            const int j = lt + i * NT;
+            const size_t i0 = row0 + (size_t)t * Q1 + j;
+            const T c0 = c[i][t].x, c1 = c[i][t].y;
+            if (mode == ROWI_PLAIN) { A.out[i0] = c0 * A.scale; A.out[i0 + L] = c1 * A.scale; continue; }
+            const T v0 = sl[2 * Q1 + j], v1 = sl[3 * Q1 + j];
+            const T val0 = sl[j] * v0 + c0, val1 = sl[Q1 + j] * v1 + c1;         // k o x + C x
+            if (mode == ROWI_RESID) {
+                const T f0 = sl[4 * Q1 + j], f1 = sl[5 * Q1 + j];
+                const T r0 = f0 - val0, r1 = f1 - val1;                           // r = f - A u
+                A.out[i0] = r0; A.out[i0 + L] = r1; A.out2[i0] = (T)0; A.out2[i0 + L] = (T)0;
+                acc[0] += (double)r0 * (double)r0; acc[0] += (double)r1 * (double)r1;
+                acc[1] += (double)f0 * (double)f0; acc[1] += (double)f1 * (double)f1;
+            } else {
+                A.out[i0] = val0; A.out[i0 + L] = val1;
+                acc[0] += (double)v0 * (double)val0; acc[0] += (double)v1 * (double)val1;   // search length p.Ap
+            }
+        }
+        if (nv && t + nks < R1) {
+            tma::mbar_warp_release(&kempty[t % nks]);
+            if (warp == 0) {
+                tma::mbar_wait(&kempty[t % nks], (uint32_t)((t / nks) & 1));
+                issue_K(t + nks);
+            }
+        }
+    }
+    row_inv_reduce_finalize<T>(A, acc, red);
+}
+
+#endif  // __CUDACC__
+
+}  // namespace fcg

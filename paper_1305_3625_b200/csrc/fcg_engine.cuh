@@ -73,6 +73,80 @@ FCG_HD void run_middle(int lt, LD ld, ST st, MUL mul)
     }
 }
 
+// ---- register-resident stages (used by the pipelined passes, fcg_async.cuh) ----------------------------
+// The same stage split into load / math / store so that barriers, asynchronous-copy waits and fused epilogues
+// can be placed between the steps.  Twiddles are not read from the [u][j] tables: each thread keeps the base
+// twiddle w = w_M^j of each of its butterflies (one table entry, fetched once at kernel start) and forms the
+// powers w^2 .. w^(R-1) by a product tree of depth log2 R (error <= ~4 ulp), which costs no memory traffic.
+template <typename P, int s> struct St {
+    static constexpr int R = P::radix(s), M = P::mlen(s), Q = M / R, NB = P::N / R, PER = NB / P::NT, TWO = P::tw_off(s);
+    static_assert(PER >= 1, "plan: NT too large for this radix");
+};
+
+template <int R, typename C> FCG_HD void tw_powers(C w, C (&pw)[R]) {
+    pw[0] = w;
+    if constexpr (R > 1) pw[1] = w;
+#pragma unroll
+    for (int u = 2; u < R; ++u) pw[u] = cmulw(pw[u / 2], pw[u - u / 2]);
+}
+
+// base twiddles of this thread's butterflies in stage s (u = 1 row of the stage's table)
+template <typename P, int s, typename T> FCG_HD void base_tw(int lt, const cx<T>* __restrict__ tw, cx<T>* w) {
+    using I = St<P, s>;
+    if constexpr (I::Q > 1) {
+#pragma unroll
+        for (int i = 0; i < I::PER; ++i) w[i] = tw[I::TWO + (lt + i * P::NT) % I::Q];
+    }
+}
+
+template <typename P, int s, typename T, typename LD>
+FCG_HD void stage_ld(int lt, LD ld, cx<T> (&a)[St<P, s>::PER][St<P, s>::R]) {
+    using I = St<P, s>;
+#pragma unroll
+    for (int i = 0; i < I::PER; ++i) {
+        const int g = lt + i * P::NT;
+        const int base = (g / I::Q) * I::M + g % I::Q;
+#pragma unroll
+        for (int t = 0; t < I::R; ++t) a[i][t] = ld(base + t * I::Q);
+    }
+}
+template <typename P, int s, typename T, typename ST>
+FCG_HD void stage_st(int lt, ST st, const cx<T> (&a)[St<P, s>::PER][St<P, s>::R]) {
+    using I = St<P, s>;
+#pragma unroll
+    for (int i = 0; i < I::PER; ++i) {
+        const int g = lt + i * P::NT;
+        const int base = (g / I::Q) * I::M + g % I::Q;
+#pragma unroll
+        for (int t = 0; t < I::R; ++t) st(base + t * I::Q, a[i][t]);
+    }
+}
+// DIR < 0: a <- DFT_R(a), a[u] *= w^(u);   DIR > 0 (adjoint, run in reverse stage order): a[u] *= conj(w^u), a <- DFT_R^H(a)
+template <typename P, int s, int DIR, typename T>
+FCG_HD void stage_math(cx<T> (&a)[St<P, s>::PER][St<P, s>::R], const cx<T>* w) {
+    using I = St<P, s>;
+#pragma unroll
+    for (int i = 0; i < I::PER; ++i) {
+        if constexpr (DIR < 0) {
+            dftR<I::R, -1>(a[i]);
+            if constexpr (I::Q > 1) {
+                cx<T> pw[I::R];
+                tw_powers<I::R>(w[i], pw);
+#pragma unroll
+                for (int u = 1; u < I::R; ++u) a[i][u] = cmulw(a[i][u], pw[u]);
+            }
+        } else {
+            if constexpr (I::Q > 1) {
+                cx<T> pw[I::R];
+                tw_powers<I::R>(w[i], pw);
+#pragma unroll
+                for (int u = 1; u < I::R; ++u) a[i][u] = cmulwc(a[i][u], pw[u]);
+            }
+            dftR<I::R, +1>(a[i]);
+        }
+    }
+}
+
 // Compile-time loops over the middle stages (everything between the first and the last stage lives in
 // shared memory and needs a barrier after each stage; `sync()` is __syncthreads on the device and a
 // no-op in the host harness, which runs whole phases thread by thread instead).

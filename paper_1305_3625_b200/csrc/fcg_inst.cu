@@ -1,8 +1,8 @@
 // fcg_inst.cu -- instantiates the transform passes for one lattice size.  Compiled once per supported L
 // with -DFCG_INST_L=<L> (paper_1305_3625_b200/build.py) so the sizes build in parallel.
 #include <cmath>
-#include "fcg_kernels.cuh"
 #include "fcg_plans.cuh"
+#include "fcg_async.cuh"
 
 #ifndef FCG_INST_L
 #error "compile with -DFCG_INST_L=<L>"
@@ -15,7 +15,10 @@ template <typename T> struct Inst {
     using P = typename PlanFor<T, FCG_INST_L>::type;
     using RS = RowShape<T, P>;
     using CS = ColShape<T, P>;
+    using AS = AsyncShape<T, P>;
     static constexpr int L = FCG_INST_L;
+    static constexpr bool V2 = AS::valid;
+    static constexpr int C_FWD = AS::ctas(AS::fwd_smem), C_COL = AS::ctas(AS::col_smem), C_INV = AS::ctas(AS::inv_smem);
 
     // opt in to > 48 KB of dynamic shared memory and ask for the largest shared-memory carveout, so that as
     // many CTAs as the register file allows are resident
@@ -38,7 +41,34 @@ template <typename T> struct Inst {
         if ((e = init_row<1>()) != cudaSuccess) return e;
         if ((e = init_row<2>()) != cudaSuccess) return e;
         if ((e = init_row<3>()) != cudaSuccess) return e;
+        if constexpr (V2) {
+            if ((e = prep(row_fwd2_kernel<T, P, C_FWD>, AS::fwd_smem)) != cudaSuccess) return e;
+            if ((e = prep(col2_kernel<T, P, C_COL>, AS::col_smem)) != cudaSuccess) return e;
+            if ((e = prep(row_inv2_kernel<T, P, C_INV>, AS::inv_smem)) != cudaSuccess) return e;
+        }
         return prep(col_kernel<T, P, CS::COLS>, CS::smem);
+    }
+    static cudaError_t row_fwd2(const void* args, cudaStream_t st) {
+        if constexpr (V2) {
+            row_fwd2_kernel<T, P, C_FWD><<<L / 2, P::NT, AS::fwd_smem, st>>>(*static_cast<const RowFwdArgs<T>*>(args));
+            return cudaGetLastError();
+        }
+        return cudaErrorInvalidValue;
+    }
+    static cudaError_t col2(const void* args, cudaStream_t st) {
+        if constexpr (V2) {
+            col2_kernel<T, P, C_COL><<<L / 2, P::NT, AS::col_smem, st>>>(*static_cast<const ColArgs<T>*>(args));
+            return cudaGetLastError();
+        }
+        return cudaErrorInvalidValue;
+    }
+    static cudaError_t row_inv2(const void* args, const void* tensor_map, cudaStream_t st) {
+        if constexpr (V2) {
+            row_inv2_kernel<T, P, C_INV><<<L / 2, P::NT, AS::inv_smem, st>>>(*static_cast<const RowInvArgs<T>*>(args),
+                                                                              *static_cast<const CUtensorMap*>(tensor_map));
+            return cudaGetLastError();
+        }
+        return cudaErrorInvalidValue;
     }
 
     template <int V> static cudaError_t row_fwd_v(const RowFwdArgs<T>& A, cudaStream_t st) {
@@ -94,6 +124,10 @@ template <typename T> struct Inst {
         t.cols = CS::COLS; t.col_threads = CS::COLS * P::NT; t.col_smem = CS::smem;
         t.tw_total = P::TW_TOTAL;
         t.fill_twiddles = [](void* buf) { fill_twiddles<T, P>(static_cast<cx<T>*>(buf)); };
+        t.v2 = V2 ? 1 : 0; t.v2_tbox = AS::TBOX; t.v2_threads = P::NT;
+        t.v2_ctas[0] = C_FWD; t.v2_ctas[1] = C_COL; t.v2_ctas[2] = C_INV;
+        t.v2_smem[0] = AS::fwd_smem; t.v2_smem[1] = AS::col_smem; t.v2_smem[2] = AS::inv_smem;
+        t.row_fwd2 = &row_fwd2; t.col2 = &col2; t.row_inv2 = &row_inv2;
         t.init = &init; t.row_fwd = &row_fwd; t.col = &col; t.row_inv = &row_inv; t.spectrum_prep = &spectrum_prep;
         return t;
     }

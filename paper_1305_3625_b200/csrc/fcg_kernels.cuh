@@ -95,14 +95,10 @@ __global__ void __launch_bounds__(COLS * P::NT) col_kernel(const ColArgs<T> A) {
     col_body<T, P, COLS>(A, (int)blockIdx.x, reinterpret_cast<cx<T>*>(smem_raw), run);
 }
 
-template <typename T, typename P, int F>
-__global__ void __launch_bounds__(F * P::NT) row_inv_kernel(const RowInvArgs<T> A) {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    __shared__ double red[2 * 32];
-    if (A.mode == ROWI_CG && A.sc->done) return;
-    DevRunner run;
-    double acc[2] = {0.0, 0.0};
-    row_inv_body<T, P, F>(A, (int)blockIdx.x, reinterpret_cast<cx<T>*>(smem_raw), run, acc);
+// Grid-wide reduction of the row pass's partial dot products and the scalar step that follows it:
+// search length alpha = rho / p.Ap in the loop, or the initial values after the residual pass.
+template <typename T>
+__device__ __forceinline__ void row_inv_reduce_finalize(const RowInvArgs<T>& A, double (&acc)[2], double* red) {
     if (A.mode != ROWI_CG && A.mode != ROWI_RESID) return;
     double tot[2];
     if (!grid_sum_last<2>(acc, A.partial, &A.sc->ticket[0], red, tot)) return;
@@ -124,6 +120,17 @@ __global__ void __launch_bounds__(F * P::NT) row_inv_kernel(const RowInvArgs<T> 
         }
         set_cond(sc, !sc->done);
     }
+}
+
+template <typename T, typename P, int F>
+__global__ void __launch_bounds__(F * P::NT) row_inv_kernel(const RowInvArgs<T> A) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    __shared__ double red[2 * 32];
+    if (A.mode == ROWI_CG && A.sc->done) return;
+    DevRunner run;
+    double acc[2] = {0.0, 0.0};
+    row_inv_body<T, P, F>(A, (int)blockIdx.x, reinterpret_cast<cx<T>*>(smem_raw), run, acc);
+    row_inv_reduce_finalize<T>(A, acc, red);
 }
 
 template <typename T, typename P>
