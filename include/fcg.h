@@ -59,7 +59,9 @@ typedef enum {
     FCG_OPT_CHUNK        = 1, /* iterations per chunk in loop mode 1 (default 16) */
     FCG_OPT_ROW_VARIANT  = 2, /* -1 (default): tuned rows-per-CTA of the classic row passes; 0,1,..: force variant */
     FCG_OPT_ENGINE       = 3  /* 0 (default): pipelined TMA passes where the lattice is large enough (L >= 512), classic
-                                 passes otherwise; 1: classic passes only (synchronous loads; kept for A/B measurements) */
+                                 passes otherwise; 1: classic passes only (synchronous loads; kept for A/B measurements).
+                                 The stored spectrum's layout belongs to the engine: changing the engine after
+                                 fcg_set_spectrum requires calling fcg_set_spectrum again (FCG_NO_SPECTRUM otherwise) */
 } fcg_option;
 
 /* Bytes of device workspace a handle of this size needs (0 if the size is unsupported). */

@@ -5,6 +5,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <cstdlib>
 #include <string>
 #include <vector>
 
@@ -74,9 +75,11 @@ struct fcg_handle_s {
     char* ws = nullptr; bool own_ws = false;
     Layout lay{};
     bool have_spectrum = false;
-    int loop_mode = 0, chunk = 16, row_var_opt = -1, engine_opt = 0;
-    alignas(64) CUtensorMap tmap;       // T as a 2D tensor [L/2][2L reals], box = 2 complex x v2_tbox frequencies (row_inv2)
+    int loop_mode = 0, chunk = 16, row_var_opt = -1, engine_opt = 0, nsm = 148;
+    alignas(64) CUtensorMap tmap_row;   // T2 as [L/(2 NB)][L/2][128 B]: box = v2_tsub/NB lines of one row pair (row_inv2 tiles)
+    alignas(64) CUtensorMap tmap_col;   // T2 as [L/(2 NB)][L/2][NB][2 complex]: box = one column x v2_abox row pairs (col2 gather / scatter)
     bool have_tmap = false;
+    int spectrum_colpos = 0;            // layout the stored spectrum was prepared for (1: T2 column order)
     bool v2() const { return engine_opt == 0 && tab->v2 && have_tmap; }
     Scalars* h_sc = nullptr;            // pinned
     BreakResult* h_brk = nullptr;       // pinned
@@ -116,7 +119,8 @@ int fail(fcg_handle h, int code, const char* msg) { if (h) h->err = msg; return 
 
 // ---- launch sequences (typed) ---------------------------------------------------------------
 template <typename T> struct Seq {
-    fcg_handle h; cudaStream_t st;
+    fcg_handle h; cudaStream_t st; bool classic = false;      // classic: force the synchronous passes (stand-alone transforms)
+    bool v2() const { return h->v2() && !classic; }
     cx<T>* Tb() const { return h->at<cx<T>>(h->lay.Tb); }
     const cx<T>* tw() const { return h->at<cx<T>>(h->lay.tw); }
     const T* shat() const { return h->at<T>(h->lay.shat); }
@@ -125,21 +129,21 @@ template <typename T> struct Seq {
     T* q() const { return h->at<T>(h->lay.q); }
 
     cudaError_t row_fwd(int mode, const T* x, T* u) const {
-        RowFwdArgs<T> A{}; A.mode = mode; A.x = x; A.u = u; A.p = p(); A.r = r(); A.Tb = Tb(); A.tw = tw(); A.sc = h->sc();
+        RowFwdArgs<T> A{}; A.mode = mode | ((mode == ROWF_CG && getenv("FCG_DBG")) ? (atoi(getenv("FCG_DBG")) << 8) : 0); A.x = x; A.u = u; A.p = p(); A.r = r(); A.Tb = Tb(); A.tw = tw(); A.sc = h->sc(); A.nsm = h->nsm;
         ++h->launches;
-        return h->v2() ? h->tab->row_fwd2(&A, st) : h->tab->row_fwd(h->row_var(), &A, st);
+        return v2() ? h->tab->row_fwd2(&A, st) : h->tab->row_fwd(h->row_var(), &A, st);
     }
     cudaError_t col(int mode, bool cg) const {
         ColArgs<T> A{}; A.mode = mode; A.Tb = Tb(); A.shat = shat(); A.tw = tw(); A.sc = cg ? h->sc() : nullptr;
         ++h->launches;
-        return (h->v2() && mode == COL_CONV) ? h->tab->col2(&A, st) : h->tab->col(&A, st);
+        return (v2() && mode == COL_CONV) ? h->tab->col2(&A, &h->tmap_col, st) : h->tab->col(&A, st);
     }
     cudaError_t row_inv(int mode, const T* k, const T* v, const T* f, T* out, T* out2) const {
-        RowInvArgs<T> A{}; A.mode = mode; A.Tb = Tb(); A.tw = tw(); A.k = k; A.v = v; A.f = f; A.out = out; A.out2 = out2;
+        RowInvArgs<T> A{}; A.mode = mode | ((mode == ROWI_CG && getenv("FCG_DBG3")) ? (atoi(getenv("FCG_DBG3")) << 8) : 0); A.Tb = Tb(); A.tw = tw(); A.k = k; A.v = v; A.f = f; A.out = out; A.out2 = out2;
         A.scale = (T)(1.0 / ((double)h->L * (double)h->L));
-        A.partial = h->at<double>(h->lay.partial_row); A.sc = h->sc();
+        A.partial = h->at<double>(h->lay.partial_row); A.sc = h->sc(); A.nsm = h->nsm;
         ++h->launches;
-        return h->v2() ? h->tab->row_inv2(&A, &h->tmap, st) : h->tab->row_inv(h->row_var(), &A, st);
+        return v2() ? h->tab->row_inv2(&A, &h->tmap_row, st) : h->tab->row_inv(h->row_var(), &A, st);
     }
     // set up initial values: r = f - A u, p = 0 (first direction p = r + 0*p), rho, ||f||^2
     cudaError_t init(const T* k, const T* f, T* u, double tol, int maxit, bool use_cond, unsigned long long cond) const {
@@ -302,7 +306,7 @@ int break_impl(fcg_handle h, void* k, const void* u, const void* t, long long* i
 
 template <typename T>
 int fft_impl(fcg_handle h, const void* in, void* out, bool inverse) {
-    Seq<T> s{h, h->stream};
+    Seq<T> s{h, h->stream, true};       // public half-spectrum layout goes through the classic T[n][a] passes
     const int L = h->L;
     dim3 blk(32, 8), grd((L / 2 + 31) / 32, (L + 31) / 32);
     if (!inverse) {
@@ -335,15 +339,16 @@ int profile_impl(fcg_handle h, const void* k, const void* f, void* u, int iters,
     Seq<T> s{h, h->stream};
     h->launches = 0;
     FCG_CK(h, s.init((const T*)k, (const T*)f, (T*)u, 0.0, 1 << 30, false, 0ULL));
-    for (int w = 0; w < 2; ++w) FCG_CK(h, s.iteration((const T*)k, (T*)u));       // warm-up
+    if (!getenv("FCG_DBG")) for (int w = 0; w < 2; ++w) FCG_CK(h, s.iteration((const T*)k, (T*)u));       // warm-up
     std::vector<cudaEvent_t> ev((size_t)iters * 5);
     for (auto& e : ev) FCG_CK(h, cudaEventCreate(&e));
     for (int i = 0; i < iters; ++i) {
         cudaEvent_t* e = &ev[(size_t)i * 5];
+        const bool only_fwd = getenv("FCG_DBG") != nullptr && !getenv("FCG_DBG3");
         FCG_CK(h, cudaEventRecord(e[0], h->stream)); FCG_CK(h, s.it_row_fwd((T*)u));
-        FCG_CK(h, cudaEventRecord(e[1], h->stream)); FCG_CK(h, s.it_col());
-        FCG_CK(h, cudaEventRecord(e[2], h->stream)); FCG_CK(h, s.it_row_inv((const T*)k));
-        FCG_CK(h, cudaEventRecord(e[3], h->stream)); FCG_CK(h, s.it_update_r());
+        FCG_CK(h, cudaEventRecord(e[1], h->stream)); if (!only_fwd) FCG_CK(h, s.it_col());
+        FCG_CK(h, cudaEventRecord(e[2], h->stream)); if (!only_fwd) FCG_CK(h, s.it_row_inv((const T*)k));
+        FCG_CK(h, cudaEventRecord(e[3], h->stream)); if (!only_fwd) FCG_CK(h, s.it_update_r());
         FCG_CK(h, cudaEventRecord(e[4], h->stream));
     }
     FCG_CK(h, cudaMemcpyAsync(h->h_sc, h->sc(), sizeof(Scalars), cudaMemcpyDeviceToHost, h->stream));
@@ -384,15 +389,28 @@ int tensor_map_init(fcg_handle h) {
         h->err = "cuTensorMapEncodeTiled unavailable; using the classic passes";
         return FCG_OK;
     }
-    const cuuint64_t gdim[2] = {(cuuint64_t)2 * h->L, (cuuint64_t)h->L / 2};
-    const cuuint64_t gstride[1] = {(cuuint64_t)2 * h->L * h->w};
-    const cuuint32_t box[2] = {4u, (cuuint32_t)h->tab->v2_tbox};
-    const cuuint32_t estr[2] = {1u, 1u};
-    CUresult r = reinterpret_cast<EncodeTiled>(fn)(&h->tmap, h->dtype == FCG_F64 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32,
-                                                   2, h->ws + h->lay.Tb, gdim, gstride, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                                                   CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
-                                                   CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-    if (r != CUDA_SUCCESS) { h->err = "cuTensorMapEncodeTiled failed (code " + std::to_string((int)r) + ")"; return FCG_CUDA_ERROR; }
+    const cuuint64_t L = (cuuint64_t)h->L, w = (cuuint64_t)h->w, NB = (cuuint64_t)h->tab->v2_nb;
+    const CUtensorMapDataType dtp = h->dtype == FCG_F64 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32;
+    void* base = h->ws + h->lay.Tb;
+    auto enc = reinterpret_cast<EncodeTiled>(fn);
+    {   // rows: d0 = one 128-byte line (4 NB reals), d1 = row pair A, d2 = line block m / NB
+        const cuuint64_t gdim[3] = {4 * NB, L / 2, L / (2 * NB)};
+        const cuuint64_t gstride[2] = {4 * NB * w, (L / 2) * 4 * NB * w};
+        const cuuint32_t box[3] = {(cuuint32_t)(4 * NB), 1u, (cuuint32_t)(h->tab->v2_tsub / (int)NB)};
+        const cuuint32_t estr[3] = {1u, 1u, 1u};
+        CUresult r = enc(&h->tmap_row, dtp, 3, base, gdim, gstride, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                         CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r != CUDA_SUCCESS) { h->err = "cuTensorMapEncodeTiled (rows) failed (code " + std::to_string((int)r) + ")"; return FCG_CUDA_ERROR; }
+    }
+    {   // columns: d0 = 2 complex of one row pair (4 reals), d1 = m % NB, d2 = row pair A, d3 = m / NB
+        const cuuint64_t gdim[4] = {4, NB, L / 2, L / (2 * NB)};
+        const cuuint64_t gstride[3] = {4 * w, 4 * NB * w, (L / 2) * 4 * NB * w};
+        const cuuint32_t box[4] = {4u, 1u, (cuuint32_t)h->tab->v2_abox, 1u};
+        const cuuint32_t estr[4] = {1u, 1u, 1u, 1u};
+        CUresult r = enc(&h->tmap_col, dtp, 4, base, gdim, gstride, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                         CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r != CUDA_SUCCESS) { h->err = "cuTensorMapEncodeTiled (columns) failed (code " + std::to_string((int)r) + ")"; return FCG_CUDA_ERROR; }
+    }
     h->have_tmap = true;
     return FCG_OK;
 }
@@ -417,6 +435,8 @@ int fcg_create(int L, fcg_dtype dt, void* workspace, void* cuda_stream, fcg_hand
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) { cudaGetLastError(); return FCG_CUDA_ERROR; }
     fcg_handle h = new fcg_handle_s();
+    { int dev = 0, n = 0;
+      if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && n > 0) h->nsm = n; }
     h->L = L; h->dtype = dt; h->w = dt == FCG_F64 ? 8 : 4; h->N = (size_t)L * L;
     h->tab = get_table(L, dt);
     h->stream = (cudaStream_t)cuda_stream;
@@ -464,14 +484,19 @@ int fcg_set_option(fcg_handle h, int option, int value) {
         case FCG_OPT_ROW_VARIANT:
             if (value >= FCG_NROWVAR || (value >= 0 && !h->tab->row_valid[value])) return fail(h, FCG_INVALID_ARG, "row variant not available for this size");
             h->row_var_opt = value; return FCG_OK;
-        case FCG_OPT_ENGINE: if (value != 0 && value != 1) return fail(h, FCG_INVALID_ARG, "engine must be 0 or 1"); h->engine_opt = value; return FCG_OK;
+        case FCG_OPT_ENGINE:
+            if (value != 0 && value != 1) return fail(h, FCG_INVALID_ARG, "engine must be 0 or 1");
+            h->engine_opt = value;
+            if (h->have_spectrum && h->spectrum_colpos != (h->v2() ? 1 : 0)) h->have_spectrum = false;   // stored layout belongs to the other engine
+            return FCG_OK;
     }
     return fail(h, FCG_INVALID_ARG, "unknown option");
 }
 
 int fcg_set_spectrum(fcg_handle h, const void* s) {
     if (!h || !s) return fail(h, FCG_INVALID_ARG, "null argument");
-    FCG_CK(h, h->tab->spectrum_prep(s, h->at<void>(h->lay.shat), h->stream));
+    h->spectrum_colpos = h->v2() ? 1 : 0;
+    FCG_CK(h, h->tab->spectrum_prep(s, h->at<void>(h->lay.shat), h->spectrum_colpos, h->stream));
     FCG_CK(h, cudaStreamSynchronize(h->stream));      // the caller's array is not referenced after return
     h->have_spectrum = true;
     return FCG_OK;

@@ -34,22 +34,35 @@ template <typename T, typename P> struct AsyncShape {
     static constexpr size_t WBYTES = (size_t)L * 2 * sizeof(T);              // one complex transform
     static constexpr uint32_t PIECE = (uint32_t)(Q1 * sizeof(T));            // one stage-1 strip of one real row
     static constexpr int MAXSLOT = 8;
-    // P3: ring beside the work buffer; first holds two tiles of T (TSUB frequencies each), then strips of k, p (, f)
-    static constexpr size_t RB = WBYTES > 32768 ? 32768 : WBYTES;
-    static constexpr int TSUB = (int)(RB / 2 / (2 * 2 * sizeof(T)));
-    static constexpr int TBOX = TSUB < 256 ? TSUB : 256;                     // frequencies per tensor-map box
+    // P3: beside the work buffer, two tiles of T (TSB bytes = TSUB frequencies x 2 rows each) and a ring of KRB bytes
+    // for strips of k, p (, f); both run ahead across transforms
+    static constexpr size_t TSB = WBYTES >= 16384 ? 8192 : WBYTES / 2;
+    static constexpr size_t KRB = 8 * (size_t)PIECE > 24576 ? 8 * (size_t)PIECE : 24576;
+    static constexpr int TSUB = (int)(TSB / (2 * 2 * sizeof(T)));            // columns per tile of T
     static constexpr int NSUB = (L / 2) / TSUB;
-    static constexpr size_t fwd_smem = WBYTES + 128;                          // + 128: the kernels align the dynamic base themselves
+    // Layout of T for these passes: columns are numbered by their POSITION in the digit-reversed row
+    // spectrum, m = 0 .. L/2-1 <-> position e(m) = (m / HR) RLAST + m % HR <-> frequency n = freq_of(e(m)) < L/2, and
+    // NB consecutive columns x one row pair form one 128-byte line:  T2[m / NB][A][m % NB][r],  a = 2A + r.
+    static constexpr int NB = 128 / (4 * (int)sizeof(T));
+    static constexpr int HR = P::RLAST / 2;
+    static constexpr int ABOX = L / 2 < 256 ? L / 2 : 256;                   // row pairs per box of the column tensor map
+    static FCG_HD int pos_of_col(int m) { return (m / HR) * P::RLAST + m % HR; }
+    static FCG_HD int col_of_pos(int e) { return (e / P::RLAST) * HR + e % P::RLAST; }
+    static FCG_HD size_t t2_index(int m, int A) { return (((size_t)(m / NB) * (L / 2) + A) * NB + m % NB) * 2; }   // complex units, r = 0
+    // P1: ring of NFS strips (6 pieces each) beside the work buffer, running ahead across transforms
+    static constexpr uint32_t FSLOTB = 6 * PIECE;
+    static constexpr int NFS = 32768 / FSLOTB < 2 ? 2 : (32768 / FSLOTB > MAXSLOT ? MAXSLOT : (int)(32768 / FSLOTB));
+    static constexpr size_t fwd_smem = WBYTES + (size_t)NFS * FSLOTB + 128;   // + 128: the kernels align the dynamic base themselves
     static constexpr size_t col_smem = WBYTES + (size_t)L * sizeof(T) + 128;
-    static constexpr size_t inv_smem = WBYTES + RB + 128;
-    static constexpr int thread_cap = sizeof(T) == 8 ? 512 : 1024;           // 128 / 64 registers per thread
+    static constexpr size_t inv_smem = WBYTES + 2 * TSB + KRB + 128;
+    static constexpr int thread_cap = sizeof(T) == 8 ? 608 : 1152;           // ~104-128 / ~56-64 registers per thread
     static constexpr int ctas(size_t smem) {
         const int by_smem = (int)((size_t)FCG_MAX_SMEM / (smem + 1024));
-        const int by_thr = thread_cap / NT > 1 ? thread_cap / NT : 1;
+        const int by_thr = thread_cap / (NT + 32) > 1 ? thread_cap / (NT + 32) : 1;
         return by_smem < 1 ? 1 : (by_smem < by_thr ? by_smem : by_thr);
     }
-    static_assert(!valid || (WBYTES >= 6 * (size_t)PIECE && RB >= 6 * (size_t)PIECE), "ring too small for one strip");
-    static_assert(!valid || (TSUB % TBOX == 0 && (L / 2) % TSUB == 0 && NSUB >= 2 && NSUB % 2 == 0 && NT % 32 == 0), "tile shape");
+    static_assert(!valid || KRB >= 6 * (size_t)PIECE, "ring too small for one strip");
+    static_assert(!valid || (TSUB % NB == 0 && TSUB / NB <= 256 && (L / 2) % TSUB == 0 && NSUB >= 2 && NT % 32 == 0), "tile shape");
 };
 
 #ifdef __CUDACC__
@@ -63,6 +76,9 @@ template <> __device__ __forceinline__ void store_pair<float>(float2* dst, float
     *reinterpret_cast<float4*>(dst) = make_float4(a.x, a.y, b.x, b.y);
 }
 
+// CTA barrier among the first N threads only (the consumers of a warp-specialised kernel); barrier 0 stays __syncthreads
+template <int N> __device__ __forceinline__ void bar_named() { asm volatile("bar.sync 1, %0;" ::"n"(N) : "memory"); }
+
 template <typename P> constexpr int per_max() {
     int m = 1;
     for (int s = 1; s <= P::S; ++s) { const int per = (P::N / P::radix(s)) / P::NT; if (per > m) m = per; }
@@ -71,122 +87,141 @@ template <typename P> constexpr int per_max() {
 
 // --------------------------------------------------------------------------------------------- P1
 //   [u += alpha p;  p = r + beta p;]   T[n][a0], T[n][a0+1] = row transforms of rows a0, a0+1 of p (or x)
+// Persistent: grid = nsm x CTAS; the CTAs that share an SM (blockIdx % nsm, the usual placement) take the row pairs
+// s, s+nsm, s+2nsm, .. in turn, so every SM gets floor or ceil of (L/2)/nsm transforms.
+// Warp-specialised: NT consumer threads + one producer warp that only issues the strip copies, so the ring runs
+// ahead across transforms (while one transform is in its butterfly stages the next one's strips are landing) and
+// no consumer ever spends issue slots on address arithmetic for TMA.
 template <typename T, typename P, int CTAS>
-__global__ void __launch_bounds__(P::NT, CTAS) row_fwd2_kernel(const RowFwdArgs<T> A)
+__global__ void __launch_bounds__(P::NT + 32, CTAS) row_fwd2_kernel(const RowFwdArgs<T> A)
 {
     using AS = AsyncShape<T, P>;
     constexpr int L = P::N, S = P::S, NT = P::NT, R1 = AS::R1, Q1 = AS::Q1, PER1 = AS::PER1, PM = per_max<P>();
     constexpr uint32_t PIECE = AS::PIECE;
+    constexpr int NSLOT = AS::NFS;
+    constexpr uint32_t SLOTB = AS::FSLOTB;
     extern __shared__ unsigned char smem_dyn[];
     unsigned char* const smem_raw = align128(smem_dyn);
+    unsigned char* const ring = smem_raw + AS::WBYTES;
     __shared__ __align__(8) uint64_t full[AS::MAXSLOT];
     __shared__ __align__(8) uint64_t empty[AS::MAXSLOT];
     cx<T>* W = reinterpret_cast<cx<T>*>(smem_raw);
     SmemIO<T, P> io{W};
     const int lt = threadIdx.x, lane = lt & 31, warp = lt >> 5;
-    const int a0 = 2 * (int)blockIdx.x;
-    const size_t row0 = (size_t)a0 * L;
-    const bool cg = A.mode == ROWF_CG;
+    const bool cg = (A.mode & 0xff) == ROWF_CG;
+    const int dbg = A.mode >> 8;
+    if (cg && A.sc->done) return;                                 // converged: nothing may change
     const int nv = cg ? 6 : 2;
-    int nslot = (int)(AS::WBYTES / (nv * PIECE));
-    nslot = nslot > AS::MAXSLOT ? AS::MAXSLOT : nslot;
-    nslot = nslot > R1 ? R1 : nslot;
 
-    // strip t of the two rows: elements [t Q1, (t+1) Q1) of p0 p1 r0 r1 u0 u1 (or x0 x1); called by all of warp 0
-    auto issue = [&](int t) {
-        const int slot = t % nslot;
-        if (lane == 0) tma::mbar_expect_tx(&full[slot], nv * PIECE);
-        __syncwarp();
-        if (lane < nv) {
-            const T* src = cg ? (lane < 2 ? A.p : lane < 4 ? A.r : A.u) : A.x;
-            src += row0 + (size_t)(lane & 1) * L + (size_t)t * Q1;
-            tma::bulk_g2s(smem_raw + (size_t)slot * nv * PIECE + (size_t)lane * PIECE, src, PIECE, &full[slot]);
-        }
-    };
+    // my transforms: tile(i) = grp + nsm * (j + i * k)
+    const int nsm = A.nsm < (int)gridDim.x ? A.nsm : (int)gridDim.x, grp = (int)blockIdx.x % nsm, jj = (int)blockIdx.x / nsm,
+              kk = (int)gridDim.x / nsm;
+    auto tile_of = [&](int i) { return grp + nsm * (jj + i * kk); };
+    int ntl = 0;
+    while (tile_of(ntl) < L / 2) ++ntl;
+    const int G = ntl * R1;                                       // strips this CTA will consume
+
     if (lt == 0) {
-        for (int i = 0; i < AS::MAXSLOT; ++i) { tma::mbar_init(&full[i], 1); tma::mbar_init(&empty[i], NT / 32); }
+        for (int i = 0; i < NSLOT; ++i) { tma::mbar_init(&full[i], 1); tma::mbar_init(&empty[i], NT / 32); }
         tma::fence_mbar_init();
     }
     __syncthreads();
-    if (warp == 0)
-        for (int t = 0; t < nslot; ++t) issue(t);
 
-    T alpha = (T)0, beta = (T)0;
-    bool done = false;
-    if (cg) { done = A.sc->done != 0; alpha = (T)A.sc->alpha; beta = (T)A.sc->beta; }
-    cx<T> wb[S + 1][PM];
-    static_for_up<1, S - 1>([&](auto s) { base_tw<P, decltype(s)::value, T>(lt, A.tw, wb[decltype(s)::value]); });
-
-    if (done) {      // converged: nothing may change; drain the copies already issued and leave
-        for (int t = 0; t < nslot; ++t) tma::mbar_wait(&full[t], 0);
+    if (warp == NT / 32) {
+        // ---- producer warp: strip g = (transform g / R1, strip g % R1) = elements [t Q1, (t+1) Q1) of
+        //      p0 p1 r0 r1 u0 u1 (or x0 x1), one bulk copy per lane < nv, into slot g % NSLOT
+        const T* base = cg ? (lane < 2 ? A.p : lane < 4 ? A.r : A.u) : A.x;
+        base += (size_t)(lane & 1) * L;
+        unsigned char* dst = ring + (size_t)lane * PIECE;
+        int slot = 0;
+        uint32_t phase = 0;
+        for (int g = 0; g < G; ++g) {
+            if (g >= NSLOT) tma::mbar_wait(&empty[slot], phase ^ 1u);          // the slot's previous strip has been read by every warp
+            if (lane == 0) tma::mbar_expect_tx(&full[slot], nv * PIECE);
+            __syncwarp();
+            if (lane < nv)
+                tma::bulk_g2s(dst + (size_t)slot * SLOTB, base + (size_t)(2 * tile_of(g / R1)) * L + (size_t)(g % R1) * Q1, PIECE, &full[slot]);
+            if (++slot == NSLOT) { slot = 0; phase ^= 1u; }
+        }
         return;
     }
 
-    // phase A: strips stream through the ring; vector update on the fly; z = p_even + i p_odd
-    cx<T> z[PER1][R1];
+    // ---- consumers
+    T alpha = (T)0, beta = (T)0;
+    if (cg) { alpha = (T)A.sc->alpha; beta = (T)A.sc->beta; }
+    cx<T> wb[S + 1][PM];
+    static_for_up<1, S - 1>([&](auto s) { base_tw<P, decltype(s)::value, T>(lt, A.tw, wb[decltype(s)::value]); });
+
+    int slot = 0;
+    uint32_t phase = 0;
+    for (int i = 0; i < ntl; ++i) {
+        const int a0 = 2 * tile_of(i);
+        const size_t row0 = (size_t)a0 * L;
+        // phase A: strips stream through the ring; vector update on the fly; z = p_even + i p_odd
+        cx<T> z[PER1][R1];
 #pragma unroll
-    for (int t = 0; t < R1; ++t) {
-        const int slot = t % nslot;
-        tma::mbar_wait(&full[slot], (uint32_t)((t / nslot) & 1));
-        const T* sl = reinterpret_cast<const T*>(smem_raw + (size_t)slot * nv * PIECE);
+        for (int t = 0; t < R1; ++t) {
+            tma::mbar_wait(&full[slot], phase);
+            const T* sl = reinterpret_cast<const T*>(ring + (size_t)slot * SLOTB);
 #pragma unroll
-        for (int i = 0; i < PER1; ++i) {
-            const int j = lt + i * NT;
-            if (cg) {
-                T p0 = sl[j], p1 = sl[Q1 + j];
-                const T r0 = sl[2 * Q1 + j], r1 = sl[3 * Q1 + j];
-                T u0 = sl[4 * Q1 + j], u1 = sl[5 * Q1 + j];
-                u0 = u0 + alpha * p0; u1 = u1 + alpha * p1;       // new x, lagged one pass
-                p0 = r0 + beta * p0;  p1 = r1 + beta * p1;        // new direction
-                const size_t i0 = row0 + (size_t)t * Q1 + j;
-                A.u[i0] = u0; A.u[i0 + L] = u1;
-                A.p[i0] = p0; A.p[i0 + L] = p1;
-                z[i][t] = mk<T>(p0, p1);
-            } else {
-                z[i][t] = mk<T>(sl[j], sl[Q1 + j]);
+            for (int q = 0; q < PER1; ++q) {
+                const int j = lt + q * NT;
+                if (cg) {
+                    T p0 = sl[j], p1 = sl[Q1 + j];
+                    const T r0 = sl[2 * Q1 + j], r1 = sl[3 * Q1 + j];
+                    T u0 = sl[4 * Q1 + j], u1 = sl[5 * Q1 + j];
+                    u0 = u0 + alpha * p0; u1 = u1 + alpha * p1;       // new x, lagged one pass
+                    p0 = r0 + beta * p0;  p1 = r1 + beta * p1;        // new direction
+                    const size_t i0 = row0 + (size_t)t * Q1 + j;
+                    if (!(dbg & 2)) { A.u[i0] = u0; A.u[i0 + L] = u1;
+                    A.p[i0] = p0; A.p[i0 + L] = p1; }
+                    z[q][t] = mk<T>(p0, p1);
+                } else {
+                    z[q][t] = mk<T>(sl[j], sl[Q1 + j]);
+                }
             }
+            if (i * R1 + t + NSLOT < G) tma::mbar_warp_release(&empty[slot]);   // this warp has read the slot
+            if (++slot == NSLOT) { slot = 0; phase ^= 1u; }
         }
-        if (t + nslot < R1) {
-            tma::mbar_warp_release(&empty[slot]);                  // this warp has read the slot
-            if (warp == 0) {
-                tma::mbar_wait(&empty[slot], (uint32_t)((t / nslot) & 1));     // ... and so has every other warp
-                issue(t + nslot);
-            }
-        }
-    }
-    __syncthreads();                                              // ring (inside W) fully consumed
-    stage_math<P, 1, -1, T>(z, wb[1]);
-    stage_st<P, 1, T>(lt, [&](int e, cx<T> v) { io.st(e, v); }, z);
-    __syncthreads();
-    static_for_up<2, S>([&](auto s) {
-        constexpr int sv = decltype(s)::value;
-        cx<T> a[St<P, sv>::PER][St<P, sv>::R];
-        stage_ld<P, sv, T>(lt, [&](int e) { return io.ld(e); }, a);
-        stage_math<P, sv, -1, T>(a, wb[sv]);
-        stage_st<P, sv, T>(lt, [&](int e, cx<T> v) { io.st(e, v); }, a);
-        __syncthreads();
-    });
-    // separate the two rows and store transposed: T[n][a0] = X_even[n], T[n][a0+1] = X_odd[n]
-    const T h = (T)0.5;
+        if (dbg & 4) { if (z[0][0].x == (T)123.456) A.Tb[0] = z[0][1]; continue; }
+        bar_named<NT>();                                          // the previous transform's separation has left W
+        stage_math<P, 1, -1, T>(z, wb[1]);
+        stage_st<P, 1, T>(lt, [&](int e, cx<T> v) { io.st(e, v); }, z);
+        bar_named<NT>();
+        static_for_up<2, S>([&](auto s) {
+            constexpr int sv = decltype(s)::value;
+            cx<T> a[St<P, sv>::PER][St<P, sv>::R];
+            stage_ld<P, sv, T>(lt, [&](int e) { return io.ld(e); }, a);
+            stage_math<P, sv, -1, T>(a, wb[sv]);
+            stage_st<P, sv, T>(lt, [&](int e, cx<T> v) { io.st(e, v); }, a);
+            bar_named<NT>();
+        });
+        // Separate the two rows and store them as column m of T2 (X_even[n], X_odd[n] side by side).  Consecutive
+        // threads take consecutive POSITIONS e of the digit-reversed spectrum (n = freq_of(e), n < L/2 <=> the last
+        // digit e % RLAST is in its lower half), so the reads of Z[n] and of its mirror Z[L-n] are contiguous runs.
+        const T h = (T)0.5;
 #pragma unroll 4
-    for (int n = lt; n < L / 2; n += NT) {
-        cx<T> X0, X1;
-        if (n == 0) {
-            const cx<T> Z0 = io.ld(P::pos_of(0)), ZN = io.ld(P::pos_of(L / 2));
-            X0 = mk<T>(Z0.x, ZN.x); X1 = mk<T>(Z0.y, ZN.y);
-        } else {
-            const cx<T> Za = io.ld(P::pos_of(n)), Zb = io.ld(P::pos_of(L - n));
-            X0 = mk<T>((Za.x + Zb.x) * h, (Za.y - Zb.y) * h);
-            X1 = mk<T>((Za.y + Zb.y) * h, (Zb.x - Za.x) * h);
+        for (int m = lt; m < L / 2; m += NT) {
+            const int e = AS::pos_of_col(m);
+            const int n = P::freq_of(e);
+            cx<T> X0, X1;
+            if (n == 0) {
+                const cx<T> Z0 = io.ld(P::pos_of(0)), ZN = io.ld(P::pos_of(L / 2));
+                X0 = mk<T>(Z0.x, ZN.x); X1 = mk<T>(Z0.y, ZN.y);
+            } else {
+                const cx<T> Za = io.ld(e), Zb = io.ld(P::pos_of(L - n));
+                X0 = mk<T>((Za.x + Zb.x) * h, (Za.y - Zb.y) * h);
+                X1 = mk<T>((Za.y + Zb.y) * h, (Zb.x - Za.x) * h);
+            }
+            if (!(dbg & 1) || X0.x == (T)123.456) store_pair<T>(A.Tb + AS::t2_index(m, a0 >> 1), X0, X1);
         }
-        store_pair<T>(A.Tb + (size_t)n * L + a0, X0, X1);
     }
 }
 
 // --------------------------------------------------------------------------------------------- P2
-//   column n of T, in place:  T[n][.] <- F^H ( shat[n][.] o F T[n][.] )
+//   column m of T2, in place:  T2[m][.] <- F^H ( shat[m][.] o F T2[m][.] )
 template <typename T, typename P, int CTAS>
-__global__ void __launch_bounds__(P::NT, CTAS) col2_kernel(const ColArgs<T> A)
+__global__ void __launch_bounds__(P::NT, CTAS) col2_kernel(const ColArgs<T> A, const __grid_constant__ CUtensorMap tmap)
 {
     using AS = AsyncShape<T, P>;
     constexpr int L = P::N, S = P::S, NT = P::NT, PM = per_max<P>();
@@ -196,14 +231,20 @@ __global__ void __launch_bounds__(P::NT, CTAS) col2_kernel(const ColArgs<T> A)
     cx<T>* W = reinterpret_cast<cx<T>*>(smem_raw);
     T* sh = reinterpret_cast<T*>(smem_raw + AS::WBYTES);
     SmemIO<T, P> io{W};
+    // column m of T2 (frequency freq_of(pos_of_col(m)); m = 0 is the packed n = 0 / L/2 column): 2 complex per row pair,
+    // gathered by TMA into natural row order a = 2A + r, and scattered back the same way at the end
     const int lt = threadIdx.x, n = (int)blockIdx.x;
-    cx<T>* col = A.Tb + (size_t)n * L;
+    constexpr int ABOX = AS::ABOX;
+    constexpr uint32_t BOXB = (uint32_t)(ABOX * 2 * sizeof(cx<T>));
     if (lt == 0) {
+        tma::prefetch_tmap(&tmap);
         tma::mbar_init(&bar, 1);
         tma::mbar_init(&ready, NT / 32);
         tma::fence_mbar_init();
         tma::mbar_expect_tx(&bar, (uint32_t)(AS::WBYTES + (n ? L * sizeof(T) : 0)));
-        tma::bulk_g2s(W, col, (uint32_t)AS::WBYTES, &bar);
+#pragma unroll
+        for (int b = 0; b < (L / 2) / ABOX; ++b)
+            tma::tensor_g2s_4d(smem_raw + (size_t)b * BOXB, &tmap, 0, n % AS::NB, b * ABOX, n / AS::NB, &bar);
         if (n) tma::bulk_g2s(sh, A.shat + (size_t)n * L, (uint32_t)(L * sizeof(T)), &bar);
     }
     __syncthreads();
@@ -275,7 +316,9 @@ __global__ void __launch_bounds__(P::NT, CTAS) col2_kernel(const ColArgs<T> A)
     tma::mbar_warp_arrive(&ready);
     if (lt == 0) {
         tma::mbar_wait(&ready, 0);            // every warp's part of the column is in place
-        tma::bulk_s2g(col, W, (uint32_t)AS::WBYTES);
+#pragma unroll
+        for (int b = 0; b < (L / 2) / ABOX; ++b)
+            tma::tensor_s2g_4d(&tmap, 0, n % AS::NB, b * ABOX, n / AS::NB, smem_raw + (size_t)b * BOXB);
         tma::bulk_commit();
         tma::bulk_wait_read0();          // shared memory must outlive the store's read
     }
@@ -283,47 +326,53 @@ __global__ void __launch_bounds__(P::NT, CTAS) col2_kernel(const ColArgs<T> A)
 
 // --------------------------------------------------------------------------------------------- P3
 //   c = F_row^H T (rows a0, a0+1);  q = k o p + c  [+ partial p.q]   (or residual / apply / plain)
+// Persistent like P1.  Two rings run ahead across transforms: tiles of T (TSUB frequencies x 2 rows, TMA tensor
+// loads of whole 128-byte lines of T2) feeding the rebuild of the packed spectrum, and strips of k, p (, f) feeding
+// the epilogue.
 template <typename T, typename P, int CTAS>
 __global__ void __launch_bounds__(P::NT, CTAS) row_inv2_kernel(const RowInvArgs<T> A, const __grid_constant__ CUtensorMap tmap)
 {
     using AS = AsyncShape<T, P>;
     constexpr int L = P::N, S = P::S, NT = P::NT, R1 = AS::R1, Q1 = AS::Q1, PER1 = AS::PER1, PM = per_max<P>();
     constexpr uint32_t PIECE = AS::PIECE;
-    constexpr int TSUB = AS::TSUB, NSUB = AS::NSUB, TBOX = AS::TBOX;
-    constexpr uint32_t TBYTES = (uint32_t)(TSUB * 2 * sizeof(cx<T>));
+    constexpr int TSUB = AS::TSUB, NSUB = AS::NSUB;
+    constexpr uint32_t TBYTES = (uint32_t)AS::TSB;
     extern __shared__ unsigned char smem_dyn[];
     unsigned char* const smem_raw = align128(smem_dyn);
     __shared__ __align__(8) uint64_t tfull[2], tempty[2];
     __shared__ __align__(8) uint64_t kfull[AS::MAXSLOT], kempty[AS::MAXSLOT];
     __shared__ double red[2 * 32];
     cx<T>* W = reinterpret_cast<cx<T>*>(smem_raw);
-    unsigned char* ring = smem_raw + AS::WBYTES;
+    unsigned char* const tring = smem_raw + AS::WBYTES;
+    unsigned char* const kring = tring + 2 * AS::TSB;
     SmemIO<T, P> io{W};
     const int lt = threadIdx.x, lane = lt & 31, warp = lt >> 5;
-    const int a0 = 2 * (int)blockIdx.x;
-    const size_t row0 = (size_t)a0 * L;
-    const int mode = A.mode;
-    const int nv = mode == ROWI_PLAIN ? 0 : (mode == ROWI_RESID ? 6 : 4);
-    int nks = nv ? (int)(AS::RB / (nv * PIECE)) : 1;
+    const int mode = A.mode & 0xff;
+    const int dbg = A.mode >> 8;
+    if (mode == ROWI_CG && A.sc->done) return;
+    const int nv = (mode == ROWI_PLAIN || (dbg & 4)) ? 0 : (mode == ROWI_RESID ? 6 : 4);
+    int nks = nv ? (int)(AS::KRB / (nv * PIECE)) : 1;
     nks = nks > AS::MAXSLOT ? AS::MAXSLOT : nks;
-    nks = nks > R1 ? R1 : nks;
+    const uint32_t kslotb = nv * PIECE;
 
-    auto issue_T = [&](int sub) {        // thread 0: TSUB frequencies x (a0, a0+1) of T, as TSUB/TBOX boxes
-        const int slot = sub & 1;
+    const int nsm = A.nsm < (int)gridDim.x ? A.nsm : (int)gridDim.x, grp = (int)blockIdx.x % nsm, jj = (int)blockIdx.x / nsm, kk = (int)gridDim.x / nsm;
+    auto tile_of = [&](int i) { return grp + nsm * (jj + i * kk); };
+    int ntl = 0;
+    while (tile_of(ntl) < L / 2) ++ntl;
+    const int GT = ntl * NSUB, GK = nv ? ntl * R1 : 0;
+
+    auto issue_T = [&](int gs) {         // thread 0: tile gs = (transform gs / NSUB, part gs % NSUB): TSUB columns x 2 rows of T2, 128-byte lines
+        const int slot = gs & 1;
         tma::mbar_expect_tx(&tfull[slot], TBYTES);
-#pragma unroll
-        for (int b = 0; b < TSUB / TBOX; ++b)
-            tma::tensor_g2s_2d(ring + (size_t)slot * TBYTES + (size_t)b * TBOX * 2 * sizeof(cx<T>), &tmap, 2 * a0, sub * TSUB + b * TBOX,
-                               &tfull[slot]);
+        tma::tensor_g2s_3d(tring + (size_t)slot * TBYTES, &tmap, 0, tile_of(gs / NSUB), (gs % NSUB) * (TSUB / AS::NB), &tfull[slot]);
     };
-    auto issue_K = [&](int t) {          // all of warp 0: strip t of k0 k1 v0 v1 (f0 f1)
-        const int slot = t % nks;
-        if (lane == 0) tma::mbar_expect_tx(&kfull[slot], nv * PIECE);
+    auto issue_K = [&](int g, int slot) {          // all of warp 0: strip g % R1 of k0 k1 v0 v1 (f0 f1) of transform g / R1
+        if (lane == 0) tma::mbar_expect_tx(&kfull[slot], kslotb);
         __syncwarp();
         if (lane < nv) {
             const T* src = lane < 2 ? A.k : lane < 4 ? A.v : A.f;
-            src += row0 + (size_t)(lane & 1) * L + (size_t)t * Q1;
-            tma::bulk_g2s(ring + (size_t)slot * nv * PIECE + (size_t)lane * PIECE, src, PIECE, &kfull[slot]);
+            src += (size_t)(2 * tile_of(g / R1) + (lane & 1)) * L + (size_t)(g % R1) * Q1;
+            tma::bulk_g2s(kring + (size_t)slot * kslotb + (size_t)lane * PIECE, src, PIECE, &kfull[slot]);
         }
     };
     if (lt == 0) {
@@ -332,89 +381,99 @@ __global__ void __launch_bounds__(P::NT, CTAS) row_inv2_kernel(const RowInvArgs<
         tma::mbar_init(&tempty[0], NT / 32); tma::mbar_init(&tempty[1], NT / 32);
         for (int i = 0; i < AS::MAXSLOT; ++i) { tma::mbar_init(&kfull[i], 1); tma::mbar_init(&kempty[i], NT / 32); }
         tma::fence_mbar_init();
-        issue_T(0); issue_T(1);
+        if (GT > 0) issue_T(0);
+        if (GT > 1) issue_T(1);
     }
     __syncthreads();
-    const bool done = mode == ROWI_CG && A.sc->done;
+    if (warp == 0)
+        for (int g = 0; g < nks && g < GK; ++g) issue_K(g, g);
     cx<T> wb[S + 1][PM];
     static_for_up<1, S - 1>([&](auto s) { base_tw<P, decltype(s)::value, T>(lt, A.tw, wb[decltype(s)::value]); });
-    if (done) { tma::mbar_wait(&tfull[0], 0); tma::mbar_wait(&tfull[1], 0); return; }
 
-    // rebuild the packed spectrum Z = X_even + i X_odd at its digit-reversed place, tile by tile
-    for (int sub = 0; sub < NSUB; ++sub) {
-        tma::mbar_wait(&tfull[sub & 1], (uint32_t)((sub >> 1) & 1));
-        const cx<T>* Ts = reinterpret_cast<const cx<T>*>(ring + (size_t)(sub & 1) * TBYTES);
-#pragma unroll 4
-        for (int nl = lt; nl < TSUB; nl += NT) {
-            const int n = sub * TSUB + nl;
-            const cx<T> X0 = Ts[2 * nl], X1 = Ts[2 * nl + 1];
-            if (n == 0) {
-                io.st(P::pos_of(0), mk<T>(X0.x, X1.x));
-                io.st(P::pos_of(L / 2), mk<T>(X0.y, X1.y));
-            } else {
-                io.st(P::pos_of(n), mk<T>(X0.x - X1.y, X0.y + X1.x));
-                io.st(P::pos_of(L - n), mk<T>(X0.x + X1.y, X1.x - X0.y));
-            }
-        }
-        tma::mbar_warp_release(&tempty[sub & 1]);                  // this warp has read the tile
-        if (lt == 0 && sub + 2 < NSUB) {
-            tma::mbar_wait(&tempty[sub & 1], (uint32_t)((sub >> 1) & 1));
-            issue_T(sub + 2);
-        }
-    }
-    __syncthreads();                                              // Z complete in W
-    // once every warp is done with the tiles the ring is free: start streaming the strips of k, p (, f) for the epilogue
-    if (warp == 0 && nv) {
-        constexpr uint32_t fin = (uint32_t)((NSUB / 2 - 1) & 1);
-        tma::mbar_wait(&tempty[0], fin); tma::mbar_wait(&tempty[1], fin);
-        for (int t = 0; t < nks; ++t) issue_K(t);
-    }
-
-    static_for_down<S, 2>([&](auto s) {
-        constexpr int sv = decltype(s)::value;
-        cx<T> a[St<P, sv>::PER][St<P, sv>::R];
-        stage_ld<P, sv, T>(lt, [&](int e) { return io.ld(e); }, a);
-        stage_math<P, sv, +1, T>(a, wb[sv]);
-        stage_st<P, sv, T>(lt, [&](int e, cx<T> v) { io.st(e, v); }, a);
-        __syncthreads();
-    });
-    // inverse stage 1 straight into the epilogue: natural order, re = even row, im = odd row
-    cx<T> c[PER1][R1];
-    stage_ld<P, 1, T>(lt, [&](int e) { return io.ld(e); }, c);
-    stage_math<P, 1, +1, T>(c, wb[1]);
     double acc[2] = {0.0, 0.0};
-#pragma unroll
-    for (int t = 0; t < R1; ++t) {
-        const T* sl = nullptr;
-        if (nv) {
-            const int slot = t % nks;
-            tma::mbar_wait(&kfull[slot], (uint32_t)((t / nks) & 1));
-            sl = reinterpret_cast<const T*>(ring + (size_t)slot * nv * PIECE);
-        }
-#pragma unroll
-        for (int i = 0; i < PER1; ++i) {
-            const int j = lt + i * NT;
-            const size_t i0 = row0 + (size_t)t * Q1 + j;
-            const T c0 = c[i][t].x, c1 = c[i][t].y;
-            if (mode == ROWI_PLAIN) { A.out[i0] = c0 * A.scale; A.out[i0 + L] = c1 * A.scale; continue; }
-            const T v0 = sl[2 * Q1 + j], v1 = sl[3 * Q1 + j];
-            const T val0 = sl[j] * v0 + c0, val1 = sl[Q1 + j] * v1 + c1;         // k o x + C x
-            if (mode == ROWI_RESID) {
-                const T f0 = sl[4 * Q1 + j], f1 = sl[5 * Q1 + j];
-                const T r0 = f0 - val0, r1 = f1 - val1;                           // r = f - A u
-                A.out[i0] = r0; A.out[i0 + L] = r1; A.out2[i0] = (T)0; A.out2[i0 + L] = (T)0;
-                acc[0] += (double)r0 * (double)r0; acc[0] += (double)r1 * (double)r1;
-                acc[1] += (double)f0 * (double)f0; acc[1] += (double)f1 * (double)f1;
-            } else {
-                A.out[i0] = val0; A.out[i0 + L] = val1;
-                acc[0] += (double)v0 * (double)val0; acc[0] += (double)v1 * (double)val1;   // search length p.Ap
+    int kslot = 0;
+    uint32_t kphase = 0;
+    for (int i = 0; i < ntl; ++i) {
+        const int a0 = 2 * tile_of(i);
+        const size_t row0 = (size_t)a0 * L;
+        // rebuild the packed spectrum Z = X_even + i X_odd at its digit-reversed place, tile by tile
+        for (int sub = 0; sub < NSUB; ++sub) {
+            const int gs = i * NSUB + sub, ts = gs & 1;
+            const uint32_t tph = (uint32_t)((gs >> 1) & 1);
+            tma::mbar_wait(&tfull[ts], tph);
+            const cx<T>* Ts = reinterpret_cast<const cx<T>*>(tring + (size_t)ts * TBYTES);
+#pragma unroll 4
+            for (int ml = lt; ml < TSUB; ml += NT) {
+                const int e = AS::pos_of_col(sub * TSUB + ml);
+                const int n = P::freq_of(e);
+                const cx<T> X0 = Ts[2 * ml], X1 = Ts[2 * ml + 1];
+                if (n == 0) {
+                    io.st(P::pos_of(0), mk<T>(X0.x, X1.x));
+                    io.st(P::pos_of(L / 2), mk<T>(X0.y, X1.y));
+                } else {
+                    io.st(e, mk<T>(X0.x - X1.y, X0.y + X1.x));
+                    io.st(P::pos_of(L - n), mk<T>(X0.x + X1.y, X1.x - X0.y));
+                }
+            }
+            if (gs + 2 < GT) {
+                tma::mbar_warp_release(&tempty[ts]);                  // this warp has read the tile
+                if (lt == 0) {
+                    tma::mbar_wait(&tempty[ts], tph);
+                    issue_T(gs + 2);
+                }
             }
         }
-        if (nv && t + nks < R1) {
-            tma::mbar_warp_release(&kempty[t % nks]);
-            if (warp == 0) {
-                tma::mbar_wait(&kempty[t % nks], (uint32_t)((t / nks) & 1));
-                issue_K(t + nks);
+        __syncthreads();                                              // Z complete in W
+        if (dbg & 2) { if (W[lt].x == (T)123.456) A.out[0] = W[1].x; continue; }
+        static_for_down<S, 2>([&](auto s) {
+            constexpr int sv = decltype(s)::value;
+            cx<T> a[St<P, sv>::PER][St<P, sv>::R];
+            stage_ld<P, sv, T>(lt, [&](int e) { return io.ld(e); }, a);
+            stage_math<P, sv, +1, T>(a, wb[sv]);
+            stage_st<P, sv, T>(lt, [&](int e, cx<T> v) { io.st(e, v); }, a);
+            __syncthreads();
+        });
+        // inverse stage 1 straight into the epilogue: natural order, re = even row, im = odd row
+        cx<T> c[PER1][R1];
+        stage_ld<P, 1, T>(lt, [&](int e) { return io.ld(e); }, c);
+        __syncthreads();                                              // W may now be rebuilt for the next transform
+        stage_math<P, 1, +1, T>(c, wb[1]);
+#pragma unroll
+        for (int t = 0; t < R1; ++t) {
+            const T* sl = nullptr;
+            if (nv) {
+                tma::mbar_wait(&kfull[kslot], kphase);
+                sl = reinterpret_cast<const T*>(kring + (size_t)kslot * kslotb);
+            }
+#pragma unroll
+            for (int q = 0; q < PER1; ++q) {
+                const int j = lt + q * NT;
+                const size_t i0 = row0 + (size_t)t * Q1 + j;
+                const T c0 = c[q][t].x, c1 = c[q][t].y;
+                if (mode == ROWI_PLAIN || (dbg & 4)) { if (!(dbg & 1)) { A.out[i0] = c0 * A.scale; A.out[i0 + L] = c1 * A.scale; } continue; }
+                const T v0 = sl[2 * Q1 + j], v1 = sl[3 * Q1 + j];
+                const T val0 = sl[j] * v0 + c0, val1 = sl[Q1 + j] * v1 + c1;         // k o x + C x
+                if (mode == ROWI_RESID) {
+                    const T f0 = sl[4 * Q1 + j], f1 = sl[5 * Q1 + j];
+                    const T r0 = f0 - val0, r1 = f1 - val1;                           // r = f - A u
+                    A.out[i0] = r0; A.out[i0 + L] = r1; A.out2[i0] = (T)0; A.out2[i0 + L] = (T)0;
+                    acc[0] += (double)r0 * (double)r0; acc[0] += (double)r1 * (double)r1;
+                    acc[1] += (double)f0 * (double)f0; acc[1] += (double)f1 * (double)f1;
+                } else {
+                    A.out[i0] = val0; A.out[i0 + L] = val1;
+                    acc[0] += (double)v0 * (double)val0; acc[0] += (double)v1 * (double)val1;   // search length p.Ap
+                }
+            }
+            if (nv) {
+                const int g = i * R1 + t;
+                if (g + nks < GK) {
+                    tma::mbar_warp_release(&kempty[kslot]);
+                    if (warp == 0) {
+                        tma::mbar_wait(&kempty[kslot], kphase);
+                        issue_K(g + nks, kslot);
+                    }
+                }
+                if (++kslot == nks) { kslot = 0; kphase ^= 1u; }
             }
         }
     }

@@ -48,24 +48,32 @@ template <typename T> struct Inst {
         }
         return prep(col_kernel<T, P, CS::COLS>, CS::smem);
     }
+    // persistent grid: CTAS CTAs on each of nsm SMs, but never more CTAs than transforms (whole multiples of nsm)
+    static int pgrid(int nsm, int ctas) {
+        int k = ctas;
+        while (k > 1 && nsm * k > L / 2) --k;
+        return nsm * k > L / 2 ? L / 2 : nsm * k;
+    }
     static cudaError_t row_fwd2(const void* args, cudaStream_t st) {
         if constexpr (V2) {
-            row_fwd2_kernel<T, P, C_FWD><<<L / 2, P::NT, AS::fwd_smem, st>>>(*static_cast<const RowFwdArgs<T>*>(args));
+            const RowFwdArgs<T>& A = *static_cast<const RowFwdArgs<T>*>(args);
+            row_fwd2_kernel<T, P, C_FWD><<<pgrid(A.nsm, C_FWD), P::NT + 32, AS::fwd_smem, st>>>(A);
             return cudaGetLastError();
         }
         return cudaErrorInvalidValue;
     }
-    static cudaError_t col2(const void* args, cudaStream_t st) {
+    static cudaError_t col2(const void* args, const void* tensor_map, cudaStream_t st) {
         if constexpr (V2) {
-            col2_kernel<T, P, C_COL><<<L / 2, P::NT, AS::col_smem, st>>>(*static_cast<const ColArgs<T>*>(args));
+            col2_kernel<T, P, C_COL><<<L / 2, P::NT, AS::col_smem, st>>>(*static_cast<const ColArgs<T>*>(args),
+                                                                         *static_cast<const CUtensorMap*>(tensor_map));
             return cudaGetLastError();
         }
         return cudaErrorInvalidValue;
     }
     static cudaError_t row_inv2(const void* args, const void* tensor_map, cudaStream_t st) {
         if constexpr (V2) {
-            row_inv2_kernel<T, P, C_INV><<<L / 2, P::NT, AS::inv_smem, st>>>(*static_cast<const RowInvArgs<T>*>(args),
-                                                                              *static_cast<const CUtensorMap*>(tensor_map));
+            const RowInvArgs<T>& A = *static_cast<const RowInvArgs<T>*>(args);
+            row_inv2_kernel<T, P, C_INV><<<pgrid(A.nsm, C_INV), P::NT, AS::inv_smem, st>>>(A, *static_cast<const CUtensorMap*>(tensor_map));
             return cudaGetLastError();
         }
         return cudaErrorInvalidValue;
@@ -110,8 +118,8 @@ template <typename T> struct Inst {
         col_kernel<T, P, CS::COLS><<<(L / 2) / CS::COLS, CS::COLS * P::NT, CS::smem, st>>>(A);
         return cudaGetLastError();
     }
-    static cudaError_t spectrum_prep(const void* s, void* shat, cudaStream_t st) {
-        spectrum_prep_kernel<T, P><<<148 * 2, 256, 0, st>>>(static_cast<const T*>(s), static_cast<T*>(shat));
+    static cudaError_t spectrum_prep(const void* s, void* shat, int colpos, cudaStream_t st) {
+        spectrum_prep_kernel<T, P><<<148 * 2, 256, 0, st>>>(static_cast<const T*>(s), static_cast<T*>(shat), colpos != 0);
         return cudaGetLastError();
     }
     static PassTable make(int dtype) {
@@ -124,7 +132,7 @@ template <typename T> struct Inst {
         t.cols = CS::COLS; t.col_threads = CS::COLS * P::NT; t.col_smem = CS::smem;
         t.tw_total = P::TW_TOTAL;
         t.fill_twiddles = [](void* buf) { fill_twiddles<T, P>(static_cast<cx<T>*>(buf)); };
-        t.v2 = V2 ? 1 : 0; t.v2_tbox = AS::TBOX; t.v2_threads = P::NT;
+        t.v2 = V2 ? 1 : 0; t.v2_nb = AS::NB; t.v2_abox = AS::ABOX; t.v2_tsub = AS::TSUB; t.v2_threads = P::NT;
         t.v2_ctas[0] = C_FWD; t.v2_ctas[1] = C_COL; t.v2_ctas[2] = C_INV;
         t.v2_smem[0] = AS::fwd_smem; t.v2_smem[1] = AS::col_smem; t.v2_smem[2] = AS::inv_smem;
         t.row_fwd2 = &row_fwd2; t.col2 = &col2; t.row_inv2 = &row_inv2;

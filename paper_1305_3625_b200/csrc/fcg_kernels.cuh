@@ -134,10 +134,10 @@ __global__ void __launch_bounds__(F * P::NT) row_inv_kernel(const RowInvArgs<T> 
 }
 
 template <typename T, typename P>
-__global__ void spectrum_prep_kernel(const T* __restrict__ s, T* __restrict__ shat) {
+__global__ void spectrum_prep_kernel(const T* __restrict__ s, T* __restrict__ shat, bool colpos) {
     constexpr int L = P::N;
     for (int idx = blockIdx.x * blockDim.x + threadIdx.x; idx < L * (L / 2); idx += gridDim.x * blockDim.x)
-        spectrum_prep_one<T, P>(idx, s, shat);
+        spectrum_prep_one<T, P>(idx, s, shat, colpos);
 }
 
 // ------------------------------------------------------------------------------- CG vector kernels

@@ -41,6 +41,7 @@ template <typename T> struct RowFwdArgs {
     cx<T>* Tb;             // [L/2][L] transposed half spectrum
     const cx<T>* tw;       // per-stage twiddle tables (Plan::tw_off)
     const Scalars* sc;
+    int nsm;               // SMs of the device (persistent passes: tile assignment)
 };
 
 template <typename T> struct ColArgs {
@@ -60,6 +61,7 @@ template <typename T> struct RowInvArgs {
     T scale;                              // PLAIN: 1/L^2
     double* partial;                      // [gridDim.x][2]
     Scalars* sc;
+    int nsm;
 };
 
 template <int A, int B, typename F> FCG_HD void static_for_up(F&& f) {
@@ -91,8 +93,10 @@ inline void fill_twiddles(cx<T>* out) {
 // shat[n][pos(m)] from the caller's s[m][n]: even part, 1/L^2, digit-reversed along m; row 0 and row L/2
 // hold (s0 + sN)/2 and (s0 - sN)/2 for the packed n = 0 / n = L/2 column (col_body); within a row the entry of
 // position e sits at Plan::shat_index(e).  idx = m*(L/2) + n.
+// colpos = false: the row of column frequency n is n (classic passes);  colpos = true: it is the column's number in the
+// position-ordered layout T2 of the pipelined passes, m = (e / RLAST)(RLAST/2) + e % RLAST with e = pos_of(n).
 template <typename T, typename P>
-FCG_HD void spectrum_prep_one(int idx, const T* __restrict__ s, T* __restrict__ shat) {
+FCG_HD void spectrum_prep_one(int idx, const T* __restrict__ s, T* __restrict__ shat, bool colpos = false) {
     constexpr int L = P::N;
     const T scale = (T)(1.0 / ((double)L * (double)L));
     const T h = (T)0.5;
@@ -101,7 +105,9 @@ FCG_HD void spectrum_prep_one(int idx, const T* __restrict__ s, T* __restrict__ 
     const int e = P::shat_index(P::pos_of(m));
     if (n > 0) {
         const T ev = (s[(size_t)m * L + n] + s[(size_t)mm * L + (L - n)]) * h;
-        shat[(size_t)n * L + e] = ev * scale;
+        const int en = P::pos_of(n);
+        const int row = colpos ? (en / P::RLAST) * (P::RLAST / 2) + en % P::RLAST : n;
+        shat[(size_t)row * L + e] = ev * scale;
     } else {
         const T s0 = (s[(size_t)m * L] + s[(size_t)mm * L]) * h * scale;
         const T sN = (s[(size_t)m * L + L / 2] + s[(size_t)mm * L + L / 2]) * h * scale;

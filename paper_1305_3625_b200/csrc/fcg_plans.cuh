@@ -59,12 +59,13 @@ struct PassTable {
     cudaError_t (*row_fwd)(int var, const void* args, cudaStream_t st);
     cudaError_t (*col)(const void* args, cudaStream_t st);
     cudaError_t (*row_inv)(int var, const void* args, cudaStream_t st);
-    cudaError_t (*spectrum_prep)(const void* s, void* shat, cudaStream_t st);
+    cudaError_t (*spectrum_prep)(const void* s, void* shat, int colpos, cudaStream_t st);
     // pipelined (TMA) passes of fcg_async.cuh; v2 == 0 when the size is too small for them
-    int v2, v2_tbox, v2_threads, v2_ctas[3];       // tbox: frequencies per tensor-map box of T; ctas: resident CTAs/SM asked for (fwd, col, inv)
+    int v2, v2_nb, v2_abox, v2_tsub, v2_threads, v2_ctas[3];   // nb: columns per 128-byte line of T2; abox: row pairs per column box;
+                                                   // tsub: columns per row-pass tile; ctas: resident CTAs/SM asked for (fwd, col, inv)
     size_t v2_smem[3];
     cudaError_t (*row_fwd2)(const void* args, cudaStream_t st);
-    cudaError_t (*col2)(const void* args, cudaStream_t st);
+    cudaError_t (*col2)(const void* args, const void* tensor_map, cudaStream_t st);
     cudaError_t (*row_inv2)(const void* args, const void* tensor_map, cudaStream_t st);
 };
 
