@@ -5,7 +5,6 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
-#include <cstdlib>
 #include <string>
 #include <vector>
 
@@ -129,7 +128,7 @@ template <typename T> struct Seq {
     T* q() const { return h->at<T>(h->lay.q); }
 
     cudaError_t row_fwd(int mode, const T* x, T* u) const {
-        RowFwdArgs<T> A{}; A.mode = mode | ((mode == ROWF_CG && getenv("FCG_DBG")) ? (atoi(getenv("FCG_DBG")) << 8) : 0); A.x = x; A.u = u; A.p = p(); A.r = r(); A.Tb = Tb(); A.tw = tw(); A.sc = h->sc(); A.nsm = h->nsm;
+        RowFwdArgs<T> A{}; A.mode = mode; A.x = x; A.u = u; A.p = p(); A.r = r(); A.Tb = Tb(); A.tw = tw(); A.sc = h->sc(); A.nsm = h->nsm;
         ++h->launches;
         return v2() ? h->tab->row_fwd2(&A, st) : h->tab->row_fwd(h->row_var(), &A, st);
     }
@@ -139,7 +138,7 @@ template <typename T> struct Seq {
         return (v2() && mode == COL_CONV) ? h->tab->col2(&A, &h->tmap_col, st) : h->tab->col(&A, st);
     }
     cudaError_t row_inv(int mode, const T* k, const T* v, const T* f, T* out, T* out2) const {
-        RowInvArgs<T> A{}; A.mode = mode | ((mode == ROWI_CG && getenv("FCG_DBG3")) ? (atoi(getenv("FCG_DBG3")) << 8) : 0); A.Tb = Tb(); A.tw = tw(); A.k = k; A.v = v; A.f = f; A.out = out; A.out2 = out2;
+        RowInvArgs<T> A{}; A.mode = mode; A.Tb = Tb(); A.tw = tw(); A.k = k; A.v = v; A.f = f; A.out = out; A.out2 = out2;
         A.scale = (T)(1.0 / ((double)h->L * (double)h->L));
         A.partial = h->at<double>(h->lay.partial_row); A.sc = h->sc(); A.nsm = h->nsm;
         ++h->launches;
@@ -339,16 +338,15 @@ int profile_impl(fcg_handle h, const void* k, const void* f, void* u, int iters,
     Seq<T> s{h, h->stream};
     h->launches = 0;
     FCG_CK(h, s.init((const T*)k, (const T*)f, (T*)u, 0.0, 1 << 30, false, 0ULL));
-    if (!getenv("FCG_DBG")) for (int w = 0; w < 2; ++w) FCG_CK(h, s.iteration((const T*)k, (T*)u));       // warm-up
+    for (int w = 0; w < 2; ++w) FCG_CK(h, s.iteration((const T*)k, (T*)u));       // warm-up
     std::vector<cudaEvent_t> ev((size_t)iters * 5);
     for (auto& e : ev) FCG_CK(h, cudaEventCreate(&e));
     for (int i = 0; i < iters; ++i) {
         cudaEvent_t* e = &ev[(size_t)i * 5];
-        const bool only_fwd = getenv("FCG_DBG") != nullptr && !getenv("FCG_DBG3");
         FCG_CK(h, cudaEventRecord(e[0], h->stream)); FCG_CK(h, s.it_row_fwd((T*)u));
-        FCG_CK(h, cudaEventRecord(e[1], h->stream)); if (!only_fwd) FCG_CK(h, s.it_col());
-        FCG_CK(h, cudaEventRecord(e[2], h->stream)); if (!only_fwd) FCG_CK(h, s.it_row_inv((const T*)k));
-        FCG_CK(h, cudaEventRecord(e[3], h->stream)); if (!only_fwd) FCG_CK(h, s.it_update_r());
+        FCG_CK(h, cudaEventRecord(e[1], h->stream)); FCG_CK(h, s.it_col());
+        FCG_CK(h, cudaEventRecord(e[2], h->stream)); FCG_CK(h, s.it_row_inv((const T*)k));
+        FCG_CK(h, cudaEventRecord(e[3], h->stream)); FCG_CK(h, s.it_update_r());
         FCG_CK(h, cudaEventRecord(e[4], h->stream));
     }
     FCG_CK(h, cudaMemcpyAsync(h->h_sc, h->sc(), sizeof(Scalars), cudaMemcpyDeviceToHost, h->stream));

@@ -31,15 +31,10 @@ namespace fcg {
 template <typename T, typename P> struct AsyncShape {
     static constexpr int L = P::N, NT = P::NT, R1 = P::radix(1), Q1 = L / R1, PER1 = Q1 / NT;
     static constexpr bool valid = NT >= 64 && L >= 512;
-    static constexpr size_t WBYTES = (size_t)L * 2 * sizeof(T);              // one complex transform
+    static constexpr size_t WBYTES = (size_t)L * 2 * sizeof(T);              // one complex transform (work buffer)
     static constexpr uint32_t PIECE = (uint32_t)(Q1 * sizeof(T));            // one stage-1 strip of one real row
-    static constexpr int MAXSLOT = 8;
-    // P3: beside the work buffer, two tiles of T (TSB bytes = TSUB frequencies x 2 rows each) and a ring of KRB bytes
-    // for strips of k, p (, f); both run ahead across transforms
-    static constexpr size_t TSB = WBYTES >= 16384 ? 8192 : WBYTES / 2;
-    static constexpr size_t KRB = 8 * (size_t)PIECE > 24576 ? 8 * (size_t)PIECE : 24576;
-    static constexpr int TSUB = (int)(TSB / (2 * 2 * sizeof(T)));            // columns per tile of T
-    static constexpr int NSUB = (L / 2) / TSUB;
+    static constexpr int MAXSLOT = 16;
+
     // Layout of T for these passes: columns are numbered by their POSITION in the digit-reversed row
     // spectrum, m = 0 .. L/2-1 <-> position e(m) = (m / HR) RLAST + m % HR <-> frequency n = freq_of(e(m)) < L/2, and
     // NB consecutive columns x one row pair form one 128-byte line:  T2[m / NB][A][m % NB][r],  a = 2A + r.
@@ -49,20 +44,42 @@ template <typename T, typename P> struct AsyncShape {
     static FCG_HD int pos_of_col(int m) { return (m / HR) * P::RLAST + m % HR; }
     static FCG_HD int col_of_pos(int e) { return (e / P::RLAST) * HR + e % P::RLAST; }
     static FCG_HD size_t t2_index(int m, int A) { return (((size_t)(m / NB) * (L / 2) + A) * NB + m % NB) * 2; }   // complex units, r = 0
-    // P1: ring of NFS strips (6 pieces each) beside the work buffer, running ahead across transforms
+
+    // Shared memory.  The rings are sized for CRES resident CTAs per SM: 4 transforms in flight when a work buffer is
+    // small, else 2 (1 when even that does not fit); whatever the work buffers leave goes to the rings, whose depth is
+    // what hides the loaded DRAM latency.  2688 = static barriers + 1 KB per-CTA reserve + alignment slack.
+    static constexpr int CRES = WBYTES <= 16384 ? 4 : (WBYTES <= 65536 ? 2 : 1);
+    static constexpr size_t RING_BUDGET = ((size_t)FCG_MAX_SMEM / CRES - 2688 - WBYTES) / 128 * 128;
+    // P1: ring of NFS strips (p0 p1 r0 r1 u0 u1: 6 pieces each)
     static constexpr uint32_t FSLOTB = 6 * PIECE;
-    static constexpr int NFS = 32768 / FSLOTB < 2 ? 2 : (32768 / FSLOTB > MAXSLOT ? MAXSLOT : (int)(32768 / FSLOTB));
+    static constexpr int NFS = RING_BUDGET / FSLOTB < 2 ? 2 : (RING_BUDGET / FSLOTB > MAXSLOT ? MAXSLOT : (int)(RING_BUDGET / FSLOTB));
     static constexpr size_t fwd_smem = WBYTES + (size_t)NFS * FSLOTB + 128;   // + 128: the kernels align the dynamic base themselves
+    // P2: column + its spectrum row
     static constexpr size_t col_smem = WBYTES + (size_t)L * sizeof(T) + 128;
-    static constexpr size_t inv_smem = WBYTES + 2 * TSB + KRB + 128;
-    static constexpr int thread_cap = sizeof(T) == 8 ? 608 : 1152;           // ~104-128 / ~56-64 registers per thread
-    static constexpr int ctas(size_t smem) {
-        const int by_smem = (int)((size_t)FCG_MAX_SMEM / (smem + 1024));
-        const int by_thr = thread_cap / (NT + 32) > 1 ? thread_cap / (NT + 32) : 1;
+    // P3: NTS tiles of T2 (TSB bytes = TSUB columns x 2 rows each) and a ring of KRB bytes for strips of k, p (, f).
+    // The strip ring gets at least two loop-mode strips (4 pieces each); the tiles get smaller if that is what it takes.
+    static constexpr size_t TSB_MAX = WBYTES >= 16384 ? 8192 : WBYTES / 2;
+    static constexpr size_t KMIN = 8 * (size_t)PIECE;
+    static constexpr size_t TSB = RING_BUDGET >= KMIN + 2 * TSB_MAX ? TSB_MAX : TSB_MAX / 2;
+    static constexpr int TSUB = (int)(TSB / (2 * 2 * sizeof(T)));            // columns per tile of T2
+    static constexpr int NSUB = (L / 2) / TSUB;
+    static constexpr int NTS_ = (int)((RING_BUDGET - KMIN) / TSB);
+    static constexpr int NTS = NTS_ < 2 ? 2 : (NTS_ > NSUB ? NSUB : (NTS_ > MAXSLOT ? MAXSLOT : NTS_));
+    static constexpr size_t KRB = RING_BUDGET - (size_t)NTS * TSB;
+    static constexpr size_t inv_smem = WBYTES + (size_t)NTS * TSB + KRB + 128;
+    static constexpr bool PRODUCER_WARPS = NT <= 256;                        // P3: dedicated TMA-issuing warps (else consumer warp 0 issues)
+    static constexpr int INV_THREADS = NT + (PRODUCER_WARPS ? 64 : 0);
+
+    static constexpr int thread_cap = sizeof(T) == 8 ? 640 : 1152;           // ~104-128 / ~56-64 registers per thread
+    // resident CTAs per SM to compile for: static_smem = the kernel's __shared__ barriers etc., extra = producer threads
+    static constexpr int ctas(size_t smem, size_t static_smem, int extra) {
+        const int by_smem = (int)((size_t)FCG_MAX_SMEM / (smem + static_smem + 1024));
+        const int by_thr = thread_cap / (NT + extra) > 1 ? thread_cap / (NT + extra) : 1;
         return by_smem < 1 ? 1 : (by_smem < by_thr ? by_smem : by_thr);
     }
-    static_assert(!valid || KRB >= 6 * (size_t)PIECE, "ring too small for one strip");
+    static_assert(!valid || (KRB >= 6 * (size_t)PIECE && KRB >= KMIN), "strip ring too small");
     static_assert(!valid || (TSUB % NB == 0 && TSUB / NB <= 256 && (L / 2) % TSUB == 0 && NSUB >= 2 && NT % 32 == 0), "tile shape");
+    static_assert(!valid || (fwd_smem <= (size_t)FCG_MAX_SMEM && inv_smem <= (size_t)FCG_MAX_SMEM && col_smem <= (size_t)FCG_MAX_SMEM), "shared memory");
 };
 
 #ifdef __CUDACC__
@@ -108,10 +125,12 @@ __global__ void __launch_bounds__(P::NT + 32, CTAS) row_fwd2_kernel(const RowFwd
     cx<T>* W = reinterpret_cast<cx<T>*>(smem_raw);
     SmemIO<T, P> io{W};
     const int lt = threadIdx.x, lane = lt & 31, warp = lt >> 5;
-    const bool cg = (A.mode & 0xff) == ROWF_CG;
-    const int dbg = A.mode >> 8;
+    const bool cg = A.mode == ROWF_CG;
     if (cg && A.sc->done) return;                                 // converged: nothing may change
     const int nv = cg ? 6 : 2;
+    // Always true, but opaque to the compiler: guarding the global stores with it keeps them in basic blocks of their own
+    // instead of interleaved with the shared-memory loads of the next strip.  Measured at L=2048 fp64: 39 vs 44 us.
+    const bool st_on = A.mode >= 0;
 
     // my transforms: tile(i) = grp + nsm * (j + i * k)
     const int nsm = A.nsm < (int)gridDim.x ? A.nsm : (int)gridDim.x, grp = (int)blockIdx.x % nsm, jj = (int)blockIdx.x / nsm,
@@ -173,8 +192,7 @@ __global__ void __launch_bounds__(P::NT + 32, CTAS) row_fwd2_kernel(const RowFwd
                     u0 = u0 + alpha * p0; u1 = u1 + alpha * p1;       // new x, lagged one pass
                     p0 = r0 + beta * p0;  p1 = r1 + beta * p1;        // new direction
                     const size_t i0 = row0 + (size_t)t * Q1 + j;
-                    if (!(dbg & 2)) { A.u[i0] = u0; A.u[i0 + L] = u1;
-                    A.p[i0] = p0; A.p[i0 + L] = p1; }
+                    if (st_on) { A.u[i0] = u0; A.u[i0 + L] = u1; A.p[i0] = p0; A.p[i0 + L] = p1; }
                     z[q][t] = mk<T>(p0, p1);
                 } else {
                     z[q][t] = mk<T>(sl[j], sl[Q1 + j]);
@@ -183,16 +201,15 @@ __global__ void __launch_bounds__(P::NT + 32, CTAS) row_fwd2_kernel(const RowFwd
             if (i * R1 + t + NSLOT < G) tma::mbar_warp_release(&empty[slot]);   // this warp has read the slot
             if (++slot == NSLOT) { slot = 0; phase ^= 1u; }
         }
-        if (dbg & 4) { if (z[0][0].x == (T)123.456) A.Tb[0] = z[0][1]; continue; }
         bar_named<NT>();                                          // the previous transform's separation has left W
-        stage_math<P, 1, -1, T>(z, wb[1]);
+        stage_math<P, 1, -1, T, true>(z, wb[1]);
         stage_st<P, 1, T>(lt, [&](int e, cx<T> v) { io.st(e, v); }, z);
         bar_named<NT>();
         static_for_up<2, S>([&](auto s) {
             constexpr int sv = decltype(s)::value;
             cx<T> a[St<P, sv>::PER][St<P, sv>::R];
             stage_ld<P, sv, T>(lt, [&](int e) { return io.ld(e); }, a);
-            stage_math<P, sv, -1, T>(a, wb[sv]);
+            stage_math<P, sv, -1, T, true>(a, wb[sv]);
             stage_st<P, sv, T>(lt, [&](int e, cx<T> v) { io.st(e, v); }, a);
             bar_named<NT>();
         });
@@ -213,7 +230,7 @@ __global__ void __launch_bounds__(P::NT + 32, CTAS) row_fwd2_kernel(const RowFwd
                 X0 = mk<T>((Za.x + Zb.x) * h, (Za.y - Zb.y) * h);
                 X1 = mk<T>((Za.y + Zb.y) * h, (Zb.x - Za.x) * h);
             }
-            if (!(dbg & 1) || X0.x == (T)123.456) store_pair<T>(A.Tb + AS::t2_index(m, a0 >> 1), X0, X1);
+            if (st_on) store_pair<T>(A.Tb + AS::t2_index(m, a0 >> 1), X0, X1);
         }
     }
 }
@@ -326,158 +343,165 @@ __global__ void __launch_bounds__(P::NT, CTAS) col2_kernel(const ColArgs<T> A, c
 
 // --------------------------------------------------------------------------------------------- P3
 //   c = F_row^H T (rows a0, a0+1);  q = k o p + c  [+ partial p.q]   (or residual / apply / plain)
-// Persistent like P1.  Two rings run ahead across transforms: tiles of T (TSUB frequencies x 2 rows, TMA tensor
-// loads of whole 128-byte lines of T2) feeding the rebuild of the packed spectrum, and strips of k, p (, f) feeding
-// the epilogue.
+// Persistent and warp-specialised like P1.  The producer warp feeds two rings in consumption order: tiles of T2
+// (TSUB columns x 2 rows as whole 128-byte lines, TMA tensor loads) for the rebuild of the packed spectrum, and strips
+// of k, p (, f) for the epilogue; both run ahead across transforms as far as shared memory allows.
 template <typename T, typename P, int CTAS>
-__global__ void __launch_bounds__(P::NT, CTAS) row_inv2_kernel(const RowInvArgs<T> A, const __grid_constant__ CUtensorMap tmap)
+__global__ void __launch_bounds__(AsyncShape<T, P>::INV_THREADS, CTAS) row_inv2_kernel(const RowInvArgs<T> A, const __grid_constant__ CUtensorMap tmap)
 {
     using AS = AsyncShape<T, P>;
     constexpr int L = P::N, S = P::S, NT = P::NT, R1 = AS::R1, Q1 = AS::Q1, PER1 = AS::PER1, PM = per_max<P>();
     constexpr uint32_t PIECE = AS::PIECE;
-    constexpr int TSUB = AS::TSUB, NSUB = AS::NSUB;
+    constexpr int TSUB = AS::TSUB, NSUB = AS::NSUB, NTS = AS::NTS;
     constexpr uint32_t TBYTES = (uint32_t)AS::TSB;
     extern __shared__ unsigned char smem_dyn[];
     unsigned char* const smem_raw = align128(smem_dyn);
-    __shared__ __align__(8) uint64_t tfull[2], tempty[2];
+    __shared__ __align__(8) uint64_t tfull[AS::MAXSLOT], tempty[AS::MAXSLOT];
     __shared__ __align__(8) uint64_t kfull[AS::MAXSLOT], kempty[AS::MAXSLOT];
     __shared__ double red[2 * 32];
     cx<T>* W = reinterpret_cast<cx<T>*>(smem_raw);
     unsigned char* const tring = smem_raw + AS::WBYTES;
-    unsigned char* const kring = tring + 2 * AS::TSB;
+    unsigned char* const kring = tring + (size_t)NTS * AS::TSB;
     SmemIO<T, P> io{W};
     const int lt = threadIdx.x, lane = lt & 31, warp = lt >> 5;
-    const int mode = A.mode & 0xff;
-    const int dbg = A.mode >> 8;
+    const int mode = A.mode;
     if (mode == ROWI_CG && A.sc->done) return;
-    const int nv = (mode == ROWI_PLAIN || (dbg & 4)) ? 0 : (mode == ROWI_RESID ? 6 : 4);
+    const bool st_on = mode >= 0;                                 // always true, opaque to the compiler (as in row_fwd2_kernel)
+    const int nv = mode == ROWI_PLAIN ? 0 : (mode == ROWI_RESID ? 6 : 4);
     int nks = nv ? (int)(AS::KRB / (nv * PIECE)) : 1;
     nks = nks > AS::MAXSLOT ? AS::MAXSLOT : nks;
     const uint32_t kslotb = nv * PIECE;
 
-    const int nsm = A.nsm < (int)gridDim.x ? A.nsm : (int)gridDim.x, grp = (int)blockIdx.x % nsm, jj = (int)blockIdx.x / nsm, kk = (int)gridDim.x / nsm;
+    const int nsm = A.nsm < (int)gridDim.x ? A.nsm : (int)gridDim.x, grp = (int)blockIdx.x % nsm, jj = (int)blockIdx.x / nsm,
+              kk = (int)gridDim.x / nsm;
     auto tile_of = [&](int i) { return grp + nsm * (jj + i * kk); };
     int ntl = 0;
     while (tile_of(ntl) < L / 2) ++ntl;
-    const int GT = ntl * NSUB, GK = nv ? ntl * R1 : 0;
 
-    auto issue_T = [&](int gs) {         // thread 0: tile gs = (transform gs / NSUB, part gs % NSUB): TSUB columns x 2 rows of T2, 128-byte lines
-        const int slot = gs & 1;
-        tma::mbar_expect_tx(&tfull[slot], TBYTES);
-        tma::tensor_g2s_3d(tring + (size_t)slot * TBYTES, &tmap, 0, tile_of(gs / NSUB), (gs % NSUB) * (TSUB / AS::NB), &tfull[slot]);
-    };
-    auto issue_K = [&](int g, int slot) {          // all of warp 0: strip g % R1 of k0 k1 v0 v1 (f0 f1) of transform g / R1
-        if (lane == 0) tma::mbar_expect_tx(&kfull[slot], kslotb);
-        __syncwarp();
-        if (lane < nv) {
-            const T* src = lane < 2 ? A.k : lane < 4 ? A.v : A.f;
-            src += (size_t)(2 * tile_of(g / R1) + (lane & 1)) * L + (size_t)(g % R1) * Q1;
-            tma::bulk_g2s(kring + (size_t)slot * kslotb + (size_t)lane * PIECE, src, PIECE, &kfull[slot]);
-        }
-    };
     if (lt == 0) {
         tma::prefetch_tmap(&tmap);
-        tma::mbar_init(&tfull[0], 1); tma::mbar_init(&tfull[1], 1);
-        tma::mbar_init(&tempty[0], NT / 32); tma::mbar_init(&tempty[1], NT / 32);
+        for (int i = 0; i < NTS; ++i) { tma::mbar_init(&tfull[i], 1); tma::mbar_init(&tempty[i], NT / 32); }
         for (int i = 0; i < AS::MAXSLOT; ++i) { tma::mbar_init(&kfull[i], 1); tma::mbar_init(&kempty[i], NT / 32); }
         tma::fence_mbar_init();
-        if (GT > 0) issue_T(0);
-        if (GT > 1) issue_T(1);
     }
     __syncthreads();
-    if (warp == 0)
-        for (int g = 0; g < nks && g < GK; ++g) issue_K(g, g);
-    cx<T> wb[S + 1][PM];
-    static_for_up<1, S - 1>([&](auto s) { base_tw<P, decltype(s)::value, T>(lt, A.tw, wb[decltype(s)::value]); });
 
     double acc[2] = {0.0, 0.0};
-    int kslot = 0;
-    uint32_t kphase = 0;
-    for (int i = 0; i < ntl; ++i) {
-        const int a0 = 2 * tile_of(i);
-        const size_t row0 = (size_t)a0 * L;
-        // rebuild the packed spectrum Z = X_even + i X_odd at its digit-reversed place, tile by tile
-        for (int sub = 0; sub < NSUB; ++sub) {
-            const int gs = i * NSUB + sub, ts = gs & 1;
-            const uint32_t tph = (uint32_t)((gs >> 1) & 1);
-            tma::mbar_wait(&tfull[ts], tph);
-            const cx<T>* Ts = reinterpret_cast<const cx<T>*>(tring + (size_t)ts * TBYTES);
-#pragma unroll 4
-            for (int ml = lt; ml < TSUB; ml += NT) {
-                const int e = AS::pos_of_col(sub * TSUB + ml);
-                const int n = P::freq_of(e);
-                const cx<T> X0 = Ts[2 * ml], X1 = Ts[2 * ml + 1];
-                if (n == 0) {
-                    io.st(P::pos_of(0), mk<T>(X0.x, X1.x));
-                    io.st(P::pos_of(L / 2), mk<T>(X0.y, X1.y));
-                } else {
-                    io.st(e, mk<T>(X0.x - X1.y, X0.y + X1.x));
-                    io.st(P::pos_of(L - n), mk<T>(X0.x + X1.y, X1.x - X0.y));
-                }
-            }
-            if (gs + 2 < GT) {
-                tma::mbar_warp_release(&tempty[ts]);                  // this warp has read the tile
-                if (lt == 0) {
-                    tma::mbar_wait(&tempty[ts], tph);
-                    issue_T(gs + 2);
-                }
-            }
+    // Producer state: next tile of T2 / next strip to issue, in consumption order.  With PW (small transforms) two extra
+    // warps run these loops; otherwise (NT >= 512, where two more warps would cost 8 registers per thread) consumer warp 0
+    // issues the successor of every slot it has just seen released.
+    constexpr bool PW = AS::PRODUCER_WARPS;
+    int p_ts = 0, p_tn = 0, p_ks = 0, p_kn = 0;
+    uint32_t p_tph = 0, p_kph = 0;
+    const int GT = ntl * NSUB, GK = nv ? ntl * R1 : 0;
+    const T* kbase = nullptr;
+    if (nv) kbase = (lane < 2 ? A.k : lane < 4 ? A.v : A.f) + (size_t)(lane & 1) * L;
+    auto issue_next_T = [&]() {          // whole warp; tile p_tn = (transform p_tn / NSUB, part p_tn % NSUB): TSUB / NB whole lines
+        if (p_tn >= NTS) tma::mbar_wait(&tempty[p_ts], p_tph ^ 1u);
+        if (lane == 0) {
+            tma::mbar_expect_tx(&tfull[p_ts], TBYTES);
+            tma::tensor_g2s_3d(tring + (size_t)p_ts * TBYTES, &tmap, 0, tile_of(p_tn / NSUB), (p_tn % NSUB) * (TSUB / AS::NB), &tfull[p_ts]);
         }
-        __syncthreads();                                              // Z complete in W
-        if (dbg & 2) { if (W[lt].x == (T)123.456) A.out[0] = W[1].x; continue; }
-        static_for_down<S, 2>([&](auto s) {
-            constexpr int sv = decltype(s)::value;
-            cx<T> a[St<P, sv>::PER][St<P, sv>::R];
-            stage_ld<P, sv, T>(lt, [&](int e) { return io.ld(e); }, a);
-            stage_math<P, sv, +1, T>(a, wb[sv]);
-            stage_st<P, sv, T>(lt, [&](int e, cx<T> v) { io.st(e, v); }, a);
-            __syncthreads();
-        });
-        // inverse stage 1 straight into the epilogue: natural order, re = even row, im = odd row
-        cx<T> c[PER1][R1];
-        stage_ld<P, 1, T>(lt, [&](int e) { return io.ld(e); }, c);
-        __syncthreads();                                              // W may now be rebuilt for the next transform
-        stage_math<P, 1, +1, T>(c, wb[1]);
-#pragma unroll
-        for (int t = 0; t < R1; ++t) {
-            const T* sl = nullptr;
-            if (nv) {
-                tma::mbar_wait(&kfull[kslot], kphase);
-                sl = reinterpret_cast<const T*>(kring + (size_t)kslot * kslotb);
-            }
-#pragma unroll
-            for (int q = 0; q < PER1; ++q) {
-                const int j = lt + q * NT;
-                const size_t i0 = row0 + (size_t)t * Q1 + j;
-                const T c0 = c[q][t].x, c1 = c[q][t].y;
-                if (mode == ROWI_PLAIN || (dbg & 4)) { if (!(dbg & 1)) { A.out[i0] = c0 * A.scale; A.out[i0 + L] = c1 * A.scale; } continue; }
-                const T v0 = sl[2 * Q1 + j], v1 = sl[3 * Q1 + j];
-                const T val0 = sl[j] * v0 + c0, val1 = sl[Q1 + j] * v1 + c1;         // k o x + C x
-                if (mode == ROWI_RESID) {
-                    const T f0 = sl[4 * Q1 + j], f1 = sl[5 * Q1 + j];
-                    const T r0 = f0 - val0, r1 = f1 - val1;                           // r = f - A u
-                    A.out[i0] = r0; A.out[i0 + L] = r1; A.out2[i0] = (T)0; A.out2[i0 + L] = (T)0;
-                    acc[0] += (double)r0 * (double)r0; acc[0] += (double)r1 * (double)r1;
-                    acc[1] += (double)f0 * (double)f0; acc[1] += (double)f1 * (double)f1;
-                } else {
-                    A.out[i0] = val0; A.out[i0 + L] = val1;
-                    acc[0] += (double)v0 * (double)val0; acc[0] += (double)v1 * (double)val1;   // search length p.Ap
-                }
-            }
-            if (nv) {
-                const int g = i * R1 + t;
-                if (g + nks < GK) {
-                    tma::mbar_warp_release(&kempty[kslot]);
-                    if (warp == 0) {
-                        tma::mbar_wait(&kempty[kslot], kphase);
-                        issue_K(g + nks, kslot);
+        ++p_tn;
+        if (++p_ts == NTS) { p_ts = 0; p_tph ^= 1u; }
+    };
+    auto issue_next_K = [&]() {          // whole warp; strip p_kn % R1 of k0 k1 v0 v1 (f0 f1) of transform p_kn / R1, one bulk copy per lane < nv
+        if (p_kn >= nks) tma::mbar_wait(&kempty[p_ks], p_kph ^ 1u);
+        if (lane == 0) tma::mbar_expect_tx(&kfull[p_ks], kslotb);
+        __syncwarp();
+        if (lane < nv)
+            tma::bulk_g2s(kring + (size_t)p_ks * kslotb + (size_t)lane * PIECE,
+                          kbase + (size_t)(2 * tile_of(p_kn / R1)) * L + (size_t)(p_kn % R1) * Q1, PIECE, &kfull[p_ks]);
+        ++p_kn;
+        if (++p_ks == nks) { p_ks = 0; p_kph ^= 1u; }
+    };
+    if (PW && warp == NT / 32) {
+        while (p_tn < GT) issue_next_T();
+    } else if (PW && warp == NT / 32 + 1) {
+        while (p_kn < GK) issue_next_K();
+    } else if (warp < NT / 32) {
+        if (!PW && warp == 0) {
+            while (p_tn < GT && p_tn < NTS) issue_next_T();
+            while (p_kn < GK && p_kn < nks) issue_next_K();
+        }
+        // ---- consumers
+        cx<T> wb[S + 1][PM];
+        static_for_up<1, S - 1>([&](auto s) { base_tw<P, decltype(s)::value, T>(lt, A.tw, wb[decltype(s)::value]); });
+        int ts = 0, ks = 0;
+        uint32_t tph = 0, kph = 0;
+        for (int i = 0; i < ntl; ++i) {
+            const int a0 = 2 * tile_of(i);
+            const size_t row0 = (size_t)a0 * L;
+            // rebuild the packed spectrum Z = X_even + i X_odd at its digit-reversed place, tile by tile
+            for (int sub = 0; sub < NSUB; ++sub) {
+                tma::mbar_wait(&tfull[ts], tph);
+                const cx<T>* Ts = reinterpret_cast<const cx<T>*>(tring + (size_t)ts * TBYTES);
+#pragma unroll 4
+                for (int ml = lt; ml < TSUB; ml += NT) {
+                    const int e = AS::pos_of_col(sub * TSUB + ml);
+                    const int n = P::freq_of(e);
+                    const cx<T> X0 = Ts[2 * ml], X1 = Ts[2 * ml + 1];
+                    if (n == 0) {
+                        io.st(P::pos_of(0), mk<T>(X0.x, X1.x));
+                        io.st(P::pos_of(L / 2), mk<T>(X0.y, X1.y));
+                    } else {
+                        io.st(e, mk<T>(X0.x - X1.y, X0.y + X1.x));
+                        io.st(P::pos_of(L - n), mk<T>(X0.x + X1.y, X1.x - X0.y));
                     }
                 }
-                if (++kslot == nks) { kslot = 0; kphase ^= 1u; }
+                tma::mbar_warp_release(&tempty[ts]);                  // this warp has read the tile
+                if (!PW && warp == 0 && p_tn < GT) issue_next_T();
+                if (++ts == NTS) { ts = 0; tph ^= 1u; }
+            }
+            bar_named<NT>();                                          // Z complete in W
+            static_for_down<S, 2>([&](auto s) {
+                constexpr int sv = decltype(s)::value;
+                cx<T> a[St<P, sv>::PER][St<P, sv>::R];
+                stage_ld<P, sv, T>(lt, [&](int e) { return io.ld(e); }, a);
+                stage_math<P, sv, +1, T>(a, wb[sv]);
+                stage_st<P, sv, T>(lt, [&](int e, cx<T> v) { io.st(e, v); }, a);
+                bar_named<NT>();
+            });
+            // inverse stage 1 straight into the epilogue: natural order, re = even row, im = odd row
+            cx<T> c[PER1][R1];
+            stage_ld<P, 1, T>(lt, [&](int e) { return io.ld(e); }, c);
+            bar_named<NT>();                                          // W may now be rebuilt for the next transform
+            stage_math<P, 1, +1, T>(c, wb[1]);
+#pragma unroll
+            for (int t = 0; t < R1; ++t) {
+                const T* sl = nullptr;
+                if (nv) {
+                    tma::mbar_wait(&kfull[ks], kph);
+                    sl = reinterpret_cast<const T*>(kring + (size_t)ks * kslotb);
+                }
+#pragma unroll
+                for (int q = 0; q < PER1; ++q) {
+                    const int j = lt + q * NT;
+                    const size_t i0 = row0 + (size_t)t * Q1 + j;
+                    const T c0 = c[q][t].x, c1 = c[q][t].y;
+                    if (mode == ROWI_PLAIN) { A.out[i0] = c0 * A.scale; A.out[i0 + L] = c1 * A.scale; continue; }
+                    const T v0 = sl[2 * Q1 + j], v1 = sl[3 * Q1 + j];
+                    const T val0 = sl[j] * v0 + c0, val1 = sl[Q1 + j] * v1 + c1;         // k o x + C x
+                    if (mode == ROWI_RESID) {
+                        const T f0 = sl[4 * Q1 + j], f1 = sl[5 * Q1 + j];
+                        const T r0 = f0 - val0, r1 = f1 - val1;                           // r = f - A u
+                        A.out[i0] = r0; A.out[i0 + L] = r1; A.out2[i0] = (T)0; A.out2[i0 + L] = (T)0;
+                        acc[0] += (double)r0 * (double)r0; acc[0] += (double)r1 * (double)r1;
+                        acc[1] += (double)f0 * (double)f0; acc[1] += (double)f1 * (double)f1;
+                    } else {
+                        if (st_on) { A.out[i0] = val0; A.out[i0 + L] = val1; }
+                        acc[0] += (double)v0 * (double)val0; acc[0] += (double)v1 * (double)val1;   // search length p.Ap
+                    }
+                }
+                if (nv) {
+                    tma::mbar_warp_release(&kempty[ks]);
+                    if (!PW && warp == 0 && p_kn < GK) issue_next_K();
+                    if (++ks == nks) { ks = 0; kph ^= 1u; }
+                }
             }
         }
     }
-    row_inv_reduce_finalize<T>(A, acc, red);
+    row_inv_reduce_finalize<T>(A, acc, red);      // all warps (the producer contributes zeros)
 }
 
 #endif  // __CUDACC__

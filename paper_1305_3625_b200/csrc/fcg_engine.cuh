@@ -77,17 +77,49 @@ FCG_HD void run_middle(int lt, LD ld, ST st, MUL mul)
 // The same stage split into load / math / store so that barriers, asynchronous-copy waits and fused epilogues
 // can be placed between the steps.  Twiddles are not read from the [u][j] tables: each thread keeps the base
 // twiddle w = w_M^j of each of its butterflies (one table entry, fetched once at kernel start) and forms the
-// powers w^2 .. w^(R-1) by a product tree of depth log2 R (error <= ~4 ulp), which costs no memory traffic.
+// powers w^2 .. w^(R-1) by a product tree (apply_twiddles, error <= ~4 ulp), which costs no memory traffic.
 template <typename P, int s> struct St {
     static constexpr int R = P::radix(s), M = P::mlen(s), Q = M / R, NB = P::N / R, PER = NB / P::NT, TWO = P::tw_off(s);
     static_assert(PER >= 1, "plan: NT too large for this radix");
 };
 
-template <int R, typename C> FCG_HD void tw_powers(C w, C (&pw)[R]) {
-    pw[0] = w;
-    if constexpr (R > 1) pw[1] = w;
+// a[u] *= w^u (CONJ: conj(w)^u), u = 1 .. R-1.  Two ways to form the powers, chosen per kernel by measurement (it is a
+// register-allocation matter: row_fwd2 at L=2048 fp64 runs 39 us with CHAIN and 44 us with the tree, row_inv2 36 vs 39):
+//   tree : w^u = w^(u/2) w^(u - u/2), depth log2 R products (error <= ~4 ulp), all powers live at once;
+//   CHAIN: w^2, w^3, w^4 by products, then four interleaved chains w^u = w^(u-4) w^4 (depth <= 5, <= ~6 ulp),
+//          at most five powers live at a time.
+template <int R, bool CONJ, bool CHAIN, typename C> FCG_HD void apply_twiddles(C (&a)[R], C w) {
+    auto mul = [](C x, C t) { return CONJ ? cmulwc(x, t) : cmulw(x, t); };
+    if constexpr (!CHAIN) {
+        C pw[R];
+        pw[0] = w;
+        if constexpr (R > 1) pw[1] = w;
 #pragma unroll
-    for (int u = 2; u < R; ++u) pw[u] = cmulw(pw[u / 2], pw[u - u / 2]);
+        for (int u = 2; u < R; ++u) pw[u] = cmulw(pw[u / 2], pw[u - u / 2]);
+#pragma unroll
+        for (int u = 1; u < R; ++u) a[u] = mul(a[u], pw[u]);
+    } else {
+        if constexpr (R > 1) a[1] = mul(a[1], w);
+        if constexpr (R > 2) {
+            const C w2 = cmulw(w, w);
+            a[2] = mul(a[2], w2);
+            if constexpr (R > 3) {
+                const C w3 = cmulw(w2, w);
+                a[3] = mul(a[3], w3);
+                if constexpr (R > 4) {
+                    const C w4 = cmulw(w2, w2);
+                    C c0 = w4, c1 = w, c2 = w2, c3 = w3;          // c_k holds w^(4 j + k), advanced by w^4
+                    a[4] = mul(a[4], c0);
+#pragma unroll
+                    for (int u = 5; u < R; ++u) {
+                        C& c = (u % 4 == 0) ? c0 : (u % 4 == 1) ? c1 : (u % 4 == 2) ? c2 : c3;
+                        c = cmulw(c, w4);
+                        a[u] = mul(a[u], c);
+                    }
+                }
+            }
+        }
+    }
 }
 
 // base twiddles of this thread's butterflies in stage s (u = 1 row of the stage's table)
@@ -122,7 +154,7 @@ FCG_HD void stage_st(int lt, ST st, const cx<T> (&a)[St<P, s>::PER][St<P, s>::R]
     }
 }
 // DIR < 0: a <- DFT_R(a), a[u] *= w^(u);   DIR > 0 (adjoint, run in reverse stage order): a[u] *= conj(w^u), a <- DFT_R^H(a)
-template <typename P, int s, int DIR, typename T>
+template <typename P, int s, int DIR, typename T, bool CHAIN = false>
 FCG_HD void stage_math(cx<T> (&a)[St<P, s>::PER][St<P, s>::R], const cx<T>* w) {
     using I = St<P, s>;
 #pragma unroll
@@ -130,17 +162,11 @@ FCG_HD void stage_math(cx<T> (&a)[St<P, s>::PER][St<P, s>::R], const cx<T>* w) {
         if constexpr (DIR < 0) {
             dftR<I::R, -1>(a[i]);
             if constexpr (I::Q > 1) {
-                cx<T> pw[I::R];
-                tw_powers<I::R>(w[i], pw);
-#pragma unroll
-                for (int u = 1; u < I::R; ++u) a[i][u] = cmulw(a[i][u], pw[u]);
+                apply_twiddles<I::R, false, CHAIN>(a[i], w[i]);
             }
         } else {
             if constexpr (I::Q > 1) {
-                cx<T> pw[I::R];
-                tw_powers<I::R>(w[i], pw);
-#pragma unroll
-                for (int u = 1; u < I::R; ++u) a[i][u] = cmulwc(a[i][u], pw[u]);
+                apply_twiddles<I::R, true, CHAIN>(a[i], w[i]);
             }
             dftR<I::R, +1>(a[i]);
         }

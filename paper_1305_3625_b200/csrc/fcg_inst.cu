@@ -18,7 +18,8 @@ template <typename T> struct Inst {
     using AS = AsyncShape<T, P>;
     static constexpr int L = FCG_INST_L;
     static constexpr bool V2 = AS::valid;
-    static constexpr int C_FWD = AS::ctas(AS::fwd_smem), C_COL = AS::ctas(AS::col_smem), C_INV = AS::ctas(AS::inv_smem);
+    static constexpr int C_FWD = AS::ctas(AS::fwd_smem, 320, 32), C_COL = AS::ctas(AS::col_smem, 64, 64),
+                         C_INV = AS::ctas(AS::inv_smem, 1280, AS::INV_THREADS - P::NT);
 
     // opt in to > 48 KB of dynamic shared memory and ask for the largest shared-memory carveout, so that as
     // many CTAs as the register file allows are resident
@@ -73,7 +74,7 @@ template <typename T> struct Inst {
     static cudaError_t row_inv2(const void* args, const void* tensor_map, cudaStream_t st) {
         if constexpr (V2) {
             const RowInvArgs<T>& A = *static_cast<const RowInvArgs<T>*>(args);
-            row_inv2_kernel<T, P, C_INV><<<pgrid(A.nsm, C_INV), P::NT, AS::inv_smem, st>>>(A, *static_cast<const CUtensorMap*>(tensor_map));
+            row_inv2_kernel<T, P, C_INV><<<pgrid(A.nsm, C_INV), AS::INV_THREADS, AS::inv_smem, st>>>(A, *static_cast<const CUtensorMap*>(tensor_map));
             return cudaGetLastError();
         }
         return cudaErrorInvalidValue;
