@@ -155,6 +155,61 @@ def bench_workload(binding, torch, w, steps, warmup, profile_iters=20, e2e_steps
     return out
 
 
+def bench_extras(binding, torch, inputs):
+    """--full: the rest of north_star's list -- stand-alone transforms (GB/s on 4 N w bytes per transform), the break step, and
+    the quasi-static loop of configs[3] (first 200 of its 2000 steps; latency-bound: us per CG iteration is the figure)."""
+    out = {}
+    to = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    for L, dt, tdt in ((2048, np.float64, torch.float64), (2048, np.float32, torch.float32), (8192, np.float32, torch.float32)):
+        h = binding.Fcg(L, tdt)
+        x = to(inputs.fft_field(L).astype(dt))
+        X = h.fcg_fft_fwd(x); xb = h.fcg_fft_inv(X)
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+        torch.cuda.synchronize()
+        reps = 10
+        ev[0].record()
+        for _ in range(reps): h.fcg_fft_fwd(x, X)
+        ev[1].record()
+        for _ in range(reps): h.fcg_fft_inv(X, xb)
+        ev[2].record(); torch.cuda.synchronize()
+        nw = L * L * np.dtype(dt).itemsize
+        tf, ti = ev[0].elapsed_time(ev[1]) / reps, ev[1].elapsed_time(ev[2]) / reps
+        out[f"fft_L{L}_{'f64' if dt == np.float64 else 'f32'}"] = {"fwd_us": 1e3 * tf, "inv_us": 1e3 * ti, "fwd_gbs": 4 * nw / (tf * 1e-3) / 1e9,
+                                                                   "inv_gbs": 4 * nw / (ti * 1e-3) / 1e9,
+                                                                   "note": "classic passes + public half-spectrum layout kernels; bytes = 4 N w per transform"}
+        h.close()
+    w = inputs.config(2)
+    h = binding.Fcg(w.L, torch.float64)
+    k, u, t = to(w.k), to(inputs.fft_field(w.L)), to(inputs.thresholds(w.L))
+    h.fcg_break_step(k, u, t)
+    torch.cuda.synchronize(); t0 = time.perf_counter()
+    for _ in range(20): h.fcg_break_step(k, u, t)
+    out["break_step_L2048_f64"] = {"us_per_call_incl_host_sync": 1e6 * (time.perf_counter() - t0) / 20, "bytes": 3 * w.N * 8}
+    h.close()
+    w3 = inputs.config(3, nsteps=200)
+    h = binding.Fcg(w3.L, torch.float64); h.fcg_set_spectrum(to(w3.s))
+    k, f, u, t = to(w3.k), to(w3.f), to(w3.u0), to(w3.t)
+    torch.cuda.synchronize(); t0 = time.perf_counter()
+    index, iters, done, st = h.fcg_fracture(k, f, u, t, 200, w3.tol, w3.maxit)
+    dt_s = time.perf_counter() - t0
+    out["fracture_cfg3_first200"] = {"steps": int(done), "cg_iterations": int(iters.sum()), "wall_s": dt_s,
+                                     "us_per_cg_iteration": 1e6 * dt_s / max(int(iters.sum()), 1), "status": int(st)}
+    h.close()
+    return out
+
+
+def aggregate_over_ranks(dist, torch, step_ms, total_it, launches, e2e_iter_s, device):
+    """Replicas only: whole-job time = MAX over ranks of the device time, whole-job work = SUM over ranks.
+    `dist` is torch.distributed with an initialised group (nccl on the GPU box, gloo in the CPU test) or None for one rank."""
+    if dist is None:
+        return float(step_ms), int(total_it), int(launches), float(e2e_iter_s)
+    t = torch.tensor([step_ms], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    c = torch.tensor([total_it, launches, e2e_iter_s], dtype=torch.float64, device=device)
+    dist.all_reduce(c, op=dist.ReduceOp.SUM)
+    return float(t.item()), int(round(c[0].item())), int(round(c[1].item())), float(c[2].item())
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -199,13 +254,8 @@ def main():
     clocks = sampler.stop() if sampler else None
 
     # replicas only: every rank solves its own copy; time = max over ranks, value = sum of work
-    step_ms = sum(res["dev_ms"]); total_it = sum(res["iters"]); launches = res["launches"]
-    if world > 1:
-        t = torch.tensor([step_ms], dtype=torch.float64, device="cuda"); dist.all_reduce(t, op=dist.ReduceOp.MAX); step_ms = float(t.item())
-        c = torch.tensor([total_it, launches], dtype=torch.float64, device="cuda"); dist.all_reduce(c, op=dist.ReduceOp.SUM)
-        total_it, launches = int(c[0].item()), int(c[1].item())
-        e = torch.tensor([res["e2e_iter_s"]], dtype=torch.float64, device="cuda"); dist.all_reduce(e, op=dist.ReduceOp.SUM)
-        res["e2e_iter_s"] = float(e.item())
+    step_ms, total_it, launches, res["e2e_iter_s"] = aggregate_over_ranks(
+        dist if world > 1 else None, torch, sum(res["dev_ms"]), sum(res["iters"]), res["launches"], res["e2e_iter_s"], "cuda")
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -222,7 +272,7 @@ def main():
     tpath = os.path.join(ROOT, "profiles", "traffic.json")          # dram bytes per launch from the committed ncu --set full capture
     if os.path.exists(tpath):
         try:
-            traffic = json.load(open(tpath)).get(f"L{w.L}_{args.dtype}", {}).get(dom)
+            traffic = json.load(open(tpath)).get(f"L{w.L}_{args.dtype}", {}).get(dom)     # cold-cache figure (profiles/r1_notes.md)
         except Exception:
             traffic = None
     line = {
@@ -258,6 +308,7 @@ def main():
                                                "us_per_iteration": t2, "iteration_gbs_16p5": B_ITER_NW * nw2 / (t2 * 1e-6) / 1e9,
                                                "frac_of_measured_peak": B_ITER_NW * nw2 / (t2 * 1e-6) / 1e9 / hbm_peak,
                                                "kernel_us": {n: 1e3 * r2["kernel_ms"][n] for n in PASS_NAMES}, "e2e_iter_per_s": r2["e2e_iter_s"]}
+        extra.update(bench_extras(binding, torch, inputs))
         line["extra"] = extra
     if not args.no_cpu_baseline and world == 1:
         v, dt, cores = oracle_sample(w, args.ref_iters)

@@ -1,13 +1,14 @@
 // fcg_async.cuh -- the three transform passes of one operator application (Listing 4) with their
 // fused vector work (Listing 2), written for sm_100a's asynchronous copy engine:
 //
-//   * one CTA per transform (P::NT threads), several CTAs resident per SM, so that one CTA's copies are in flight
-//     while its neighbours run butterflies;
+//   * persistent CTAs, one transform (P::NT consumer threads) in flight per CTA, 2-4 CTAs resident per SM;
 //   * every global read arrives through TMA (cp.async.bulk / cp.async.bulk.tensor) into shared memory and signals
 //     an mbarrier: no register staging, no load latency on the instruction stream, depth bounded by shared memory;
-//   * vectors that are read strip-wise (p, r, u in P1; k, p in P3) stream through a small ring of shared-memory
-//     slots that lives inside the transform's own work buffer while that buffer is idle;
-//   * the column pass runs in place in shared memory and leaves through one bulk store;
+//   * vectors that are read strip-wise (p, r, u in P1; k, p in P3) stream through rings of shared-memory slots beside
+//     the transform's work buffer; producer warps keep the rings full ACROSS transforms, so the next transform's
+//     inputs land while the current one is in its butterfly stages;
+//   * T is kept in the line layout T2 (AsyncShape): the row passes move whole 128-byte lines, the
+//     column pass gathers / scatters its column with 4-D TMA tensor copies and runs in place in shared memory;
 //   * twiddles: one base twiddle per butterfly in registers + powers (fcg_engine.cuh), no table traffic.
 //
 // Every hand-over between the threads' own (generic-proxy) accesses to a shared-memory slot and a TMA (async-proxy)
@@ -17,9 +18,9 @@
 // still-queued ld.shared can be overtaken by the refill (measured, see fcg_tma.cuh).  bar.sync is used between
 // butterfly stages only.
 //
-// Same mathematics, data layout (T[n][a], packed n=0/L/2 column, digit-reversed spectrum) and modes as
-// fcg_passes.cuh, which remains the path for small lattices (NT < 64) and the host-replayable statement of the
-// index algebra.  Byte counts per launch: DESIGN.md section 4.
+// Same mathematics (two rows per complex transform, packed n = 0 / L/2 column, digit-reversed spectrum) and modes as
+// fcg_passes.cuh, which remains the path for small lattices (NT < 64), for the stand-alone transforms, and the
+// host-replayable statement of the index algebra.  Byte counts per launch: DESIGN.md section 4.
 #pragma once
 #include <cuda.h>
 #include "fcg_kernels.cuh"
@@ -103,7 +104,7 @@ template <typename P> constexpr int per_max() {
 }
 
 // --------------------------------------------------------------------------------------------- P1
-//   [u += alpha p;  p = r + beta p;]   T[n][a0], T[n][a0+1] = row transforms of rows a0, a0+1 of p (or x)
+//   [u += alpha p;  p = r + beta p;]   columns of T2 at row pair a0/2 = row transforms of rows a0, a0+1 of p (or x)
 // Persistent: grid = nsm x CTAS; the CTAs that share an SM (blockIdx % nsm, the usual placement) take the row pairs
 // s, s+nsm, s+2nsm, .. in turn, so every SM gets floor or ceil of (L/2)/nsm transforms.
 // Warp-specialised: NT consumer threads + one producer warp that only issues the strip copies, so the ring runs

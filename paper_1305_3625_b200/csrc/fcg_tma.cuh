@@ -1,6 +1,6 @@
 // fcg_tma.cuh -- sm_100a asynchronous-copy primitives used by the pipelined passes (fcg_async.cuh):
 // mbarrier (transaction-count completion), TMA bulk copies global <-> shared (cp.async.bulk, SASS UBLKCP),
-// TMA 2D tensor tile loads (cp.async.bulk.tensor, SASS UTMALDG), proxy fences and L2 cache-policy hints.
+// TMA tensor tile loads / stores (cp.async.bulk.tensor.{2,3,4}d, SASS UTMALDG / UTMASTG), proxy fences and L2 cache-policy hints.
 // Device-only inline PTX; nothing here computes anything.
 #pragma once
 #include <cstdint>

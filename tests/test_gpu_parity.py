@@ -108,6 +108,46 @@ def test_apply_matches_oracle_all_variants(B, L, dt):
     assert seen >= 1
 
 
+@pytest.mark.parametrize("L,dt", [(512, np.float64), (1024, np.float64), (2048, np.float64), (2048, np.float32), (1024, np.float32)])
+def test_apply_both_engines(B, L, dt):
+    """FCG_OPT_ENGINE: the pipelined TMA passes (0, default where the lattice is large enough) and the classic passes (1)
+    apply the same operator; each is compared with the oracle and with the other."""
+    s = inputs.spectrum(L, dt); k = inputs.uniform_k(L).astype(dt); k[inputs.broken_mask(L, 10)] = 0
+    x = inputs.fft_field(L).astype(dt)
+    y_or = orc.apply(s, k, x)
+    ys = []
+    for eng in (0, 1):
+        h = handle(B, L, dt, s, FCG_OPT_ENGINE=eng)
+        for rep in range(3):                                   # repeated launches: the TMA rings must not leak state
+            y = h.fcg_apply(dev(k), dev(x)).cpu().numpy()
+            assert rel(y, y_or) <= TOL_OP[dt], (eng, rep)
+        ys.append(y)
+        h.close()
+    assert rel(ys[0], ys[1]) <= TOL_OP[dt]
+
+
+def test_engine_switch_invalidates_spectrum(B):
+    """The stored spectrum's layout belongs to the engine (include/fcg.h): switching needs a new fcg_set_spectrum."""
+    L = 512
+    w = inputs.config(0, L=L)
+    h = handle(B, L, np.float64, w.s)
+    y0 = h.fcg_apply(dev(w.k), dev(w.f)).cpu().numpy()
+    h.fcg_set_option(B.FCG_OPT_ENGINE, 1)
+    with pytest.raises(B.FcgError) as ei:
+        h.fcg_apply(dev(w.k), dev(w.f))
+    assert ei.value.status == B.FCG_NO_SPECTRUM
+    h.fcg_set_spectrum(dev(w.s))
+    y1 = h.fcg_apply(dev(w.k), dev(w.f)).cpu().numpy()
+    assert rel(y1, y0) <= 1e-12
+    h.close()
+
+
+@pytest.mark.parametrize("L,dt", [(512, np.float64), (1024, np.float32)])
+def test_cg_classic_engine(B, L, dt):
+    """The classic passes stay a complete, tested path (A/B measurements, small lattices)."""
+    cg_parity(B, inputs.config(1, dt, L=L), FCG_OPT_ENGINE=1)
+
+
 def test_apply_nonsymmetric_spectrum(B):
     L = 64
     s = np.random.default_rng(9).random((L, L)) + 0.5      # real, not even: only the even part acts (cpyReal)
