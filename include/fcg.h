@@ -58,6 +58,10 @@ typedef enum {
                                     exit early on the device flag, host polls once per chunk */
     FCG_OPT_CHUNK        = 1, /* iterations per chunk in loop mode 1 (default 16) */
     FCG_OPT_ROW_VARIANT  = 2, /* -1 (default): tuned rows-per-CTA of the classic row passes; 0,1,..: force variant */
+    FCG_OPT_UNROLL       = 4, /* loop mode 0: CG iterations per evaluation of the graph's WHILE condition (default 4, 1..64);
+                                 iterations after the stop are no-op launches, results do not depend on it */
+    FCG_OPT_PDL          = 5, /* 1: launch the loop kernels with programmatic stream serialization (the next kernel's
+                                 prologue overlaps the current kernel's tail); 0: plain stream order */
     FCG_OPT_ENGINE       = 3  /* 0 (default): pipelined TMA passes where the lattice is large enough (L >= 512), classic
                                  passes otherwise; 1: classic passes only (synchronous loads; kept for A/B measurements).
                                  The stored spectrum's layout belongs to the engine: changing the engine after

@@ -61,7 +61,7 @@ Layout make_layout(int L, size_t w) {
 }
 
 struct GraphEntry {
-    const void *k, *f; void* u; double tol; int maxit, var;
+    const void *k, *f; void* u; double tol; int maxit, var, unroll, pdl;
     cudaGraph_t graph; cudaGraphExec_t exec; unsigned long long stamp;
 };
 
@@ -74,7 +74,7 @@ struct fcg_handle_s {
     char* ws = nullptr; bool own_ws = false;
     Layout lay{};
     bool have_spectrum = false;
-    int loop_mode = 0, chunk = 16, row_var_opt = -1, engine_opt = 0, nsm = 148;
+    int loop_mode = 0, chunk = 16, row_var_opt = -1, engine_opt = 0, nsm = 148, unroll = 4, pdl = 0;
     alignas(64) CUtensorMap tmap_row;   // T2 as [L/(2 NB)][L/2][128 B]: box = v2_tsub/NB lines of one row pair (row_inv2 tiles)
     alignas(64) CUtensorMap tmap_col;   // T2 as [L/(2 NB)][L/2][NB][2 complex]: box = one column x v2_abox row pairs (col2 gather / scatter)
     bool have_tmap = false;
@@ -128,19 +128,19 @@ template <typename T> struct Seq {
     T* q() const { return h->at<T>(h->lay.q); }
 
     cudaError_t row_fwd(int mode, const T* x, T* u) const {
-        RowFwdArgs<T> A{}; A.mode = mode; A.x = x; A.u = u; A.p = p(); A.r = r(); A.Tb = Tb(); A.tw = tw(); A.sc = h->sc(); A.nsm = h->nsm;
+        RowFwdArgs<T> A{}; A.mode = mode; A.x = x; A.u = u; A.p = p(); A.r = r(); A.Tb = Tb(); A.tw = tw(); A.sc = h->sc(); A.nsm = h->nsm; A.pdl = h->pdl;
         ++h->launches;
         return v2() ? h->tab->row_fwd2(&A, st) : h->tab->row_fwd(h->row_var(), &A, st);
     }
     cudaError_t col(int mode, bool cg) const {
-        ColArgs<T> A{}; A.mode = mode; A.Tb = Tb(); A.shat = shat(); A.tw = tw(); A.sc = cg ? h->sc() : nullptr;
+        ColArgs<T> A{}; A.mode = mode; A.Tb = Tb(); A.shat = shat(); A.tw = tw(); A.sc = cg ? h->sc() : nullptr; A.pdl = h->pdl;
         ++h->launches;
         return (v2() && mode == COL_CONV) ? h->tab->col2(&A, &h->tmap_col, st) : h->tab->col(&A, st);
     }
     cudaError_t row_inv(int mode, const T* k, const T* v, const T* f, T* out, T* out2) const {
         RowInvArgs<T> A{}; A.mode = mode; A.Tb = Tb(); A.tw = tw(); A.k = k; A.v = v; A.f = f; A.out = out; A.out2 = out2;
         A.scale = (T)(1.0 / ((double)h->L * (double)h->L));
-        A.partial = h->at<double>(h->lay.partial_row); A.sc = h->sc(); A.nsm = h->nsm;
+        A.partial = h->at<double>(h->lay.partial_row); A.sc = h->sc(); A.nsm = h->nsm; A.pdl = h->pdl;
         ++h->launches;
         return v2() ? h->tab->row_inv2(&A, &h->tmap_row, st) : h->tab->row_inv(h->row_var(), &A, st);
     }
@@ -160,9 +160,14 @@ template <typename T> struct Seq {
     cudaError_t it_row_inv(const T* k) const { return row_inv(ROWI_CG, k, p(), nullptr, q(), nullptr); }   // q = A p, p.q, alpha
     cudaError_t it_update_r() const {                                                              // r, r.r, beta, convergence
         const size_t nvec = h->N / Vec<T>::W;
-        cg_update_r_kernel<T><<<h->vec_blocks(), 256, 0, st>>>(r(), q(), nvec, h->at<double>(h->lay.partial_vec), h->sc());
         ++h->launches;
-        return cudaGetLastError();
+        cudaLaunchConfig_t cfg{};
+        cfg.gridDim = dim3((unsigned)h->vec_blocks()); cfg.blockDim = dim3(256); cfg.dynamicSmemBytes = 0; cfg.stream = st;
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        at[0].val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = at; cfg.numAttrs = h->pdl ? 1u : 0u;
+        return cudaLaunchKernelEx(&cfg, cg_update_r_kernel<T>, r(), (const T*)q(), nvec, h->at<double>(h->lay.partial_vec), h->sc());
     }
     cudaError_t iteration(const T* k, T* u) const {
         cudaError_t e;
@@ -220,7 +225,9 @@ cudaError_t build_graph(fcg_handle h, GraphEntry& ge) {
     cudaGraph_t body = np.conditional.phGraph_out[0];
 
     if ((e = cudaStreamBeginCaptureToGraph(cs, body, nullptr, nullptr, 0, cudaStreamCaptureModeRelaxed)) != cudaSuccess) return e;
-    e = s.iteration((const T*)ge.k, (T*)ge.u);
+    // `unroll` iterations per evaluation of the WHILE condition (each evaluation costs ~6 us on B200); once the device flag
+    // is set the remaining kernels of the body return at once without touching anything
+    for (int r = 0; r < ge.unroll && e == cudaSuccess; ++r) e = s.iteration((const T*)ge.k, (T*)ge.u);
     e3 = cudaStreamEndCapture(cs, &tmp);
     if (e != cudaSuccess) return e;
     if (e3 != cudaSuccess) return e3;
@@ -242,14 +249,14 @@ int solve_impl(fcg_handle h, const void* k, const void* f, void* u, double tol, 
         const int var = h->v2() ? 100 : h->row_var();
         GraphEntry* hit = nullptr;
         for (auto& g : h->graphs)
-            if (g.k == k && g.f == f && g.u == u && g.tol == tol && g.maxit == maxit && g.var == var) { hit = &g; break; }
+            if (g.k == k && g.f == f && g.u == u && g.tol == tol && g.maxit == maxit && g.var == var && g.unroll == h->unroll && g.pdl == h->pdl) { hit = &g; break; }
         if (!hit) {
             if (h->graphs.size() >= 8) {
                 size_t lru = 0;
                 for (size_t i = 1; i < h->graphs.size(); ++i) if (h->graphs[i].stamp < h->graphs[lru].stamp) lru = i;
                 drop_graph(h->graphs[lru]); h->graphs.erase(h->graphs.begin() + lru);
             }
-            GraphEntry ge{k, f, u, tol, maxit, var, nullptr, nullptr, 0};
+            GraphEntry ge{k, f, u, tol, maxit, var, h->unroll, h->pdl, nullptr, nullptr, 0};
             cudaError_t e = build_graph<T>(h, ge);
             if (e != cudaSuccess) {
                 // conditional graph nodes unavailable: fall back to direct launches for the rest of this handle's life
@@ -268,7 +275,8 @@ int solve_impl(fcg_handle h, const void* k, const void* f, void* u, double tol, 
             hit->stamp = ++h->stamp;
             FCG_CK(h, cudaGraphLaunch(hit->exec, h->stream));
             FCG_CK(h, cudaStreamSynchronize(h->stream));
-            h->launches = 5 + 4LL * h->h_sc->it;
+            const long long U = hit->unroll;
+            h->launches = 5 + 4LL * U * ((h->h_sc->it + U - 1) / U);      // no-op kernels after the stop are launches too
         }
     }
     if (h->loop_mode != 0) {
@@ -482,6 +490,8 @@ int fcg_set_option(fcg_handle h, int option, int value) {
         case FCG_OPT_ROW_VARIANT:
             if (value >= FCG_NROWVAR || (value >= 0 && !h->tab->row_valid[value])) return fail(h, FCG_INVALID_ARG, "row variant not available for this size");
             h->row_var_opt = value; return FCG_OK;
+        case FCG_OPT_PDL: if (value != 0 && value != 1) return fail(h, FCG_INVALID_ARG, "pdl must be 0 or 1"); h->pdl = value; return FCG_OK;
+        case FCG_OPT_UNROLL: if (value < 1 || value > 64) return fail(h, FCG_INVALID_ARG, "unroll must be 1..64"); h->unroll = value; return FCG_OK;
         case FCG_OPT_ENGINE:
             if (value != 0 && value != 1) return fail(h, FCG_INVALID_ARG, "engine must be 0 or 1");
             h->engine_opt = value;

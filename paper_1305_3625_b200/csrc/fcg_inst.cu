@@ -49,6 +49,18 @@ template <typename T> struct Inst {
         }
         return prep(col_kernel<T, P, CS::COLS>, CS::smem);
     }
+    // launch, optionally with programmatic stream serialization (the kernels call griddepcontrol.wait before their first
+    // dependent access, so the next kernel's prologue overlaps this one's tail)
+    template <typename K, typename... Args>
+    static cudaError_t launch(K kernel, int grid, int block, size_t smem, cudaStream_t st, int pdl, Args... args) {
+        cudaLaunchConfig_t cfg{};
+        cfg.gridDim = dim3((unsigned)grid); cfg.blockDim = dim3((unsigned)block); cfg.dynamicSmemBytes = smem; cfg.stream = st;
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        at[0].val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = at; cfg.numAttrs = pdl ? 1u : 0u;
+        return cudaLaunchKernelEx(&cfg, kernel, args...);
+    }
     // persistent grid: CTAS CTAs on each of nsm SMs, but never more CTAs than transforms (whole multiples of nsm)
     static int pgrid(int nsm, int ctas) {
         int k = ctas;
@@ -58,24 +70,22 @@ template <typename T> struct Inst {
     static cudaError_t row_fwd2(const void* args, cudaStream_t st) {
         if constexpr (V2) {
             const RowFwdArgs<T>& A = *static_cast<const RowFwdArgs<T>*>(args);
-            row_fwd2_kernel<T, P, C_FWD><<<pgrid(A.nsm, C_FWD), P::NT + 32, AS::fwd_smem, st>>>(A);
-            return cudaGetLastError();
+            return launch(row_fwd2_kernel<T, P, C_FWD>, pgrid(A.nsm, C_FWD), P::NT + 32, AS::fwd_smem, st, A.pdl, A);
         }
         return cudaErrorInvalidValue;
     }
     static cudaError_t col2(const void* args, const void* tensor_map, cudaStream_t st) {
         if constexpr (V2) {
-            col2_kernel<T, P, C_COL><<<L / 2, P::NT, AS::col_smem, st>>>(*static_cast<const ColArgs<T>*>(args),
-                                                                         *static_cast<const CUtensorMap*>(tensor_map));
-            return cudaGetLastError();
+            const ColArgs<T>& A = *static_cast<const ColArgs<T>*>(args);
+            return launch(col2_kernel<T, P, C_COL>, L / 2, P::NT, AS::col_smem, st, A.pdl, A, *static_cast<const CUtensorMap*>(tensor_map));
         }
         return cudaErrorInvalidValue;
     }
     static cudaError_t row_inv2(const void* args, const void* tensor_map, cudaStream_t st) {
         if constexpr (V2) {
             const RowInvArgs<T>& A = *static_cast<const RowInvArgs<T>*>(args);
-            row_inv2_kernel<T, P, C_INV><<<pgrid(A.nsm, C_INV), AS::INV_THREADS, AS::inv_smem, st>>>(A, *static_cast<const CUtensorMap*>(tensor_map));
-            return cudaGetLastError();
+            return launch(row_inv2_kernel<T, P, C_INV>, pgrid(A.nsm, C_INV), AS::INV_THREADS, AS::inv_smem, st, A.pdl, A,
+                          *static_cast<const CUtensorMap*>(tensor_map));
         }
         return cudaErrorInvalidValue;
     }

@@ -174,6 +174,8 @@ __global__ void __launch_bounds__(256) cg_update_r_kernel(T* __restrict__ r, con
                                                            double* partial, Scalars* sc) {
     __shared__ double red[32];
     using V = typename Vec<T>::type;
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");    // programmatic dependent launch (fcg_tma.cuh)
+    asm volatile("griddepcontrol.wait;" ::: "memory");
     if (sc->done) {      // breakdown in this iteration, or (loop mode 1) already finished
         if (blockIdx.x == 0 && threadIdx.x == 0) set_cond(sc, false);
         return;

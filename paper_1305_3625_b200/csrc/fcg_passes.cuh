@@ -42,6 +42,7 @@ template <typename T> struct RowFwdArgs {
     const cx<T>* tw;       // per-stage twiddle tables (Plan::tw_off)
     const Scalars* sc;
     int nsm;               // SMs of the device (persistent passes: tile assignment)
+    int pdl;               // host side: launch with programmatic stream serialization
 };
 
 template <typename T> struct ColArgs {
@@ -50,6 +51,7 @@ template <typename T> struct ColArgs {
     const T* shat;         // [(L/2)+1][L], digit-reversed along m, pre-scaled by 1/L^2
     const cx<T>* tw;
     const Scalars* sc;
+    int pdl;
 };
 
 template <typename T> struct RowInvArgs {
@@ -62,6 +64,7 @@ template <typename T> struct RowInvArgs {
     double* partial;                      // [gridDim.x][2]
     Scalars* sc;
     int nsm;
+    int pdl;
 };
 
 template <int A, int B, typename F> FCG_HD void static_for_up(F&& f) {

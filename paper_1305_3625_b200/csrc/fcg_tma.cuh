@@ -129,6 +129,11 @@ __device__ __forceinline__ void tensor_s2g_4d(const void* tmap, int c0, int c1, 
 __device__ __forceinline__ void prefetch_tmap(const void* tmap) {
     asm volatile("prefetch.tensormap [%0];" ::"l"(tmap) : "memory");
 }
+// Programmatic dependent launch: let the next kernel of the stream start its prologue while this grid drains
+// (launch_dependents), and block until the previous grid has completed and its writes are visible (wait).  Both are
+// no-ops for a kernel launched without the programmatic-serialization attribute.
+__device__ __forceinline__ void grid_dep_launch() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void grid_dep_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 // generic-proxy writes to shared memory -> visible to the async proxy (before a bulk store reads them)
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 

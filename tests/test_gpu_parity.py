@@ -170,7 +170,7 @@ def cg_parity(B, w, **opts):
     it, rr, st = h.fcg_solve(kd, fd, u, w.tol, w.maxit)
     assert st == ref["status"]
     assert abs(it - ref["iters"]) <= 2, (it, ref["iters"], ref["hist"][-4:])
-    assert h.fcg_last_launch_count() == 5 + 4 * it or opts
+    assert h.fcg_last_launch_count() == 5 + 16 * ((it + 3) // 4) or opts      # set-up 4 + finish 1 + 4 kernels x (iterations rounded up to the WHILE body's 4)
     u_nat = u.cpu().numpy()
     d_nat = rel(u_nat, ref["u"])
     d_pin = d_nat
@@ -214,8 +214,8 @@ def test_cg_loop_modes_and_determinism(B):
     """Graph-WHILE and direct-launch modes run the same kernels: bit-identical u, and repeated runs agree bitwise."""
     w = inputs.config(1, L=256)
     outs = []
-    for mode, chunk in ((0, 16), (0, 16), (1, 16), (1, 5)):
-        h = handle(B, w.L, np.float64, w.s, FCG_OPT_LOOP_MODE=mode, FCG_OPT_CHUNK=chunk)
+    for mode, chunk, unroll in ((0, 16, 4), (0, 16, 1), (0, 16, 7), (1, 16, 4), (1, 5, 4)):
+        h = handle(B, w.L, np.float64, w.s, FCG_OPT_LOOP_MODE=mode, FCG_OPT_CHUNK=chunk, FCG_OPT_UNROLL=unroll)
         u = dev(w.u0)
         it, rr, st = h.fcg_solve(dev(w.k), dev(w.f), u, w.tol, w.maxit)
         outs.append((it, rr, st, u.cpu().numpy().copy()))
