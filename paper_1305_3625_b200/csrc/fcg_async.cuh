@@ -31,7 +31,7 @@ namespace fcg {
 
 template <typename T, typename P> struct AsyncShape {
     static constexpr int L = P::N, NT = P::NT, R1 = P::radix(1), Q1 = L / R1, PER1 = Q1 / NT;
-    static constexpr bool valid = NT >= 64 && L >= 512;
+    static constexpr bool valid = NT >= 64 && L >= 256;
     static constexpr size_t WBYTES = (size_t)L * 2 * sizeof(T);              // one complex transform (work buffer)
     static constexpr uint32_t PIECE = (uint32_t)(Q1 * sizeof(T));            // one stage-1 strip of one real row
     static constexpr int MAXSLOT = 16;

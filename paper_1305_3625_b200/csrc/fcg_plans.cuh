@@ -17,9 +17,9 @@ FCG_PLAN(double, 16, 4, 4, 1, 1)      FCG_PLAN(float, 16, 4, 4, 1, 1)
 FCG_PLAN(double, 32, 4, 8, 1, 1)      FCG_PLAN(float, 32, 4, 8, 1, 1)
 FCG_PLAN(double, 64, 8, 8, 1, 1)      FCG_PLAN(float, 64, 4, 16, 1, 1)
 FCG_PLAN(double, 128, 16, 8, 1, 1)    FCG_PLAN(float, 128, 8, 16, 1, 1)
-FCG_PLAN(double, 256, 16, 16, 1, 1)   FCG_PLAN(float, 256, 16, 16, 1, 1)
+FCG_PLAN(double, 256, 4, 4, 4, 4)     FCG_PLAN(float, 256, 4, 4, 4, 4)
 FCG_PLAN(double, 512, 8, 8, 8, 1)     FCG_PLAN(float, 512, 4, 8, 16, 1)
-FCG_PLAN(double, 1024, 16, 8, 8, 1)   FCG_PLAN(float, 1024, 8, 8, 16, 1)
+FCG_PLAN(double, 1024, 8, 8, 4, 4)   FCG_PLAN(float, 1024, 8, 8, 16, 1)
 FCG_PLAN(double, 2048, 16, 16, 8, 1)  FCG_PLAN(float, 2048, 8, 16, 16, 1)
 FCG_PLAN(double, 4096, 16, 16, 16, 1) FCG_PLAN(float, 4096, 16, 16, 16, 1)
 FCG_PLAN(double, 8192, 16, 8, 8, 8)   FCG_PLAN(float, 8192, 8, 8, 8, 16)
