@@ -176,7 +176,7 @@ def bench_extras(binding, torch, inputs):
         tf, ti = ev[0].elapsed_time(ev[1]) / reps, ev[1].elapsed_time(ev[2]) / reps
         out[f"fft_L{L}_{'f64' if dt == np.float64 else 'f32'}"] = {"fwd_us": 1e3 * tf, "inv_us": 1e3 * ti, "fwd_gbs": 4 * nw / (tf * 1e-3) / 1e9,
                                                                    "inv_gbs": 4 * nw / (ti * 1e-3) / 1e9,
-                                                                   "note": "classic passes + public half-spectrum layout kernels; bytes = 4 N w per transform"}
+                                                                   "note": "row pass + column pass + layout kernel; bytes = 4 N w per transform"}
         h.close()
     w = inputs.config(2)
     h = binding.Fcg(w.L, torch.float64)

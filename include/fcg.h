@@ -62,7 +62,7 @@ typedef enum {
                                  iterations after the stop are no-op launches, results do not depend on it */
     FCG_OPT_PDL          = 5, /* 1: launch the loop kernels with programmatic stream serialization (the next kernel's
                                  prologue overlaps the current kernel's tail); 0: plain stream order */
-    FCG_OPT_ENGINE       = 3  /* 0 (default): pipelined TMA passes where the lattice is large enough (L >= 512), classic
+    FCG_OPT_ENGINE       = 3  /* 0 (default): pipelined TMA passes where the lattice is large enough (L >= 256), classic
                                  passes otherwise; 1: classic passes only (synchronous loads; kept for A/B measurements).
                                  The stored spectrum's layout belongs to the engine: changing the engine after
                                  fcg_set_spectrum requires calling fcg_set_spectrum again (FCG_NO_SPECTRUM otherwise) */

@@ -313,8 +313,23 @@ int break_impl(fcg_handle h, void* k, const void* u, const void* t, long long* i
 
 template <typename T>
 int fft_impl(fcg_handle h, const void* in, void* out, bool inverse) {
-    Seq<T> s{h, h->stream, true};       // public half-spectrum layout goes through the classic T[n][a] passes
     const int L = h->L;
+    if (h->v2()) {
+        // pipelined passes on the T2 layout; T2 <-> public half spectrum X[m][n] by one line-wise permutation kernel
+        Seq<T> s{h, h->stream};
+        ColArgs<T> CA{}; CA.mode = inverse ? COL_INV : COL_FWD; CA.Tb = s.Tb(); CA.tw = s.tw();
+        if (!inverse) {
+            FCG_CK(h, s.row_fwd(ROWF_PLAIN, (const T*)in, nullptr));
+            FCG_CK(h, h->tab->col2_xform(&CA, &h->tmap_col, 0, h->stream));
+            FCG_CK(h, h->tab->t2_export(s.Tb(), out, h->stream));
+        } else {
+            FCG_CK(h, h->tab->t2_import(in, s.Tb(), h->stream));
+            FCG_CK(h, h->tab->col2_xform(&CA, &h->tmap_col, 1, h->stream));
+            FCG_CK(h, s.row_inv(ROWI_PLAIN, nullptr, nullptr, nullptr, (T*)out, nullptr));
+        }
+        return FCG_OK;
+    }
+    Seq<T> s{h, h->stream, true};       // classic T[n][a] passes + transposing layout kernels
     dim3 blk(32, 8), grd((L / 2 + 31) / 32, (L + 31) / 32);
     if (!inverse) {
         FCG_CK(h, s.row_fwd(ROWF_PLAIN, (const T*)in, nullptr));

@@ -348,6 +348,154 @@ __global__ void __launch_bounds__(P::NT, CTAS) col2_kernel(const ColArgs<T> A, c
     }
 }
 
+// --------------------------------------------------------------------------------------------- stand-alone transforms
+// Column pass of fcg_fft_fwd / fcg_fft_inv on the T2 layout: forward only (DIR < 0, natural row-frequency order out) or
+// inverse only (DIR > 0, natural order in).  Same gather / in-place / scatter plumbing as col2_kernel; kept as a kernel
+// of its own so that the loop kernel's register allocation is not disturbed.
+template <typename T, typename P, int CTAS, int DIR>
+__global__ void __launch_bounds__(P::NT, CTAS) col2_xform_kernel(const ColArgs<T> A, const __grid_constant__ CUtensorMap tmap)
+{
+    using AS = AsyncShape<T, P>;
+    constexpr int L = P::N, S = P::S, NT = P::NT, PM = per_max<P>(), EPT = L / NT;
+    extern __shared__ unsigned char smem_dyn[];
+    unsigned char* const smem_raw = align128(smem_dyn);
+    __shared__ __align__(8) uint64_t bar, ready;
+    cx<T>* W = reinterpret_cast<cx<T>*>(smem_raw);
+    SmemIO<T, P> io{W};
+    const int lt = threadIdx.x, n = (int)blockIdx.x;
+    constexpr int ABOX = AS::ABOX;
+    constexpr uint32_t BOXB = (uint32_t)(ABOX * 2 * sizeof(cx<T>));
+    if (lt == 0) {
+        tma::prefetch_tmap(&tmap);
+        tma::mbar_init(&bar, 1);
+        tma::mbar_init(&ready, NT / 32);
+        tma::fence_mbar_init();
+        tma::mbar_expect_tx(&bar, (uint32_t)AS::WBYTES);
+#pragma unroll
+        for (int b = 0; b < (L / 2) / ABOX; ++b)
+            tma::tensor_g2s_4d(smem_raw + (size_t)b * BOXB, &tmap, 0, n % AS::NB, b * ABOX, n / AS::NB, &bar);
+    }
+    __syncthreads();
+    cx<T> wb[S + 1][PM];
+    static_for_up<1, S - 1>([&](auto s) { base_tw<P, decltype(s)::value, T>(lt, A.tw, wb[decltype(s)::value]); });
+    tma::mbar_wait(&bar, 0);
+    auto ld_sw = [&](int e) { return io.ld(e); };
+    auto st_sw = [&](int e, cx<T> v) { io.st(e, v); };
+    if constexpr (DIR < 0) {
+        {   // stage 1: linear in, swizzled out
+            cx<T> a[St<P, 1>::PER][St<P, 1>::R];
+            stage_ld<P, 1, T>(lt, [&](int e) { return W[e]; }, a);
+            __syncthreads();
+            stage_math<P, 1, -1, T>(a, wb[1]);
+            stage_st<P, 1, T>(lt, st_sw, a);
+            __syncthreads();
+        }
+        static_for_up<2, S>([&](auto s) {
+            constexpr int sv = decltype(s)::value;
+            cx<T> a[St<P, sv>::PER][St<P, sv>::R];
+            stage_ld<P, sv, T>(lt, ld_sw, a);
+            stage_math<P, sv, -1, T>(a, wb[sv]);
+            stage_st<P, sv, T>(lt, st_sw, a);
+            __syncthreads();
+        });
+        cx<T> v[EPT];                       // digit-reversed -> natural order, through registers
+#pragma unroll
+        for (int i = 0; i < EPT; ++i) v[i] = io.ld(P::pos_of(lt + i * NT));
+        __syncthreads();
+#pragma unroll
+        for (int i = 0; i < EPT; ++i) W[lt + i * NT] = v[i];
+    } else {
+        cx<T> v[EPT];                       // natural order -> digit-reversed positions
+#pragma unroll
+        for (int i = 0; i < EPT; ++i) v[i] = W[lt + i * NT];
+        __syncthreads();
+#pragma unroll
+        for (int i = 0; i < EPT; ++i) io.st(P::pos_of(lt + i * NT), v[i]);
+        __syncthreads();
+        static_for_down<S, 2>([&](auto s) {
+            constexpr int sv = decltype(s)::value;
+            cx<T> a[St<P, sv>::PER][St<P, sv>::R];
+            stage_ld<P, sv, T>(lt, ld_sw, a);
+            stage_math<P, sv, +1, T>(a, wb[sv]);
+            stage_st<P, sv, T>(lt, st_sw, a);
+            __syncthreads();
+        });
+        cx<T> a[St<P, 1>::PER][St<P, 1>::R];
+        stage_ld<P, 1, T>(lt, ld_sw, a);
+        stage_math<P, 1, +1, T>(a, wb[1]);
+        __syncthreads();
+        stage_st<P, 1, T>(lt, [&](int e, cx<T> x) { W[e] = x; }, a);
+    }
+    tma::fence_proxy_async();
+    tma::mbar_warp_arrive(&ready);
+    if (lt == 0) {
+        tma::mbar_wait(&ready, 0);
+#pragma unroll
+        for (int b = 0; b < (L / 2) / ABOX; ++b)
+            tma::tensor_s2g_4d(&tmap, 0, n % AS::NB, b * ABOX, n / AS::NB, smem_raw + (size_t)b * BOXB);
+        tma::bulk_commit();
+        tma::bulk_wait_read0();
+    }
+}
+
+// T2 (columns in position order, row frequencies m in natural order after col2_xform<-1>) -> public half spectrum
+// X[m][n], n = 0 .. L/2.  One CTA per row pair (m = 2A, 2A+1): its L complex numbers are whole 128-byte lines of T2; they are
+// permuted to frequency order through shared memory and leave as two contiguous rows.  The packed column 0 (W = Y0 + i YN)
+// is unpacked with its mirror row L - m, read straight from T2.
+template <typename T, typename P>
+__global__ void __launch_bounds__(256) t2_export_kernel(const cx<T>* __restrict__ T2, cx<T>* __restrict__ X)
+{
+    using AS = AsyncShape<T, P>;
+    constexpr int L = P::N, XW = L / 2 + 1, SK = L / P::radix(1);     // consecutive frequencies sit SK tile entries apart: skew them
+    auto sk = [](int i) { return i + i / SK; };
+    extern __shared__ unsigned char smem_dyn[];
+    cx<T>* tile = reinterpret_cast<cx<T>*>(smem_dyn);                 // [m][r]
+    const int A2 = (int)blockIdx.x, tid = threadIdx.x;
+    for (int i = tid; i < L; i += 256) {                               // i = 2 m + r; 2 NB consecutive i are one line
+        const int m = i >> 1;
+        tile[sk(i)] = T2[AS::t2_index(m, A2) + (i & 1)];
+    }
+    __syncthreads();
+    const T h = (T)0.5;
+    for (int i = tid; i < 2 * XW; i += 256) {
+        const int r = i / XW, nn = i % XW, mrow = 2 * A2 + r;
+        cx<T> out;
+        if (nn == 0 || nn == L / 2) {
+            const int mm = (L - mrow) % L;
+            const cx<T> a = tile[sk(r)], b = T2[AS::t2_index(0, mm >> 1) + (mm & 1)];
+            out = nn == 0 ? mk<T>((a.x + b.x) * h, (a.y - b.y) * h) : mk<T>((a.y + b.y) * h, (b.x - a.x) * h);
+        } else {
+            out = tile[sk(2 * AS::col_of_pos(P::pos_of(nn)) + r)];
+        }
+        X[(size_t)mrow * XW + nn] = out;
+    }
+}
+
+// public half spectrum -> T2 (the inverse of t2_export_kernel)
+template <typename T, typename P>
+__global__ void __launch_bounds__(256) t2_import_kernel(const cx<T>* __restrict__ X, cx<T>* __restrict__ T2)
+{
+    using AS = AsyncShape<T, P>;
+    constexpr int L = P::N, XW = L / 2 + 1, SK = L / P::radix(1);
+    auto sk = [](int i) { return i + i / SK; };
+    extern __shared__ unsigned char smem_dyn[];
+    cx<T>* tile = reinterpret_cast<cx<T>*>(smem_dyn);                 // [m][r]
+    const int A2 = (int)blockIdx.x, tid = threadIdx.x;
+    for (int i = tid; i < 2 * XW; i += 256) {
+        const int r = i / XW, nn = i % XW, mrow = 2 * A2 + r;
+        if (nn == L / 2) continue;
+        const cx<T> v = X[(size_t)mrow * XW + nn];
+        if (nn == 0) {
+            const cx<T> xN = X[(size_t)mrow * XW + L / 2];
+            tile[sk(r)] = mk<T>(v.x - xN.y, v.y + xN.x);
+        } else {
+            tile[sk(2 * AS::col_of_pos(P::pos_of(nn)) + r)] = v;
+        }
+    }
+    __syncthreads();
+    for (int i = tid; i < L; i += 256) T2[AS::t2_index(i >> 1, A2) + (i & 1)] = tile[sk(i)];
+}
+
 // --------------------------------------------------------------------------------------------- P3
 //   c = F_row^H T (rows a0, a0+1);  q = k o p + c  [+ partial p.q]   (or residual / apply / plain)
 // Persistent and warp-specialised like P1.  The producer warp feeds two rings in consumption order: tiles of T2

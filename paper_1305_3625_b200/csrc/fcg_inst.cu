@@ -46,6 +46,10 @@ template <typename T> struct Inst {
             if ((e = prep(row_fwd2_kernel<T, P, C_FWD>, AS::fwd_smem)) != cudaSuccess) return e;
             if ((e = prep(col2_kernel<T, P, C_COL>, AS::col_smem)) != cudaSuccess) return e;
             if ((e = prep(row_inv2_kernel<T, P, C_INV>, AS::inv_smem)) != cudaSuccess) return e;
+            if ((e = prep(col2_xform_kernel<T, P, C_COL, -1>, AS::WBYTES + 128)) != cudaSuccess) return e;
+            if ((e = prep(col2_xform_kernel<T, P, C_COL, +1>, AS::WBYTES + 128)) != cudaSuccess) return e;
+            if ((e = prep(t2_export_kernel<T, P>, AS::WBYTES + 1024)) != cudaSuccess) return e;
+            if ((e = prep(t2_import_kernel<T, P>, AS::WBYTES + 1024)) != cudaSuccess) return e;
         }
         return prep(col_kernel<T, P, CS::COLS>, CS::smem);
     }
@@ -78,6 +82,30 @@ template <typename T> struct Inst {
         if constexpr (V2) {
             const ColArgs<T>& A = *static_cast<const ColArgs<T>*>(args);
             return launch(col2_kernel<T, P, C_COL>, L / 2, P::NT, AS::col_smem, st, A.pdl, A, *static_cast<const CUtensorMap*>(tensor_map));
+        }
+        return cudaErrorInvalidValue;
+    }
+    static cudaError_t col2_xform(const void* args, const void* tensor_map, int inverse, cudaStream_t st) {
+        if constexpr (V2) {
+            const ColArgs<T>& A = *static_cast<const ColArgs<T>*>(args);
+            const CUtensorMap& tm = *static_cast<const CUtensorMap*>(tensor_map);
+            if (inverse) col2_xform_kernel<T, P, C_COL, +1><<<L / 2, P::NT, AS::WBYTES + 128, st>>>(A, tm);
+            else col2_xform_kernel<T, P, C_COL, -1><<<L / 2, P::NT, AS::WBYTES + 128, st>>>(A, tm);
+            return cudaGetLastError();
+        }
+        return cudaErrorInvalidValue;
+    }
+    static cudaError_t t2_export(const void* T2, void* X, cudaStream_t st) {
+        if constexpr (V2) {
+            t2_export_kernel<T, P><<<L / 2, 256, AS::WBYTES + 1024, st>>>(static_cast<const cx<T>*>(T2), static_cast<cx<T>*>(X));
+            return cudaGetLastError();
+        }
+        return cudaErrorInvalidValue;
+    }
+    static cudaError_t t2_import(const void* X, void* T2, cudaStream_t st) {
+        if constexpr (V2) {
+            t2_import_kernel<T, P><<<L / 2, 256, AS::WBYTES + 1024, st>>>(static_cast<const cx<T>*>(X), static_cast<cx<T>*>(T2));
+            return cudaGetLastError();
         }
         return cudaErrorInvalidValue;
     }
@@ -147,6 +175,7 @@ template <typename T> struct Inst {
         t.v2_ctas[0] = C_FWD; t.v2_ctas[1] = C_COL; t.v2_ctas[2] = C_INV;
         t.v2_smem[0] = AS::fwd_smem; t.v2_smem[1] = AS::col_smem; t.v2_smem[2] = AS::inv_smem;
         t.row_fwd2 = &row_fwd2; t.col2 = &col2; t.row_inv2 = &row_inv2;
+        t.col2_xform = &col2_xform; t.t2_export = &t2_export; t.t2_import = &t2_import;
         t.init = &init; t.row_fwd = &row_fwd; t.col = &col; t.row_inv = &row_inv; t.spectrum_prep = &spectrum_prep;
         return t;
     }

@@ -67,6 +67,9 @@ struct PassTable {
     cudaError_t (*row_fwd2)(const void* args, cudaStream_t st);
     cudaError_t (*col2)(const void* args, const void* tensor_map, cudaStream_t st);
     cudaError_t (*row_inv2)(const void* args, const void* tensor_map, cudaStream_t st);
+    cudaError_t (*col2_xform)(const void* args, const void* tensor_map, int inverse, cudaStream_t st);   // stand-alone transforms
+    cudaError_t (*t2_export)(const void* T2, void* X, cudaStream_t st);
+    cudaError_t (*t2_import)(const void* X, void* T2, cudaStream_t st);
 };
 
 #define FCG_DECL_TABLE(L) const PassTable* fcg_pass_table_##L(int dtype);
