@@ -201,7 +201,10 @@ __global__ void __launch_bounds__(P::NT + 32, CTAS) row_fwd2_kernel(const RowFwd
                     z[q][t] = mk<T>(sl[j], sl[Q1 + j]);
                 }
             }
-            if (i * R1 + t + NSLOT < G) tma::mbar_warp_release(&empty[slot]);   // this warp has read the slot
+            if (i * R1 + t + NSLOT < G) {                               // this warp has read the slot
+                if (cg) tma::mbar_warp_release_consumed(&empty[slot]);  // (values already used by the update above)
+                else tma::mbar_warp_release(&empty[slot]);
+            }
             if (++slot == NSLOT) { slot = 0; phase ^= 1u; }
         }
         bar_named<NT>();                                          // the previous transform's separation has left W
@@ -606,7 +609,7 @@ __global__ void __launch_bounds__(AsyncShape<T, P>::INV_THREADS, CTAS) row_inv2_
                         io.st(P::pos_of(L - n), mk<T>(X0.x + X1.y, X1.x - X0.y));
                     }
                 }
-                tma::mbar_warp_release(&tempty[ts]);                  // this warp has read the tile
+                tma::mbar_warp_release_consumed(&tempty[ts]);         // this warp has read the tile (and used every value)
                 if (!PW && warp == 0 && p_tn < GT) issue_next_T();
                 if (++ts == NTS) { ts = 0; tph ^= 1u; }
             }
@@ -651,7 +654,7 @@ __global__ void __launch_bounds__(AsyncShape<T, P>::INV_THREADS, CTAS) row_inv2_
                     }
                 }
                 if (nv) {
-                    tma::mbar_warp_release(&kempty[ks]);
+                    tma::mbar_warp_release_consumed(&kempty[ks]);
                     if (!PW && warp == 0 && p_kn < GK) issue_next_K();
                     if (++ks == nks) { ks = 0; kph ^= 1u; }
                 }

@@ -37,6 +37,12 @@ __device__ __forceinline__ void mbar_warp_release(uint64_t* bar) {
     __syncwarp();
     if ((threadIdx.x & 31) == 0) mbar_arrive(bar);
 }
+// Release without the proxy fence, for slots whose every loaded value has already been USED by an arithmetic instruction
+// of the same thread (in-order issue + scoreboard: the ld.shared has then completed before the arrival is issued).
+__device__ __forceinline__ void mbar_warp_release_consumed(uint64_t* bar) {
+    __syncwarp();
+    if ((threadIdx.x & 31) == 0) mbar_arrive(bar);
+}
 // one arrival per warp after generic-proxy WRITES that the async proxy will read (the caller fences)
 __device__ __forceinline__ void mbar_warp_arrive(uint64_t* bar) {
     __syncwarp();

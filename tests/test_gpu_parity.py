@@ -225,6 +225,24 @@ def test_cg_loop_modes_and_determinism(B):
         assert np.array_equal(o[3], outs[0][3])
 
 
+@pytest.mark.parametrize("dt", [np.float64, np.float32])
+def test_cg_repeatable_bitwise_full_size(B, dt):
+    """L=2048 in the bench configuration: repeated solves are bit-identical (fixed reduction order; and any ordering bug
+    between the TMA rings and their consumers would show up here as a run-to-run difference)."""
+    w = inputs.config(2, dt)
+    h = handle(B, w.L, dt, w.s)
+    kd, fd = dev(w.k), dev(w.f)
+    ref = None
+    for rep in range(6):
+        u = dev(w.u0)
+        it, rr, st = h.fcg_solve(kd, fd, u, 0.0, 24)
+        if ref is None:
+            ref = (it, rr, st, u.clone())
+        else:
+            assert (it, rr, st) == ref[:3] and torch.equal(u, ref[3]), rep
+    h.close()
+
+
 def test_cg_edge_cases(B):
     L = 64
     w = inputs.config(0)
