@@ -62,6 +62,9 @@ typedef enum {
                                  iterations after the stop are no-op launches, results do not depend on it */
     FCG_OPT_PDL          = 5, /* 1: launch the loop kernels with programmatic stream serialization (the next kernel's
                                  prologue overlaps the current kernel's tail); 0: plain stream order */
+    FCG_OPT_FUSED        = 6, /* 1 (default): for L = 256 and 512 (pipelined engine, loop mode 0) a whole solve is ONE cooperative
+                                 kernel with the vectors resident in shared memory and grid barriers between the phases;
+                                 0: the graph of four kernels per iteration at every size */
     FCG_OPT_ENGINE       = 3  /* 0 (default): pipelined TMA passes where the lattice is large enough (L >= 256), classic
                                  passes otherwise; 1: classic passes only (synchronous loads; kept for A/B measurements).
                                  The stored spectrum's layout belongs to the engine: changing the engine after

@@ -13,6 +13,7 @@
 #include "../../include/fcg.h"
 #include "fcg_kernels.cuh"
 #include "fcg_plans.cuh"
+#include "fcg_fused.cuh"
 
 using namespace fcg;
 
@@ -74,12 +75,13 @@ struct fcg_handle_s {
     char* ws = nullptr; bool own_ws = false;
     Layout lay{};
     bool have_spectrum = false;
-    int loop_mode = 0, chunk = 16, row_var_opt = -1, engine_opt = 0, nsm = 148, unroll = 4, pdl = 0;
+    int loop_mode = 0, chunk = 16, row_var_opt = -1, engine_opt = 0, nsm = 148, unroll = 4, pdl = 0, fused_opt = 1;
     alignas(64) CUtensorMap tmap_row;   // T2 as [L/(2 NB)][L/2][128 B]: box = v2_tsub/NB lines of one row pair (row_inv2 tiles)
     alignas(64) CUtensorMap tmap_col;   // T2 as [L/(2 NB)][L/2][NB][2 complex]: box = one column x v2_abox row pairs (col2 gather / scatter)
     bool have_tmap = false;
     int spectrum_colpos = 0;            // layout the stored spectrum was prepared for (1: T2 column order)
     bool v2() const { return engine_opt == 0 && tab->v2 && have_tmap; }
+    bool fused() const { return fused_opt && tab->fused && v2() && loop_mode == 0; }   // whole solve in one cooperative kernel
     Scalars* h_sc = nullptr;            // pinned
     BreakResult* h_brk = nullptr;       // pinned
     void *hk = nullptr, *hf = nullptr, *hu = nullptr;   // device staging of fcg_solve_host
@@ -245,6 +247,26 @@ cudaError_t build_graph(fcg_handle h, GraphEntry& ge) {
 template <typename T>
 int solve_impl(fcg_handle h, const void* k, const void* f, void* u, double tol, int maxit, int* iters, double* relres) {
     h->launches = 0;
+    if (h->fused()) {
+        // small lattices: the whole solve is one cooperative kernel with the vectors resident in shared memory (fcg_fused.cuh)
+        FusedArgs A{};
+        A.k = k; A.f = f; A.u = u; A.Tf = h->ws + h->lay.Tb; A.shat = h->ws + h->lay.shat; A.tw = h->ws + h->lay.tw;
+        A.partial = h->at<double>(h->lay.partial_row); A.counter = &h->sc()->ticket[3]; A.sc = h->sc(); A.tol = tol; A.maxit = maxit;
+        FCG_CK(h, cudaMemsetAsync(h->sc(), 0, sizeof(Scalars), h->stream));
+        cudaError_t e = h->tab->fused_solve(&A, h->stream);
+        if (e == cudaSuccess) {
+            FCG_CK(h, cudaMemcpyAsync(h->h_sc, h->sc(), sizeof(Scalars), cudaMemcpyDeviceToHost, h->stream));
+            FCG_CK(h, cudaStreamSynchronize(h->stream));
+            h->launches = 1;
+            if (iters) *iters = h->h_sc->it;
+            if (relres) *relres = h->h_sc->relres;
+            if (h->h_sc->status == FCG_CUDA_ERROR) h->err = "fused solve: grid barrier timed out";
+            return h->h_sc->status;
+        }
+        cudaGetLastError();
+        h->err = std::string("cooperative launch failed (") + cudaGetErrorString(e) + "); using the graph path";
+        h->fused_opt = 0;
+    }
     if (h->loop_mode == 0) {
         const int var = h->v2() ? 100 : h->row_var();
         GraphEntry* hit = nullptr;
@@ -505,6 +527,7 @@ int fcg_set_option(fcg_handle h, int option, int value) {
         case FCG_OPT_ROW_VARIANT:
             if (value >= FCG_NROWVAR || (value >= 0 && !h->tab->row_valid[value])) return fail(h, FCG_INVALID_ARG, "row variant not available for this size");
             h->row_var_opt = value; return FCG_OK;
+        case FCG_OPT_FUSED: if (value != 0 && value != 1) return fail(h, FCG_INVALID_ARG, "fused must be 0 or 1"); h->fused_opt = value; return FCG_OK;
         case FCG_OPT_PDL: if (value != 0 && value != 1) return fail(h, FCG_INVALID_ARG, "pdl must be 0 or 1"); h->pdl = value; return FCG_OK;
         case FCG_OPT_UNROLL: if (value < 1 || value > 64) return fail(h, FCG_INVALID_ARG, "unroll must be 1..64"); h->unroll = value; return FCG_OK;
         case FCG_OPT_ENGINE:

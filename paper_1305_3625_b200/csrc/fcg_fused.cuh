@@ -1,0 +1,354 @@
+// fcg_fused.cuh -- a whole CG solve (Listing 2, around the operator of Listing 4, 141-151) as ONE
+// cooperative kernel, for lattices small enough that launch latency, not bandwidth, sets the pace (L = 256, 512:
+// BASELINE.json configs[3] is ~75 000 iterations of a 0.5 MiB problem).
+//
+//   * grid = G <= 256 co-resident CTAs (cudaLaunchCooperativeKernel); CTA c owns the row pairs c, c+G, .. and the columns
+//     c, c+G, .. of T for the whole solve;
+//   * its rows of k, f, u, r, p, q live in shared memory from the first iteration to the last; only T (the transposition
+//     between the row and the column transforms) goes through global memory, i.e. through L2;
+//   * per iteration four grid barriers (an atomic counter in global memory): T complete -> columns done -> p.q known ->
+//     r.r known.  Every CTA adds the G partial sums itself, in the same fixed order, so alpha, beta and the convergence
+//     decision are bit-identical in all CTAs and no CTA ever waits for a broadcast;
+//   * same stage arithmetic as the pipelined passes (fcg_engine.cuh: register twiddle powers, swizzled work buffer) and the
+//     same column numbering / stored spectrum as them (AsyncShape, colpos layout), so fcg_set_spectrum is shared.
+//
+// Order of operations = the oracle's (u is updated as soon as alpha is known).  A spin that exceeds SPIN_CAP polls sets
+// status FCG_CUDA_ERROR instead of hanging the device.
+#pragma once
+#include "fcg_async.cuh"
+
+namespace fcg {
+
+struct FusedArgs {
+    const void* k; const void* f; void* u;     // caller vectors (device), N reals
+    void* Tf;                                   // workspace: L/2 columns x L complex, column m contiguous
+    const void* shat; const void* tw;
+    double* partial;                            // 4 x G doubles
+    unsigned int* counter;                      // grid barrier (zeroed by the host before the launch)
+    Scalars* sc;                                // result: it, relres, status
+    double tol; int maxit;
+};
+
+template <typename T, typename P> struct FusedShape {
+    static constexpr int L = P::N, NT = P::NT;
+    static constexpr bool valid = AsyncShape<T, P>::valid && (L == 256 || L == 512) && NT % 32 == 0;
+    static constexpr int G = L / 2 < 256 ? L / 2 : 256;          // CTAs (all co-resident: <= 2 per SM)
+    static constexpr int TPC = (L / 2) / G;                      // row pairs (and columns) per CTA
+    static constexpr size_t WBYTES = (size_t)L * 2 * sizeof(T);
+    static constexpr size_t VBYTES = (size_t)2 * L * sizeof(T);  // one vector's two rows
+    static constexpr size_t smem = WBYTES + (size_t)TPC * 6 * VBYTES + 128;
+};
+
+#ifdef __CUDACC__
+
+constexpr unsigned int SPIN_CAP = 1u << 26;
+
+__device__ __forceinline__ unsigned int ld_acquire_u32(const unsigned int* p) {
+    unsigned int v;
+    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+
+// all CTAs of the (co-resident) grid; returns false if the spin cap was hit
+__device__ __forceinline__ bool grid_barrier(unsigned int* counter, unsigned int& target, unsigned int G, int* ok_smem) {
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        target += G;
+        __threadfence();
+        atomicAdd(counter, 1u);
+        unsigned int spins = 0;
+        while (ld_acquire_u32(counter) < target && ++spins < SPIN_CAP) {}
+        *ok_smem = spins < SPIN_CAP;
+        __threadfence();
+    }
+    __syncthreads();
+    return *ok_smem != 0;
+}
+
+template <typename T, typename P>
+__global__ void __launch_bounds__(P::NT) cg_fused_kernel(const FusedArgs A)
+{
+    using AS = AsyncShape<T, P>;
+    using FS = FusedShape<T, P>;
+    constexpr int L = P::N, S = P::S, NT = P::NT, R1 = AS::R1, Q1 = AS::Q1, PER1 = AS::PER1, PM = per_max<P>();
+    constexpr int G = FS::G, TPC = FS::TPC;
+    extern __shared__ unsigned char smem_dyn[];
+    unsigned char* const smem_raw = align128(smem_dyn);
+    __shared__ double red[32];
+    __shared__ double bcast;
+    __shared__ int ok_smem;
+    cx<T>* W = reinterpret_cast<cx<T>*>(smem_raw);
+    T* const vecs = reinterpret_cast<T*>(smem_raw + FS::WBYTES);
+    // vector v (0 k, 1 f, 2 u, 3 r, 4 p, 5 q) of own tile j, row r (0/1)
+    auto V = [&](int j, int v, int r) { return vecs + ((size_t)(j * 6 + v) * 2 + r) * L; };
+    SmemIO<T, P> io{W};
+    const int lt = threadIdx.x, cta = (int)blockIdx.x;
+    const T* gk = static_cast<const T*>(A.k); const T* gf = static_cast<const T*>(A.f); T* gu = static_cast<T*>(A.u);
+    cx<T>* Tf = static_cast<cx<T>*>(A.Tf);
+    const T* shat = static_cast<const T*>(A.shat);
+    const cx<T>* tw = static_cast<const cx<T>*>(A.tw);
+    unsigned int target = 0;
+    int slot = 0;                                  // partial-sum slot, rotates over 4
+    auto ld_sw = [&](int e) { return io.ld(e); };
+    auto st_sw = [&](int e, cx<T> v) { io.st(e, v); };
+
+    cx<T> wb[S + 1][PM];
+    static_for_up<1, S - 1>([&](auto s) { base_tw<P, decltype(s)::value, T>(lt, tw, wb[decltype(s)::value]); });
+
+    // sum of one double per thread over the CTA (fixed tree), result in every thread
+    auto cta_sum = [&](double v) {
+        double a[1] = {v};
+        block_sum<1>(a, red);
+        if (lt == 0) bcast = a[0];
+        __syncthreads();
+        const double r = bcast;
+        __syncthreads();
+        return r;
+    };
+    // grid-wide sum: publish the CTA's partial, barrier, every CTA adds all G partials in the same order
+    auto grid_sum = [&](double part, bool& ok) {
+        const double mine = cta_sum(part);
+        double* ps = A.partial + (size_t)slot * G;
+        if (lt == 0) ps[cta] = mine;
+        ok = grid_barrier(A.counter, target, G, &ok_smem);
+        double v = 0.0;
+        for (int i = lt; i < G; i += NT) v += __ldcg(ps + i);
+        slot = (slot + 1) & 3;
+        return cta_sum(v);
+    };
+
+    // ---- the three phases of one operator application c = C x (x = vector `vx` of the own tiles); c is left in `out`
+    // phase R1: row transforms of x -> columns of Tf
+    auto rows_forward = [&](int vx) {
+        for (int j = 0; j < TPC; ++j) {
+            const int A2 = cta + j * G;
+            const T* x0 = V(j, vx, 0); const T* x1 = V(j, vx, 1);
+            {
+                cx<T> a[PER1][R1];
+                stage_ld<P, 1, T>(lt, [&](int e) { return mk<T>(x0[e], x1[e]); }, a);
+                stage_math<P, 1, -1, T>(a, wb[1]);
+                stage_st<P, 1, T>(lt, st_sw, a);
+                __syncthreads();
+            }
+            static_for_up<2, S>([&](auto s) {
+                constexpr int sv = decltype(s)::value;
+                cx<T> a[St<P, sv>::PER][St<P, sv>::R];
+                stage_ld<P, sv, T>(lt, ld_sw, a);
+                stage_math<P, sv, -1, T>(a, wb[sv]);
+                stage_st<P, sv, T>(lt, st_sw, a);
+                __syncthreads();
+            });
+            const T h = (T)0.5;
+            for (int m = lt; m < L / 2; m += NT) {
+                const int e = AS::pos_of_col(m);
+                const int n = P::freq_of(e);
+                cx<T> X0, X1;
+                if (n == 0) {
+                    const cx<T> Z0 = io.ld(P::pos_of(0)), ZN = io.ld(P::pos_of(L / 2));
+                    X0 = mk<T>(Z0.x, ZN.x); X1 = mk<T>(Z0.y, ZN.y);
+                } else {
+                    const cx<T> Za = io.ld(e), Zb = io.ld(P::pos_of(L - n));
+                    X0 = mk<T>((Za.x + Zb.x) * h, (Za.y - Zb.y) * h);
+                    X1 = mk<T>((Za.y + Zb.y) * h, (Zb.x - Za.x) * h);
+                }
+                store_pair<T>(Tf + (size_t)m * L + 2 * A2, X0, X1);
+            }
+            __syncthreads();
+        }
+    };
+    // phase C: own columns, in place: forward, spectral multiply, inverse
+    auto columns = [&]() {
+        for (int j = 0; j < TPC; ++j) {
+            const int m = cta + j * G;
+            cx<T>* col = Tf + (size_t)m * L;
+            for (int e = lt; e < L; e += NT) W[e] = __ldcg(col + e);
+            __syncthreads();
+            {
+                cx<T> a[St<P, 1>::PER][St<P, 1>::R];
+                stage_ld<P, 1, T>(lt, [&](int e) { return W[e]; }, a);
+                __syncthreads();
+                stage_math<P, 1, -1, T>(a, wb[1]);
+                stage_st<P, 1, T>(lt, st_sw, a);
+                __syncthreads();
+            }
+            auto fwd_stage = [&](auto s) {
+                constexpr int sv = decltype(s)::value;
+                cx<T> a[St<P, sv>::PER][St<P, sv>::R];
+                stage_ld<P, sv, T>(lt, ld_sw, a);
+                stage_math<P, sv, -1, T>(a, wb[sv]);
+                stage_st<P, sv, T>(lt, st_sw, a);
+                __syncthreads();
+            };
+            auto inv_stage = [&](auto s) {
+                constexpr int sv = decltype(s)::value;
+                cx<T> a[St<P, sv>::PER][St<P, sv>::R];
+                stage_ld<P, sv, T>(lt, ld_sw, a);
+                stage_math<P, sv, +1, T>(a, wb[sv]);
+                stage_st<P, sv, T>(lt, st_sw, a);
+                __syncthreads();
+            };
+            if (m != 0) {
+                const T* sh = shat + (size_t)m * L;
+                static_for_up<2, S - 1>(fwd_stage);
+                run_middle<P, T>(lt, ld_sw, st_sw, [&](int g, int u) { return sh[u * (L / P::RLAST) + g]; });
+                __syncthreads();
+                static_for_down<S - 1, 2>(inv_stage);
+            } else {     // packed n = 0 / L/2 column (see col2_kernel)
+                static_for_up<2, S>(fwd_stage);
+                const T* sp_ = shat;
+                const T* sm_ = shat + (size_t)(L / 2) * L;
+                for (int mm = lt; mm <= L / 2; mm += NT) {
+                    const int e = P::pos_of(mm), e2 = P::pos_of((L - mm) % L);
+                    const cx<T> Wa = io.ld(e), Wb = io.ld(e2);
+                    cx<T> va, vb;
+                    const int i1 = P::shat_index(e), i2 = P::shat_index(e2);
+                    va.x = sp_[i1] * Wa.x + sm_[i1] * Wb.x; va.y = sp_[i1] * Wa.y - sm_[i1] * Wb.y;
+                    vb.x = sp_[i2] * Wb.x + sm_[i2] * Wa.x; vb.y = sp_[i2] * Wb.y - sm_[i2] * Wa.y;
+                    io.st(e, va);
+                    if (e2 != e) io.st(e2, vb);
+                }
+                __syncthreads();
+                static_for_down<S, 2>(inv_stage);
+            }
+            {
+                cx<T> a[St<P, 1>::PER][St<P, 1>::R];
+                stage_ld<P, 1, T>(lt, ld_sw, a);
+                stage_math<P, 1, +1, T>(a, wb[1]);
+                __syncthreads();
+                stage_st<P, 1, T>(lt, [&](int e, cx<T> v) { W[e] = v; }, a);
+            }
+            __syncthreads();
+            for (int e = lt; e < L; e += NT) col[e] = W[e];
+            __syncthreads();
+        }
+    };
+    // phase R2: inverse row transforms; emit(j, e, c0, c1) receives c = (C x) at element e of rows 0/1 of own tile j
+    auto rows_inverse = [&](auto emit) {
+        for (int j = 0; j < TPC; ++j) {
+            const int A2 = cta + j * G;
+            for (int m = lt; m < L / 2; m += NT) {
+                const int e = AS::pos_of_col(m);
+                const int n = P::freq_of(e);
+                const cx<T>* src = Tf + (size_t)m * L + 2 * A2;
+                const cx<T> X0 = __ldcg(src), X1 = __ldcg(src + 1);
+                if (n == 0) {
+                    io.st(P::pos_of(0), mk<T>(X0.x, X1.x));
+                    io.st(P::pos_of(L / 2), mk<T>(X0.y, X1.y));
+                } else {
+                    io.st(e, mk<T>(X0.x - X1.y, X0.y + X1.x));
+                    io.st(P::pos_of(L - n), mk<T>(X0.x + X1.y, X1.x - X0.y));
+                }
+            }
+            __syncthreads();
+            static_for_down<S, 2>([&](auto s) {
+                constexpr int sv = decltype(s)::value;
+                cx<T> a[St<P, sv>::PER][St<P, sv>::R];
+                stage_ld<P, sv, T>(lt, ld_sw, a);
+                stage_math<P, sv, +1, T>(a, wb[sv]);
+                stage_st<P, sv, T>(lt, st_sw, a);
+                __syncthreads();
+            });
+            cx<T> c[PER1][R1];
+            stage_ld<P, 1, T>(lt, ld_sw, c);
+            __syncthreads();
+            stage_math<P, 1, +1, T>(c, wb[1]);
+#pragma unroll
+            for (int q = 0; q < PER1; ++q)
+#pragma unroll
+                for (int t = 0; t < R1; ++t) emit(j, lt + q * NT + t * Q1, c[q][t].x, c[q][t].y);
+        }
+    };
+
+    // ---- set up initial values: r = f - A u, rho = r.r, ||f||^2
+    for (int j = 0; j < TPC; ++j) {
+        const size_t row0 = (size_t)(2 * (cta + j * G)) * L;
+        for (int e = lt; e < 2 * L; e += NT) {         // the two rows are adjacent in memory
+            V(j, 0, 0)[e] = gk[row0 + e]; V(j, 1, 0)[e] = gf[row0 + e]; V(j, 2, 0)[e] = gu[row0 + e];
+            V(j, 4, 0)[e] = (T)0;
+        }
+    }
+    __syncthreads();
+    bool ok = true, okb = true;
+    double acc_r = 0.0, acc_f = 0.0;
+    rows_forward(2);
+    ok = grid_barrier(A.counter, target, G, &ok_smem) && ok;
+    columns();
+    ok = grid_barrier(A.counter, target, G, &ok_smem) && ok;
+    rows_inverse([&](int j, int e, T c0, T c1) {
+        const T* kk = V(j, 0, 0); const T* ff = V(j, 1, 0); const T* uu = V(j, 2, 0); T* rr = V(j, 3, 0);
+        const T f0 = ff[e], f1 = ff[L + e];
+        const T r0 = f0 - (kk[e] * uu[e] + c0), r1 = f1 - (kk[L + e] * uu[L + e] + c1);
+        rr[e] = r0; rr[L + e] = r1;
+        acc_r += (double)r0 * (double)r0; acc_r += (double)r1 * (double)r1;
+        acc_f += (double)f0 * (double)f0; acc_f += (double)f1 * (double)f1;
+    });
+    double rho = grid_sum(acc_r, okb); ok = ok && okb;
+    const double fn2 = grid_sum(acc_f, okb); ok = ok && okb;
+    int it = 0, status = ST_OK;
+    bool done = false, zero_u = false;
+    double beta = 0.0;
+    if (!ok) { done = true; status = -3; }
+    else if (fn2 == 0.0) { done = true; zero_u = true; rho = 0.0; }
+    else if (sqrt(rho) <= A.tol * sqrt(fn2)) done = true;
+    else if (A.maxit <= 0) { done = true; status = ST_NOT_CONVERGED; }
+
+    // ---- Listing 2
+    while (!done) {
+        for (int j = 0; j < TPC; ++j) {                                   // update calculation variables: new direction (98)
+            const T* rr = V(j, 3, 0); T* pp = V(j, 4, 0);
+            const T b = (T)beta;
+            for (int e = lt; e < 2 * L; e += NT) pp[e] = rr[e] + b * pp[e];
+        }
+        __syncthreads();
+        rows_forward(4);                                                  // A * p (93)
+        ok = grid_barrier(A.counter, target, G, &ok_smem) && ok;
+        columns();
+        ok = grid_barrier(A.counter, target, G, &ok_smem) && ok;
+        double acc = 0.0;
+        rows_inverse([&](int j, int e, T c0, T c1) {
+            const T* kk = V(j, 0, 0); const T* pp = V(j, 4, 0); T* qq = V(j, 5, 0);
+            const T p0 = pp[e], p1 = pp[L + e];
+            const T q0 = kk[e] * p0 + c0, q1 = kk[L + e] * p1 + c1;       // k o p + C p
+            qq[e] = q0; qq[L + e] = q1;
+            acc += (double)p0 * (double)q0; acc += (double)p1 * (double)q1;
+        });
+        const double pq = grid_sum(acc, okb); ok = ok && okb;             // search length (94)
+        if (!ok) { status = -3; break; }
+        if (!(pq > 0.0) || !isfinite(pq)) { status = ST_BREAKDOWN; break; }
+        const double alpha = rho / pq;
+        const T al = (T)alpha;
+        double accr = 0.0;
+        __syncthreads();
+        for (int j = 0; j < TPC; ++j) {                                   // new x (95), residue (96), residue length (97)
+            T* uu = V(j, 2, 0); T* rr = V(j, 3, 0); const T* pp = V(j, 4, 0); const T* qq = V(j, 5, 0);
+            for (int e = lt; e < 2 * L; e += NT) {
+                uu[e] = uu[e] + al * pp[e];
+                const T rn = rr[e] - al * qq[e];
+                rr[e] = rn;
+                accr += (double)rn * (double)rn;
+            }
+        }
+        const double rho_new = grid_sum(accr, okb); ok = ok && okb;
+        if (!ok) { status = -3; break; }
+        ++it;
+        if (sqrt(rho_new) <= A.tol * sqrt(fn2)) { rho = rho_new; break; }                 // check convergence (99)
+        if (it >= A.maxit) { rho = rho_new; status = ST_NOT_CONVERGED; break; }
+        beta = rho_new / rho;
+        rho = rho_new;
+    }
+    __syncthreads();
+    for (int j = 0; j < TPC; ++j) {
+        const size_t row0 = (size_t)(2 * (cta + j * G)) * L;
+        const T* uu = V(j, 2, 0);
+        for (int e = lt; e < 2 * L; e += NT) gu[row0 + e] = zero_u ? (T)0 : uu[e];
+    }
+    if (cta == 0 && lt == 0) {
+        Scalars* sc = A.sc;
+        sc->it = it; sc->status = status; sc->done = 1; sc->rho = rho; sc->fn2 = fn2;
+        sc->relres = fn2 > 0.0 ? sqrt(rho) / sqrt(fn2) : 0.0;
+    }
+}
+
+#endif  // __CUDACC__
+
+}  // namespace fcg

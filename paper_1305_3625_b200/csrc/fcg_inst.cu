@@ -3,6 +3,7 @@
 #include <cmath>
 #include "fcg_plans.cuh"
 #include "fcg_async.cuh"
+#include "fcg_fused.cuh"
 
 #ifndef FCG_INST_L
 #error "compile with -DFCG_INST_L=<L>"
@@ -50,6 +51,9 @@ template <typename T> struct Inst {
             if ((e = prep(col2_xform_kernel<T, P, C_COL, +1>, AS::WBYTES + 128)) != cudaSuccess) return e;
             if ((e = prep(t2_export_kernel<T, P>, AS::WBYTES + 1024)) != cudaSuccess) return e;
             if ((e = prep(t2_import_kernel<T, P>, AS::WBYTES + 1024)) != cudaSuccess) return e;
+        }
+        if constexpr (FS::valid) {
+            if ((e = prep(cg_fused_kernel<T, P>, FS::smem)) != cudaSuccess) return e;
         }
         return prep(col_kernel<T, P, CS::COLS>, CS::smem);
     }
@@ -106,6 +110,15 @@ template <typename T> struct Inst {
         if constexpr (V2) {
             t2_import_kernel<T, P><<<L / 2, 256, AS::WBYTES + 1024, st>>>(static_cast<const cx<T>*>(X), static_cast<cx<T>*>(T2));
             return cudaGetLastError();
+        }
+        return cudaErrorInvalidValue;
+    }
+    using FS = FusedShape<T, P>;
+    static cudaError_t fused_solve(const void* fused_args, cudaStream_t st) {
+        if constexpr (FS::valid) {
+            FusedArgs A = *static_cast<const FusedArgs*>(fused_args);
+            void* params[] = {&A};
+            return cudaLaunchCooperativeKernel((const void*)cg_fused_kernel<T, P>, dim3(FS::G), dim3(P::NT), params, FS::smem, st);
         }
         return cudaErrorInvalidValue;
     }
@@ -176,6 +189,7 @@ template <typename T> struct Inst {
         t.v2_smem[0] = AS::fwd_smem; t.v2_smem[1] = AS::col_smem; t.v2_smem[2] = AS::inv_smem;
         t.row_fwd2 = &row_fwd2; t.col2 = &col2; t.row_inv2 = &row_inv2;
         t.col2_xform = &col2_xform; t.t2_export = &t2_export; t.t2_import = &t2_import;
+        t.fused = FS::valid ? 1 : 0; t.fused_grid = FS::G; t.fused_solve = &fused_solve;
         t.init = &init; t.row_fwd = &row_fwd; t.col = &col; t.row_inv = &row_inv; t.spectrum_prep = &spectrum_prep;
         return t;
     }

@@ -70,6 +70,9 @@ struct PassTable {
     cudaError_t (*col2_xform)(const void* args, const void* tensor_map, int inverse, cudaStream_t st);   // stand-alone transforms
     cudaError_t (*t2_export)(const void* T2, void* X, cudaStream_t st);
     cudaError_t (*t2_import)(const void* X, void* T2, cudaStream_t st);
+    // whole solve as one cooperative kernel (fcg_fused.cuh); fused == 0 when the size has none
+    int fused, fused_grid;
+    cudaError_t (*fused_solve)(const void* fused_args, cudaStream_t st);
 };
 
 #define FCG_DECL_TABLE(L) const PassTable* fcg_pass_table_##L(int dtype);

@@ -170,7 +170,8 @@ def cg_parity(B, w, **opts):
     it, rr, st = h.fcg_solve(kd, fd, u, w.tol, w.maxit)
     assert st == ref["status"]
     assert abs(it - ref["iters"]) <= 2, (it, ref["iters"], ref["hist"][-4:])
-    assert h.fcg_last_launch_count() == 5 + 16 * ((it + 3) // 4) or opts      # set-up 4 + finish 1 + 4 kernels x (iterations rounded up to the WHILE body's 4)
+    # graph path: set-up 4 + finish 1 + 4 kernels x (iterations rounded up to the WHILE body's 4); fused path (L = 256, 512): 1
+    assert h.fcg_last_launch_count() in (1, 5 + 16 * ((it + 3) // 4)) or opts
     u_nat = u.cpu().numpy()
     d_nat = rel(u_nat, ref["u"])
     d_pin = d_nat
@@ -215,7 +216,7 @@ def test_cg_loop_modes_and_determinism(B):
     w = inputs.config(1, L=256)
     outs = []
     for mode, chunk, unroll in ((0, 16, 4), (0, 16, 1), (0, 16, 7), (1, 16, 4), (1, 5, 4)):
-        h = handle(B, w.L, np.float64, w.s, FCG_OPT_LOOP_MODE=mode, FCG_OPT_CHUNK=chunk, FCG_OPT_UNROLL=unroll)
+        h = handle(B, w.L, np.float64, w.s, FCG_OPT_FUSED=0, FCG_OPT_LOOP_MODE=mode, FCG_OPT_CHUNK=chunk, FCG_OPT_UNROLL=unroll)
         u = dev(w.u0)
         it, rr, st = h.fcg_solve(dev(w.k), dev(w.f), u, w.tol, w.maxit)
         outs.append((it, rr, st, u.cpu().numpy().copy()))
@@ -241,6 +242,24 @@ def test_cg_repeatable_bitwise_full_size(B, dt):
         else:
             assert (it, rr, st) == ref[:3] and torch.equal(u, ref[3]), rep
     h.close()
+
+
+@pytest.mark.parametrize("cfg,L", [(1, 256), (1, 512), (2, 256), (4, 256)])
+def test_cg_fused_kernel(B, cfg, L):
+    """L = 256, 512: the whole solve as one cooperative kernel (FCG_OPT_FUSED, default on).  Parity with the oracle, agreement
+    with the four-kernel graph path, one launch, bitwise repeatability."""
+    w = inputs.config(cfg, np.float64, L=L)
+    it_f, it_or = cg_parity(B, w)                                   # default = fused at these sizes
+    us = []
+    for fused in (1, 1, 0):
+        h = handle(B, L, np.float64, w.s, FCG_OPT_FUSED=fused)
+        u = dev(w.u0)
+        it, rr, st = h.fcg_solve(dev(w.k), dev(w.f), u, w.tol, w.maxit)
+        assert st == 0 and h.fcg_last_launch_count() == (1 if fused else 5 + 16 * ((it + 3) // 4))
+        us.append((it, u.cpu().numpy()))
+        h.close()
+    assert us[0][0] == us[1][0] and np.array_equal(us[0][1], us[1][1])          # repeatable
+    assert abs(us[0][0] - us[2][0]) <= 2 and rel(us[0][1], us[2][1]) <= 1e-9    # same answer as the graph path
 
 
 def test_cg_edge_cases(B):
