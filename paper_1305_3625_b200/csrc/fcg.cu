@@ -85,6 +85,7 @@ struct fcg_handle_s {
     Scalars* h_sc = nullptr;            // pinned
     BreakResult* h_brk = nullptr;       // pinned
     void *hk = nullptr, *hf = nullptr, *hu = nullptr;   // device staging of fcg_solve_host
+    long long* frac_idx = nullptr; int* frac_it = nullptr; int frac_cap = 0;   // device results of the fused quasi-static loop
     std::vector<GraphEntry> graphs; unsigned long long stamp = 0;
     long long launches = 0;
     std::string err;
@@ -514,6 +515,8 @@ int fcg_destroy(fcg_handle h) {
     if (h->hk) cudaFree(h->hk);
     if (h->hf) cudaFree(h->hf);
     if (h->hu) cudaFree(h->hu);
+    if (h->frac_idx) cudaFree(h->frac_idx);
+    if (h->frac_it) cudaFree(h->frac_it);
     cudaGetLastError();
     delete h;
     return FCG_OK;
@@ -598,6 +601,40 @@ int fcg_break_step(fcg_handle h, void* k, const void* u, const void* t, long lon
 int fcg_fracture(fcg_handle h, void* k, const void* f, void* u, const void* t, int nsteps, double tol, int maxit,
                  long long* index_host, int* iters_host, int* steps_done_host) {
     if (!h || !k || !f || !u || !t || nsteps < 0 || !index_host || !iters_host) return fail(h, FCG_INVALID_ARG, "bad argument");
+    if (h->fused() && h->have_spectrum && nsteps > 0 && tol >= 0.0 && maxit >= 0) {
+        // small lattices: the whole quasi-static loop -- every solve and every break step -- is one cooperative kernel
+        if (h->frac_cap < nsteps) {
+            if (h->frac_idx) cudaFree(h->frac_idx);
+            if (h->frac_it) cudaFree(h->frac_it);
+            h->frac_idx = nullptr; h->frac_it = nullptr; h->frac_cap = 0;
+            FCG_CK(h, cudaMalloc((void**)&h->frac_idx, (size_t)nsteps * sizeof(long long)));
+            FCG_CK(h, cudaMalloc((void**)&h->frac_it, (size_t)nsteps * sizeof(int)));
+            h->frac_cap = nsteps;
+        }
+        FusedArgs A{};
+        A.k = k; A.f = f; A.u = u; A.Tf = h->ws + h->lay.Tb; A.shat = h->ws + h->lay.shat; A.tw = h->ws + h->lay.tw;
+        A.partial = h->at<double>(h->lay.partial_row); A.counter = &h->sc()->ticket[3]; A.sc = h->sc(); A.tol = tol; A.maxit = maxit;
+        A.nsteps = nsteps; A.t = t; A.k_out = k; A.out_index = h->frac_idx; A.out_iters = h->frac_it;
+        A.brk_r = h->at<double>(h->lay.brk_r); A.brk_i = h->at<long long>(h->lay.brk_i);
+        FCG_CK(h, cudaMemsetAsync(h->sc(), 0, sizeof(Scalars), h->stream));
+        cudaError_t e = h->tab->fused_solve(&A, h->stream);
+        if (e == cudaSuccess) {
+            FCG_CK(h, cudaMemcpyAsync(h->h_sc, h->sc(), sizeof(Scalars), cudaMemcpyDeviceToHost, h->stream));
+            FCG_CK(h, cudaStreamSynchronize(h->stream));
+            const int done = h->h_sc->steps_done;
+            if (done > 0) {
+                FCG_CK(h, cudaMemcpy(index_host, h->frac_idx, (size_t)done * sizeof(long long), cudaMemcpyDeviceToHost));
+                FCG_CK(h, cudaMemcpy(iters_host, h->frac_it, (size_t)done * sizeof(int), cudaMemcpyDeviceToHost));
+            }
+            if (steps_done_host) *steps_done_host = done;
+            h->launches = 1;
+            if (h->h_sc->status == FCG_CUDA_ERROR) h->err = "fused quasi-static loop: grid barrier timed out";
+            return h->h_sc->status < 0 ? h->h_sc->status : FCG_OK;
+        }
+        cudaGetLastError();
+        h->err = std::string("cooperative launch failed (") + cudaGetErrorString(e) + "); using the graph path";
+        h->fused_opt = 0;
+    }
     long long total = 0; int done = 0, st = FCG_OK;
     for (int step = 0; step < nsteps; ++step) {
         int it = 0; double rr = 0.0;

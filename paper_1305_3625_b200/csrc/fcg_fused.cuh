@@ -27,6 +27,8 @@ struct FusedArgs {
     unsigned int* counter;                      // grid barrier (zeroed by the host before the launch)
     Scalars* sc;                                // result: it, relres, status
     double tol; int maxit;
+    // quasi-static loop (nsteps > 0): thresholds, k written back, per-step results, arg-max scratch (G entries each)
+    int nsteps; const void* t; void* k_out; long long* out_index; int* out_iters; double* brk_r; long long* brk_i;
 };
 
 template <typename T, typename P> struct FusedShape {
@@ -36,7 +38,7 @@ template <typename T, typename P> struct FusedShape {
     static constexpr int TPC = (L / 2) / G;                      // row pairs (and columns) per CTA
     static constexpr size_t WBYTES = (size_t)L * 2 * sizeof(T);
     static constexpr size_t VBYTES = (size_t)2 * L * sizeof(T);  // one vector's two rows
-    static constexpr size_t smem = WBYTES + (size_t)TPC * 6 * VBYTES + 128;
+    static constexpr size_t smem = WBYTES + (size_t)TPC * 7 * VBYTES + 128;     // k f u r p q t
 };
 
 #ifdef __CUDACC__
@@ -79,8 +81,8 @@ __global__ void __launch_bounds__(P::NT) cg_fused_kernel(const FusedArgs A)
     __shared__ int ok_smem;
     cx<T>* W = reinterpret_cast<cx<T>*>(smem_raw);
     T* const vecs = reinterpret_cast<T*>(smem_raw + FS::WBYTES);
-    // vector v (0 k, 1 f, 2 u, 3 r, 4 p, 5 q) of own tile j, row r (0/1)
-    auto V = [&](int j, int v, int r) { return vecs + ((size_t)(j * 6 + v) * 2 + r) * L; };
+    // vector v (0 k, 1 f, 2 u, 3 r, 4 p, 5 q, 6 t) of own tile j, row r (0/1)
+    auto V = [&](int j, int v, int r) { return vecs + ((size_t)(j * 7 + v) * 2 + r) * L; };
     SmemIO<T, P> io{W};
     const int lt = threadIdx.x, cta = (int)blockIdx.x;
     const T* gk = static_cast<const T*>(A.k); const T* gf = static_cast<const T*>(A.f); T* gu = static_cast<T*>(A.u);
@@ -115,6 +117,25 @@ __global__ void __launch_bounds__(P::NT) cg_fused_kernel(const FusedArgs A)
         for (int i = lt; i < G; i += NT) v += __ldcg(ps + i);
         slot = (slot + 1) & 3;
         return cta_sum(v);
+    };
+
+    // arg-max of (ratio, index) over the CTA, "larger ratio, then lower index" (better(), fcg_kernels.cuh); result in all threads
+    __shared__ double am_r[32];
+    __shared__ long long am_i[32];
+    auto cta_argmax = [&](double& r, long long& i) {
+        const int lane = lt & 31, w = lt >> 5;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            const double r2 = __shfl_down_sync(0xffffffffu, r, o);
+            const long long i2 = __shfl_down_sync(0xffffffffu, i, o);
+            if (better(r2, i2, r, i)) { r = r2; i = i2; }
+        }
+        if (lane == 0) { am_r[w] = r; am_i[w] = i; }
+        __syncthreads();
+        r = am_r[0]; i = am_i[0];
+        for (int k2 = 1; k2 < NT / 32; ++k2)
+            if (better(am_r[k2], am_i[k2], r, i)) { r = am_r[k2]; i = am_i[k2]; }
+        __syncthreads();
     };
 
     // ---- the three phases of one operator application c = C x (x = vector `vx` of the own tiles); c is left in `out`
@@ -259,92 +280,151 @@ __global__ void __launch_bounds__(P::NT) cg_fused_kernel(const FusedArgs A)
         }
     };
 
-    // ---- set up initial values: r = f - A u, rho = r.r, ||f||^2
+    // ---- load the CTA's rows once; they stay in shared memory for the whole solve (or the whole quasi-static loop)
+    const bool frac = A.nsteps > 0;
     for (int j = 0; j < TPC; ++j) {
         const size_t row0 = (size_t)(2 * (cta + j * G)) * L;
         for (int e = lt; e < 2 * L; e += NT) {         // the two rows are adjacent in memory
             V(j, 0, 0)[e] = gk[row0 + e]; V(j, 1, 0)[e] = gf[row0 + e]; V(j, 2, 0)[e] = gu[row0 + e];
-            V(j, 4, 0)[e] = (T)0;
+            if (frac) V(j, 6, 0)[e] = static_cast<const T*>(A.t)[row0 + e];
         }
     }
     __syncthreads();
     bool ok = true, okb = true;
-    double acc_r = 0.0, acc_f = 0.0;
-    rows_forward(2);
-    ok = grid_barrier(A.counter, target, G, &ok_smem) && ok;
-    columns();
-    ok = grid_barrier(A.counter, target, G, &ok_smem) && ok;
-    rows_inverse([&](int j, int e, T c0, T c1) {
-        const T* kk = V(j, 0, 0); const T* ff = V(j, 1, 0); const T* uu = V(j, 2, 0); T* rr = V(j, 3, 0);
-        const T f0 = ff[e], f1 = ff[L + e];
-        const T r0 = f0 - (kk[e] * uu[e] + c0), r1 = f1 - (kk[L + e] * uu[L + e] + c1);
-        rr[e] = r0; rr[L + e] = r1;
-        acc_r += (double)r0 * (double)r0; acc_r += (double)r1 * (double)r1;
-        acc_f += (double)f0 * (double)f0; acc_f += (double)f1 * (double)f1;
-    });
-    double rho = grid_sum(acc_r, okb); ok = ok && okb;
-    const double fn2 = grid_sum(acc_f, okb); ok = ok && okb;
-    int it = 0, status = ST_OK;
-    bool done = false, zero_u = false;
-    double beta = 0.0;
-    if (!ok) { done = true; status = -3; }
-    else if (fn2 == 0.0) { done = true; zero_u = true; rho = 0.0; }
-    else if (sqrt(rho) <= A.tol * sqrt(fn2)) done = true;
-    else if (A.maxit <= 0) { done = true; status = ST_NOT_CONVERGED; }
+    int it = 0, status = ST_OK, steps_done = 0;
+    double rho = 0.0, fn2 = 0.0;
+    bool zero_u = false;
 
-    // ---- Listing 2
-    while (!done) {
-        for (int j = 0; j < TPC; ++j) {                                   // update calculation variables: new direction (98)
-            const T* rr = V(j, 3, 0); T* pp = V(j, 4, 0);
-            const T b = (T)beta;
-            for (int e = lt; e < 2 * L; e += NT) pp[e] = rr[e] + b * pp[e];
+    for (int step = 0; step < (frac ? A.nsteps : 1); ++step) {
+        // ---- set up initial values: r = f - A u, rho = r.r, ||f||^2; first direction from p = 0, beta = 0
+        for (int j = 0; j < TPC; ++j) {
+            T* pp = V(j, 4, 0);
+            for (int e = lt; e < 2 * L; e += NT) pp[e] = (T)0;
         }
-        __syncthreads();
-        rows_forward(4);                                                  // A * p (93)
+        double acc_r = 0.0, acc_f = 0.0;
+        rows_forward(2);
         ok = grid_barrier(A.counter, target, G, &ok_smem) && ok;
         columns();
         ok = grid_barrier(A.counter, target, G, &ok_smem) && ok;
-        double acc = 0.0;
         rows_inverse([&](int j, int e, T c0, T c1) {
-            const T* kk = V(j, 0, 0); const T* pp = V(j, 4, 0); T* qq = V(j, 5, 0);
-            const T p0 = pp[e], p1 = pp[L + e];
-            const T q0 = kk[e] * p0 + c0, q1 = kk[L + e] * p1 + c1;       // k o p + C p
-            qq[e] = q0; qq[L + e] = q1;
-            acc += (double)p0 * (double)q0; acc += (double)p1 * (double)q1;
+            const T* kk = V(j, 0, 0); const T* ff = V(j, 1, 0); const T* uu = V(j, 2, 0); T* rr = V(j, 3, 0);
+            const T f0 = ff[e], f1 = ff[L + e];
+            const T r0 = f0 - (kk[e] * uu[e] + c0), r1 = f1 - (kk[L + e] * uu[L + e] + c1);
+            rr[e] = r0; rr[L + e] = r1;
+            acc_r += (double)r0 * (double)r0; acc_r += (double)r1 * (double)r1;
+            acc_f += (double)f0 * (double)f0; acc_f += (double)f1 * (double)f1;
         });
-        const double pq = grid_sum(acc, okb); ok = ok && okb;             // search length (94)
-        if (!ok) { status = -3; break; }
-        if (!(pq > 0.0) || !isfinite(pq)) { status = ST_BREAKDOWN; break; }
-        const double alpha = rho / pq;
-        const T al = (T)alpha;
-        double accr = 0.0;
+        rho = grid_sum(acc_r, okb); ok = ok && okb;
+        fn2 = grid_sum(acc_f, okb); ok = ok && okb;
+        it = 0; status = ST_OK; zero_u = false;
+        bool done = false;
+        double beta = 0.0;
+        if (!ok) { done = true; status = -3; }
+        else if (fn2 == 0.0) { done = true; zero_u = true; rho = 0.0; }
+        else if (sqrt(rho) <= A.tol * sqrt(fn2)) done = true;
+        else if (A.maxit <= 0) { done = true; status = ST_NOT_CONVERGED; }
+
+        // ---- Listing 2
+        while (!done) {
+            for (int j = 0; j < TPC; ++j) {                                   // update calculation variables: new direction (98)
+                const T* rr = V(j, 3, 0); T* pp = V(j, 4, 0);
+                const T b = (T)beta;
+                for (int e = lt; e < 2 * L; e += NT) pp[e] = rr[e] + b * pp[e];
+            }
+            __syncthreads();
+            rows_forward(4);                                                  // A * p (93)
+            ok = grid_barrier(A.counter, target, G, &ok_smem) && ok;
+            columns();
+            ok = grid_barrier(A.counter, target, G, &ok_smem) && ok;
+            double acc = 0.0;
+            rows_inverse([&](int j, int e, T c0, T c1) {
+                const T* kk = V(j, 0, 0); const T* pp = V(j, 4, 0); T* qq = V(j, 5, 0);
+                const T p0 = pp[e], p1 = pp[L + e];
+                const T q0 = kk[e] * p0 + c0, q1 = kk[L + e] * p1 + c1;       // k o p + C p
+                qq[e] = q0; qq[L + e] = q1;
+                acc += (double)p0 * (double)q0; acc += (double)p1 * (double)q1;
+            });
+            const double pq = grid_sum(acc, okb); ok = ok && okb;             // search length (94)
+            if (!ok) { status = -3; break; }
+            if (!(pq > 0.0) || !isfinite(pq)) { status = ST_BREAKDOWN; break; }
+            const double alpha = rho / pq;
+            const T al = (T)alpha;
+            double accr = 0.0;
+            __syncthreads();
+            for (int j = 0; j < TPC; ++j) {                                   // new x (95), residue (96), residue length (97)
+                T* uu = V(j, 2, 0); T* rr = V(j, 3, 0); const T* pp = V(j, 4, 0); const T* qq = V(j, 5, 0);
+                for (int e = lt; e < 2 * L; e += NT) {
+                    uu[e] = uu[e] + al * pp[e];
+                    const T rn = rr[e] - al * qq[e];
+                    rr[e] = rn;
+                    accr += (double)rn * (double)rn;
+                }
+            }
+            const double rho_new = grid_sum(accr, okb); ok = ok && okb;
+            if (!ok) { status = -3; break; }
+            ++it;
+            if (sqrt(rho_new) <= A.tol * sqrt(fn2)) { rho = rho_new; break; }                 // check convergence (99)
+            if (it >= A.maxit) { rho = rho_new; status = ST_NOT_CONVERGED; break; }
+            beta = rho_new / rho;
+            rho = rho_new;
+        }
         __syncthreads();
-        for (int j = 0; j < TPC; ++j) {                                   // new x (95), residue (96), residue length (97)
-            T* uu = V(j, 2, 0); T* rr = V(j, 3, 0); const T* pp = V(j, 4, 0); const T* qq = V(j, 5, 0);
+        if (zero_u)
+            for (int j = 0; j < TPC; ++j) {
+                T* uu = V(j, 2, 0);
+                for (int e = lt; e < 2 * L; e += NT) uu[e] = (T)0;
+            }
+        if (!frac || status < 0) break;
+
+        // ---- break step (rule of BASELINE.json configs[3]): arg-max over {k_i > 0} of (k_i u_i) / t_i, one IEEE
+        //      multiply and one IEEE divide in double, ties -> lowest index, NaN skipped; the winner's k becomes 0
+        __syncthreads();
+        double br = 0.0; long long bi = -1;
+        for (int j = 0; j < TPC; ++j) {
+            const long long row0 = (long long)(2 * (cta + j * G)) * L;
+            const T* kk = V(j, 0, 0); const T* uu = V(j, 2, 0); const T* tt = V(j, 6, 0);
             for (int e = lt; e < 2 * L; e += NT) {
-                uu[e] = uu[e] + al * pp[e];
-                const T rn = rr[e] - al * qq[e];
-                rr[e] = rn;
-                accr += (double)rn * (double)rn;
+                const T ki = kk[e];
+                if (!(ki > (T)0)) continue;
+                const double load = (double)ki * (double)uu[e];
+                const double rt = load / (double)tt[e];
+                if (rt != rt) continue;
+                if (better(rt, row0 + e, br, bi)) { br = rt; bi = row0 + e; }
             }
         }
-        const double rho_new = grid_sum(accr, okb); ok = ok && okb;
+        cta_argmax(br, bi);
+        if (lt == 0) { A.brk_r[cta] = br; A.brk_i[cta] = bi; }
+        ok = grid_barrier(A.counter, target, G, &ok_smem) && ok;
+        br = 0.0; bi = -1;
+        for (int i = lt; i < G; i += NT) {
+            const double r2 = __ldcg(A.brk_r + i); const long long i2 = __ldcg(A.brk_i + i);
+            if (better(r2, i2, br, bi)) { br = r2; bi = i2; }
+        }
+        cta_argmax(br, bi);
         if (!ok) { status = -3; break; }
-        ++it;
-        if (sqrt(rho_new) <= A.tol * sqrt(fn2)) { rho = rho_new; break; }                 // check convergence (99)
-        if (it >= A.maxit) { rho = rho_new; status = ST_NOT_CONVERGED; break; }
-        beta = rho_new / rho;
-        rho = rho_new;
+        if (bi < 0) { status = -6; break; }                                   // FCG_NO_CANDIDATE
+        {
+            const int A2 = (int)(bi / (2 * L));
+            if (A2 % G == cta && lt == 0) V(A2 / G, 0, 0)[bi - (long long)A2 * 2 * L] = (T)0;
+        }
+        if (cta == 0 && lt == 0) { A.out_index[step] = bi; A.out_iters[step] = it; }
+        steps_done = step + 1;
+        status = ST_OK;
+        __syncthreads();
+        // the winners' slots are reused two barriers later at the earliest (the next step's set-up has three)
     }
     __syncthreads();
     for (int j = 0; j < TPC; ++j) {
         const size_t row0 = (size_t)(2 * (cta + j * G)) * L;
-        const T* uu = V(j, 2, 0);
-        for (int e = lt; e < 2 * L; e += NT) gu[row0 + e] = zero_u ? (T)0 : uu[e];
+        const T* uu = V(j, 2, 0); const T* kk = V(j, 0, 0);
+        for (int e = lt; e < 2 * L; e += NT) {
+            gu[row0 + e] = uu[e];
+            if (frac) static_cast<T*>(A.k_out)[row0 + e] = kk[e];
+        }
     }
     if (cta == 0 && lt == 0) {
         Scalars* sc = A.sc;
-        sc->it = it; sc->status = status; sc->done = 1; sc->rho = rho; sc->fn2 = fn2;
+        sc->it = it; sc->status = status; sc->done = 1; sc->rho = rho; sc->fn2 = fn2; sc->steps_done = steps_done;
         sc->relres = fn2 > 0.0 ? sqrt(rho) / sqrt(fn2) : 0.0;
     }
 }

@@ -28,6 +28,7 @@ struct Scalars {
     int it, maxit, done, status, zero_u, use_cond;
     unsigned int ticket[4];
     unsigned long long cond;       // cudaGraphConditionalHandle of the WHILE node (loop mode 0)
+    int steps_done, pad_;          // fused quasi-static loop: completed break steps
 };
 
 enum { ROWF_PLAIN = 0, ROWF_CG = 1 };

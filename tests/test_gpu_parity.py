@@ -409,6 +409,26 @@ def test_fracture_small_matches_oracle(B, L, steps):
     h.close()
 
 
+def test_fracture_fused_one_launch(B):
+    """L = 256: the whole quasi-static loop (every solve and every break step) is ONE cooperative kernel; it must give the
+    break sequence of the four-kernel path and of the oracle's golden file, and leave the same k and u."""
+    steps = 150
+    gold = np.loadtxt(os.path.join(GOLD, "cfg3_breaks.txt"), comments="#")[:steps]
+    w = inputs.config(3, nsteps=steps)
+    res = []
+    for fused in (1, 0):
+        h = handle(B, w.L, np.float64, w.s, FCG_OPT_FUSED=fused)
+        kd, ud = dev(w.k), dev(w.u0)
+        index, iters, done, st = h.fcg_fracture(kd, dev(w.f), ud, dev(w.t), steps, w.tol, w.maxit)
+        assert done == steps and st == 0
+        assert (h.fcg_last_launch_count() == 1) == bool(fused)
+        res.append((index, iters, kd.cpu().numpy(), ud.cpu().numpy()))
+        h.close()
+    assert np.array_equal(res[0][0], gold[:, 1].astype(np.int64)) and np.array_equal(res[1][0], res[0][0])
+    assert np.abs(res[0][1].astype(int) - gold[:, 2].astype(int)).max() <= 2
+    assert np.array_equal(res[0][2], res[1][2]) and rel(res[0][3], res[1][3]) <= 1e-8
+
+
 def test_fracture_config3_full(B):
     """configs[3] at full size: 2000 break steps at L=256 against the oracle's stored sequence
     (tests/golden/cfg3_breaks.txt, written by tests/golden/make_golden.py from oracle/ only)."""
