@@ -55,13 +55,13 @@ __device__ __forceinline__ unsigned int ld_acquire_u32(const unsigned int* p) {
 __device__ __forceinline__ bool grid_barrier(unsigned int* counter, unsigned int& target, unsigned int G, int* ok_smem) {
     __syncthreads();
     if (threadIdx.x == 0) {
+        // arrive with release, poll with acquire (gpu scope): the CTA's earlier writes -- ordered before this thread by the
+        // bar.sync above -- are visible to every CTA that sees the count, without the two full membar.gpu of the classic form
         target += G;
-        __threadfence();
-        atomicAdd(counter, 1u);
+        asm volatile("red.release.gpu.global.add.u32 [%0], %1;" ::"l"(counter), "r"(1u) : "memory");
         unsigned int spins = 0;
         while (ld_acquire_u32(counter) < target && ++spins < SPIN_CAP) {}
         *ok_smem = spins < SPIN_CAP;
-        __threadfence();
     }
     __syncthreads();
     return *ok_smem != 0;
