@@ -66,6 +66,9 @@ def _declare(L: C.CDLL) -> None:
         f = getattr(L, "oracle_cg" + suf)
         f.argtypes = [_i, _vp, _vp, _vp, _vp, _d, _i, C.POINTER(_i), C.POINTER(_d), _vp, _vp, _vp]
         f.restype = _i
+        f = getattr(L, "oracle_pcg" + suf)
+        f.argtypes = [_i, _vp, _vp, _vp, _vp, _d, _d, _i, C.POINTER(_i), C.POINTER(_d), _vp, _vp, _vp, _vp]
+        f.restype = _i
         f = getattr(L, "oracle_break_step" + suf)
         f.argtypes = [_ll, _vp, _vp, _vp, C.POINTER(_ll), C.POINTER(_d), C.POINTER(_d)]
         f.restype = _i
@@ -172,6 +175,26 @@ def cg(s, k, f, u0, tol: float, maxit: int, history: bool = False, directions: b
         out["hist"] = hist[: it.value + 1]
     if directions:
         out["P"] = P[: it.value]; out["R"] = R[: it.value]
+    return out
+
+
+def pcg(s, k, f, u0, kbar: float, tol: float, maxit: int, history: bool = False, directions: bool = False):
+    """Preconditioned CG with M = kbar I + C.  Returns dict(u, iters, relres, status[, hist][, P, Z, R])."""
+    f = np.asarray(f); dt = f.dtype; L = f.shape[0]; N = L * L
+    s = _arr(s, dt, (L, L)); k = _arr(k, dt, (L, L)); f = _arr(f, dt, (L, L))
+    u = np.array(u0, dtype=dt, order="C", copy=True).reshape(L, L)
+    hist = np.full(maxit + 1, np.nan, np.float64) if history else None
+    P = np.zeros((maxit, N), dt) if directions else None
+    Z = np.zeros((maxit, N), dt) if directions else None
+    R = np.zeros((maxit, N), dt) if directions else None
+    it = C.c_int(0); rr = C.c_double(0.0)
+    st = getattr(lib(), "oracle_pcg" + _suf(dt))(L, _p(s), _p(k), _p(f), _p(u), float(kbar), float(tol), int(maxit),
+                                                  C.byref(it), C.byref(rr), _p(hist), _p(P), _p(Z), _p(R))
+    out = dict(u=u, iters=int(it.value), relres=float(rr.value), status=int(st))
+    if history:
+        out["hist"] = hist[: it.value + 1]
+    if directions:
+        out["P"] = P[: it.value]; out["Z"] = Z[: it.value]; out["R"] = R[: it.value]
     return out
 
 

@@ -14,6 +14,7 @@
  *   oracle_fft2_{f64,f32}      textbook radix-2 FFT, rows then columns
  *   oracle_apply_{f64,f32}     y = k o x + F^-1(s o F x)   (Listing 4)
  *   oracle_cg_{f64,f32}        conjugate gradient          (Listing 2)
+ *   oracle_pcg_{f64,f32}       the same with the spectral preconditioner M = kbar I + C
  *   oracle_break_step_*, oracle_fracture_*   break rule + quasi-static loop (PAPER.md:78,
  *                              BASELINE.json configs[3])
  * Pins (tests/test_oracle_*.py): none of these functions is "parity unpinned".

@@ -189,6 +189,76 @@ done:
     return status;
 }
 
+/* Preconditioned conjugate gradient (the paper "used [a preconditioner] for a while",
+ * PAPER.md:175, without giving one).  Textbook PCG with the spectral preconditioner
+ *     M = kbar I + C,   M^-1 = F^-1 diag( 1 / (kbar + s) ) F            (reading D4)
+ * i.e. the operator with the stiffnesses replaced by one constant.  m = 1 / (kbar + s) is formed element by element in
+ * the working precision (one add, one divide).  Same stopping rule as oracle_cg: first iteration with
+ * sqrt(r.r) <= tol sqrt(f.f), r the recurrence residual.
+ *   hist    optional, capacity maxit+1: relative residual after 0,1,2,.. iterations
+ *   Phist / Zhist / Rhist optional, capacity maxit*N each: p_i, z_i, r_i before the update of iteration i (pins)
+ * returns 0 converged, 1 maxit reached, -4 breakdown (p.Ap <= 0, r.z <= 0 or not finite), -1 bad argument. */
+int FN(oracle_pcg)(int L, const REAL* s, const REAL* k, const REAL* f, REAL* u, double kbar, double tol, int maxit,
+                   int* iters, double* relres, double* hist, REAL* Phist, REAL* Zhist, REAL* Rhist)
+{
+    if (L < 1 || (L & (L - 1)) || maxit < 0 || !(tol >= 0.0)) return -1;
+    size_t N = (size_t)L * L;
+    int status = 1, it = 0;
+    double fn = sqrt(FN(dot)(N, f, f));
+    if (fn == 0.0) {
+        for (size_t i = 0; i < N; ++i) u[i] = (REAL)0;
+        *iters = 0; *relres = 0.0; if (hist) hist[0] = 0.0;
+        return 0;
+    }
+    REAL* r = (REAL*)malloc(sizeof(REAL) * N);
+    REAL* p = (REAL*)malloc(sizeof(REAL) * N);
+    REAL* q = (REAL*)malloc(sizeof(REAL) * N);
+    REAL* z = (REAL*)malloc(sizeof(REAL) * N);
+    REAL* m = (REAL*)malloc(sizeof(REAL) * N);
+    CPLX* work = (CPLX*)malloc(sizeof(CPLX) * N);
+    for (size_t i = 0; i < N; ++i) m[i] = (REAL)1 / ((REAL)kbar + s[i]);
+
+    FN(apply)(L, s, k, u, q, work);
+    for (size_t i = 0; i < N; ++i) r[i] = f[i] - q[i];
+    double rr = FN(dot)(N, r, r);
+    double rho = 0.0;
+    if (hist) hist[0] = sqrt(rr) / fn;
+    if (sqrt(rr) <= tol * fn) { status = 0; goto done; }
+    FN(convolve)(L, m, r, z, work);                               /* z = M^-1 r */
+    for (size_t i = 0; i < N; ++i) p[i] = z[i];
+    rho = FN(dot)(N, r, z);
+    if (!(rho > 0.0) || !isfinite(rho)) { status = -4; goto done; }
+
+    while (it < maxit) {
+        if (Phist) memcpy(Phist + (size_t)it * N, p, sizeof(REAL) * N);
+        if (Zhist) memcpy(Zhist + (size_t)it * N, z, sizeof(REAL) * N);
+        if (Rhist) memcpy(Rhist + (size_t)it * N, r, sizeof(REAL) * N);
+        FN(apply)(L, s, k, p, q, work);
+        double pq = FN(dot)(N, p, q);
+        if (!(pq > 0.0) || !isfinite(pq)) { status = -4; goto done; }
+        double alpha = rho / pq;
+        REAL al = (REAL)alpha;
+        for (size_t i = 0; i < N; ++i) u[i] = u[i] + al * p[i];
+        for (size_t i = 0; i < N; ++i) r[i] = r[i] - al * q[i];
+        rr = FN(dot)(N, r, r);
+        ++it;
+        if (hist) hist[it] = sqrt(rr) / fn;
+        if (sqrt(rr) <= tol * fn) { status = 0; break; }
+        FN(convolve)(L, m, r, z, work);
+        double rho_new = FN(dot)(N, r, z);
+        if (!(rho_new > 0.0) || !isfinite(rho_new)) { status = -4; goto done; }
+        double beta = rho_new / rho;
+        REAL be = (REAL)beta;
+        for (size_t i = 0; i < N; ++i) p[i] = z[i] + be * p[i];
+        rho = rho_new;
+    }
+done:
+    *iters = it;
+    *relres = sqrt(rr) / fn;
+    free(r); free(p); free(q); free(z); free(m); free(work);
+    return status;
+}
+
 /* Break step (BASELINE.json configs[3]; readings S5, S13): over candidates {i : k_i > 0}
  * ratio_i = (k_i * u_i) / t_i  -- one IEEE multiply and one IEEE divide in double -- pick the
  * maximum, ties -> lowest i, NaN skipped; set k_i = 0.  second = runner-up ratio (for the top-2

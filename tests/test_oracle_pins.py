@@ -342,3 +342,85 @@ def test_p14_indicative_iteration_counts():
     assert abs(orc.cg(w.s, w.k, w.f, w.u0, w.tol, w.maxit)["iters"] - 28) <= 2
     w = inputs.config(1)
     assert abs(orc.cg(w.s, w.k, w.f, w.u0, w.tol, w.maxit)["iters"] - 105) <= 2
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# Preconditioned CG: M = kbar I + C.  Pins chosen so that a wrong preconditioner spectrum, a
+# swapped r/z in a dot product, or p built from r instead of z fails at least one of them.
+def _dense_A(L, s, k):
+    N = L * L
+    A = np.zeros((N, N))
+    for j in range(N):
+        e = np.zeros(N); e[j] = 1.0
+        A[:, j] = orc.apply(s, k, e.reshape(L, L)).ravel()
+    return A
+
+
+def test_pcg_exact_preconditioner_one_iteration():
+    """k uniform = kbar  =>  M = A  =>  z0 = A^-1 r0 and PCG stops after exactly ONE iteration for any f."""
+    L = 16
+    s = inputs.spectrum(L); k = np.full((L, L), 0.8); f = np.random.default_rng(11).standard_normal((L, L))
+    r = orc.pcg(s, k, f, np.zeros((L, L)), 0.8, 1e-12, 50)
+    assert r["status"] == 0 and r["iters"] == 1
+    assert np.linalg.norm(orc.apply(s, k, r["u"]) - f) <= 1e-12 * np.linalg.norm(f)
+
+
+def test_pcg_matches_dense_solve():
+    L = 8
+    s = inputs.spectrum(L); k = inputs.uniform_k(L); k[inputs.broken_mask(L, 10)] = 0.0
+    f = inputs.normal_f(L)
+    u_dense = np.linalg.solve(_dense_A(L, s, k), f.ravel()).reshape(L, L)
+    r = orc.pcg(s, k, f, np.zeros((L, L)), float(k.mean()), 1e-13, 200)
+    assert r["status"] == 0
+    assert np.linalg.norm(r["u"] - u_dense) <= 1e-11 * np.linalg.norm(u_dense)
+
+
+def test_pcg_with_scalar_preconditioner_reproduces_cg():
+    """s_M constant: with a huge kbar, M^-1 = (1/kbar) I up to O(s/kbar); PCG with M = c I is CG itself (same iterates).
+    kbar = 1e12 makes the deviation ~1e-11, far below the comparison tolerance, and pins PCG to the already-pinned CG."""
+    L = 16
+    s = inputs.spectrum(L); k = inputs.uniform_k(L); f = inputs.normal_f(L)
+    a = orc.cg(s, k, f, np.zeros((L, L)), 1e-10, 200, history=True)
+    b = orc.pcg(s, k, f, np.zeros((L, L)), 1e12, 1e-10, 200, history=True)
+    assert a["iters"] == b["iters"]
+    assert np.allclose(a["hist"], b["hist"], rtol=1e-6)
+    assert np.linalg.norm(a["u"] - b["u"]) <= 1e-9 * np.linalg.norm(a["u"])
+
+
+def test_pcg_invariants_and_iteration_gain():
+    """p_i A-orthogonal, r_i M^-1-orthogonal (r_i . z_j = 0, i != j), z = M^-1 r with M = kbar I + C, and fewer iterations
+    than CG: kappa(M^-1 A) <= (kbar + s_min + dk) / (kbar + s_min - dk) with dk = max |k - kbar|."""
+    L = 16
+    s = inputs.spectrum(L); k = inputs.uniform_k(L); f = inputs.normal_f(L); kbar = float(k.mean())
+    r = orc.pcg(s, k, f, np.zeros((L, L)), kbar, 1e-12, 100, directions=True)
+    P, Z, R = r["P"].astype(np.float64), r["Z"].astype(np.float64), r["R"].astype(np.float64)
+    n = P.shape[0]
+    AP = np.stack([orc.apply(s, k, P[i].reshape(L, L)).ravel() for i in range(n)])
+    G = P @ AP.T
+    off = G - np.diag(np.diag(G))
+    assert np.abs(off).max() <= 1e-9 * np.abs(np.diag(G)).max()
+    RZ = R @ Z.T
+    offz = RZ - np.diag(np.diag(RZ))
+    assert np.abs(offz).max() <= 1e-9 * np.abs(np.diag(RZ)).max()
+    for i in (0, n // 2, n - 1):                                     # M z = r
+        Mz = orc.apply(s, np.full((L, L), kbar), Z[i].reshape(L, L)).ravel()
+        assert np.linalg.norm(Mz - R[i]) <= 1e-12 * np.linalg.norm(R[i])
+    cg_it = orc.cg(s, k, f, np.zeros((L, L)), 1e-12, 100)["iters"]
+    assert r["iters"] < cg_it
+    dk = np.abs(k - kbar).max(); lo = kbar + 1 / np.sqrt(8.0)
+    kappa = (lo + dk) / (lo - dk)
+    bound = int(np.ceil(np.log(2.0 / 1e-12) / -np.log((np.sqrt(kappa) - 1) / (np.sqrt(kappa) + 1)))) + 2
+    assert r["iters"] <= bound
+
+
+def test_pcg_fp32_and_edge_cases():
+    L = 32
+    s = inputs.spectrum(L, np.float32); k = inputs.uniform_k(L).astype(np.float32); f = np.ones((L, L), np.float32)
+    r32 = orc.pcg(s, k, f, np.zeros((L, L), np.float32), 1.0, 1e-5, 100)
+    r64 = orc.pcg(s.astype(np.float64), k.astype(np.float64), f.astype(np.float64), np.zeros((L, L)), 1.0, 1e-5, 100)
+    assert r32["status"] == 0 and abs(r32["iters"] - r64["iters"]) <= 1
+    assert np.linalg.norm(r32["u"] - r64["u"]) <= 1e-4 * np.linalg.norm(r64["u"])
+    z = orc.pcg(s, k, np.zeros((L, L), np.float32), np.ones((L, L), np.float32), 1.0, 1e-5, 10)
+    assert z["iters"] == 0 and not z["u"].any()
+    m = orc.pcg(s, k, f, np.zeros((L, L), np.float32), 1.0, 1e-12, 3)
+    assert (m["iters"], m["status"]) == (3, orc.NOT_CONVERGED)
