@@ -106,6 +106,24 @@ int fcg_apply(fcg_handle h, const void* k, const void* x, void* y);
 int fcg_solve(fcg_handle h, const void* k, const void* f, void* u, double tol, int maxit,
               int* iters_host, double* rel_residual_host);
 
+/* Preconditioned conjugate gradient (the paper "used [a preconditioner] for a while",
+ * PAPER.md:175, and gives no formula: reading D4 of DESIGN.md section 10).  Textbook PCG with the spectral preconditioner
+ *     M = kbar I + C,    M^-1 r = F^-1 ( 1/(kbar + s) o F r ),
+ * the operator with every stiffness replaced by one constant kbar (e.g. the mean of k): one more transform pair per
+ * iteration, condition number of M^-1 A bounded by (max k + s_min)/(kbar + s_min) / ((min k + s_min)/(kbar + s_min))
+ * independently of L.
+ *   fcg_set_preconditioner   s: device, the same L x L spectrum given to fcg_set_spectrum (not referenced afterwards);
+ *                            kbar >= 0.  m = 1/(kbar + s) is formed element by element in the handle's dtype (one add,
+ *                            one divide) and stored like the operator's spectrum.  Requires fcg_set_spectrum first;
+ *                            a later fcg_set_spectrum or engine change invalidates it (FCG_NO_SPECTRUM from fcg_pcg_solve).
+ *   fcg_pcg_solve            arguments, stopping rule (||r||_2 <= tol ||f||_2, recurrence residual, first crossing),
+ *                            iteration count, scalars in double and determinism as fcg_solve.  FCG_BREAKDOWN also when
+ *                            r.z <= 0 or not finite (u then holds the iterate of the completed update).
+ * The loop is one CUDA graph with a device-side WHILE node at every size (6 launches per iteration). */
+int fcg_set_preconditioner(fcg_handle h, const void* s, double kbar);
+int fcg_pcg_solve(fcg_handle h, const void* k, const void* f, void* u, double tol, int maxit,
+                  int* iters_host, double* rel_residual_host);
+
 /* Same solve with HOST arrays (N reals each): copies k, f, u to library-owned device buffers, solves,
  * copies u back.  This is the end-to-end entry point timed by bench.py ("e2e"). */
 int fcg_solve_host(fcg_handle h, const void* k_host, const void* f_host, void* u_host, double tol,
@@ -141,6 +159,11 @@ int fcg_fracture(fcg_handle h, void* k, const void* f, void* u, const void* t, i
  * leaves.  u is overwritten with an unfinished iterate.  Blocks until done.  Returns FCG_NOT_CONVERGED if the
  * loop flagged completion (times then include early exits and are not meaningful). */
 int fcg_profile_iteration(fcg_handle h, const void* k, const void* f, void* u, int iters, double* ms_host);
+
+/* The same for one iteration of fcg_pcg_solve (pipelined engine only, else FCG_UNSUPPORTED): ms_host[0..5] =
+ * { P1 (u, p updates + row transforms), P2 (spectrum), P3 (q, p.q), r update + r.r + row transforms of r,
+ *   P2 (preconditioner), P3 (z, r.z) }. */
+int fcg_profile_pcg_iteration(fcg_handle h, const void* k, const void* f, void* u, int iters, double* ms_host);
 
 /* Number of this library's kernel launches enqueued by the last fcg_solve / fcg_solve_host /
  * fcg_fracture call on this handle (graph kernel nodes counted once per execution). */

@@ -21,7 +21,8 @@ FCG_OPT_LOOP_MODE, FCG_OPT_CHUNK, FCG_OPT_ROW_VARIANT, FCG_OPT_ENGINE, FCG_OPT_U
 
 EXPORTS = ["fcg_workspace_bytes", "fcg_create", "fcg_destroy", "fcg_set_option", "fcg_set_spectrum", "fcg_apply",
            "fcg_solve", "fcg_solve_host", "fcg_profile_iteration", "fcg_fft_fwd", "fcg_fft_inv", "fcg_break_step", "fcg_fracture",
-           "fcg_last_launch_count", "fcg_last_error", "fcg_version"]
+           "fcg_last_launch_count", "fcg_last_error", "fcg_version",
+           "fcg_set_preconditioner", "fcg_pcg_solve", "fcg_profile_pcg_iteration"]
 
 _lib = None
 
@@ -53,6 +54,9 @@ def lib() -> C.CDLL:
         L.fcg_break_step.argtypes = [vp, vp, vp, vp, C.POINTER(ll), C.POINTER(d)]; L.fcg_break_step.restype = i
         L.fcg_fracture.argtypes = [vp, vp, vp, vp, vp, i, d, i, vp, vp, C.POINTER(i)]; L.fcg_fracture.restype = i
         L.fcg_profile_iteration.argtypes = [vp, vp, vp, vp, i, C.POINTER(d)]; L.fcg_profile_iteration.restype = i
+        L.fcg_set_preconditioner.argtypes = [vp, vp, d]; L.fcg_set_preconditioner.restype = i
+        L.fcg_pcg_solve.argtypes = [vp, vp, vp, vp, d, i, C.POINTER(i), C.POINTER(d)]; L.fcg_pcg_solve.restype = i
+        L.fcg_profile_pcg_iteration.argtypes = [vp, vp, vp, vp, i, C.POINTER(d)]; L.fcg_profile_pcg_iteration.restype = i
         L.fcg_last_launch_count.argtypes = [vp]; L.fcg_last_launch_count.restype = ll
         L.fcg_last_error.argtypes = [vp]; L.fcg_last_error.restype = C.c_char_p
         L.fcg_version.argtypes = []; L.fcg_version.restype = C.c_char_p
@@ -142,6 +146,20 @@ class Fcg:
             self._raise(st)
         return int(it.value), float(rr.value), int(st)
 
+    def fcg_set_preconditioner(self, s: torch.Tensor, kbar: float):
+        st = self._lib.fcg_set_preconditioner(self._h, self._chk(s, self.N), float(kbar))
+        if st != FCG_OK:
+            self._raise(st)
+
+    def fcg_pcg_solve(self, k: torch.Tensor, f: torch.Tensor, u: torch.Tensor, tol: float, maxit: int):
+        """Preconditioned CG, in place on u. Returns (iters, rel_residual, status) like fcg_solve."""
+        it = C.c_int(0); rr = C.c_double(0.0)
+        st = self._lib.fcg_pcg_solve(self._h, self._chk(k, self.N), self._chk(f, self.N), self._chk(u, self.N),
+                                     float(tol), int(maxit), C.byref(it), C.byref(rr))
+        if st < 0 and st != FCG_BREAKDOWN:
+            self._raise(st)
+        return int(it.value), float(rr.value), int(st)
+
     def fcg_solve_host(self, k: torch.Tensor, f: torch.Tensor, u: torch.Tensor, tol: float, maxit: int):
         """Same with HOST tensors (pinned for full copy speed); u updated in place."""
         for t in (k, f, u):
@@ -196,6 +214,15 @@ class Fcg:
         ms = (C.c_double * 4)()
         st = self._lib.fcg_profile_iteration(self._h, self._chk(k, self.N), self._chk(f, self.N), self._chk(u, self.N),
                                              int(iters), ms)
+        if st != FCG_OK:
+            self._raise(st)
+        return [float(x) for x in ms]
+
+    def fcg_profile_pcg_iteration(self, k: torch.Tensor, f: torch.Tensor, u: torch.Tensor, iters: int):
+        """Mean device milliseconds of the six kernels of one PCG iteration; overwrites u."""
+        ms = (C.c_double * 6)()
+        st = self._lib.fcg_profile_pcg_iteration(self._h, self._chk(k, self.N), self._chk(f, self.N), self._chk(u, self.N),
+                                                 int(iters), ms)
         if st != FCG_OK:
             self._raise(st)
         return [float(x) for x in ms]

@@ -40,7 +40,7 @@ const PassTable* get_table(int L, int dtype) {
 }
 
 struct Layout {            // byte offsets into the workspace
-    size_t Tb, shat, r, p, q, tw, partial_row, partial_vec, brk_r, brk_i, scalars, brk_out, brk_ticket, total;
+    size_t Tb, shat, mhat, r, p, q, z, tw, partial_row, partial_vec, brk_r, brk_i, scalars, brk_out, brk_ticket, total;
 };
 Layout make_layout(int L, size_t w) {
     const size_t N = (size_t)L * L;
@@ -48,7 +48,9 @@ Layout make_layout(int L, size_t w) {
     auto take = [&](size_t bytes) { size_t at = off; off = align_up(off + bytes); return at; };
     o.Tb = take(N * w);                                   // (L/2) x L complex
     o.shat = take(((size_t)L / 2 + 1) * L * w);
+    o.mhat = take(((size_t)L / 2 + 1) * L * w);           // PCG: eigenvalues of M^-1, same layout as shat
     o.r = take(N * w); o.p = take(N * w); o.q = take(N * w);
+    o.z = take(N * w);                                    // PCG: z = M^-1 r
     o.tw = take((size_t)L * 2 * w);
     o.partial_row = take((size_t)L * 2 * sizeof(double));
     o.partial_vec = take(VEC_BLOCKS_MAX * sizeof(double));
@@ -62,7 +64,7 @@ Layout make_layout(int L, size_t w) {
 }
 
 struct GraphEntry {
-    const void *k, *f; void* u; double tol; int maxit, var, unroll, pdl;
+    const void *k, *f; void* u; double tol; int maxit, var, unroll, pdl, pcg;
     cudaGraph_t graph; cudaGraphExec_t exec; unsigned long long stamp;
 };
 
@@ -74,7 +76,7 @@ struct fcg_handle_s {
     cudaStream_t stream = nullptr, cap_stream = nullptr;
     char* ws = nullptr; bool own_ws = false;
     Layout lay{};
-    bool have_spectrum = false;
+    bool have_spectrum = false, have_precond = false;
     int loop_mode = 0, chunk = 16, row_var_opt = -1, engine_opt = 0, nsm = 148, unroll = 4, pdl = 0, fused_opt = 1;
     alignas(64) CUtensorMap tmap_row;   // T2 as [L/(2 NB)][L/2][128 B]: box = v2_tsub/NB lines of one row pair (row_inv2 tiles)
     alignas(64) CUtensorMap tmap_col;   // T2 as [L/(2 NB)][L/2][NB][2 complex]: box = one column x v2_abox row pairs (col2 gather / scatter)
@@ -122,7 +124,10 @@ int fail(fcg_handle h, int code, const char* msg) { if (h) h->err = msg; return 
 // ---- launch sequences (typed) ---------------------------------------------------------------
 template <typename T> struct Seq {
     fcg_handle h; cudaStream_t st; bool classic = false;      // classic: force the synchronous passes (stand-alone transforms)
+    bool pcg = false;                                         // preconditioned CG: directions from z = M^-1 r
     bool v2() const { return h->v2() && !classic; }
+    const T* mhat() const { return h->at<T>(h->lay.mhat); }
+    T* z() const { return h->at<T>(h->lay.z); }
     cx<T>* Tb() const { return h->at<cx<T>>(h->lay.Tb); }
     const cx<T>* tw() const { return h->at<cx<T>>(h->lay.tw); }
     const T* shat() const { return h->at<T>(h->lay.shat); }
@@ -130,13 +135,13 @@ template <typename T> struct Seq {
     T* p() const { return h->at<T>(h->lay.p); }
     T* q() const { return h->at<T>(h->lay.q); }
 
-    cudaError_t row_fwd(int mode, const T* x, T* u) const {
-        RowFwdArgs<T> A{}; A.mode = mode; A.x = x; A.u = u; A.p = p(); A.r = r(); A.Tb = Tb(); A.tw = tw(); A.sc = h->sc(); A.nsm = h->nsm; A.pdl = h->pdl;
+    cudaError_t row_fwd(int mode, const T* x, T* u, int check_done = 0) const {
+        RowFwdArgs<T> A{}; A.mode = mode; A.x = x; A.u = u; A.p = p(); A.r = pcg ? z() : r(); A.check_done = check_done; A.Tb = Tb(); A.tw = tw(); A.sc = h->sc(); A.nsm = h->nsm; A.pdl = h->pdl;
         ++h->launches;
         return v2() ? h->tab->row_fwd2(&A, st) : h->tab->row_fwd(h->row_var(), &A, st);
     }
-    cudaError_t col(int mode, bool cg) const {
-        ColArgs<T> A{}; A.mode = mode; A.Tb = Tb(); A.shat = shat(); A.tw = tw(); A.sc = cg ? h->sc() : nullptr; A.pdl = h->pdl;
+    cudaError_t col(int mode, bool cg, bool precond = false) const {
+        ColArgs<T> A{}; A.mode = mode; A.Tb = Tb(); A.shat = precond ? mhat() : shat(); A.tw = tw(); A.sc = cg ? h->sc() : nullptr; A.pdl = h->pdl;
         ++h->launches;
         return (v2() && mode == COL_CONV) ? h->tab->col2(&A, &h->tmap_col, st) : h->tab->col(&A, st);
     }
@@ -148,15 +153,45 @@ template <typename T> struct Seq {
         return v2() ? h->tab->row_inv2(&A, &h->tmap_row, st) : h->tab->row_inv(h->row_var(), &A, st);
     }
     // set up initial values: r = f - A u, p = 0 (first direction p = r + 0*p), rho, ||f||^2
+    // PCG: then z = M^-1 r, rho = r.z (first direction p = z + 0*p)
     cudaError_t init(const T* k, const T* f, T* u, double tol, int maxit, bool use_cond, unsigned long long cond) const {
-        SetupArgs sa{tol, maxit, use_cond ? 1 : 0, cond};
+        SetupArgs sa{tol, maxit, use_cond ? 1 : 0, cond, pcg ? 1 : 0};
         cg_setup_kernel<<<1, 32, 0, st>>>(h->sc(), sa); ++h->launches;
         cudaError_t e;
         if ((e = cudaGetLastError()) != cudaSuccess) return e;
         if ((e = row_fwd(ROWF_PLAIN, u, nullptr)) != cudaSuccess) return e;
         if ((e = col(COL_CONV, false)) != cudaSuccess) return e;
-        return row_inv(ROWI_RESID, k, u, f, r(), p());
+        if ((e = row_inv(ROWI_RESID, k, u, f, r(), p())) != cudaSuccess) return e;
+        if (!pcg) return e;
+        if ((e = row_fwd(ROWF_PLAIN, r(), nullptr, 1)) != cudaSuccess) return e;
+        return it_precond();
     }
+    // PCG: column pass with the preconditioner's spectrum, then z = inverse row transforms, r.z -> rho', beta
+    cudaError_t it_col_m() const { return col(COL_CONV, true, true); }
+    cudaError_t it_row_pre() const {
+        RowInvArgs<T> A{}; A.mode = ROWI_PRECOND; A.Tb = Tb(); A.tw = tw(); A.k = r(); A.out = z();
+        A.partial = h->at<double>(h->lay.partial_row); A.sc = h->sc(); A.nsm = h->nsm; A.pdl = h->pdl;
+        ++h->launches;
+        return v2() ? h->tab->row_inv2_pre(&A, &h->tmap_row, st) : h->tab->row_inv(h->row_var(), &A, st);
+    }
+    cudaError_t it_precond() const {
+        cudaError_t e = it_col_m();
+        return e != cudaSuccess ? e : it_row_pre();
+    }
+    // PCG: r -= alpha q, r.r, count, convergence, and the row transforms of the new r -- one pass with the pipelined
+    // engine, the vector kernel followed by a plain row pass with the classic one
+    cudaError_t it_rupd() const {
+        if (!v2()) {
+            cudaError_t e = it_update_r();
+            return e != cudaSuccess ? e : row_fwd(ROWF_PLAIN, r(), nullptr, 1);
+        }
+        RowFwdArgs<T> A{}; A.mode = ROWF_RUPD; A.rw = r(); A.q = q(); A.Tb = Tb(); A.tw = tw(); A.sc = h->sc(); A.nsm = h->nsm; A.pdl = h->pdl;
+        A.partial = h->at<double>(h->lay.partial_vec);
+        ++h->launches;
+        return h->tab->row_fwd2_rupd(&A, st);
+    }
+    int launches_per_iteration() const { return pcg ? (v2() ? 6 : 7) : 4; }
+    int launches_outside_loop() const { return pcg ? 8 : 5; }
     // one pass of Listing 2, as four launches
     cudaError_t it_row_fwd(T* u) const { return row_fwd(ROWF_CG, nullptr, u); }                    // new x (lagged), new p, row transform
     cudaError_t it_col() const { return col(COL_CONV, true); }                                     // column transform * spectrum * inverse
@@ -177,7 +212,9 @@ template <typename T> struct Seq {
         if ((e = it_row_fwd(u)) != cudaSuccess) return e;
         if ((e = it_col()) != cudaSuccess) return e;
         if ((e = it_row_inv(k)) != cudaSuccess) return e;
-        return it_update_r();
+        if (!pcg) return it_update_r();
+        if ((e = it_rupd()) != cudaSuccess) return e;
+        return it_precond();
     }
     cudaError_t finish(T* u) const {
         const size_t nvec = h->N / Vec<T>::W;
@@ -200,7 +237,7 @@ template <typename T>
 cudaError_t build_graph(fcg_handle h, GraphEntry& ge) {
     cudaError_t e;
     cudaStream_t cs = h->cap_stream;
-    Seq<T> s{h, cs};
+    Seq<T> s{h, cs}; s.pcg = ge.pcg != 0;
     const long long saved = h->launches;
     ge.graph = nullptr; ge.exec = nullptr;
     if ((e = cudaGraphCreate(&ge.graph, 0)) != cudaSuccess) return e;
@@ -246,9 +283,9 @@ cudaError_t build_graph(fcg_handle h, GraphEntry& ge) {
 }
 
 template <typename T>
-int solve_impl(fcg_handle h, const void* k, const void* f, void* u, double tol, int maxit, int* iters, double* relres) {
+int solve_impl(fcg_handle h, const void* k, const void* f, void* u, double tol, int maxit, int* iters, double* relres, bool pcg = false) {
     h->launches = 0;
-    if (h->fused()) {
+    if (h->fused() && !pcg) {
         // small lattices: the whole solve is one cooperative kernel with the vectors resident in shared memory (fcg_fused.cuh)
         FusedArgs A{};
         A.k = k; A.f = f; A.u = u; A.Tf = h->ws + h->lay.Tb; A.shat = h->ws + h->lay.shat; A.tw = h->ws + h->lay.tw;
@@ -272,14 +309,14 @@ int solve_impl(fcg_handle h, const void* k, const void* f, void* u, double tol, 
         const int var = h->v2() ? 100 : h->row_var();
         GraphEntry* hit = nullptr;
         for (auto& g : h->graphs)
-            if (g.k == k && g.f == f && g.u == u && g.tol == tol && g.maxit == maxit && g.var == var && g.unroll == h->unroll && g.pdl == h->pdl) { hit = &g; break; }
+            if (g.k == k && g.f == f && g.u == u && g.tol == tol && g.maxit == maxit && g.var == var && g.unroll == h->unroll && g.pdl == h->pdl && g.pcg == (pcg ? 1 : 0)) { hit = &g; break; }
         if (!hit) {
             if (h->graphs.size() >= 8) {
                 size_t lru = 0;
                 for (size_t i = 1; i < h->graphs.size(); ++i) if (h->graphs[i].stamp < h->graphs[lru].stamp) lru = i;
                 drop_graph(h->graphs[lru]); h->graphs.erase(h->graphs.begin() + lru);
             }
-            GraphEntry ge{k, f, u, tol, maxit, var, h->unroll, h->pdl, nullptr, nullptr, 0};
+            GraphEntry ge{k, f, u, tol, maxit, var, h->unroll, h->pdl, pcg ? 1 : 0, nullptr, nullptr, 0};
             cudaError_t e = build_graph<T>(h, ge);
             if (e != cudaSuccess) {
                 // conditional graph nodes unavailable: fall back to direct launches for the rest of this handle's life
@@ -299,11 +336,12 @@ int solve_impl(fcg_handle h, const void* k, const void* f, void* u, double tol, 
             FCG_CK(h, cudaGraphLaunch(hit->exec, h->stream));
             FCG_CK(h, cudaStreamSynchronize(h->stream));
             const long long U = hit->unroll;
-            h->launches = 5 + 4LL * U * ((h->h_sc->it + U - 1) / U);      // no-op kernels after the stop are launches too
+            Seq<T> sq{h, h->stream}; sq.pcg = pcg;
+            h->launches = sq.launches_outside_loop() + sq.launches_per_iteration() * U * ((h->h_sc->it + U - 1) / U);   // no-op kernels after the stop are launches too
         }
     }
     if (h->loop_mode != 0) {
-        Seq<T> s{h, h->stream};
+        Seq<T> s{h, h->stream}; s.pcg = pcg;
         FCG_CK(h, s.init((const T*)k, (const T*)f, (T*)u, tol, maxit, false, 0ULL));
         FCG_CK(h, cudaMemcpyAsync(h->h_sc, h->sc(), sizeof(Scalars), cudaMemcpyDeviceToHost, h->stream));
         FCG_CK(h, cudaStreamSynchronize(h->stream));
@@ -406,6 +444,49 @@ int profile_impl(fcg_handle h, const void* k, const void* f, void* u, int iters,
         }
     for (auto& e : ev) cudaEventDestroy(e);
     return h->h_sc->done ? FCG_NOT_CONVERGED : FCG_OK;       // done would mean the loop kernels exited early
+}
+
+// PCG: per-kernel device times of one iteration, ms[0..5] = { P1, P2 (spectrum), P3, r update + row transforms of r,
+// P2 (preconditioner), P3 (z, r.z) }; pipelined engine only.
+template <typename T>
+int profile_pcg_impl(fcg_handle h, const void* k, const void* f, void* u, int iters, double* ms) {
+    Seq<T> s{h, h->stream}; s.pcg = true;
+    h->launches = 0;
+    FCG_CK(h, s.init((const T*)k, (const T*)f, (T*)u, 0.0, 1 << 30, false, 0ULL));
+    for (int w = 0; w < 2; ++w) FCG_CK(h, s.iteration((const T*)k, (T*)u));
+    std::vector<cudaEvent_t> ev((size_t)iters * 7);
+    for (auto& e : ev) FCG_CK(h, cudaEventCreate(&e));
+    for (int i = 0; i < iters; ++i) {
+        cudaEvent_t* e = &ev[(size_t)i * 7];
+        FCG_CK(h, cudaEventRecord(e[0], h->stream)); FCG_CK(h, s.it_row_fwd((T*)u));
+        FCG_CK(h, cudaEventRecord(e[1], h->stream)); FCG_CK(h, s.it_col());
+        FCG_CK(h, cudaEventRecord(e[2], h->stream)); FCG_CK(h, s.it_row_inv((const T*)k));
+        FCG_CK(h, cudaEventRecord(e[3], h->stream)); FCG_CK(h, s.it_rupd());
+        FCG_CK(h, cudaEventRecord(e[4], h->stream)); FCG_CK(h, s.it_col_m());
+        FCG_CK(h, cudaEventRecord(e[5], h->stream)); FCG_CK(h, s.it_row_pre());
+        FCG_CK(h, cudaEventRecord(e[6], h->stream));
+    }
+    FCG_CK(h, cudaMemcpyAsync(h->h_sc, h->sc(), sizeof(Scalars), cudaMemcpyDeviceToHost, h->stream));
+    FCG_CK(h, cudaStreamSynchronize(h->stream));
+    for (int q = 0; q < 6; ++q) ms[q] = 0.0;
+    for (int i = 0; i < iters; ++i)
+        for (int q = 0; q < 6; ++q) {
+            float t = 0.f;
+            FCG_CK(h, cudaEventElapsedTime(&t, ev[(size_t)i * 7 + q], ev[(size_t)i * 7 + q + 1]));
+            ms[q] += (double)t / iters;
+        }
+    for (auto& e : ev) cudaEventDestroy(e);
+    return h->h_sc->done ? FCG_NOT_CONVERGED : FCG_OK;
+}
+
+template <typename T>
+int precond_impl(fcg_handle h, const void* s, double kbar) {
+    // m = 1 / (kbar + s) into z (free between solves), then the same preparation as the operator's spectrum
+    precond_spectrum_kernel<T><<<h->vec_blocks(), 256, 0, h->stream>>>((const T*)s, h->at<T>(h->lay.z), h->N, (T)kbar);
+    FCG_CK(h, cudaGetLastError());
+    FCG_CK(h, h->tab->spectrum_prep(h->at<void>(h->lay.z), h->at<void>(h->lay.mhat), h->spectrum_colpos, h->stream));
+    FCG_CK(h, cudaStreamSynchronize(h->stream));
+    return FCG_OK;
 }
 
 template <typename T>
@@ -536,7 +617,7 @@ int fcg_set_option(fcg_handle h, int option, int value) {
         case FCG_OPT_ENGINE:
             if (value != 0 && value != 1) return fail(h, FCG_INVALID_ARG, "engine must be 0 or 1");
             h->engine_opt = value;
-            if (h->have_spectrum && h->spectrum_colpos != (h->v2() ? 1 : 0)) h->have_spectrum = false;   // stored layout belongs to the other engine
+            if (h->have_spectrum && h->spectrum_colpos != (h->v2() ? 1 : 0)) { h->have_spectrum = false; h->have_precond = false; }   // stored layout belongs to the other engine
             return FCG_OK;
     }
     return fail(h, FCG_INVALID_ARG, "unknown option");
@@ -547,7 +628,7 @@ int fcg_set_spectrum(fcg_handle h, const void* s) {
     h->spectrum_colpos = h->v2() ? 1 : 0;
     FCG_CK(h, h->tab->spectrum_prep(s, h->at<void>(h->lay.shat), h->spectrum_colpos, h->stream));
     FCG_CK(h, cudaStreamSynchronize(h->stream));      // the caller's array is not referenced after return
-    h->have_spectrum = true;
+    h->have_spectrum = true; h->have_precond = false;
     return FCG_OK;
 }
 
@@ -564,6 +645,31 @@ int fcg_solve(fcg_handle h, const void* k, const void* f, void* u, double tol, i
     if (!h->have_spectrum) return fail(h, FCG_NO_SPECTRUM, "fcg_set_spectrum has not been called");
     return h->dtype == FCG_F64 ? solve_impl<double>(h, k, f, u, tol, maxit, iters_host, rel_residual_host)
                                : solve_impl<float>(h, k, f, u, tol, maxit, iters_host, rel_residual_host);
+}
+
+int fcg_set_preconditioner(fcg_handle h, const void* s, double kbar) {
+    if (!h || !s) return fail(h, FCG_INVALID_ARG, "null argument");
+    if (!(kbar >= 0.0) || !std::isfinite(kbar)) return fail(h, FCG_INVALID_ARG, "kbar must be finite and >= 0");
+    if (!h->have_spectrum) return fail(h, FCG_NO_SPECTRUM, "fcg_set_spectrum has not been called");
+    int st = h->dtype == FCG_F64 ? precond_impl<double>(h, s, kbar) : precond_impl<float>(h, s, kbar);
+    if (st == FCG_OK) h->have_precond = true;
+    return st;
+}
+
+int fcg_pcg_solve(fcg_handle h, const void* k, const void* f, void* u, double tol, int maxit, int* iters_host, double* rel_residual_host) {
+    if (!h || !k || !f || !u) return fail(h, FCG_INVALID_ARG, "null argument");
+    if (!(tol >= 0.0) || maxit < 0) return fail(h, FCG_INVALID_ARG, "tol must be >= 0 and maxit >= 0");
+    if (!h->have_spectrum) return fail(h, FCG_NO_SPECTRUM, "fcg_set_spectrum has not been called");
+    if (!h->have_precond) return fail(h, FCG_NO_SPECTRUM, "fcg_set_preconditioner has not been called");
+    return h->dtype == FCG_F64 ? solve_impl<double>(h, k, f, u, tol, maxit, iters_host, rel_residual_host, true)
+                               : solve_impl<float>(h, k, f, u, tol, maxit, iters_host, rel_residual_host, true);
+}
+
+int fcg_profile_pcg_iteration(fcg_handle h, const void* k, const void* f, void* u, int iters, double* ms_host) {
+    if (!h || !k || !f || !u || iters < 1 || !ms_host) return fail(h, FCG_INVALID_ARG, "bad argument");
+    if (!h->have_spectrum || !h->have_precond) return fail(h, FCG_NO_SPECTRUM, "spectrum or preconditioner not set");
+    if (!h->v2()) return fail(h, FCG_UNSUPPORTED, "pipelined engine only");
+    return h->dtype == FCG_F64 ? profile_pcg_impl<double>(h, k, f, u, iters, ms_host) : profile_pcg_impl<float>(h, k, f, u, iters, ms_host);
 }
 
 int fcg_solve_host(fcg_handle h, const void* k_host, const void* f_host, void* u_host, double tol, int maxit,

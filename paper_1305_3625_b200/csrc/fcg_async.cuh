@@ -110,14 +110,17 @@ template <typename P> constexpr int per_max() {
 // Warp-specialised: NT consumer threads + one producer warp that only issues the strip copies, so the ring runs
 // ahead across transforms (while one transform is in its butterfly stages the next one's strips are landing) and
 // no consumer ever spends issue slots on address arithmetic for TMA.
-template <typename T, typename P, int CTAS>
+// RUPD = true (a separate instantiation, so that the CG kernel's register allocation is untouched) is the PCG pass
+//   r -= alpha q;  partial r.r -> last CTA: count, convergence;  columns of T2 = row transforms of the new r
+// whose strips are r0 r1 q0 q1 (4 pieces) and which ends with the grid-wide reduction of cg_update_r_kernel.
+template <typename T, typename P, int CTAS, bool RUPD = false>
 __global__ void __launch_bounds__(P::NT + 32, CTAS) row_fwd2_kernel(const RowFwdArgs<T> A)
 {
     using AS = AsyncShape<T, P>;
     constexpr int L = P::N, S = P::S, NT = P::NT, R1 = AS::R1, Q1 = AS::Q1, PER1 = AS::PER1, PM = per_max<P>();
     constexpr uint32_t PIECE = AS::PIECE;
-    constexpr int NSLOT = AS::NFS;
-    constexpr uint32_t SLOTB = AS::FSLOTB;
+    constexpr int NSLOT = RUPD ? (AS::NFS * 6 / 4 > AS::MAXSLOT ? AS::MAXSLOT : AS::NFS * 6 / 4) : AS::NFS;
+    constexpr uint32_t SLOTB = RUPD ? 4 * PIECE : AS::FSLOTB;
     extern __shared__ unsigned char smem_dyn[];
     unsigned char* const smem_raw = align128(smem_dyn);
     unsigned char* const ring = smem_raw + AS::WBYTES;
@@ -126,8 +129,8 @@ __global__ void __launch_bounds__(P::NT + 32, CTAS) row_fwd2_kernel(const RowFwd
     cx<T>* W = reinterpret_cast<cx<T>*>(smem_raw);
     SmemIO<T, P> io{W};
     const int lt = threadIdx.x, lane = lt & 31, warp = lt >> 5;
-    const bool cg = A.mode == ROWF_CG;
-    const int nv = cg ? 6 : 2;
+    const bool cg = !RUPD && A.mode == ROWF_CG;
+    const int nv = RUPD ? 4 : (cg ? 6 : 2);
     tma::grid_dep_launch();
     // Always true, but opaque to the compiler: guarding the global stores with it keeps them in basic blocks of their own
     // instead of interleaved with the shared-memory loads of the next strip.  Measured at L=2048 fp64: 39 vs 44 us.
@@ -147,12 +150,13 @@ __global__ void __launch_bounds__(P::NT + 32, CTAS) row_fwd2_kernel(const RowFwd
     }
     __syncthreads();
     tma::grid_dep_wait();                                         // everything above overlaps the previous kernel's tail
-    if (cg && A.sc->done) return;                                 // converged: nothing may change
+    if ((cg || RUPD || A.check_done) && A.sc->done) return;       // converged: nothing may change
+    double acc[1] = {0.0};
 
     if (warp == NT / 32) {
         // ---- producer warp: strip g = (transform g / R1, strip g % R1) = elements [t Q1, (t+1) Q1) of
         //      p0 p1 r0 r1 u0 u1 (or x0 x1), one bulk copy per lane < nv, into slot g % NSLOT
-        const T* base = cg ? (lane < 2 ? A.p : lane < 4 ? A.r : A.u) : A.x;
+        const T* base = RUPD ? (lane < 2 ? (const T*)A.rw : A.q) : cg ? (lane < 2 ? A.p : lane < 4 ? A.r : A.u) : A.x;
         base += (size_t)(lane & 1) * L;
         unsigned char* dst = ring + (size_t)lane * PIECE;
         int slot = 0;
@@ -165,12 +169,14 @@ __global__ void __launch_bounds__(P::NT + 32, CTAS) row_fwd2_kernel(const RowFwd
                 tma::bulk_g2s(dst + (size_t)slot * SLOTB, base + (size_t)(2 * tile_of(g / R1)) * L + (size_t)(g % R1) * Q1, PIECE, &full[slot]);
             if (++slot == NSLOT) { slot = 0; phase ^= 1u; }
         }
-        return;
+        if constexpr (!RUPD) return;
     }
 
     // ---- consumers
+    if (!RUPD || warp < NT / 32) {
     T alpha = (T)0, beta = (T)0;
     if (cg) { alpha = (T)A.sc->alpha; beta = (T)A.sc->beta; }
+    if (RUPD) alpha = (T)A.sc->alpha;
     cx<T> wb[S + 1][PM];
     static_for_up<1, S - 1>([&](auto s) { base_tw<P, decltype(s)::value, T>(lt, A.tw, wb[decltype(s)::value]); });
 
@@ -188,7 +194,15 @@ __global__ void __launch_bounds__(P::NT + 32, CTAS) row_fwd2_kernel(const RowFwd
 #pragma unroll
             for (int q = 0; q < PER1; ++q) {
                 const int j = lt + q * NT;
-                if (cg) {
+                if constexpr (RUPD) {
+                    T r0 = sl[j], r1 = sl[Q1 + j];
+                    const T q0 = sl[2 * Q1 + j], q1 = sl[3 * Q1 + j];
+                    r0 = r0 - alpha * q0; r1 = r1 - alpha * q1;       // residue
+                    const size_t i0 = row0 + (size_t)t * Q1 + j;
+                    if (st_on) { A.rw[i0] = r0; A.rw[i0 + L] = r1; }
+                    acc[0] += (double)r0 * (double)r0; acc[0] += (double)r1 * (double)r1;   // residue length
+                    z[q][t] = mk<T>(r0, r1);
+                } else if (cg) {
                     T p0 = sl[j], p1 = sl[Q1 + j];
                     const T r0 = sl[2 * Q1 + j], r1 = sl[3 * Q1 + j];
                     T u0 = sl[4 * Q1 + j], u1 = sl[5 * Q1 + j];
@@ -202,7 +216,7 @@ __global__ void __launch_bounds__(P::NT + 32, CTAS) row_fwd2_kernel(const RowFwd
                 }
             }
             if (i * R1 + t + NSLOT < G) {                               // this warp has read the slot
-                if (cg) tma::mbar_warp_release_consumed(&empty[slot]);  // (values already used by the update above)
+                if (cg || RUPD) tma::mbar_warp_release_consumed(&empty[slot]);  // (values already used by the update above)
                 else tma::mbar_warp_release(&empty[slot]);
             }
             if (++slot == NSLOT) { slot = 0; phase ^= 1u; }
@@ -238,6 +252,13 @@ __global__ void __launch_bounds__(P::NT + 32, CTAS) row_fwd2_kernel(const RowFwd
             }
             if (st_on) store_pair<T>(A.Tb + AS::t2_index(m, a0 >> 1), X0, X1);
         }
+    }
+    }
+    if constexpr (RUPD) {        // all warps (the producer contributes zero): r.r, count, convergence
+        __shared__ double red[32];
+        double tot[1];
+        if (!grid_sum_last<1>(acc, A.partial, &A.sc->ticket[1], red, tot)) return;
+        if (threadIdx.x == 0) cg_after_rr(A.sc, tot[0]);
     }
 }
 
@@ -504,7 +525,8 @@ __global__ void __launch_bounds__(256) t2_import_kernel(const cx<T>* __restrict_
 // Persistent and warp-specialised like P1.  The producer warp feeds two rings in consumption order: tiles of T2
 // (TSUB columns x 2 rows as whole 128-byte lines, TMA tensor loads) for the rebuild of the packed spectrum, and strips
 // of k, p (, f) for the epilogue; both run ahead across transforms as far as shared memory allows.
-template <typename T, typename P, int CTAS>
+// PRE = true (a separate instantiation) is the preconditioner pass of PCG: z = c, partial r.z, strips r0 r1 (k = r).
+template <typename T, typename P, int CTAS, bool PRE = false>
 __global__ void __launch_bounds__(AsyncShape<T, P>::INV_THREADS, CTAS) row_inv2_kernel(const RowInvArgs<T> A, const __grid_constant__ CUtensorMap tmap)
 {
     using AS = AsyncShape<T, P>;
@@ -522,10 +544,10 @@ __global__ void __launch_bounds__(AsyncShape<T, P>::INV_THREADS, CTAS) row_inv2_
     unsigned char* const kring = tring + (size_t)NTS * AS::TSB;
     SmemIO<T, P> io{W};
     const int lt = threadIdx.x, lane = lt & 31, warp = lt >> 5;
-    const int mode = A.mode;
+    const int mode = PRE ? (int)ROWI_PRECOND : A.mode;
     tma::grid_dep_launch();
-    const bool st_on = mode >= 0;                                 // always true, opaque to the compiler (as in row_fwd2_kernel)
-    const int nv = mode == ROWI_PLAIN ? 0 : (mode == ROWI_RESID ? 6 : 4);
+    const bool st_on = A.mode >= 0;                               // always true, opaque to the compiler (as in row_fwd2_kernel)
+    const int nv = PRE ? 2 : (mode == ROWI_PLAIN ? 0 : (mode == ROWI_RESID ? 6 : 4));
     int nks = nv ? (int)(AS::KRB / (nv * PIECE)) : 1;
     nks = nks > AS::MAXSLOT ? AS::MAXSLOT : nks;
     const uint32_t kslotb = nv * PIECE;
@@ -544,7 +566,7 @@ __global__ void __launch_bounds__(AsyncShape<T, P>::INV_THREADS, CTAS) row_inv2_
     }
     __syncthreads();
     tma::grid_dep_wait();                                         // everything above overlaps the previous kernel's tail
-    if (mode == ROWI_CG && A.sc->done) return;
+    if ((mode == ROWI_CG || PRE) && A.sc->done) return;
 
     double acc[2] = {0.0, 0.0};
     // Producer state: next tile of T2 / next strip to issue, in consumption order.  With PW (small transforms) two extra
@@ -640,6 +662,11 @@ __global__ void __launch_bounds__(AsyncShape<T, P>::INV_THREADS, CTAS) row_inv2_
                     const size_t i0 = row0 + (size_t)t * Q1 + j;
                     const T c0 = c[q][t].x, c1 = c[q][t].y;
                     if (mode == ROWI_PLAIN) { A.out[i0] = c0 * A.scale; A.out[i0 + L] = c1 * A.scale; continue; }
+                    if constexpr (PRE) {                                                   // z = M^-1 r, r.z
+                        if (st_on) { A.out[i0] = c0; A.out[i0 + L] = c1; }
+                        acc[0] += (double)sl[j] * (double)c0; acc[0] += (double)sl[Q1 + j] * (double)c1;
+                        continue;
+                    }
                     const T v0 = sl[2 * Q1 + j], v1 = sl[3 * Q1 + j];
                     const T val0 = sl[j] * v0 + c0, val1 = sl[Q1 + j] * v1 + c1;         // k o x + C x
                     if (mode == ROWI_RESID) {

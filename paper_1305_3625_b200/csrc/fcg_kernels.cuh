@@ -82,7 +82,7 @@ __device__ __forceinline__ bool grid_sum_last(double (&v)[NV], double* partial, 
 template <typename T, typename P, int F>
 __global__ void __launch_bounds__(F * P::NT) row_fwd_kernel(const RowFwdArgs<T> A) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    if (A.mode == ROWF_CG && A.sc->done) return;
+    if ((A.mode == ROWF_CG || A.check_done) && A.sc->done) return;
     DevRunner run;
     row_fwd_body<T, P, F>(A, (int)blockIdx.x, reinterpret_cast<cx<T>*>(smem_raw), run);
 }
@@ -99,7 +99,7 @@ __global__ void __launch_bounds__(COLS * P::NT) col_kernel(const ColArgs<T> A) {
 // search length alpha = rho / p.Ap in the loop, or the initial values after the residual pass.
 template <typename T>
 __device__ __forceinline__ void row_inv_reduce_finalize(const RowInvArgs<T>& A, double (&acc)[2], double* red) {
-    if (A.mode != ROWI_CG && A.mode != ROWI_RESID) return;
+    if (A.mode != ROWI_CG && A.mode != ROWI_RESID && A.mode != ROWI_PRECOND) return;
     double tot[2];
     if (!grid_sum_last<2>(acc, A.partial, &A.sc->ticket[0], red, tot)) return;
     if (threadIdx.x != 0) return;
@@ -109,9 +109,14 @@ __device__ __forceinline__ void row_inv_reduce_finalize(const RowInvArgs<T>& A, 
         sc->pq = pq;
         if (!(pq > 0.0) || !isfinite(pq)) { sc->status = ST_BREAKDOWN; sc->done = 1; sc->alpha = 0.0; }
         else sc->alpha = sc->rho / pq;                                   // search length
+    } else if (A.mode == ROWI_PRECOND) {                                 // PCG: rho' = r.z, beta = rho'/rho (first direction: p = z)
+        const double rho_new = tot[0];
+        if (!(rho_new > 0.0) || !isfinite(rho_new)) { sc->status = ST_BREAKDOWN; sc->done = 1; }
+        else { sc->beta = sc->it == 0 ? 0.0 : rho_new / sc->rho; sc->rho = rho_new; }
+        set_cond(sc, !sc->done);
     } else {                                                             // set up initial values
         const double rho = tot[0], fn2 = tot[1];
-        sc->rho = rho; sc->fn2 = fn2; sc->it = 0; sc->alpha = 0.0; sc->beta = 0.0;
+        sc->rho = rho; sc->rr = rho; sc->fn2 = fn2; sc->it = 0; sc->alpha = 0.0; sc->beta = 0.0;
         if (fn2 == 0.0) { sc->zero_u = 1; sc->done = 1; sc->status = ST_OK; sc->rho = 0.0; sc->relres = 0.0; }
         else {
             sc->relres = sqrt(rho) / sqrt(fn2);
@@ -126,7 +131,7 @@ template <typename T, typename P, int F>
 __global__ void __launch_bounds__(F * P::NT) row_inv_kernel(const RowInvArgs<T> A) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ double red[2 * 32];
-    if (A.mode == ROWI_CG && A.sc->done) return;
+    if ((A.mode == ROWI_CG || A.mode == ROWI_PRECOND) && A.sc->done) return;
     DevRunner run;
     double acc[2] = {0.0, 0.0};
     row_inv_body<T, P, F>(A, (int)blockIdx.x, reinterpret_cast<cx<T>*>(smem_raw), run, acc);
@@ -140,15 +145,23 @@ __global__ void spectrum_prep_kernel(const T* __restrict__ s, T* __restrict__ sh
         spectrum_prep_one<T, P>(idx, s, shat, colpos);
 }
 
+// Eigenvalues of the spectral preconditioner's inverse: M = kbar I + C  =>  m = 1 / (kbar + s),
+// element by element in the working precision (one add, one divide), as the oracle forms it.
+template <typename T>
+__global__ void __launch_bounds__(256) precond_spectrum_kernel(const T* __restrict__ s, T* __restrict__ m, size_t n, T kbar) {
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x)
+        m[i] = (T)1 / (kbar + s[i]);
+}
+
 // ------------------------------------------------------------------------------- CG vector kernels
-struct SetupArgs { double tol; int maxit; int use_cond; unsigned long long cond; };
+struct SetupArgs { double tol; int maxit; int use_cond; unsigned long long cond; int pcg; };
 
 #ifdef FCG_MAIN_TU   // non-template kernel: defined in fcg.cu only
 __global__ void cg_setup_kernel(Scalars* sc, SetupArgs a) {
     if (threadIdx.x == 0 && blockIdx.x == 0) {
         sc->rho = 0; sc->pq = 0; sc->alpha = 0; sc->beta = 0; sc->fn2 = 0; sc->relres = 0;
         sc->tol = a.tol; sc->maxit = a.maxit; sc->it = 0; sc->done = 0; sc->status = 0; sc->zero_u = 0;
-        sc->use_cond = a.use_cond; sc->cond = a.cond;
+        sc->use_cond = a.use_cond; sc->cond = a.cond; sc->pcg = a.pcg; sc->rr = 0;
         sc->ticket[0] = sc->ticket[1] = sc->ticket[2] = sc->ticket[3] = 0u;
     }
 }
@@ -166,6 +179,20 @@ __device__ __forceinline__ void axpy_sq(float4& r, const float4 q, float a, doub
     r.x = r.x - a * q.x; r.y = r.y - a * q.y; r.z = r.z - a * q.z; r.w = r.w - a * q.w;
     acc += (double)r.x * (double)r.x; acc += (double)r.y * (double)r.y;
     acc += (double)r.z * (double)r.z; acc += (double)r.w * (double)r.w;
+}
+
+// scalar step after the residue length r.r is known: count, convergence / maxit, beta.
+// PCG keeps rho = r.z: there beta follows from the preconditioner pass (row_inv_reduce_finalize, ROWI_PRECOND).
+__device__ __forceinline__ void cg_after_rr(Scalars* sc, double rho_new) {
+    const double fn2 = sc->fn2;
+    const int it = sc->it + 1;
+    sc->it = it;
+    if (sqrt(rho_new) <= sc->tol * sqrt(fn2)) { sc->done = 1; sc->status = ST_OK; }
+    else if (it >= sc->maxit) { sc->done = 1; sc->status = ST_NOT_CONVERGED; }
+    else if (!sc->pcg) sc->beta = rho_new / sc->rho;
+    if (sc->pcg) sc->rr = rho_new; else sc->rho = rho_new;
+    sc->relres = sqrt(rho_new) / sqrt(fn2);
+    set_cond(sc, !sc->done);
 }
 
 // residue, residue length (97), update calculation variables (98: beta), check convergence (99)
@@ -203,15 +230,7 @@ __global__ void __launch_bounds__(256) cg_update_r_kernel(T* __restrict__ r, con
     double tot[1];
     if (!grid_sum_last<1>(acc, partial, &sc->ticket[1], red, tot)) return;
     if (threadIdx.x != 0) return;
-    const double rho_new = tot[0], fn2 = sc->fn2;
-    const int it = sc->it + 1;
-    sc->it = it;
-    if (sqrt(rho_new) <= sc->tol * sqrt(fn2)) { sc->done = 1; sc->status = ST_OK; }
-    else if (it >= sc->maxit) { sc->done = 1; sc->status = ST_NOT_CONVERGED; }
-    else sc->beta = rho_new / sc->rho;
-    sc->rho = rho_new;
-    sc->relres = sqrt(rho_new) / sqrt(fn2);
-    set_cond(sc, !sc->done);
+    cg_after_rr(sc, tot[0]);
 }
 
 // last lagged "new x" after the loop has ended; u = 0 when f = 0

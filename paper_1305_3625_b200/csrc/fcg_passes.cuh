@@ -29,10 +29,12 @@ struct Scalars {
     unsigned int ticket[4];
     unsigned long long cond;       // cudaGraphConditionalHandle of the WHILE node (loop mode 0)
     int steps_done, pad_;          // fused quasi-static loop: completed break steps
+    int pcg, pad2_;                // 1: preconditioned CG (rho = r.z, rr = r.r kept apart)
+    double rr;                     // PCG: r.r of the current residual
 };
 
-enum { ROWF_PLAIN = 0, ROWF_CG = 1 };
-enum { ROWI_PLAIN = 0, ROWI_CG = 1, ROWI_RESID = 2, ROWI_APPLY = 3 };
+enum { ROWF_PLAIN = 0, ROWF_CG = 1, ROWF_RUPD = 2 };   // RUPD (PCG): r -= alpha q, partial r.r, row transforms of r
+enum { ROWI_PLAIN = 0, ROWI_CG = 1, ROWI_RESID = 2, ROWI_APPLY = 3, ROWI_PRECOND = 4 };   // PRECOND (PCG): z = M^-1 r, partial r.z (k = r)
 enum { COL_CONV = 0, COL_FWD = 1, COL_INV = 2 };
 
 template <typename T> struct RowFwdArgs {
@@ -41,9 +43,13 @@ template <typename T> struct RowFwdArgs {
     T* u; T* p; const T* r;        // CG: vectors updated in place / read
     cx<T>* Tb;             // [L/2][L] transposed half spectrum
     const cx<T>* tw;       // per-stage twiddle tables (Plan::tw_off)
-    const Scalars* sc;
+    Scalars* sc;
     int nsm;               // SMs of the device (persistent passes: tile assignment)
     int pdl;               // host side: launch with programmatic stream serialization
+    int check_done;        // PLAIN inside the PCG loop: return at once when sc->done
+    const T* q;            // RUPD: q = A p (read);  r is updated in place through rw
+    T* rw;                 // RUPD: r (read / write)
+    double* partial;       // RUPD: [gridDim.x] partial r.r
 };
 
 template <typename T> struct ColArgs {
@@ -312,6 +318,9 @@ FCG_HD void row_inv_body(const RowInvArgs<T>& A, int block, cx<T>* smem, Runner&
         const size_t row0 = (size_t)(a0 + 2 * f) * L, row1 = row0 + L;
         auto emit = [&](size_t i, T c) {
             if (A.mode == ROWI_PLAIN) { A.out[i] = c * A.scale; return; }
+            if (A.mode == ROWI_PRECOND) {                          // z = M^-1 r, r.z  (PCG; k = r)
+                A.out[i] = c; acc[0] += (double)A.k[i] * (double)c; return;
+            }
             const T vi = A.v[i];
             const T val = A.k[i] * vi + c;                         // k o x + C x
             if (A.mode == ROWI_RESID) {

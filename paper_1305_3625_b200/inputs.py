@@ -108,3 +108,9 @@ def config(i: int, dtype=None, L: int | None = None, nsteps: int | None = None) 
         k = uniform_k(L); k[broken_mask(L, 20)] = 0.0
         return _mk("cfg4", L, dtype or np.float32, k, normal_f(L), 1e-5, 2000, broken="N//20")
     raise ValueError("config index must be 0..4")
+
+
+def precond_kbar(k: np.ndarray) -> float:
+    """Constant of the spectral preconditioner M = kbar I + C (reading D4): the mean stiffness,
+    accumulated in fp64.  A parameter recipe, handed unchanged to oracle and GPU."""
+    return float(np.mean(np.asarray(k, dtype=np.float64)))

@@ -1,0 +1,160 @@
+"""Parity of the preconditioned CG path (fcg_set_preconditioner / fcg_pcg_solve) with the
+oracle's oracle_pcg on the same seeded inputs, through the C ABI.  Same protocol and tolerances as test_gpu_parity.py:
+status equal, iteration count within +-2, u within 1e-9 (fp64) / 1e-4 (fp32) at equal iteration count."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import api as orc
+from paper_1305_3625_b200 import inputs
+from test_gpu_parity import B, TOL_CG, dev, handle, rel  # noqa: F401  (B is a fixture)
+
+pytestmark = pytest.mark.gpu
+
+
+def pcg_handle(B, w, kbar, **opts):
+    dt = w.dtype.type
+    h = handle(B, w.L, dt, w.s, **opts)
+    h.fcg_set_preconditioner(dev(w.s, dt), kbar)
+    return h
+
+
+def pcg_parity(B, w, **opts):
+    dt = w.dtype.type
+    kbar = inputs.precond_kbar(w.k)
+    h = pcg_handle(B, w, kbar, **opts)
+    ref = orc.pcg(w.s, w.k, w.f, w.u0, kbar, w.tol, w.maxit, history=True)
+    kd, fd = dev(w.k), dev(w.f)
+    u = dev(w.u0)
+    it, rr, st = h.fcg_pcg_solve(kd, fd, u, w.tol, w.maxit)
+    assert st == ref["status"]
+    assert abs(it - ref["iters"]) <= 2, (it, ref["iters"], ref["hist"][-4:])
+    d_nat = rel(u.cpu().numpy(), ref["u"])
+    d_pin = d_nat
+    if it != ref["iters"] and d_nat > TOL_CG[dt]:
+        u2 = dev(w.u0)
+        it2, _, _ = h.fcg_pcg_solve(kd, fd, u2, 0.0, ref["iters"])
+        assert it2 == ref["iters"]
+        d_pin = rel(u2.cpu().numpy(), ref["u"])
+    assert min(d_nat, d_pin) <= TOL_CG[dt], (d_nat, d_pin, it, ref["iters"])
+    assert rr <= w.tol and abs(rr - ref["hist"][ref["iters"]]) <= 0.6 * ref["hist"][ref["iters"]] + 1e-15
+    # pinned count, element by element: a few iterations in, where nothing depends on the stopping decision
+    npin = min(4, ref["iters"])
+    refp = orc.pcg(w.s, w.k, w.f, w.u0, kbar, 0.0, npin, history=True)
+    u3 = dev(w.u0)
+    it3, rr3, _ = h.fcg_pcg_solve(kd, fd, u3, 0.0, npin)
+    assert it3 == npin and rel(u3.cpu().numpy(), refp["u"]) <= TOL_CG[dt] * 0.1
+    assert abs(rr3 - refp["hist"][npin]) <= 1e-3 * refp["hist"][npin] + 1e-15
+    h.close()
+    return it, ref["iters"]
+
+
+@pytest.mark.parametrize("L", [16, 64, 128, 256, 512, 1024])
+@pytest.mark.parametrize("dt", [np.float64, np.float32])
+def test_pcg_config2_recipe(B, L, dt):
+    it, it_or = pcg_parity(B, inputs.config(2, dt, L=L))
+    assert it <= 16                                         # kappa(M^-1 A) <= 2.2 for k in [0.5, 1.5]: L-independent
+
+
+@pytest.mark.parametrize("cfg,L,dt", [(0, 64, np.float64), (1, 256, np.float64), (1, 512, np.float64), (4, 512, np.float32),
+                                      (4, 1024, np.float32)])
+def test_pcg_broken_sites(B, cfg, L, dt):
+    pcg_parity(B, inputs.config(cfg, dt, L=L))
+
+
+@pytest.mark.parametrize("L,dt", [(128, np.float64), (512, np.float64), (1024, np.float32)])
+def test_pcg_classic_engine_and_loop_modes(B, L, dt):
+    """Classic passes (7 launches per iteration) and direct-launch mode give the oracle's answer too; the graph and the
+    direct-launch modes of one engine are bit-identical."""
+    w = inputs.config(1, dt, L=L)
+    pcg_parity(B, w, FCG_OPT_ENGINE=1)
+    kbar = inputs.precond_kbar(w.k)
+    outs = []
+    for opts in (dict(), dict(FCG_OPT_LOOP_MODE=1, FCG_OPT_CHUNK=3), dict(FCG_OPT_UNROLL=1)):
+        h = pcg_handle(B, w, kbar, **opts)
+        u = dev(w.u0)
+        r = h.fcg_pcg_solve(dev(w.k), dev(w.f), u, w.tol, w.maxit)
+        outs.append((r, u.cpu().numpy().copy()))
+        h.close()
+    for o in outs[1:]:
+        assert o[0] == outs[0][0] and np.array_equal(o[1], outs[0][1])
+
+
+def test_pcg_exact_preconditioner_one_iteration(B):
+    """Uniform k = kbar: M = A, so PCG stops after exactly one iteration (the oracle pin, through the GPU path)."""
+    L = 256
+    w = inputs.config(2, L=L)
+    k = np.full((L, L), 0.75)
+    f = inputs.normal_f(L)
+    h = handle(B, L, np.float64, w.s)
+    h.fcg_set_preconditioner(dev(w.s), 0.75)
+    u = dev(w.u0)
+    it, rr, st = h.fcg_pcg_solve(dev(k), dev(f), u, 1e-10, 100)
+    ref = orc.pcg(w.s, k, f, w.u0, 0.75, 1e-10, 100)
+    assert (it, st) == (1, 0) and ref["iters"] == 1
+    assert rel(u.cpu().numpy(), ref["u"]) <= 1e-12
+    h.close()
+
+
+def test_pcg_edge_cases(B):
+    L = 64
+    w = inputs.config(0)
+    kbar = inputs.precond_kbar(w.k)
+    h = handle(B, L, np.float64, w.s)
+    kd, fd = dev(w.k), dev(w.f)
+    u = dev(w.u0)
+    with pytest.raises(B.FcgError) as ei:                   # preconditioner not set
+        h.fcg_pcg_solve(kd, fd, u, 1e-10, 10)
+    assert ei.value.status == B.FCG_NO_SPECTRUM
+    h.fcg_set_preconditioner(dev(w.s), kbar)
+    assert h.fcg_pcg_solve(kd, fd, u, 1e-10, 0) == (0, 1.0, B.FCG_NOT_CONVERGED)
+    assert torch.count_nonzero(u) == 0
+    it, rr, st = h.fcg_pcg_solve(kd, fd, u, 1e-10, 3)       # maxit reached
+    ref = orc.pcg(w.s, w.k, w.f, w.u0, kbar, 1e-10, 3)
+    assert (it, st) == (3, B.FCG_NOT_CONVERGED) and rel(u.cpu().numpy(), ref["u"]) <= 1e-12
+    u = dev(w.u0)                                            # warm start from the solution: zero iterations
+    it, _, st = h.fcg_pcg_solve(kd, fd, u, 1e-10, 1000)
+    assert st == 0 and h.fcg_pcg_solve(kd, fd, u, 1e-9, 1000)[::2] == (0, 0)
+    u = dev(np.ones((L, L)))                                 # f = 0
+    assert h.fcg_pcg_solve(kd, dev(np.zeros((L, L))), u, 1e-10, 10) == (0, 0.0, 0)
+    assert torch.count_nonzero(u) == 0
+    kneg = np.full((L, L), -50.0)                            # indefinite operator: breakdown, same verdict and count
+    ref = orc.pcg(w.s, kneg, w.f, w.u0, kbar, 1e-10, 50)
+    u = dev(w.u0)
+    it, rr, st = h.fcg_pcg_solve(dev(kneg), fd, u, 1e-10, 50)
+    assert ref["status"] == orc.BREAKDOWN and st == B.FCG_BREAKDOWN and it == ref["iters"]
+    assert rel(u.cpu().numpy(), ref["u"]) <= 1e-9 or np.linalg.norm(ref["u"]) == 0
+    h.fcg_set_spectrum(dev(w.s))                             # a new spectrum invalidates the preconditioner
+    with pytest.raises(B.FcgError):
+        h.fcg_pcg_solve(kd, fd, u, 1e-10, 10)
+    # CG after PCG on the same handle still works (the scalar block's mode flag is reset by every set-up)
+    h.fcg_set_preconditioner(dev(w.s), kbar)
+    u1 = dev(w.u0); h.fcg_pcg_solve(kd, fd, u1, 1e-10, 100)
+    u2 = dev(w.u0); it2, _, st2 = h.fcg_solve(kd, fd, u2, 1e-10, 100)
+    assert st2 == 0 and abs(it2 - 28) <= 2 and rel(u1.cpu().numpy(), u2.cpu().numpy()) <= 1e-8
+    h.close()
+
+
+@pytest.mark.parametrize("dt,tolpin", [(np.float64, 1e-10), (np.float32, 1e-5)])
+def test_pcg_config2_full_size(B, dt, tolpin):
+    """L = 2048 in the configuration bench.py --solver pcg times: pinned count 3 vs the oracle element by element; the
+    finished solve satisfies ||f - A_oracle u|| / ||f|| <= 2 tol with one oracle operator application; bitwise repeatable."""
+    w = inputs.config(2, dt)
+    kbar = inputs.precond_kbar(w.k)
+    h = pcg_handle(B, w, kbar)
+    kd, fd = dev(w.k), dev(w.f)
+    ref = orc.pcg(w.s, w.k, w.f, w.u0, kbar, 0.0, 3, history=True)
+    u = dev(w.u0)
+    it, rr, _ = h.fcg_pcg_solve(kd, fd, u, 0.0, 3)
+    assert it == 3 and rel(u.cpu().numpy(), ref["u"]) <= tolpin
+    assert abs(rr - ref["hist"][3]) <= 1e-3 * ref["hist"][3]
+    u = dev(w.u0)
+    it, rr, st = h.fcg_pcg_solve(kd, fd, u, w.tol, w.maxit)
+    assert st == 0 and rr <= w.tol and it <= 16
+    uh = u.cpu().numpy()
+    true_res = np.linalg.norm((w.f - orc.apply(w.s, w.k, uh)).astype(np.float64)) / np.linalg.norm(w.f.astype(np.float64))
+    assert true_res <= 2 * w.tol
+    u2 = dev(w.u0)
+    assert h.fcg_pcg_solve(kd, fd, u2, w.tol, w.maxit) == (it, rr, st) and torch.equal(u, u2)
+    assert h.fcg_last_launch_count() == 8 + 6 * 4 * ((it + 3) // 4)
+    h.close()
