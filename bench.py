@@ -29,6 +29,9 @@ METRIC, UNIT = "cg_iterations_per_s", "iter/s"
 B_ITER_NW = 16.5          # algorithmic bytes per CG iteration in units of N*w
 PASS_NW = {"row_fwd": 6.0, "col": 2.5, "row_inv": 4.0, "update_r": 3.0}   # this implementation's per-kernel algorithmic bytes / (N*w)
 PASS_NAMES = ["row_fwd", "col", "row_inv", "update_r"]
+# preconditioned CG: six kernels per iteration, 22 N*w algorithmic bytes
+PCG_NAMES = ["row_fwd", "col", "row_inv", "rupd_row_fwd", "col_precond", "row_inv_precond"]
+PCG_NW = {"row_fwd": 6.0, "col": 2.5, "row_inv": 4.0, "rupd_row_fwd": 4.0, "col_precond": 2.5, "row_inv_precond": 3.0}
 
 
 def peaks():
@@ -108,7 +111,7 @@ def run_reference(args, rank: int):
     print(json.dumps(line))
 
 
-def bench_workload(binding, torch, w, steps, warmup, profile_iters=20, e2e_steps=None, loop_mode=0):
+def bench_workload(binding, torch, w, steps, warmup, profile_iters=20, e2e_steps=None, loop_mode=0, pcg_steps=0, inputs_mod=None):
     """Times `steps` solves of workload w on the current device. Returns a dict of measurements."""
     tdt = torch.float64 if w.dtype == np.float64 else torch.float32
     wbytes = w.dtype.itemsize
@@ -151,6 +154,30 @@ def bench_workload(binding, torch, w, steps, warmup, profile_iters=20, e2e_steps
         e_it += it
     out["e2e_iter_s"] = e_it / (time.perf_counter() - t0)
     out["h2d"] = 3 * w.N * wbytes; out["d2h"] = w.N * wbytes
+    if pcg_steps:
+        # the same workload solved by preconditioned CG (time to the same tolerance; reported beside the headline, not as it)
+        kbar = inputs_mod.precond_kbar(w.k)
+        h.fcg_set_preconditioner(to(w.s), kbar)
+        for _ in range(2):
+            u.zero_(); h.fcg_pcg_solve(k, f, u, w.tol, w.maxit)
+        pev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(pcg_steps)]
+        for s in range(pcg_steps):
+            pev[s][0].record(); u.zero_()
+            pit, prr, pst = h.fcg_pcg_solve(k, f, u, w.tol, w.maxit)
+            pev[s][1].record()
+        torch.cuda.synchronize()
+        plaunch = h.fcg_last_launch_count()
+        pms = [a.elapsed_time(b) for a, b in pev]
+        u.zero_()
+        pk = h.fcg_profile_pcg_iteration(k, f, u, profile_iters)
+        out["pcg"] = {"kbar": kbar, "iterations": pit, "status": pst, "final_rel_residual": prr, "ms_per_solve": statistics.median(pms),
+                      "us_per_iteration": 1e3 * statistics.median(pms) / max(pit, 1),
+                      "cg_ms_per_solve": statistics.median(dev_ms), "solve_time_ratio_cg_over_pcg": statistics.median(dev_ms) / statistics.median(pms),
+                      "kernel_us": {n: 1e3 * x for n, x in zip(PCG_NAMES, pk)},
+                      "kernel_gbs": {n: PCG_NW[n] * w.N * wbytes / (x * 1e-3) / 1e9 for n, x in zip(PCG_NAMES, pk)},
+                      "bytes_per_iteration": sum(PCG_NW.values()) * w.N * wbytes,
+                      "iteration_gbs": sum(PCG_NW.values()) * w.N * wbytes / (statistics.median(pms) * 1e-3 / max(pit, 1)) / 1e9,
+                      "launches_per_solve": plaunch}
     h.close()
     return out
 
@@ -221,6 +248,7 @@ def main():
     ap.add_argument("--ref-iters", type=int, default=8, help="oracle CG iterations per reference step / cpu_baseline sample")
     ap.add_argument("--full", action="store_true", help="also time configs[2] fp32 and configs[4] (reported under 'extra')")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-pcg", action="store_true", help="skip the preconditioned-CG time-to-solution of the same workload ('pcg' key)")
     ap.add_argument("--loop-mode", type=int, default=0, choices=[0, 1],
                     help="0: whole solve as one CUDA graph with a device-side WHILE node (default); 1: direct launches (for ncu)")
     args = ap.parse_args()
@@ -252,6 +280,8 @@ def main():
         sampler.start()
     res = bench_workload(binding, torch, w, args.steps, args.warmup, loop_mode=args.loop_mode)
     clocks = sampler.stop() if sampler else None
+    if rank == 0 and world == 1 and not args.no_pcg and args.loop_mode == 0:      # outside the timed region of the headline
+        res["pcg"] = bench_workload(binding, torch, w, 3, 1, loop_mode=0, pcg_steps=5, inputs_mod=inputs, e2e_steps=1)["pcg"]
 
     # replicas only: every rank solves its own copy; time = max over ranks, value = sum of work
     step_ms, total_it, launches, res["e2e_iter_s"] = aggregate_over_ranks(
@@ -298,6 +328,8 @@ def main():
         "clocks": clocks,
         "final_rel_residual": res["relres"], "status": res["status"],
     }
+    if "pcg" in res:
+        line["pcg"] = res["pcg"]
     if args.full and world == 1:
         extra = {}
         for cfg, dt in ((2, np.float32), (4, np.float32)):

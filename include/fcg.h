@@ -65,6 +65,9 @@ typedef enum {
     FCG_OPT_FUSED        = 6, /* 1 (default): for L = 256 and 512 (pipelined engine, loop mode 0) a whole solve is ONE cooperative
                                  kernel with the vectors resident in shared memory and grid barriers between the phases;
                                  0: the graph of four kernels per iteration at every size */
+    FCG_OPT_L2_HINTS     = 7, /* bit mask (default 63: all) of L2 eviction-priority hints in the pipelined passes:
+                                 1 u strips (P1 loads) evict-first, 2 u stores evict-first, 4 spectrum rows (P2) evict-first,
+                                 8 T2 tiles (P3 loads) evict-first, 16 k strips (P3) evict-first, 32 q loads (P4) evict-first */
     FCG_OPT_ENGINE       = 3  /* 0 (default): pipelined TMA passes where the lattice is large enough (L >= 256), classic
                                  passes otherwise; 1: classic passes only (synchronous loads; kept for A/B measurements).
                                  The stored spectrum's layout belongs to the engine: changing the engine after

@@ -69,6 +69,9 @@ def _declare(L: C.CDLL) -> None:
         f = getattr(L, "oracle_pcg" + suf)
         f.argtypes = [_i, _vp, _vp, _vp, _vp, _d, _d, _i, C.POINTER(_i), C.POINTER(_d), _vp, _vp, _vp, _vp]
         f.restype = _i
+        f = getattr(L, "oracle_pcg_fracture" + suf)
+        f.argtypes = [_i, _vp, _vp, _vp, _vp, _vp, _d, _i, _d, _i, _vp, _vp, _vp]
+        f.restype = _i
         f = getattr(L, "oracle_break_step" + suf)
         f.argtypes = [_ll, _vp, _vp, _vp, C.POINTER(_ll), C.POINTER(_d), C.POINTER(_d)]
         f.restype = _i
@@ -220,4 +223,17 @@ def fracture(s, k, f, u, t, nsteps: int, tol: float, maxit: int):
     gap = np.full(nsteps, np.nan, np.float64)
     done = getattr(lib(), "oracle_fracture" + _suf(dt))(L, _p(s), _p(k), _p(f), _p(u), _p(t), int(nsteps),
                                                         float(tol), int(maxit), _p(index), _p(iters), _p(gap))
+    return dict(index=index, iters=iters, gap=gap, steps=int(done))
+
+
+def pcg_fracture(s, k, f, u, t, kbar: float, nsteps: int, tol: float, maxit: int):
+    """Quasi-static loop with PCG solves.  In-place on k and u. Returns dict(index, iters, gap, steps)."""
+    dt = k.dtype; L = k.shape[0]
+    s = _arr(s, dt, (L, L)); f = _arr(f, dt, (L, L)); t = _arr(t, dt, (L, L))
+    if not (k.flags.c_contiguous and u.flags.c_contiguous and u.dtype == dt):
+        raise ValueError("k, u must be C-contiguous arrays of one dtype (modified in place)")
+    index = np.full(nsteps, -1, np.int64); iters = np.zeros(nsteps, np.int32)
+    gap = np.full(nsteps, np.nan, np.float64)
+    done = getattr(lib(), "oracle_pcg_fracture" + _suf(dt))(L, _p(s), _p(k), _p(f), _p(u), _p(t), float(kbar), int(nsteps),
+                                                            float(tol), int(maxit), _p(index), _p(iters), _p(gap))
     return dict(index=index, iters=iters, gap=gap, steps=int(done))

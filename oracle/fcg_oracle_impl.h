@@ -304,3 +304,24 @@ int FN(oracle_fracture)(int L, const REAL* s, REAL* k, const REAL* f, REAL* u, c
     }
     return nsteps;
 }
+
+/* The same quasi-static loop with every solve done by oracle_pcg (preconditioner M = kbar I + C, kbar fixed for the whole
+ * loop).  The break sequence is a property of the exact solutions, so it must coincide with
+ * oracle_fracture's wherever the top-2 gap exceeds the solver error; only the iteration counts differ. */
+int FN(oracle_pcg_fracture)(int L, const REAL* s, REAL* k, const REAL* f, REAL* u, const REAL* t, double kbar,
+                            int nsteps, double tol, int maxit,
+                            long long* out_index, int* out_iters, double* out_gap)
+{
+    long long N = (long long)L * L;
+    for (int step = 0; step < nsteps; ++step) {
+        int it; double rr;
+        int st = FN(oracle_pcg)(L, s, k, f, u, kbar, tol, maxit, &it, &rr, NULL, NULL, NULL, NULL);
+        if (st < 0) return st;
+        long long idx; double ratio, second;
+        int bs = FN(oracle_break_step)(N, k, u, t, &idx, &ratio, &second);
+        if (bs < 0) return step;
+        out_index[step] = idx; out_iters[step] = it;
+        if (out_gap) out_gap[step] = (ratio - second) / fabs(ratio);
+    }
+    return nsteps;
+}

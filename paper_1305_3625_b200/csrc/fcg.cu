@@ -77,7 +77,7 @@ struct fcg_handle_s {
     char* ws = nullptr; bool own_ws = false;
     Layout lay{};
     bool have_spectrum = false, have_precond = false;
-    int loop_mode = 0, chunk = 16, row_var_opt = -1, engine_opt = 0, nsm = 148, unroll = 4, pdl = 0, fused_opt = 1;
+    int loop_mode = 0, chunk = 16, row_var_opt = -1, engine_opt = 0, nsm = 148, unroll = 4, pdl = 0, fused_opt = 1, hints = 63;
     alignas(64) CUtensorMap tmap_row;   // T2 as [L/(2 NB)][L/2][128 B]: box = v2_tsub/NB lines of one row pair (row_inv2 tiles)
     alignas(64) CUtensorMap tmap_col;   // T2 as [L/(2 NB)][L/2][NB][2 complex]: box = one column x v2_abox row pairs (col2 gather / scatter)
     bool have_tmap = false;
@@ -136,18 +136,18 @@ template <typename T> struct Seq {
     T* q() const { return h->at<T>(h->lay.q); }
 
     cudaError_t row_fwd(int mode, const T* x, T* u, int check_done = 0) const {
-        RowFwdArgs<T> A{}; A.mode = mode; A.x = x; A.u = u; A.p = p(); A.r = pcg ? z() : r(); A.check_done = check_done; A.Tb = Tb(); A.tw = tw(); A.sc = h->sc(); A.nsm = h->nsm; A.pdl = h->pdl;
+        RowFwdArgs<T> A{}; A.mode = mode; A.x = x; A.u = u; A.p = p(); A.r = pcg ? z() : r(); A.check_done = check_done; A.hints = h->hints; A.Tb = Tb(); A.tw = tw(); A.sc = h->sc(); A.nsm = h->nsm; A.pdl = h->pdl;
         ++h->launches;
         return v2() ? h->tab->row_fwd2(&A, st) : h->tab->row_fwd(h->row_var(), &A, st);
     }
     cudaError_t col(int mode, bool cg, bool precond = false) const {
-        ColArgs<T> A{}; A.mode = mode; A.Tb = Tb(); A.shat = precond ? mhat() : shat(); A.tw = tw(); A.sc = cg ? h->sc() : nullptr; A.pdl = h->pdl;
+        ColArgs<T> A{}; A.mode = mode; A.Tb = Tb(); A.shat = precond ? mhat() : shat(); A.hints = h->hints; A.tw = tw(); A.sc = cg ? h->sc() : nullptr; A.pdl = h->pdl;
         ++h->launches;
         return (v2() && mode == COL_CONV) ? h->tab->col2(&A, &h->tmap_col, st) : h->tab->col(&A, st);
     }
     cudaError_t row_inv(int mode, const T* k, const T* v, const T* f, T* out, T* out2) const {
         RowInvArgs<T> A{}; A.mode = mode; A.Tb = Tb(); A.tw = tw(); A.k = k; A.v = v; A.f = f; A.out = out; A.out2 = out2;
-        A.scale = (T)(1.0 / ((double)h->L * (double)h->L));
+        A.scale = (T)(1.0 / ((double)h->L * (double)h->L)); A.hints = h->hints;
         A.partial = h->at<double>(h->lay.partial_row); A.sc = h->sc(); A.nsm = h->nsm; A.pdl = h->pdl;
         ++h->launches;
         return v2() ? h->tab->row_inv2(&A, &h->tmap_row, st) : h->tab->row_inv(h->row_var(), &A, st);
@@ -169,7 +169,7 @@ template <typename T> struct Seq {
     // PCG: column pass with the preconditioner's spectrum, then z = inverse row transforms, r.z -> rho', beta
     cudaError_t it_col_m() const { return col(COL_CONV, true, true); }
     cudaError_t it_row_pre() const {
-        RowInvArgs<T> A{}; A.mode = ROWI_PRECOND; A.Tb = Tb(); A.tw = tw(); A.k = r(); A.out = z();
+        RowInvArgs<T> A{}; A.mode = ROWI_PRECOND; A.Tb = Tb(); A.tw = tw(); A.k = r(); A.out = z(); A.hints = h->hints;
         A.partial = h->at<double>(h->lay.partial_row); A.sc = h->sc(); A.nsm = h->nsm; A.pdl = h->pdl;
         ++h->launches;
         return v2() ? h->tab->row_inv2_pre(&A, &h->tmap_row, st) : h->tab->row_inv(h->row_var(), &A, st);
@@ -185,7 +185,7 @@ template <typename T> struct Seq {
             cudaError_t e = it_update_r();
             return e != cudaSuccess ? e : row_fwd(ROWF_PLAIN, r(), nullptr, 1);
         }
-        RowFwdArgs<T> A{}; A.mode = ROWF_RUPD; A.rw = r(); A.q = q(); A.Tb = Tb(); A.tw = tw(); A.sc = h->sc(); A.nsm = h->nsm; A.pdl = h->pdl;
+        RowFwdArgs<T> A{}; A.mode = ROWF_RUPD; A.hints = h->hints; A.rw = r(); A.q = q(); A.Tb = Tb(); A.tw = tw(); A.sc = h->sc(); A.nsm = h->nsm; A.pdl = h->pdl;
         A.partial = h->at<double>(h->lay.partial_vec);
         ++h->launches;
         return h->tab->row_fwd2_rupd(&A, st);
@@ -205,7 +205,7 @@ template <typename T> struct Seq {
         at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
         at[0].val.programmaticStreamSerializationAllowed = 1;
         cfg.attrs = at; cfg.numAttrs = h->pdl ? 1u : 0u;
-        return cudaLaunchKernelEx(&cfg, cg_update_r_kernel<T>, r(), (const T*)q(), nvec, h->at<double>(h->lay.partial_vec), h->sc());
+        return cudaLaunchKernelEx(&cfg, cg_update_r_kernel<T>, r(), (const T*)q(), nvec, h->at<double>(h->lay.partial_vec), h->sc(), h->hints);
     }
     cudaError_t iteration(const T* k, T* u) const {
         cudaError_t e;
@@ -237,7 +237,7 @@ template <typename T>
 cudaError_t build_graph(fcg_handle h, GraphEntry& ge) {
     cudaError_t e;
     cudaStream_t cs = h->cap_stream;
-    Seq<T> s{h, cs}; s.pcg = ge.pcg != 0;
+    Seq<T> s{h, cs}; s.pcg = (ge.pcg & 1) != 0;
     const long long saved = h->launches;
     ge.graph = nullptr; ge.exec = nullptr;
     if ((e = cudaGraphCreate(&ge.graph, 0)) != cudaSuccess) return e;
@@ -309,14 +309,14 @@ int solve_impl(fcg_handle h, const void* k, const void* f, void* u, double tol, 
         const int var = h->v2() ? 100 : h->row_var();
         GraphEntry* hit = nullptr;
         for (auto& g : h->graphs)
-            if (g.k == k && g.f == f && g.u == u && g.tol == tol && g.maxit == maxit && g.var == var && g.unroll == h->unroll && g.pdl == h->pdl && g.pcg == (pcg ? 1 : 0)) { hit = &g; break; }
+            if (g.k == k && g.f == f && g.u == u && g.tol == tol && g.maxit == maxit && g.var == var && g.unroll == h->unroll && g.pdl == h->pdl && g.pcg == (pcg ? 1 : 0) + 2 * h->hints) { hit = &g; break; }
         if (!hit) {
             if (h->graphs.size() >= 8) {
                 size_t lru = 0;
                 for (size_t i = 1; i < h->graphs.size(); ++i) if (h->graphs[i].stamp < h->graphs[lru].stamp) lru = i;
                 drop_graph(h->graphs[lru]); h->graphs.erase(h->graphs.begin() + lru);
             }
-            GraphEntry ge{k, f, u, tol, maxit, var, h->unroll, h->pdl, pcg ? 1 : 0, nullptr, nullptr, 0};
+            GraphEntry ge{k, f, u, tol, maxit, var, h->unroll, h->pdl, (pcg ? 1 : 0) + 2 * h->hints, nullptr, nullptr, 0};
             cudaError_t e = build_graph<T>(h, ge);
             if (e != cudaSuccess) {
                 // conditional graph nodes unavailable: fall back to direct launches for the rest of this handle's life
@@ -613,6 +613,7 @@ int fcg_set_option(fcg_handle h, int option, int value) {
             h->row_var_opt = value; return FCG_OK;
         case FCG_OPT_FUSED: if (value != 0 && value != 1) return fail(h, FCG_INVALID_ARG, "fused must be 0 or 1"); h->fused_opt = value; return FCG_OK;
         case FCG_OPT_PDL: if (value != 0 && value != 1) return fail(h, FCG_INVALID_ARG, "pdl must be 0 or 1"); h->pdl = value; return FCG_OK;
+        case FCG_OPT_L2_HINTS: if (value < 0 || value > 63) return fail(h, FCG_INVALID_ARG, "hints must be 0..63"); h->hints = value; return FCG_OK;
         case FCG_OPT_UNROLL: if (value < 1 || value > 64) return fail(h, FCG_INVALID_ARG, "unroll must be 1..64"); h->unroll = value; return FCG_OK;
         case FCG_OPT_ENGINE:
             if (value != 0 && value != 1) return fail(h, FCG_INVALID_ARG, "engine must be 0 or 1");

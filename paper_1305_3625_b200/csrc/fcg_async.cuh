@@ -161,12 +161,14 @@ __global__ void __launch_bounds__(P::NT + 32, CTAS) row_fwd2_kernel(const RowFwd
         unsigned char* dst = ring + (size_t)lane * PIECE;
         int slot = 0;
         uint32_t phase = 0;
+        // L2 hints (bit 0): u is not touched again before the next iteration's P1 -- its strips should not displace T2, q, r
+        const uint64_t pol = (cg && lane >= 4 && (A.hints & 1)) ? tma::policy_evict_first() : tma::policy_evict_normal();
         for (int g = 0; g < G; ++g) {
             if (g >= NSLOT) tma::mbar_wait(&empty[slot], phase ^ 1u);          // the slot's previous strip has been read by every warp
             if (lane == 0) tma::mbar_expect_tx(&full[slot], nv * PIECE);
             __syncwarp();
             if (lane < nv)
-                tma::bulk_g2s(dst + (size_t)slot * SLOTB, base + (size_t)(2 * tile_of(g / R1)) * L + (size_t)(g % R1) * Q1, PIECE, &full[slot]);
+                tma::bulk_g2s_hint(dst + (size_t)slot * SLOTB, base + (size_t)(2 * tile_of(g / R1)) * L + (size_t)(g % R1) * Q1, PIECE, &full[slot], pol);
             if (++slot == NSLOT) { slot = 0; phase ^= 1u; }
         }
         if constexpr (!RUPD) return;
@@ -177,6 +179,7 @@ __global__ void __launch_bounds__(P::NT + 32, CTAS) row_fwd2_kernel(const RowFwd
     T alpha = (T)0, beta = (T)0;
     if (cg) { alpha = (T)A.sc->alpha; beta = (T)A.sc->beta; }
     if (RUPD) alpha = (T)A.sc->alpha;
+    const uint64_t pol_u = (A.hints & 2) ? tma::policy_evict_first() : tma::policy_evict_normal();   // L2 hints (bit 1): the u stores
     cx<T> wb[S + 1][PM];
     static_for_up<1, S - 1>([&](auto s) { base_tw<P, decltype(s)::value, T>(lt, A.tw, wb[decltype(s)::value]); });
 
@@ -209,7 +212,7 @@ __global__ void __launch_bounds__(P::NT + 32, CTAS) row_fwd2_kernel(const RowFwd
                     u0 = u0 + alpha * p0; u1 = u1 + alpha * p1;       // new x, lagged one pass
                     p0 = r0 + beta * p0;  p1 = r1 + beta * p1;        // new direction
                     const size_t i0 = row0 + (size_t)t * Q1 + j;
-                    if (st_on) { A.u[i0] = u0; A.u[i0 + L] = u1; A.p[i0] = p0; A.p[i0 + L] = p1; }
+                    if (st_on) { tma::st_hint(A.u + i0, u0, pol_u); tma::st_hint(A.u + i0 + L, u1, pol_u); A.p[i0] = p0; A.p[i0 + L] = p1; }
                     z[q][t] = mk<T>(p0, p1);
                 } else {
                     z[q][t] = mk<T>(sl[j], sl[Q1 + j]);
@@ -295,7 +298,8 @@ __global__ void __launch_bounds__(P::NT, CTAS) col2_kernel(const ColArgs<T> A, c
 #pragma unroll
         for (int b = 0; b < (L / 2) / ABOX; ++b)
             tma::tensor_g2s_4d(smem_raw + (size_t)b * BOXB, &tmap, 0, n % AS::NB, b * ABOX, n / AS::NB, &bar);
-        if (n) tma::bulk_g2s(sh, A.shat + (size_t)n * L, (uint32_t)(L * sizeof(T)), &bar);
+        if (n) tma::bulk_g2s_hint(sh, A.shat + (size_t)n * L, (uint32_t)(L * sizeof(T)), &bar,
+                                  (A.hints & 4) ? tma::policy_evict_first() : tma::policy_evict_normal());   // read once per iteration
     }
     __syncthreads();
     const bool done = A.sc && A.sc->done;
@@ -578,11 +582,14 @@ __global__ void __launch_bounds__(AsyncShape<T, P>::INV_THREADS, CTAS) row_inv2_
     const int GT = ntl * NSUB, GK = nv ? ntl * R1 : 0;
     const T* kbase = nullptr;
     if (nv) kbase = (lane < 2 ? A.k : lane < 4 ? A.v : A.f) + (size_t)(lane & 1) * L;
+    // L2 hints: T2 is dead once this pass has read it (bit 3); k comes back only in the next iteration (bit 4)
+    const uint64_t pol_t = (A.hints & 8) ? tma::policy_evict_first() : tma::policy_evict_normal();
+    const uint64_t pol_k = (lane < 2 && !PRE && (A.hints & 16)) ? tma::policy_evict_first() : tma::policy_evict_normal();
     auto issue_next_T = [&]() {          // whole warp; tile p_tn = (transform p_tn / NSUB, part p_tn % NSUB): TSUB / NB whole lines
         if (p_tn >= NTS) tma::mbar_wait(&tempty[p_ts], p_tph ^ 1u);
         if (lane == 0) {
             tma::mbar_expect_tx(&tfull[p_ts], TBYTES);
-            tma::tensor_g2s_3d(tring + (size_t)p_ts * TBYTES, &tmap, 0, tile_of(p_tn / NSUB), (p_tn % NSUB) * (TSUB / AS::NB), &tfull[p_ts]);
+            tma::tensor_g2s_3d_hint(tring + (size_t)p_ts * TBYTES, &tmap, 0, tile_of(p_tn / NSUB), (p_tn % NSUB) * (TSUB / AS::NB), &tfull[p_ts], pol_t);
         }
         ++p_tn;
         if (++p_ts == NTS) { p_ts = 0; p_tph ^= 1u; }
@@ -592,8 +599,8 @@ __global__ void __launch_bounds__(AsyncShape<T, P>::INV_THREADS, CTAS) row_inv2_
         if (lane == 0) tma::mbar_expect_tx(&kfull[p_ks], kslotb);
         __syncwarp();
         if (lane < nv)
-            tma::bulk_g2s(kring + (size_t)p_ks * kslotb + (size_t)lane * PIECE,
-                          kbase + (size_t)(2 * tile_of(p_kn / R1)) * L + (size_t)(p_kn % R1) * Q1, PIECE, &kfull[p_ks]);
+            tma::bulk_g2s_hint(kring + (size_t)p_ks * kslotb + (size_t)lane * PIECE,
+                               kbase + (size_t)(2 * tile_of(p_kn / R1)) * L + (size_t)(p_kn % R1) * Q1, PIECE, &kfull[p_ks], pol_k);
         ++p_kn;
         if (++p_ks == nks) { p_ks = 0; p_kph ^= 1u; }
     };

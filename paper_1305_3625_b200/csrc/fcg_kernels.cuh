@@ -7,6 +7,7 @@
 #pragma once
 #include <cuda_runtime.h>
 #include "fcg_passes.cuh"
+#include "fcg_tma.cuh"
 
 namespace fcg {
 
@@ -198,7 +199,7 @@ __device__ __forceinline__ void cg_after_rr(Scalars* sc, double rho_new) {
 // residue, residue length (97), update calculation variables (98: beta), check convergence (99)
 template <typename T>
 __global__ void __launch_bounds__(256) cg_update_r_kernel(T* __restrict__ r, const T* __restrict__ q, size_t nvec,
-                                                           double* partial, Scalars* sc) {
+                                                           double* partial, Scalars* sc, int hints) {
     __shared__ double red[32];
     using V = typename Vec<T>::type;
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");    // programmatic dependent launch (fcg_tma.cuh)
@@ -209,6 +210,8 @@ __global__ void __launch_bounds__(256) cg_update_r_kernel(T* __restrict__ r, con
     }
     const T a = (T)sc->alpha;
     double acc[1] = {0.0};
+    // L2 hints (bit 5): q is dead after this pass
+    const uint64_t pol_q = (hints & 32) ? tma::policy_evict_first() : tma::policy_evict_normal();
     V* rv = reinterpret_cast<V*>(r);
     const V* qv = reinterpret_cast<const V*>(q);
     // four independent 16-byte loads of r and of q in flight per thread before any use
@@ -218,7 +221,7 @@ __global__ void __launch_bounds__(256) cg_update_r_kernel(T* __restrict__ r, con
     for (; i + (UN - 1) * stride < nvec; i += UN * stride) {
         V x[UN], y[UN];
 #pragma unroll
-        for (int c = 0; c < UN; ++c) { x[c] = rv[i + c * stride]; y[c] = __ldg(qv + i + c * stride); }
+        for (int c = 0; c < UN; ++c) { x[c] = rv[i + c * stride]; y[c] = tma::ld_hint(qv + i + c * stride, pol_q); }
 #pragma unroll
         for (int c = 0; c < UN; ++c) { axpy_sq(x[c], y[c], a, acc[0]); rv[i + c * stride] = x[c]; }
     }

@@ -50,6 +50,7 @@ template <typename T> struct RowFwdArgs {
     const T* q;            // RUPD: q = A p (read);  r is updated in place through rw
     T* rw;                 // RUPD: r (read / write)
     double* partial;       // RUPD: [gridDim.x] partial r.r
+    int hints;             // L2 eviction-priority hints (FCG_OPT_L2_HINTS bit mask; pipelined passes only)
 };
 
 template <typename T> struct ColArgs {
@@ -59,6 +60,7 @@ template <typename T> struct ColArgs {
     const cx<T>* tw;
     const Scalars* sc;
     int pdl;
+    int hints;
 };
 
 template <typename T> struct RowInvArgs {
@@ -72,6 +74,7 @@ template <typename T> struct RowInvArgs {
     Scalars* sc;
     int nsm;
     int pdl;
+    int hints;
 };
 
 template <int A, int B, typename F> FCG_HD void static_for_up(F&& f) {
