@@ -424,3 +424,39 @@ def test_pcg_fp32_and_edge_cases():
     assert z["iters"] == 0 and not z["u"].any()
     m = orc.pcg(s, k, f, np.zeros((L, L), np.float32), 1.0, 1e-12, 3)
     assert (m["iters"], m["status"]) == (3, orc.NOT_CONVERGED)
+
+
+# ---------------------------------------------------------------- quasi-static loop with PCG solves
+def test_pcg_fracture_step0_closed_form_and_sherman_morrison():
+    """P9 / P10 for the PCG loop: k = kbar = 1 makes M = A, so step 0 is ONE iteration to u = 1/(1 + L/2pi) and the first
+    break is argmin t; the second break follows from the rank-one (Sherman-Morrison) closed form."""
+    L = 32
+    s = orc.spectrum(L)
+    one = np.ones((L, L))
+    t = inputs.thresholds(L)
+    u0 = 1.0 / (1.0 + s[0, 0])
+    b = int(np.argmin(t)); ba, bb = divmod(b, L)
+    g = np.real(np.fft.ifft2(1.0 / (1.0 + s)))
+    u_sm = u0 + np.roll(g, (ba, bb), axis=(0, 1)) * u0 / (1.0 - g[0, 0])
+    k = one.copy(); u = np.zeros((L, L))
+    out = orc.pcg_fracture(s, k, one, u, t, 1.0, 2, 1e-13, 500)
+    assert out["steps"] == 2 and out["index"][0] == b and out["iters"][0] == 1
+    cand = (one * u_sm / t).ravel().copy(); cand[b] = -np.inf
+    assert out["index"][1] == int(np.argmax(cand))
+    assert np.count_nonzero(k == 0) == 2 and k.ravel()[b] == 0.0
+
+
+@pytest.mark.parametrize("L,steps", [(16, 60), (32, 120)])
+def test_pcg_fracture_same_break_sequence_as_cg_loop(L, steps):
+    """The break sequence belongs to the exact solutions: the PCG loop must reproduce the (independently pinned) CG loop's
+    indices wherever the top-2 gap is far above the solver error, with fewer iterations in total."""
+    w = inputs.config(3, L=L, nsteps=steps)
+    k1 = w.k.copy(); u1 = w.u0.copy()
+    a = orc.fracture(w.s, k1, w.f, u1, w.t, steps, 1e-12, 2000)
+    k2 = w.k.copy(); u2 = w.u0.copy()
+    b = orc.pcg_fracture(w.s, k2, w.f, u2, w.t, 1.0, steps, 1e-12, 2000)
+    assert a["steps"] == steps and b["steps"] == steps
+    assert a["gap"].min() > 1e-9
+    assert np.array_equal(a["index"], b["index"]) and np.array_equal(k1, k2)
+    assert rel(u2, u1) < 1e-10
+    assert b["iters"].sum() < a["iters"].sum()
