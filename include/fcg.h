@@ -122,7 +122,8 @@ int fcg_solve(fcg_handle h, const void* k, const void* f, void* u, double tol, i
  *   fcg_pcg_solve            arguments, stopping rule (||r||_2 <= tol ||f||_2, recurrence residual, first crossing),
  *                            iteration count, scalars in double and determinism as fcg_solve.  FCG_BREAKDOWN also when
  *                            r.z <= 0 or not finite (u then holds the iterate of the completed update).
- * The loop is one CUDA graph with a device-side WHILE node at every size (6 launches per iteration). */
+ * The loop is one CUDA graph with a device-side WHILE node (6 launches per iteration); for L = 256, 512 the whole solve
+ * is the one cooperative kernel of FCG_OPT_FUSED, as for fcg_solve. */
 int fcg_set_preconditioner(fcg_handle h, const void* s, double kbar);
 int fcg_pcg_solve(fcg_handle h, const void* k, const void* f, void* u, double tol, int maxit,
                   int* iters_host, double* rel_residual_host);
@@ -154,6 +155,21 @@ int fcg_break_step(fcg_handle h, void* k, const void* u, const void* t,
  * status) on a negative status; steps_done_host receives the number of completed steps. */
 int fcg_fracture(fcg_handle h, void* k, const void* f, void* u, const void* t, int nsteps, double tol,
                  int maxit, long long* index_host, int* iters_host, int* steps_done_host);
+
+/* The same loop with every solve done by fcg_pcg_solve (the preconditioner's kbar stays what fcg_set_preconditioner
+ * was given for all steps).  One cooperative launch for L = 256, 512 like fcg_fracture. */
+int fcg_pcg_fracture(fcg_handle h, void* k, const void* f, void* u, const void* t, int nsteps, double tol,
+                     int maxit, long long* index_host, int* iters_host, int* steps_done_host);
+
+/* Ensembles of independent samples ("good statistics"): the quasi-static loop in two
+ * halves, so that ONE host thread can keep several handles busy, each created on its own stream.  For L = 256, 512 (one
+ * cooperative kernel of L/2 CTAs per loop) _begin returns as soon as the launch is enqueued and up to three such kernels are
+ * resident on a B200 at once; at other sizes _begin runs the loop to its end.  _end blocks and fills the host arrays like
+ * fcg_fracture.  k, f, u, t must stay valid and untouched between the two calls; one loop pending per handle.
+ *   use_pcg  0: fcg_solve per step, 1: fcg_pcg_solve (fcg_set_preconditioner first). */
+int fcg_fracture_begin(fcg_handle h, void* k, const void* f, void* u, const void* t, int nsteps, double tol,
+                       int maxit, int use_pcg);
+int fcg_fracture_end(fcg_handle h, long long* index_host, int* iters_host, int* steps_done_host);
 
 /* Measurement aid: runs the set-up of fcg_solve and then `iters` iterations of the CG loop body as direct
  * launches with CUDA events between the four kernels (tol = 0: never stops early), and returns their mean

@@ -23,7 +23,8 @@ FCG_OPT_L2_HINTS = 7
 EXPORTS = ["fcg_workspace_bytes", "fcg_create", "fcg_destroy", "fcg_set_option", "fcg_set_spectrum", "fcg_apply",
            "fcg_solve", "fcg_solve_host", "fcg_profile_iteration", "fcg_fft_fwd", "fcg_fft_inv", "fcg_break_step", "fcg_fracture",
            "fcg_last_launch_count", "fcg_last_error", "fcg_version",
-           "fcg_set_preconditioner", "fcg_pcg_solve", "fcg_profile_pcg_iteration"]
+           "fcg_set_preconditioner", "fcg_pcg_solve", "fcg_profile_pcg_iteration", "fcg_pcg_fracture",
+           "fcg_fracture_begin", "fcg_fracture_end"]
 
 _lib = None
 
@@ -54,6 +55,9 @@ def lib() -> C.CDLL:
         L.fcg_fft_inv.argtypes = [vp, vp, vp]; L.fcg_fft_inv.restype = i
         L.fcg_break_step.argtypes = [vp, vp, vp, vp, C.POINTER(ll), C.POINTER(d)]; L.fcg_break_step.restype = i
         L.fcg_fracture.argtypes = [vp, vp, vp, vp, vp, i, d, i, vp, vp, C.POINTER(i)]; L.fcg_fracture.restype = i
+        L.fcg_pcg_fracture.argtypes = [vp, vp, vp, vp, vp, i, d, i, vp, vp, C.POINTER(i)]; L.fcg_pcg_fracture.restype = i
+        L.fcg_fracture_begin.argtypes = [vp, vp, vp, vp, vp, i, d, i, i]; L.fcg_fracture_begin.restype = i
+        L.fcg_fracture_end.argtypes = [vp, vp, vp, C.POINTER(i)]; L.fcg_fracture_end.restype = i
         L.fcg_profile_iteration.argtypes = [vp, vp, vp, vp, i, C.POINTER(d)]; L.fcg_profile_iteration.restype = i
         L.fcg_set_preconditioner.argtypes = [vp, vp, d]; L.fcg_set_preconditioner.restype = i
         L.fcg_pcg_solve.argtypes = [vp, vp, vp, vp, d, i, C.POINTER(i), C.POINTER(d)]; L.fcg_pcg_solve.restype = i
@@ -198,12 +202,35 @@ class Fcg:
             self._raise(st)
         return int(idx.value), float(ratio.value), int(st)
 
+    def fcg_fracture_begin(self, k, f, u, t, nsteps: int, tol: float, maxit: int, use_pcg: bool = False):
+        """Enqueue a quasi-static loop (returns at once where the loop is one cooperative kernel); finish with fcg_fracture_end."""
+        self._pending = (k, f, u, t, int(nsteps))              # keep the tensors alive
+        st = self._lib.fcg_fracture_begin(self._h, self._chk(k, self.N), self._chk(f, self.N), self._chk(u, self.N),
+                                          self._chk(t, self.N), int(nsteps), float(tol), int(maxit), 1 if use_pcg else 0)
+        if st < 0 and st not in (FCG_BREAKDOWN, FCG_NO_CANDIDATE):
+            self._raise(st)
+
+    def fcg_fracture_end(self):
+        """Returns (index, iters, steps_done, status) of the loop started by fcg_fracture_begin."""
+        import numpy as np
+        nsteps = self._pending[4]
+        index = np.full(nsteps, -1, np.int64); iters = np.zeros(nsteps, np.int32); done = C.c_int(0)
+        st = self._lib.fcg_fracture_end(self._h, index.ctypes.data_as(C.c_void_p), iters.ctypes.data_as(C.c_void_p), C.byref(done))
+        self._pending = None
+        if st < 0 and st not in (FCG_BREAKDOWN, FCG_NO_CANDIDATE):
+            self._raise(st)
+        return index, iters, int(done.value), int(st)
+
+    def fcg_pcg_fracture(self, k, f, u, t, nsteps: int, tol: float, maxit: int):
+        """fcg_fracture with preconditioned-CG solves (fcg_set_preconditioner first)."""
+        return self.fcg_fracture(k, f, u, t, nsteps, tol, maxit, _fn="fcg_pcg_fracture")
+
     def fcg_fracture(self, k: torch.Tensor, f: torch.Tensor, u: torch.Tensor, t: torch.Tensor, nsteps: int,
-                     tol: float, maxit: int):
+                     tol: float, maxit: int, _fn: str = "fcg_fracture"):
         """In place on k and u. Returns (index[int64 numpy], iters[int32 numpy], steps_done, status)."""
         import numpy as np
         index = np.full(nsteps, -1, np.int64); iters = np.zeros(nsteps, np.int32); done = C.c_int(0)
-        st = self._lib.fcg_fracture(self._h, self._chk(k, self.N), self._chk(f, self.N), self._chk(u, self.N),
+        st = getattr(self._lib, _fn)(self._h, self._chk(k, self.N), self._chk(f, self.N), self._chk(u, self.N),
                                     self._chk(t, self.N), int(nsteps), float(tol), int(maxit),
                                     index.ctypes.data_as(C.c_void_p), iters.ctypes.data_as(C.c_void_p), C.byref(done))
         if st < 0 and st not in (FCG_BREAKDOWN, FCG_NO_CANDIDATE):

@@ -88,6 +88,8 @@ struct fcg_handle_s {
     BreakResult* h_brk = nullptr;       // pinned
     void *hk = nullptr, *hf = nullptr, *hu = nullptr;   // device staging of fcg_solve_host
     long long* frac_idx = nullptr; int* frac_it = nullptr; int frac_cap = 0;   // device results of the fused quasi-static loop
+    int pend_nsteps = -1, pend_done = 0, pend_status = 0; bool pend_async = false;   // fcg_fracture_begin / _end
+    std::vector<long long> pend_idx; std::vector<int> pend_it;
     std::vector<GraphEntry> graphs; unsigned long long stamp = 0;
     long long launches = 0;
     std::string err;
@@ -285,9 +287,10 @@ cudaError_t build_graph(fcg_handle h, GraphEntry& ge) {
 template <typename T>
 int solve_impl(fcg_handle h, const void* k, const void* f, void* u, double tol, int maxit, int* iters, double* relres, bool pcg = false) {
     h->launches = 0;
-    if (h->fused() && !pcg) {
+    if (h->fused()) {
         // small lattices: the whole solve is one cooperative kernel with the vectors resident in shared memory (fcg_fused.cuh)
         FusedArgs A{};
+        A.mhat = pcg ? h->ws + h->lay.mhat : nullptr;
         A.k = k; A.f = f; A.u = u; A.Tf = h->ws + h->lay.Tb; A.shat = h->ws + h->lay.shat; A.tw = h->ws + h->lay.tw;
         A.partial = h->at<double>(h->lay.partial_row); A.counter = &h->sc()->ticket[3]; A.sc = h->sc(); A.tol = tol; A.maxit = maxit;
         FCG_CK(h, cudaMemsetAsync(h->sc(), 0, sizeof(Scalars), h->stream));
@@ -705,9 +708,12 @@ int fcg_break_step(fcg_handle h, void* k, const void* u, const void* t, long lon
                                : break_impl<float>(h, k, u, t, index_host, ratio_host);
 }
 
-int fcg_fracture(fcg_handle h, void* k, const void* f, void* u, const void* t, int nsteps, double tol, int maxit,
-                 long long* index_host, int* iters_host, int* steps_done_host) {
-    if (!h || !k || !f || !u || !t || nsteps < 0 || !index_host || !iters_host) return fail(h, FCG_INVALID_ARG, "bad argument");
+// Quasi-static loop in two halves, so that one host thread can keep several handles (streams) busy: begin enqueues (and, where the
+// loop is one cooperative kernel, returns at once); end blocks and hands out the results.
+static int fracture_begin(fcg_handle h, void* k, const void* f, void* u, const void* t, int nsteps, double tol, int maxit, bool pcg) {
+    if (!h || !k || !f || !u || !t || nsteps < 0) return fail(h, FCG_INVALID_ARG, "bad argument");
+    if (pcg && !h->have_precond) return fail(h, FCG_NO_SPECTRUM, "fcg_set_preconditioner has not been called");
+    h->pend_nsteps = -1; h->pend_async = false; h->pend_done = 0; h->pend_status = FCG_OK;
     if (h->fused() && h->have_spectrum && nsteps > 0 && tol >= 0.0 && maxit >= 0) {
         // small lattices: the whole quasi-static loop -- every solve and every break step -- is one cooperative kernel
         if (h->frac_cap < nsteps) {
@@ -721,42 +727,83 @@ int fcg_fracture(fcg_handle h, void* k, const void* f, void* u, const void* t, i
         FusedArgs A{};
         A.k = k; A.f = f; A.u = u; A.Tf = h->ws + h->lay.Tb; A.shat = h->ws + h->lay.shat; A.tw = h->ws + h->lay.tw;
         A.partial = h->at<double>(h->lay.partial_row); A.counter = &h->sc()->ticket[3]; A.sc = h->sc(); A.tol = tol; A.maxit = maxit;
+        A.mhat = pcg ? h->ws + h->lay.mhat : nullptr;
         A.nsteps = nsteps; A.t = t; A.k_out = k; A.out_index = h->frac_idx; A.out_iters = h->frac_it;
         A.brk_r = h->at<double>(h->lay.brk_r); A.brk_i = h->at<long long>(h->lay.brk_i);
         FCG_CK(h, cudaMemsetAsync(h->sc(), 0, sizeof(Scalars), h->stream));
         cudaError_t e = h->tab->fused_solve(&A, h->stream);
         if (e == cudaSuccess) {
             FCG_CK(h, cudaMemcpyAsync(h->h_sc, h->sc(), sizeof(Scalars), cudaMemcpyDeviceToHost, h->stream));
-            FCG_CK(h, cudaStreamSynchronize(h->stream));
-            const int done = h->h_sc->steps_done;
-            if (done > 0) {
-                FCG_CK(h, cudaMemcpy(index_host, h->frac_idx, (size_t)done * sizeof(long long), cudaMemcpyDeviceToHost));
-                FCG_CK(h, cudaMemcpy(iters_host, h->frac_it, (size_t)done * sizeof(int), cudaMemcpyDeviceToHost));
-            }
-            if (steps_done_host) *steps_done_host = done;
-            h->launches = 1;
-            if (h->h_sc->status == FCG_CUDA_ERROR) h->err = "fused quasi-static loop: grid barrier timed out";
-            return h->h_sc->status < 0 ? h->h_sc->status : FCG_OK;
+            h->pend_nsteps = nsteps; h->pend_async = true; h->launches = 1;
+            return FCG_OK;
         }
         cudaGetLastError();
         h->err = std::string("cooperative launch failed (") + cudaGetErrorString(e) + "); using the graph path";
         h->fused_opt = 0;
     }
+    h->pend_idx.assign((size_t)nsteps, -1); h->pend_it.assign((size_t)nsteps, 0);
     long long total = 0; int done = 0, st = FCG_OK;
     for (int step = 0; step < nsteps; ++step) {
         int it = 0; double rr = 0.0;
-        st = fcg_solve(h, k, f, u, tol, maxit, &it, &rr);
+        st = pcg ? fcg_pcg_solve(h, k, f, u, tol, maxit, &it, &rr) : fcg_solve(h, k, f, u, tol, maxit, &it, &rr);
         total += h->launches;
         if (st < 0) break;
         long long idx = -1; double ratio = 0.0;
         st = fcg_break_step(h, k, u, t, &idx, &ratio);
         total += h->launches;
         if (st < 0) break;
-        index_host[step] = idx; iters_host[step] = it; ++done; st = FCG_OK;
+        h->pend_idx[step] = idx; h->pend_it[step] = it; ++done; st = FCG_OK;
     }
-    if (steps_done_host) *steps_done_host = done;
-    h->launches = total;
-    return st;
+    h->pend_nsteps = nsteps; h->pend_done = done; h->pend_status = st; h->launches = total;
+    return st < 0 ? st : FCG_OK;
+}
+
+static int fracture_end(fcg_handle h, long long* index_host, int* iters_host, int* steps_done_host) {
+    if (!h || !index_host || !iters_host) return fail(h, FCG_INVALID_ARG, "bad argument");
+    if (h->pend_nsteps < 0) return fail(h, FCG_INVALID_ARG, "no quasi-static loop pending on this handle");
+    h->pend_nsteps = -1;
+    if (h->pend_async) {
+        FCG_CK(h, cudaStreamSynchronize(h->stream));
+        const int done = h->h_sc->steps_done;
+        if (done > 0) {
+            FCG_CK(h, cudaMemcpyAsync(index_host, h->frac_idx, (size_t)done * sizeof(long long), cudaMemcpyDeviceToHost, h->stream));
+            FCG_CK(h, cudaMemcpyAsync(iters_host, h->frac_it, (size_t)done * sizeof(int), cudaMemcpyDeviceToHost, h->stream));
+            FCG_CK(h, cudaStreamSynchronize(h->stream));
+        }
+        if (steps_done_host) *steps_done_host = done;
+        if (h->h_sc->status == FCG_CUDA_ERROR) h->err = "fused quasi-static loop: grid barrier timed out";
+        return h->h_sc->status < 0 ? h->h_sc->status : FCG_OK;
+    }
+    for (int i = 0; i < h->pend_done; ++i) { index_host[i] = h->pend_idx[(size_t)i]; iters_host[i] = h->pend_it[(size_t)i]; }
+    if (steps_done_host) *steps_done_host = h->pend_done;
+    return h->pend_status;
+}
+
+static int fracture_impl(fcg_handle h, void* k, const void* f, void* u, const void* t, int nsteps, double tol, int maxit,
+                         long long* index_host, int* iters_host, int* steps_done_host, bool pcg) {
+    if (!index_host || !iters_host) return fail(h, FCG_INVALID_ARG, "bad argument");
+    int st = fracture_begin(h, k, f, u, t, nsteps, tol, maxit, pcg);
+    if (st < 0 && (!h || h->pend_nsteps < 0)) return st;
+    return fracture_end(h, index_host, iters_host, steps_done_host);
+}
+
+int fcg_fracture_begin(fcg_handle h, void* k, const void* f, void* u, const void* t, int nsteps, double tol, int maxit, int use_pcg) {
+    return fracture_begin(h, k, f, u, t, nsteps, tol, maxit, use_pcg != 0);
+}
+
+int fcg_fracture_end(fcg_handle h, long long* index_host, int* iters_host, int* steps_done_host) {
+    return fracture_end(h, index_host, iters_host, steps_done_host);
+}
+
+int fcg_fracture(fcg_handle h, void* k, const void* f, void* u, const void* t, int nsteps, double tol, int maxit,
+                 long long* index_host, int* iters_host, int* steps_done_host) {
+    return fracture_impl(h, k, f, u, t, nsteps, tol, maxit, index_host, iters_host, steps_done_host, false);
+}
+
+int fcg_pcg_fracture(fcg_handle h, void* k, const void* f, void* u, const void* t, int nsteps, double tol, int maxit,
+                     long long* index_host, int* iters_host, int* steps_done_host) {
+    if (h && !h->have_precond) return fail(h, FCG_NO_SPECTRUM, "fcg_set_preconditioner has not been called");
+    return fracture_impl(h, k, f, u, t, nsteps, tol, maxit, index_host, iters_host, steps_done_host, true);
 }
 
 int fcg_profile_iteration(fcg_handle h, const void* k, const void* f, void* u, int iters, double* ms_host) {

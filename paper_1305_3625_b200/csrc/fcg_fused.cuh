@@ -6,6 +6,8 @@
 //     c, c+G, .. of T for the whole solve;
 //   * its rows of k, f, u, r, p, q live in shared memory from the first iteration to the last; only T (the transposition
 //     between the row and the column transforms) goes through global memory, i.e. through L2;
+//   * preconditioned CG (A.mhat != nullptr): z = M^-1 r is one more operator-shaped round trip per iteration (rows of r ->
+//     columns with the preconditioner's spectrum -> rows of z, r.z), three more grid barriers; z lives in q's slot;
 //   * per iteration four grid barriers (an atomic counter in global memory): T complete -> columns done -> p.q known ->
 //     r.r known.  Every CTA adds the G partial sums itself, in the same fixed order, so alpha, beta and the convergence
 //     decision are bit-identical in all CTAs and no CTA ever waits for a broadcast;
@@ -29,6 +31,7 @@ struct FusedArgs {
     double tol; int maxit;
     // quasi-static loop (nsteps > 0): thresholds, k written back, per-step results, arg-max scratch (G entries each)
     int nsteps; const void* t; void* k_out; long long* out_index; int* out_iters; double* brk_r; long long* brk_i;
+    const void* mhat;                           // preconditioned CG: stored spectrum of M^-1, or nullptr for plain CG
 };
 
 template <typename T, typename P> struct FusedShape {
@@ -178,7 +181,7 @@ __global__ void __launch_bounds__(P::NT) cg_fused_kernel(const FusedArgs A)
         }
     };
     // phase C: own columns, in place: forward, spectral multiply, inverse
-    auto columns = [&]() {
+    auto columns = [&](const T* spec) {
         for (int j = 0; j < TPC; ++j) {
             const int m = cta + j * G;
             cx<T>* col = Tf + (size_t)m * L;
@@ -209,15 +212,15 @@ __global__ void __launch_bounds__(P::NT) cg_fused_kernel(const FusedArgs A)
                 __syncthreads();
             };
             if (m != 0) {
-                const T* sh = shat + (size_t)m * L;
+                const T* sh = spec + (size_t)m * L;
                 static_for_up<2, S - 1>(fwd_stage);
                 run_middle<P, T>(lt, ld_sw, st_sw, [&](int g, int u) { return sh[u * (L / P::RLAST) + g]; });
                 __syncthreads();
                 static_for_down<S - 1, 2>(inv_stage);
             } else {     // packed n = 0 / L/2 column (see col2_kernel)
                 static_for_up<2, S>(fwd_stage);
-                const T* sp_ = shat;
-                const T* sm_ = shat + (size_t)(L / 2) * L;
+                const T* sp_ = spec;
+                const T* sm_ = spec + (size_t)(L / 2) * L;
                 for (int mm = lt; mm <= L / 2; mm += NT) {
                     const int e = P::pos_of(mm), e2 = P::pos_of((L - mm) % L);
                     const cx<T> Wa = io.ld(e), Wb = io.ld(e2);
@@ -290,83 +293,104 @@ __global__ void __launch_bounds__(P::NT) cg_fused_kernel(const FusedArgs A)
         }
     }
     __syncthreads();
-    bool ok = true, okb = true;
+    // One solve is a small state machine, so that every phase of the operator-shaped round trip (rows -> columns -> rows) and the
+    // grid-wide sum exist ONCE in the instruction stream (with several call sites the compiler stops inlining them: 64 registers,
+    // a stack frame, and 17.7 instead of 12.4 us per iteration at L = 256):
+    //   FN (once per launch: ||f||^2) -> RESID (r = f - A u, r.r) -> [Z (z = M^-1 r, r.z)] -> Q (p, q = A p, p.q) -> RR (u, r, r.r)
+    //   -> [Z] -> Q -> RR -> ..          Z only for preconditioned CG; z lives in q's slot (q is dead once r has been updated).
+    enum { PH_FN = 0, PH_RESID = 1, PH_Z = 2, PH_Q = 3, PH_RR = 4 };
+    bool ok = true, okb = true, have_fn = false;
     int it = 0, status = ST_OK, steps_done = 0;
-    double rho = 0.0, fn2 = 0.0;
+    double rho = 0.0, fn2 = 0.0, rr = 0.0;         // rho = r.r (CG) or r.z (PCG); rr = r.r
     bool zero_u = false;
+    const T* mhat = static_cast<const T*>(A.mhat);
+    const bool pcg = mhat != nullptr;
 
     for (int step = 0; step < (frac ? A.nsteps : 1); ++step) {
-        // ---- set up initial values: r = f - A u, rho = r.r, ||f||^2; first direction from p = 0, beta = 0
+        // ---- set up initial values: first direction from p = 0, beta = 0
         for (int j = 0; j < TPC; ++j) {
             T* pp = V(j, 4, 0);
             for (int e = lt; e < 2 * L; e += NT) pp[e] = (T)0;
         }
-        double acc_r = 0.0, acc_f = 0.0;
-        rows_forward(2);
-        ok = grid_barrier(A.counter, target, G, &ok_smem) && ok;
-        columns();
-        ok = grid_barrier(A.counter, target, G, &ok_smem) && ok;
-        rows_inverse([&](int j, int e, T c0, T c1) {
-            const T* kk = V(j, 0, 0); const T* ff = V(j, 1, 0); const T* uu = V(j, 2, 0); T* rr = V(j, 3, 0);
-            const T f0 = ff[e], f1 = ff[L + e];
-            const T r0 = f0 - (kk[e] * uu[e] + c0), r1 = f1 - (kk[L + e] * uu[L + e] + c1);
-            rr[e] = r0; rr[L + e] = r1;
-            acc_r += (double)r0 * (double)r0; acc_r += (double)r1 * (double)r1;
-            acc_f += (double)f0 * (double)f0; acc_f += (double)f1 * (double)f1;
-        });
-        rho = grid_sum(acc_r, okb); ok = ok && okb;
-        fn2 = grid_sum(acc_f, okb); ok = ok && okb;
         it = 0; status = ST_OK; zero_u = false;
-        bool done = false;
-        double beta = 0.0;
-        if (!ok) { done = true; status = -3; }
-        else if (fn2 == 0.0) { done = true; zero_u = true; rho = 0.0; }
-        else if (sqrt(rho) <= A.tol * sqrt(fn2)) done = true;
-        else if (A.maxit <= 0) { done = true; status = ST_NOT_CONVERGED; }
-
-        // ---- Listing 2
-        while (!done) {
-            for (int j = 0; j < TPC; ++j) {                                   // update calculation variables: new direction (98)
-                const T* rr = V(j, 3, 0); T* pp = V(j, 4, 0);
-                const T b = (T)beta;
-                for (int e = lt; e < 2 * L; e += NT) pp[e] = rr[e] + b * pp[e];
-            }
-            __syncthreads();
-            rows_forward(4);                                                  // A * p (93)
-            ok = grid_barrier(A.counter, target, G, &ok_smem) && ok;
-            columns();
-            ok = grid_barrier(A.counter, target, G, &ok_smem) && ok;
+        double beta = 0.0, alpha = 0.0;
+        int phase = have_fn ? PH_RESID : PH_FN;
+        while (true) {
             double acc = 0.0;
-            rows_inverse([&](int j, int e, T c0, T c1) {
-                const T* kk = V(j, 0, 0); const T* pp = V(j, 4, 0); T* qq = V(j, 5, 0);
-                const T p0 = pp[e], p1 = pp[L + e];
-                const T q0 = kk[e] * p0 + c0, q1 = kk[L + e] * p1 + c1;       // k o p + C p
-                qq[e] = q0; qq[L + e] = q1;
-                acc += (double)p0 * (double)q0; acc += (double)p1 * (double)q1;
-            });
-            const double pq = grid_sum(acc, okb); ok = ok && okb;             // search length (94)
-            if (!ok) { status = -3; break; }
-            if (!(pq > 0.0) || !isfinite(pq)) { status = ST_BREAKDOWN; break; }
-            const double alpha = rho / pq;
-            const T al = (T)alpha;
-            double accr = 0.0;
-            __syncthreads();
-            for (int j = 0; j < TPC; ++j) {                                   // new x (95), residue (96), residue length (97)
-                T* uu = V(j, 2, 0); T* rr = V(j, 3, 0); const T* pp = V(j, 4, 0); const T* qq = V(j, 5, 0);
-                for (int e = lt; e < 2 * L; e += NT) {
-                    uu[e] = uu[e] + al * pp[e];
-                    const T rn = rr[e] - al * qq[e];
-                    rr[e] = rn;
-                    accr += (double)rn * (double)rn;
+            // ---- vector work of this phase on the CTA's own rows
+            if (phase == PH_FN) {
+                for (int j = 0; j < TPC; ++j) {
+                    const T* ff = V(j, 1, 0);
+                    for (int e = lt; e < 2 * L; e += NT) acc += (double)ff[e] * (double)ff[e];
+                }
+            } else if (phase == PH_Q) {                                       // update calculation variables: new direction (98)
+                for (int j = 0; j < TPC; ++j) {
+                    const T* dv = V(j, pcg ? 5 : 3, 0); T* pp = V(j, 4, 0);      // r, or z = M^-1 r
+                    const T b = (T)beta;
+                    for (int e = lt; e < 2 * L; e += NT) pp[e] = dv[e] + b * pp[e];
+                }
+                __syncthreads();
+            } else if (phase == PH_RR) {                                      // new x (95), residue (96), residue length (97)
+                const T al = (T)alpha;
+                for (int j = 0; j < TPC; ++j) {
+                    T* uu = V(j, 2, 0); T* rv = V(j, 3, 0); const T* pp = V(j, 4, 0); const T* qq = V(j, 5, 0);
+                    for (int e = lt; e < 2 * L; e += NT) {
+                        uu[e] = uu[e] + al * pp[e];
+                        const T rn = rv[e] - al * qq[e];
+                        rv[e] = rn;
+                        acc += (double)rn * (double)rn;
+                    }
                 }
             }
-            const double rho_new = grid_sum(accr, okb); ok = ok && okb;
+            // ---- operator-shaped round trip: C u (RESID), C p (Q: A * p) or M^-1 r (Z)
+            if (phase == PH_RESID || phase == PH_Z || phase == PH_Q) {
+                rows_forward(phase == PH_RESID ? 2 : (phase == PH_Q ? 4 : 3));
+                ok = grid_barrier(A.counter, target, G, &ok_smem) && ok;
+                columns(phase == PH_Z ? mhat : shat);
+                ok = grid_barrier(A.counter, target, G, &ok_smem) && ok;
+                rows_inverse([&](int j, int e, T c0, T c1) {
+                    if (phase == PH_RESID) {                                  // r = f - (k o u + C u)
+                        const T* kk = V(j, 0, 0); const T* ff = V(j, 1, 0); const T* uu = V(j, 2, 0); T* rv = V(j, 3, 0);
+                        const T r0 = ff[e] - (kk[e] * uu[e] + c0), r1 = ff[L + e] - (kk[L + e] * uu[L + e] + c1);
+                        rv[e] = r0; rv[L + e] = r1;
+                        acc += (double)r0 * (double)r0; acc += (double)r1 * (double)r1;
+                    } else if (phase == PH_Q) {                               // q = k o p + C p, p.q
+                        const T* kk = V(j, 0, 0); const T* pp = V(j, 4, 0); T* qq = V(j, 5, 0);
+                        const T p0 = pp[e], p1 = pp[L + e];
+                        const T q0 = kk[e] * p0 + c0, q1 = kk[L + e] * p1 + c1;
+                        qq[e] = q0; qq[L + e] = q1;
+                        acc += (double)p0 * (double)q0; acc += (double)p1 * (double)q1;
+                    } else {                                                  // z = M^-1 r (into q's slot), r.z
+                        const T* rv = V(j, 3, 0); T* zz = V(j, 5, 0);
+                        zz[e] = c0; zz[L + e] = c1;
+                        acc += (double)rv[e] * (double)c0; acc += (double)rv[L + e] * (double)c1;
+                    }
+                });
+            }
+            const double s0 = grid_sum(acc, okb); ok = ok && okb;
             if (!ok) { status = -3; break; }
-            ++it;
-            if (sqrt(rho_new) <= A.tol * sqrt(fn2)) { rho = rho_new; break; }                 // check convergence (99)
-            if (it >= A.maxit) { rho = rho_new; status = ST_NOT_CONVERGED; break; }
-            beta = rho_new / rho;
-            rho = rho_new;
+            // ---- scalar step, identical in every CTA
+            if (phase == PH_FN) { fn2 = s0; have_fn = true; phase = PH_RESID; }
+            else if (phase == PH_RESID) {
+                rr = s0; rho = rr;
+                if (fn2 == 0.0) { zero_u = true; rho = 0.0; rr = 0.0; break; }
+                if (sqrt(rr) <= A.tol * sqrt(fn2)) break;
+                if (A.maxit <= 0) { status = ST_NOT_CONVERGED; break; }
+                phase = pcg ? PH_Z : PH_Q;
+            } else if (phase == PH_Z) {
+                if (!(s0 > 0.0) || !isfinite(s0)) { status = ST_BREAKDOWN; break; }
+                beta = it == 0 ? 0.0 : s0 / rho;
+                rho = s0; phase = PH_Q;
+            } else if (phase == PH_Q) {                                       // search length (94)
+                if (!(s0 > 0.0) || !isfinite(s0)) { status = ST_BREAKDOWN; break; }
+                alpha = rho / s0; phase = PH_RR;
+            } else {
+                rr = s0; ++it;
+                if (sqrt(rr) <= A.tol * sqrt(fn2)) { if (!pcg) rho = rr; break; }                 // check convergence (99)
+                if (it >= A.maxit) { if (!pcg) rho = rr; status = ST_NOT_CONVERGED; break; }
+                if (pcg) phase = PH_Z;
+                else { beta = rr / rho; rho = rr; phase = PH_Q; }
+            }
         }
         __syncthreads();
         if (zero_u)
@@ -424,8 +448,8 @@ __global__ void __launch_bounds__(P::NT) cg_fused_kernel(const FusedArgs A)
     }
     if (cta == 0 && lt == 0) {
         Scalars* sc = A.sc;
-        sc->it = it; sc->status = status; sc->done = 1; sc->rho = rho; sc->fn2 = fn2; sc->steps_done = steps_done;
-        sc->relres = fn2 > 0.0 ? sqrt(rho) / sqrt(fn2) : 0.0;
+        sc->it = it; sc->status = status; sc->done = 1; sc->rho = rho; sc->rr = rr; sc->fn2 = fn2; sc->steps_done = steps_done;
+        sc->relres = fn2 > 0.0 ? sqrt(rr) / sqrt(fn2) : 0.0;
     }
 }
 

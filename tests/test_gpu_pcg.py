@@ -1,6 +1,8 @@
 """Parity of the preconditioned CG path (fcg_set_preconditioner / fcg_pcg_solve) with the
 oracle's oracle_pcg on the same seeded inputs, through the C ABI.  Same protocol and tolerances as test_gpu_parity.py:
 status equal, iteration count within +-2, u within 1e-9 (fp64) / 1e-4 (fp32) at equal iteration count."""
+import os
+
 import numpy as np
 import pytest
 import torch
@@ -70,7 +72,7 @@ def test_pcg_classic_engine_and_loop_modes(B, L, dt):
     pcg_parity(B, w, FCG_OPT_ENGINE=1)
     kbar = inputs.precond_kbar(w.k)
     outs = []
-    for opts in (dict(), dict(FCG_OPT_LOOP_MODE=1, FCG_OPT_CHUNK=3), dict(FCG_OPT_UNROLL=1)):
+    for opts in (dict(FCG_OPT_FUSED=0), dict(FCG_OPT_FUSED=0, FCG_OPT_LOOP_MODE=1, FCG_OPT_CHUNK=3), dict(FCG_OPT_FUSED=0, FCG_OPT_UNROLL=1)):
         h = pcg_handle(B, w, kbar, **opts)
         u = dev(w.u0)
         r = h.fcg_pcg_solve(dev(w.k), dev(w.f), u, w.tol, w.maxit)
@@ -158,3 +160,95 @@ def test_pcg_config2_full_size(B, dt, tolpin):
     assert h.fcg_pcg_solve(kd, fd, u2, w.tol, w.maxit) == (it, rr, st) and torch.equal(u, u2)
     assert h.fcg_last_launch_count() == 8 + 6 * 4 * ((it + 3) // 4)
     h.close()
+
+
+@pytest.mark.parametrize("cfg,L", [(1, 256), (1, 512), (2, 512), (4, 256)])
+def test_pcg_fused_kernel_and_graph_path(B, cfg, L):
+    """L = 256, 512: the whole PCG solve is ONE cooperative launch (z in q's shared-memory slot); the graph path
+    (FCG_OPT_FUSED = 0) of the same sizes is checked against the oracle too."""
+    w = inputs.config(cfg, np.float64, L=L)
+    pcg_parity(B, w)
+    pcg_parity(B, w, FCG_OPT_FUSED=0)
+    h = pcg_handle(B, w, inputs.precond_kbar(w.k))
+    u = dev(w.u0)
+    r1 = h.fcg_pcg_solve(dev(w.k), dev(w.f), u, w.tol, w.maxit)
+    assert h.fcg_last_launch_count() == 1
+    u2 = dev(w.u0)
+    assert h.fcg_pcg_solve(dev(w.k), dev(w.f), u2, w.tol, w.maxit) == r1 and torch.equal(u, u2)      # bitwise repeatable
+    h.close()
+
+
+@pytest.mark.parametrize("L,steps", [(32, 200), (64, 150), (256, 60)])
+def test_pcg_fracture_matches_oracle(B, L, steps):
+    """Quasi-static loop with PCG solves vs oracle_pcg_fracture: break indices bit-exact, iteration counts within +-2,
+    final k identical, final u within tolerance (graph path for L < 256, the one-launch kernel at L = 256)."""
+    w = inputs.config(3, L=L, nsteps=steps)
+    ko = w.k.copy(); uo = w.u0.copy()
+    ref = orc.pcg_fracture(w.s, ko, w.f, uo, w.t, 1.0, steps, w.tol, w.maxit)
+    assert ref["steps"] == steps
+    h = pcg_handle(B, w, 1.0)
+    k, u = dev(w.k), dev(w.u0)
+    index, iters, done, st = h.fcg_pcg_fracture(k, dev(w.f), u, dev(w.t), steps, w.tol, w.maxit)
+    assert st == 0 and done == steps
+    assert np.array_equal(index, ref["index"]), (np.flatnonzero(index != ref["index"])[:5], ref["gap"].min())
+    assert np.abs(iters.astype(int) - ref["iters"].astype(int)).max() <= 2
+    assert np.array_equal(k.cpu().numpy(), ko)
+    assert rel(u.cpu().numpy(), uo) <= 1e-8
+    if L == 256:
+        assert h.fcg_last_launch_count() == 1
+    h.close()
+
+
+def test_pcg_fracture_config3_full(B):
+    """BASELINE.json configs[3] with PCG solves, all 2000 steps in one launch, against tests/golden/cfg3_pcg_breaks.txt
+    (written from oracle/ only): indices bit-exact -- and identical to the CG loop's golden sequence -- counts +-2."""
+    rows = np.loadtxt(os.path.join(os.path.dirname(__file__), "golden", "cfg3_pcg_breaks.txt"), comments="#")
+    cg_rows = np.loadtxt(os.path.join(os.path.dirname(__file__), "golden", "cfg3_breaks.txt"), comments="#")
+    gidx, git = rows[:, 1].astype(np.int64), rows[:, 2].astype(np.int64)
+    w = inputs.config(3)
+    h = pcg_handle(B, w, 1.0)
+    k, u = dev(w.k), dev(w.u0)
+    index, iters, done, st = h.fcg_pcg_fracture(k, dev(w.f), u, dev(w.t), w.nsteps, w.tol, w.maxit)
+    assert st == 0 and done == w.nsteps and h.fcg_last_launch_count() == 1
+    assert np.array_equal(index, gidx)
+    assert np.array_equal(index, cg_rows[:, 1].astype(np.int64))
+    assert np.abs(iters.astype(np.int64) - git).max() <= 2
+    assert iters.sum() < 0.5 * cg_rows[:, 2].sum()
+    h.close()
+
+
+@pytest.mark.parametrize("L,use_pcg", [(256, True), (256, False), (64, True)])
+def test_fracture_ensemble_begin_end(B, L, use_pcg):
+    """Independent samples (different threshold seeds) on three handles / streams driven by one host thread with
+    fcg_fracture_begin / _end: every sample equals what the blocking call gives for it (bitwise), and sample 0 equals the oracle."""
+    steps, nrep = 40, 3
+    w = inputs.config(3, L=L, nsteps=steps)
+    ts = [w.t if r == 0 else inputs.thresholds(L, seed=100 + r) for r in range(nrep)]
+    reps = []
+    for r in range(nrep):
+        st = torch.cuda.Stream()
+        with torch.cuda.stream(st):
+            h = B.Fcg(L, torch.float64, stream=st)
+            s = dev(w.s); h.fcg_set_spectrum(s); h.fcg_set_preconditioner(s, 1.0)
+            reps.append((h, dev(w.k), dev(w.f), dev(w.u0), dev(ts[r]), st))
+    torch.cuda.synchronize()
+    for h, k, f, u, t, st in reps:
+        h.fcg_fracture_begin(k, f, u, t, steps, w.tol, w.maxit, use_pcg)
+    outs = [h.fcg_fracture_end() for h, *_ in reps]
+    for r, (h, k, f, u, t, st) in enumerate(reps):
+        index, iters, done, status = outs[r]
+        assert status == 0 and done == steps
+        k2, u2 = dev(w.k), dev(w.u0)
+        torch.cuda.synchronize()
+        with torch.cuda.stream(st):
+            fn = h.fcg_pcg_fracture if use_pcg else h.fcg_fracture
+            i2, it2, d2, s2 = fn(k2, dev(w.f), u2, dev(ts[r]), steps, w.tol, w.maxit)
+        assert np.array_equal(index, i2) and np.array_equal(iters, it2) and torch.equal(k, k2) and torch.equal(u, u2)
+    ko = w.k.copy(); uo = w.u0.copy()
+    ref = (orc.pcg_fracture(w.s, ko, w.f, uo, w.t, 1.0, steps, w.tol, w.maxit) if use_pcg
+           else orc.fracture(w.s, ko, w.f, uo, w.t, steps, w.tol, w.maxit))
+    assert np.array_equal(outs[0][0], ref["index"]) and np.abs(outs[0][1].astype(int) - ref["iters"].astype(int)).max() <= 2
+    with pytest.raises(B.FcgError):                          # nothing pending any more
+        reps[0][0]._pending = (None, None, None, None, 1); reps[0][0].fcg_fracture_end()
+    for h, *_ in reps:
+        h.close()
