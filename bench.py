@@ -111,7 +111,8 @@ def run_reference(args, rank: int):
     print(json.dumps(line))
 
 
-def bench_workload(binding, torch, w, steps, warmup, profile_iters=20, e2e_steps=None, loop_mode=0, pcg_steps=0, inputs_mod=None):
+def bench_workload(binding, torch, w, steps, warmup, profile_iters=20, e2e_steps=None, loop_mode=0, pcg_steps=0, inputs_mod=None,
+                   solver="cg"):
     """Times `steps` solves of workload w on the current device. Returns a dict of measurements."""
     tdt = torch.float64 if w.dtype == np.float64 else torch.float32
     wbytes = w.dtype.itemsize
@@ -120,9 +121,13 @@ def bench_workload(binding, torch, w, steps, warmup, profile_iters=20, e2e_steps
     to = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
     h.fcg_set_spectrum(to(w.s))
     k, f, u = to(w.k), to(w.f), to(w.u0)
+    solve = h.fcg_solve
+    if solver == "pcg":                                    # --solver pcg: the whole bench line is about preconditioned CG
+        h.fcg_set_preconditioner(to(w.s), inputs_mod.precond_kbar(w.k))
+        solve = h.fcg_pcg_solve
     for _ in range(warmup):
         u.zero_()
-        it, rr, st = h.fcg_solve(k, f, u, w.tol, w.maxit)
+        it, rr, st = solve(k, f, u, w.tol, w.maxit)
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
     iters, launches = [], 0
     torch.cuda.synchronize()
@@ -130,7 +135,7 @@ def bench_workload(binding, torch, w, steps, warmup, profile_iters=20, e2e_steps
     for s in range(steps):
         ev[s][0].record()
         u.zero_()                                          # u0 = 0 is part of the workload (otherwise a warm start)
-        it, rr, st = h.fcg_solve(k, f, u, w.tol, w.maxit)
+        it, rr, st = solve(k, f, u, w.tol, w.maxit)
         ev[s][1].record()
         iters.append(it); launches += h.fcg_last_launch_count()
     torch.cuda.synchronize()
@@ -139,6 +144,11 @@ def bench_workload(binding, torch, w, steps, warmup, profile_iters=20, e2e_steps
     out = {"iters": iters, "status": st, "relres": rr, "dev_ms": dev_ms, "wall_s": wall, "launches": launches}
     # per-kernel times, in loop order, CUDA events on the library's stream
     u.zero_()
+    if solver == "pcg":
+        out["kernel_ms"] = dict(zip(PCG_NAMES, h.fcg_profile_pcg_iteration(k, f, u, profile_iters)))
+        out["e2e_iter_s"] = None; out["h2d"] = 0; out["d2h"] = 0
+        h.close()
+        return out
     ms = h.fcg_profile_iteration(k, f, u, profile_iters)
     out["kernel_ms"] = dict(zip(PASS_NAMES, ms))
     # end to end with HOST buffers through the C ABI
@@ -184,7 +194,7 @@ def bench_workload(binding, torch, w, steps, warmup, profile_iters=20, e2e_steps
 
 def bench_extras(binding, torch, inputs):
     """--full: the rest of north_star's list -- stand-alone transforms (GB/s on 4 N w bytes per transform), the break step, and
-    the quasi-static loop of configs[3] (first 200 of its 2000 steps; latency-bound: us per CG iteration is the figure)."""
+    the quasi-static loop of configs[3] (all 2000 steps, CG and PCG solves, and ensembles; latency-bound: us per CG iteration and break steps per second are the figures)."""
     out = {}
     to = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
     for L, dt, tdt in ((2048, np.float64, torch.float64), (2048, np.float32, torch.float32), (8192, np.float32, torch.float32)):
@@ -213,15 +223,40 @@ def bench_extras(binding, torch, inputs):
     for _ in range(20): h.fcg_break_step(k, u, t)
     out["break_step_L2048_f64"] = {"us_per_call_incl_host_sync": 1e6 * (time.perf_counter() - t0) / 20, "bytes": 3 * w.N * 8}
     h.close()
-    w3 = inputs.config(3, nsteps=200)
-    h = binding.Fcg(w3.L, torch.float64); h.fcg_set_spectrum(to(w3.s))
-    k, f, u, t = to(w3.k), to(w3.f), to(w3.u0), to(w3.t)
-    torch.cuda.synchronize(); t0 = time.perf_counter()
-    index, iters, done, st = h.fcg_fracture(k, f, u, t, 200, w3.tol, w3.maxit)
-    dt_s = time.perf_counter() - t0
-    out["fracture_cfg3_first200"] = {"steps": int(done), "cg_iterations": int(iters.sum()), "wall_s": dt_s,
-                                     "us_per_cg_iteration": 1e6 * dt_s / max(int(iters.sum()), 1), "status": int(st)}
-    h.close()
+    # quasi-static loop of configs[3], all 2000 steps in one cooperative launch: CG solves, PCG solves, and an ensemble of
+    # independent samples (different threshold seeds) on several streams through fcg_fracture_begin / _end
+    w3 = inputs.config(3)
+    for name, pcg in (("fracture_cfg3", False), ("fracture_cfg3_pcg", True)):
+        h = binding.Fcg(w3.L, torch.float64); s3 = to(w3.s); h.fcg_set_spectrum(s3)
+        if pcg:
+            h.fcg_set_preconditioner(s3, 1.0)
+        best = None
+        for rep in range(2):
+            k, f, u, t = to(w3.k), to(w3.f), to(w3.u0), to(w3.t)
+            torch.cuda.synchronize(); t0 = time.perf_counter()
+            index, iters, done, st = (h.fcg_pcg_fracture if pcg else h.fcg_fracture)(k, f, u, t, w3.nsteps, w3.tol, w3.maxit)
+            dt_s = time.perf_counter() - t0
+            best = dt_s if best is None else min(best, dt_s)
+        out[name] = {"steps": int(done), "iterations": int(iters.sum()), "wall_s": best, "steps_per_s": int(done) / best,
+                     "us_per_iteration": 1e6 * best / max(int(iters.sum()), 1), "status": int(st), "launches": h.fcg_last_launch_count()}
+        h.close()
+    for nrep in (2, 4, 6):
+        reps = []
+        for r in range(nrep):
+            stream = torch.cuda.Stream()
+            with torch.cuda.stream(stream):
+                h = binding.Fcg(w3.L, torch.float64, stream=stream); s3 = to(w3.s); h.fcg_set_spectrum(s3); h.fcg_set_preconditioner(s3, 1.0)
+                reps.append((h, to(w3.k), to(w3.f), to(w3.u0), to(inputs.thresholds(w3.L, seed=100 + r))))
+        torch.cuda.synchronize(); t0 = time.perf_counter()
+        for h, k, f, u, t in reps:
+            h.fcg_fracture_begin(k, f, u, t, w3.nsteps, w3.tol, w3.maxit, True)
+        res = [h.fcg_fracture_end() for h, *_ in reps]
+        dt_s = time.perf_counter() - t0
+        out[f"fracture_cfg3_pcg_ensemble{nrep}"] = {"samples": nrep, "steps": sum(int(r[2]) for r in res), "wall_s": dt_s,
+                                                    "steps_per_s": sum(int(r[2]) for r in res) / dt_s,
+                                                    "iterations": sum(int(r[1].sum()) for r in res)}
+        for h, *_ in reps:
+            h.close()
     return out
 
 
@@ -247,6 +282,9 @@ def main():
     ap.add_argument("--impl", choices=["fcg", "reference"], default="fcg")
     ap.add_argument("--ref-iters", type=int, default=8, help="oracle CG iterations per reference step / cpu_baseline sample")
     ap.add_argument("--full", action="store_true", help="also time configs[2] fp32 and configs[4] (reported under 'extra')")
+    ap.add_argument("--solver", choices=["cg", "pcg"], default="cg",
+                    help="pcg: time fcg_pcg_solve instead (metric pcg_iterations_per_s, 22 N w bytes per iteration; no e2e leg) -- "
+                         "for profiling the PCG kernels; the headline BASELINE.json names is the default")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-pcg", action="store_true", help="skip the preconditioned-CG time-to-solution of the same workload ('pcg' key)")
     ap.add_argument("--loop-mode", type=int, default=0, choices=[0, 1],
@@ -278,8 +316,28 @@ def main():
     torch.cuda.synchronize()
     if sampler:
         sampler.start()
-    res = bench_workload(binding, torch, w, args.steps, args.warmup, loop_mode=args.loop_mode)
+    res = bench_workload(binding, torch, w, args.steps, args.warmup, loop_mode=args.loop_mode, solver=args.solver, inputs_mod=inputs)
     clocks = sampler.stop() if sampler else None
+    if args.solver == "pcg":
+        if world > 1:
+            raise SystemExit("--solver pcg is a single-GPU profiling mode")
+        names, nws, b_iter = PCG_NAMES, PCG_NW, sum(PCG_NW.values())
+        kms = res["kernel_ms"]; nw = w.N * wbytes; it0 = res["iters"][0]
+        t_iter_us = 1e3 * (sum(res["dev_ms"]) / len(res["dev_ms"])) / max(it0, 1)
+        dom = max(names, key=lambda n: kms[n])
+        ach = nws[dom] * nw / (kms[dom] * 1e-3) / 1e9
+        print(json.dumps({
+            "metric": "pcg_iterations_per_s", "value": sum(res["iters"]) / (sum(res["dev_ms"]) * 1e-3), "unit": UNIT, "n_gpus": 1,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": sum(res["dev_ms"]) / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": args.dtype, "data": "synthetic",
+            "config": {"workload": f"BASELINE.json configs[{args.config}] L={w.L} {args.dtype} solved by preconditioned CG ({it0} iterations)"},
+            "us_per_iteration": t_iter_us, "kernel_us": {n: 1e3 * kms[n] for n in names},
+            "kernel_gbs": {n: nws[n] * nw / (kms[n] * 1e-3) / 1e9 for n in names},
+            "iteration_roofline": {"bound": "hbm", "bytes_per_iteration": b_iter * nw, "achieved": b_iter * nw / (t_iter_us * 1e-6) / 1e9,
+                                   "peak": hbm_peak, "unit": "GB/s", "frac": b_iter * nw / (t_iter_us * 1e-6) / 1e9 / hbm_peak},
+            "roofline": {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": hbm_peak, "unit": "GB/s", "frac": ach / hbm_peak, "traffic": None},
+            "gpu_launches": res["launches"], "clocks": clocks, "final_rel_residual": res["relres"], "status": res["status"]}))
+        return
     if rank == 0 and world == 1 and not args.no_pcg and args.loop_mode == 0:      # outside the timed region of the headline
         res["pcg"] = bench_workload(binding, torch, w, 3, 1, loop_mode=0, pcg_steps=5, inputs_mod=inputs, e2e_steps=1)["pcg"]
 
