@@ -27,8 +27,11 @@ sys.path.insert(0, ROOT)
 
 METRIC, UNIT = "cg_iterations_per_s", "iter/s"
 B_ITER_NW = 16.5          # algorithmic bytes per CG iteration in units of N*w
-PASS_NW = {"row_fwd": 6.0, "col": 2.5, "row_inv": 4.0, "update_r": 3.0}   # this implementation's per-kernel algorithmic bytes / (N*w)
-PASS_NAMES = ["row_fwd", "col", "row_inv", "update_r"]
+# this implementation's per-kernel algorithmic bytes / (N*w) (DESIGN.md sections 4 and 12).  Default path (spectral search length):
+# three launches, the residual update rides in the last pass and q is never stored; --no-spectral-alpha: four launches.
+PASS_NW_SL = {"row_fwd": 6.0, "col": 2.5, "row_inv": 5.0}
+PASS_NW_4K = {"row_fwd": 6.0, "col": 2.5, "row_inv": 4.0, "update_r": 3.0}
+PASS_NW, PASS_NAMES = PASS_NW_SL, list(PASS_NW_SL)
 # preconditioned CG: six kernels per iteration, 22 N*w algorithmic bytes
 PCG_NAMES = ["row_fwd", "col", "row_inv", "rupd_row_fwd", "col_precond", "row_inv_precond"]
 PCG_NW = {"row_fwd": 6.0, "col": 2.5, "row_inv": 4.0, "rupd_row_fwd": 4.0, "col_precond": 2.5, "row_inv_precond": 3.0}
@@ -118,6 +121,7 @@ def bench_workload(binding, torch, w, steps, warmup, profile_iters=20, e2e_steps
     wbytes = w.dtype.itemsize
     h = binding.Fcg(w.L, tdt)
     h.fcg_set_option(binding.FCG_OPT_LOOP_MODE, loop_mode)
+    h.fcg_set_option(binding.FCG_OPT_SPECTRAL_ALPHA, 1 if len(PASS_NAMES) == 3 else 0)
     to = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
     h.fcg_set_spectrum(to(w.s))
     k, f, u = to(w.k), to(w.f), to(w.u0)
@@ -150,7 +154,7 @@ def bench_workload(binding, torch, w, steps, warmup, profile_iters=20, e2e_steps
         h.close()
         return out
     ms = h.fcg_profile_iteration(k, f, u, profile_iters)
-    out["kernel_ms"] = dict(zip(PASS_NAMES, ms))
+    out["kernel_ms"] = dict(zip(PASS_NAMES, ms))          # (with three launches ms[3] is the empty event pair)
     # end to end with HOST buffers through the C ABI
     e2e_steps = e2e_steps or max(1, min(steps, 3))
     kh, fh = torch.from_numpy(w.k.copy()).pin_memory(), torch.from_numpy(w.f.copy()).pin_memory()
@@ -286,11 +290,16 @@ def main():
                     help="pcg: time fcg_pcg_solve instead (metric pcg_iterations_per_s, 22 N w bytes per iteration; no e2e leg) -- "
                          "for profiling the PCG kernels; the headline BASELINE.json names is the default")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-spectral-alpha", action="store_true",
+                    help="four launches per iteration: p.Ap as a dot product after the last pass + a residual-update kernel")
     ap.add_argument("--no-pcg", action="store_true", help="skip the preconditioned-CG time-to-solution of the same workload ('pcg' key)")
     ap.add_argument("--loop-mode", type=int, default=0, choices=[0, 1],
                     help="0: whole solve as one CUDA graph with a device-side WHILE node (default); 1: direct launches (for ncu)")
     args = ap.parse_args()
 
+    global PASS_NW, PASS_NAMES
+    if args.no_spectral_alpha:
+        PASS_NW, PASS_NAMES = PASS_NW_4K, list(PASS_NW_4K)
     rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
     if args.impl == "reference":
@@ -370,7 +379,8 @@ def main():
         "config": {"workload": f"BASELINE.json configs[{args.config}]: L={w.L} {args.dtype}, tol={w.tol:g}, one step = one full CG solve from u0=0 "
                                f"({it_per_solve} iterations)", "L": w.L, "iterations_per_solve": it_per_solve,
                    "l2_policy": f"inputs larger than L2: working set {7.5 * nw / 2**20:.0f} MiB per solve vs 126 MB L2; no flush",
-                   "parallelism": "replicas only" if world > 1 else "single GPU"},
+                   "parallelism": "replicas only" if world > 1 else "single GPU",
+                   "launches_per_iteration": len(PASS_NAMES)},
         "site_iterations_per_s": value * w.N,
         "us_per_iteration": t_iter_us,
         "iteration_roofline": {"bound": "hbm", "bytes_per_iteration": B_ITER_NW * nw, "achieved": B_ITER_NW * nw / (t_iter_us * 1e-6) / 1e9,

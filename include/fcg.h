@@ -68,6 +68,11 @@ typedef enum {
     FCG_OPT_L2_HINTS     = 7, /* bit mask (default 63: all) of L2 eviction-priority hints in the pipelined passes:
                                  1 u strips (P1 loads) evict-first, 2 u stores evict-first, 4 spectrum rows (P2) evict-first,
                                  8 T2 tiles (P3 loads) evict-first, 16 k strips (P3) evict-first, 32 q loads (P4) evict-first */
+    FCG_OPT_SPECTRAL_ALPHA = 8, /* 1 (default): fcg_solve evaluates the search length's p.Ap as sum k p^2 (a scalar recurrence fed by the
+                                 last pass) + sum shat |P|^2 (Parseval, accumulated in the column pass), so alpha is known before the
+                                 last pass and r -= alpha q, r.r ride in it: 3 launches and 13.5 N w bytes per iteration, q never
+                                 stored (pipelined engine).  0: p.q as a dot product after the last pass and a
+                                 fourth kernel for the residual update (15.5 N w) */
     FCG_OPT_ENGINE       = 3  /* 0 (default): pipelined TMA passes where the lattice is large enough (L >= 256), classic
                                  passes otherwise; 1: classic passes only (synchronous loads; kept for A/B measurements).
                                  The stored spectrum's layout belongs to the engine: changing the engine after

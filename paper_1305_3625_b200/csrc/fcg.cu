@@ -40,7 +40,7 @@ const PassTable* get_table(int L, int dtype) {
 }
 
 struct Layout {            // byte offsets into the workspace
-    size_t Tb, shat, mhat, r, p, q, z, tw, partial_row, partial_vec, brk_r, brk_i, scalars, brk_out, brk_ticket, total;
+    size_t Tb, shat, mhat, r, p, q, z, tw, partial_row, partial_col, partial_vec, brk_r, brk_i, scalars, brk_out, brk_ticket, total;
 };
 Layout make_layout(int L, size_t w) {
     const size_t N = (size_t)L * L;
@@ -53,6 +53,7 @@ Layout make_layout(int L, size_t w) {
     o.z = take(N * w);                                    // PCG: z = M^-1 r
     o.tw = take((size_t)L * 2 * w);
     o.partial_row = take((size_t)L * 2 * sizeof(double));
+    o.partial_col = take((size_t)L / 2 * sizeof(double));      // spectral search length: one partial sum per column
     o.partial_vec = take(VEC_BLOCKS_MAX * sizeof(double));
     o.brk_r = take(VEC_BLOCKS_MAX * sizeof(double));
     o.brk_i = take(VEC_BLOCKS_MAX * sizeof(long long));
@@ -77,12 +78,13 @@ struct fcg_handle_s {
     char* ws = nullptr; bool own_ws = false;
     Layout lay{};
     bool have_spectrum = false, have_precond = false;
-    int loop_mode = 0, chunk = 16, row_var_opt = -1, engine_opt = 0, nsm = 148, unroll = 4, pdl = 0, fused_opt = 1, hints = 63;
+    int loop_mode = 0, chunk = 16, row_var_opt = -1, engine_opt = 0, nsm = 148, unroll = 4, pdl = 0, fused_opt = 1, hints = 63, sl_opt = 1;
     alignas(64) CUtensorMap tmap_row;   // T2 as [L/(2 NB)][L/2][128 B]: box = v2_tsub/NB lines of one row pair (row_inv2 tiles)
     alignas(64) CUtensorMap tmap_col;   // T2 as [L/(2 NB)][L/2][NB][2 complex]: box = one column x v2_abox row pairs (col2 gather / scatter)
     bool have_tmap = false;
     int spectrum_colpos = 0;            // layout the stored spectrum was prepared for (1: T2 column order)
     bool v2() const { return engine_opt == 0 && tab->v2 && have_tmap; }
+    bool sl() const { return sl_opt && v2() && tab->sl_ok; }     // spectral search length: 3 launches per CG iteration
     bool fused() const { return fused_opt && tab->fused && v2() && loop_mode == 0; }   // whole solve in one cooperative kernel
     Scalars* h_sc = nullptr;            // pinned
     BreakResult* h_brk = nullptr;       // pinned
@@ -100,6 +102,18 @@ struct fcg_handle_s {
         size_t nvec = N / (dtype == FCG_F64 ? 2 : 4);
         size_t b = (nvec + 255) / 256;
         return (int)(b < (size_t)VEC_BLOCKS_MAX ? b : (size_t)VEC_BLOCKS_MAX);
+    }
+    // Grid of cg_update_r_kernel: every thread makes the same whole number of unrolled trips (4 vectors of 16 bytes each), so
+    // that no thread is left with a tail of serially dependent single loads: at L = 2048 fp64 1184 CTAs meant one unrolled
+    // trip + up to three dependent ones, 1024 CTAs are exactly two unrolled trips
+    int update_blocks() const {
+        const size_t nvec = N / (dtype == FCG_F64 ? 2 : 4), per = 256 * 4;
+        size_t b = (nvec + per - 1) / per;
+        if (b > (size_t)VEC_BLOCKS_MAX) {
+            const size_t trips = (nvec + (size_t)VEC_BLOCKS_MAX * per - 1) / ((size_t)VEC_BLOCKS_MAX * per);
+            b = (nvec + per * trips - 1) / (per * trips);
+        }
+        return (int)(b < 1 ? 1 : b);
     }
     int row_var() const {
         if (row_var_opt >= 0 && row_var_opt < FCG_NROWVAR && tab->row_valid[row_var_opt]) return row_var_opt;
@@ -164,6 +178,11 @@ template <typename T> struct Seq {
         if ((e = row_fwd(ROWF_PLAIN, u, nullptr)) != cudaSuccess) return e;
         if ((e = col(COL_CONV, false)) != cudaSuccess) return e;
         if ((e = row_inv(ROWI_RESID, k, u, f, r(), p())) != cudaSuccess) return e;
+        if (sl()) {      // start value of the sum k p^2 recurrence: the first direction is p = r
+            cg_kpp0_kernel<T><<<h->vec_blocks(), 256, 0, st>>>(k, (const T*)r(), h->N / Vec<T>::W, h->at<double>(h->lay.partial_vec), h->sc());
+            ++h->launches;
+            return cudaGetLastError();
+        }
         if (!pcg) return e;
         if ((e = row_fwd(ROWF_PLAIN, r(), nullptr, 1)) != cudaSuccess) return e;
         return it_precond();
@@ -192,8 +211,8 @@ template <typename T> struct Seq {
         ++h->launches;
         return h->tab->row_fwd2_rupd(&A, st);
     }
-    int launches_per_iteration() const { return pcg ? (v2() ? 6 : 7) : 4; }
-    int launches_outside_loop() const { return pcg ? 8 : 5; }
+    int launches_per_iteration() const { return pcg ? (v2() ? 6 : 7) : (sl() ? 3 : 4); }
+    int launches_outside_loop() const { return pcg ? 8 : (sl() ? 6 : 5); }
     // one pass of Listing 2, as four launches
     cudaError_t it_row_fwd(T* u) const { return row_fwd(ROWF_CG, nullptr, u); }                    // new x (lagged), new p, row transform
     cudaError_t it_col() const { return col(COL_CONV, true); }                                     // column transform * spectrum * inverse
@@ -202,15 +221,35 @@ template <typename T> struct Seq {
         const size_t nvec = h->N / Vec<T>::W;
         ++h->launches;
         cudaLaunchConfig_t cfg{};
-        cfg.gridDim = dim3((unsigned)h->vec_blocks()); cfg.blockDim = dim3(256); cfg.dynamicSmemBytes = 0; cfg.stream = st;
+        cfg.gridDim = dim3((unsigned)h->update_blocks()); cfg.blockDim = dim3(256); cfg.dynamicSmemBytes = 0; cfg.stream = st;
         cudaLaunchAttribute at[1];
         at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
         at[0].val.programmaticStreamSerializationAllowed = 1;
         cfg.attrs = at; cfg.numAttrs = h->pdl ? 1u : 0u;
         return cudaLaunchKernelEx(&cfg, cg_update_r_kernel<T>, r(), (const T*)q(), nvec, h->at<double>(h->lay.partial_vec), h->sc(), h->hints);
     }
+    // spectral search length: alpha is known after the column pass, so the residual update rides in P3
+    cudaError_t it_col_e() const {
+        ColArgs<T> A{}; A.mode = COL_CONV; A.Tb = Tb(); A.shat = shat(); A.hints = h->hints; A.tw = tw(); A.sc = h->sc(); A.pdl = h->pdl;
+        A.partial = h->at<double>(h->lay.partial_col);
+        ++h->launches;
+        return h->tab->col2_energy(&A, &h->tmap_col, st);
+    }
+    cudaError_t it_row_inv_f(const T* k) const {
+        RowInvArgs<T> A{}; A.mode = ROWI_CGF; A.Tb = Tb(); A.tw = tw(); A.k = k; A.v = p(); A.f = r(); A.out = r(); A.hints = h->hints;
+        A.partial = h->at<double>(h->lay.partial_row); A.colsum = h->at<double>(h->lay.partial_col);
+        A.sc = h->sc(); A.nsm = h->nsm; A.pdl = h->pdl;
+        ++h->launches;
+        return h->tab->row_inv2_cgf(&A, &h->tmap_row, st);
+    }
+    bool sl() const { return !pcg && !classic && h->sl(); }
     cudaError_t iteration(const T* k, T* u) const {
         cudaError_t e;
+        if (sl()) {
+            if ((e = it_row_fwd(u)) != cudaSuccess) return e;
+            if ((e = it_col_e()) != cudaSuccess) return e;
+            return it_row_inv_f(k);
+        }
         if ((e = it_row_fwd(u)) != cudaSuccess) return e;
         if ((e = it_col()) != cudaSuccess) return e;
         if ((e = it_row_inv(k)) != cudaSuccess) return e;
@@ -309,7 +348,7 @@ int solve_impl(fcg_handle h, const void* k, const void* f, void* u, double tol, 
         h->fused_opt = 0;
     }
     if (h->loop_mode == 0) {
-        const int var = h->v2() ? 100 : h->row_var();
+        const int var = h->v2() ? 100 + (h->sl() ? 1 : 0) : h->row_var();
         GraphEntry* hit = nullptr;
         for (auto& g : h->graphs)
             if (g.k == k && g.f == f && g.u == u && g.tol == tol && g.maxit == maxit && g.var == var && g.unroll == h->unroll && g.pdl == h->pdl && g.pcg == (pcg ? 1 : 0) + 2 * h->hints) { hit = &g; break; }
@@ -430,6 +469,14 @@ int profile_impl(fcg_handle h, const void* k, const void* f, void* u, int iters,
     for (auto& e : ev) FCG_CK(h, cudaEventCreate(&e));
     for (int i = 0; i < iters; ++i) {
         cudaEvent_t* e = &ev[(size_t)i * 5];
+        if (s.sl()) {       // three launches: the residual update is part of P3 (ms[3] = 0)
+            FCG_CK(h, cudaEventRecord(e[0], h->stream)); FCG_CK(h, s.it_row_fwd((T*)u));
+            FCG_CK(h, cudaEventRecord(e[1], h->stream)); FCG_CK(h, s.it_col_e());
+            FCG_CK(h, cudaEventRecord(e[2], h->stream)); FCG_CK(h, s.it_row_inv_f((const T*)k));
+            FCG_CK(h, cudaEventRecord(e[3], h->stream));
+            FCG_CK(h, cudaEventRecord(e[4], h->stream));
+            continue;
+        }
         FCG_CK(h, cudaEventRecord(e[0], h->stream)); FCG_CK(h, s.it_row_fwd((T*)u));
         FCG_CK(h, cudaEventRecord(e[1], h->stream)); FCG_CK(h, s.it_col());
         FCG_CK(h, cudaEventRecord(e[2], h->stream)); FCG_CK(h, s.it_row_inv((const T*)k));
@@ -617,6 +664,7 @@ int fcg_set_option(fcg_handle h, int option, int value) {
         case FCG_OPT_FUSED: if (value != 0 && value != 1) return fail(h, FCG_INVALID_ARG, "fused must be 0 or 1"); h->fused_opt = value; return FCG_OK;
         case FCG_OPT_PDL: if (value != 0 && value != 1) return fail(h, FCG_INVALID_ARG, "pdl must be 0 or 1"); h->pdl = value; return FCG_OK;
         case FCG_OPT_L2_HINTS: if (value < 0 || value > 63) return fail(h, FCG_INVALID_ARG, "hints must be 0..63"); h->hints = value; return FCG_OK;
+        case FCG_OPT_SPECTRAL_ALPHA: if (value != 0 && value != 1) return fail(h, FCG_INVALID_ARG, "spectral alpha must be 0 or 1"); h->sl_opt = value; return FCG_OK;
         case FCG_OPT_UNROLL: if (value < 1 || value > 64) return fail(h, FCG_INVALID_ARG, "unroll must be 1..64"); h->unroll = value; return FCG_OK;
         case FCG_OPT_ENGINE:
             if (value != 0 && value != 1) return fail(h, FCG_INVALID_ARG, "engine must be 0 or 1");

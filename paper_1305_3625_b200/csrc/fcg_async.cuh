@@ -113,9 +113,10 @@ template <typename P> constexpr int per_max() {
 // RUPD = true (a separate instantiation, so that the CG kernel's register allocation is untouched) is the PCG pass
 //   r -= alpha q;  partial r.r -> last CTA: count, convergence;  columns of T2 = row transforms of the new r
 // whose strips are r0 r1 q0 q1 (4 pieces) and which ends with the grid-wide reduction of cg_update_r_kernel.
-template <typename T, typename P, int CTAS, bool RUPD = false>
+template <typename T, typename P, int CTAS, int VAR = 0>
 __global__ void __launch_bounds__(P::NT + 32, CTAS) row_fwd2_kernel(const RowFwdArgs<T> A)
 {
+    constexpr bool RUPD = VAR == 1;
     using AS = AsyncShape<T, P>;
     constexpr int L = P::N, S = P::S, NT = P::NT, R1 = AS::R1, Q1 = AS::Q1, PER1 = AS::PER1, PM = per_max<P>();
     constexpr uint32_t PIECE = AS::PIECE;
@@ -267,7 +268,10 @@ __global__ void __launch_bounds__(P::NT + 32, CTAS) row_fwd2_kernel(const RowFwd
 
 // --------------------------------------------------------------------------------------------- P2
 //   column m of T2, in place:  T2[m][.] <- F^H ( shat[m][.] o F T2[m][.] )
-template <typename T, typename P, int CTAS>
+// ENERGY = true (a separate instantiation) also accumulates the spectral half of the search length,
+//   p.Cp = sum over the full spectrum of shat |P|^2 = 2 x (columns 0 < n < L/2) + (columns n = 0, L/2)      (Parseval),
+// in the registers of the spectral multiply, and leaves one partial sum per column; row_inv2_kernel<.., 2> adds them up.
+template <typename T, typename P, int CTAS, bool ENERGY = false>
 __global__ void __launch_bounds__(P::NT, CTAS) col2_kernel(const ColArgs<T> A, const __grid_constant__ CUtensorMap tmap)
 {
     using AS = AsyncShape<T, P>;
@@ -305,6 +309,7 @@ __global__ void __launch_bounds__(P::NT, CTAS) col2_kernel(const ColArgs<T> A, c
     const bool done = A.sc && A.sc->done;
     tma::mbar_wait(&bar, 0);
     if (done) return;
+    double energy = 0.0;
 
     auto ld_sw = [&](int e) { return io.ld(e); };
     auto st_sw = [&](int e, cx<T> v) { io.st(e, v); };
@@ -335,7 +340,12 @@ __global__ void __launch_bounds__(P::NT, CTAS) col2_kernel(const ColArgs<T> A, c
     if (n != 0) {
         static_for_up<2, S - 1>(fwd_smem_stage);
         // last forward stage * shat * first inverse stage, in registers
-        run_middle<P, T>(lt, ld_sw, st_sw, [&](int g, int u) { return sh[u * (L / P::RLAST) + g]; });
+        if constexpr (ENERGY) {
+            run_middle<P, T, true>(lt, ld_sw, st_sw, [&](int g, int u) { return sh[u * (L / P::RLAST) + g]; }, &energy);
+            energy *= 2.0;                                       // column n stands for n and L - n
+        } else {
+            run_middle<P, T>(lt, ld_sw, st_sw, [&](int g, int u) { return sh[u * (L / P::RLAST) + g]; });
+        }
         __syncthreads();
         static_for_down<S - 1, 2>(inv_smem_stage);
     } else {
@@ -351,6 +361,14 @@ __global__ void __launch_bounds__(P::NT, CTAS) col2_kernel(const ColArgs<T> A, c
             const int i1 = P::shat_index(e), i2 = P::shat_index(e2);
             va.x = sp_[i1] * Wa.x + sm_[i1] * Wb.x; va.y = sp_[i1] * Wa.y - sm_[i1] * Wb.y;
             vb.x = sp_[i2] * Wb.x + sm_[i2] * Wa.x; vb.y = sp_[i2] * Wb.y - sm_[i2] * Wa.y;
+            if constexpr (ENERGY) {
+                // s0 |Y0|^2 + sN |YN|^2 at m (and the same again at -m) = sp/2 (|Wa|^2 + |Wb|^2) + sm Re(Wa Wb)
+                const double na = (double)Wa.x * (double)Wa.x + (double)Wa.y * (double)Wa.y;
+                const double nb = (double)Wb.x * (double)Wb.x + (double)Wb.y * (double)Wb.y;
+                const double re = (double)Wa.x * (double)Wb.x - (double)Wa.y * (double)Wb.y;
+                const double term = 0.5 * (double)sp_[i1] * (na + nb) + (double)sm_[i1] * re;
+                energy += e2 != e ? 2.0 * term : term;
+            }
             io.st(e, va);
             if (e2 != e) io.st(e2, vb);
         }
@@ -372,8 +390,14 @@ __global__ void __launch_bounds__(P::NT, CTAS) col2_kernel(const ColArgs<T> A, c
         for (int b = 0; b < (L / 2) / ABOX; ++b)
             tma::tensor_s2g_4d(&tmap, 0, n % AS::NB, b * ABOX, n / AS::NB, smem_raw + (size_t)b * BOXB);
         tma::bulk_commit();
-        tma::bulk_wait_read0();          // shared memory must outlive the store's read
     }
+    if constexpr (ENERGY) {      // this column's share of sum shat |P|^2, while the scatter drains; the next pass adds the L/2 shares
+        __shared__ double red[32];
+        double ev[1] = {energy};
+        block_sum<1>(ev, red);
+        if (lt == 0) A.partial[n] = ev[0];
+    }
+    if (lt == 0) tma::bulk_wait_read0();          // shared memory must outlive the store's read
 }
 
 // --------------------------------------------------------------------------------------------- stand-alone transforms
@@ -530,14 +554,30 @@ __global__ void __launch_bounds__(256) t2_import_kernel(const cx<T>* __restrict_
 // (TSUB columns x 2 rows as whole 128-byte lines, TMA tensor loads) for the rebuild of the packed spectrum, and strips
 // of k, p (, f) for the epilogue; both run ahead across transforms as far as shared memory allows.
 // PRE = true (a separate instantiation) is the preconditioner pass of PCG: z = c, partial r.z, strips r0 r1 (k = r).
-template <typename T, typename P, int CTAS, bool PRE = false>
+// VAR = 2 (CGF) is the last pass of the spectral-search-length path.  p.Ap = sum k p^2 + sum shat |P|^2
+// (Parseval) is known before the pass starts: the first term is carried by a scalar recurrence (below), the second is the sum
+// of the column pass's L/2 partial sums, which every CTA adds up itself in the same fixed order (bit-identical alpha in all
+// CTAs, no broadcast).  So q = k o p + c is consumed on the spot -- r -= alpha q, r.r -> count, convergence, beta -- and never
+// stored: strips k0 k1 p0 p1 r0 r1, output r in place.  The pass also accumulates t = sum k r'^2 and v = sum k r' p for
+//     sum k p'^2 = t + 2 beta v + beta^2 sum k p^2        (p' = r' + beta p, the next direction).
+template <typename T, typename P, int CTAS, int VAR = 0>
 __global__ void __launch_bounds__(AsyncShape<T, P>::INV_THREADS, CTAS) row_inv2_kernel(const RowInvArgs<T> A, const __grid_constant__ CUtensorMap tmap)
 {
     using AS = AsyncShape<T, P>;
     constexpr int L = P::N, S = P::S, NT = P::NT, R1 = AS::R1, Q1 = AS::Q1, PER1 = AS::PER1, PM = per_max<P>();
-    constexpr uint32_t PIECE = AS::PIECE;
-    constexpr int TSUB = AS::TSUB, NSUB = AS::NSUB, NTS = AS::NTS;
+    constexpr bool PRE = VAR == 1, CGF = VAR == 2;
+    constexpr int TSUB = AS::TSUB, NSUB = AS::NSUB;
     constexpr uint32_t TBYTES = (uint32_t)AS::TSB;
+    // CGF moves three vectors of strips per transform against one of tiles: its strips are NT elements long (SPT of them per
+    // stage-1 strip), the tile ring holds one transform (NSUB tiles) if that leaves two strip slots, and the strips get the rest
+    // (whole stage-1 strips where three slots of those fit beside two tiles: 512-byte pieces cost more than they bring)
+    constexpr bool FINE = CGF && (AS::RING_BUDGET - 2 * AS::TSB) / (6 * (size_t)AS::PIECE) < 3;
+    constexpr int SPT = FINE ? PER1 : 1, QV = FINE ? NT : Q1;
+    constexpr uint32_t PIECE = (uint32_t)(QV * sizeof(T));
+    constexpr int NTSF_ = (int)((AS::RING_BUDGET - 12 * (size_t)PIECE) / AS::TSB);
+    constexpr int NTS = CGF ? (NTSF_ < 2 ? 2 : (NTSF_ > NSUB ? NSUB : NTSF_)) : AS::NTS;
+    constexpr size_t KRB = CGF ? AS::RING_BUDGET - (size_t)NTS * AS::TSB : AS::KRB;
+    static_assert(NTS <= AS::MAXSLOT && KRB >= 6 * (size_t)PIECE, "P3 rings");
     extern __shared__ unsigned char smem_dyn[];
     unsigned char* const smem_raw = align128(smem_dyn);
     __shared__ __align__(8) uint64_t tfull[AS::MAXSLOT], tempty[AS::MAXSLOT];
@@ -548,11 +588,11 @@ __global__ void __launch_bounds__(AsyncShape<T, P>::INV_THREADS, CTAS) row_inv2_
     unsigned char* const kring = tring + (size_t)NTS * AS::TSB;
     SmemIO<T, P> io{W};
     const int lt = threadIdx.x, lane = lt & 31, warp = lt >> 5;
-    const int mode = PRE ? (int)ROWI_PRECOND : A.mode;
+    const int mode = PRE ? (int)ROWI_PRECOND : CGF ? (int)ROWI_CGF : A.mode;
     tma::grid_dep_launch();
     const bool st_on = A.mode >= 0;                               // always true, opaque to the compiler (as in row_fwd2_kernel)
-    const int nv = PRE ? 2 : (mode == ROWI_PLAIN ? 0 : (mode == ROWI_RESID ? 6 : 4));
-    int nks = nv ? (int)(AS::KRB / (nv * PIECE)) : 1;
+    const int nv = PRE ? 2 : CGF ? 6 : (mode == ROWI_PLAIN ? 0 : (mode == ROWI_RESID ? 6 : 4));
+    int nks = nv ? (int)(KRB / (nv * PIECE)) : 1;
     nks = nks > AS::MAXSLOT ? AS::MAXSLOT : nks;
     const uint32_t kslotb = nv * PIECE;
 
@@ -570,16 +610,19 @@ __global__ void __launch_bounds__(AsyncShape<T, P>::INV_THREADS, CTAS) row_inv2_
     }
     __syncthreads();
     tma::grid_dep_wait();                                         // everything above overlaps the previous kernel's tail
-    if ((mode == ROWI_CG || PRE) && A.sc->done) return;
+    if ((mode == ROWI_CG || PRE || CGF) && A.sc->done) return;
 
     double acc[2] = {0.0, 0.0};
+    double acc3[3] = {0.0, 0.0, 0.0};            // CGF: r'.r', sum k r'^2, sum k r' p
+    double alpha_d = 0.0, pq_d = 0.0;
+    T alpha = (T)0;
     // Producer state: next tile of T2 / next strip to issue, in consumption order.  With PW (small transforms) two extra
     // warps run these loops; otherwise (NT >= 512, where two more warps would cost 8 registers per thread) consumer warp 0
     // issues the successor of every slot it has just seen released.
     constexpr bool PW = AS::PRODUCER_WARPS;
     int p_ts = 0, p_tn = 0, p_ks = 0, p_kn = 0;
     uint32_t p_tph = 0, p_kph = 0;
-    const int GT = ntl * NSUB, GK = nv ? ntl * R1 : 0;
+    const int GT = ntl * NSUB, GK = nv ? ntl * R1 * SPT : 0;
     const T* kbase = nullptr;
     if (nv) kbase = (lane < 2 ? A.k : lane < 4 ? A.v : A.f) + (size_t)(lane & 1) * L;
     // L2 hints: T2 is dead once this pass has read it (bit 3); k comes back only in the next iteration (bit 4)
@@ -594,16 +637,37 @@ __global__ void __launch_bounds__(AsyncShape<T, P>::INV_THREADS, CTAS) row_inv2_
         ++p_tn;
         if (++p_ts == NTS) { p_ts = 0; p_tph ^= 1u; }
     };
-    auto issue_next_K = [&]() {          // whole warp; strip p_kn % R1 of k0 k1 v0 v1 (f0 f1) of transform p_kn / R1, one bulk copy per lane < nv
+    auto issue_next_K = [&]() {          // whole warp; strip p_kn % (R1 SPT) of k0 k1 v0 v1 (f0 f1) of transform p_kn / (R1 SPT), one bulk copy per lane < nv
         if (p_kn >= nks) tma::mbar_wait(&kempty[p_ks], p_kph ^ 1u);
         if (lane == 0) tma::mbar_expect_tx(&kfull[p_ks], kslotb);
         __syncwarp();
         if (lane < nv)
             tma::bulk_g2s_hint(kring + (size_t)p_ks * kslotb + (size_t)lane * PIECE,
-                               kbase + (size_t)(2 * tile_of(p_kn / R1)) * L + (size_t)(p_kn % R1) * Q1, PIECE, &kfull[p_ks], pol_k);
+                               kbase + (size_t)(2 * tile_of(p_kn / (R1 * SPT))) * L + (size_t)((p_kn % (R1 * SPT)) / SPT) * Q1 + (size_t)(p_kn % SPT) * QV,
+                               PIECE, &kfull[p_ks], pol_k);
         ++p_kn;
         if (++p_ks == nks) { p_ks = 0; p_kph ^= 1u; }
     };
+    if constexpr (CGF) {
+        // search length from the column pass's partial sums, by ALL threads before the roles split (a breakdown must
+        // stop producers and consumers alike); same order in every CTA, so alpha is bit-identical everywhere
+        double e = 0.0;
+        for (int i = lt; i < L / 2; i += (int)blockDim.x) e += __ldcg(A.colsum + i);
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) e += __shfl_xor_sync(0xffffffffu, e, o);
+        if (lane == 0) red[warp] = e;
+        __syncthreads();
+        e = 0.0;
+        for (int w2 = 0; w2 < (int)(blockDim.x >> 5); ++w2) e += red[w2];
+        __syncthreads();
+        pq_d = A.sc->kpp + e;
+        if (!(pq_d > 0.0) || !isfinite(pq_d)) {                   // breakdown: nothing may change; CTA 0 reports it
+            if (blockIdx.x == 0 && lt == 0) { A.sc->pq = pq_d; A.sc->status = ST_BREAKDOWN; A.sc->done = 1; A.sc->alpha = 0.0; set_cond(A.sc, false); }
+            return;
+        }
+        alpha_d = A.sc->rho / pq_d;
+        alpha = (T)alpha_d;
+    }
     if (PW && warp == NT / 32) {
         while (p_tn < GT) issue_next_T();
     } else if (PW && warp == NT / 32 + 1) {
@@ -656,28 +720,40 @@ __global__ void __launch_bounds__(AsyncShape<T, P>::INV_THREADS, CTAS) row_inv2_
             stage_ld<P, 1, T>(lt, [&](int e) { return io.ld(e); }, c);
             bar_named<NT>();                                          // W may now be rebuilt for the next transform
             stage_math<P, 1, +1, T>(c, wb[1]);
+            T f_rr = (T)0, f_t = (T)0, f_v = (T)0;                   // CGF: one transform's sums in the working precision, then double
 #pragma unroll
             for (int t = 0; t < R1; ++t) {
+#pragma unroll
+              for (int qq = 0; qq < SPT; ++qq) {
                 const T* sl = nullptr;
                 if (nv) {
                     tma::mbar_wait(&kfull[ks], kph);
                     sl = reinterpret_cast<const T*>(kring + (size_t)ks * kslotb);
                 }
 #pragma unroll
-                for (int q = 0; q < PER1; ++q) {
-                    const int j = lt + q * NT;
-                    const size_t i0 = row0 + (size_t)t * Q1 + j;
+                for (int q = FINE ? qq : 0; q < (FINE ? qq + 1 : PER1); ++q) {
+                    const int j = FINE ? lt : lt + q * NT;              // element within the piece
+                    const size_t i0 = row0 + (size_t)t * Q1 + lt + q * NT;
                     const T c0 = c[q][t].x, c1 = c[q][t].y;
                     if (mode == ROWI_PLAIN) { A.out[i0] = c0 * A.scale; A.out[i0 + L] = c1 * A.scale; continue; }
                     if constexpr (PRE) {                                                   // z = M^-1 r, r.z
                         if (st_on) { A.out[i0] = c0; A.out[i0 + L] = c1; }
-                        acc[0] += (double)sl[j] * (double)c0; acc[0] += (double)sl[Q1 + j] * (double)c1;
+                        acc[0] += (double)sl[j] * (double)c0; acc[0] += (double)sl[QV + j] * (double)c1;
                         continue;
                     }
-                    const T v0 = sl[2 * Q1 + j], v1 = sl[3 * Q1 + j];
-                    const T val0 = sl[j] * v0 + c0, val1 = sl[Q1 + j] * v1 + c1;         // k o x + C x
+                    const T v0 = sl[2 * QV + j], v1 = sl[3 * QV + j];
+                    const T val0 = sl[j] * v0 + c0, val1 = sl[QV + j] * v1 + c1;         // k o x + C x
+                    if constexpr (CGF) {
+                        const T r0 = sl[4 * QV + j] - alpha * val0, r1 = sl[5 * QV + j] - alpha * val1;   // residue
+                        if (st_on) { A.out[i0] = r0; A.out[i0 + L] = r1; }
+                        f_rr += r0 * r0; f_rr += r1 * r1;                                                   // residue length (97)
+                        const T kr0 = sl[j] * r0, kr1 = sl[QV + j] * r1;
+                        f_t += kr0 * r0; f_t += kr1 * r1;
+                        f_v += kr0 * v0; f_v += kr1 * v1;
+                        continue;
+                    }
                     if (mode == ROWI_RESID) {
-                        const T f0 = sl[4 * Q1 + j], f1 = sl[5 * Q1 + j];
+                        const T f0 = sl[4 * QV + j], f1 = sl[5 * QV + j];
                         const T r0 = f0 - val0, r1 = f1 - val1;                           // r = f - A u
                         A.out[i0] = r0; A.out[i0 + L] = r1; A.out2[i0] = (T)0; A.out2[i0 + L] = (T)0;
                         acc[0] += (double)r0 * (double)r0; acc[0] += (double)r1 * (double)r1;
@@ -692,8 +768,23 @@ __global__ void __launch_bounds__(AsyncShape<T, P>::INV_THREADS, CTAS) row_inv2_
                     if (!PW && warp == 0 && p_kn < GK) issue_next_K();
                     if (++ks == nks) { ks = 0; kph ^= 1u; }
                 }
+              }
             }
+            if constexpr (CGF) { acc3[0] += (double)f_rr; acc3[1] += (double)f_t; acc3[2] += (double)f_v; }
         }
+    }
+    if constexpr (CGF) {         // all warps (the producers contribute zeros)
+        __shared__ double red3[3 * 32];
+        double tot[3];
+        if (!grid_sum_last<3>(acc3, A.partial, &A.sc->ticket[0], red3, tot)) return;
+        if (threadIdx.x == 0) {
+            Scalars* sc = A.sc;
+            sc->alpha = alpha_d; sc->pq = pq_d;
+            const double kpp = sc->kpp;
+            cg_after_rr(sc, tot[0]);                                                  // count, convergence, beta, rho
+            if (!sc->done) sc->kpp = tot[1] + 2.0 * sc->beta * tot[2] + sc->beta * sc->beta * kpp;
+        }
+        return;
     }
     row_inv_reduce_finalize<T>(A, acc, red);      // all warps (the producer contributes zeros)
 }

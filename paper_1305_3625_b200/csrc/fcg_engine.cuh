@@ -52,8 +52,10 @@ FCG_HD void run_stage(int lt, const cx<T>* __restrict__ tw, LD ld, ST st)
 // Last forward stage, a pointwise real multiply, and the first inverse stage, all in registers:
 //   a <- DFT_R(a);  a[u] *= mul(e_u);  a <- DFT_R^H(a)
 // (the last stage has Q = 1, so no twiddles are involved).  mul(g, u) returns the real factor for position g*R + u.
-template <typename P, typename T, typename LD, typename ST, typename MUL>
-FCG_HD void run_middle(int lt, LD ld, ST st, MUL mul)
+// ENERGY: *energy += sum of mul * |a|^2 over this thread's elements after the forward stage: the R products of one butterfly
+// are summed in the working precision, the butterflies' sums in double.
+template <typename P, typename T, bool ENERGY = false, typename LD, typename ST, typename MUL>
+FCG_HD void run_middle(int lt, LD ld, ST st, MUL mul, double* energy = nullptr)
 {
     constexpr int R = P::RLAST;
     constexpr int NB = P::N / R;
@@ -66,7 +68,14 @@ FCG_HD void run_middle(int lt, LD ld, ST st, MUL mul)
         for (int t = 0; t < R; ++t) a[t] = ld(base + t);
         dftR<R, -1>(a);
 #pragma unroll
-        for (int u = 0; u < R; ++u) { const T sv = mul(lt + i * P::NT, u); a[u].x *= sv; a[u].y *= sv; }
+        T e = (T)0;
+#pragma unroll
+        for (int u = 0; u < R; ++u) {
+            const T sv = mul(lt + i * P::NT, u);
+            if constexpr (ENERGY) e += sv * (a[u].x * a[u].x + a[u].y * a[u].y);
+            a[u].x *= sv; a[u].y *= sv;
+        }
+        if constexpr (ENERGY) *energy += (double)e;
         dftR<R, +1>(a);
 #pragma unroll
         for (int t = 0; t < R; ++t) st(base + t, a[t]);

@@ -47,8 +47,10 @@ template <typename T> struct Inst {
             if ((e = prep(row_fwd2_kernel<T, P, C_FWD>, AS::fwd_smem)) != cudaSuccess) return e;
             if ((e = prep(col2_kernel<T, P, C_COL>, AS::col_smem)) != cudaSuccess) return e;
             if ((e = prep(row_inv2_kernel<T, P, C_INV>, AS::inv_smem)) != cudaSuccess) return e;
-            if ((e = prep(row_fwd2_kernel<T, P, C_FWD, true>, AS::fwd_smem)) != cudaSuccess) return e;
-            if ((e = prep(row_inv2_kernel<T, P, C_INV, true>, AS::inv_smem)) != cudaSuccess) return e;
+            if ((e = prep(row_fwd2_kernel<T, P, C_FWD, 1>, AS::fwd_smem)) != cudaSuccess) return e;
+            if ((e = prep(row_inv2_kernel<T, P, C_INV, 1>, AS::inv_smem)) != cudaSuccess) return e;
+            if ((e = prep(col2_kernel<T, P, C_COL, true>, AS::col_smem)) != cudaSuccess) return e;
+            if ((e = prep(row_inv2_kernel<T, P, C_INV, 2>, AS::inv_smem)) != cudaSuccess) return e;
             if ((e = prep(col2_xform_kernel<T, P, C_COL, -1>, AS::WBYTES + 128)) != cudaSuccess) return e;
             if ((e = prep(col2_xform_kernel<T, P, C_COL, +1>, AS::WBYTES + 128)) != cudaSuccess) return e;
             if ((e = prep(t2_export_kernel<T, P>, AS::WBYTES + 1024)) != cudaSuccess) return e;
@@ -87,14 +89,30 @@ template <typename T> struct Inst {
     static cudaError_t row_fwd2_rupd(const void* args, cudaStream_t st) {
         if constexpr (V2) {
             const RowFwdArgs<T>& A = *static_cast<const RowFwdArgs<T>*>(args);
-            return launch(row_fwd2_kernel<T, P, C_FWD, true>, pgrid(A.nsm, C_FWD), P::NT + 32, AS::fwd_smem, st, A.pdl, A);
+            return launch(row_fwd2_kernel<T, P, C_FWD, 1>, pgrid(A.nsm, C_FWD), P::NT + 32, AS::fwd_smem, st, A.pdl, A);
+        }
+        return cudaErrorInvalidValue;
+    }
+    static constexpr bool SL = V2;
+    static cudaError_t col2_energy(const void* args, const void* tensor_map, cudaStream_t st) {
+        if constexpr (SL) {
+            const ColArgs<T>& A = *static_cast<const ColArgs<T>*>(args);
+            return launch(col2_kernel<T, P, C_COL, true>, L / 2, P::NT, AS::col_smem, st, A.pdl, A, *static_cast<const CUtensorMap*>(tensor_map));
+        }
+        return cudaErrorInvalidValue;
+    }
+    static cudaError_t row_inv2_cgf(const void* args, const void* tensor_map, cudaStream_t st) {
+        if constexpr (SL) {
+            const RowInvArgs<T>& A = *static_cast<const RowInvArgs<T>*>(args);
+            return launch(row_inv2_kernel<T, P, C_INV, 2>, pgrid(A.nsm, C_INV), AS::INV_THREADS, AS::inv_smem, st, A.pdl, A,
+                          *static_cast<const CUtensorMap*>(tensor_map));
         }
         return cudaErrorInvalidValue;
     }
     static cudaError_t row_inv2_pre(const void* args, const void* tensor_map, cudaStream_t st) {
         if constexpr (V2) {
             const RowInvArgs<T>& A = *static_cast<const RowInvArgs<T>*>(args);
-            return launch(row_inv2_kernel<T, P, C_INV, true>, pgrid(A.nsm, C_INV), AS::INV_THREADS, AS::inv_smem, st, A.pdl, A,
+            return launch(row_inv2_kernel<T, P, C_INV, 1>, pgrid(A.nsm, C_INV), AS::INV_THREADS, AS::inv_smem, st, A.pdl, A,
                           *static_cast<const CUtensorMap*>(tensor_map));
         }
         return cudaErrorInvalidValue;
@@ -205,6 +223,7 @@ template <typename T> struct Inst {
         t.v2_ctas[0] = C_FWD; t.v2_ctas[1] = C_COL; t.v2_ctas[2] = C_INV;
         t.v2_smem[0] = AS::fwd_smem; t.v2_smem[1] = AS::col_smem; t.v2_smem[2] = AS::inv_smem;
         t.row_fwd2 = &row_fwd2; t.col2 = &col2; t.row_inv2 = &row_inv2; t.row_fwd2_rupd = &row_fwd2_rupd; t.row_inv2_pre = &row_inv2_pre;
+        t.sl_ok = SL ? 1 : 0; t.col2_energy = &col2_energy; t.row_inv2_cgf = &row_inv2_cgf;
         t.col2_xform = &col2_xform; t.t2_export = &t2_export; t.t2_import = &t2_import;
         t.fused = FS::valid ? 1 : 0; t.fused_grid = FS::G; t.fused_solve = &fused_solve;
         t.init = &init; t.row_fwd = &row_fwd; t.col = &col; t.row_inv = &row_inv; t.spectrum_prep = &spectrum_prep;

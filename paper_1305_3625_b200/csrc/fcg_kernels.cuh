@@ -96,15 +96,30 @@ __global__ void __launch_bounds__(COLS * P::NT) col_kernel(const ColArgs<T> A) {
     col_body<T, P, COLS>(A, (int)blockIdx.x, reinterpret_cast<cx<T>*>(smem_raw), run);
 }
 
+// scalar step after the residue length r.r is known (PAPER.md:97-99): count, convergence / maxit, beta.
+// PCG keeps rho = r.z: there beta follows from the preconditioner pass (row_inv_reduce_finalize, ROWI_PRECOND).
+__device__ __forceinline__ void cg_after_rr(Scalars* sc, double rho_new) {
+    const double fn2 = sc->fn2;
+    const int it = sc->it + 1;
+    sc->it = it;
+    if (sqrt(rho_new) <= sc->tol * sqrt(fn2)) { sc->done = 1; sc->status = ST_OK; }
+    else if (it >= sc->maxit) { sc->done = 1; sc->status = ST_NOT_CONVERGED; }
+    else if (!sc->pcg) sc->beta = rho_new / sc->rho;
+    if (sc->pcg) sc->rr = rho_new; else sc->rho = rho_new;
+    sc->relres = sqrt(rho_new) / sqrt(fn2);
+    set_cond(sc, !sc->done);
+}
+
 // Grid-wide reduction of the row pass's partial dot products and the scalar step that follows it:
 // search length alpha = rho / p.Ap in the loop, or the initial values after the residual pass.
 template <typename T>
 __device__ __forceinline__ void row_inv_reduce_finalize(const RowInvArgs<T>& A, double (&acc)[2], double* red) {
-    if (A.mode != ROWI_CG && A.mode != ROWI_RESID && A.mode != ROWI_PRECOND) return;
+    if (A.mode != ROWI_CG && A.mode != ROWI_RESID && A.mode != ROWI_PRECOND && A.mode != ROWI_CGF) return;
     double tot[2];
     if (!grid_sum_last<2>(acc, A.partial, &A.sc->ticket[0], red, tot)) return;
     if (threadIdx.x != 0) return;
     Scalars* sc = A.sc;
+    if (A.mode == ROWI_CGF) { cg_after_rr(sc, tot[0]); return; }           // fused residual update: r.r is this pass's sum
     if (A.mode == ROWI_CG) {
         const double pq = tot[0];
         sc->pq = pq;
@@ -164,6 +179,7 @@ __global__ void cg_setup_kernel(Scalars* sc, SetupArgs a) {
         sc->tol = a.tol; sc->maxit = a.maxit; sc->it = 0; sc->done = 0; sc->status = 0; sc->zero_u = 0;
         sc->use_cond = a.use_cond; sc->cond = a.cond; sc->pcg = a.pcg; sc->rr = 0;
         sc->ticket[0] = sc->ticket[1] = sc->ticket[2] = sc->ticket[3] = 0u;
+        sc->kpp = 0; sc->ticket2[0] = sc->ticket2[1] = 0u;
     }
 }
 #endif
@@ -180,20 +196,6 @@ __device__ __forceinline__ void axpy_sq(float4& r, const float4 q, float a, doub
     r.x = r.x - a * q.x; r.y = r.y - a * q.y; r.z = r.z - a * q.z; r.w = r.w - a * q.w;
     acc += (double)r.x * (double)r.x; acc += (double)r.y * (double)r.y;
     acc += (double)r.z * (double)r.z; acc += (double)r.w * (double)r.w;
-}
-
-// scalar step after the residue length r.r is known (PAPER.md:97-99): count, convergence / maxit, beta.
-// PCG keeps rho = r.z: there beta follows from the preconditioner pass (row_inv_reduce_finalize, ROWI_PRECOND).
-__device__ __forceinline__ void cg_after_rr(Scalars* sc, double rho_new) {
-    const double fn2 = sc->fn2;
-    const int it = sc->it + 1;
-    sc->it = it;
-    if (sqrt(rho_new) <= sc->tol * sqrt(fn2)) { sc->done = 1; sc->status = ST_OK; }
-    else if (it >= sc->maxit) { sc->done = 1; sc->status = ST_NOT_CONVERGED; }
-    else if (!sc->pcg) sc->beta = rho_new / sc->rho;
-    if (sc->pcg) sc->rr = rho_new; else sc->rho = rho_new;
-    sc->relres = sqrt(rho_new) / sqrt(fn2);
-    set_cond(sc, !sc->done);
 }
 
 // residue, residue length (97), update calculation variables (98: beta), check convergence (99)
@@ -234,6 +236,26 @@ __global__ void __launch_bounds__(256) cg_update_r_kernel(T* __restrict__ r, con
     if (!grid_sum_last<1>(acc, partial, &sc->ticket[1], red, tot)) return;
     if (threadIdx.x != 0) return;
     cg_after_rr(sc, tot[0]);
+}
+
+// spectral search length: start value of the recurrence for sum k p^2 -- the first direction is p = r
+template <typename T>
+__global__ void __launch_bounds__(256) cg_kpp0_kernel(const T* __restrict__ k, const T* __restrict__ r, size_t nvec, double* partial, Scalars* sc) {
+    __shared__ double red[32];
+    using V = typename Vec<T>::type;
+    if (sc->done) return;
+    double acc[1] = {0.0};
+    const V* kv = reinterpret_cast<const V*>(k);
+    const V* rv = reinterpret_cast<const V*>(r);
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < nvec; i += (size_t)gridDim.x * blockDim.x) {
+        const V a = __ldg(kv + i), b = __ldg(rv + i);
+        const T* as = reinterpret_cast<const T*>(&a); const T* bs = reinterpret_cast<const T*>(&b);
+#pragma unroll
+        for (int c = 0; c < Vec<T>::W; ++c) acc[0] += (double)as[c] * ((double)bs[c] * (double)bs[c]);
+    }
+    double tot[1];
+    if (!grid_sum_last<1>(acc, partial, &sc->ticket2[0], red, tot)) return;
+    if (threadIdx.x == 0) sc->kpp = tot[0];
 }
 
 // last lagged "new x" after the loop has ended; u = 0 when f = 0

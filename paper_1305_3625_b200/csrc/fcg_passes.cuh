@@ -31,10 +31,12 @@ struct Scalars {
     int steps_done, pad_;          // fused quasi-static loop: completed break steps
     int pcg, pad2_;                // 1: preconditioned CG (rho = r.z, rr = r.r kept apart)
     double rr;                     // PCG: r.r of the current residual
+    double kpp;                    // spectral search length: sum k p^2 from P1; P2 adds sum shat |P|^2
+    unsigned int ticket2[2];       // [0] P1's k p^2 reduction, [1] P2's spectral-energy reduction
 };
 
 enum { ROWF_PLAIN = 0, ROWF_CG = 1, ROWF_RUPD = 2 };   // RUPD (PCG): r -= alpha q, partial r.r, row transforms of r
-enum { ROWI_PLAIN = 0, ROWI_CG = 1, ROWI_RESID = 2, ROWI_APPLY = 3, ROWI_PRECOND = 4 };   // PRECOND (PCG): z = M^-1 r, partial r.z (k = r)
+enum { ROWI_PLAIN = 0, ROWI_CG = 1, ROWI_RESID = 2, ROWI_APPLY = 3, ROWI_PRECOND = 4, ROWI_CGF = 5 };   // PRECOND (PCG): z = M^-1 r, partial r.z (k = r)
 enum { COL_CONV = 0, COL_FWD = 1, COL_INV = 2 };
 
 template <typename T> struct RowFwdArgs {
@@ -61,6 +63,7 @@ template <typename T> struct ColArgs {
     const Scalars* sc;
     int pdl;
     int hints;
+    double* partial;       // ENERGY instantiation: [gridDim.x] partial sums of shat |P|^2
 };
 
 template <typename T> struct RowInvArgs {
@@ -75,6 +78,7 @@ template <typename T> struct RowInvArgs {
     int nsm;
     int pdl;
     int hints;
+    const double* colsum;                 // CGF: the column pass's L/2 partial sums of shat |P|^2
 };
 
 template <int A, int B, typename F> FCG_HD void static_for_up(F&& f) {

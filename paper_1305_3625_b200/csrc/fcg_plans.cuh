@@ -67,6 +67,11 @@ struct PassTable {
     cudaError_t (*row_fwd2)(const void* args, cudaStream_t st);
     cudaError_t (*col2)(const void* args, const void* tensor_map, cudaStream_t st);
     cudaError_t (*row_inv2)(const void* args, const void* tensor_map, cudaStream_t st);
+    // spectral search length: P2 with the spectral energy, P3 with alpha and the residual update fused
+    // (q never stored); sl_ok == 0 when the size has no such instantiation
+    int sl_ok;
+    cudaError_t (*col2_energy)(const void* args, const void* tensor_map, cudaStream_t st);
+    cudaError_t (*row_inv2_cgf)(const void* args, const void* tensor_map, cudaStream_t st);
     cudaError_t (*row_fwd2_rupd)(const void* args, cudaStream_t st);                                // PCG: r update + r.r + row transforms of r
     cudaError_t (*row_inv2_pre)(const void* args, const void* tensor_map, cudaStream_t st);        // PCG: z = M^-1 r, r.z
     cudaError_t (*col2_xform)(const void* args, const void* tensor_map, int inverse, cudaStream_t st);   // stand-alone transforms

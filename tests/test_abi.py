@@ -38,7 +38,7 @@ def test_workspace_bytes(lib):
         for L in (16, 64, 2048, 8192):
             n = lib.fcg_workspace_bytes(L, dt)
             N = L * L
-            assert 6 * N * w <= n <= 6 * N * w + 64 * L * w + 64 * 1024     # T (1) + shat, mhat (1/2 each) + r,p,q,z (4), + tables
+            assert 6 * N * w <= n <= 6 * N * w + 72 * L * w + 64 * 1024     # T (1) + shat, mhat (1/2 each) + r,p,q,z (4), + tables
     for L in (0, 8, 24, 100, 16384, -4):
         assert lib.fcg_workspace_bytes(L, 1) == 0
     assert lib.fcg_workspace_bytes(64, 7) == 0

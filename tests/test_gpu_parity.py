@@ -171,7 +171,8 @@ def cg_parity(B, w, **opts):
     assert st == ref["status"]
     assert abs(it - ref["iters"]) <= 2, (it, ref["iters"], ref["hist"][-4:])
     # graph path: set-up 4 + finish 1 + 4 kernels x (iterations rounded up to the WHILE body's 4); fused path (L = 256, 512): 1
-    assert h.fcg_last_launch_count() in (1, 5 + 16 * ((it + 3) // 4)) or opts
+    # spectral search length (default): set-up 5 + finish 1 + 3 kernels x ...
+    assert h.fcg_last_launch_count() in (1, 5 + 16 * ((it + 3) // 4), 6 + 12 * ((it + 3) // 4)) or opts
     u_nat = u.cpu().numpy()
     d_nat = rel(u_nat, ref["u"])
     d_pin = d_nat
@@ -255,7 +256,7 @@ def test_cg_fused_kernel(B, cfg, L):
         h = handle(B, L, np.float64, w.s, FCG_OPT_FUSED=fused)
         u = dev(w.u0)
         it, rr, st = h.fcg_solve(dev(w.k), dev(w.f), u, w.tol, w.maxit)
-        assert st == 0 and h.fcg_last_launch_count() == (1 if fused else 5 + 16 * ((it + 3) // 4))
+        assert st == 0 and h.fcg_last_launch_count() == (1 if fused else 6 + 12 * ((it + 3) // 4))
         us.append((it, u.cpu().numpy()))
         h.close()
     assert us[0][0] == us[1][0] and np.array_equal(us[0][1], us[1][1])          # repeatable
@@ -315,6 +316,29 @@ def test_cg_solve_host_matches_device(B):
     assert h.fcg_solve_host(kh, fh, uh, w.tol, w.maxit) == (it, rr, st)
     assert np.array_equal(uh.numpy(), u.cpu().numpy())
     h.close()
+
+
+@pytest.mark.parametrize("cfg,L,dt", [(0, 64, np.float64), (1, 256, np.float64), (1, 512, np.float64), (2, 1024, np.float64),
+                                      (2, 1024, np.float32), (4, 512, np.float32), (4, 1024, np.float32)])
+def test_cg_both_search_length_evaluations(B, cfg, L, dt):
+    """fcg_solve with p.Ap as a dot product after the last pass (4 launches per iteration, FCG_OPT_SPECTRAL_ALPHA = 0) and as
+    sum k p^2 + sum shat |P|^2 known before it (3 launches, default): both against the oracle, and
+    against each other to rounding (same iteration count or +-1, u to 100x the working precision's resolution of the solve)."""
+    w = inputs.config(cfg, dt, L=L)
+    outs = []
+    for sl in (0, 1):
+        it, it_or = cg_parity(B, w, FCG_OPT_FUSED=0, FCG_OPT_SPECTRAL_ALPHA=sl)
+        h = handle(B, L, dt, w.s, FCG_OPT_FUSED=0, FCG_OPT_SPECTRAL_ALPHA=sl)
+        u = dev(w.u0)
+        r = h.fcg_solve(dev(w.k), dev(w.f), u, 0.0, it_or)          # pinned count
+        c = (it_or + 3) // 4                                        # the classic engine (small transforms) always takes 4 launches
+        assert h.fcg_last_launch_count() == 5 + 16 * c or (sl == 1 and h.fcg_last_launch_count() == 6 + 12 * c)
+        if sl == 1 and (L >= 1024 or dt == np.float64 and L >= 256):
+            assert h.fcg_last_launch_count() == 6 + 12 * c
+        outs.append((it, r, u.cpu().numpy()))
+        h.close()
+    assert abs(outs[0][0] - outs[1][0]) <= 1
+    assert rel(outs[0][2], outs[1][2]) <= (1e-10 if dt == np.float64 else 2e-5)
 
 
 # ------------------------------------------------------------------------------------ full-size configs
