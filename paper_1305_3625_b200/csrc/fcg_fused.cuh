@@ -8,8 +8,10 @@
 //     between the row and the column transforms) goes through global memory, i.e. through L2;
 //   * preconditioned CG (A.mhat != nullptr): z = M^-1 r is one more operator-shaped round trip per iteration (rows of r ->
 //     columns with the preconditioner's spectrum -> rows of z, r.z), three more grid barriers; z lives in q's slot;
-//   * per iteration four grid barriers (an atomic counter in global memory): T complete -> columns done -> p.q known ->
-//     r.r known.  Every CTA adds the G partial sums itself, in the same fixed order, so alpha, beta and the convergence
+//   * per iteration THREE grid barriers (an atomic counter in global memory): T complete -> columns done -> r.r known.  The
+//     search length needs no barrier of its own: p.Ap = sum k p^2 (formed with the new direction, in shared memory) + sum shat |P|^2
+//     (accumulated in the column phase), published before the "columns done" barrier and added up by
+//     every CTA after it, so u and r are updated in the epilogue of the inverse row transforms and q is never stored.  Every CTA adds the G partial sums itself, in the same fixed order, so alpha, beta and the convergence
 //     decision are bit-identical in all CTAs and no CTA ever waits for a broadcast;
 //   * same stage arithmetic as the pipelined passes (fcg_engine.cuh: register twiddle powers, swizzled work buffer) and the
 //     same column numbering / stored spectrum as them (AsyncShape, colpos layout), so fcg_set_spectrum is shared.
@@ -181,7 +183,7 @@ __global__ void __launch_bounds__(P::NT) cg_fused_kernel(const FusedArgs A)
         }
     };
     // phase C: own columns, in place: forward, spectral multiply, inverse
-    auto columns = [&](const T* spec) {
+    auto columns = [&](const T* spec, double* en) {      // en != nullptr: *en += this CTA's share of sum spec |P|^2
         for (int j = 0; j < TPC; ++j) {
             const int m = cta + j * G;
             cx<T>* col = Tf + (size_t)m * L;
@@ -214,7 +216,13 @@ __global__ void __launch_bounds__(P::NT) cg_fused_kernel(const FusedArgs A)
             if (m != 0) {
                 const T* sh = spec + (size_t)m * L;
                 static_for_up<2, S - 1>(fwd_stage);
-                run_middle<P, T>(lt, ld_sw, st_sw, [&](int g, int u) { return sh[u * (L / P::RLAST) + g]; });
+                if (en) {
+                    double e2 = 0.0;
+                    run_middle<P, T, true>(lt, ld_sw, st_sw, [&](int g, int u) { return sh[u * (L / P::RLAST) + g]; }, &e2);
+                    *en += 2.0 * e2;                                 // column m stands for frequencies n and L - n
+                } else {
+                    run_middle<P, T>(lt, ld_sw, st_sw, [&](int g, int u) { return sh[u * (L / P::RLAST) + g]; });
+                }
                 __syncthreads();
                 static_for_down<S - 1, 2>(inv_stage);
             } else {     // packed n = 0 / L/2 column (see col2_kernel)
@@ -228,6 +236,13 @@ __global__ void __launch_bounds__(P::NT) cg_fused_kernel(const FusedArgs A)
                     const int i1 = P::shat_index(e), i2 = P::shat_index(e2);
                     va.x = sp_[i1] * Wa.x + sm_[i1] * Wb.x; va.y = sp_[i1] * Wa.y - sm_[i1] * Wb.y;
                     vb.x = sp_[i2] * Wb.x + sm_[i2] * Wa.x; vb.y = sp_[i2] * Wb.y - sm_[i2] * Wa.y;
+                    if (en) {        // s0 |Y0|^2 + sN |YN|^2 at mm (and again at -mm), see col2_kernel
+                        const double na = (double)Wa.x * (double)Wa.x + (double)Wa.y * (double)Wa.y;
+                        const double nb = (double)Wb.x * (double)Wb.x + (double)Wb.y * (double)Wb.y;
+                        const double re = (double)Wa.x * (double)Wb.x - (double)Wa.y * (double)Wb.y;
+                        const double term = 0.5 * (double)sp_[i1] * (na + nb) + (double)sm_[i1] * re;
+                        *en += e2 != e ? 2.0 * term : term;
+                    }
                     io.st(e, va);
                     if (e2 != e) io.st(e2, vb);
                 }
@@ -296,9 +311,9 @@ __global__ void __launch_bounds__(P::NT) cg_fused_kernel(const FusedArgs A)
     // One solve is a small state machine, so that every phase of the operator-shaped round trip (rows -> columns -> rows) and the
     // grid-wide sum exist ONCE in the instruction stream (with several call sites the compiler stops inlining them: 64 registers,
     // a stack frame, and 17.7 instead of 12.4 us per iteration at L = 256):
-    //   FN (once per launch: ||f||^2) -> RESID (r = f - A u, r.r) -> [Z (z = M^-1 r, r.z)] -> Q (p, q = A p, p.q) -> RR (u, r, r.r)
-    //   -> [Z] -> Q -> RR -> ..          Z only for preconditioned CG; z lives in q's slot (q is dead once r has been updated).
-    enum { PH_FN = 0, PH_RESID = 1, PH_Z = 2, PH_Q = 3, PH_RR = 4 };
+    //   FN (once per launch: ||f||^2) -> RESID (r = f - A u, r.r) -> [Z (z = M^-1 r, r.z)] -> Q (p, A p, alpha, u, r, r.r) -> [Z] -> Q -> ..
+    // Z only for preconditioned CG; z lives in the slot that used to hold q (q is consumed as it is formed).
+    enum { PH_FN = 0, PH_RESID = 1, PH_Z = 2, PH_Q = 3 };
     bool ok = true, okb = true, have_fn = false;
     int it = 0, status = ST_OK, steps_done = 0;
     double rho = 0.0, fn2 = 0.0, rr = 0.0;         // rho = r.r (CG) or r.z (PCG); rr = r.r
@@ -313,60 +328,72 @@ __global__ void __launch_bounds__(P::NT) cg_fused_kernel(const FusedArgs A)
             for (int e = lt; e < 2 * L; e += NT) pp[e] = (T)0;
         }
         it = 0; status = ST_OK; zero_u = false;
-        double beta = 0.0, alpha = 0.0;
+        double beta = 0.0;
         int phase = have_fn ? PH_RESID : PH_FN;
         while (true) {
-            double acc = 0.0;
+            double acc = 0.0, kpp = 0.0;
+            bool bd = false;
             // ---- vector work of this phase on the CTA's own rows
             if (phase == PH_FN) {
                 for (int j = 0; j < TPC; ++j) {
                     const T* ff = V(j, 1, 0);
                     for (int e = lt; e < 2 * L; e += NT) acc += (double)ff[e] * (double)ff[e];
                 }
-            } else if (phase == PH_Q) {                                       // update calculation variables: new direction (98)
+            } else if (phase == PH_Q) {                 // update calculation variables: new direction (98); sum k p^2 on the way
                 for (int j = 0; j < TPC; ++j) {
-                    const T* dv = V(j, pcg ? 5 : 3, 0); T* pp = V(j, 4, 0);      // r, or z = M^-1 r
+                    const T* dv = V(j, pcg ? 5 : 3, 0); T* pp = V(j, 4, 0); const T* kk = V(j, 0, 0);     // r, or z = M^-1 r
                     const T b = (T)beta;
-                    for (int e = lt; e < 2 * L; e += NT) pp[e] = dv[e] + b * pp[e];
-                }
-                __syncthreads();
-            } else if (phase == PH_RR) {                                      // new x (95), residue (96), residue length (97)
-                const T al = (T)alpha;
-                for (int j = 0; j < TPC; ++j) {
-                    T* uu = V(j, 2, 0); T* rv = V(j, 3, 0); const T* pp = V(j, 4, 0); const T* qq = V(j, 5, 0);
                     for (int e = lt; e < 2 * L; e += NT) {
-                        uu[e] = uu[e] + al * pp[e];
-                        const T rn = rv[e] - al * qq[e];
-                        rv[e] = rn;
-                        acc += (double)rn * (double)rn;
+                        const T pn = dv[e] + b * pp[e];
+                        pp[e] = pn;
+                        kpp += (double)kk[e] * ((double)pn * (double)pn);
                     }
                 }
+                __syncthreads();
             }
             // ---- operator-shaped round trip: C u (RESID), C p (Q: A * p) or M^-1 r (Z)
-            if (phase == PH_RESID || phase == PH_Z || phase == PH_Q) {
+            if (phase != PH_FN) {
                 rows_forward(phase == PH_RESID ? 2 : (phase == PH_Q ? 4 : 3));
                 ok = grid_barrier(A.counter, target, G, &ok_smem) && ok;
-                columns(phase == PH_Z ? mhat : shat);
+                double en = 0.0;
+                columns(phase == PH_Z ? mhat : shat, phase == PH_Q ? &en : nullptr);
+                double* ps = A.partial + (size_t)slot * G;
+                if (phase == PH_Q) {                    // this CTA's share of p.Ap = sum k p^2 + sum shat |P|^2, published before the barrier
+                    const double mine = cta_sum(kpp + en);
+                    if (lt == 0) ps[cta] = mine;
+                }
                 ok = grid_barrier(A.counter, target, G, &ok_smem) && ok;
-                rows_inverse([&](int j, int e, T c0, T c1) {
+                T al = (T)0;
+                if (phase == PH_Q) {                    // search length (94): every CTA adds the G shares in the same order
+                    double v = 0.0;
+                    for (int i = lt; i < G; i += NT) v += __ldcg(ps + i);
+                    slot = (slot + 1) & 3;
+                    const double pq = cta_sum(v);
+                    if (!(pq > 0.0) || !isfinite(pq)) bd = true;
+                    else al = (T)(rho / pq);
+                }
+                if (!bd) rows_inverse([&](int j, int e, T c0, T c1) {
                     if (phase == PH_RESID) {                                  // r = f - (k o u + C u)
                         const T* kk = V(j, 0, 0); const T* ff = V(j, 1, 0); const T* uu = V(j, 2, 0); T* rv = V(j, 3, 0);
                         const T r0 = ff[e] - (kk[e] * uu[e] + c0), r1 = ff[L + e] - (kk[L + e] * uu[L + e] + c1);
                         rv[e] = r0; rv[L + e] = r1;
                         acc += (double)r0 * (double)r0; acc += (double)r1 * (double)r1;
-                    } else if (phase == PH_Q) {                               // q = k o p + C p, p.q
-                        const T* kk = V(j, 0, 0); const T* pp = V(j, 4, 0); T* qq = V(j, 5, 0);
+                    } else if (phase == PH_Q) {         // q = k o p + C p; new x (95), residue (96), residue length (97)
+                        const T* kk = V(j, 0, 0); const T* pp = V(j, 4, 0); T* uu = V(j, 2, 0); T* rv = V(j, 3, 0);
                         const T p0 = pp[e], p1 = pp[L + e];
                         const T q0 = kk[e] * p0 + c0, q1 = kk[L + e] * p1 + c1;
-                        qq[e] = q0; qq[L + e] = q1;
-                        acc += (double)p0 * (double)q0; acc += (double)p1 * (double)q1;
-                    } else {                                                  // z = M^-1 r (into q's slot), r.z
+                        uu[e] = uu[e] + al * p0; uu[L + e] = uu[L + e] + al * p1;
+                        const T r0 = rv[e] - al * q0, r1 = rv[L + e] - al * q1;
+                        rv[e] = r0; rv[L + e] = r1;
+                        acc += (double)r0 * (double)r0; acc += (double)r1 * (double)r1;
+                    } else {                                                  // z = M^-1 r, r.z
                         const T* rv = V(j, 3, 0); T* zz = V(j, 5, 0);
                         zz[e] = c0; zz[L + e] = c1;
                         acc += (double)rv[e] * (double)c0; acc += (double)rv[L + e] * (double)c1;
                     }
                 });
             }
+            if (bd) { status = ST_BREAKDOWN; break; }
             const double s0 = grid_sum(acc, okb); ok = ok && okb;
             if (!ok) { status = -3; break; }
             // ---- scalar step, identical in every CTA
@@ -381,15 +408,12 @@ __global__ void __launch_bounds__(P::NT) cg_fused_kernel(const FusedArgs A)
                 if (!(s0 > 0.0) || !isfinite(s0)) { status = ST_BREAKDOWN; break; }
                 beta = it == 0 ? 0.0 : s0 / rho;
                 rho = s0; phase = PH_Q;
-            } else if (phase == PH_Q) {                                       // search length (94)
-                if (!(s0 > 0.0) || !isfinite(s0)) { status = ST_BREAKDOWN; break; }
-                alpha = rho / s0; phase = PH_RR;
             } else {
                 rr = s0; ++it;
                 if (sqrt(rr) <= A.tol * sqrt(fn2)) { if (!pcg) rho = rr; break; }                 // check convergence (99)
                 if (it >= A.maxit) { if (!pcg) rho = rr; status = ST_NOT_CONVERGED; break; }
                 if (pcg) phase = PH_Z;
-                else { beta = rr / rho; rho = rr; phase = PH_Q; }
+                else { beta = rr / rho; rho = rr; }
             }
         }
         __syncthreads();
