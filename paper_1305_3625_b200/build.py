@@ -17,7 +17,7 @@ LIB = os.path.join(HERE, "libfcg.so")
 SIZES = [16, 32, 64, 128, 256, 512, 1024, 2048, 4096, 8192]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
-         "--expt-relaxed-constexpr", "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
+         "--expt-relaxed-constexpr", "-Xcompiler", "-fPIC", "-Xptxas", "-v"] + os.environ.get("FCG_EXTRA_FLAGS", "").split()
 
 
 def _sources():

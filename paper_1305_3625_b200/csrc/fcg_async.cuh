@@ -568,14 +568,15 @@ __global__ void __launch_bounds__(AsyncShape<T, P>::INV_THREADS, CTAS) row_inv2_
     constexpr bool PRE = VAR == 1, CGF = VAR == 2;
     constexpr int TSUB = AS::TSUB, NSUB = AS::NSUB;
     constexpr uint32_t TBYTES = (uint32_t)AS::TSB;
-    // CGF moves three vectors of strips per transform against one of tiles: its strips are NT elements long (SPT of them per
-    // stage-1 strip), the tile ring holds one transform (NSUB tiles) if that leaves two strip slots, and the strips get the rest
+    // CGF moves three vectors of strips per transform against one of tiles: the tile ring is kept short (TCAP) and the strips
+    // get the rest; where whole stage-1 strips would leave too few slots they are NT elements long (SPT of them per stage-1 strip)
     // (whole stage-1 strips where three slots of those fit beside two tiles: 512-byte pieces cost more than they bring)
     constexpr bool FINE = CGF && (AS::RING_BUDGET - 2 * AS::TSB) / (6 * (size_t)AS::PIECE) < 3;
     constexpr int SPT = FINE ? PER1 : 1, QV = FINE ? NT : Q1;
     constexpr uint32_t PIECE = (uint32_t)(QV * sizeof(T));
     constexpr int NTSF_ = (int)((AS::RING_BUDGET - 12 * (size_t)PIECE) / AS::TSB);
-    constexpr int NTS = CGF ? (NTSF_ < 2 ? 2 : (NTSF_ > NSUB ? NSUB : NTSF_)) : AS::NTS;
+    constexpr int TCAP = (int)(20480 / AS::TSB) < 2 ? 2 : (int)(20480 / AS::TSB);     // ~20 KB of tiles in flight (measured: 2 x 8 KB at L = 2048 fp64, 5 x 4 KB at L = 8192 fp32)
+    constexpr int NTS = CGF ? (NTSF_ < 2 ? 2 : (NTSF_ > TCAP ? TCAP : NTSF_)) : AS::NTS;
     constexpr size_t KRB = CGF ? AS::RING_BUDGET - (size_t)NTS * AS::TSB : AS::KRB;
     static_assert(NTS <= AS::MAXSLOT && KRB >= 6 * (size_t)PIECE, "P3 rings");
     extern __shared__ unsigned char smem_dyn[];
