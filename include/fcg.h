@@ -73,6 +73,9 @@ typedef enum {
                                  last pass and r -= alpha q, r.r ride in it: 3 launches and 13.5 N w bytes per iteration, q never
                                  stored (pipelined engine).  0: p.q as a dot product after the last pass and a
                                  fourth kernel for the residual update (15.5 N w) */
+    FCG_OPT_COL_PERSISTENT = 9, /* 1: column pass as persistent CTAs with two column buffers each, the next column's gather in flight
+                                 while the current one is transformed (sizes where two buffers fit twice per SM); 0: one CTA per column;
+                                 -1 (default): persistent for FCG_F32 and for L <= 1024, where it measured faster */
     FCG_OPT_ENGINE       = 3  /* 0 (default): pipelined TMA passes where the lattice is large enough (L >= 256), classic
                                  passes otherwise; 1: classic passes only (synchronous loads; kept for A/B measurements).
                                  The stored spectrum's layout belongs to the engine: changing the engine after

@@ -20,6 +20,7 @@ FCG_INVALID_ARG, FCG_UNSUPPORTED, FCG_CUDA_ERROR, FCG_BREAKDOWN, FCG_NO_SPECTRUM
 FCG_OPT_LOOP_MODE, FCG_OPT_CHUNK, FCG_OPT_ROW_VARIANT, FCG_OPT_ENGINE, FCG_OPT_UNROLL, FCG_OPT_PDL, FCG_OPT_FUSED = 0, 1, 2, 3, 4, 5, 6
 FCG_OPT_L2_HINTS = 7
 FCG_OPT_SPECTRAL_ALPHA = 8
+FCG_OPT_COL_PERSISTENT = 9
 
 EXPORTS = ["fcg_workspace_bytes", "fcg_create", "fcg_destroy", "fcg_set_option", "fcg_set_spectrum", "fcg_apply",
            "fcg_solve", "fcg_solve_host", "fcg_profile_iteration", "fcg_fft_fwd", "fcg_fft_inv", "fcg_break_step", "fcg_fracture",

@@ -78,12 +78,15 @@ struct fcg_handle_s {
     char* ws = nullptr; bool own_ws = false;
     Layout lay{};
     bool have_spectrum = false, have_precond = false;
-    int loop_mode = 0, chunk = 16, row_var_opt = -1, engine_opt = 0, nsm = 148, unroll = 4, pdl = 0, fused_opt = 1, hints = 63, sl_opt = 1;
+    int loop_mode = 0, chunk = 16, row_var_opt = -1, engine_opt = 0, nsm = 148, unroll = 4, pdl = 0, fused_opt = 1, hints = 63, sl_opt = 1, colp_opt = -1;
     alignas(64) CUtensorMap tmap_row;   // T2 as [L/(2 NB)][L/2][128 B]: box = v2_tsub/NB lines of one row pair (row_inv2 tiles)
     alignas(64) CUtensorMap tmap_col;   // T2 as [L/(2 NB)][L/2][NB][2 complex]: box = one column x v2_abox row pairs (col2 gather / scatter)
     bool have_tmap = false;
     int spectrum_colpos = 0;            // layout the stored spectrum was prepared for (1: T2 column order)
     bool v2() const { return engine_opt == 0 && tab->v2 && have_tmap; }
+    // persistent column pass: measured faster for fp32 (L = 2048: 23.2 -> 20.6 us, L = 4096: 59.1 -> 53.1) and for fp64 up to
+    // L = 1024; slower at L = 2048 fp64 (two CTAs of 4 warps per SM instead of three: 26.5 -> 31.0 us), hence the automatic rule
+    bool colp() const { return tab->colp_ok && (colp_opt < 0 ? (dtype == FCG_F32 || L <= 1024) : colp_opt != 0); }
     bool sl() const { return sl_opt && v2() && tab->sl_ok; }     // spectral search length: 3 launches per CG iteration
     bool fused() const { return fused_opt && tab->fused && v2() && loop_mode == 0; }   // whole solve in one cooperative kernel
     Scalars* h_sc = nullptr;            // pinned
@@ -158,7 +161,9 @@ template <typename T> struct Seq {
     }
     cudaError_t col(int mode, bool cg, bool precond = false) const {
         ColArgs<T> A{}; A.mode = mode; A.Tb = Tb(); A.shat = precond ? mhat() : shat(); A.hints = h->hints; A.tw = tw(); A.sc = cg ? h->sc() : nullptr; A.pdl = h->pdl;
+        A.nsm = h->nsm;
         ++h->launches;
+        if (v2() && mode == COL_CONV && h->colp()) return h->tab->col2p(&A, &h->tmap_col, 0, st);
         return (v2() && mode == COL_CONV) ? h->tab->col2(&A, &h->tmap_col, st) : h->tab->col(&A, st);
     }
     cudaError_t row_inv(int mode, const T* k, const T* v, const T* f, T* out, T* out2) const {
@@ -231,8 +236,9 @@ template <typename T> struct Seq {
     // spectral search length: alpha is known after the column pass, so the residual update rides in P3
     cudaError_t it_col_e() const {
         ColArgs<T> A{}; A.mode = COL_CONV; A.Tb = Tb(); A.shat = shat(); A.hints = h->hints; A.tw = tw(); A.sc = h->sc(); A.pdl = h->pdl;
-        A.partial = h->at<double>(h->lay.partial_col);
+        A.partial = h->at<double>(h->lay.partial_col); A.nsm = h->nsm;
         ++h->launches;
+        if (h->colp()) return h->tab->col2p(&A, &h->tmap_col, 1, st);
         return h->tab->col2_energy(&A, &h->tmap_col, st);
     }
     cudaError_t it_row_inv_f(const T* k) const {
@@ -351,14 +357,14 @@ int solve_impl(fcg_handle h, const void* k, const void* f, void* u, double tol, 
         const int var = h->v2() ? 100 + (h->sl() ? 1 : 0) : h->row_var();
         GraphEntry* hit = nullptr;
         for (auto& g : h->graphs)
-            if (g.k == k && g.f == f && g.u == u && g.tol == tol && g.maxit == maxit && g.var == var && g.unroll == h->unroll && g.pdl == h->pdl && g.pcg == (pcg ? 1 : 0) + 2 * h->hints) { hit = &g; break; }
+            if (g.k == k && g.f == f && g.u == u && g.tol == tol && g.maxit == maxit && g.var == var && g.unroll == h->unroll && g.pdl == h->pdl && g.pcg == (pcg ? 1 : 0) + 2 * h->hints + 256 * (h->colp() ? 1 : 0)) { hit = &g; break; }
         if (!hit) {
             if (h->graphs.size() >= 8) {
                 size_t lru = 0;
                 for (size_t i = 1; i < h->graphs.size(); ++i) if (h->graphs[i].stamp < h->graphs[lru].stamp) lru = i;
                 drop_graph(h->graphs[lru]); h->graphs.erase(h->graphs.begin() + lru);
             }
-            GraphEntry ge{k, f, u, tol, maxit, var, h->unroll, h->pdl, (pcg ? 1 : 0) + 2 * h->hints, nullptr, nullptr, 0};
+            GraphEntry ge{k, f, u, tol, maxit, var, h->unroll, h->pdl, (pcg ? 1 : 0) + 2 * h->hints + 256 * (h->colp() ? 1 : 0), nullptr, nullptr, 0};
             cudaError_t e = build_graph<T>(h, ge);
             if (e != cudaSuccess) {
                 // conditional graph nodes unavailable: fall back to direct launches for the rest of this handle's life
@@ -665,6 +671,7 @@ int fcg_set_option(fcg_handle h, int option, int value) {
         case FCG_OPT_PDL: if (value != 0 && value != 1) return fail(h, FCG_INVALID_ARG, "pdl must be 0 or 1"); h->pdl = value; return FCG_OK;
         case FCG_OPT_L2_HINTS: if (value < 0 || value > 63) return fail(h, FCG_INVALID_ARG, "hints must be 0..63"); h->hints = value; return FCG_OK;
         case FCG_OPT_SPECTRAL_ALPHA: if (value != 0 && value != 1) return fail(h, FCG_INVALID_ARG, "spectral alpha must be 0 or 1"); h->sl_opt = value; return FCG_OK;
+        case FCG_OPT_COL_PERSISTENT: if (value < -1 || value > 1) return fail(h, FCG_INVALID_ARG, "col persistent must be -1, 0 or 1"); h->colp_opt = value; return FCG_OK;
         case FCG_OPT_UNROLL: if (value < 1 || value > 64) return fail(h, FCG_INVALID_ARG, "unroll must be 1..64"); h->unroll = value; return FCG_OK;
         case FCG_OPT_ENGINE:
             if (value != 0 && value != 1) return fail(h, FCG_INVALID_ARG, "engine must be 0 or 1");

@@ -400,6 +400,171 @@ __global__ void __launch_bounds__(P::NT, CTAS) col2_kernel(const ColArgs<T> A, c
     if (lt == 0) tma::bulk_wait_read0();          // shared memory must outlive the store's read
 }
 
+// --------------------------------------------------------------------------------------------- P2, persistent
+// The same column pass with the gather of the NEXT column in flight while the current one is being transformed: grid = SMs x
+// CTAS persistent CTAs, two column buffers (column + spectrum row) per CTA, NT consumer threads + one producer warp whose lane 0
+// owns every asynchronous copy:   G(0) G(1) | ready(0) -> S(0) -> read of S(0) done -> G(2) | ready(1) -> S(1) -> G(3) | ..
+// (G = TMA gather of a column into its buffer, S = TMA scatter back).  col2_kernel leaves that overlap to the 3-6 CTAs that
+// share an SM and loses the gather latency (~2 us of ~8 us per column at L = 2048 fp64) whenever they fall into step.
+// Used where two buffers fit at least twice per SM (ColPShape::valid); otherwise col2_kernel.
+template <typename T, typename P> struct ColPShape {
+    using AS = AsyncShape<T, P>;
+    static constexpr size_t BUF = AS::WBYTES + (size_t)P::N * sizeof(T);
+    static constexpr size_t smem = 2 * BUF + 128;
+    static constexpr int by_smem = (int)((size_t)FCG_MAX_SMEM / (smem + 1024 + 512));
+    static constexpr int by_thr = AS::thread_cap / (P::NT + 32);
+    static constexpr int CTAS = by_smem < by_thr ? by_smem : by_thr;
+    static constexpr bool valid = AS::valid && CTAS >= 2;
+};
+
+template <typename T, typename P, int CTAS, bool ENERGY = false>
+__global__ void __launch_bounds__(P::NT + 32, CTAS) col2p_kernel(const ColArgs<T> A, const __grid_constant__ CUtensorMap tmap)
+{
+    using AS = AsyncShape<T, P>;
+    using CP = ColPShape<T, P>;
+    constexpr int L = P::N, S = P::S, NT = P::NT, PM = per_max<P>();
+    constexpr int ABOX = AS::ABOX;
+    constexpr uint32_t BOXB = (uint32_t)(ABOX * 2 * sizeof(cx<T>));
+    extern __shared__ unsigned char smem_dyn[];
+    unsigned char* const smem_raw = align128(smem_dyn);
+    __shared__ __align__(8) uint64_t full[2], ready[2];
+    __shared__ double red[32];
+    const int lt = threadIdx.x, lane = lt & 31, warp = lt >> 5;
+    int cnt = 0;
+    while ((int)blockIdx.x + cnt * (int)gridDim.x < L / 2) ++cnt;
+    auto col_of = [&](int i) { return (int)blockIdx.x + i * (int)gridDim.x; };
+    tma::grid_dep_launch();
+    if (lt == 0) {
+        tma::prefetch_tmap(&tmap);
+        for (int b = 0; b < 2; ++b) { tma::mbar_init(&full[b], 1); tma::mbar_init(&ready[b], NT / 32); }
+        tma::fence_mbar_init();
+    }
+    __syncthreads();
+    tma::grid_dep_wait();
+    if (A.sc && A.sc->done) return;                              // before any copy is issued
+
+    if (warp == NT / 32) {
+        if (lane == 0) {
+            const uint64_t pol = (A.hints & 4) ? tma::policy_evict_first() : tma::policy_evict_normal();   // spectrum rows: read once per iteration
+            auto gather = [&](int i) {
+                const int n = col_of(i), b = i & 1;
+                unsigned char* Wb = smem_raw + (size_t)b * CP::BUF;
+                tma::mbar_expect_tx(&full[b], (uint32_t)(AS::WBYTES + (n ? L * sizeof(T) : 0)));
+#pragma unroll
+                for (int q = 0; q < (L / 2) / ABOX; ++q)
+                    tma::tensor_g2s_4d(Wb + (size_t)q * BOXB, &tmap, 0, n % AS::NB, q * ABOX, n / AS::NB, &full[b]);
+                if (n) tma::bulk_g2s_hint(Wb + AS::WBYTES, A.shat + (size_t)n * L, (uint32_t)(L * sizeof(T)), &full[b], pol);
+            };
+            if (cnt > 0) gather(0);
+            if (cnt > 1) gather(1);
+            for (int i = 0; i < cnt; ++i) {
+                const int n = col_of(i), b = i & 1;
+                unsigned char* Wb = smem_raw + (size_t)b * CP::BUF;
+                tma::mbar_wait(&ready[b], (uint32_t)((i >> 1) & 1));          // every consumer warp's part of column i is in place
+#pragma unroll
+                for (int q = 0; q < (L / 2) / ABOX; ++q)
+                    tma::tensor_s2g_4d(&tmap, 0, n % AS::NB, q * ABOX, n / AS::NB, Wb + (size_t)q * BOXB);
+                tma::bulk_commit();
+                tma::bulk_wait_read0();                                        // the buffer may be refilled (or the CTA may exit)
+                if (i + 2 < cnt) gather(i + 2);
+            }
+        }
+        return;
+    }
+
+    // ---- consumers
+    cx<T> wb[S + 1][PM];
+    static_for_up<1, S - 1>([&](auto s) { base_tw<P, decltype(s)::value, T>(lt, A.tw, wb[decltype(s)::value]); });
+    for (int i = 0; i < cnt; ++i) {
+        const int n = col_of(i), b = i & 1;
+        cx<T>* W = reinterpret_cast<cx<T>*>(smem_raw + (size_t)b * CP::BUF);
+        const T* sh = reinterpret_cast<const T*>(smem_raw + (size_t)b * CP::BUF + AS::WBYTES);
+        SmemIO<T, P> io{W};
+        double energy = 0.0;
+        tma::mbar_wait(&full[b], (uint32_t)((i >> 1) & 1));
+        auto ld_sw = [&](int e) { return io.ld(e); };
+        auto st_sw = [&](int e, cx<T> v) { io.st(e, v); };
+        auto fwd_smem_stage = [&](auto s) {
+            constexpr int sv = decltype(s)::value;
+            cx<T> a[St<P, sv>::PER][St<P, sv>::R];
+            stage_ld<P, sv, T>(lt, ld_sw, a);
+            stage_math<P, sv, -1, T>(a, wb[sv]);
+            stage_st<P, sv, T>(lt, st_sw, a);
+            bar_named<NT>();
+        };
+        auto inv_smem_stage = [&](auto s) {
+            constexpr int sv = decltype(s)::value;
+            cx<T> a[St<P, sv>::PER][St<P, sv>::R];
+            stage_ld<P, sv, T>(lt, ld_sw, a);
+            stage_math<P, sv, +1, T>(a, wb[sv]);
+            stage_st<P, sv, T>(lt, st_sw, a);
+            bar_named<NT>();
+        };
+        {   // forward stage 1: the column arrived in natural (linear) order; it leaves the stage swizzled
+            cx<T> a[St<P, 1>::PER][St<P, 1>::R];
+            stage_ld<P, 1, T>(lt, [&](int e) { return W[e]; }, a);
+            bar_named<NT>();
+            stage_math<P, 1, -1, T>(a, wb[1]);
+            stage_st<P, 1, T>(lt, st_sw, a);
+            bar_named<NT>();
+        }
+        if (n != 0) {
+            static_for_up<2, S - 1>(fwd_smem_stage);
+            if constexpr (ENERGY) {
+                run_middle<P, T, true>(lt, ld_sw, st_sw, [&](int g, int u) { return sh[u * (L / P::RLAST) + g]; }, &energy);
+                energy *= 2.0;
+            } else {
+                run_middle<P, T>(lt, ld_sw, st_sw, [&](int g, int u) { return sh[u * (L / P::RLAST) + g]; });
+            }
+            bar_named<NT>();
+            static_for_down<S - 1, 2>(inv_smem_stage);
+        } else {         // packed n = 0 / L/2 column, see col2_kernel
+            static_for_up<2, S>(fwd_smem_stage);
+            const T* sp_ = A.shat;
+            const T* sm_ = A.shat + (size_t)(L / 2) * L;
+            for (int m = lt; m <= L / 2; m += NT) {
+                const int e = P::pos_of(m), e2 = P::pos_of((L - m) % L);
+                const cx<T> Wa = io.ld(e), Wb = io.ld(e2);
+                cx<T> va, vb;
+                const int i1 = P::shat_index(e), i2 = P::shat_index(e2);
+                va.x = sp_[i1] * Wa.x + sm_[i1] * Wb.x; va.y = sp_[i1] * Wa.y - sm_[i1] * Wb.y;
+                vb.x = sp_[i2] * Wb.x + sm_[i2] * Wa.x; vb.y = sp_[i2] * Wb.y - sm_[i2] * Wa.y;
+                if constexpr (ENERGY) {
+                    const double na = (double)Wa.x * (double)Wa.x + (double)Wa.y * (double)Wa.y;
+                    const double nb = (double)Wb.x * (double)Wb.x + (double)Wb.y * (double)Wb.y;
+                    const double re = (double)Wa.x * (double)Wb.x - (double)Wa.y * (double)Wb.y;
+                    const double term = 0.5 * (double)sp_[i1] * (na + nb) + (double)sm_[i1] * re;
+                    energy += e2 != e ? 2.0 * term : term;
+                }
+                io.st(e, va);
+                if (e2 != e) io.st(e2, vb);
+            }
+            bar_named<NT>();
+            static_for_down<S, 2>(inv_smem_stage);
+        }
+        {   // inverse stage 1: swizzled in, natural order out, ready for the scatter
+            cx<T> a[St<P, 1>::PER][St<P, 1>::R];
+            stage_ld<P, 1, T>(lt, ld_sw, a);
+            stage_math<P, 1, +1, T>(a, wb[1]);
+            bar_named<NT>();
+            stage_st<P, 1, T>(lt, [&](int e, cx<T> v) { W[e] = v; }, a);
+        }
+        tma::fence_proxy_async();                 // my writes -> visible to the async proxy
+        tma::mbar_warp_arrive(&ready[b]);
+        if constexpr (ENERGY) {                   // this column's share of sum shat |P|^2 (consumers only; fixed order)
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) energy += __shfl_down_sync(0xffffffffu, energy, o);
+            if (lane == 0) red[warp] = energy;
+            bar_named<NT>();
+            if (lt == 0) {
+                double e = 0.0;
+                for (int w2 = 0; w2 < NT / 32; ++w2) e += red[w2];
+                A.partial[n] = e;
+            }
+        }
+    }
+}
+
 // --------------------------------------------------------------------------------------------- stand-alone transforms
 // Column pass of fcg_fft_fwd / fcg_fft_inv on the T2 layout: forward only (DIR < 0, natural row-frequency order out) or
 // inverse only (DIR > 0, natural order in).  Same gather / in-place / scatter plumbing as col2_kernel; kept as a kernel
@@ -576,7 +741,8 @@ __global__ void __launch_bounds__(AsyncShape<T, P>::INV_THREADS, CTAS) row_inv2_
     constexpr uint32_t PIECE = (uint32_t)(QV * sizeof(T));
     constexpr int NTSF_ = (int)((AS::RING_BUDGET - 12 * (size_t)PIECE) / AS::TSB);
     constexpr int TCAP = (int)(20480 / AS::TSB) < 2 ? 2 : (int)(20480 / AS::TSB);     // ~20 KB of tiles in flight (measured: 2 x 8 KB at L = 2048 fp64, 5 x 4 KB at L = 8192 fp32)
-    constexpr int NTS = CGF ? (NTSF_ < 2 ? 2 : (NTSF_ > TCAP ? TCAP : NTSF_)) : AS::NTS;
+    constexpr int TCAP2 = TCAP > NSUB ? NSUB : (TCAP > AS::MAXSLOT ? AS::MAXSLOT : TCAP);
+    constexpr int NTS = CGF ? (NTSF_ < 2 ? 2 : (NTSF_ > TCAP2 ? TCAP2 : NTSF_)) : AS::NTS;
     constexpr size_t KRB = CGF ? AS::RING_BUDGET - (size_t)NTS * AS::TSB : AS::KRB;
     static_assert(NTS <= AS::MAXSLOT && KRB >= 6 * (size_t)PIECE, "P3 rings");
     extern __shared__ unsigned char smem_dyn[];

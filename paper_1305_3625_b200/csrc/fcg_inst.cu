@@ -50,6 +50,10 @@ template <typename T> struct Inst {
             if ((e = prep(row_fwd2_kernel<T, P, C_FWD, 1>, AS::fwd_smem)) != cudaSuccess) return e;
             if ((e = prep(row_inv2_kernel<T, P, C_INV, 1>, AS::inv_smem)) != cudaSuccess) return e;
             if ((e = prep(col2_kernel<T, P, C_COL, true>, AS::col_smem)) != cudaSuccess) return e;
+            if constexpr (COLP) {
+                if ((e = prep(col2p_kernel<T, P, CPS::CTAS, true>, CPS::smem)) != cudaSuccess) return e;
+                if ((e = prep(col2p_kernel<T, P, CPS::CTAS, false>, CPS::smem)) != cudaSuccess) return e;
+            }
             if ((e = prep(row_inv2_kernel<T, P, C_INV, 2>, AS::inv_smem)) != cudaSuccess) return e;
             if ((e = prep(col2_xform_kernel<T, P, C_COL, -1>, AS::WBYTES + 128)) != cudaSuccess) return e;
             if ((e = prep(col2_xform_kernel<T, P, C_COL, +1>, AS::WBYTES + 128)) != cudaSuccess) return e;
@@ -94,6 +98,19 @@ template <typename T> struct Inst {
         return cudaErrorInvalidValue;
     }
     static constexpr bool SL = V2;
+    using CPS = ColPShape<T, P>;
+    static constexpr bool COLP = V2 && CPS::valid;
+    static cudaError_t col2p(const void* args, const void* tensor_map, int energy, cudaStream_t st) {
+        if constexpr (COLP) {
+            const ColArgs<T>& A = *static_cast<const ColArgs<T>*>(args);
+            int grid = A.nsm * CPS::CTAS;
+            if (grid > L / 2) grid = L / 2;
+            const CUtensorMap& tm = *static_cast<const CUtensorMap*>(tensor_map);
+            if (energy) return launch(col2p_kernel<T, P, CPS::CTAS, true>, grid, P::NT + 32, CPS::smem, st, A.pdl, A, tm);
+            return launch(col2p_kernel<T, P, CPS::CTAS, false>, grid, P::NT + 32, CPS::smem, st, A.pdl, A, tm);
+        }
+        return cudaErrorInvalidValue;
+    }
     static cudaError_t col2_energy(const void* args, const void* tensor_map, cudaStream_t st) {
         if constexpr (SL) {
             const ColArgs<T>& A = *static_cast<const ColArgs<T>*>(args);
@@ -223,6 +240,7 @@ template <typename T> struct Inst {
         t.v2_ctas[0] = C_FWD; t.v2_ctas[1] = C_COL; t.v2_ctas[2] = C_INV;
         t.v2_smem[0] = AS::fwd_smem; t.v2_smem[1] = AS::col_smem; t.v2_smem[2] = AS::inv_smem;
         t.row_fwd2 = &row_fwd2; t.col2 = &col2; t.row_inv2 = &row_inv2; t.row_fwd2_rupd = &row_fwd2_rupd; t.row_inv2_pre = &row_inv2_pre;
+        t.colp_ok = COLP ? 1 : 0; t.colp_ctas = COLP ? CPS::CTAS : 0; t.col2p = &col2p;
         t.sl_ok = SL ? 1 : 0; t.col2_energy = &col2_energy; t.row_inv2_cgf = &row_inv2_cgf;
         t.col2_xform = &col2_xform; t.t2_export = &t2_export; t.t2_import = &t2_import;
         t.fused = FS::valid ? 1 : 0; t.fused_grid = FS::G; t.fused_solve = &fused_solve;

@@ -63,7 +63,8 @@ template <typename T> struct ColArgs {
     const Scalars* sc;
     int pdl;
     int hints;
-    double* partial;       // ENERGY instantiation: [gridDim.x] partial sums of shat |P|^2
+    double* partial;       // ENERGY instantiation: [L/2] partial sums of shat |P|^2, one per column
+    int nsm;               // persistent column pass: SMs of the device
 };
 
 template <typename T> struct RowInvArgs {

@@ -72,6 +72,9 @@ struct PassTable {
     int sl_ok;
     cudaError_t (*col2_energy)(const void* args, const void* tensor_map, cudaStream_t st);
     cudaError_t (*row_inv2_cgf)(const void* args, const void* tensor_map, cudaStream_t st);
+    // persistent, double-buffered column pass (col2p_kernel); colp_ok == 0 where two column buffers do not fit twice per SM
+    int colp_ok, colp_ctas;
+    cudaError_t (*col2p)(const void* args, const void* tensor_map, int energy, cudaStream_t st);
     cudaError_t (*row_fwd2_rupd)(const void* args, cudaStream_t st);                                // PCG: r update + r.r + row transforms of r
     cudaError_t (*row_inv2_pre)(const void* args, const void* tensor_map, cudaStream_t st);        // PCG: z = M^-1 r, r.z
     cudaError_t (*col2_xform)(const void* args, const void* tensor_map, int inverse, cudaStream_t st);   // stand-alone transforms

@@ -341,6 +341,29 @@ def test_cg_both_search_length_evaluations(B, cfg, L, dt):
     assert rel(outs[0][2], outs[1][2]) <= (1e-10 if dt == np.float64 else 2e-5)
 
 
+@pytest.mark.parametrize("L,dt", [(256, np.float64), (1024, np.float64), (2048, np.float64), (2048, np.float32), (4096, np.float32)])
+def test_column_pass_persistent_and_per_column(B, L, dt):
+    """The column pass as one CTA per column (col2_kernel) and as persistent CTAs with two column buffers (col2p_kernel,
+    several columns per CTA with refills at L = 2048 fp64 and L = 4096 fp32): the operator against the oracle (or, at
+    L = 4096, against the other variant), repeatable bitwise, and a CG solve with each."""
+    w = inputs.config(2, dt, L=L)
+    x = inputs.fft_field(L).astype(dt)
+    ref = orc.apply(w.s, w.k, x) if L <= 2048 else None
+    ys = []
+    for cp in (0, 1, 1):
+        h = handle(B, L, dt, w.s, FCG_OPT_COL_PERSISTENT=cp)
+        y = h.fcg_apply(dev(w.k), dev(x)).cpu().numpy()
+        if ref is not None:
+            assert rel(y, ref) <= TOL_OP[dt]
+        ys.append(y)
+        h.close()
+    assert np.array_equal(ys[1], ys[2])
+    assert rel(ys[0], ys[1]) <= (1e-14 if dt == np.float64 else 1e-6)
+    if L <= 1024:
+        for cp in (0, 1):
+            cg_parity(B, w, FCG_OPT_FUSED=0, FCG_OPT_COL_PERSISTENT=cp)
+
+
 # ------------------------------------------------------------------------------------ full-size configs
 @pytest.mark.parametrize("dt,count", [(np.float64, 100), (np.float32, 33)])
 def test_cg_config2_full_size(B, dt, count):
