@@ -749,7 +749,7 @@ __global__ void __launch_bounds__(AsyncShape<T, P>::INV_THREADS, CTAS) row_inv2_
     unsigned char* const smem_raw = align128(smem_dyn);
     __shared__ __align__(8) uint64_t tfull[AS::MAXSLOT], tempty[AS::MAXSLOT];
     __shared__ __align__(8) uint64_t kfull[AS::MAXSLOT], kempty[AS::MAXSLOT];
-    __shared__ double red[2 * 32];
+    __shared__ double red[3 * 32];                // (one array for all variants: a second one costs the fourth CTA per SM at L = 2048 fp32)
     cx<T>* W = reinterpret_cast<cx<T>*>(smem_raw);
     unsigned char* const tring = smem_raw + AS::WBYTES;
     unsigned char* const kring = tring + (size_t)NTS * AS::TSB;
@@ -941,9 +941,8 @@ __global__ void __launch_bounds__(AsyncShape<T, P>::INV_THREADS, CTAS) row_inv2_
         }
     }
     if constexpr (CGF) {         // all warps (the producers contribute zeros)
-        __shared__ double red3[3 * 32];
         double tot[3];
-        if (!grid_sum_last<3>(acc3, A.partial, &A.sc->ticket[0], red3, tot)) return;
+        if (!grid_sum_last<3>(acc3, A.partial, &A.sc->ticket[0], red, tot)) return;
         if (threadIdx.x == 0) {
             Scalars* sc = A.sc;
             sc->alpha = alpha_d; sc->pq = pq_d;
