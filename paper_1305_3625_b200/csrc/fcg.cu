@@ -622,6 +622,7 @@ int fcg_create(int L, fcg_dtype dt, void* workspace, void* cuda_stream, fcg_hand
     h->tab = get_table(L, dt);
     h->stream = (cudaStream_t)cuda_stream;
     h->lay = make_layout(L, h->w);
+    h->hints = h->N * h->w <= ((size_t)32 << 20) ? 127 : 63;      // bit 6 (T2 stores evict-last) pays while T2 is a quarter of L2 or less
     auto bail = [&](int code) { fcg_destroy(h); return code; };
     if (workspace) { h->ws = (char*)workspace; }
     else {
@@ -669,7 +670,7 @@ int fcg_set_option(fcg_handle h, int option, int value) {
             h->row_var_opt = value; return FCG_OK;
         case FCG_OPT_FUSED: if (value != 0 && value != 1) return fail(h, FCG_INVALID_ARG, "fused must be 0 or 1"); h->fused_opt = value; return FCG_OK;
         case FCG_OPT_PDL: if (value != 0 && value != 1) return fail(h, FCG_INVALID_ARG, "pdl must be 0 or 1"); h->pdl = value; return FCG_OK;
-        case FCG_OPT_L2_HINTS: if (value < 0 || value > 63) return fail(h, FCG_INVALID_ARG, "hints must be 0..63"); h->hints = value; return FCG_OK;
+        case FCG_OPT_L2_HINTS: if (value < 0 || value > 255) return fail(h, FCG_INVALID_ARG, "hints must be 0..255"); h->hints = value; return FCG_OK;
         case FCG_OPT_SPECTRAL_ALPHA: if (value != 0 && value != 1) return fail(h, FCG_INVALID_ARG, "spectral alpha must be 0 or 1"); h->sl_opt = value; return FCG_OK;
         case FCG_OPT_COL_PERSISTENT: if (value < -1 || value > 1) return fail(h, FCG_INVALID_ARG, "col persistent must be -1, 0 or 1"); h->colp_opt = value; return FCG_OK;
         case FCG_OPT_UNROLL: if (value < 1 || value > 64) return fail(h, FCG_INVALID_ARG, "unroll must be 1..64"); h->unroll = value; return FCG_OK;

@@ -94,6 +94,12 @@ template <> __device__ __forceinline__ void store_pair<float>(float2* dst, float
     *reinterpret_cast<float4*>(dst) = make_float4(a.x, a.y, b.x, b.y);
 }
 
+// the same with an L2 eviction-priority policy
+__device__ __forceinline__ void store_pair_hint(double2* dst, double2 a, double2 b, uint64_t pol) { tma::st_hint(dst, a, pol); tma::st_hint(dst + 1, b, pol); }
+__device__ __forceinline__ void store_pair_hint(float2* dst, float2 a, float2 b, uint64_t pol) {
+    tma::st_hint(reinterpret_cast<float4*>(dst), make_float4(a.x, a.y, b.x, b.y), pol);
+}
+
 // CTA barrier among the first N threads only (the consumers of a warp-specialised kernel); barrier 0 stays __syncthreads
 template <int N> __device__ __forceinline__ void bar_named() { asm volatile("bar.sync 1, %0;" ::"n"(N) : "memory"); }
 
@@ -181,6 +187,7 @@ __global__ void __launch_bounds__(P::NT + 32, CTAS) row_fwd2_kernel(const RowFwd
     if (cg) { alpha = (T)A.sc->alpha; beta = (T)A.sc->beta; }
     if (RUPD) alpha = (T)A.sc->alpha;
     const uint64_t pol_u = (A.hints & 2) ? tma::policy_evict_first() : tma::policy_evict_normal();   // L2 hints (bit 1): the u stores
+    const uint64_t pol_t2 = (A.hints & 64) ? tma::policy_evict_last() : tma::policy_evict_normal(); // (bit 6): T2 is read back by the next two passes
     cx<T> wb[S + 1][PM];
     static_for_up<1, S - 1>([&](auto s) { base_tw<P, decltype(s)::value, T>(lt, A.tw, wb[decltype(s)::value]); });
 
@@ -254,7 +261,7 @@ __global__ void __launch_bounds__(P::NT + 32, CTAS) row_fwd2_kernel(const RowFwd
                 X0 = mk<T>((Za.x + Zb.x) * h, (Za.y - Zb.y) * h);
                 X1 = mk<T>((Za.y + Zb.y) * h, (Zb.x - Za.x) * h);
             }
-            if (st_on) store_pair<T>(A.Tb + AS::t2_index(m, a0 >> 1), X0, X1);
+            if (st_on) store_pair_hint(A.Tb + AS::t2_index(m, a0 >> 1), X0, X1, pol_t2);
         }
     }
     }
@@ -414,7 +421,7 @@ template <typename T, typename P> struct ColPShape {
     static constexpr int by_smem = (int)((size_t)FCG_MAX_SMEM / (smem + 1024 + 512));
     static constexpr int by_thr = AS::thread_cap / (P::NT + 32);
     static constexpr int CTAS = by_smem < by_thr ? by_smem : by_thr;
-    static constexpr bool valid = AS::valid && CTAS >= 2;
+    static constexpr bool valid = AS::valid && CTAS >= 1;
 };
 
 template <typename T, typename P, int CTAS, bool ENERGY = false>
