@@ -49,11 +49,15 @@ template <typename T, typename P> struct AsyncShape {
     // Shared memory.  The rings are sized for CRES resident CTAs per SM: 4 transforms in flight when a work buffer is
     // small, else 2 (1 when even that does not fit); whatever the work buffers leave goes to the rings, whose depth is
     // what hides the loaded DRAM latency.  2688 = static barriers + 1 KB per-CTA reserve + alignment slack.
-    static constexpr int CRES = WBYTES <= 16384 ? 4 : (WBYTES <= 65536 ? 2 : 1);
-    static constexpr size_t RING_BUDGET = ((size_t)FCG_MAX_SMEM / CRES - 2688 - WBYTES) / 128 * 128;
+    // Measured at the 64 KB work buffers (L = 4096 fp64, L = 8192 fp32): ONE resident CTA with rings of 160 KB beats two with
+    // 47 KB each in P1 at both (178 -> 145 us, 325 -> 277 us) and in P3 for fp32 (378 -> 361); P3 at L = 4096 fp64 prefers two (157 vs 166).
+    static constexpr int CRES = WBYTES <= 16384 ? 4 : (WBYTES < 65536 ? 2 : 1);                                   // P1
+    static constexpr int CRES_I = WBYTES <= 16384 ? 4 : ((WBYTES < 65536 || (WBYTES == 65536 && sizeof(T) == 8)) ? 2 : 1);   // P3
+    static constexpr size_t RING_BUDGET_F = ((size_t)FCG_MAX_SMEM / CRES - 2688 - WBYTES) / 128 * 128;
+    static constexpr size_t RING_BUDGET = ((size_t)FCG_MAX_SMEM / CRES_I - 2688 - WBYTES) / 128 * 128;
     // P1: ring of NFS strips (p0 p1 r0 r1 u0 u1: 6 pieces each)
     static constexpr uint32_t FSLOTB = 6 * PIECE;
-    static constexpr int NFS = RING_BUDGET / FSLOTB < 2 ? 2 : (RING_BUDGET / FSLOTB > MAXSLOT ? MAXSLOT : (int)(RING_BUDGET / FSLOTB));
+    static constexpr int NFS = RING_BUDGET_F / FSLOTB < 2 ? 2 : (RING_BUDGET_F / FSLOTB > MAXSLOT ? MAXSLOT : (int)(RING_BUDGET_F / FSLOTB));
     static constexpr size_t fwd_smem = WBYTES + (size_t)NFS * FSLOTB + 128;   // + 128: the kernels align the dynamic base themselves
     // P2: column + its spectrum row
     static constexpr size_t col_smem = WBYTES + (size_t)L * sizeof(T) + 128;
