@@ -26,6 +26,7 @@
  *   - Return value: fcg_status.  >= 0 means the outputs are valid.  On error the outputs are
  *     unspecified unless stated; fcg_last_error() gives a message.  A handle is not thread-safe.
  *   - L must be a power of two, 16 <= L <= 8192 (S8); otherwise FCG_UNSUPPORTED.
+ *   - Workspace: fcg_workspace_bytes() ~ 6 N w (T2, two stored spectra, r, p, q, z) + tables.
  */
 #ifndef FCG_H
 #define FCG_H
@@ -184,7 +185,8 @@ int fcg_fracture_end(fcg_handle h, long long* index_host, int* iters_host, int* 
 /* Measurement aid: runs the set-up of fcg_solve and then `iters` iterations of the CG loop body as direct
  * launches with CUDA events between the four kernels (tol = 0: never stops early), and returns their mean
  * device times in milliseconds, ms_host[0..3] = { row pass forward (P1), column pass (P2), row pass inverse
- * (P3), residual update (P4) }.  Kernels run in loop order, so each sees the cache state its predecessor
+ * (P3), residual update (P4) }; with the default three-launch iteration (FCG_OPT_SPECTRAL_ALPHA = 1) P3 includes the residual
+ * update and ms_host[3] is the time between two adjacent events (~2.6 us).  Kernels run in loop order, so each sees the cache state its predecessor
  * leaves.  u is overwritten with an unfinished iterate.  Blocks until done.  Returns FCG_NOT_CONVERGED if the
  * loop flagged completion (times then include early exits and are not meaningful). */
 int fcg_profile_iteration(fcg_handle h, const void* k, const void* f, void* u, int iters, double* ms_host);
