@@ -50,9 +50,11 @@ template <typename T, typename P> struct AsyncShape {
     // small, else 2 (1 when even that does not fit); whatever the work buffers leave goes to the rings, whose depth is
     // what hides the loaded DRAM latency.  2688 = static barriers + 1 KB per-CTA reserve + alignment slack.
     // Measured at the 64 KB work buffers (L = 4096 fp64, L = 8192 fp32): ONE resident CTA with rings of 160 KB beats two with
-    // 47 KB each in P1 at both (178 -> 145 us, 325 -> 277 us) and in P3 for fp32 (378 -> 361); P3 at L = 4096 fp64 prefers two (157 vs 166).
+    // 47 KB each: P1 178 -> 145 us, 325 -> 277 us; the fused last pass 157 -> 128 us, 378 -> 290 us once its tile ring holds a whole
+    // transform (with nobody else on the SM the wait for the tiles at the start of a transform is fully exposed otherwise).
+    // At the 32 KB work buffers (L = 2048 fp64, L = 4096 fp32) one CTA loses in both passes (4-8 warps do not cover the stages).
     static constexpr int CRES = WBYTES <= 16384 ? 4 : (WBYTES < 65536 ? 2 : 1);                                   // P1
-    static constexpr int CRES_I = WBYTES <= 16384 ? 4 : ((WBYTES < 65536 || (WBYTES == 65536 && sizeof(T) == 8)) ? 2 : 1);   // P3
+    static constexpr int CRES_I = WBYTES <= 16384 ? 4 : (WBYTES < 65536 ? 2 : 1);   // P3
     static constexpr size_t RING_BUDGET_F = ((size_t)FCG_MAX_SMEM / CRES - 2688 - WBYTES) / 128 * 128;
     static constexpr size_t RING_BUDGET = ((size_t)FCG_MAX_SMEM / CRES_I - 2688 - WBYTES) / 128 * 128;
     // P1: ring of NFS strips (p0 p1 r0 r1 u0 u1: 6 pieces each)
@@ -752,7 +754,8 @@ __global__ void __launch_bounds__(AsyncShape<T, P>::INV_THREADS, CTAS) row_inv2_
     constexpr uint32_t PIECE = (uint32_t)(QV * sizeof(T));
     constexpr int NTSF_ = (int)((AS::RING_BUDGET - 12 * (size_t)PIECE) / AS::TSB);
     constexpr int TCAP = (int)(20480 / AS::TSB) < 2 ? 2 : (int)(20480 / AS::TSB);     // ~20 KB of tiles in flight (measured: 2 x 8 KB at L = 2048 fp64, 5 x 4 KB at L = 8192 fp32)
-    constexpr int TCAP2 = TCAP > NSUB ? NSUB : (TCAP > AS::MAXSLOT ? AS::MAXSLOT : TCAP);
+    constexpr int TCAP1 = AS::CRES_I == 1 ? NSUB : TCAP;   // one resident CTA: nobody else covers the rebuild's wait, keep a whole transform of tiles
+    constexpr int TCAP2 = TCAP1 > NSUB ? NSUB : (TCAP1 > AS::MAXSLOT ? AS::MAXSLOT : TCAP1);
     constexpr int NTS = CGF ? (NTSF_ < 2 ? 2 : (NTSF_ > TCAP2 ? TCAP2 : NTSF_)) : AS::NTS;
     constexpr size_t KRB = CGF ? AS::RING_BUDGET - (size_t)NTS * AS::TSB : AS::KRB;
     static_assert(NTS <= AS::MAXSLOT && KRB >= 6 * (size_t)PIECE, "P3 rings");
