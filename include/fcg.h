@@ -67,10 +67,10 @@ typedef enum {
                                  kernel with the vectors resident in shared memory and grid barriers between the phases;
                                  0: the graph of four kernels per iteration at every size */
     FCG_OPT_L2_HINTS     = 7, /* bit mask of L2 eviction-priority hints in the pipelined passes (default: all, bit 6
-                                 only while one vector is <= 32 MiB):
+                                 only while one vector is <= 32 MiB; 0..255):
                                  1 u strips (P1 loads) evict-first, 2 u stores evict-first, 4 spectrum rows (P2) evict-first,
                                  8 T2 tiles (P3 loads) evict-first, 16 k strips (P3) evict-first, 32 q loads (P4) evict-first,
-                                 64 T2 stores of P1 evict-last */
+                                 64 T2 stores of P1 evict-last, 128 r stores of the fused last pass evict-last (read back by the next P1) */
     FCG_OPT_SPECTRAL_ALPHA = 8, /* 1 (default): fcg_solve evaluates the search length's p.Ap as sum k p^2 (a scalar recurrence fed by the
                                  last pass) + sum shat |P|^2 (Parseval, accumulated in the column pass), so alpha is known before the
                                  last pass and r -= alpha q, r.r ride in it: 3 launches and 13.5 N w bytes per iteration, q never

@@ -622,7 +622,8 @@ int fcg_create(int L, fcg_dtype dt, void* workspace, void* cuda_stream, fcg_hand
     h->tab = get_table(L, dt);
     h->stream = (cudaStream_t)cuda_stream;
     h->lay = make_layout(L, h->w);
-    h->hints = h->N * h->w <= ((size_t)32 << 20) ? 127 : 63;      // bit 6 (T2 stores evict-last) pays while T2 is a quarter of L2 or less
+    // bit 6 (T2 stores evict-last) pays while T2 is a quarter of L2 or less, bit 7 (r stores evict-last) while r fits in L2
+    h->hints = 63 + (h->N * h->w <= ((size_t)32 << 20) ? 64 : 0) + (h->N * h->w <= ((size_t)128 << 20) ? 128 : 0);
     auto bail = [&](int code) { fcg_destroy(h); return code; };
     if (workspace) { h->ws = (char*)workspace; }
     else {

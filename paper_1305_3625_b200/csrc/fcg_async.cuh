@@ -808,6 +808,7 @@ __global__ void __launch_bounds__(AsyncShape<T, P>::INV_THREADS, CTAS) row_inv2_
     if (nv) kbase = (lane < 2 ? A.k : lane < 4 ? A.v : A.f) + (size_t)(lane & 1) * L;
     // L2 hints: T2 is dead once this pass has read it (bit 3); k comes back only in the next iteration (bit 4)
     const uint64_t pol_t = (A.hints & 8) ? tma::policy_evict_first() : tma::policy_evict_normal();
+    const uint64_t pol_r = (A.hints & 128) ? tma::policy_evict_last() : tma::policy_evict_normal();   // (bit 7) the new r is read back by the next P1
     const uint64_t pol_k = (lane < 2 && !PRE && (A.hints & 16)) ? tma::policy_evict_first() : tma::policy_evict_normal();
     auto issue_next_T = [&]() {          // whole warp; tile p_tn = (transform p_tn / NSUB, part p_tn % NSUB): TSUB / NB whole lines
         if (p_tn >= NTS) tma::mbar_wait(&tempty[p_ts], p_tph ^ 1u);
@@ -926,7 +927,7 @@ __global__ void __launch_bounds__(AsyncShape<T, P>::INV_THREADS, CTAS) row_inv2_
                     const T val0 = sl[j] * v0 + c0, val1 = sl[QV + j] * v1 + c1;         // k o x + C x
                     if constexpr (CGF) {
                         const T r0 = sl[4 * QV + j] - alpha * val0, r1 = sl[5 * QV + j] - alpha * val1;   // residue
-                        if (st_on) { A.out[i0] = r0; A.out[i0 + L] = r1; }
+                        if (st_on) { tma::st_hint(A.out + i0, r0, pol_r); tma::st_hint(A.out + i0 + L, r1, pol_r); }
                         f_rr += r0 * r0; f_rr += r1 * r1;                                                   // residue length (97)
                         const T kr0 = sl[j] * r0, kr1 = sl[QV + j] * r1;
                         f_t += kr0 * r0; f_t += kr1 * r1;
