@@ -56,6 +56,8 @@ def _declare(L: C.CDLL) -> None:
     L.oracle_idft2_brute.restype = None
     L.oracle_conv_direct.argtypes = [_i, _vp, _vp, _vp]
     L.oracle_conv_direct.restype = None
+    L.oracle_green_function.argtypes = [_i, _d, _d, _d, _vp]
+    L.oracle_green_function.restype = None
     L.oracle_num_threads.restype = _i
     L.oracle_set_num_threads.argtypes = [_i]
     for suf in ("_f64", "_f32"):
@@ -77,6 +79,19 @@ def _declare(L: C.CDLL) -> None:
         f.restype = _i
         f = getattr(L, "oracle_fracture" + suf)
         f.argtypes = [_i, _vp, _vp, _vp, _vp, _vp, _i, _d, _i, _vp, _vp, _vp]
+        f.restype = _i
+        f = getattr(L, "oracle_kernel_spectrum" + suf)
+        f.argtypes = [_i, _vp, _vp]; f.restype = _i
+        f = getattr(L, "oracle_force_apply" + suf)
+        f.argtypes = [_i, _vp, _vp, _vp, _vp]; f.restype = _i
+        f = getattr(L, "oracle_force_cg" + suf)
+        f.argtypes = [_i, _vp, _vp, _d, _vp, _d, _i, C.POINTER(_i), C.POINTER(_d), _vp, _vp, _vp]
+        f.restype = _i
+        f = getattr(L, "oracle_force_break_step" + suf)
+        f.argtypes = [_ll, _vp, _vp, _vp, C.POINTER(_ll), C.POINTER(_d), C.POINTER(_d)]
+        f.restype = _i
+        f = getattr(L, "oracle_force_fracture" + suf)
+        f.argtypes = [_i, _vp, _vp, _d, _vp, _vp, _i, _d, _i, _vp, _vp, _vp, _vp]
         f.restype = _i
 
 
@@ -237,3 +252,76 @@ def pcg_fracture(s, k, f, u, t, kbar: float, nsteps: int, tol: float, maxit: int
     done = getattr(lib(), "oracle_pcg_fracture" + _suf(dt))(L, _p(s), _p(k), _p(f), _p(u), _p(t), float(kbar), int(nsteps),
                                                             float(tol), int(maxit), _p(index), _p(iters), _p(gap))
     return dict(index=index, iters=iters, gap=gap, steps=int(done))
+
+
+# ---- the paper's formulation in the bond forces, (I + K G) f = K D (eq. (2)) ----------------
+
+def green_function(L: int, nu: float, E: float, a: float) -> np.ndarray:
+    """Real-space Green's function of eq. (1c) on the periodic lattice, G[da][db], fp64."""
+    G = np.empty((L, L), np.float64)
+    lib().oracle_green_function(int(L), float(nu), float(E), float(a), _p(G))
+    return G
+
+
+def kernel_spectrum(G) -> np.ndarray:
+    """s = Re F G in the dtype of G."""
+    G = np.asarray(G); dt = G.dtype; L = G.shape[0]
+    G = _arr(G, dt, (L, L))
+    s = np.empty((L, L), dt)
+    if getattr(lib(), "oracle_kernel_spectrum" + _suf(dt))(L, _p(G), _p(s)) != 0:
+        raise ValueError("oracle_kernel_spectrum: L must be a power of two")
+    return s
+
+
+def force_apply(g, k, x) -> np.ndarray:
+    """y = x + k o F^-1(g o F x) in the dtype of x."""
+    x = np.asarray(x); dt = x.dtype; L = x.shape[0]
+    g = _arr(g, dt, (L, L)); k = _arr(k, dt, (L, L)); x = _arr(x, dt, (L, L))
+    y = np.empty((L, L), dt)
+    if getattr(lib(), "oracle_force_apply" + _suf(dt))(L, _p(g), _p(k), _p(x), _p(y)) != 0:
+        raise ValueError("oracle_force_apply: bad argument")
+    return y
+
+
+def force_cg(g, k, D: float, f0, tol: float, maxit: int, history: bool = False, directions: bool = False):
+    """CG on (I + K G) f = K D.  Returns dict(f, iters, relres, status[, hist][, P, R]); dtype taken from k."""
+    k = np.asarray(k); dt = k.dtype; L = k.shape[0]; N = L * L
+    g = _arr(g, dt, (L, L)); k = _arr(k, dt, (L, L))
+    f = np.array(f0, dtype=dt, order="C", copy=True).reshape(L, L)
+    hist = np.full(maxit + 1, np.nan, np.float64) if history else None
+    P = np.zeros((maxit, N), dt) if directions else None
+    R = np.zeros((maxit, N), dt) if directions else None
+    it = C.c_int(0); rr = C.c_double(0.0)
+    st = getattr(lib(), "oracle_force_cg" + _suf(dt))(L, _p(g), _p(k), float(D), _p(f), float(tol), int(maxit),
+                                                       C.byref(it), C.byref(rr), _p(hist), _p(P), _p(R))
+    out = dict(f=f, iters=int(it.value), relres=float(rr.value), status=int(st))
+    if history:
+        out["hist"] = hist[: it.value + 1]
+    if directions:
+        out["P"] = P[: it.value]; out["R"] = R[: it.value]
+    return out
+
+
+def force_break_step(k: np.ndarray, f: np.ndarray, t):
+    """In-place on k and f. Returns (index, ratio, second, status)."""
+    dt = k.dtype
+    if not (k.flags.c_contiguous and f.flags.c_contiguous and f.dtype == dt):
+        raise ValueError("k, f must be C-contiguous arrays of one dtype (modified in place)")
+    t = _arr(t, dt)
+    idx = C.c_longlong(-1); ratio = C.c_double(0.0); second = C.c_double(0.0)
+    st = getattr(lib(), "oracle_force_break_step" + _suf(dt))(k.size, _p(k), _p(f), _p(t),
+                                                               C.byref(idx), C.byref(ratio), C.byref(second))
+    return int(idx.value), float(ratio.value), float(second.value), int(st)
+
+
+def force_fracture(g, k, D: float, f, t, nsteps: int, tol: float, maxit: int):
+    """Quasi-static loop in the forces.  In-place on k and f. Returns dict(index, iters, ratio, gap, steps)."""
+    dt = k.dtype; L = k.shape[0]
+    g = _arr(g, dt, (L, L)); t = _arr(t, dt, (L, L))
+    if not (k.flags.c_contiguous and f.flags.c_contiguous and f.dtype == dt):
+        raise ValueError("k, f must be C-contiguous arrays of one dtype (modified in place)")
+    index = np.full(nsteps, -1, np.int64); iters = np.zeros(nsteps, np.int32)
+    ratio = np.full(nsteps, np.nan, np.float64); gap = np.full(nsteps, np.nan, np.float64)
+    done = getattr(lib(), "oracle_force_fracture" + _suf(dt))(L, _p(g), _p(k), float(D), _p(f), _p(t), int(nsteps),
+                                                              float(tol), int(maxit), _p(index), _p(iters), _p(ratio), _p(gap))
+    return dict(index=index, iters=iters, ratio=ratio, gap=gap, steps=int(done))

@@ -17,6 +17,10 @@
  *   oracle_pcg_{f64,f32}       the same with the spectral preconditioner M = kbar I + C
  *   oracle_break_step_*, oracle_fracture_*   break rule + quasi-static loop (PAPER.md:78,
  *                              BASELINE.json configs[3])
+ *   oracle_green_function      eq. (1c): real-space Green's function, closed form of the integral
+ *   oracle_kernel_spectrum_*   s = Re F G, the static transform of the kernel
+ *   oracle_force_{apply,cg,break_step,fracture}_*   the paper's formulation in the bond forces, (I + K G) f = K D
+ *                              (eq. (2))
  * Pins (tests/test_oracle_*.py): none of these functions is "parity unpinned".
  *
  * Build: gcc -O2 -fopenmp -ffp-contract=off -fPIC -shared fcg_oracle.c -o libfcg_oracle.so -lm
@@ -116,6 +120,32 @@ void oracle_conv_direct(int L, const double* c, const double* x, double* y)
                     acc += c[(size_t)da * L + db] * x[(size_t)a2 * L + b2];
                 }
             y[(size_t)a * L + b] = acc;
+        }
+}
+
+/* Real-space Green's function of eq. (1c), PAPER.md:63:
+ *     G_ij = (1 - nu^2) / (pi E a^2)  *  int int_{-a/2}^{a/2} dx' dy' / | r_i - r_j(x', y') |
+ * i.e. the surface displacement at bond i of an elastic half space under a unit force spread uniformly over the a x a
+ * square of bond j.  The integral of 1/r over a rectangle has the closed form (antiderivative checked by differentiation:
+ * d^2/dxdy [ x asinh(y/|x|) + y asinh(x/|y|) ] = 1/sqrt(x^2+y^2))
+ *     I(X, Y) = sum over the four corners (x, y) = (X +- a/2, Y +- a/2) of  sign * ( x asinh(y/|x|) + y asinh(x/|y|) ),
+ * sign = + for (+,+) and (-,-), - otherwise.  Corners are odd multiples of a/2, never on an axis.
+ * Reading F3 (the paper does not state the boundary condition; Fourier acceleration implies a periodic lattice):
+ * r_i - r_j is the minimum-image offset, da -> da - L for da > L/2 (I is even in X and in Y, so da = L/2 is unambiguous).
+ * Output: G[da][db], da, db = 0..L-1, row-major, fp64.  G is even, so its transform is real. */
+static double oracle_corner(double x, double y) { return x * asinh(y / fabs(x)) + y * asinh(x / fabs(y)); }
+
+void oracle_green_function(int L, double nu, double E, double a, double* G)
+{
+    double pref = (1.0 - nu * nu) / (M_PI * E * a * a);
+    double h = 0.5 * a;
+    for (int da = 0; da < L; ++da)
+        for (int db = 0; db < L; ++db) {
+            double X = a * (double)(da <= L / 2 ? da : da - L);
+            double Y = a * (double)(db <= L / 2 ? db : db - L);
+            double I = oracle_corner(X + h, Y + h) - oracle_corner(X - h, Y + h)
+                     - oracle_corner(X + h, Y - h) + oracle_corner(X - h, Y - h);
+            G[(size_t)da * L + db] = pref * I;
         }
 }
 

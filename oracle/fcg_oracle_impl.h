@@ -325,3 +325,150 @@ int FN(oracle_pcg_fracture)(int L, const REAL* s, REAL* k, const REAL* f, REAL* 
     }
     return nsteps;
 }
+
+/* ================================================================================================
+ * The paper's own formulation in the bond forces:
+ *     f_i = -k_i (u_i - D)   (1a),      u_i = sum_j G_ij f_j   (1b, with the typo f_i -> f_j: reading G1)
+ *     =>  (I + K G) f = K D             (2)
+ * solved for f by conjugate gradient as Listing 2 says.  G is applied by Fourier acceleration,
+ * G x = F^-1( g o F x ) with g = F G "static and performed during initialization".
+ * Reading F1: I + K G is symmetric positive definite on the unbroken bonds when every unbroken bond has the same
+ * elastic constant ("For simplicity, all fibers have the same elastic constant"), k_i in {0, kappa}: there
+ * it is I + kappa P G P (P = projection on the unbroken bonds), and every CG vector stays in range(P) because b = K D and
+ * K G x lie in it and the start vector has f_i = 0 on broken bonds.  That is the case the functions below are for.
+ * ------------------------------------------------------------------------------------------------ */
+
+/* s = Re F G: the static transform of a real-space kernel G (L x L, G[da][db], offsets mod L).  For an even kernel
+ * (G[-da][-db] = G[da][db]) the transform is real; the imaginary part (rounding) is dropped like cpyReal does. */
+int FN(oracle_kernel_spectrum)(int L, const REAL* G, REAL* s)
+{
+    if (L < 1 || (L & (L - 1))) return -1;
+    size_t N = (size_t)L * L;
+    CPLX* work = (CPLX*)malloc(sizeof(CPLX) * N);
+    for (size_t i = 0; i < N; ++i) { work[i].re = G[i]; work[i].im = (REAL)0; }
+    FN(fft2d)(work, L, -1);
+    for (size_t i = 0; i < N; ++i) s[i] = work[i].re;
+    free(work);
+    return 0;
+}
+
+/* y = (I + K G) x = x + k o (G x)      (left side of eq. (2)) */
+static void FN(force_apply)(int L, const REAL* g, const REAL* k, const REAL* x, REAL* y, CPLX* work)
+{
+    size_t N = (size_t)L * L;
+    FN(convolve)(L, g, x, y, work);
+    for (size_t i = 0; i < N; ++i) y[i] = x[i] + k[i] * y[i];
+}
+
+int FN(oracle_force_apply)(int L, const REAL* g, const REAL* k, const REAL* x, REAL* y)
+{
+    if (L < 1 || (L & (L - 1))) return -1;
+    CPLX* work = (CPLX*)malloc(sizeof(CPLX) * (size_t)L * L);
+    FN(force_apply)(L, g, k, x, y, work);
+    free(work);
+    return 0;
+}
+
+/* Conjugate gradient on (I + K G) f = K D, Listing 2 step by step (same scalars, stopping rule and return values as
+ * oracle_cg above; the right-hand side is b_i = k_i * D, one multiply in REAL, and the stop is sqrt(r.r) <= tol sqrt(b.b)).
+ *   f   in: initial guess (must be 0 on broken bonds), out: the bond forces */
+int FN(oracle_force_cg)(int L, const REAL* g, const REAL* k, double D, REAL* f, double tol, int maxit,
+                        int* iters, double* relres, double* hist, REAL* Phist, REAL* Rhist)
+{
+    if (L < 1 || (L & (L - 1)) || maxit < 0 || !(tol >= 0.0)) return -1;
+    size_t N = (size_t)L * L;
+    int status = 1, it = 0;
+    REAL* b = (REAL*)malloc(sizeof(REAL) * N);
+    for (size_t i = 0; i < N; ++i) b[i] = k[i] * (REAL)D;         /* K D */
+    double bn = sqrt(FN(dot)(N, b, b));
+    if (bn == 0.0) {
+        for (size_t i = 0; i < N; ++i) f[i] = (REAL)0;
+        *iters = 0; *relres = 0.0; if (hist) hist[0] = 0.0;
+        free(b);
+        return 0;
+    }
+    REAL* r = (REAL*)malloc(sizeof(REAL) * N);
+    REAL* p = (REAL*)malloc(sizeof(REAL) * N);
+    REAL* q = (REAL*)malloc(sizeof(REAL) * N);
+    CPLX* work = (CPLX*)malloc(sizeof(CPLX) * N);
+
+    FN(force_apply)(L, g, k, f, q, work);                        /* set up initial values */
+    for (size_t i = 0; i < N; ++i) { r[i] = b[i] - q[i]; p[i] = r[i]; }
+    double rho = FN(dot)(N, r, r);
+    if (hist) hist[0] = sqrt(rho) / bn;
+    if (sqrt(rho) <= tol * bn) { status = 0; goto done; }
+
+    while (it < maxit) {
+        if (Phist) memcpy(Phist + (size_t)it * N, p, sizeof(REAL) * N);
+        if (Rhist) memcpy(Rhist + (size_t)it * N, r, sizeof(REAL) * N);
+        FN(force_apply)(L, g, k, p, q, work);                    /* calculate A*x */
+        double pq = FN(dot)(N, p, q);                            /* search length (dot product) */
+        if (!(pq > 0.0) || !isfinite(pq)) { status = -4; goto done; }
+        double alpha = rho / pq;
+        REAL al = (REAL)alpha;
+        for (size_t i = 0; i < N; ++i) f[i] = f[i] + al * p[i];  /* new x */
+        for (size_t i = 0; i < N; ++i) r[i] = r[i] - al * q[i];  /* residue */
+        double rho_new = FN(dot)(N, r, r);                       /* residue length */
+        ++it;
+        if (hist) hist[it] = sqrt(rho_new) / bn;
+        if (sqrt(rho_new) <= tol * bn) { rho = rho_new; status = 0; break; }   /* check convergence */
+        double beta = rho_new / rho;                             /* update calculation variables */
+        REAL be = (REAL)beta;
+        for (size_t i = 0; i < N; ++i) p[i] = r[i] + be * p[i];
+        rho = rho_new;
+    }
+done:
+    *iters = it;
+    *relres = sqrt(rho) / bn;
+    free(b); free(r); free(p); free(q); free(work);
+    return status;
+}
+
+/* Break step in the force formulation (reading F2): the response is linear in D, so the bond that reaches its threshold
+ * first as D grows is the one with the largest f_i / t_i (one IEEE divide in double) among the unbroken bonds; ties ->
+ * lowest i, NaN skipped.  The bond is removed: k_i = 0 and f_i = 0 (a broken bond carries no force; keeps the warm start
+ * inside range(P)).  ratio: with the forces computed at displacement D the bond breaks at D_c = D / ratio.
+ * returns 0, or -6 when there is no candidate (index = -1). */
+int FN(oracle_force_break_step)(long long N, REAL* k, REAL* f, const REAL* t,
+                                long long* index, double* ratio, double* second)
+{
+    long long best = -1;
+    double rbest = 0.0, rsecond = -INFINITY;
+    for (long long i = 0; i < N; ++i) {
+        if (!(k[i] > (REAL)0)) continue;
+        double rt = (double)f[i] / (double)t[i];
+        if (rt != rt) continue;
+        if (best < 0) { best = i; rbest = rt; }
+        else if (rt > rbest) { rsecond = rbest; rbest = rt; best = i; }
+        else if (rt > rsecond) rsecond = rt;
+    }
+    *index = best; *ratio = rbest; if (second) *second = rsecond;
+    if (best < 0) return -6;
+    k[best] = (REAL)0;
+    f[best] = (REAL)0;
+    return 0;
+}
+
+/* Quasi-static loop in the force formulation ("For each step in the simulation, the displacement is set, and the
+ * resulting distribution of forces is calculated.  For large enough local strain, bonds break"):
+ * each step solves (I + K G) f = K D from the previous forces and breaks one bond.
+ * out_index, out_iters, out_ratio (winning f/t; D_c = D/ratio), out_gap (relative top-2 gap, may be NULL): [nsteps].
+ * returns the number of completed steps, or a negative CG status. */
+int FN(oracle_force_fracture)(int L, const REAL* g, REAL* k, double D, REAL* f, const REAL* t,
+                              int nsteps, double tol, int maxit,
+                              long long* out_index, int* out_iters, double* out_ratio, double* out_gap)
+{
+    long long N = (long long)L * L;
+    for (int step = 0; step < nsteps; ++step) {
+        int it; double rr;
+        int st = FN(oracle_force_cg)(L, g, k, D, f, tol, maxit, &it, &rr, NULL, NULL, NULL);
+        if (st < 0) return st;
+        long long idx; double ratio, second;
+        int bs = FN(oracle_force_break_step)(N, k, f, t, &idx, &ratio, &second);
+        if (bs < 0) return step;
+        out_index[step] = idx; out_iters[step] = it;
+        if (out_ratio) out_ratio[step] = ratio;
+        if (out_gap) out_gap[step] = (ratio - second) / fabs(ratio);
+    }
+    return nsteps;
+}

@@ -114,3 +114,23 @@ def precond_kbar(k: np.ndarray) -> float:
     """Constant of the spectral preconditioner M = kbar I + C (reading D4): the mean stiffness,
     accumulated in fp64.  A parameter recipe, handed unchanged to oracle and GPU."""
     return float(np.mean(np.asarray(k, dtype=np.float64)))
+
+
+# ---- the paper's formulation in the bond forces (SURVEY.md 8(f) NEXT #2, DESIGN.md section 15) -----------------------------
+# Constants of eq. (1c): the paper gives no values (PAPER.md:63-66), these are the recipe's (reading F4).
+GREEN_NU, GREEN_E, GREEN_A = 0.3, 1.0, 1.0
+FORCE_KAPPA, FORCE_D = 1.0, 1.0
+
+
+def gradient_thresholds(L: int, gradient: float, seed: int = SEED_T) -> np.ndarray:
+    """t_i = U[0,1] + gradient * a / L for row a: "insert a gradient in the threshold distribution", which
+    turns the damage into a front that advances along the rows."""
+    return thresholds(L, seed) + gradient * (np.arange(L, dtype=np.float64) / L)[:, None]
+
+
+def force_k(L: int, broken_den: int | None = None, kappa: float = FORCE_KAPPA) -> np.ndarray:
+    """All unbroken bonds share one elastic constant; a seeded 1/broken_den of the bonds is broken."""
+    k = np.full((L, L), kappa, np.float64)
+    if broken_den:
+        k[broken_mask(L, broken_den)] = 0.0
+    return k
