@@ -182,6 +182,45 @@ int fcg_fracture_begin(fcg_handle h, void* k, const void* f, void* u, const void
                        int maxit, int use_pcg);
 int fcg_fracture_end(fcg_handle h, long long* index_host, int* iters_host, int* steps_done_host);
 
+/* ---- The paper's own formulation in the bond forces ------------------------
+ * Model:   f_i = -k_i (u_i - D)  (1a),   u_i = sum_j G_ij f_j  (1b; "f_i" in the print is a typo, reading G1),
+ *                          G_ij = (1 - nu^2)/(pi E a^2) * int int_{-a/2}^{a/2} dx' dy' / |r_i - r_j(x', y')|          (1c)
+ *                     =>   (I + K G) f = K D                                                                          (2)
+ * solved for the forces f by conjugate gradient (Listing 2) with G applied by Fourier acceleration (eq. (3)):
+ * G x = F^-1( g o F x ), g = Re F G "static and performed during initialization" and handed to fcg_set_spectrum.
+ * Reading F1: I + K G is symmetric positive definite on the unbroken bonds when they all share one elastic constant, k_i in
+ * {0, kappa} ("all fibers have the same elastic constant"), and every CG vector then stays zero on broken bonds
+ * provided the start vector is; for other k the iteration is not conjugate gradient and the result is unspecified.
+ *
+ *   fcg_green_function   G[da][db] (L x L, written) = eq. (1c) on the periodic lattice with minimum-image offsets (reading F3),
+ *                        the integral in closed form, evaluated in double and rounded once to the handle's dtype.
+ *                        E > 0, a > 0.  Asynchronous.
+ *   fcg_kernel_spectrum  s (L x L, written, row-major [m][n]) = Re F G for a real kernel G[da][db] (L x L, read-only): forward
+ *                        transform by the library's own passes, real part expanded from the half spectrum.  Uses the handle's
+ *                        workspace (r, p): not while a solve is pending.  s must not alias G.  Asynchronous.
+ *   fcg_force_apply      y = (I + K G) x = x + k o (G x); y must not alias k or x.  Asynchronous.
+ *   fcg_force_solve      CG on eq. (2): right-hand side b_i = k_i * D formed in the residual pass (one multiply in the handle's dtype);
+ *                        f in: initial guess (0 on broken bonds), out: forces; stop at the first iteration with
+ *                        ||r||_2 <= tol ||b||_2; iters / rel_residual / status / scalars in double / determinism as fcg_solve.
+ *                        k == 0 everywhere or D == 0 gives f = 0, 0 iterations.  One CUDA graph per solve, four launches
+ *                        per iteration (the textbook order; the spectral search length of fcg_solve is not used).  Blocks.
+ *   fcg_force_break_step reading F2: the response is linear in D, so the bond that reaches its threshold first is
+ *                        argmax over {k_i > 0} of f_i / t_i (one IEEE divide in double; ties -> lowest i; NaN skipped);
+ *                        sets k_i = 0 AND f_i = 0 (a broken bond carries nothing).  ratio_host = the winning f/t: with f
+ *                        computed at displacement D the bond breaks at D_c = D / ratio.  Blocks.
+ *   fcg_force_fracture   nsteps times { fcg_force_solve warm-started from the current f; fcg_force_break_step } ("For each
+ *                        step in the simulation, the displacement is set, and the resulting distribution of forces is
+ *                        calculated ... bonds break").  index_host, iters_host, ratio_host (may be NULL): HOST
+ *                        arrays of nsteps; stops early on a negative status; steps_done_host = completed steps. */
+int fcg_green_function(fcg_handle h, double nu, double E, double a, void* G);
+int fcg_kernel_spectrum(fcg_handle h, const void* G, void* s);
+int fcg_force_apply(fcg_handle h, const void* k, const void* x, void* y);
+int fcg_force_solve(fcg_handle h, const void* k, double D, void* f, double tol, int maxit,
+                    int* iters_host, double* rel_residual_host);
+int fcg_force_break_step(fcg_handle h, void* k, void* f, const void* t, long long* index_host, double* ratio_host);
+int fcg_force_fracture(fcg_handle h, void* k, double D, void* f, const void* t, int nsteps, double tol, int maxit,
+                       long long* index_host, int* iters_host, double* ratio_host, int* steps_done_host);
+
 /* Measurement aid: runs the set-up of fcg_solve and then `iters` iterations of the CG loop body as direct
  * launches with CUDA events between the four kernels (tol = 0: never stops early), and returns their mean
  * device times in milliseconds, ms_host[0..3] = { row pass forward (P1), column pass (P2), row pass inverse

@@ -26,7 +26,9 @@ EXPORTS = ["fcg_workspace_bytes", "fcg_create", "fcg_destroy", "fcg_set_option",
            "fcg_solve", "fcg_solve_host", "fcg_profile_iteration", "fcg_fft_fwd", "fcg_fft_inv", "fcg_break_step", "fcg_fracture",
            "fcg_last_launch_count", "fcg_last_error", "fcg_version",
            "fcg_set_preconditioner", "fcg_pcg_solve", "fcg_profile_pcg_iteration", "fcg_pcg_fracture",
-           "fcg_fracture_begin", "fcg_fracture_end"]
+           "fcg_fracture_begin", "fcg_fracture_end",
+           "fcg_green_function", "fcg_kernel_spectrum", "fcg_force_apply", "fcg_force_solve", "fcg_force_break_step",
+           "fcg_force_fracture"]
 
 _lib = None
 
@@ -64,6 +66,12 @@ def lib() -> C.CDLL:
         L.fcg_set_preconditioner.argtypes = [vp, vp, d]; L.fcg_set_preconditioner.restype = i
         L.fcg_pcg_solve.argtypes = [vp, vp, vp, vp, d, i, C.POINTER(i), C.POINTER(d)]; L.fcg_pcg_solve.restype = i
         L.fcg_profile_pcg_iteration.argtypes = [vp, vp, vp, vp, i, C.POINTER(d)]; L.fcg_profile_pcg_iteration.restype = i
+        L.fcg_green_function.argtypes = [vp, d, d, d, vp]; L.fcg_green_function.restype = i
+        L.fcg_kernel_spectrum.argtypes = [vp, vp, vp]; L.fcg_kernel_spectrum.restype = i
+        L.fcg_force_apply.argtypes = [vp, vp, vp, vp]; L.fcg_force_apply.restype = i
+        L.fcg_force_solve.argtypes = [vp, vp, d, vp, d, i, C.POINTER(i), C.POINTER(d)]; L.fcg_force_solve.restype = i
+        L.fcg_force_break_step.argtypes = [vp, vp, vp, vp, C.POINTER(ll), C.POINTER(d)]; L.fcg_force_break_step.restype = i
+        L.fcg_force_fracture.argtypes = [vp, vp, d, vp, vp, i, d, i, vp, vp, vp, C.POINTER(i)]; L.fcg_force_fracture.restype = i
         L.fcg_last_launch_count.argtypes = [vp]; L.fcg_last_launch_count.restype = ll
         L.fcg_last_error.argtypes = [vp]; L.fcg_last_error.restype = C.c_char_p
         L.fcg_version.argtypes = []; L.fcg_version.restype = C.c_char_p
@@ -256,6 +264,58 @@ class Fcg:
         if st != FCG_OK:
             self._raise(st)
         return [float(x) for x in ms]
+
+    # -- the paper's formulation in the bond forces, (I + K G) f = K D (include/fcg.h) ---------------------
+    def fcg_green_function(self, nu: float, E: float, a: float, G: torch.Tensor | None = None) -> torch.Tensor:
+        G = torch.empty((self.L, self.L), dtype=self.dtype, device=self.device) if G is None else G
+        st = self._lib.fcg_green_function(self._h, float(nu), float(E), float(a), self._chk(G, self.N))
+        if st != FCG_OK:
+            self._raise(st)
+        return G
+
+    def fcg_kernel_spectrum(self, G: torch.Tensor, s: torch.Tensor | None = None) -> torch.Tensor:
+        s = torch.empty((self.L, self.L), dtype=self.dtype, device=G.device) if s is None else s
+        st = self._lib.fcg_kernel_spectrum(self._h, self._chk(G, self.N), self._chk(s, self.N))
+        if st != FCG_OK:
+            self._raise(st)
+        return s
+
+    def fcg_force_apply(self, k: torch.Tensor, x: torch.Tensor, y: torch.Tensor | None = None) -> torch.Tensor:
+        y = torch.empty_like(x) if y is None else y
+        st = self._lib.fcg_force_apply(self._h, self._chk(k, self.N), self._chk(x, self.N), self._chk(y, self.N))
+        if st != FCG_OK:
+            self._raise(st)
+        return y
+
+    def fcg_force_solve(self, k: torch.Tensor, D: float, f: torch.Tensor, tol: float, maxit: int):
+        """In place on f. Returns (iters, rel_residual, status) like fcg_solve."""
+        it = C.c_int(0); rr = C.c_double(0.0)
+        st = self._lib.fcg_force_solve(self._h, self._chk(k, self.N), float(D), self._chk(f, self.N), float(tol), int(maxit),
+                                       C.byref(it), C.byref(rr))
+        if st < 0 and st != FCG_BREAKDOWN:
+            self._raise(st)
+        return int(it.value), float(rr.value), int(st)
+
+    def fcg_force_break_step(self, k: torch.Tensor, f: torch.Tensor, t: torch.Tensor):
+        """In place on k and f. Returns (index, ratio, status)."""
+        idx = C.c_longlong(-1); ratio = C.c_double(0.0)
+        st = self._lib.fcg_force_break_step(self._h, self._chk(k, self.N), self._chk(f, self.N), self._chk(t, self.N),
+                                            C.byref(idx), C.byref(ratio))
+        if st < 0 and st != FCG_NO_CANDIDATE:
+            self._raise(st)
+        return int(idx.value), float(ratio.value), int(st)
+
+    def fcg_force_fracture(self, k: torch.Tensor, D: float, f: torch.Tensor, t: torch.Tensor, nsteps: int, tol: float, maxit: int):
+        """In place on k and f. Returns (index[int64], iters[int32], ratio[float64], steps_done, status)."""
+        import numpy as np
+        index = np.full(nsteps, -1, np.int64); iters = np.zeros(nsteps, np.int32); ratio = np.full(nsteps, np.nan, np.float64)
+        done = C.c_int(0)
+        st = self._lib.fcg_force_fracture(self._h, self._chk(k, self.N), float(D), self._chk(f, self.N), self._chk(t, self.N),
+                                          int(nsteps), float(tol), int(maxit), index.ctypes.data_as(C.c_void_p),
+                                          iters.ctypes.data_as(C.c_void_p), ratio.ctypes.data_as(C.c_void_p), C.byref(done))
+        if st < 0 and st not in (FCG_BREAKDOWN, FCG_NO_CANDIDATE):
+            self._raise(st)
+        return index, iters, ratio, int(done.value), int(st)
 
     def fcg_last_launch_count(self) -> int:
         return int(self._lib.fcg_last_launch_count(self._h))

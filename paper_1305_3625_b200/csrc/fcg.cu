@@ -65,7 +65,7 @@ Layout make_layout(int L, size_t w) {
 }
 
 struct GraphEntry {
-    const void *k, *f; void* u; double tol; int maxit, var, unroll, pdl, pcg;
+    const void *k, *f; void* u; double tol; int maxit, var, unroll, pdl, pcg, force; double D;   // pcg: bit 0 = preconditioned, the rest = launch options (key)
     cudaGraph_t graph; cudaGraphExec_t exec; unsigned long long stamp;
 };
 
@@ -144,6 +144,7 @@ int fail(fcg_handle h, int code, const char* msg) { if (h) h->err = msg; return 
 template <typename T> struct Seq {
     fcg_handle h; cudaStream_t st; bool classic = false;      // classic: force the synchronous passes (stand-alone transforms)
     bool pcg = false;                                         // preconditioned CG: directions from z = M^-1 r
+    bool force = false; double D = 0.0;                       // force formulation (I + K G) f = K D (eq. (2))
     bool v2() const { return h->v2() && !classic; }
     const T* mhat() const { return h->at<T>(h->lay.mhat); }
     T* z() const { return h->at<T>(h->lay.z); }
@@ -168,7 +169,7 @@ template <typename T> struct Seq {
     }
     cudaError_t row_inv(int mode, const T* k, const T* v, const T* f, T* out, T* out2) const {
         RowInvArgs<T> A{}; A.mode = mode; A.Tb = Tb(); A.tw = tw(); A.k = k; A.v = v; A.f = f; A.out = out; A.out2 = out2;
-        A.scale = (T)(1.0 / ((double)h->L * (double)h->L)); A.hints = h->hints;
+        A.scale = (T)(1.0 / ((double)h->L * (double)h->L)); A.hints = h->hints; A.form = force ? 1 : 0; A.dval = (T)D;
         A.partial = h->at<double>(h->lay.partial_row); A.sc = h->sc(); A.nsm = h->nsm; A.pdl = h->pdl;
         ++h->launches;
         return v2() ? h->tab->row_inv2(&A, &h->tmap_row, st) : h->tab->row_inv(h->row_var(), &A, st);
@@ -182,7 +183,7 @@ template <typename T> struct Seq {
         if ((e = cudaGetLastError()) != cudaSuccess) return e;
         if ((e = row_fwd(ROWF_PLAIN, u, nullptr)) != cudaSuccess) return e;
         if ((e = col(COL_CONV, false)) != cudaSuccess) return e;
-        if ((e = row_inv(ROWI_RESID, k, u, f, r(), p())) != cudaSuccess) return e;
+        if ((e = row_inv(ROWI_RESID, k, u, force ? k : f, r(), p())) != cudaSuccess) return e;   // (force: b = K D is formed in the pass)
         if (sl()) {      // start value of the sum k p^2 recurrence: the first direction is p = r
             cg_kpp0_kernel<T><<<h->vec_blocks(), 256, 0, st>>>(k, (const T*)r(), h->N / Vec<T>::W, h->at<double>(h->lay.partial_vec), h->sc());
             ++h->launches;
@@ -248,7 +249,7 @@ template <typename T> struct Seq {
         ++h->launches;
         return h->tab->row_inv2_cgf(&A, &h->tmap_row, st);
     }
-    bool sl() const { return !pcg && !classic && h->sl(); }
+    bool sl() const { return !pcg && !force && !classic && h->sl(); }
     cudaError_t iteration(const T* k, T* u) const {
         cudaError_t e;
         if (sl()) {
@@ -284,7 +285,7 @@ template <typename T>
 cudaError_t build_graph(fcg_handle h, GraphEntry& ge) {
     cudaError_t e;
     cudaStream_t cs = h->cap_stream;
-    Seq<T> s{h, cs}; s.pcg = (ge.pcg & 1) != 0;
+    Seq<T> s{h, cs}; s.pcg = (ge.pcg & 1) != 0; s.force = ge.force != 0; s.D = ge.D;
     const long long saved = h->launches;
     ge.graph = nullptr; ge.exec = nullptr;
     if ((e = cudaGraphCreate(&ge.graph, 0)) != cudaSuccess) return e;
@@ -330,9 +331,10 @@ cudaError_t build_graph(fcg_handle h, GraphEntry& ge) {
 }
 
 template <typename T>
-int solve_impl(fcg_handle h, const void* k, const void* f, void* u, double tol, int maxit, int* iters, double* relres, bool pcg = false) {
+int solve_impl(fcg_handle h, const void* k, const void* f, void* u, double tol, int maxit, int* iters, double* relres, bool pcg = false,
+               bool force = false, double D = 0.0) {
     h->launches = 0;
-    if (h->fused()) {
+    if (h->fused() && !force) {
         // small lattices: the whole solve is one cooperative kernel with the vectors resident in shared memory (fcg_fused.cuh)
         FusedArgs A{};
         A.mhat = pcg ? h->ws + h->lay.mhat : nullptr;
@@ -354,17 +356,18 @@ int solve_impl(fcg_handle h, const void* k, const void* f, void* u, double tol, 
         h->fused_opt = 0;
     }
     if (h->loop_mode == 0) {
-        const int var = h->v2() ? 100 + (h->sl() ? 1 : 0) : h->row_var();
+        const int var = h->v2() ? 100 + (h->sl() && !force ? 1 : 0) : h->row_var();
+        const int key = (pcg ? 1 : 0) + 2 * (h->colp() ? 1 : 0) + 4 * h->hints;
         GraphEntry* hit = nullptr;
         for (auto& g : h->graphs)
-            if (g.k == k && g.f == f && g.u == u && g.tol == tol && g.maxit == maxit && g.var == var && g.unroll == h->unroll && g.pdl == h->pdl && g.pcg == (pcg ? 1 : 0) + 2 * h->hints + 256 * (h->colp() ? 1 : 0)) { hit = &g; break; }
+            if (g.k == k && g.f == f && g.u == u && g.tol == tol && g.maxit == maxit && g.var == var && g.unroll == h->unroll && g.pdl == h->pdl && g.pcg == key && g.force == (force ? 1 : 0) && g.D == D) { hit = &g; break; }
         if (!hit) {
             if (h->graphs.size() >= 8) {
                 size_t lru = 0;
                 for (size_t i = 1; i < h->graphs.size(); ++i) if (h->graphs[i].stamp < h->graphs[lru].stamp) lru = i;
                 drop_graph(h->graphs[lru]); h->graphs.erase(h->graphs.begin() + lru);
             }
-            GraphEntry ge{k, f, u, tol, maxit, var, h->unroll, h->pdl, (pcg ? 1 : 0) + 2 * h->hints + 256 * (h->colp() ? 1 : 0), nullptr, nullptr, 0};
+            GraphEntry ge{k, f, u, tol, maxit, var, h->unroll, h->pdl, key, force ? 1 : 0, D, nullptr, nullptr, 0};
             cudaError_t e = build_graph<T>(h, ge);
             if (e != cudaSuccess) {
                 // conditional graph nodes unavailable: fall back to direct launches for the rest of this handle's life
@@ -384,12 +387,12 @@ int solve_impl(fcg_handle h, const void* k, const void* f, void* u, double tol, 
             FCG_CK(h, cudaGraphLaunch(hit->exec, h->stream));
             FCG_CK(h, cudaStreamSynchronize(h->stream));
             const long long U = hit->unroll;
-            Seq<T> sq{h, h->stream}; sq.pcg = pcg;
+            Seq<T> sq{h, h->stream}; sq.pcg = pcg; sq.force = force; sq.D = D;
             h->launches = sq.launches_outside_loop() + sq.launches_per_iteration() * U * ((h->h_sc->it + U - 1) / U);   // no-op kernels after the stop are launches too
         }
     }
     if (h->loop_mode != 0) {
-        Seq<T> s{h, h->stream}; s.pcg = pcg;
+        Seq<T> s{h, h->stream}; s.pcg = pcg; s.force = force; s.D = D;
         FCG_CK(h, s.init((const T*)k, (const T*)f, (T*)u, tol, maxit, false, 0ULL));
         FCG_CK(h, cudaMemcpyAsync(h->h_sc, h->sc(), sizeof(Scalars), cudaMemcpyDeviceToHost, h->stream));
         FCG_CK(h, cudaStreamSynchronize(h->stream));
@@ -407,10 +410,10 @@ int solve_impl(fcg_handle h, const void* k, const void* f, void* u, double tol, 
 }
 
 template <typename T>
-int break_impl(fcg_handle h, void* k, const void* u, const void* t, long long* index, double* ratio) {
+int break_impl(fcg_handle h, void* k, const void* u, const void* t, long long* index, double* ratio, void* fzero = nullptr) {
     break_argmax_kernel<T><<<h->vec_blocks(), 256, 0, h->stream>>>(
         (T*)k, (const T*)u, (const T*)t, (long long)h->N, h->at<double>(h->lay.brk_r), h->at<long long>(h->lay.brk_i),
-        h->at<unsigned int>(h->lay.brk_ticket), h->at<BreakResult>(h->lay.brk_out));
+        h->at<unsigned int>(h->lay.brk_ticket), h->at<BreakResult>(h->lay.brk_out), (T*)fzero);
     ++h->launches;
     FCG_CK(h, cudaGetLastError());
     FCG_CK(h, cudaMemcpyAsync(h->h_brk, h->at<BreakResult>(h->lay.brk_out), sizeof(BreakResult), cudaMemcpyDeviceToHost, h->stream));
@@ -455,8 +458,8 @@ int fft_impl(fcg_handle h, const void* in, void* out, bool inverse) {
 }
 
 template <typename T>
-int apply_impl(fcg_handle h, const void* k, const void* x, void* y) {
-    Seq<T> s{h, h->stream};
+int apply_impl(fcg_handle h, const void* k, const void* x, void* y, bool force = false) {
+    Seq<T> s{h, h->stream}; s.force = force;
     FCG_CK(h, s.row_fwd(ROWF_PLAIN, (const T*)x, nullptr));
     FCG_CK(h, s.col(COL_CONV, false));
     FCG_CK(h, s.row_inv(ROWI_APPLY, (const T*)k, (const T*)x, nullptr, (T*)y, nullptr));
@@ -542,6 +545,25 @@ int precond_impl(fcg_handle h, const void* s, double kbar) {
     FCG_CK(h, cudaGetLastError());
     FCG_CK(h, h->tab->spectrum_prep(h->at<void>(h->lay.z), h->at<void>(h->lay.mhat), h->spectrum_colpos, h->stream));
     FCG_CK(h, cudaStreamSynchronize(h->stream));
+    return FCG_OK;
+}
+
+// Force formulation, static part: eq. (1c) in closed form, and s = Re F G through the library's own transform
+template <typename T>
+int green_impl(fcg_handle h, double nu, double E, double a, void* G) {
+    green_function_kernel<T><<<h->vec_blocks(), 256, 0, h->stream>>>((T*)G, h->L, (1.0 - nu * nu) / (3.14159265358979323846 * E * a * a), a);
+    FCG_CK(h, cudaGetLastError());
+    return FCG_OK;
+}
+
+template <typename T>
+int kernel_spectrum_impl(fcg_handle h, const void* G, void* s) {
+    // half spectrum X[m][0..L/2] into r and p (adjacent in the workspace: (L/2+1) L complex <= 2 N reals; free between solves)
+    void* X = h->at<void>(h->lay.r);
+    int st = fft_impl<T>(h, G, X, false);
+    if (st != FCG_OK) return st;
+    halfspec_real_expand_kernel<T><<<h->vec_blocks(), 256, 0, h->stream>>>((const cx<T>*)X, (T*)s, h->L);
+    FCG_CK(h, cudaGetLastError());
     return FCG_OK;
 }
 
@@ -861,6 +883,64 @@ int fcg_pcg_fracture(fcg_handle h, void* k, const void* f, void* u, const void* 
                      long long* index_host, int* iters_host, int* steps_done_host) {
     if (h && !h->have_precond) return fail(h, FCG_NO_SPECTRUM, "fcg_set_preconditioner has not been called");
     return fracture_impl(h, k, f, u, t, nsteps, tol, maxit, index_host, iters_host, steps_done_host, true);
+}
+
+// ---- the paper's formulation in the bond forces, (I + K G) f = K D (eq. (2))
+int fcg_green_function(fcg_handle h, double nu, double E, double a, void* G) {
+    if (!h || !G) return fail(h, FCG_INVALID_ARG, "null argument");
+    if (!(E > 0.0) || !(a > 0.0) || !std::isfinite(nu) || !std::isfinite(E) || !std::isfinite(a)) return fail(h, FCG_INVALID_ARG, "E and a must be positive and finite, nu finite");
+    return h->dtype == FCG_F64 ? green_impl<double>(h, nu, E, a, G) : green_impl<float>(h, nu, E, a, G);
+}
+
+int fcg_kernel_spectrum(fcg_handle h, const void* G, void* s) {
+    if (!h || !G || !s) return fail(h, FCG_INVALID_ARG, "null argument");
+    if (G == s) return fail(h, FCG_INVALID_ARG, "s must not alias G");
+    static_assert(ALIGN % 16 == 0, "workspace alignment");
+    if (h->lay.p != h->lay.r + h->N * h->w) return fail(h, FCG_UNSUPPORTED, "workspace layout: r and p not adjacent");
+    return h->dtype == FCG_F64 ? kernel_spectrum_impl<double>(h, G, s) : kernel_spectrum_impl<float>(h, G, s);
+}
+
+int fcg_force_apply(fcg_handle h, const void* k, const void* x, void* y) {
+    if (!h || !k || !x || !y) return fail(h, FCG_INVALID_ARG, "null argument");
+    if (y == k || y == x) return fail(h, FCG_INVALID_ARG, "y must not alias k or x");
+    if (!h->have_spectrum) return fail(h, FCG_NO_SPECTRUM, "fcg_set_spectrum has not been called");
+    return h->dtype == FCG_F64 ? apply_impl<double>(h, k, x, y, true) : apply_impl<float>(h, k, x, y, true);
+}
+
+int fcg_force_solve(fcg_handle h, const void* k, double D, void* f, double tol, int maxit, int* iters_host, double* rel_residual_host) {
+    if (!h || !k || !f) return fail(h, FCG_INVALID_ARG, "null argument");
+    if (!(tol >= 0.0) || maxit < 0 || !std::isfinite(D)) return fail(h, FCG_INVALID_ARG, "tol must be >= 0, maxit >= 0, D finite");
+    if (!h->have_spectrum) return fail(h, FCG_NO_SPECTRUM, "fcg_set_spectrum has not been called");
+    return h->dtype == FCG_F64 ? solve_impl<double>(h, k, nullptr, f, tol, maxit, iters_host, rel_residual_host, false, true, D)
+                               : solve_impl<float>(h, k, nullptr, f, tol, maxit, iters_host, rel_residual_host, false, true, D);
+}
+
+int fcg_force_break_step(fcg_handle h, void* k, void* f, const void* t, long long* index_host, double* ratio_host) {
+    if (!h || !k || !f || !t) return fail(h, FCG_INVALID_ARG, "null argument");
+    h->launches = 0;
+    return h->dtype == FCG_F64 ? break_impl<double>(h, k, f, t, index_host, ratio_host, f)
+                               : break_impl<float>(h, k, f, t, index_host, ratio_host, f);
+}
+
+int fcg_force_fracture(fcg_handle h, void* k, double D, void* f, const void* t, int nsteps, double tol, int maxit,
+                       long long* index_host, int* iters_host, double* ratio_host, int* steps_done_host) {
+    if (!h || !k || !f || !t || nsteps < 0 || !index_host || !iters_host) return fail(h, FCG_INVALID_ARG, "bad argument");
+    long long total = 0; int done = 0, st = FCG_OK;
+    for (int step = 0; step < nsteps; ++step) {
+        int it = 0; double rr = 0.0;
+        st = fcg_force_solve(h, k, D, f, tol, maxit, &it, &rr);
+        total += h->launches;
+        if (st < 0) break;
+        long long idx = -1; double ratio = 0.0;
+        st = fcg_force_break_step(h, k, f, t, &idx, &ratio);
+        total += h->launches;
+        if (st < 0) break;
+        index_host[step] = idx; iters_host[step] = it; if (ratio_host) ratio_host[step] = ratio;
+        ++done; st = FCG_OK;
+    }
+    if (steps_done_host) *steps_done_host = done;
+    h->launches = total;
+    return st < 0 ? st : FCG_OK;
 }
 
 int fcg_profile_iteration(fcg_handle h, const void* k, const void* f, void* u, int iters, double* ms_host) {

@@ -770,6 +770,7 @@ __global__ void __launch_bounds__(AsyncShape<T, P>::INV_THREADS, CTAS) row_inv2_
     SmemIO<T, P> io{W};
     const int lt = threadIdx.x, lane = lt & 31, warp = lt >> 5;
     const int mode = PRE ? (int)ROWI_PRECOND : CGF ? (int)ROWI_CGF : A.mode;
+    const bool force = !PRE && !CGF && A.form != 0;
     tma::grid_dep_launch();
     const bool st_on = A.mode >= 0;                               // always true, opaque to the compiler (as in row_fwd2_kernel)
     const int nv = PRE ? 2 : CGF ? 6 : (mode == ROWI_PLAIN ? 0 : (mode == ROWI_RESID ? 6 : 4));
@@ -924,7 +925,8 @@ __global__ void __launch_bounds__(AsyncShape<T, P>::INV_THREADS, CTAS) row_inv2_
                         continue;
                     }
                     const T v0 = sl[2 * QV + j], v1 = sl[3 * QV + j];
-                    const T val0 = sl[j] * v0 + c0, val1 = sl[QV + j] * v1 + c1;         // k o x + C x
+                    const T val0 = force ? v0 + sl[j] * c0 : sl[j] * v0 + c0,            // k o x + C x, or the force
+                            val1 = force ? v1 + sl[QV + j] * c1 : sl[QV + j] * v1 + c1;  // formulation x + k o (G x) (eq. (2))
                     if constexpr (CGF) {
                         const T r0 = sl[4 * QV + j] - alpha * val0, r1 = sl[5 * QV + j] - alpha * val1;   // residue
                         if (st_on) { tma::st_hint(A.out + i0, r0, pol_r); tma::st_hint(A.out + i0 + L, r1, pol_r); }
@@ -935,7 +937,7 @@ __global__ void __launch_bounds__(AsyncShape<T, P>::INV_THREADS, CTAS) row_inv2_
                         continue;
                     }
                     if (mode == ROWI_RESID) {
-                        const T f0 = sl[4 * QV + j], f1 = sl[5 * QV + j];
+                        const T f0 = force ? sl[j] * A.dval : sl[4 * QV + j], f1 = force ? sl[QV + j] * A.dval : sl[5 * QV + j];   // form 1: f = K D
                         const T r0 = f0 - val0, r1 = f1 - val1;                           // r = f - A u
                         A.out[i0] = r0; A.out[i0 + L] = r1; A.out2[i0] = (T)0; A.out2[i0 + L] = (T)0;
                         acc[0] += (double)r0 * (double)r0; acc[0] += (double)r1 * (double)r1;

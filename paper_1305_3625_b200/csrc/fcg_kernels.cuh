@@ -293,9 +293,11 @@ __device__ __forceinline__ bool better(double ra, long long ia, double rb, long 
 }
 
 template <typename T>
-__global__ void __launch_bounds__(256) break_argmax_kernel(T* __restrict__ k, const T* __restrict__ u, const T* __restrict__ t,
+__global__ void __launch_bounds__(256) break_argmax_kernel(T* __restrict__ k, const T* u, const T* __restrict__ t,
                                                             long long n, double* pr, long long* pi, unsigned int* ticket,
-                                                            BreakResult* out) {
+                                                            BreakResult* out, T* fzero) {
+    // fzero != nullptr: force formulation (reading F2) -- u holds the bond forces, the ratio is f_i / t_i
+    // (one IEEE divide), and the broken bond's force is set to zero with its elastic constant (fzero == u)
     __shared__ double sr[32];
     __shared__ long long si[32];
     __shared__ int is_last;
@@ -304,7 +306,7 @@ __global__ void __launch_bounds__(256) break_argmax_kernel(T* __restrict__ k, co
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
         const T ki = k[i];
         if (!(ki > (T)0)) continue;
-        const double load = (double)ki * (double)u[i];      // l_i = k_i u_i   (one IEEE multiply)
+        const double load = fzero ? (double)u[i] : (double)ki * (double)u[i];      // l_i = k_i u_i   (one IEEE multiply)
         const double rt = load / (double)t[i];              // l_i / t_i       (one IEEE divide)
         if (rt != rt) continue;
         consider(rt, i);
@@ -345,6 +347,35 @@ __global__ void __launch_bounds__(256) break_argmax_kernel(T* __restrict__ k, co
         *ticket = 0u;
         out->index = bi; out->ratio = br; out->status = bi < 0 ? -6 : 0;
         if (bi >= 0) k[bi] = (T)0;
+        if (bi >= 0 && fzero) fzero[bi] = (T)0;
+    }
+}
+
+// ------------------------------------------------------------------------------- force formulation: static kernel
+// Real-space Green's function of eq. (1c): G = (1 - nu^2)/(pi E a^2) * integral of 1/r over the a x a square of the
+// other bond, in closed form (four-corner sum of x asinh(y/|x|) + y asinh(x/|y|)), minimum-image offsets on the periodic lattice
+// (reading F3).  Evaluated in double, rounded once to T.  One thread per offset.
+__device__ __forceinline__ double green_corner(double x, double y) { return x * asinh(y / fabs(x)) + y * asinh(x / fabs(y)); }
+
+template <typename T>
+__global__ void __launch_bounds__(256) green_function_kernel(T* __restrict__ G, int L, double pref, double a) {
+    const double hf = 0.5 * a;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < (long long)L * L; i += (long long)gridDim.x * blockDim.x) {
+        const int da = (int)(i / L), db = (int)(i % L);
+        const double X = a * (double)(da <= L / 2 ? da : da - L), Y = a * (double)(db <= L / 2 ? db : db - L);
+        const double I = green_corner(X + hf, Y + hf) - green_corner(X - hf, Y + hf) - green_corner(X + hf, Y - hf) + green_corner(X - hf, Y - hf);
+        G[i] = (T)(pref * I);
+    }
+}
+
+// s[m][n] = Re X[m][n] over the full L x L plane from the half spectrum X[m][0..L/2] of a real field (X[-m,-n] = conj X[m,n]):
+// "the FFT of G is static and performed during initialization"; the imaginary part is dropped like cpyReal does.
+template <typename T>
+__global__ void __launch_bounds__(256) halfspec_real_expand_kernel(const cx<T>* __restrict__ X, T* __restrict__ s, int L) {
+    const int W = L / 2 + 1;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < (long long)L * L; i += (long long)gridDim.x * blockDim.x) {
+        const int m = (int)(i / L), n = (int)(i % L);
+        s[i] = n <= L / 2 ? X[(size_t)m * W + n].x : X[(size_t)((L - m) % L) * W + (L - n)].x;
     }
 }
 

@@ -80,6 +80,9 @@ template <typename T> struct RowInvArgs {
     int pdl;
     int hints;
     const double* colsum;                 // CGF: the column pass's L/2 partial sums of shat |P|^2
+    int form;                             // 0: A x = k o x + C x (BASELINE.json);  1: force formulation B x = x + k o (C x), the left side
+                                          //    of eq. (2), PAPER.md:74 (CG, RESID, APPLY)
+    T dval;                               // form 1, RESID: right-hand side b = k * dval (K D of eq. (2)); f is not read
 };
 
 template <int A, int B, typename F> FCG_HD void static_for_up(F&& f) {
@@ -329,10 +332,10 @@ FCG_HD void row_inv_body(const RowInvArgs<T>& A, int block, cx<T>* smem, Runner&
             if (A.mode == ROWI_PRECOND) {                          // z = M^-1 r, r.z  (PCG; k = r)
                 A.out[i] = c; acc[0] += (double)A.k[i] * (double)c; return;
             }
-            const T vi = A.v[i];
-            const T val = A.k[i] * vi + c;                         // k o x + C x
+            const T vi = A.v[i], ki = A.k[i];
+            const T val = A.form ? vi + ki * c : ki * vi + c;      // k o x + C x, or x + k o (G x) (eq. (2))
             if (A.mode == ROWI_RESID) {
-                const T fi = A.f[i], ri = fi - val;                // r = f - A u
+                const T fi = A.form ? ki * A.dval : A.f[i], ri = fi - val;   // r = f - A u;  form 1: f = K D
                 A.out[i] = ri; A.out2[i] = (T)0;
                 acc[0] += (double)ri * (double)ri; acc[1] += (double)fi * (double)fi;
             } else {

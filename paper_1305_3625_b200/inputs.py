@@ -120,6 +120,9 @@ def precond_kbar(k: np.ndarray) -> float:
 # Constants of eq. (1c): the paper gives no values, these are the recipe's (reading F4).
 GREEN_NU, GREEN_E, GREEN_A = 0.3, 1.0, 1.0
 FORCE_KAPPA, FORCE_D = 1.0, 1.0
+# Stopping tolerance of the force recipe: two converged CG runs differ by up to cond(I + K G) * tol in f, and cond ~ 0.7 L here
+# (eigenvalues between 1 + kappa g_min ~ 1.5 and 1 + kappa g(0) ~ 1 + L), so a 1e-9 comparison needs tol well below 1e-9 / L.
+FORCE_TOL = {np.dtype(np.float64): 1e-12, np.dtype(np.float32): 1e-5}
 
 
 def gradient_thresholds(L: int, gradient: float, seed: int = SEED_T) -> np.ndarray:
