@@ -261,6 +261,62 @@ def bench_extras(binding, torch, inputs):
                                                     "iterations": sum(int(r[1].sum()) for r in res)}
         for h, *_ in reps:
             h.close()
+    out.update(bench_force(binding, torch, inputs))
+    return out
+
+
+def bench_force(binding, torch, inputs):
+    """The paper's own formulation in the bond forces: the static chain
+    eq. (1c) -> g = Re F G on the device, CG on (I + K G) f = K D at L = 2048 (one bond in 20 broken, tol 1e-12 fp64 / 1e-5 fp32),
+    and the quasi-static loop in the forces at L = 256 (threshold gradient 1.0, 500 break steps)."""
+    out = {}
+    to = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    for L, dt, tdt, name in ((2048, np.float64, torch.float64, "f64"), (2048, np.float32, torch.float32, "f32")):
+        h = binding.Fcg(L, tdt)
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+        G = h.fcg_green_function(inputs.GREEN_NU, inputs.GREEN_E, inputs.GREEN_A); g = h.fcg_kernel_spectrum(G)     # warm
+        torch.cuda.synchronize()
+        ev[0].record(); h.fcg_green_function(inputs.GREEN_NU, inputs.GREEN_E, inputs.GREEN_A, G)
+        ev[1].record(); h.fcg_kernel_spectrum(G, g)
+        ev[2].record(); torch.cuda.synchronize()
+        h.fcg_set_spectrum(g)
+        k = to(inputs.force_k(L, 20).astype(dt)); f = torch.zeros((L, L), dtype=tdt, device="cuda")
+        tol = inputs.FORCE_TOL[np.dtype(dt)]
+        for _ in range(2):
+            f.zero_(); h.fcg_force_solve(k, inputs.FORCE_D, f, tol, 2000)
+        reps = 5
+        sev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(reps)]
+        for a, b in sev:
+            f.zero_(); a.record()
+            it, rr, st = h.fcg_force_solve(k, inputs.FORCE_D, f, tol, 2000)
+            b.record()
+        torch.cuda.synchronize()
+        ms = statistics.median(a.elapsed_time(b) for a, b in sev)
+        nw = L * L * np.dtype(dt).itemsize
+        launches = h.fcg_last_launch_count()
+        per_it = round((launches - 4) / max(it, 1))      # the set-up (residual pass) and finish kernels are not per-iteration
+        b_nw = 13.5 if per_it == 3 else 15.5             # DESIGN.md sections 4, 12: three launches never store q
+        out[f"force_solve_L{L}_{name}"] = {
+            "iterations": it, "status": st, "final_rel_residual": rr, "ms_per_solve": ms, "us_per_iteration": 1e3 * ms / max(it, 1),
+            "launches_per_solve": launches, "launches_per_iteration": per_it,
+            "iteration_gbs": b_nw * nw / (1e-3 * ms / max(it, 1)) / 1e9, "bytes_per_iteration_Nw": b_nw,
+            "green_function_us": 1e3 * ev[0].elapsed_time(ev[1]), "kernel_spectrum_us": 1e3 * ev[1].elapsed_time(ev[2])}
+        h.close()
+    L, nsteps = 256, 500
+    h = binding.Fcg(L, torch.float64)
+    h.fcg_set_spectrum(h.fcg_kernel_spectrum(h.fcg_green_function(inputs.GREEN_NU, inputs.GREEN_E, inputs.GREEN_A)))
+    t = to(inputs.gradient_thresholds(L, 1.0))
+    best = None
+    for rep in range(2):
+        k = to(inputs.force_k(L)); f = torch.zeros((L, L), dtype=torch.float64, device="cuda")
+        torch.cuda.synchronize(); t0 = time.perf_counter()
+        index, iters, ratio, done, st = h.fcg_force_fracture(k, inputs.FORCE_D, f, t, nsteps, 1e-12, 1000)
+        dt_s = time.perf_counter() - t0
+        best = dt_s if best is None else min(best, dt_s)
+    out["force_fracture_L256_f64"] = {"steps": int(done), "iterations": int(iters.sum()), "wall_s": best, "steps_per_s": int(done) / best,
+                                      "us_per_iteration": 1e6 * best / max(int(iters.sum()), 1), "status": int(st),
+                                      "launches": h.fcg_last_launch_count()}
+    h.close()
     return out
 
 
@@ -286,7 +342,7 @@ def main():
     ap.add_argument("--impl", choices=["fcg", "reference"], default="fcg")
     ap.add_argument("--ref-iters", type=int, default=8, help="oracle CG iterations per reference step / cpu_baseline sample")
     ap.add_argument("--full", action="store_true", help="also time configs[2] fp32 and configs[4] (reported under 'extra')")
-    ap.add_argument("--solver", choices=["cg", "pcg"], default="cg",
+    ap.add_argument("--solver", choices=["cg", "pcg", "force"], default="cg",
                     help="pcg: time fcg_pcg_solve instead (metric pcg_iterations_per_s, 22 N w bytes per iteration; no e2e leg) -- "
                          "for profiling the PCG kernels; the headline BASELINE.json names is the default")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -325,8 +381,49 @@ def main():
     torch.cuda.synchronize()
     if sampler:
         sampler.start()
-    res = bench_workload(binding, torch, w, args.steps, args.warmup, loop_mode=args.loop_mode, solver=args.solver, inputs_mod=inputs)
-    clocks = sampler.stop() if sampler else None
+    res = None
+    if args.solver != "force":
+        res = bench_workload(binding, torch, w, args.steps, args.warmup, loop_mode=args.loop_mode, solver=args.solver, inputs_mod=inputs)
+        clocks = sampler.stop() if sampler else None
+    if args.solver == "force":
+        # profiling mode for the force formulation: CG on (I + K G) f = K D at L = 2048, one bond in 20 broken
+        if world > 1:
+            raise SystemExit("--solver force is a single-GPU profiling mode")
+        tdt = torch.float64 if args.dtype == "f64" else torch.float32
+        L = 2048
+        h = binding.Fcg(L, tdt)
+        h.fcg_set_option(binding.FCG_OPT_LOOP_MODE, args.loop_mode)
+        h.fcg_set_spectrum(h.fcg_kernel_spectrum(h.fcg_green_function(inputs.GREEN_NU, inputs.GREEN_E, inputs.GREEN_A)))
+        k = torch.from_numpy(inputs.force_k(L, 20).astype(w.dtype)).cuda(); f = torch.zeros((L, L), dtype=tdt, device="cuda")
+        tol = inputs.FORCE_TOL[np.dtype(w.dtype)]
+        for _ in range(args.warmup):
+            f.zero_(); h.fcg_force_solve(k, inputs.FORCE_D, f, tol, 2000)
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+        its, launches = 0, 0
+        for a, b in ev:
+            f.zero_(); a.record()
+            it, rr, st = h.fcg_force_solve(k, inputs.FORCE_D, f, tol, 2000)
+            b.record(); its += it; launches += h.fcg_last_launch_count()
+        torch.cuda.synchronize()
+        clocks = sampler.stop() if sampler else None
+        ms = sum(a.elapsed_time(b) for a, b in ev)
+        nw = L * L * wbytes
+        per_it = h.fcg_last_launch_count() // max(it, 1)
+        b_iter = 13.5 if per_it == 3 else 15.5
+        t_iter_us = 1e3 * ms / max(its, 1)
+        ach = b_iter * nw / (t_iter_us * 1e-6) / 1e9
+        print(json.dumps({
+            "metric": "force_cg_iterations_per_s", "value": its / (ms * 1e-3), "unit": UNIT, "n_gpus": 1, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": args.dtype, "data": "synthetic",
+            "config": {"workload": f"force formulation (I + K G) f = K D, L={L} {args.dtype}, 1/20 of the bonds broken, tol={tol:g} ({it} iterations)",
+                       "launches_per_iteration": per_it},
+            "us_per_iteration": t_iter_us,
+            "roofline": {"bound": "hbm", "kernel": "whole iteration", "achieved": ach, "peak": hbm_peak, "unit": "GB/s", "frac": ach / hbm_peak,
+                         "traffic": None, "algorithmic_bytes_per_launch": b_iter * nw, "peak_source": peak_src},
+            "gpu_launches": launches, "clocks": clocks, "final_rel_residual": rr, "status": st}))
+        h.close()
+        return
     if args.solver == "pcg":
         if world > 1:
             raise SystemExit("--solver pcg is a single-GPU profiling mode")

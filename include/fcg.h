@@ -203,7 +203,8 @@ int fcg_fracture_end(fcg_handle h, long long* index_host, int* iters_host, int* 
  *                        f in: initial guess (0 on broken bonds), out: forces; stop at the first iteration with
  *                        ||r||_2 <= tol ||b||_2; iters / rel_residual / status / scalars in double / determinism as fcg_solve.
  *                        k == 0 everywhere or D == 0 gives f = 0, 0 iterations.  One CUDA graph per solve, four launches
- *                        per iteration (the textbook order; the spectral search length of fcg_solve is not used).  Blocks.
+ *                        per iteration (the textbook order; the spectral search length of fcg_solve is not used); at L = 256
+ *                        and 512 one cooperative launch for the whole solve, as fcg_solve (FCG_OPT_FUSED).  Blocks.
  *   fcg_force_break_step reading F2: the response is linear in D, so the bond that reaches its threshold first is
  *                        argmax over {k_i > 0} of f_i / t_i (one IEEE divide in double; ties -> lowest i; NaN skipped);
  *                        sets k_i = 0 AND f_i = 0 (a broken bond carries nothing).  ratio_host = the winning f/t: with f
@@ -211,7 +212,10 @@ int fcg_fracture_end(fcg_handle h, long long* index_host, int* iters_host, int* 
  *   fcg_force_fracture   nsteps times { fcg_force_solve warm-started from the current f; fcg_force_break_step } ("For each
  *                        step in the simulation, the displacement is set, and the resulting distribution of forces is
  *                        calculated ... bonds break").  index_host, iters_host, ratio_host (may be NULL): HOST
- *                        arrays of nsteps; stops early on a negative status; steps_done_host = completed steps. */
+ *                        arrays of nsteps; stops early on a negative status; steps_done_host = completed steps.
+ *                        At L = 256 and 512 the whole loop -- every solve and every break step -- is ONE cooperative launch
+ *                        with k, f, t resident in shared memory (fcg_fused.cuh, FORCE variant); else one graph per solve
+ *                        and one break kernel per step, driven from the host.  Blocks. */
 int fcg_green_function(fcg_handle h, double nu, double E, double a, void* G);
 int fcg_kernel_spectrum(fcg_handle h, const void* G, void* s);
 int fcg_force_apply(fcg_handle h, const void* k, const void* x, void* y);

@@ -92,7 +92,7 @@ struct fcg_handle_s {
     Scalars* h_sc = nullptr;            // pinned
     BreakResult* h_brk = nullptr;       // pinned
     void *hk = nullptr, *hf = nullptr, *hu = nullptr;   // device staging of fcg_solve_host
-    long long* frac_idx = nullptr; int* frac_it = nullptr; int frac_cap = 0;   // device results of the fused quasi-static loop
+    long long* frac_idx = nullptr; int* frac_it = nullptr; double* frac_ratio = nullptr; int frac_cap = 0;   // device results of the fused quasi-static loop
     int pend_nsteps = -1, pend_done = 0, pend_status = 0; bool pend_async = false;   // fcg_fracture_begin / _end
     std::vector<long long> pend_idx; std::vector<int> pend_it;
     std::vector<GraphEntry> graphs; unsigned long long stamp = 0;
@@ -334,10 +334,11 @@ template <typename T>
 int solve_impl(fcg_handle h, const void* k, const void* f, void* u, double tol, int maxit, int* iters, double* relres, bool pcg = false,
                bool force = false, double D = 0.0) {
     h->launches = 0;
-    if (h->fused() && !force) {
+    if (h->fused() && !(force && pcg)) {
         // small lattices: the whole solve is one cooperative kernel with the vectors resident in shared memory (fcg_fused.cuh)
         FusedArgs A{};
         A.mhat = pcg ? h->ws + h->lay.mhat : nullptr;
+        A.form = force ? 1 : 0; A.D = D;
         A.k = k; A.f = f; A.u = u; A.Tf = h->ws + h->lay.Tb; A.shat = h->ws + h->lay.shat; A.tw = h->ws + h->lay.tw;
         A.partial = h->at<double>(h->lay.partial_row); A.counter = &h->sc()->ticket[3]; A.sc = h->sc(); A.tol = tol; A.maxit = maxit;
         FCG_CK(h, cudaMemsetAsync(h->sc(), 0, sizeof(Scalars), h->stream));
@@ -678,6 +679,7 @@ int fcg_destroy(fcg_handle h) {
     if (h->hu) cudaFree(h->hu);
     if (h->frac_idx) cudaFree(h->frac_idx);
     if (h->frac_it) cudaFree(h->frac_it);
+    if (h->frac_ratio) cudaFree(h->frac_ratio);
     cudaGetLastError();
     delete h;
     return FCG_OK;
@@ -787,6 +789,20 @@ int fcg_break_step(fcg_handle h, void* k, const void* u, const void* t, long lon
                                : break_impl<float>(h, k, u, t, index_host, ratio_host);
 }
 
+// device arrays for the per-step results of the fused quasi-static loops
+static int frac_reserve(fcg_handle h, int nsteps) {
+    if (h->frac_cap >= nsteps) return FCG_OK;
+    if (h->frac_idx) cudaFree(h->frac_idx);
+    if (h->frac_it) cudaFree(h->frac_it);
+    if (h->frac_ratio) cudaFree(h->frac_ratio);
+    h->frac_idx = nullptr; h->frac_it = nullptr; h->frac_ratio = nullptr; h->frac_cap = 0;
+    FCG_CK(h, cudaMalloc((void**)&h->frac_idx, (size_t)nsteps * sizeof(long long)));
+    FCG_CK(h, cudaMalloc((void**)&h->frac_it, (size_t)nsteps * sizeof(int)));
+    FCG_CK(h, cudaMalloc((void**)&h->frac_ratio, (size_t)nsteps * sizeof(double)));
+    h->frac_cap = nsteps;
+    return FCG_OK;
+}
+
 // Quasi-static loop in two halves, so that one host thread can keep several handles (streams) busy: begin enqueues (and, where the
 // loop is one cooperative kernel, returns at once); end blocks and hands out the results.
 static int fracture_begin(fcg_handle h, void* k, const void* f, void* u, const void* t, int nsteps, double tol, int maxit, bool pcg) {
@@ -795,14 +811,7 @@ static int fracture_begin(fcg_handle h, void* k, const void* f, void* u, const v
     h->pend_nsteps = -1; h->pend_async = false; h->pend_done = 0; h->pend_status = FCG_OK;
     if (h->fused() && h->have_spectrum && nsteps > 0 && tol >= 0.0 && maxit >= 0) {
         // small lattices: the whole quasi-static loop -- every solve and every break step -- is one cooperative kernel
-        if (h->frac_cap < nsteps) {
-            if (h->frac_idx) cudaFree(h->frac_idx);
-            if (h->frac_it) cudaFree(h->frac_it);
-            h->frac_idx = nullptr; h->frac_it = nullptr; h->frac_cap = 0;
-            FCG_CK(h, cudaMalloc((void**)&h->frac_idx, (size_t)nsteps * sizeof(long long)));
-            FCG_CK(h, cudaMalloc((void**)&h->frac_it, (size_t)nsteps * sizeof(int)));
-            h->frac_cap = nsteps;
-        }
+        { const int e0 = frac_reserve(h, nsteps); if (e0 != FCG_OK) return e0; }
         FusedArgs A{};
         A.k = k; A.f = f; A.u = u; A.Tf = h->ws + h->lay.Tb; A.shat = h->ws + h->lay.shat; A.tw = h->ws + h->lay.tw;
         A.partial = h->at<double>(h->lay.partial_row); A.counter = &h->sc()->ticket[3]; A.sc = h->sc(); A.tol = tol; A.maxit = maxit;
@@ -925,6 +934,37 @@ int fcg_force_break_step(fcg_handle h, void* k, void* f, const void* t, long lon
 int fcg_force_fracture(fcg_handle h, void* k, double D, void* f, const void* t, int nsteps, double tol, int maxit,
                        long long* index_host, int* iters_host, double* ratio_host, int* steps_done_host) {
     if (!h || !k || !f || !t || nsteps < 0 || !index_host || !iters_host) return fail(h, FCG_INVALID_ARG, "bad argument");
+    if (!(tol >= 0.0) || maxit < 0 || !std::isfinite(D)) return fail(h, FCG_INVALID_ARG, "tol must be >= 0, maxit >= 0, D finite");
+    if (!h->have_spectrum) return fail(h, FCG_NO_SPECTRUM, "fcg_set_spectrum has not been called");
+    if (h->fused() && nsteps > 0) {
+        // small lattices: every solve and every break step of the loop in one cooperative kernel (fcg_fused.cuh, FORCE variant)
+        { const int e0 = frac_reserve(h, nsteps); if (e0 != FCG_OK) return e0; }
+        FusedArgs A{};
+        A.form = 1; A.D = D; A.k = k; A.f = nullptr; A.u = f; A.Tf = h->ws + h->lay.Tb; A.shat = h->ws + h->lay.shat; A.tw = h->ws + h->lay.tw;
+        A.partial = h->at<double>(h->lay.partial_row); A.counter = &h->sc()->ticket[3]; A.sc = h->sc(); A.tol = tol; A.maxit = maxit;
+        A.nsteps = nsteps; A.t = t; A.k_out = k; A.out_index = h->frac_idx; A.out_iters = h->frac_it; A.out_ratio = h->frac_ratio;
+        A.brk_r = h->at<double>(h->lay.brk_r); A.brk_i = h->at<long long>(h->lay.brk_i);
+        FCG_CK(h, cudaMemsetAsync(h->sc(), 0, sizeof(Scalars), h->stream));
+        cudaError_t e = h->tab->fused_solve(&A, h->stream);
+        if (e == cudaSuccess) {
+            FCG_CK(h, cudaMemcpyAsync(h->h_sc, h->sc(), sizeof(Scalars), cudaMemcpyDeviceToHost, h->stream));
+            FCG_CK(h, cudaStreamSynchronize(h->stream));
+            h->launches = 1;
+            const int done = h->h_sc->steps_done;
+            if (done > 0) {
+                FCG_CK(h, cudaMemcpyAsync(index_host, h->frac_idx, (size_t)done * sizeof(long long), cudaMemcpyDeviceToHost, h->stream));
+                FCG_CK(h, cudaMemcpyAsync(iters_host, h->frac_it, (size_t)done * sizeof(int), cudaMemcpyDeviceToHost, h->stream));
+                if (ratio_host) FCG_CK(h, cudaMemcpyAsync(ratio_host, h->frac_ratio, (size_t)done * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+                FCG_CK(h, cudaStreamSynchronize(h->stream));
+            }
+            if (steps_done_host) *steps_done_host = done;
+            if (h->h_sc->status == FCG_CUDA_ERROR) h->err = "fused quasi-static loop: grid barrier timed out";
+            return h->h_sc->status < 0 ? h->h_sc->status : FCG_OK;
+        }
+        cudaGetLastError();
+        h->err = std::string("cooperative launch failed (") + cudaGetErrorString(e) + "); using the graph path";
+        h->fused_opt = 0;
+    }
     long long total = 0; int done = 0, st = FCG_OK;
     for (int step = 0; step < nsteps; ++step) {
         int it = 0; double rr = 0.0;

@@ -34,6 +34,9 @@ struct FusedArgs {
     // quasi-static loop (nsteps > 0): thresholds, k written back, per-step results, arg-max scratch (G entries each)
     int nsteps; const void* t; void* k_out; long long* out_index; int* out_iters; double* brk_r; long long* brk_i;
     const void* mhat;                           // preconditioned CG: stored spectrum of M^-1, or nullptr for plain CG
+    // force formulation (I + K G) f = K D (eq. (2)): u holds the bond forces, f is not read
+    // (b = k * D is formed in shared memory), out_ratio[step] = the winning f/t of the break step (may be nullptr)
+    int form; double D; double* out_ratio;
 };
 
 template <typename T, typename P> struct FusedShape {
@@ -72,7 +75,10 @@ __device__ __forceinline__ bool grid_barrier(unsigned int* counter, unsigned int
     return *ok_smem != 0;
 }
 
-template <typename T, typename P>
+// FORCE: the paper's own system in the bond forces, in the textbook order of Listing 2 (q = (I + K G) p is formed and kept, p.q is a
+// dot product, then u and r are updated: one more grid barrier per iteration than the spectral search length of the displacement
+// form, which would need k o p = kappa p, i.e. reading F1, to hold exactly) -- the same arithmetic as the oracle for any k.
+template <typename T, typename P, bool FORCE = false>
 __global__ void __launch_bounds__(P::NT) cg_fused_kernel(const FusedArgs A)
 {
     using AS = AsyncShape<T, P>;
@@ -303,7 +309,8 @@ __global__ void __launch_bounds__(P::NT) cg_fused_kernel(const FusedArgs A)
     for (int j = 0; j < TPC; ++j) {
         const size_t row0 = (size_t)(2 * (cta + j * G)) * L;
         for (int e = lt; e < 2 * L; e += NT) {         // the two rows are adjacent in memory
-            V(j, 0, 0)[e] = gk[row0 + e]; V(j, 1, 0)[e] = gf[row0 + e]; V(j, 2, 0)[e] = gu[row0 + e];
+            V(j, 0, 0)[e] = gk[row0 + e]; V(j, 2, 0)[e] = gu[row0 + e];
+            if (!FORCE) V(j, 1, 0)[e] = gf[row0 + e];
             if (frac) V(j, 6, 0)[e] = static_cast<const T*>(A.t)[row0 + e];
         }
     }
@@ -313,7 +320,8 @@ __global__ void __launch_bounds__(P::NT) cg_fused_kernel(const FusedArgs A)
     // a stack frame, and 17.7 instead of 12.4 us per iteration at L = 256):
     //   FN (once per launch: ||f||^2) -> RESID (r = f - A u, r.r) -> [Z (z = M^-1 r, r.z)] -> Q (p, A p, alpha, u, r, r.r) -> [Z] -> Q -> ..
     // Z only for preconditioned CG; z lives in the slot that used to hold q (q is consumed as it is formed).
-    enum { PH_FN = 0, PH_RESID = 1, PH_Z = 2, PH_Q = 3 };
+    // FORCE: .. -> Q (p, q = p + k o G p, p.q) -> U (alpha, u, r, r.r) -> Q -> ..; ||b||^2 once per solve (b = K D changes with k).
+    enum { PH_FN = 0, PH_RESID = 1, PH_Z = 2, PH_Q = 3, PH_U = 4 };
     bool ok = true, okb = true, have_fn = false;
     int it = 0, status = ST_OK, steps_done = 0;
     double rho = 0.0, fn2 = 0.0, rr = 0.0;         // rho = r.r (CG) or r.z (PCG); rr = r.r
@@ -327,9 +335,18 @@ __global__ void __launch_bounds__(P::NT) cg_fused_kernel(const FusedArgs A)
             T* pp = V(j, 4, 0);
             for (int e = lt; e < 2 * L; e += NT) pp[e] = (T)0;
         }
+        if (FORCE) {                                   // right-hand side b = K D (eq. (2)), one multiply in the working precision
+            const T dv = (T)A.D;
+            for (int j = 0; j < TPC; ++j) {
+                const T* kk = V(j, 0, 0); T* bb = V(j, 1, 0);
+                for (int e = lt; e < 2 * L; e += NT) bb[e] = kk[e] * dv;
+            }
+            __syncthreads();
+        }
         it = 0; status = ST_OK; zero_u = false;
         double beta = 0.0;
-        int phase = have_fn ? PH_RESID : PH_FN;
+        T al_u = (T)0;                                 // FORCE: the search length between phases Q and U
+        int phase = (have_fn && !FORCE) ? PH_RESID : PH_FN;
         while (true) {
             double acc = 0.0, kpp = 0.0;
             bool bd = false;
@@ -350,21 +367,31 @@ __global__ void __launch_bounds__(P::NT) cg_fused_kernel(const FusedArgs A)
                     }
                 }
                 __syncthreads();
+            } else if (FORCE && phase == PH_U) {        // new x (95), residue (96), residue length (97)
+                for (int j = 0; j < TPC; ++j) {
+                    T* uu = V(j, 2, 0); T* rv = V(j, 3, 0); const T* pp = V(j, 4, 0); const T* qq = V(j, 5, 0);
+                    for (int e = lt; e < 2 * L; e += NT) {
+                        uu[e] = uu[e] + al_u * pp[e];
+                        const T rn = rv[e] - al_u * qq[e];
+                        rv[e] = rn;
+                        acc += (double)rn * (double)rn;
+                    }
+                }
             }
             // ---- operator-shaped round trip: C u (RESID), C p (Q: A * p) or M^-1 r (Z)
-            if (phase != PH_FN) {
+            if (phase != PH_FN && !(FORCE && phase == PH_U)) {
                 rows_forward(phase == PH_RESID ? 2 : (phase == PH_Q ? 4 : 3));
                 ok = grid_barrier(A.counter, target, G, &ok_smem) && ok;
                 double en = 0.0;
-                columns(phase == PH_Z ? mhat : shat, phase == PH_Q ? &en : nullptr);
+                columns(phase == PH_Z ? mhat : shat, (!FORCE && phase == PH_Q) ? &en : nullptr);
                 double* ps = A.partial + (size_t)slot * G;
-                if (phase == PH_Q) {                    // this CTA's share of p.Ap = sum k p^2 + sum shat |P|^2, published before the barrier
+                if (!FORCE && phase == PH_Q) {                    // this CTA's share of p.Ap = sum k p^2 + sum shat |P|^2, published before the barrier
                     const double mine = cta_sum(kpp + en);
                     if (lt == 0) ps[cta] = mine;
                 }
                 ok = grid_barrier(A.counter, target, G, &ok_smem) && ok;
                 T al = (T)0;
-                if (phase == PH_Q) {                    // search length (94): every CTA adds the G shares in the same order
+                if (!FORCE && phase == PH_Q) {          // search length (94): every CTA adds the G shares in the same order
                     double v = 0.0;
                     for (int i = lt; i < G; i += NT) v += __ldcg(ps + i);
                     slot = (slot + 1) & 3;
@@ -373,11 +400,18 @@ __global__ void __launch_bounds__(P::NT) cg_fused_kernel(const FusedArgs A)
                     else al = (T)(rho / pq);
                 }
                 if (!bd) rows_inverse([&](int j, int e, T c0, T c1) {
-                    if (phase == PH_RESID) {                                  // r = f - (k o u + C u)
+                    if (phase == PH_RESID) {                                  // r = f - (k o u + C u);  FORCE: r = b - (u + k o G u)
                         const T* kk = V(j, 0, 0); const T* ff = V(j, 1, 0); const T* uu = V(j, 2, 0); T* rv = V(j, 3, 0);
-                        const T r0 = ff[e] - (kk[e] * uu[e] + c0), r1 = ff[L + e] - (kk[L + e] * uu[L + e] + c1);
+                        const T r0 = ff[e] - (FORCE ? uu[e] + kk[e] * c0 : kk[e] * uu[e] + c0),
+                                r1 = ff[L + e] - (FORCE ? uu[L + e] + kk[L + e] * c1 : kk[L + e] * uu[L + e] + c1);
                         rv[e] = r0; rv[L + e] = r1;
                         acc += (double)r0 * (double)r0; acc += (double)r1 * (double)r1;
+                    } else if (FORCE && phase == PH_Q) {                      // q = p + k o (G p) (eq. (2)), kept; p.q
+                        const T* kk = V(j, 0, 0); const T* pp = V(j, 4, 0); T* qq = V(j, 5, 0);
+                        const T p0 = pp[e], p1 = pp[L + e];
+                        const T q0 = p0 + kk[e] * c0, q1 = p1 + kk[L + e] * c1;
+                        qq[e] = q0; qq[L + e] = q1;
+                        acc += (double)p0 * (double)q0; acc += (double)p1 * (double)q1;
                     } else if (phase == PH_Q) {         // q = k o p + C p; new x (95), residue (96), residue length (97)
                         const T* kk = V(j, 0, 0); const T* pp = V(j, 4, 0); T* uu = V(j, 2, 0); T* rv = V(j, 3, 0);
                         const T p0 = pp[e], p1 = pp[L + e];
@@ -408,7 +442,11 @@ __global__ void __launch_bounds__(P::NT) cg_fused_kernel(const FusedArgs A)
                 if (!(s0 > 0.0) || !isfinite(s0)) { status = ST_BREAKDOWN; break; }
                 beta = it == 0 ? 0.0 : s0 / rho;
                 rho = s0; phase = PH_Q;
+            } else if (FORCE && phase == PH_Q) {        // search length (94): a dot product, as the oracle forms it
+                if (!(s0 > 0.0) || !isfinite(s0)) { status = ST_BREAKDOWN; break; }
+                al_u = (T)(rho / s0); phase = PH_U;
             } else {
+                if (FORCE) phase = PH_Q;
                 rr = s0; ++it;
                 if (sqrt(rr) <= A.tol * sqrt(fn2)) { if (!pcg) rho = rr; break; }                 // check convergence (99)
                 if (it >= A.maxit) { if (!pcg) rho = rr; status = ST_NOT_CONVERGED; break; }
@@ -434,7 +472,7 @@ __global__ void __launch_bounds__(P::NT) cg_fused_kernel(const FusedArgs A)
             for (int e = lt; e < 2 * L; e += NT) {
                 const T ki = kk[e];
                 if (!(ki > (T)0)) continue;
-                const double load = (double)ki * (double)uu[e];
+                const double load = FORCE ? (double)uu[e] : (double)ki * (double)uu[e];      // FORCE (reading F2): f_i / t_i
                 const double rt = load / (double)tt[e];
                 if (rt != rt) continue;
                 if (better(rt, row0 + e, br, bi)) { br = rt; bi = row0 + e; }
@@ -453,9 +491,15 @@ __global__ void __launch_bounds__(P::NT) cg_fused_kernel(const FusedArgs A)
         if (bi < 0) { status = -6; break; }                                   // FCG_NO_CANDIDATE
         {
             const int A2 = (int)(bi / (2 * L));
-            if (A2 % G == cta && lt == 0) V(A2 / G, 0, 0)[bi - (long long)A2 * 2 * L] = (T)0;
+            if (A2 % G == cta && lt == 0) {
+                V(A2 / G, 0, 0)[bi - (long long)A2 * 2 * L] = (T)0;
+                if (FORCE) V(A2 / G, 2, 0)[bi - (long long)A2 * 2 * L] = (T)0;        // a broken bond carries no force
+            }
         }
-        if (cta == 0 && lt == 0) { A.out_index[step] = bi; A.out_iters[step] = it; }
+        if (cta == 0 && lt == 0) {
+            A.out_index[step] = bi; A.out_iters[step] = it;
+            if (FORCE && A.out_ratio) A.out_ratio[step] = br;
+        }
         steps_done = step + 1;
         status = ST_OK;
         __syncthreads();

@@ -62,6 +62,7 @@ template <typename T> struct Inst {
         }
         if constexpr (FS::valid) {
             if ((e = prep(cg_fused_kernel<T, P>, FS::smem)) != cudaSuccess) return e;
+            if ((e = prep(cg_fused_kernel<T, P, true>, FS::smem)) != cudaSuccess) return e;
         }
         return prep(col_kernel<T, P, CS::COLS>, CS::smem);
     }
@@ -170,7 +171,8 @@ template <typename T> struct Inst {
         if constexpr (FS::valid) {
             FusedArgs A = *static_cast<const FusedArgs*>(fused_args);
             void* params[] = {&A};
-            return cudaLaunchCooperativeKernel((const void*)cg_fused_kernel<T, P>, dim3(FS::G), dim3(P::NT), params, FS::smem, st);
+            const void* fn = A.form ? (const void*)cg_fused_kernel<T, P, true> : (const void*)cg_fused_kernel<T, P>;
+            return cudaLaunchCooperativeKernel(fn, dim3(FS::G), dim3(P::NT), params, FS::smem, st);
         }
         return cudaErrorInvalidValue;
     }

@@ -125,7 +125,7 @@ def test_force_solve_classic_engine_loop_modes_and_constants(B, L, dt):
     _, g = green_spectrum_oracle(L, dt)
     k = inputs.force_k(L, 10).astype(dt)
     outs = []
-    for opts in (dict(), dict(FCG_OPT_LOOP_MODE=1, FCG_OPT_CHUNK=5), dict(FCG_OPT_UNROLL=1)):
+    for opts in (dict(FCG_OPT_FUSED=0), dict(FCG_OPT_LOOP_MODE=1, FCG_OPT_CHUNK=5), dict(FCG_OPT_UNROLL=1, FCG_OPT_FUSED=0)):   # (the one-launch kernel is its own path)
         h = handle(B, L, dt, g, **opts)
         f = dev(np.zeros((L, L), dt))
         r = h.fcg_force_solve(dev(k), 1.0, f, 1e-8 if dt == np.float64 else 1e-5, 1000)
@@ -242,4 +242,88 @@ def test_force_full_size_sampled(B):
     res = np.linalg.norm(k - orc.force_apply(g, k, fh)) / np.linalg.norm(k)
     assert res <= 2e-12
     assert np.all(fh[k == 0] == 0) and fh[k > 0].min() > 1.0 / (1 + g[0, 0])      # every bond carries more than in the intact plate
+    h.close()
+
+
+# ------------------------------------------------------------------------------------ one-launch kernel, FORCE variant (L = 256, 512)
+@pytest.mark.parametrize("L,dt", [(256, np.float64), (512, np.float64), (256, np.float32), (512, np.float32)])
+def test_force_solve_fused_and_graph_paths(B, L, dt):
+    """fcg_force_solve through the one-launch cooperative kernel (default at L = 256, 512) and through the four-launch graph:
+    each against the oracle (force_parity), launch counts tell which path ran, and the two agree with each other."""
+    sols = []
+    for fused in (1, 0):
+        force_parity(B, L, dt, 10, FCG_OPT_FUSED=fused)
+        _, g = green_spectrum_oracle(L, dt)
+        h = handle(B, L, dt, g, FCG_OPT_FUSED=fused)
+        k = inputs.force_k(L, 10).astype(dt); f = dev(np.zeros((L, L), dt))
+        # pinned count, two iterations in (nothing depends on the stop; later iterates amplify rounding, see force_parity)
+        it, rr, st = h.fcg_force_solve(dev(k), inputs.FORCE_D, f, 0.0, 2)
+        assert (it, st) == (2, B.FCG_NOT_CONVERGED)
+        has_fused = not (L == 512 and dt == np.float32)                               # (no one-launch kernel for that plan)
+        assert (h.fcg_last_launch_count() == 1) == bool(fused and has_fused)
+        sols.append(f.cpu().numpy()); h.close()
+    assert rel(sols[0], sols[1]) <= TOL_CG[dt] * 0.1
+
+
+def test_force_fused_edge_cases(B):
+    L, dt = 256, np.float64
+    _, g = green_spectrum_oracle(L, dt)
+    h = handle(B, L, dt, g)
+    f = dev(np.ones((L, L)))
+    it, rr, st = h.fcg_force_solve(dev(np.zeros((L, L))), 1.0, f, 1e-12, 100)       # every bond broken: b = 0 -> f = 0
+    assert (it, rr, st) == (0, 0.0, 0) and float(f.abs().max()) == 0.0 and h.fcg_last_launch_count() == 1
+    k = inputs.force_k(L, 10)
+    f = dev(np.zeros((L, L)))
+    it, rr, st = h.fcg_force_solve(dev(k), 0.0, f, 1e-12, 100)                      # D = 0
+    assert (it, st) == (0, 0) and float(f.abs().max()) == 0.0
+    it, rr, st = h.fcg_force_solve(dev(k), 1.0, f, 1e-12, 0)                        # maxit = 0
+    assert (it, st) == (0, B.FCG_NOT_CONVERGED)
+    # non-uniform k (outside reading F1): not conjugate gradient, but the same arithmetic as the oracle, iterate by iterate
+    kn = (inputs.uniform_k(L) * (k > 0)).astype(dt)
+    ref = orc.force_cg(g, kn, 0.7, np.zeros((L, L)), 0.0, 3)
+    f = dev(np.zeros((L, L)))
+    it, rr, st = h.fcg_force_solve(dev(kn), 0.7, f, 0.0, 3)
+    assert it == 3 and rel(f.cpu().numpy(), ref["f"]) <= 1e-10
+    h.close()
+
+
+@pytest.mark.parametrize("L,nsteps,grad", [(256, 300, 1.0), (512, 60, 2.0)])
+def test_force_fracture_fused_one_launch(B, L, nsteps, grad):
+    """The quasi-static loop in the forces as ONE cooperative launch: identical break indices to the oracle and to the host-driven
+    graph path, critical ratios to 1e-8, k and f written back."""
+    dt = np.float64
+    _, g = green_spectrum_oracle(L, dt)
+    t = inputs.gradient_thresholds(L, grad)
+    k_or = inputs.force_k(L); f_or = np.zeros((L, L))
+    ref = orc.force_fracture(g, k_or, 1.0, f_or, t, nsteps, 1e-12, 1000)
+    assert ref["steps"] == nsteps and ref["gap"].min() > 1e-7
+    outs = []
+    for fused in (1, 0):
+        h = handle(B, L, dt, g, FCG_OPT_FUSED=fused)
+        kd = dev(inputs.force_k(L)); fd = dev(np.zeros((L, L)))
+        index, iters, ratio, done, st = h.fcg_force_fracture(kd, 1.0, fd, dev(t), nsteps, 1e-12, 1000)
+        assert (done, st) == (nsteps, 0)
+        assert (h.fcg_last_launch_count() == 1) == bool(fused)
+        assert np.array_equal(index, ref["index"])
+        dit = np.abs(iters.astype(int) - ref["iters"].astype(int))
+        assert dit.max() <= 4 and np.mean(dit <= 2) >= 0.9 and abs(int(iters.sum()) - int(ref["iters"].sum())) <= 0.05 * ref["iters"].sum()
+        assert np.abs(ratio / ref["ratio"] - 1).max() < 1e-8
+        assert np.array_equal(kd.cpu().numpy(), k_or) and rel(fd.cpu().numpy(), f_or) < 1e-8
+        assert np.all(fd.cpu().numpy()[k_or == 0] == 0)
+        outs.append(index); h.close()
+    assert np.array_equal(outs[0], outs[1])
+
+
+def test_force_fracture_fused_no_candidate(B):
+    """Runs out of bonds: the loop stops with FCG_NO_CANDIDATE after the last unbroken bond, steps_done says how far it got."""
+    L, dt = 256, np.float64
+    _, g = green_spectrum_oracle(L, dt)
+    k = np.zeros((L, L)); k[3, 5] = k[100, 7] = k[200, 250] = 1.0
+    h = handle(B, L, dt, g)
+    kd, fd = dev(k), dev(np.zeros((L, L)))
+    index, iters, ratio, done, st = h.fcg_force_fracture(kd, 1.0, fd, dev(inputs.thresholds(L)), 5, 1e-12, 100)
+    k_or = k.copy(); f_or = np.zeros((L, L))
+    ref = orc.force_fracture(g, k_or, 1.0, f_or, inputs.thresholds(L), 5, 1e-12, 100)
+    assert done == ref["steps"] == 3 and st == B.FCG_NO_CANDIDATE
+    assert np.array_equal(index[:3], ref["index"][:3]) and float(kd.abs().max()) == 0.0
     h.close()
