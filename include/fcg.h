@@ -202,9 +202,12 @@ int fcg_fracture_end(fcg_handle h, long long* index_host, int* iters_host, int* 
  *   fcg_force_solve      CG on eq. (2): right-hand side b_i = k_i * D formed in the residual pass (one multiply in the handle's dtype);
  *                        f in: initial guess (0 on broken bonds), out: forces; stop at the first iteration with
  *                        ||r||_2 <= tol ||b||_2; iters / rel_residual / status / scalars in double / determinism as fcg_solve.
- *                        k == 0 everywhere or D == 0 gives f = 0, 0 iterations.  One CUDA graph per solve, four launches
- *                        per iteration (the textbook order; the spectral search length of fcg_solve is not used); at L = 256
- *                        and 512 one cooperative launch for the whole solve, as fcg_solve (FCG_OPT_FUSED).  Blocks.
+ *                        k == 0 everywhere or D == 0 gives f = 0, 0 iterations.  One CUDA graph per solve.  Where reading
+ *                        F1 holds for the call -- checked on the device first (one kernel over k and f, a 32-byte read-back):
+ *                        all k_i in {0, kappa} and the start vector zero on the broken bonds -- the iteration is three
+ *                        launches, with p.(I + K G)p = sum p^2 + kappa sum g |P|^2 as in fcg_solve (FCG_OPT_SPECTRAL_ALPHA);
+ *                        otherwise four launches in the textbook order, for any k.  At L = 256 and 512 one cooperative launch
+ *                        for the whole solve, textbook order (FCG_OPT_FUSED).  Blocks.
  *   fcg_force_break_step reading F2: the response is linear in D, so the bond that reaches its threshold first is
  *                        argmax over {k_i > 0} of f_i / t_i (one IEEE divide in double; ties -> lowest i; NaN skipped);
  *                        sets k_i = 0 AND f_i = 0 (a broken bond carries nothing).  ratio_host = the winning f/t: with f

@@ -40,7 +40,7 @@ const PassTable* get_table(int L, int dtype) {
 }
 
 struct Layout {            // byte offsets into the workspace
-    size_t Tb, shat, mhat, r, p, q, z, tw, partial_row, partial_col, partial_vec, brk_r, brk_i, scalars, brk_out, brk_ticket, total;
+    size_t Tb, shat, mhat, r, p, q, z, tw, partial_row, partial_col, partial_vec, brk_r, brk_i, scalars, brk_out, brk_ticket, uni, total;
 };
 Layout make_layout(int L, size_t w) {
     const size_t N = (size_t)L * L;
@@ -60,12 +60,13 @@ Layout make_layout(int L, size_t w) {
     o.scalars = take(sizeof(Scalars));
     o.brk_out = take(sizeof(BreakResult));
     o.brk_ticket = take(sizeof(unsigned int));
+    o.uni = take(4 * sizeof(unsigned long long));         // force_uniform_kernel's result (reading F1 check)
     o.total = off;
     return o;
 }
 
 struct GraphEntry {
-    const void *k, *f; void* u; double tol; int maxit, var, unroll, pdl, pcg, force; double D;   // pcg: bit 0 = preconditioned, the rest = launch options (key)
+    const void *k, *f; void* u; double tol; int maxit, var, unroll, pdl, pcg, force; double D, kappa;   // pcg: bit 0 = preconditioned, the rest = launch options (key)
     cudaGraph_t graph; cudaGraphExec_t exec; unsigned long long stamp;
 };
 
@@ -91,6 +92,7 @@ struct fcg_handle_s {
     bool fused() const { return fused_opt && tab->fused && v2() && loop_mode == 0; }   // whole solve in one cooperative kernel
     Scalars* h_sc = nullptr;            // pinned
     BreakResult* h_brk = nullptr;       // pinned
+    unsigned long long* h_uni = nullptr; // pinned: result of the reading-F1 check of fcg_force_solve
     void *hk = nullptr, *hf = nullptr, *hu = nullptr;   // device staging of fcg_solve_host
     long long* frac_idx = nullptr; int* frac_it = nullptr; double* frac_ratio = nullptr; int frac_cap = 0;   // device results of the fused quasi-static loop
     int pend_nsteps = -1, pend_done = 0, pend_status = 0; bool pend_async = false;   // fcg_fracture_begin / _end
@@ -145,6 +147,7 @@ template <typename T> struct Seq {
     fcg_handle h; cudaStream_t st; bool classic = false;      // classic: force the synchronous passes (stand-alone transforms)
     bool pcg = false;                                         // preconditioned CG: directions from z = M^-1 r
     bool force = false; double D = 0.0;                       // force formulation (I + K G) f = K D (eq. (2))
+    double kappa = 0.0;                                       // force: > 0 when reading F1 was verified for this call (k in {0, kappa}): three launches
     bool v2() const { return h->v2() && !classic; }
     const T* mhat() const { return h->at<T>(h->lay.mhat); }
     T* z() const { return h->at<T>(h->lay.z); }
@@ -184,8 +187,8 @@ template <typename T> struct Seq {
         if ((e = row_fwd(ROWF_PLAIN, u, nullptr)) != cudaSuccess) return e;
         if ((e = col(COL_CONV, false)) != cudaSuccess) return e;
         if ((e = row_inv(ROWI_RESID, k, u, force ? k : f, r(), p())) != cudaSuccess) return e;   // (force: b = K D is formed in the pass)
-        if (sl()) {      // start value of the sum k p^2 recurrence: the first direction is p = r
-            cg_kpp0_kernel<T><<<h->vec_blocks(), 256, 0, st>>>(k, (const T*)r(), h->N / Vec<T>::W, h->at<double>(h->lay.partial_vec), h->sc());
+        if (sl()) {      // start value of the sum k p^2 recurrence: the first direction is p = r  (force: sum p^2)
+            cg_kpp0_kernel<T><<<h->vec_blocks(), 256, 0, st>>>(force ? (const T*)nullptr : k, (const T*)r(), h->N / Vec<T>::W, h->at<double>(h->lay.partial_vec), h->sc());
             ++h->launches;
             return cudaGetLastError();
         }
@@ -247,9 +250,10 @@ template <typename T> struct Seq {
         A.partial = h->at<double>(h->lay.partial_row); A.colsum = h->at<double>(h->lay.partial_col);
         A.sc = h->sc(); A.nsm = h->nsm; A.pdl = h->pdl;
         ++h->launches;
+        if (force) { A.form = 1; A.kappa = kappa; return h->tab->row_inv2_cgf_force(&A, &h->tmap_row, st); }
         return h->tab->row_inv2_cgf(&A, &h->tmap_row, st);
     }
-    bool sl() const { return !pcg && !force && !classic && h->sl(); }
+    bool sl() const { return !pcg && !classic && h->sl() && (!force || kappa > 0.0); }
     cudaError_t iteration(const T* k, T* u) const {
         cudaError_t e;
         if (sl()) {
@@ -285,7 +289,7 @@ template <typename T>
 cudaError_t build_graph(fcg_handle h, GraphEntry& ge) {
     cudaError_t e;
     cudaStream_t cs = h->cap_stream;
-    Seq<T> s{h, cs}; s.pcg = (ge.pcg & 1) != 0; s.force = ge.force != 0; s.D = ge.D;
+    Seq<T> s{h, cs}; s.pcg = (ge.pcg & 1) != 0; s.force = ge.force != 0; s.D = ge.D; s.kappa = ge.kappa;
     const long long saved = h->launches;
     ge.graph = nullptr; ge.exec = nullptr;
     if ((e = cudaGraphCreate(&ge.graph, 0)) != cudaSuccess) return e;
@@ -356,19 +360,34 @@ int solve_impl(fcg_handle h, const void* k, const void* f, void* u, double tol, 
         h->err = std::string("cooperative launch failed (") + cudaGetErrorString(e) + "); using the graph path";
         h->fused_opt = 0;
     }
+    // force formulation: the three-launch iteration needs reading F1 (k in {0, kappa}, start vector zero on broken bonds); one small
+    // kernel and a 32-byte read-back decide it per call (~30 us against milliseconds of solve); otherwise four launches, any k
+    double kappa = 0.0;
+    if (force && !pcg && h->sl() && !(h->fused())) {
+        unsigned long long* d_uni = h->at<unsigned long long>(h->lay.uni);
+        FCG_CK(h, cudaMemsetAsync(d_uni, 0, 4 * sizeof(unsigned long long), h->stream));
+        force_uniform_kernel<T><<<h->vec_blocks(), 256, 0, h->stream>>>((const T*)k, (const T*)u, h->N, d_uni);
+        ++h->launches;
+        FCG_CK(h, cudaGetLastError());
+        FCG_CK(h, cudaMemcpyAsync(h->h_uni, d_uni, 4 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, h->stream));
+        FCG_CK(h, cudaStreamSynchronize(h->stream));
+        double kmax, kmin; const unsigned long long b0 = h->h_uni[0], b1 = ~h->h_uni[1];
+        std::memcpy(&kmax, &b0, 8); std::memcpy(&kmin, &b1, 8);
+        if (h->h_uni[2] == 0 && kmax > 0.0 && kmax == kmin && std::isfinite(kmax)) kappa = kmax;
+    }
     if (h->loop_mode == 0) {
-        const int var = h->v2() ? 100 + (h->sl() && !force ? 1 : 0) : h->row_var();
+        const int var = h->v2() ? 100 + (h->sl() && (!force || kappa > 0.0) ? 1 : 0) : h->row_var();
         const int key = (pcg ? 1 : 0) + 2 * (h->colp() ? 1 : 0) + 4 * h->hints;
         GraphEntry* hit = nullptr;
         for (auto& g : h->graphs)
-            if (g.k == k && g.f == f && g.u == u && g.tol == tol && g.maxit == maxit && g.var == var && g.unroll == h->unroll && g.pdl == h->pdl && g.pcg == key && g.force == (force ? 1 : 0) && g.D == D) { hit = &g; break; }
+            if (g.k == k && g.f == f && g.u == u && g.tol == tol && g.maxit == maxit && g.var == var && g.unroll == h->unroll && g.pdl == h->pdl && g.pcg == key && g.force == (force ? 1 : 0) && g.D == D && g.kappa == kappa) { hit = &g; break; }
         if (!hit) {
             if (h->graphs.size() >= 8) {
                 size_t lru = 0;
                 for (size_t i = 1; i < h->graphs.size(); ++i) if (h->graphs[i].stamp < h->graphs[lru].stamp) lru = i;
                 drop_graph(h->graphs[lru]); h->graphs.erase(h->graphs.begin() + lru);
             }
-            GraphEntry ge{k, f, u, tol, maxit, var, h->unroll, h->pdl, key, force ? 1 : 0, D, nullptr, nullptr, 0};
+            GraphEntry ge{k, f, u, tol, maxit, var, h->unroll, h->pdl, key, force ? 1 : 0, D, kappa, nullptr, nullptr, 0};
             cudaError_t e = build_graph<T>(h, ge);
             if (e != cudaSuccess) {
                 // conditional graph nodes unavailable: fall back to direct launches for the rest of this handle's life
@@ -388,12 +407,12 @@ int solve_impl(fcg_handle h, const void* k, const void* f, void* u, double tol, 
             FCG_CK(h, cudaGraphLaunch(hit->exec, h->stream));
             FCG_CK(h, cudaStreamSynchronize(h->stream));
             const long long U = hit->unroll;
-            Seq<T> sq{h, h->stream}; sq.pcg = pcg; sq.force = force; sq.D = D;
-            h->launches = sq.launches_outside_loop() + sq.launches_per_iteration() * U * ((h->h_sc->it + U - 1) / U);   // no-op kernels after the stop are launches too
+            Seq<T> sq{h, h->stream}; sq.pcg = pcg; sq.force = force; sq.D = D; sq.kappa = kappa;
+            h->launches = (kappa > 0.0 ? 1 : 0) + sq.launches_outside_loop() + sq.launches_per_iteration() * U * ((h->h_sc->it + U - 1) / U);   // no-op kernels after the stop are launches too
         }
     }
     if (h->loop_mode != 0) {
-        Seq<T> s{h, h->stream}; s.pcg = pcg; s.force = force; s.D = D;
+        Seq<T> s{h, h->stream}; s.pcg = pcg; s.force = force; s.D = D; s.kappa = kappa;
         FCG_CK(h, s.init((const T*)k, (const T*)f, (T*)u, tol, maxit, false, 0ULL));
         FCG_CK(h, cudaMemcpyAsync(h->h_sc, h->sc(), sizeof(Scalars), cudaMemcpyDeviceToHost, h->stream));
         FCG_CK(h, cudaStreamSynchronize(h->stream));
@@ -655,6 +674,7 @@ int fcg_create(int L, fcg_dtype dt, void* workspace, void* cuda_stream, fcg_hand
     }
     if (cudaMallocHost((void**)&h->h_sc, sizeof(Scalars)) != cudaSuccess) return bail(FCG_CUDA_ERROR);
     if (cudaMallocHost((void**)&h->h_brk, sizeof(BreakResult)) != cudaSuccess) return bail(FCG_CUDA_ERROR);
+    if (cudaMallocHost((void**)&h->h_uni, 4 * sizeof(unsigned long long)) != cudaSuccess) return bail(FCG_CUDA_ERROR);
     std::memset(h->h_sc, 0, sizeof(Scalars));
     if (cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking) != cudaSuccess) return bail(FCG_CUDA_ERROR);
     if (h->tab->init() != cudaSuccess) return bail(FCG_CUDA_ERROR);
@@ -674,6 +694,7 @@ int fcg_destroy(fcg_handle h) {
     if (h->own_ws && h->ws) cudaFree(h->ws);
     if (h->h_sc) cudaFreeHost(h->h_sc);
     if (h->h_brk) cudaFreeHost(h->h_brk);
+    if (h->h_uni) cudaFreeHost(h->h_uni);
     if (h->hk) cudaFree(h->hk);
     if (h->hf) cudaFree(h->hf);
     if (h->hu) cudaFree(h->hu);

@@ -738,12 +738,15 @@ __global__ void __launch_bounds__(256) t2_import_kernel(const cx<T>* __restrict_
 // CTAs, no broadcast).  So q = k o p + c is consumed on the spot -- r -= alpha q, r.r -> count, convergence, beta -- and never
 // stored: strips k0 k1 p0 p1 r0 r1, output r in place.  The pass also accumulates t = sum k r'^2 and v = sum k r' p for
 //     sum k p'^2 = t + 2 beta v + beta^2 sum k p^2        (p' = r' + beta p, the next direction).
+// VAR = 3 is the same pass for the force formulation under reading F1: q = p + k o G p, and because every
+// CG vector is zero on the broken bonds and k = kappa on the others, p.q = sum p^2 + kappa sum g |P|^2 -- the recurrence runs with
+// unit weights (t = sum r'^2, v = sum r' p) and the column pass's energy is scaled by kappa.
 template <typename T, typename P, int CTAS, int VAR = 0>
 __global__ void __launch_bounds__(AsyncShape<T, P>::INV_THREADS, CTAS) row_inv2_kernel(const RowInvArgs<T> A, const __grid_constant__ CUtensorMap tmap)
 {
     using AS = AsyncShape<T, P>;
     constexpr int L = P::N, S = P::S, NT = P::NT, R1 = AS::R1, Q1 = AS::Q1, PER1 = AS::PER1, PM = per_max<P>();
-    constexpr bool PRE = VAR == 1, CGF = VAR == 2;
+    constexpr bool PRE = VAR == 1, CGF = VAR == 2 || VAR == 3, FCGF = VAR == 3;
     constexpr int TSUB = AS::TSUB, NSUB = AS::NSUB;
     constexpr uint32_t TBYTES = (uint32_t)AS::TSB;
     // CGF moves three vectors of strips per transform against one of tiles: the tile ring is kept short (TCAP) and the strips
@@ -770,7 +773,7 @@ __global__ void __launch_bounds__(AsyncShape<T, P>::INV_THREADS, CTAS) row_inv2_
     SmemIO<T, P> io{W};
     const int lt = threadIdx.x, lane = lt & 31, warp = lt >> 5;
     const int mode = PRE ? (int)ROWI_PRECOND : CGF ? (int)ROWI_CGF : A.mode;
-    const bool force = !PRE && !CGF && A.form != 0;
+    const bool force = FCGF || (!PRE && !CGF && A.form != 0);
     tma::grid_dep_launch();
     const bool st_on = A.mode >= 0;                               // always true, opaque to the compiler (as in row_fwd2_kernel)
     const int nv = PRE ? 2 : CGF ? 6 : (mode == ROWI_PLAIN ? 0 : (mode == ROWI_RESID ? 6 : 4));
@@ -843,7 +846,7 @@ __global__ void __launch_bounds__(AsyncShape<T, P>::INV_THREADS, CTAS) row_inv2_
         e = 0.0;
         for (int w2 = 0; w2 < (int)(blockDim.x >> 5); ++w2) e += red[w2];
         __syncthreads();
-        pq_d = A.sc->kpp + e;
+        pq_d = A.sc->kpp + (FCGF ? A.kappa * e : e);
         if (!(pq_d > 0.0) || !isfinite(pq_d)) {                   // breakdown: nothing may change; CTA 0 reports it
             if (blockIdx.x == 0 && lt == 0) { A.sc->pq = pq_d; A.sc->status = ST_BREAKDOWN; A.sc->done = 1; A.sc->alpha = 0.0; set_cond(A.sc, false); }
             return;
@@ -931,7 +934,7 @@ __global__ void __launch_bounds__(AsyncShape<T, P>::INV_THREADS, CTAS) row_inv2_
                         const T r0 = sl[4 * QV + j] - alpha * val0, r1 = sl[5 * QV + j] - alpha * val1;   // residue
                         if (st_on) { tma::st_hint(A.out + i0, r0, pol_r); tma::st_hint(A.out + i0 + L, r1, pol_r); }
                         f_rr += r0 * r0; f_rr += r1 * r1;                                                   // residue length (97)
-                        const T kr0 = sl[j] * r0, kr1 = sl[QV + j] * r1;
+                        const T kr0 = FCGF ? r0 : sl[j] * r0, kr1 = FCGF ? r1 : sl[QV + j] * r1;
                         f_t += kr0 * r0; f_t += kr1 * r1;
                         f_v += kr0 * v0; f_v += kr1 * v1;
                         continue;

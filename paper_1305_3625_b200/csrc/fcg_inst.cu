@@ -55,6 +55,7 @@ template <typename T> struct Inst {
                 if ((e = prep(col2p_kernel<T, P, CPS::CTAS, false>, CPS::smem)) != cudaSuccess) return e;
             }
             if ((e = prep(row_inv2_kernel<T, P, C_INV, 2>, AS::inv_smem)) != cudaSuccess) return e;
+            if ((e = prep(row_inv2_kernel<T, P, C_INV, 3>, AS::inv_smem)) != cudaSuccess) return e;
             if ((e = prep(col2_xform_kernel<T, P, C_COL, -1>, AS::WBYTES + 128)) != cudaSuccess) return e;
             if ((e = prep(col2_xform_kernel<T, P, C_COL, +1>, AS::WBYTES + 128)) != cudaSuccess) return e;
             if ((e = prep(t2_export_kernel<T, P>, AS::WBYTES + 1024)) != cudaSuccess) return e;
@@ -123,6 +124,14 @@ template <typename T> struct Inst {
         if constexpr (SL) {
             const RowInvArgs<T>& A = *static_cast<const RowInvArgs<T>*>(args);
             return launch(row_inv2_kernel<T, P, C_INV, 2>, pgrid(A.nsm, C_INV), AS::INV_THREADS, AS::inv_smem, st, A.pdl, A,
+                          *static_cast<const CUtensorMap*>(tensor_map));
+        }
+        return cudaErrorInvalidValue;
+    }
+    static cudaError_t row_inv2_cgf_force(const void* args, const void* tensor_map, cudaStream_t st) {
+        if constexpr (SL) {
+            const RowInvArgs<T>& A = *static_cast<const RowInvArgs<T>*>(args);
+            return launch(row_inv2_kernel<T, P, C_INV, 3>, pgrid(A.nsm, C_INV), AS::INV_THREADS, AS::inv_smem, st, A.pdl, A,
                           *static_cast<const CUtensorMap*>(tensor_map));
         }
         return cudaErrorInvalidValue;
@@ -243,7 +252,7 @@ template <typename T> struct Inst {
         t.v2_smem[0] = AS::fwd_smem; t.v2_smem[1] = AS::col_smem; t.v2_smem[2] = AS::inv_smem;
         t.row_fwd2 = &row_fwd2; t.col2 = &col2; t.row_inv2 = &row_inv2; t.row_fwd2_rupd = &row_fwd2_rupd; t.row_inv2_pre = &row_inv2_pre;
         t.colp_ok = COLP ? 1 : 0; t.colp_ctas = COLP ? CPS::CTAS : 0; t.col2p = &col2p;
-        t.sl_ok = SL ? 1 : 0; t.col2_energy = &col2_energy; t.row_inv2_cgf = &row_inv2_cgf;
+        t.sl_ok = SL ? 1 : 0; t.col2_energy = &col2_energy; t.row_inv2_cgf = &row_inv2_cgf; t.row_inv2_cgf_force = &row_inv2_cgf_force;
         t.col2_xform = &col2_xform; t.t2_export = &t2_export; t.t2_import = &t2_import;
         t.fused = FS::valid ? 1 : 0; t.fused_grid = FS::G; t.fused_solve = &fused_solve;
         t.init = &init; t.row_fwd = &row_fwd; t.col = &col; t.row_inv = &row_inv; t.spectrum_prep = &spectrum_prep;

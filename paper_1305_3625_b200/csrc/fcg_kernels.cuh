@@ -248,14 +248,47 @@ __global__ void __launch_bounds__(256) cg_kpp0_kernel(const T* __restrict__ k, c
     const V* kv = reinterpret_cast<const V*>(k);
     const V* rv = reinterpret_cast<const V*>(r);
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < nvec; i += (size_t)gridDim.x * blockDim.x) {
-        const V a = __ldg(kv + i), b = __ldg(rv + i);
-        const T* as = reinterpret_cast<const T*>(&a); const T* bs = reinterpret_cast<const T*>(&b);
+        const V b = __ldg(rv + i);
+        const T* bs = reinterpret_cast<const T*>(&b);
+        if (k == nullptr) {          // force formulation: unit weights, sum p^2
+#pragma unroll
+            for (int c = 0; c < Vec<T>::W; ++c) acc[0] += (double)bs[c] * (double)bs[c];
+            continue;
+        }
+        const V a = __ldg(kv + i);
+        const T* as = reinterpret_cast<const T*>(&a);
 #pragma unroll
         for (int c = 0; c < Vec<T>::W; ++c) acc[0] += (double)as[c] * ((double)bs[c] * (double)bs[c]);
     }
     double tot[1];
     if (!grid_sum_last<1>(acc, partial, &sc->ticket2[0], red, tot)) return;
     if (threadIdx.x == 0) sc->kpp = tot[0];
+}
+
+// Reading F1 checked on the device before a force solve chooses the three-launch iteration: are all k_i in {0, kappa} with kappa > 0,
+// and is the start vector zero on the broken bonds?  Doubles >= 0 order like their bit patterns, so max k and min positive k are
+// integer atomics: out[0] = bits(max k), out[1] = ~bits(min positive k) (so that a memset to 0 initialises both), out[2] = 1 if any
+// k_i is negative or NaN, or f_i != 0 where k_i == 0.
+template <typename T>
+__global__ void __launch_bounds__(256) force_uniform_kernel(const T* __restrict__ k, const T* __restrict__ f, size_t n, unsigned long long* out) {
+    double kmax = 0.0, kmin = INFINITY; unsigned int bad = 0u;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+        const double ki = (double)k[i];
+        if (!(ki >= 0.0)) { bad = 1u; continue; }
+        if (ki > 0.0) { kmax = fmax(kmax, ki); kmin = fmin(kmin, ki); }
+        else if (f[i] != (T)0) bad = 1u;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        kmax = fmax(kmax, __shfl_xor_sync(0xffffffffu, kmax, o));
+        kmin = fmin(kmin, __shfl_xor_sync(0xffffffffu, kmin, o));
+        bad |= __shfl_xor_sync(0xffffffffu, bad, o);
+    }
+    if ((threadIdx.x & 31) == 0) {
+        atomicMax(out, (unsigned long long)__double_as_longlong(kmax));
+        atomicMax(out + 1, ~(unsigned long long)__double_as_longlong(kmin));
+        if (bad) atomicOr(out + 2, 1ULL);
+    }
 }
 
 // last lagged "new x" after the loop has ended; u = 0 when f = 0

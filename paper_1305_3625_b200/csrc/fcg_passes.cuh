@@ -83,6 +83,8 @@ template <typename T> struct RowInvArgs {
     int form;                             // 0: A x = k o x + C x (BASELINE.json);  1: force formulation B x = x + k o (C x), the left side
                                           //    of eq. (2), PAPER.md:74 (CG, RESID, APPLY)
     T dval;                               // form 1, RESID: right-hand side b = k * dval (K D of eq. (2)); f is not read
+    double kappa;                         // form 1, CGF (three launches, reading F1: k in {0, kappa}, vectors zero on broken bonds):
+                                          //    p.(I + K G)p = sum p^2 + kappa sum g |P|^2
 };
 
 template <int A, int B, typename F> FCG_HD void static_for_up(F&& f) {

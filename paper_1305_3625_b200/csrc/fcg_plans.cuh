@@ -72,6 +72,7 @@ struct PassTable {
     int sl_ok;
     cudaError_t (*col2_energy)(const void* args, const void* tensor_map, cudaStream_t st);
     cudaError_t (*row_inv2_cgf)(const void* args, const void* tensor_map, cudaStream_t st);
+    cudaError_t (*row_inv2_cgf_force)(const void* args, const void* tensor_map, cudaStream_t st);   // force formulation under reading F1
     // persistent, double-buffered column pass (col2p_kernel); colp_ok == 0 where two column buffers do not fit twice per SM
     int colp_ok, colp_ctas;
     cudaError_t (*col2p)(const void* args, const void* tensor_map, int energy, cudaStream_t st);

@@ -327,3 +327,40 @@ def test_force_fracture_fused_no_candidate(B):
     assert done == ref["steps"] == 3 and st == B.FCG_NO_CANDIDATE
     assert np.array_equal(index[:3], ref["index"][:3]) and float(kd.abs().max()) == 0.0
     h.close()
+
+
+# ------------------------------------------------------------------------------------ three launches per iteration under reading F1
+@pytest.mark.parametrize("L,dt", [(1024, np.float64), (1024, np.float32), (256, np.float64)])
+def test_force_three_launch_iteration(B, L, dt):
+    """Graph path (one-launch kernel off): with k in {0, kappa} and a start vector that is zero on the broken bonds the solve runs
+    three launches per iteration (p.q = sum p^2 + kappa sum g |P|^2), otherwise -- or with FCG_OPT_SPECTRAL_ALPHA = 0 -- four;
+    the launch count tells which, and each is checked against the oracle."""
+    tol = inputs.FORCE_TOL[np.dtype(dt)]
+    force_parity(B, L, dt, 10, FCG_OPT_FUSED=0)                                     # three launches
+    force_parity(B, L, dt, 10, FCG_OPT_FUSED=0, FCG_OPT_SPECTRAL_ALPHA=0)           # four
+    _, g = green_spectrum_oracle(L, dt)
+    k = inputs.force_k(L, 7, 2.5 if dt == np.float64 else 1.0).astype(dt)           # (another elastic constant: kappa must reach the pass)
+    count = lambda it, per, extra: extra + per * 4 * ((it + 3) // 4)
+    sols = []
+    for sa in (1, 0):
+        h = handle(B, L, dt, g, FCG_OPT_FUSED=0, FCG_OPT_SPECTRAL_ALPHA=sa)
+        f = dev(np.zeros((L, L), dt))
+        it, rr, st = h.fcg_force_solve(dev(k), 1.0, f, tol, 1000)
+        assert st == 0 and h.fcg_last_launch_count() == (count(it, 3, 7) if sa else count(it, 4, 5))
+        sols.append(f.cpu().numpy()); h.close()
+    assert rel(sols[0], sols[1]) <= TOL_CG[dt]
+    # outside reading F1 the library must notice and keep the textbook order: (a) two different elastic constants, (b) a start
+    # vector that is not zero on a broken bond -- both against the oracle at a pinned count
+    h = handle(B, L, dt, g, FCG_OPT_FUSED=0)
+    k2 = k.copy(); k2[k2 > 0] = np.where(np.arange((k2 > 0).sum()) % 2, 2.5, 1.5).astype(dt)
+    f0 = np.zeros((L, L), dt)
+    f = dev(f0)
+    it, rr, st = h.fcg_force_solve(dev(k2), 1.0, f, 0.0, 3)
+    assert it == 3 and h.fcg_last_launch_count() == count(3, 4, 5)
+    assert rel(f.cpu().numpy(), orc.force_cg(g, k2, 1.0, f0, 0.0, 3)["f"]) <= TOL_CG[dt] * (0.1 if dt == np.float64 else 1.0)
+    f1 = f0.copy(); f1[k == 0] = 0.25
+    f = dev(f1)
+    it, rr, st = h.fcg_force_solve(dev(k), 1.0, f, 0.0, 3)
+    assert it == 3 and h.fcg_last_launch_count() == count(3, 4, 5)
+    assert rel(f.cpu().numpy(), orc.force_cg(g, k, 1.0, f1, 0.0, 3)["f"]) <= TOL_CG[dt] * (0.1 if dt == np.float64 else 1.0)
+    h.close()
