@@ -87,6 +87,10 @@ def _declare(L: C.CDLL) -> None:
         f = getattr(L, "oracle_force_cg" + suf)
         f.argtypes = [_i, _vp, _vp, _d, _vp, _d, _i, C.POINTER(_i), C.POINTER(_d), _vp, _vp, _vp]
         f.restype = _i
+        f = getattr(L, "oracle_inverse_spectrum" + suf)
+        f.argtypes = [_ll, _vp, _vp]; f.restype = None
+        f = getattr(L, "oracle_force_from_displacement" + suf)
+        f.argtypes = [_ll, _vp, _d, _vp, _vp]; f.restype = None
         f = getattr(L, "oracle_force_break_step" + suf)
         f.argtypes = [_ll, _vp, _vp, _vp, C.POINTER(_ll), C.POINTER(_d), C.POINTER(_d)]
         f.restype = _i
@@ -300,6 +304,20 @@ def force_cg(g, k, D: float, f0, tol: float, maxit: int, history: bool = False, 
     if directions:
         out["P"] = P[: it.value]; out["R"] = R[: it.value]
     return out
+
+
+def inverse_spectrum(g) -> np.ndarray:
+    """s = 1 / g element by element, in the dtype of g: the spectrum of G^-1 (reading F7)."""
+    g = np.ascontiguousarray(g); s = np.empty_like(g)
+    getattr(lib(), "oracle_inverse_spectrum" + _suf(g.dtype))(g.size, _p(g), _p(s))
+    return s
+
+
+def force_from_displacement(k, D: float, u) -> np.ndarray:
+    """f = -k (u - D), eq. (1a), in the dtype of k."""
+    k = np.ascontiguousarray(k); u = _arr(u, k.dtype, k.shape); f = np.empty_like(k)
+    getattr(lib(), "oracle_force_from_displacement" + _suf(k.dtype))(k.size, _p(k), float(D), _p(u), _p(f))
+    return f
 
 
 def force_break_step(k: np.ndarray, f: np.ndarray, t):

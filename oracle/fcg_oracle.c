@@ -21,6 +21,8 @@
  *   oracle_kernel_spectrum_*   s = Re F G, the static transform of the kernel
  *   oracle_force_{apply,cg,break_step,fracture}_*   the paper's formulation in the bond forces, (I + K G) f = K D
  *                              (eq. (2))
+ *   oracle_inverse_spectrum_*, oracle_force_from_displacement_*   the same state through the displacements:
+ *                              (K + G^-1) u = K D by oracle_cg / oracle_pcg with s = 1 / g, then eq. (1a) (reading F7)
  * Pins (tests/test_oracle_*.py): none of these functions is "parity unpinned".
  *
  * Build: gcc -O2 -fopenmp -ffp-contract=off -fPIC -shared fcg_oracle.c -o libfcg_oracle.so -lm

@@ -424,6 +424,23 @@ done:
     return status;
 }
 
+/* The same state through the displacements (reading F7).  Eliminating f instead of u from (1a), (1b): u = G f and f = K (D - u)
+ * give G^-1 u = K (D - u), i.e.
+ *     (K + G^-1) u = K D,        G^-1 = F^-1 diag(1 / g) F,
+ * which is the symmetric system A u = b of BASELINE.json with spectrum s = 1 / g and right-hand side b = K D -- solved by
+ * oracle_cg / oracle_pcg as they stand -- followed by eq. (1a) for the forces.  The two functions below are the two
+ * element-by-element maps of that route; each is one IEEE operation per step in REAL. */
+void FN(oracle_inverse_spectrum)(long long N, const REAL* g, REAL* s)
+{
+    for (long long i = 0; i < N; ++i) s[i] = (REAL)1 / g[i];
+}
+
+/* f_i = -k_i (u_i - D)     eq. (1a), evaluated as k_i * (D - u_i): one subtraction, one multiplication */
+void FN(oracle_force_from_displacement)(long long N, const REAL* k, double D, const REAL* u, REAL* f)
+{
+    for (long long i = 0; i < N; ++i) f[i] = k[i] * ((REAL)D - u[i]);
+}
+
 /* Break step in the force formulation (reading F2): the response is linear in D, so the bond that reaches its threshold
  * first as D grows is the one with the largest f_i / t_i (one IEEE divide in double) among the unbroken bonds; ties ->
  * lowest i, NaN skipped.  The bond is removed: k_i = 0 and f_i = 0 (a broken bond carries no force; keeps the warm start

@@ -163,6 +163,31 @@ def test_force_cg_equals_displacement_form():
     assert rel(k * (D - u), f) < 1e-10
 
 
+@pytest.mark.parametrize("L,den", [(8, 4), (16, 6)])
+def test_displacement_route_maps_and_dense_solve(L, den):
+    """Reading F7: the oracle's two element-wise maps (s = 1/g, f = -k (u - D)) and the whole route -- CG or PCG on
+    (K + G^-1) u = K D, then (1a) -- against LAPACK on the dense matrices: u = (K + G^-1)^-1 K D with G^-1 inverted as a matrix,
+    and the forces against the dense solve of eq. (2)."""
+    G = orc.green_function(L, NU, E, A); g = orc.kernel_spectrum(G)
+    k = inputs.force_k(L, den, kappa=1.3); D = 0.8
+    s = orc.inverse_spectrum(g)
+    assert np.array_equal(s, 1.0 / g) and s.dtype == g.dtype
+    assert orc.inverse_spectrum(g.astype(np.float32)).dtype == np.float32
+    GG = dense_G(G); K = np.diag(k.ravel())
+    u_dense = np.linalg.solve(K + np.linalg.inv(GG), k.ravel() * D)
+    f_dense = np.linalg.solve(np.eye(L * L) + K @ GG, k.ravel() * D)
+    for solve in (lambda: orc.cg(s, k, k * D, np.zeros((L, L)), 1e-13, 2000),
+                  lambda: orc.pcg(s, k, k * D, np.zeros((L, L)), float(k.mean()), 1e-13, 2000)):
+        out = solve()
+        assert out["status"] == 0 and rel(out["u"], u_dense) < 1e-10
+        f = orc.force_from_displacement(k, D, out["u"])
+        assert rel(f, f_dense) < 1e-10 and np.all(f[k == 0] == 0)
+        assert np.abs(orc.conv_direct(G, f) - out["u"]).max() < 1e-10          # (1b): u = G f by the direct sum
+    # the map itself on hand-made numbers, sign included: f = -k (u - D)
+    kk = np.array([[2.0, 0.0], [0.5, 1.0]]); uu = np.array([[0.25, 9.0], [-1.0, 3.0]])
+    assert np.array_equal(orc.force_from_displacement(kk, 1.0, uu), np.array([[1.5, 0.0], [1.0, -2.0]]))
+
+
 # ---------------------------------------------------------------- F-P3: break rule and quasi-static loop
 def test_force_break_step_rule():
     k = np.array([1.0, 0.0, 1.0, 1.0, 1.0]); f = np.array([0.25, 9.0, 0.75, 0.375, np.nan]); t = np.array([0.5, 0.125, 1.0, 0.5, 0.5])
