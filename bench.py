@@ -302,6 +302,29 @@ def bench_force(binding, torch, inputs):
             "iteration_gbs": b_nw * nw / (1e-3 * ms / max(it, 1)) / 1e9, "bytes_per_iteration_Nw": b_nw,
             "green_function_us": 1e3 * ev[0].elapsed_time(ev[1]), "kernel_spectrum_us": 1e3 * ev[1].elapsed_time(ev[2])}
         h.close()
+    # the same forces through the displacements (reading F7): (K + G^-1) u = K D by fcg_solve / fcg_pcg_solve with s = 1/g, then (1a)
+    L = 2048
+    h = binding.Fcg(L, torch.float64)
+    s = h.fcg_inverse_spectrum(h.fcg_kernel_spectrum(h.fcg_green_function(inputs.GREEN_NU, inputs.GREEN_E, inputs.GREEN_A)))
+    h.fcg_set_spectrum(s)
+    kh = inputs.force_k(L, 20); k = to(kh)
+    h.fcg_set_preconditioner(s, inputs.precond_kbar(kh))
+    u = torch.zeros((L, L), dtype=torch.float64, device="cuda"); f = torch.empty_like(u); b = torch.empty_like(u)
+    for name, solve in (("cg", h.fcg_solve), ("pcg", h.fcg_pcg_solve)):
+        for _ in range(2):
+            u.zero_(); h.fcg_force_rhs(k, inputs.FORCE_D, b); solve(k, b, u, 1e-12, 2000); h.fcg_force_from_displacement(k, inputs.FORCE_D, u, f)
+        sev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(5)]
+        for a, c in sev:
+            u.zero_(); a.record()
+            h.fcg_force_rhs(k, inputs.FORCE_D, b); it, rr, st = solve(k, b, u, 1e-12, 2000); h.fcg_force_from_displacement(k, inputs.FORCE_D, u, f)
+            c.record()
+        torch.cuda.synchronize()
+        ms = statistics.median(a.elapsed_time(c) for a, c in sev)
+        out[f"force_via_displacement_{name}_L2048_f64"] = {
+            "iterations": it, "status": st, "final_rel_residual": rr, "ms_per_solve": ms,
+            "speedup_over_force_solve": out["force_solve_L2048_f64"]["ms_per_solve"] / ms,
+            "note": "b = K D, (K + G^-1) u = b to 1e-12, f = -k (u - D); same forces as force_solve_L2048_f64 to ~1e-10 (tests)"}
+    h.close()
     L, nsteps = 256, 500
     h = binding.Fcg(L, torch.float64)
     h.fcg_set_spectrum(h.fcg_kernel_spectrum(h.fcg_green_function(inputs.GREEN_NU, inputs.GREEN_E, inputs.GREEN_A)))

@@ -219,6 +219,16 @@ int fcg_fracture_end(fcg_handle h, long long* index_host, int* iters_host, int* 
  *                        At L = 256 and 512 the whole loop -- every solve and every break step -- is ONE cooperative launch
  *                        with k, f, t resident in shared memory (fcg_fused.cuh, FORCE variant); else one graph per solve
  *                        and one break kernel per step, driven from the host.  Blocks. */
+/* The same state through the displacements (reading F7): eliminating f instead of u from (1a), (1b) gives
+ * (K + G^-1) u = K D, the symmetric system of fcg_solve / fcg_pcg_solve with the spectrum 1 / g and the right-hand side K D; its
+ * iteration count does not grow with L (24-34 against 60, 83, 144, .. of eq. (2) at L = 256, 512, 2048), so this is the fast
+ * way to the forces.  The three element-wise maps of that route (all asynchronous, one IEEE operation per element and step):
+ *   fcg_inverse_spectrum         s = 1 / g  (L x L, row-major [m][n]; may be in place): the spectrum of G^-1, for fcg_set_spectrum
+ *   fcg_force_rhs                b = k * D  (the right-hand side K D; b must not alias k)
+ *   fcg_force_from_displacement  f = -k (u - D), eq. (1a), evaluated as k * (D - u); f may alias u */
+int fcg_inverse_spectrum(fcg_handle h, const void* g, void* s);
+int fcg_force_rhs(fcg_handle h, const void* k, double D, void* b);
+int fcg_force_from_displacement(fcg_handle h, const void* k, double D, const void* u, void* f);
 int fcg_green_function(fcg_handle h, double nu, double E, double a, void* G);
 int fcg_kernel_spectrum(fcg_handle h, const void* G, void* s);
 int fcg_force_apply(fcg_handle h, const void* k, const void* x, void* y);

@@ -28,7 +28,7 @@ EXPORTS = ["fcg_workspace_bytes", "fcg_create", "fcg_destroy", "fcg_set_option",
            "fcg_set_preconditioner", "fcg_pcg_solve", "fcg_profile_pcg_iteration", "fcg_pcg_fracture",
            "fcg_fracture_begin", "fcg_fracture_end",
            "fcg_green_function", "fcg_kernel_spectrum", "fcg_force_apply", "fcg_force_solve", "fcg_force_break_step",
-           "fcg_force_fracture"]
+           "fcg_force_fracture", "fcg_inverse_spectrum", "fcg_force_rhs", "fcg_force_from_displacement"]
 
 _lib = None
 
@@ -69,6 +69,9 @@ def lib() -> C.CDLL:
         L.fcg_green_function.argtypes = [vp, d, d, d, vp]; L.fcg_green_function.restype = i
         L.fcg_kernel_spectrum.argtypes = [vp, vp, vp]; L.fcg_kernel_spectrum.restype = i
         L.fcg_force_apply.argtypes = [vp, vp, vp, vp]; L.fcg_force_apply.restype = i
+        L.fcg_inverse_spectrum.argtypes = [vp, vp, vp]; L.fcg_inverse_spectrum.restype = i
+        L.fcg_force_rhs.argtypes = [vp, vp, d, vp]; L.fcg_force_rhs.restype = i
+        L.fcg_force_from_displacement.argtypes = [vp, vp, d, vp, vp]; L.fcg_force_from_displacement.restype = i
         L.fcg_force_solve.argtypes = [vp, vp, d, vp, d, i, C.POINTER(i), C.POINTER(d)]; L.fcg_force_solve.restype = i
         L.fcg_force_break_step.argtypes = [vp, vp, vp, vp, C.POINTER(ll), C.POINTER(d)]; L.fcg_force_break_step.restype = i
         L.fcg_force_fracture.argtypes = [vp, vp, d, vp, vp, i, d, i, vp, vp, vp, C.POINTER(i)]; L.fcg_force_fracture.restype = i
@@ -279,6 +282,27 @@ class Fcg:
         if st != FCG_OK:
             self._raise(st)
         return s
+
+    def fcg_inverse_spectrum(self, g: torch.Tensor, s: torch.Tensor | None = None) -> torch.Tensor:
+        s = torch.empty_like(g) if s is None else s
+        st = self._lib.fcg_inverse_spectrum(self._h, self._chk(g, self.N), self._chk(s, self.N))
+        if st != FCG_OK:
+            self._raise(st)
+        return s
+
+    def fcg_force_rhs(self, k: torch.Tensor, D: float, b: torch.Tensor | None = None) -> torch.Tensor:
+        b = torch.empty_like(k) if b is None else b
+        st = self._lib.fcg_force_rhs(self._h, self._chk(k, self.N), float(D), self._chk(b, self.N))
+        if st != FCG_OK:
+            self._raise(st)
+        return b
+
+    def fcg_force_from_displacement(self, k: torch.Tensor, D: float, u: torch.Tensor, f: torch.Tensor | None = None) -> torch.Tensor:
+        f = torch.empty_like(u) if f is None else f
+        st = self._lib.fcg_force_from_displacement(self._h, self._chk(k, self.N), float(D), self._chk(u, self.N), self._chk(f, self.N))
+        if st != FCG_OK:
+            self._raise(st)
+        return f
 
     def fcg_force_apply(self, k: torch.Tensor, x: torch.Tensor, y: torch.Tensor | None = None) -> torch.Tensor:
         y = torch.empty_like(x) if y is None else y

@@ -930,6 +930,30 @@ int fcg_kernel_spectrum(fcg_handle h, const void* G, void* s) {
     return h->dtype == FCG_F64 ? kernel_spectrum_impl<double>(h, G, s) : kernel_spectrum_impl<float>(h, G, s);
 }
 
+int fcg_inverse_spectrum(fcg_handle h, const void* g, void* s) {
+    if (!h || !g || !s) return fail(h, FCG_INVALID_ARG, "null argument");
+    if (h->dtype == FCG_F64) inverse_spectrum_kernel<double><<<h->vec_blocks(), 256, 0, h->stream>>>((const double*)g, (double*)s, h->N);
+    else inverse_spectrum_kernel<float><<<h->vec_blocks(), 256, 0, h->stream>>>((const float*)g, (float*)s, h->N);
+    FCG_CK(h, cudaGetLastError());
+    return FCG_OK;
+}
+
+int fcg_force_rhs(fcg_handle h, const void* k, double D, void* b) {
+    if (!h || !k || !b || !std::isfinite(D)) return fail(h, FCG_INVALID_ARG, "null argument or D not finite");
+    if (h->dtype == FCG_F64) scale_kernel<double><<<h->vec_blocks(), 256, 0, h->stream>>>((const double*)k, (double*)b, h->N, D);
+    else scale_kernel<float><<<h->vec_blocks(), 256, 0, h->stream>>>((const float*)k, (float*)b, h->N, (float)D);
+    FCG_CK(h, cudaGetLastError());
+    return FCG_OK;
+}
+
+int fcg_force_from_displacement(fcg_handle h, const void* k, double D, const void* u, void* f) {
+    if (!h || !k || !u || !f || !std::isfinite(D)) return fail(h, FCG_INVALID_ARG, "null argument or D not finite");
+    if (h->dtype == FCG_F64) force_from_displacement_kernel<double><<<h->vec_blocks(), 256, 0, h->stream>>>((const double*)k, (const double*)u, (double*)f, h->N, D);
+    else force_from_displacement_kernel<float><<<h->vec_blocks(), 256, 0, h->stream>>>((const float*)k, (const float*)u, (float*)f, h->N, (float)D);
+    FCG_CK(h, cudaGetLastError());
+    return FCG_OK;
+}
+
 int fcg_force_apply(fcg_handle h, const void* k, const void* x, void* y) {
     if (!h || !k || !x || !y) return fail(h, FCG_INVALID_ARG, "null argument");
     if (y == k || y == x) return fail(h, FCG_INVALID_ARG, "y must not alias k or x");

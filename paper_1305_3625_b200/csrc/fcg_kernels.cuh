@@ -265,6 +265,22 @@ __global__ void __launch_bounds__(256) cg_kpp0_kernel(const T* __restrict__ k, c
     if (threadIdx.x == 0) sc->kpp = tot[0];
 }
 
+// The force problem through the displacements (reading F7): (K + G^-1) u = K D is fcg_solve / fcg_pcg_solve
+// with the spectrum 1 / g and the right-hand side K D; the two element-wise maps around it, one IEEE operation per step.
+template <typename T>
+__global__ void __launch_bounds__(256) inverse_spectrum_kernel(const T* __restrict__ g, T* __restrict__ s, size_t n) {
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) s[i] = (T)1 / g[i];
+}
+// f = -k (u - D), eq. (1a), as k * (D - u);  b != nullptr: also the right-hand side b = k * D
+template <typename T>
+__global__ void __launch_bounds__(256) force_from_displacement_kernel(const T* __restrict__ k, const T* __restrict__ u, T* __restrict__ f, size_t n, T D) {
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) f[i] = k[i] * (D - u[i]);
+}
+template <typename T>
+__global__ void __launch_bounds__(256) scale_kernel(const T* __restrict__ k, T* __restrict__ b, size_t n, T D) {
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) b[i] = k[i] * D;
+}
+
 // Reading F1 checked on the device before a force solve chooses the three-launch iteration: are all k_i in {0, kappa} with kappa > 0,
 // and is the start vector zero on the broken bonds?  Doubles >= 0 order like their bit patterns, so max k and min positive k are
 // integer atomics: out[0] = bits(max k), out[1] = ~bits(min positive k) (so that a memset to 0 initialises both), out[2] = 1 if any
