@@ -91,6 +91,9 @@ def _declare(L: C.CDLL) -> None:
         f.argtypes = [_ll, _vp, _vp]; f.restype = None
         f = getattr(L, "oracle_force_from_displacement" + suf)
         f.argtypes = [_ll, _vp, _d, _vp, _vp]; f.restype = None
+        f = getattr(L, "oracle_force_fracture_displacement" + suf)
+        f.argtypes = [_i, _vp, _vp, _d, _vp, _vp, _vp, _i, _d, _i, _d, _i, _vp, _vp, _vp, _vp]
+        f.restype = _i
         f = getattr(L, "oracle_force_break_step" + suf)
         f.argtypes = [_ll, _vp, _vp, _vp, C.POINTER(_ll), C.POINTER(_d), C.POINTER(_d)]
         f.restype = _i
@@ -343,3 +346,20 @@ def force_fracture(g, k, D: float, f, t, nsteps: int, tol: float, maxit: int):
     done = getattr(lib(), "oracle_force_fracture" + _suf(dt))(L, _p(g), _p(k), float(D), _p(f), _p(t), int(nsteps),
                                                               float(tol), int(maxit), _p(index), _p(iters), _p(ratio), _p(gap))
     return dict(index=index, iters=iters, ratio=ratio, gap=gap, steps=int(done))
+
+
+def force_fracture_displacement(sinv, k, D: float, u, t, nsteps: int, tol: float, maxit: int, kbar: float | None = None):
+    """Quasi-static loop of the force model through the displacements (reading F7); PCG solves when kbar is given.
+    In-place on k and u. Returns dict(index, iters, ratio, gap, steps, f)."""
+    dt = k.dtype; L = k.shape[0]
+    sinv = _arr(sinv, dt, (L, L)); t = _arr(t, dt, (L, L))
+    if not (k.flags.c_contiguous and u.flags.c_contiguous and u.dtype == dt):
+        raise ValueError("k, u must be C-contiguous arrays of one dtype (modified in place)")
+    index = np.full(nsteps, -1, np.int64); iters = np.zeros(nsteps, np.int32)
+    ratio = np.full(nsteps, np.nan, np.float64); gap = np.full(nsteps, np.nan, np.float64)
+    f = np.zeros((L, L), dt)
+    done = getattr(lib(), "oracle_force_fracture_displacement" + _suf(dt))(
+        L, _p(sinv), _p(k), float(D), _p(u), _p(f), _p(t), 0 if kbar is None else 1, 0.0 if kbar is None else float(kbar),
+        int(nsteps), float(tol), int(maxit), _p(index), _p(iters), _p(ratio), _p(gap))
+    return dict(index=index, iters=iters, ratio=ratio, gap=gap, steps=int(done), f=f)
+

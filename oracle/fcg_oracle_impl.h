@@ -489,3 +489,36 @@ int FN(oracle_force_fracture)(int L, const REAL* g, REAL* k, double D, REAL* f, 
     }
     return nsteps;
 }
+
+/* The quasi-static loop of the force model through the displacements (reading F7): each step forms b = K D, solves
+ * (K + G^-1) u = b from the previous u -- by oracle_cg, or by oracle_pcg when use_pcg (preconditioner M = kbar I + G^-1, kbar
+ * fixed for the whole loop) --, evaluates the forces by eq. (1a), f_i = k_i (D - u_i), and breaks the bond with the largest
+ * f_i / t_i (reading F2: one IEEE divide in double over {k_i > 0}, ties -> lowest i, NaN skipped; k_i = 0).  u is NOT changed by
+ * the break (it is the plate's displacement, and the warm start of the next solve).  The break sequence is a property of the
+ * exact solutions, so it coincides with oracle_force_fracture's wherever the top-2 gap exceeds the solver error.
+ *   sinv  = 1 / g (oracle_inverse_spectrum);  f: work array of N, on return the forces of the LAST solve with the broken bond zeroed
+ * returns the number of completed steps, or a negative solver status. */
+int FN(oracle_force_fracture_displacement)(int L, const REAL* sinv, REAL* k, double D, REAL* u, REAL* f, const REAL* t, int use_pcg,
+                                           double kbar, int nsteps, double tol, int maxit,
+                                           long long* out_index, int* out_iters, double* out_ratio, double* out_gap)
+{
+    long long N = (long long)L * L;
+    REAL* b = (REAL*)malloc(sizeof(REAL) * (size_t)N);
+    int step = 0;
+    for (; step < nsteps; ++step) {
+        int it; double rr;
+        for (long long i = 0; i < N; ++i) b[i] = k[i] * (REAL)D;
+        int st = use_pcg ? FN(oracle_pcg)(L, sinv, k, b, u, kbar, tol, maxit, &it, &rr, NULL, NULL, NULL, NULL)
+                         : FN(oracle_cg)(L, sinv, k, b, u, tol, maxit, &it, &rr, NULL, NULL, NULL);
+        if (st < 0) { free(b); return st; }
+        FN(oracle_force_from_displacement)(N, k, D, u, f);
+        long long idx; double ratio, second;
+        int bs = FN(oracle_force_break_step)(N, k, f, t, &idx, &ratio, &second);
+        if (bs < 0) break;
+        out_index[step] = idx; out_iters[step] = it;
+        if (out_ratio) out_ratio[step] = ratio;
+        if (out_gap) out_gap[step] = (ratio - second) / fabs(ratio);
+    }
+    free(b);
+    return step;
+}

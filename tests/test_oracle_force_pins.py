@@ -232,3 +232,39 @@ def test_force_fracture_gradient_makes_a_front():
     k = inputs.force_k(L); f = np.zeros((L, L))
     out = orc.force_fracture(g, k, 1.0, f, t, 2 * L, 1e-10, 500)
     assert out["steps"] == 2 * L and np.all(out["index"] // L < 4)
+
+
+def test_force_fracture_through_displacements_same_sequence_and_brute_force():
+    """Reading F7 applied to the loop: the break sequence and the critical ratios are properties of the exact states, so the loop
+    through the displacements (CG and PCG solves) must reproduce the loop on eq. (2) and a dense-LAPACK replay, step by step."""
+    L = 8
+    G = orc.green_function(L, NU, E, A); g = orc.kernel_spectrum(G); sinv = orc.inverse_spectrum(g)
+    t = inputs.gradient_thresholds(L, 0.5)
+    nsteps = 14
+    ref = orc.force_fracture(g, inputs.force_k(L), 1.0, np.zeros((L, L)), t, nsteps, 1e-13, 500)
+    kk = inputs.force_k(L).ravel(); GG = dense_G(G)
+    dense_idx, dense_ratio = [], []
+    for s in range(nsteps):
+        fd = np.linalg.solve(np.eye(L * L) + np.diag(kk) @ GG, kk)
+        r = np.where(kk > 0, fd / t.ravel(), -np.inf)
+        dense_idx.append(int(np.argmax(r))); dense_ratio.append(r.max()); kk[dense_idx[-1]] = 0.0
+    for kbar in (None, 1.0):
+        k = inputs.force_k(L); u = np.zeros((L, L))
+        out = orc.force_fracture_displacement(sinv, k, 1.0, u, t, nsteps, 1e-13, 2000, kbar=kbar)
+        assert out["steps"] == nsteps
+        assert np.array_equal(out["index"], ref["index"]) and list(out["index"]) == dense_idx
+        assert np.abs(out["ratio"] / np.array(dense_ratio) - 1).max() < 1e-9
+        assert np.array_equal(k.ravel() == 0, kk == 0)
+        # u is the plate's displacement of the last solved state: (1b) with that state's forces, broken bond still carrying
+        f_last = out["f"].copy(); f_last.ravel()[out["index"][-1]] = dense_ratio[-1] * t.ravel()[out["index"][-1]]
+        assert np.abs(orc.conv_direct(G, f_last) - u).max() < 1e-9
+        assert out["f"].ravel()[out["index"][-1]] == 0 and out["gap"].min() > 0
+    # first step from the intact plate: the weakest bond, at D_c = t_min (1 + kappa g(0)) / kappa, after a uniform solve
+    assert out["index"][0] == int(np.argmin(t)) and abs(1.0 / out["ratio"][0] - t.min() * (1 + G.sum())) < 1e-9
+    # PCG needs fewer iterations than CG on the same route once bonds are broken
+    k = inputs.force_k(L); cg_it = orc.force_fracture_displacement(sinv, k, 1.0, np.zeros((L, L)), t, nsteps, 1e-13, 2000)["iters"].sum()
+    assert out["iters"].sum() < cg_it
+    # running out of bonds
+    k = np.zeros((L, L)); k[1, 2] = k[5, 5] = 1.0
+    o2 = orc.force_fracture_displacement(sinv, k, 1.0, np.zeros((L, L)), t, 5, 1e-12, 500)
+    assert o2["steps"] == 2 and not k.any()
