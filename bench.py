@@ -336,10 +336,30 @@ def bench_force(binding, torch, inputs):
         index, iters, ratio, done, st = h.fcg_force_fracture(k, inputs.FORCE_D, f, t, nsteps, 1e-12, 1000)
         dt_s = time.perf_counter() - t0
         best = dt_s if best is None else min(best, dt_s)
+    eq2_wall, eq2_steps = best, int(done)
     out["force_fracture_L256_f64"] = {"steps": int(done), "iterations": int(iters.sum()), "wall_s": best, "steps_per_s": int(done) / best,
                                       "us_per_iteration": 1e6 * best / max(int(iters.sum()), 1), "status": int(st),
                                       "launches": h.fcg_last_launch_count()}
     h.close()
+    # the same loop through the displacements (reading F7), CG and PCG solves: same break sequence (tests), a fraction of the iterations
+    for name, pcg in (("cg", False), ("pcg", True)):
+        h = binding.Fcg(L, torch.float64)
+        s = h.fcg_inverse_spectrum(h.fcg_kernel_spectrum(h.fcg_green_function(inputs.GREEN_NU, inputs.GREEN_E, inputs.GREEN_A)))
+        h.fcg_set_spectrum(s)
+        if pcg:
+            h.fcg_set_preconditioner(s, 1.0)
+        best = None
+        for rep in range(2):
+            k = to(inputs.force_k(L)); u = torch.zeros((L, L), dtype=torch.float64, device="cuda")
+            torch.cuda.synchronize(); t0 = time.perf_counter()
+            index, iters, ratio, done, st = h.fcg_force_fracture_displacement(k, inputs.FORCE_D, u, t, nsteps, 1e-12, 2000, use_pcg=pcg)
+            dt_s = time.perf_counter() - t0
+            best = dt_s if best is None else min(best, dt_s)
+        out[f"force_fracture_via_displacement_{name}_L256_f64"] = {
+            "steps": int(done), "iterations": int(iters.sum()), "wall_s": best, "steps_per_s": int(done) / best,
+            "us_per_iteration": 1e6 * best / max(int(iters.sum()), 1), "status": int(st), "launches": h.fcg_last_launch_count(),
+            "speedup_over_force_fracture": (eq2_wall / max(eq2_steps, 1)) / (best / max(int(done), 1))}
+        h.close()
     return out
 
 

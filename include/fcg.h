@@ -225,7 +225,18 @@ int fcg_fracture_end(fcg_handle h, long long* index_host, int* iters_host, int* 
  * way to the forces.  The three element-wise maps of that route (all asynchronous, one IEEE operation per element and step):
  *   fcg_inverse_spectrum         s = 1 / g  (L x L, row-major [m][n]; may be in place): the spectrum of G^-1, for fcg_set_spectrum
  *   fcg_force_rhs                b = k * D  (the right-hand side K D; b must not alias k)
- *   fcg_force_from_displacement  f = -k (u - D), eq. (1a), evaluated as k * (D - u); f may alias u */
+ *   fcg_force_from_displacement  f = -k (u - D), eq. (1a), evaluated as k * (D - u); f may alias u
+ *
+ *   fcg_force_fracture_displacement  the quasi-static loop of the force model on that route: nsteps times { b = K D;
+ *                        (K + G^-1) u = b by fcg_solve, or fcg_pcg_solve when use_pcg != 0, warm-started from the current u;
+ *                        f = -k (u - D); break argmax over {k_i > 0} of f_i / t_i (reading F2), k_i = 0 }.  u is the plate's
+ *                        displacement and is not changed by a break.  Before the call: fcg_set_spectrum with 1 / g, and for
+ *                        use_pcg fcg_set_preconditioner with the same spectrum and a kbar (fixed for the whole loop).  Results
+ *                        as fcg_force_fracture (ratio = winning f/t: the bond breaks at D_c = D / ratio); the break sequence is
+ *                        that of fcg_force_fracture wherever the top-2 gap exceeds the solver error.  At L = 256 and 512 ONE
+ *                        cooperative launch for the whole loop (fcg_fused.cuh, FORCE = 2).  Blocks. */
+int fcg_force_fracture_displacement(fcg_handle h, void* k, double D, void* u, const void* t, int nsteps, double tol, int maxit,
+                                    int use_pcg, long long* index_host, int* iters_host, double* ratio_host, int* steps_done_host);
 int fcg_inverse_spectrum(fcg_handle h, const void* g, void* s);
 int fcg_force_rhs(fcg_handle h, const void* k, double D, void* b);
 int fcg_force_from_displacement(fcg_handle h, const void* k, double D, const void* u, void* f);

@@ -1028,6 +1028,68 @@ int fcg_force_fracture(fcg_handle h, void* k, double D, void* f, const void* t, 
     return st < 0 ? st : FCG_OK;
 }
 
+// quasi-static loop of the force model through the displacements (reading F7)
+int fcg_force_fracture_displacement(fcg_handle h, void* k, double D, void* u, const void* t, int nsteps, double tol, int maxit, int use_pcg,
+                                    long long* index_host, int* iters_host, double* ratio_host, int* steps_done_host) {
+    if (!h || !k || !u || !t || nsteps < 0 || !index_host || !iters_host) return fail(h, FCG_INVALID_ARG, "bad argument");
+    if (!(tol >= 0.0) || maxit < 0 || !std::isfinite(D)) return fail(h, FCG_INVALID_ARG, "tol must be >= 0, maxit >= 0, D finite");
+    if (!h->have_spectrum) return fail(h, FCG_NO_SPECTRUM, "fcg_set_spectrum has not been called");
+    if (use_pcg && !h->have_precond) return fail(h, FCG_NO_SPECTRUM, "fcg_set_preconditioner has not been called");
+    if (steps_done_host) *steps_done_host = 0;
+    if (h->fused() && nsteps > 0) {
+        // small lattices: the whole loop in one cooperative kernel (fcg_fused.cuh, FORCE = 2)
+        { const int e0 = frac_reserve(h, nsteps); if (e0 != FCG_OK) return e0; }
+        FusedArgs A{};
+        A.form = 2; A.D = D; A.k = k; A.f = nullptr; A.u = u; A.Tf = h->ws + h->lay.Tb; A.shat = h->ws + h->lay.shat; A.tw = h->ws + h->lay.tw;
+        A.mhat = use_pcg ? h->ws + h->lay.mhat : nullptr;
+        A.partial = h->at<double>(h->lay.partial_row); A.counter = &h->sc()->ticket[3]; A.sc = h->sc(); A.tol = tol; A.maxit = maxit;
+        A.nsteps = nsteps; A.t = t; A.k_out = k; A.out_index = h->frac_idx; A.out_iters = h->frac_it; A.out_ratio = h->frac_ratio;
+        A.brk_r = h->at<double>(h->lay.brk_r); A.brk_i = h->at<long long>(h->lay.brk_i);
+        FCG_CK(h, cudaMemsetAsync(h->sc(), 0, sizeof(Scalars), h->stream));
+        cudaError_t e = h->tab->fused_solve(&A, h->stream);
+        if (e == cudaSuccess) {
+            FCG_CK(h, cudaMemcpyAsync(h->h_sc, h->sc(), sizeof(Scalars), cudaMemcpyDeviceToHost, h->stream));
+            FCG_CK(h, cudaStreamSynchronize(h->stream));
+            h->launches = 1;
+            const int done = h->h_sc->steps_done;
+            if (done > 0) {
+                FCG_CK(h, cudaMemcpyAsync(index_host, h->frac_idx, (size_t)done * sizeof(long long), cudaMemcpyDeviceToHost, h->stream));
+                FCG_CK(h, cudaMemcpyAsync(iters_host, h->frac_it, (size_t)done * sizeof(int), cudaMemcpyDeviceToHost, h->stream));
+                if (ratio_host) FCG_CK(h, cudaMemcpyAsync(ratio_host, h->frac_ratio, (size_t)done * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+                FCG_CK(h, cudaStreamSynchronize(h->stream));
+            }
+            if (steps_done_host) *steps_done_host = done;
+            if (h->h_sc->status == FCG_CUDA_ERROR) h->err = "fused quasi-static loop: grid barrier timed out";
+            return h->h_sc->status < 0 ? h->h_sc->status : FCG_OK;
+        }
+        cudaGetLastError();
+        h->err = std::string("cooperative launch failed (") + cudaGetErrorString(e) + "); using the graph path";
+        h->fused_opt = 0;
+    }
+    // larger lattices: the library's own calls in turn, with two scratch vectors (b = K D and the forces)
+    const size_t bytes = h->N * h->w;
+    if (!h->hk) { FCG_CK(h, cudaMalloc(&h->hk, bytes)); FCG_CK(h, cudaMalloc(&h->hf, bytes)); FCG_CK(h, cudaMalloc(&h->hu, bytes)); }
+    void* b = h->hf; void* frc = h->hk;
+    long long total = 0; int done = 0, st = FCG_OK;
+    for (int step = 0; step < nsteps; ++step) {
+        int it = 0; double rr = 0.0;
+        if ((st = fcg_force_rhs(h, k, D, b)) < 0) break;
+        st = use_pcg ? fcg_pcg_solve(h, k, b, u, tol, maxit, &it, &rr) : fcg_solve(h, k, b, u, tol, maxit, &it, &rr);
+        total += h->launches + 2;
+        if (st < 0) break;
+        if ((st = fcg_force_from_displacement(h, k, D, u, frc)) < 0) break;
+        long long idx = -1; double ratio = 0.0;
+        st = fcg_force_break_step(h, k, frc, t, &idx, &ratio);
+        total += h->launches;
+        if (st < 0) break;
+        index_host[step] = idx; iters_host[step] = it; if (ratio_host) ratio_host[step] = ratio;
+        ++done; st = FCG_OK;
+    }
+    if (steps_done_host) *steps_done_host = done;
+    h->launches = total;
+    return st < 0 ? st : FCG_OK;
+}
+
 int fcg_profile_iteration(fcg_handle h, const void* k, const void* f, void* u, int iters, double* ms_host) {
     if (!h || !k || !f || !u || iters < 1 || !ms_host) return fail(h, FCG_INVALID_ARG, "bad argument");
     if (!h->have_spectrum) return fail(h, FCG_NO_SPECTRUM, "fcg_set_spectrum has not been called");

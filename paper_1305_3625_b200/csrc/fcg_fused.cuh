@@ -78,9 +78,13 @@ __device__ __forceinline__ bool grid_barrier(unsigned int* counter, unsigned int
 // FORCE: the paper's own system in the bond forces, in the textbook order of Listing 2 (q = (I + K G) p is formed and kept, p.q is a
 // dot product, then u and r are updated: one more grid barrier per iteration than the spectral search length of the displacement
 // form, which would need k o p = kappa p, i.e. reading F1, to hold exactly) -- the same arithmetic as the oracle for any k.
-template <typename T, typename P, bool FORCE = false>
+// FORCE = 2: the force model through the displacements (reading F7): the arithmetic of FORCE = 0 (spectral
+// search length, optional preconditioner) on (K + G^-1) u = K D, with b = K D re-formed in shared memory at every step and the
+// break rule of the force model, f_i / t_i with f_i = k_i (D - u_i) by eq. (1a); u is not touched by the break.
+template <typename T, typename P, int FORCE = 0>
 __global__ void __launch_bounds__(P::NT) cg_fused_kernel(const FusedArgs A)
 {
+    constexpr bool FQ = FORCE == 1, FD = FORCE == 2;
     using AS = AsyncShape<T, P>;
     using FS = FusedShape<T, P>;
     constexpr int L = P::N, S = P::S, NT = P::NT, R1 = AS::R1, Q1 = AS::Q1, PER1 = AS::PER1, PM = per_max<P>();
@@ -310,7 +314,7 @@ __global__ void __launch_bounds__(P::NT) cg_fused_kernel(const FusedArgs A)
         const size_t row0 = (size_t)(2 * (cta + j * G)) * L;
         for (int e = lt; e < 2 * L; e += NT) {         // the two rows are adjacent in memory
             V(j, 0, 0)[e] = gk[row0 + e]; V(j, 2, 0)[e] = gu[row0 + e];
-            if (!FORCE) V(j, 1, 0)[e] = gf[row0 + e];
+            if (FORCE == 0) V(j, 1, 0)[e] = gf[row0 + e];
             if (frac) V(j, 6, 0)[e] = static_cast<const T*>(A.t)[row0 + e];
         }
     }
@@ -335,7 +339,7 @@ __global__ void __launch_bounds__(P::NT) cg_fused_kernel(const FusedArgs A)
             T* pp = V(j, 4, 0);
             for (int e = lt; e < 2 * L; e += NT) pp[e] = (T)0;
         }
-        if (FORCE) {                                   // right-hand side b = K D (eq. (2)), one multiply in the working precision
+        if (FORCE != 0) {                                   // right-hand side b = K D (eq. (2)), one multiply in the working precision
             const T dv = (T)A.D;
             for (int j = 0; j < TPC; ++j) {
                 const T* kk = V(j, 0, 0); T* bb = V(j, 1, 0);
@@ -346,7 +350,7 @@ __global__ void __launch_bounds__(P::NT) cg_fused_kernel(const FusedArgs A)
         it = 0; status = ST_OK; zero_u = false;
         double beta = 0.0;
         T al_u = (T)0;                                 // FORCE: the search length between phases Q and U
-        int phase = (have_fn && !FORCE) ? PH_RESID : PH_FN;
+        int phase = (have_fn && FORCE == 0) ? PH_RESID : PH_FN;
         while (true) {
             double acc = 0.0, kpp = 0.0;
             bool bd = false;
@@ -367,7 +371,7 @@ __global__ void __launch_bounds__(P::NT) cg_fused_kernel(const FusedArgs A)
                     }
                 }
                 __syncthreads();
-            } else if (FORCE && phase == PH_U) {        // new x (95), residue (96), residue length (97)
+            } else if (FQ && phase == PH_U) {        // new x (95), residue (96), residue length (97)
                 for (int j = 0; j < TPC; ++j) {
                     T* uu = V(j, 2, 0); T* rv = V(j, 3, 0); const T* pp = V(j, 4, 0); const T* qq = V(j, 5, 0);
                     for (int e = lt; e < 2 * L; e += NT) {
@@ -379,19 +383,19 @@ __global__ void __launch_bounds__(P::NT) cg_fused_kernel(const FusedArgs A)
                 }
             }
             // ---- operator-shaped round trip: C u (RESID), C p (Q: A * p) or M^-1 r (Z)
-            if (phase != PH_FN && !(FORCE && phase == PH_U)) {
+            if (phase != PH_FN && !(FQ && phase == PH_U)) {
                 rows_forward(phase == PH_RESID ? 2 : (phase == PH_Q ? 4 : 3));
                 ok = grid_barrier(A.counter, target, G, &ok_smem) && ok;
                 double en = 0.0;
-                columns(phase == PH_Z ? mhat : shat, (!FORCE && phase == PH_Q) ? &en : nullptr);
+                columns(phase == PH_Z ? mhat : shat, (!FQ && phase == PH_Q) ? &en : nullptr);
                 double* ps = A.partial + (size_t)slot * G;
-                if (!FORCE && phase == PH_Q) {                    // this CTA's share of p.Ap = sum k p^2 + sum shat |P|^2, published before the barrier
+                if (!FQ && phase == PH_Q) {                    // this CTA's share of p.Ap = sum k p^2 + sum shat |P|^2, published before the barrier
                     const double mine = cta_sum(kpp + en);
                     if (lt == 0) ps[cta] = mine;
                 }
                 ok = grid_barrier(A.counter, target, G, &ok_smem) && ok;
                 T al = (T)0;
-                if (!FORCE && phase == PH_Q) {          // search length (94): every CTA adds the G shares in the same order
+                if (!FQ && phase == PH_Q) {          // search length (94): every CTA adds the G shares in the same order
                     double v = 0.0;
                     for (int i = lt; i < G; i += NT) v += __ldcg(ps + i);
                     slot = (slot + 1) & 3;
@@ -402,11 +406,11 @@ __global__ void __launch_bounds__(P::NT) cg_fused_kernel(const FusedArgs A)
                 if (!bd) rows_inverse([&](int j, int e, T c0, T c1) {
                     if (phase == PH_RESID) {                                  // r = f - (k o u + C u);  FORCE: r = b - (u + k o G u)
                         const T* kk = V(j, 0, 0); const T* ff = V(j, 1, 0); const T* uu = V(j, 2, 0); T* rv = V(j, 3, 0);
-                        const T r0 = ff[e] - (FORCE ? uu[e] + kk[e] * c0 : kk[e] * uu[e] + c0),
-                                r1 = ff[L + e] - (FORCE ? uu[L + e] + kk[L + e] * c1 : kk[L + e] * uu[L + e] + c1);
+                        const T r0 = ff[e] - (FQ ? uu[e] + kk[e] * c0 : kk[e] * uu[e] + c0),
+                                r1 = ff[L + e] - (FQ ? uu[L + e] + kk[L + e] * c1 : kk[L + e] * uu[L + e] + c1);
                         rv[e] = r0; rv[L + e] = r1;
                         acc += (double)r0 * (double)r0; acc += (double)r1 * (double)r1;
-                    } else if (FORCE && phase == PH_Q) {                      // q = p + k o (G p) (eq. (2)), kept; p.q
+                    } else if (FQ && phase == PH_Q) {                      // q = p + k o (G p) (eq. (2)), kept; p.q
                         const T* kk = V(j, 0, 0); const T* pp = V(j, 4, 0); T* qq = V(j, 5, 0);
                         const T p0 = pp[e], p1 = pp[L + e];
                         const T q0 = p0 + kk[e] * c0, q1 = p1 + kk[L + e] * c1;
@@ -442,11 +446,11 @@ __global__ void __launch_bounds__(P::NT) cg_fused_kernel(const FusedArgs A)
                 if (!(s0 > 0.0) || !isfinite(s0)) { status = ST_BREAKDOWN; break; }
                 beta = it == 0 ? 0.0 : s0 / rho;
                 rho = s0; phase = PH_Q;
-            } else if (FORCE && phase == PH_Q) {        // search length (94): a dot product, as the oracle forms it
+            } else if (FQ && phase == PH_Q) {        // search length (94): a dot product, as the oracle forms it
                 if (!(s0 > 0.0) || !isfinite(s0)) { status = ST_BREAKDOWN; break; }
                 al_u = (T)(rho / s0); phase = PH_U;
             } else {
-                if (FORCE) phase = PH_Q;
+                if (FQ) phase = PH_Q;
                 rr = s0; ++it;
                 if (sqrt(rr) <= A.tol * sqrt(fn2)) { if (!pcg) rho = rr; break; }                 // check convergence (99)
                 if (it >= A.maxit) { if (!pcg) rho = rr; status = ST_NOT_CONVERGED; break; }
@@ -472,7 +476,7 @@ __global__ void __launch_bounds__(P::NT) cg_fused_kernel(const FusedArgs A)
             for (int e = lt; e < 2 * L; e += NT) {
                 const T ki = kk[e];
                 if (!(ki > (T)0)) continue;
-                const double load = FORCE ? (double)uu[e] : (double)ki * (double)uu[e];      // FORCE (reading F2): f_i / t_i
+                const double load = FQ ? (double)uu[e] : FD ? (double)(ki * ((T)A.D - uu[e])) : (double)ki * (double)uu[e];      // FORCE (reading F2): f_i / t_i
                 const double rt = load / (double)tt[e];
                 if (rt != rt) continue;
                 if (better(rt, row0 + e, br, bi)) { br = rt; bi = row0 + e; }
@@ -493,12 +497,12 @@ __global__ void __launch_bounds__(P::NT) cg_fused_kernel(const FusedArgs A)
             const int A2 = (int)(bi / (2 * L));
             if (A2 % G == cta && lt == 0) {
                 V(A2 / G, 0, 0)[bi - (long long)A2 * 2 * L] = (T)0;
-                if (FORCE) V(A2 / G, 2, 0)[bi - (long long)A2 * 2 * L] = (T)0;        // a broken bond carries no force
+                if (FQ) V(A2 / G, 2, 0)[bi - (long long)A2 * 2 * L] = (T)0;        // a broken bond carries no force
             }
         }
         if (cta == 0 && lt == 0) {
             A.out_index[step] = bi; A.out_iters[step] = it;
-            if (FORCE && A.out_ratio) A.out_ratio[step] = br;
+            if (FORCE != 0 && A.out_ratio) A.out_ratio[step] = br;
         }
         steps_done = step + 1;
         status = ST_OK;

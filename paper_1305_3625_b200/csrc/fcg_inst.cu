@@ -63,7 +63,8 @@ template <typename T> struct Inst {
         }
         if constexpr (FS::valid) {
             if ((e = prep(cg_fused_kernel<T, P>, FS::smem)) != cudaSuccess) return e;
-            if ((e = prep(cg_fused_kernel<T, P, true>, FS::smem)) != cudaSuccess) return e;
+            if ((e = prep(cg_fused_kernel<T, P, 1>, FS::smem)) != cudaSuccess) return e;
+            if ((e = prep(cg_fused_kernel<T, P, 2>, FS::smem)) != cudaSuccess) return e;
         }
         return prep(col_kernel<T, P, CS::COLS>, CS::smem);
     }
@@ -180,7 +181,8 @@ template <typename T> struct Inst {
         if constexpr (FS::valid) {
             FusedArgs A = *static_cast<const FusedArgs*>(fused_args);
             void* params[] = {&A};
-            const void* fn = A.form ? (const void*)cg_fused_kernel<T, P, true> : (const void*)cg_fused_kernel<T, P>;
+            const void* fn = A.form == 1 ? (const void*)cg_fused_kernel<T, P, 1> : A.form == 2 ? (const void*)cg_fused_kernel<T, P, 2>
+                                                                                         : (const void*)cg_fused_kernel<T, P>;
             return cudaLaunchCooperativeKernel(fn, dim3(FS::G), dim3(P::NT), params, FS::smem, st);
         }
         return cudaErrorInvalidValue;

@@ -404,3 +404,56 @@ def test_force_through_displacements(B, L, dt):
         assert np.all(f.cpu().numpy()[k == 0] == 0)
         assert it < f_eq2["iters"]                                 # and in fewer iterations (the point of the route)
     h.close()
+
+
+@pytest.mark.parametrize("L,nsteps,grad,opts", [(64, 120, 0.0, {}), (256, 300, 1.0, {}), (256, 60, 1.0, dict(FCG_OPT_FUSED=0)),
+                                               (512, 60, 2.0, {}), (1024, 12, 1.0, {})])
+def test_force_fracture_through_displacements(B, L, nsteps, grad, opts):
+    """The quasi-static loop of the force model through the displacements (reading F7), CG and PCG solves: break indices identical
+    to the oracle's same loop AND to the oracle's loop on eq. (2); critical ratios to 1e-8; iteration counts within the CG parity
+    rules; k written back, u = the oracle's u; one launch where the loop is the cooperative kernel."""
+    dt = np.float64
+    _, g = green_spectrum_oracle(L, dt)
+    sinv = orc.inverse_spectrum(g)
+    t = inputs.gradient_thresholds(L, grad)
+    eq2 = orc.force_fracture(g, inputs.force_k(L), 1.0, np.zeros((L, L)), t, nsteps, 1e-12, 1000)
+    assert eq2["steps"] == nsteps and eq2["gap"].min() > 1e-7
+    for pcg in (False, True):
+        kbar = 1.0 if pcg else None
+        k_or = inputs.force_k(L); u_or = np.zeros((L, L))
+        ref = orc.force_fracture_displacement(sinv, k_or, 1.0, u_or, t, nsteps, 1e-12, 2000, kbar=kbar)
+        assert ref["steps"] == nsteps and np.array_equal(ref["index"], eq2["index"])
+        h = handle(B, L, dt, sinv, **opts)
+        if pcg:
+            h.fcg_set_preconditioner(dev(sinv), 1.0)
+        kd = dev(inputs.force_k(L)); ud = dev(np.zeros((L, L)))
+        index, iters, ratio, done, st = h.fcg_force_fracture_displacement(kd, 1.0, ud, dev(t), nsteps, 1e-12, 2000, use_pcg=pcg)
+        assert (done, st) == (nsteps, 0)
+        fused = L in (256, 512) and not opts
+        assert (h.fcg_last_launch_count() == 1) == fused
+        assert np.array_equal(index, ref["index"])
+        dit = np.abs(iters.astype(int) - ref["iters"].astype(int))
+        assert dit.max() <= 3 and np.mean(dit <= 2) >= 0.9, (dit.max(), np.mean(dit <= 2))
+        assert np.abs(ratio / ref["ratio"] - 1).max() < 1e-8 and np.abs(ratio / eq2["ratio"] - 1).max() < 1e-7
+        assert np.array_equal(kd.cpu().numpy(), k_or) and rel(ud.cpu().numpy(), u_or) < 1e-9
+        assert int(iters.sum()) < 0.6 * int(eq2["iters"].sum())          # the point of the route
+        h.close()
+
+
+def test_force_fracture_through_displacements_edges(B):
+    L, dt = 256, np.float64
+    _, g = green_spectrum_oracle(L, dt); sinv = orc.inverse_spectrum(g)
+    t = inputs.thresholds(L)
+    k = np.zeros((L, L)); k[3, 5] = k[100, 7] = k[200, 250] = 1.0
+    for opts in ({}, dict(FCG_OPT_FUSED=0)):
+        h = handle(B, L, dt, sinv, **opts)
+        kd, ud = dev(k), dev(np.zeros((L, L)))
+        index, iters, ratio, done, st = h.fcg_force_fracture_displacement(kd, 1.0, ud, dev(t), 5, 1e-12, 200)
+        k_or = k.copy(); u_or = np.zeros((L, L))
+        ref = orc.force_fracture_displacement(sinv, k_or, 1.0, u_or, t, 5, 1e-12, 200)
+        assert done == ref["steps"] == 3 and st == B.FCG_NO_CANDIDATE
+        assert np.array_equal(index[:3], ref["index"][:3]) and float(kd.abs().max()) == 0.0
+        assert np.abs(ratio[:3] / ref["ratio"][:3] - 1).max() < 1e-9
+        with pytest.raises(B.FcgError):
+            h.fcg_force_fracture_displacement(kd, 1.0, ud, dev(t), 5, 1e-12, 200, use_pcg=True)      # no preconditioner set
+        h.close()
