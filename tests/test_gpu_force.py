@@ -457,3 +457,35 @@ def test_force_fracture_through_displacements_edges(B):
         with pytest.raises(B.FcgError):
             h.fcg_force_fracture_displacement(kd, 1.0, ud, dev(t), 5, 1e-12, 200, use_pcg=True)      # no preconditioner set
         h.close()
+
+
+def test_force_through_displacements_full_size_sampled(B):
+    """L = 2048 fp64, the configuration bench.py --full times: forces from the displacement route (CG and PCG) must satisfy
+    eq. (2) -- residual by ONE oracle application of I + K G -- and the model equation (1a) with u = G f at sampled bonds
+    (direct sums of (1b) over all 4.2 M bonds), and agree with fcg_force_solve."""
+    L, dt = 2048, np.float64
+    G, g = green_spectrum_oracle(L, dt)
+    kh = inputs.force_k(L, 20); D = inputs.FORCE_D
+    h = handle(B, L, dt)
+    s = h.fcg_inverse_spectrum(dev(g)); h.fcg_set_spectrum(s); h.fcg_set_preconditioner(s, inputs.precond_kbar(kh))
+    k = dev(kh); b = h.fcg_force_rhs(k, D)
+    fs = []
+    for solve in (h.fcg_solve, h.fcg_pcg_solve):
+        u = dev(np.zeros((L, L)))
+        it, rr, st = solve(k, b, u, 1e-12, 2000)
+        assert st == 0 and it <= 40
+        f = h.fcg_force_from_displacement(k, D, u).cpu().numpy()
+        assert np.linalg.norm(kh * D - orc.force_apply(g, kh, f)) / np.linalg.norm(kh * D) <= 1e-9
+        assert np.all(f[kh == 0] == 0)
+        uh = u.cpu().numpy()
+        rng = np.random.default_rng(12)
+        for a, c in rng.integers(0, L, (4, 2)):
+            ui = float(np.sum(np.roll(np.roll(G[::-1, ::-1], a + 1, 0), c + 1, 1) * f))      # (1b) at bond (a, c)
+            assert abs(ui - uh[a, c]) < 1e-9 and abs(f[a, c] - (-kh[a, c] * (ui - D))) < 1e-9
+        fs.append(f)
+    h2 = handle(B, L, dt, g)
+    f2 = dev(np.zeros((L, L)))
+    it2, _, st2 = h2.fcg_force_solve(k, D, f2, 1e-12, 2000)
+    assert st2 == 0 and it2 > 3 * it
+    assert rel(fs[0], f2.cpu().numpy()) <= 1e-9 and rel(fs[1], f2.cpu().numpy()) <= 1e-9
+    h.close(); h2.close()
