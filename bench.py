@@ -505,13 +505,15 @@ def main():
     kms = res["kernel_ms"]
     dom = max(PASS_NAMES, key=lambda n: kms[n])
     achieved = PASS_NW[dom] * nw / (kms[dom] * 1e-3) / 1e9
-    traffic = None
+    traffic = traffic_warm = None
     tpath = os.path.join(ROOT, "profiles", "traffic.json")          # dram bytes per launch from the committed ncu --set full capture
     if os.path.exists(tpath):
         try:
-            traffic = json.load(open(tpath)).get(f"L{w.L}_{args.dtype}", {}).get(dom)     # cold-cache figure (profiles/r1_notes.md)
+            tj = json.load(open(tpath))
+            traffic = tj.get(f"L{w.L}_{args.dtype}", {}).get(dom)     # cold-cache figure (profiles/r1_notes.md)
+            traffic_warm = tj.get(f"warm_L{w.L}_{args.dtype}", {}).get(dom)   # single-pass capture with warm caches (profiles/r1_warm_traffic.md)
         except Exception:
-            traffic = None
+            traffic = traffic_warm = None
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": step_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -530,7 +532,7 @@ def main():
         "kernel_us": {n: 1e3 * kms[n] for n in PASS_NAMES},
         "kernel_gbs": {n: PASS_NW[n] * nw / (kms[n] * 1e-3) / 1e9 for n in PASS_NAMES},
         "roofline": {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": hbm_peak, "unit": "GB/s", "frac": achieved / hbm_peak,
-                     "traffic": traffic, "algorithmic_bytes_per_launch": PASS_NW[dom] * nw, "peak_source": peak_src},
+                     "traffic": traffic, "traffic_warm_caches": traffic_warm, "algorithmic_bytes_per_launch": PASS_NW[dom] * nw, "peak_source": peak_src},
         "e2e": {"value": res["e2e_iter_s"], "unit": UNIT, "h2d_bytes_per_step": res["h2d"], "d2h_bytes_per_step": res["d2h"]},
         "gpu_launches": launches,
         "clocks": clocks,
