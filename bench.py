@@ -360,6 +360,27 @@ def bench_force(binding, torch, inputs):
             "us_per_iteration": 1e6 * best / max(int(iters.sum()), 1), "status": int(st), "launches": h.fcg_last_launch_count(),
             "speedup_over_force_fracture": (eq2_wall / max(eq2_steps, 1)) / (best / max(int(done), 1))}
         h.close()
+    # ensembles of independent samples (different threshold seeds) of that loop, PCG solves, several streams from one host thread
+    for nrep in (2, 4, 6):
+        reps = []
+        for r in range(nrep):
+            stream = torch.cuda.Stream()
+            with torch.cuda.stream(stream):
+                h = binding.Fcg(L, torch.float64, stream=stream)
+                s = h.fcg_inverse_spectrum(h.fcg_kernel_spectrum(h.fcg_green_function(inputs.GREEN_NU, inputs.GREEN_E, inputs.GREEN_A)))
+                h.fcg_set_spectrum(s); h.fcg_set_preconditioner(s, 1.0)
+                reps.append((h, to(inputs.force_k(L)), torch.zeros((L, L), dtype=torch.float64, device="cuda"),
+                             to(inputs.gradient_thresholds(L, 1.0, seed=300 + r))))
+        torch.cuda.synchronize(); t0 = time.perf_counter()
+        for h, k, u, tt in reps:
+            h.fcg_force_fracture_displacement_begin(k, inputs.FORCE_D, u, tt, nsteps, 1e-12, 2000, True)
+        res = [h.fcg_force_fracture_displacement_end() for h, *_ in reps]
+        dt_s = time.perf_counter() - t0
+        out[f"force_fracture_via_displacement_pcg_ensemble{nrep}_L256_f64"] = {
+            "samples": nrep, "steps": sum(int(r[3]) for r in res), "wall_s": dt_s, "steps_per_s": sum(int(r[3]) for r in res) / dt_s,
+            "iterations": sum(int(r[1].sum()) for r in res)}
+        for h, *_ in reps:
+            h.close()
     return out
 
 

@@ -234,9 +234,17 @@ int fcg_fracture_end(fcg_handle h, long long* index_host, int* iters_host, int* 
  *                        use_pcg fcg_set_preconditioner with the same spectrum and a kbar (fixed for the whole loop).  Results
  *                        as fcg_force_fracture (ratio = winning f/t: the bond breaks at D_c = D / ratio); the break sequence is
  *                        that of fcg_force_fracture wherever the top-2 gap exceeds the solver error.  At L = 256 and 512 ONE
- *                        cooperative launch for the whole loop (fcg_fused.cuh, FORCE = 2).  Blocks. */
+ *                        cooperative launch for the whole loop (fcg_fused.cuh, FORCE = 2).  Blocks.
+ *   fcg_force_fracture_displacement_begin / _end   the same loop in two halves, as fcg_fracture_begin / _end: _begin enqueues (and
+ *                        returns at once where the loop is the cooperative kernel; elsewhere it runs the loop to its end), _end
+ *                        blocks and fills the host arrays.  For ensembles of samples: one handle per sample, each on its own
+ *                        stream, all in flight from one host thread.  k, u, t must stay valid and untouched in between. */
 int fcg_force_fracture_displacement(fcg_handle h, void* k, double D, void* u, const void* t, int nsteps, double tol, int maxit,
                                     int use_pcg, long long* index_host, int* iters_host, double* ratio_host, int* steps_done_host);
+int fcg_force_fracture_displacement_begin(fcg_handle h, void* k, double D, void* u, const void* t, int nsteps, double tol,
+                                          int maxit, int use_pcg);
+int fcg_force_fracture_displacement_end(fcg_handle h, long long* index_host, int* iters_host, double* ratio_host,
+                                        int* steps_done_host);
 int fcg_inverse_spectrum(fcg_handle h, const void* g, void* s);
 int fcg_force_rhs(fcg_handle h, const void* k, double D, void* b);
 int fcg_force_from_displacement(fcg_handle h, const void* k, double D, const void* u, void* f);

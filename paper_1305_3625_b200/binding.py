@@ -29,7 +29,7 @@ EXPORTS = ["fcg_workspace_bytes", "fcg_create", "fcg_destroy", "fcg_set_option",
            "fcg_fracture_begin", "fcg_fracture_end",
            "fcg_green_function", "fcg_kernel_spectrum", "fcg_force_apply", "fcg_force_solve", "fcg_force_break_step",
            "fcg_force_fracture", "fcg_inverse_spectrum", "fcg_force_rhs", "fcg_force_from_displacement",
-           "fcg_force_fracture_displacement"]
+           "fcg_force_fracture_displacement", "fcg_force_fracture_displacement_begin", "fcg_force_fracture_displacement_end"]
 
 _lib = None
 
@@ -73,6 +73,10 @@ def lib() -> C.CDLL:
         L.fcg_inverse_spectrum.argtypes = [vp, vp, vp]; L.fcg_inverse_spectrum.restype = i
         L.fcg_force_fracture_displacement.argtypes = [vp, vp, d, vp, vp, i, d, i, i, vp, vp, vp, C.POINTER(i)]
         L.fcg_force_fracture_displacement.restype = i
+        L.fcg_force_fracture_displacement_begin.argtypes = [vp, vp, d, vp, vp, i, d, i, i]
+        L.fcg_force_fracture_displacement_begin.restype = i
+        L.fcg_force_fracture_displacement_end.argtypes = [vp, vp, vp, vp, C.POINTER(i)]
+        L.fcg_force_fracture_displacement_end.restype = i
         L.fcg_force_rhs.argtypes = [vp, vp, d, vp]; L.fcg_force_rhs.restype = i
         L.fcg_force_from_displacement.argtypes = [vp, vp, d, vp, vp]; L.fcg_force_from_displacement.restype = i
         L.fcg_force_solve.argtypes = [vp, vp, d, vp, d, i, C.POINTER(i), C.POINTER(d)]; L.fcg_force_solve.restype = i
@@ -354,6 +358,28 @@ class Fcg:
                                                        int(nsteps), float(tol), int(maxit), 1 if use_pcg else 0,
                                                        index.ctypes.data_as(C.c_void_p), iters.ctypes.data_as(C.c_void_p),
                                                        ratio.ctypes.data_as(C.c_void_p), C.byref(done))
+        if st < 0 and st not in (FCG_BREAKDOWN, FCG_NO_CANDIDATE):
+            self._raise(st)
+        return index, iters, ratio, int(done.value), int(st)
+
+    def fcg_force_fracture_displacement_begin(self, k: torch.Tensor, D: float, u: torch.Tensor, t: torch.Tensor, nsteps: int, tol: float,
+                                              maxit: int, use_pcg: bool = False) -> None:
+        """Enqueue half; keep k, u, t alive and untouched until fcg_force_fracture_displacement_end()."""
+        self._pend = (k, u, t, int(nsteps))
+        st = self._lib.fcg_force_fracture_displacement_begin(self._h, self._chk(k, self.N), float(D), self._chk(u, self.N),
+                                                             self._chk(t, self.N), int(nsteps), float(tol), int(maxit), 1 if use_pcg else 0)
+        if st < 0 and st not in (FCG_BREAKDOWN, FCG_NO_CANDIDATE):
+            self._raise(st)
+
+    def fcg_force_fracture_displacement_end(self):
+        """Collect half. Returns (index[int64], iters[int32], ratio[float64], steps_done, status)."""
+        import numpy as np
+        nsteps = self._pend[3]
+        index = np.full(nsteps, -1, np.int64); iters = np.zeros(nsteps, np.int32); ratio = np.full(nsteps, np.nan, np.float64)
+        done = C.c_int(0)
+        st = self._lib.fcg_force_fracture_displacement_end(self._h, index.ctypes.data_as(C.c_void_p), iters.ctypes.data_as(C.c_void_p),
+                                                           ratio.ctypes.data_as(C.c_void_p), C.byref(done))
+        self._pend = None
         if st < 0 and st not in (FCG_BREAKDOWN, FCG_NO_CANDIDATE):
             self._raise(st)
         return index, iters, ratio, int(done.value), int(st)

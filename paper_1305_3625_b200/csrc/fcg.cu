@@ -96,7 +96,8 @@ struct fcg_handle_s {
     void *hk = nullptr, *hf = nullptr, *hu = nullptr;   // device staging of fcg_solve_host
     long long* frac_idx = nullptr; int* frac_it = nullptr; double* frac_ratio = nullptr; int frac_cap = 0;   // device results of the fused quasi-static loop
     int pend_nsteps = -1, pend_done = 0, pend_status = 0; bool pend_async = false;   // fcg_fracture_begin / _end
-    std::vector<long long> pend_idx; std::vector<int> pend_it;
+    std::vector<long long> pend_idx; std::vector<int> pend_it; std::vector<double> pend_ratio;
+    int pend_kind = 0;                  // 0: fcg_fracture_begin, 1: fcg_force_fracture_displacement_begin
     std::vector<GraphEntry> graphs; unsigned long long stamp = 0;
     long long launches = 0;
     std::string err;
@@ -829,7 +830,7 @@ static int frac_reserve(fcg_handle h, int nsteps) {
 static int fracture_begin(fcg_handle h, void* k, const void* f, void* u, const void* t, int nsteps, double tol, int maxit, bool pcg) {
     if (!h || !k || !f || !u || !t || nsteps < 0) return fail(h, FCG_INVALID_ARG, "bad argument");
     if (pcg && !h->have_precond) return fail(h, FCG_NO_SPECTRUM, "fcg_set_preconditioner has not been called");
-    h->pend_nsteps = -1; h->pend_async = false; h->pend_done = 0; h->pend_status = FCG_OK;
+    h->pend_nsteps = -1; h->pend_async = false; h->pend_done = 0; h->pend_status = FCG_OK; h->pend_kind = 0;
     if (h->fused() && h->have_spectrum && nsteps > 0 && tol >= 0.0 && maxit >= 0) {
         // small lattices: the whole quasi-static loop -- every solve and every break step -- is one cooperative kernel
         { const int e0 = frac_reserve(h, nsteps); if (e0 != FCG_OK) return e0; }
@@ -869,7 +870,7 @@ static int fracture_begin(fcg_handle h, void* k, const void* f, void* u, const v
 
 static int fracture_end(fcg_handle h, long long* index_host, int* iters_host, int* steps_done_host) {
     if (!h || !index_host || !iters_host) return fail(h, FCG_INVALID_ARG, "bad argument");
-    if (h->pend_nsteps < 0) return fail(h, FCG_INVALID_ARG, "no quasi-static loop pending on this handle");
+    if (h->pend_nsteps < 0 || h->pend_kind != 0) return fail(h, FCG_INVALID_ARG, "no quasi-static loop of this kind pending on this handle");
     h->pend_nsteps = -1;
     if (h->pend_async) {
         FCG_CK(h, cudaStreamSynchronize(h->stream));
@@ -1028,14 +1029,14 @@ int fcg_force_fracture(fcg_handle h, void* k, double D, void* f, const void* t, 
     return st < 0 ? st : FCG_OK;
 }
 
-// quasi-static loop of the force model through the displacements (reading F7)
-int fcg_force_fracture_displacement(fcg_handle h, void* k, double D, void* u, const void* t, int nsteps, double tol, int maxit, int use_pcg,
-                                    long long* index_host, int* iters_host, double* ratio_host, int* steps_done_host) {
-    if (!h || !k || !u || !t || nsteps < 0 || !index_host || !iters_host) return fail(h, FCG_INVALID_ARG, "bad argument");
+// quasi-static loop of the force model through the displacements (reading F7), in two halves like
+// fcg_fracture_begin / _end so that one host thread can keep an ensemble of samples (handles on their own streams) in flight
+int fcg_force_fracture_displacement_begin(fcg_handle h, void* k, double D, void* u, const void* t, int nsteps, double tol, int maxit, int use_pcg) {
+    if (!h || !k || !u || !t || nsteps < 0) return fail(h, FCG_INVALID_ARG, "bad argument");
     if (!(tol >= 0.0) || maxit < 0 || !std::isfinite(D)) return fail(h, FCG_INVALID_ARG, "tol must be >= 0, maxit >= 0, D finite");
     if (!h->have_spectrum) return fail(h, FCG_NO_SPECTRUM, "fcg_set_spectrum has not been called");
     if (use_pcg && !h->have_precond) return fail(h, FCG_NO_SPECTRUM, "fcg_set_preconditioner has not been called");
-    if (steps_done_host) *steps_done_host = 0;
+    h->pend_nsteps = -1; h->pend_async = false; h->pend_done = 0; h->pend_status = FCG_OK; h->pend_kind = 1;
     if (h->fused() && nsteps > 0) {
         // small lattices: the whole loop in one cooperative kernel (fcg_fused.cuh, FORCE = 2)
         { const int e0 = frac_reserve(h, nsteps); if (e0 != FCG_OK) return e0; }
@@ -1049,27 +1050,18 @@ int fcg_force_fracture_displacement(fcg_handle h, void* k, double D, void* u, co
         cudaError_t e = h->tab->fused_solve(&A, h->stream);
         if (e == cudaSuccess) {
             FCG_CK(h, cudaMemcpyAsync(h->h_sc, h->sc(), sizeof(Scalars), cudaMemcpyDeviceToHost, h->stream));
-            FCG_CK(h, cudaStreamSynchronize(h->stream));
-            h->launches = 1;
-            const int done = h->h_sc->steps_done;
-            if (done > 0) {
-                FCG_CK(h, cudaMemcpyAsync(index_host, h->frac_idx, (size_t)done * sizeof(long long), cudaMemcpyDeviceToHost, h->stream));
-                FCG_CK(h, cudaMemcpyAsync(iters_host, h->frac_it, (size_t)done * sizeof(int), cudaMemcpyDeviceToHost, h->stream));
-                if (ratio_host) FCG_CK(h, cudaMemcpyAsync(ratio_host, h->frac_ratio, (size_t)done * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
-                FCG_CK(h, cudaStreamSynchronize(h->stream));
-            }
-            if (steps_done_host) *steps_done_host = done;
-            if (h->h_sc->status == FCG_CUDA_ERROR) h->err = "fused quasi-static loop: grid barrier timed out";
-            return h->h_sc->status < 0 ? h->h_sc->status : FCG_OK;
+            h->pend_nsteps = nsteps; h->pend_async = true; h->launches = 1;
+            return FCG_OK;
         }
         cudaGetLastError();
         h->err = std::string("cooperative launch failed (") + cudaGetErrorString(e) + "); using the graph path";
         h->fused_opt = 0;
     }
-    // larger lattices: the library's own calls in turn, with two scratch vectors (b = K D and the forces)
+    // larger lattices: the library's own calls in turn, with two scratch vectors (b = K D and the forces); runs to its end here
     const size_t bytes = h->N * h->w;
     if (!h->hk) { FCG_CK(h, cudaMalloc(&h->hk, bytes)); FCG_CK(h, cudaMalloc(&h->hf, bytes)); FCG_CK(h, cudaMalloc(&h->hu, bytes)); }
     void* b = h->hf; void* frc = h->hk;
+    h->pend_idx.assign((size_t)nsteps, -1); h->pend_it.assign((size_t)nsteps, 0); h->pend_ratio.assign((size_t)nsteps, 0.0);
     long long total = 0; int done = 0, st = FCG_OK;
     for (int step = 0; step < nsteps; ++step) {
         int it = 0; double rr = 0.0;
@@ -1082,12 +1074,45 @@ int fcg_force_fracture_displacement(fcg_handle h, void* k, double D, void* u, co
         st = fcg_force_break_step(h, k, frc, t, &idx, &ratio);
         total += h->launches;
         if (st < 0) break;
-        index_host[step] = idx; iters_host[step] = it; if (ratio_host) ratio_host[step] = ratio;
+        h->pend_idx[step] = idx; h->pend_it[step] = it; h->pend_ratio[step] = ratio;
         ++done; st = FCG_OK;
     }
-    if (steps_done_host) *steps_done_host = done;
-    h->launches = total;
+    h->pend_nsteps = nsteps; h->pend_done = done; h->pend_status = st; h->launches = total;
     return st < 0 ? st : FCG_OK;
+}
+
+int fcg_force_fracture_displacement_end(fcg_handle h, long long* index_host, int* iters_host, double* ratio_host, int* steps_done_host) {
+    if (!h || !index_host || !iters_host) return fail(h, FCG_INVALID_ARG, "bad argument");
+    if (h->pend_nsteps < 0 || h->pend_kind != 1) return fail(h, FCG_INVALID_ARG, "no quasi-static loop of this kind pending on this handle");
+    h->pend_nsteps = -1; h->pend_kind = 0;
+    if (h->pend_async) {
+        FCG_CK(h, cudaStreamSynchronize(h->stream));
+        const int done = h->h_sc->steps_done;
+        if (done > 0) {
+            FCG_CK(h, cudaMemcpyAsync(index_host, h->frac_idx, (size_t)done * sizeof(long long), cudaMemcpyDeviceToHost, h->stream));
+            FCG_CK(h, cudaMemcpyAsync(iters_host, h->frac_it, (size_t)done * sizeof(int), cudaMemcpyDeviceToHost, h->stream));
+            if (ratio_host) FCG_CK(h, cudaMemcpyAsync(ratio_host, h->frac_ratio, (size_t)done * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+            FCG_CK(h, cudaStreamSynchronize(h->stream));
+        }
+        if (steps_done_host) *steps_done_host = done;
+        if (h->h_sc->status == FCG_CUDA_ERROR) h->err = "fused quasi-static loop: grid barrier timed out";
+        return h->h_sc->status < 0 ? h->h_sc->status : FCG_OK;
+    }
+    for (int i = 0; i < h->pend_done; ++i) {
+        index_host[i] = h->pend_idx[(size_t)i]; iters_host[i] = h->pend_it[(size_t)i];
+        if (ratio_host) ratio_host[i] = h->pend_ratio[(size_t)i];
+    }
+    if (steps_done_host) *steps_done_host = h->pend_done;
+    return h->pend_status;
+}
+
+int fcg_force_fracture_displacement(fcg_handle h, void* k, double D, void* u, const void* t, int nsteps, double tol, int maxit, int use_pcg,
+                                    long long* index_host, int* iters_host, double* ratio_host, int* steps_done_host) {
+    if (!index_host || !iters_host) return fail(h, FCG_INVALID_ARG, "bad argument");
+    if (steps_done_host) *steps_done_host = 0;
+    const int st = fcg_force_fracture_displacement_begin(h, k, D, u, t, nsteps, tol, maxit, use_pcg);
+    if (st < 0 && (!h || h->pend_nsteps < 0)) return st;
+    return fcg_force_fracture_displacement_end(h, index_host, iters_host, ratio_host, steps_done_host);
 }
 
 int fcg_profile_iteration(fcg_handle h, const void* k, const void* f, void* u, int iters, double* ms_host) {

@@ -489,3 +489,48 @@ def test_force_through_displacements_full_size_sampled(B):
     assert st2 == 0 and it2 > 3 * it
     assert rel(fs[0], f2.cpu().numpy()) <= 1e-9 and rel(fs[1], f2.cpu().numpy()) <= 1e-9
     h.close(); h2.close()
+
+
+@pytest.mark.parametrize("L,use_pcg", [(256, True), (256, False), (64, True)])
+def test_force_fracture_displacement_ensemble_begin_end(B, L, use_pcg):
+    """Independent samples (different threshold seeds) on three handles / streams driven by one host thread with
+    fcg_force_fracture_displacement_begin / _end: every sample equals its blocking run bitwise, sample 0 equals the oracle's loop."""
+    dt, steps, nrep = np.float64, 40, 3
+    _, g = green_spectrum_oracle(L, dt); sinv = orc.inverse_spectrum(g)
+    ts = [inputs.gradient_thresholds(L, 1.0, seed=inputs.SEED_T if r == 0 else 200 + r) for r in range(nrep)]
+    reps = []
+    for r in range(nrep):
+        st = torch.cuda.Stream()
+        with torch.cuda.stream(st):
+            h = B.Fcg(L, torch.float64, stream=st)
+            s = dev(sinv); h.fcg_set_spectrum(s); h.fcg_set_preconditioner(s, 1.0)
+            reps.append((h, dev(inputs.force_k(L)), dev(np.zeros((L, L))), dev(ts[r]), st))
+    torch.cuda.synchronize()
+    for h, k, u, t, st in reps:
+        h.fcg_force_fracture_displacement_begin(k, 1.0, u, t, steps, 1e-12, 2000, use_pcg)
+    outs = [h.fcg_force_fracture_displacement_end() for h, *_ in reps]
+    for r, (h, k, u, t, st) in enumerate(reps):
+        index, iters, ratio, done, status = outs[r]
+        assert status == 0 and done == steps
+        k2, u2 = dev(inputs.force_k(L)), dev(np.zeros((L, L)))
+        torch.cuda.synchronize()
+        with torch.cuda.stream(st):
+            i2, it2, r2, d2, s2 = h.fcg_force_fracture_displacement(k2, 1.0, u2, dev(ts[r]), steps, 1e-12, 2000, use_pcg=use_pcg)
+        assert np.array_equal(index, i2) and np.array_equal(iters, it2) and np.array_equal(ratio, r2)
+        assert torch.equal(k, k2) and torch.equal(u, u2)
+    ko = inputs.force_k(L); uo = np.zeros((L, L))
+    ref = orc.force_fracture_displacement(sinv, ko, 1.0, uo, ts[0], steps, 1e-12, 2000, kbar=1.0 if use_pcg else None)
+    assert np.array_equal(outs[0][0], ref["index"]) and np.abs(outs[0][1].astype(int) - ref["iters"].astype(int)).max() <= 3
+    with pytest.raises(B.FcgError):                          # nothing pending any more
+        reps[0][0]._pend = (None, None, None, 1); reps[0][0].fcg_force_fracture_displacement_end()
+    # a loop of the other kind pending: the wrong _end is refused, the right one still works
+    h, k, u, t, st = reps[0]
+    w3 = inputs.config(3, L=L, nsteps=4)
+    k3, u3 = dev(w3.k), dev(w3.u0)
+    with torch.cuda.stream(st):
+        h.fcg_fracture_begin(k3, dev(w3.f), u3, dev(w3.t), 4, 1e-8, 500, False)
+        with pytest.raises(B.FcgError):
+            h._pend = (None, None, None, 4); h.fcg_force_fracture_displacement_end()
+        assert h.fcg_fracture_end()[2] == 4
+    for h, *_ in reps:
+        h.close()
