@@ -75,7 +75,7 @@ __device__ __forceinline__ bool grid_barrier(unsigned int* counter, unsigned int
     return *ok_smem != 0;
 }
 
-// FORCE: the paper's own system in the bond forces, in the textbook order of Listing 2 (q = (I + K G) p is formed and kept, p.q is a
+// FORCE = 1: the paper's own system in the bond forces, in the textbook order of Listing 2 (q = (I + K G) p is formed and kept, p.q is a
 // dot product, then u and r are updated: one more grid barrier per iteration than the spectral search length of the displacement
 // form, which would need k o p = kappa p, i.e. reading F1, to hold exactly) -- the same arithmetic as the oracle for any k.
 // FORCE = 2: the force model through the displacements (reading F7): the arithmetic of FORCE = 0 (spectral
