@@ -404,7 +404,9 @@ def main():
     ap.add_argument("--dtype", choices=["f64", "f32"], default="f64")
     ap.add_argument("--config", type=int, default=2, choices=[0, 1, 2, 4])
     ap.add_argument("--impl", choices=["fcg", "reference"], default="fcg")
-    ap.add_argument("--ref-iters", type=int, default=8, help="oracle CG iterations per reference step / cpu_baseline sample")
+    ap.add_argument("--ref-iters", type=int, default=8, help="oracle CG iterations per step of --impl reference")
+    ap.add_argument("--cpu-baseline-iters", type=int, default=None,
+                    help="oracle CG iterations of the cpu_baseline sample (default: sized for ~12 s of host work from a 2-iteration probe)")
     ap.add_argument("--full", action="store_true", help="also time configs[2] fp32 and configs[4] (reported under 'extra')")
     ap.add_argument("--solver", choices=["cg", "pcg", "force"], default="cg",
                     help="pcg: time fcg_pcg_solve instead (metric pcg_iterations_per_s, 22 N w bytes per iteration; no e2e leg) -- "
@@ -574,9 +576,13 @@ def main():
         extra.update(bench_extras(binding, torch, inputs))
         line["extra"] = extra
     if not args.no_cpu_baseline and world == 1:
-        v, dt, cores = oracle_sample(w, args.ref_iters)
+        n_cpu = args.cpu_baseline_iters
+        if n_cpu is None:                                  # bounded sample: about 12 s of host work, at least 8 iterations
+            v0, _, _ = oracle_sample(w, 2)
+            n_cpu = int(min(max(8, round(12.0 * v0)), 4000))
+        v, dt, cores = oracle_sample(w, n_cpu)
         line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
-                                "sample": f"{args.ref_iters} CG iterations (tol=0) of the same workload, {dt:.1f} s"}
+                                "sample": f"{n_cpu} CG iterations (tol=0) of the same workload from u0, {dt:.1f} s"}
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
