@@ -46,7 +46,8 @@ template <typename T, typename P> struct FusedShape {
     static constexpr int TPC = (L / 2) / G;                      // row pairs (and columns) per CTA
     static constexpr size_t WBYTES = (size_t)L * 2 * sizeof(T);
     static constexpr size_t VBYTES = (size_t)2 * L * sizeof(T);  // one vector's two rows
-    static constexpr size_t smem = WBYTES + (size_t)TPC * 7 * VBYTES + 128;     // k f u r p q t
+    static constexpr size_t SPECB = (size_t)TPC * 2 * L * sizeof(T);             // one spectrum's rows for the CTA's columns (column 0: two rows)
+    static constexpr size_t smem = WBYTES + (size_t)TPC * 7 * VBYTES + 2 * SPECB + 128;     // k f u r p q t, shat rows, mhat rows
 };
 
 #ifdef __CUDACC__
@@ -96,6 +97,11 @@ __global__ void __launch_bounds__(P::NT) cg_fused_kernel(const FusedArgs A)
     __shared__ int ok_smem;
     cx<T>* W = reinterpret_cast<cx<T>*>(smem_raw);
     T* const vecs = reinterpret_cast<T*>(smem_raw + FS::WBYTES);
+    // the rows of the stored spectrum (and of the preconditioner's) that belong to the CTA's own columns: the same values every
+    // iteration, so they are copied to shared memory once -- the column phase no longer waits on L2 for them, and CTA 0, whose packed
+    // n = 0 / L/2 column reads two rows in a loop and is the straggler at every "columns done" barrier, least of all
+    T* const sspec = reinterpret_cast<T*>(smem_raw + FS::WBYTES + (size_t)TPC * 7 * FS::VBYTES);
+    T* const smspec = sspec + (size_t)TPC * 2 * L;
     // vector v (0 k, 1 f, 2 u, 3 r, 4 p, 5 q, 6 t) of own tile j, row r (0/1)
     auto V = [&](int j, int v, int r) { return vecs + ((size_t)(j * 7 + v) * 2 + r) * L; };
     SmemIO<T, P> io{W};
@@ -122,14 +128,25 @@ __global__ void __launch_bounds__(P::NT) cg_fused_kernel(const FusedArgs A)
         __syncthreads();
         return r;
     };
+    // this thread's share of G doubles, all loads in flight before the first add (same order of additions as a plain loop; the loop
+    // form serialised G / NT L2 round trips per sum -- 10 % of the kernel's stall samples at L = 512, profiles/r1_ncu_fused_L512_f64.txt)
+    auto sum_partials = [&](const double* ps) {
+        constexpr int NP = (G + NT - 1) / NT;
+        double t[NP];
+#pragma unroll
+        for (int c = 0; c < NP; ++c) t[c] = lt + c * NT < G ? __ldcg(ps + lt + c * NT) : 0.0;
+        double v = 0.0;
+#pragma unroll
+        for (int c = 0; c < NP; ++c) v += t[c];
+        return v;
+    };
     // grid-wide sum: publish the CTA's partial, barrier, every CTA adds all G partials in the same order
     auto grid_sum = [&](double part, bool& ok) {
         const double mine = cta_sum(part);
         double* ps = A.partial + (size_t)slot * G;
         if (lt == 0) ps[cta] = mine;
         ok = grid_barrier(A.counter, target, G, &ok_smem);
-        double v = 0.0;
-        for (int i = lt; i < G; i += NT) v += __ldcg(ps + i);
+        const double v = sum_partials(ps);
         slot = (slot + 1) & 3;
         return cta_sum(v);
     };
@@ -193,7 +210,7 @@ __global__ void __launch_bounds__(P::NT) cg_fused_kernel(const FusedArgs A)
         }
     };
     // phase C: own columns, in place: forward, spectral multiply, inverse
-    auto columns = [&](const T* spec, double* en) {      // en != nullptr: *en += this CTA's share of sum spec |P|^2
+    auto columns = [&](const T* spec, double* en) {      // spec: sspec or smspec (shared-memory copies); en != nullptr: *en += this CTA's share of sum spec |P|^2
         for (int j = 0; j < TPC; ++j) {
             const int m = cta + j * G;
             cx<T>* col = Tf + (size_t)m * L;
@@ -224,7 +241,7 @@ __global__ void __launch_bounds__(P::NT) cg_fused_kernel(const FusedArgs A)
                 __syncthreads();
             };
             if (m != 0) {
-                const T* sh = spec + (size_t)m * L;
+                const T* sh = spec + (size_t)j * 2 * L;
                 static_for_up<2, S - 1>(fwd_stage);
                 if (en) {
                     double e2 = 0.0;
@@ -237,8 +254,8 @@ __global__ void __launch_bounds__(P::NT) cg_fused_kernel(const FusedArgs A)
                 static_for_down<S - 1, 2>(inv_stage);
             } else {     // packed n = 0 / L/2 column (see col2_kernel)
                 static_for_up<2, S>(fwd_stage);
-                const T* sp_ = spec;
-                const T* sm_ = spec + (size_t)(L / 2) * L;
+                const T* sp_ = spec + (size_t)j * 2 * L;
+                const T* sm_ = sp_ + L;
                 for (int mm = lt; mm <= L / 2; mm += NT) {
                     const int e = P::pos_of(mm), e2 = P::pos_of((L - mm) % L);
                     const cx<T> Wa = io.ld(e), Wb = io.ld(e2);
@@ -275,11 +292,22 @@ __global__ void __launch_bounds__(P::NT) cg_fused_kernel(const FusedArgs A)
     auto rows_inverse = [&](auto emit) {
         for (int j = 0; j < TPC; ++j) {
             const int A2 = cta + j * G;
-            for (int m = lt; m < L / 2; m += NT) {
+            // all of this thread's loads of T in flight before the first use (the plain loop, with its branch, serialised
+            // L / (2 NT) L2 round trips per phase: the largest single stall site at L = 512, profiles/r1_ncu_fused_L512_f64.txt)
+            constexpr int NM = (L / 2 + NT - 1) / NT;
+            cx<T> xa[NM], xb[NM];
+#pragma unroll
+            for (int c = 0; c < NM; ++c) {
+                const int m = lt + c * NT;
+                if (m < L / 2) { const cx<T>* src = Tf + (size_t)m * L + 2 * A2; xa[c] = __ldcg(src); xb[c] = __ldcg(src + 1); }
+            }
+#pragma unroll
+            for (int c = 0; c < NM; ++c) {
+                const int m = lt + c * NT;
+                if (m >= L / 2) break;
                 const int e = AS::pos_of_col(m);
                 const int n = P::freq_of(e);
-                const cx<T>* src = Tf + (size_t)m * L + 2 * A2;
-                const cx<T> X0 = __ldcg(src), X1 = __ldcg(src + 1);
+                const cx<T> X0 = xa[c], X1 = xb[c];
                 if (n == 0) {
                     io.st(P::pos_of(0), mk<T>(X0.x, X1.x));
                     io.st(P::pos_of(L / 2), mk<T>(X0.y, X1.y));
@@ -332,6 +360,18 @@ __global__ void __launch_bounds__(P::NT) cg_fused_kernel(const FusedArgs A)
     bool zero_u = false;
     const T* mhat = static_cast<const T*>(A.mhat);
     const bool pcg = mhat != nullptr;
+    for (int j = 0; j < TPC; ++j) {
+        const int m = cta + j * G;
+        for (int e = lt; e < L; e += NT) {
+            sspec[(size_t)j * 2 * L + e] = shat[(size_t)m * L + e];
+            if (m == 0) sspec[(size_t)j * 2 * L + L + e] = shat[(size_t)(L / 2) * L + e];
+            if (pcg) {
+                smspec[(size_t)j * 2 * L + e] = mhat[(size_t)m * L + e];
+                if (m == 0) smspec[(size_t)j * 2 * L + L + e] = mhat[(size_t)(L / 2) * L + e];
+            }
+        }
+    }
+    __syncthreads();
 
     for (int step = 0; step < (frac ? A.nsteps : 1); ++step) {
         // ---- set up initial values: first direction from p = 0, beta = 0
@@ -387,7 +427,7 @@ __global__ void __launch_bounds__(P::NT) cg_fused_kernel(const FusedArgs A)
                 rows_forward(phase == PH_RESID ? 2 : (phase == PH_Q ? 4 : 3));
                 ok = grid_barrier(A.counter, target, G, &ok_smem) && ok;
                 double en = 0.0;
-                columns(phase == PH_Z ? mhat : shat, (!FQ && phase == PH_Q) ? &en : nullptr);
+                columns(phase == PH_Z ? smspec : sspec, (!FQ && phase == PH_Q) ? &en : nullptr);
                 double* ps = A.partial + (size_t)slot * G;
                 if (!FQ && phase == PH_Q) {                    // this CTA's share of p.Ap = sum k p^2 + sum shat |P|^2, published before the barrier
                     const double mine = cta_sum(kpp + en);
@@ -396,8 +436,7 @@ __global__ void __launch_bounds__(P::NT) cg_fused_kernel(const FusedArgs A)
                 ok = grid_barrier(A.counter, target, G, &ok_smem) && ok;
                 T al = (T)0;
                 if (!FQ && phase == PH_Q) {          // search length (94): every CTA adds the G shares in the same order
-                    double v = 0.0;
-                    for (int i = lt; i < G; i += NT) v += __ldcg(ps + i);
+                    const double v = sum_partials(ps);
                     slot = (slot + 1) & 3;
                     const double pq = cta_sum(v);
                     if (!(pq > 0.0) || !isfinite(pq)) bd = true;
