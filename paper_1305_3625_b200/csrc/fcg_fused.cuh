@@ -60,6 +60,12 @@ __device__ __forceinline__ unsigned int ld_acquire_u32(const unsigned int* p) {
     return v;
 }
 
+__device__ __forceinline__ unsigned int ld_relaxed_u32(const unsigned int* p) {
+    unsigned int v;
+    asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+
 // all CTAs of the (co-resident) grid; returns false if the spin cap was hit
 __device__ __forceinline__ bool grid_barrier(unsigned int* counter, unsigned int& target, unsigned int G, int* ok_smem) {
     __syncthreads();
@@ -69,7 +75,10 @@ __device__ __forceinline__ bool grid_barrier(unsigned int* counter, unsigned int
         target += G;
         asm volatile("red.release.gpu.global.add.u32 [%0], %1;" ::"l"(counter), "r"(1u) : "memory");
         unsigned int spins = 0;
-        while (ld_acquire_u32(counter) < target && ++spins < SPIN_CAP) {}
+        // poll relaxed (no L1 invalidate per poll), with a short back-off so that G pollers do not crowd the arrivals out of
+        // the counter's L2 slice; one acquire load once the count is there orders the other CTAs' writes before what follows
+        while (ld_relaxed_u32(counter) < target && ++spins < SPIN_CAP) { __nanosleep(32); }
+        (void)ld_acquire_u32(counter);
         *ok_smem = spins < SPIN_CAP;
     }
     __syncthreads();
