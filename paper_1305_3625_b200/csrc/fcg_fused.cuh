@@ -46,8 +46,7 @@ template <typename T, typename P> struct FusedShape {
     static constexpr int TPC = (L / 2) / G;                      // row pairs (and columns) per CTA
     static constexpr size_t WBYTES = (size_t)L * 2 * sizeof(T);
     static constexpr size_t VBYTES = (size_t)2 * L * sizeof(T);  // one vector's two rows
-    static constexpr size_t SPECB = (size_t)TPC * 2 * L * sizeof(T);             // one spectrum's rows for the CTA's columns (column 0: two rows)
-    static constexpr size_t smem = WBYTES + (size_t)TPC * 7 * VBYTES + 2 * SPECB + 128;     // k f u r p q t, shat rows, mhat rows
+    static constexpr size_t smem = WBYTES + (size_t)TPC * 7 * VBYTES + 128;     // k f u r p q t
 };
 
 #ifdef __CUDACC__
@@ -106,11 +105,6 @@ __global__ void __launch_bounds__(P::NT) cg_fused_kernel(const FusedArgs A)
     __shared__ int ok_smem;
     cx<T>* W = reinterpret_cast<cx<T>*>(smem_raw);
     T* const vecs = reinterpret_cast<T*>(smem_raw + FS::WBYTES);
-    // the rows of the stored spectrum (and of the preconditioner's) that belong to the CTA's own columns: the same values every
-    // iteration, so they are copied to shared memory once -- the column phase no longer waits on L2 for them, and CTA 0, whose packed
-    // n = 0 / L/2 column reads two rows in a loop and is the straggler at every "columns done" barrier, least of all
-    T* const sspec = reinterpret_cast<T*>(smem_raw + FS::WBYTES + (size_t)TPC * 7 * FS::VBYTES);
-    T* const smspec = sspec + (size_t)TPC * 2 * L;
     // vector v (0 k, 1 f, 2 u, 3 r, 4 p, 5 q, 6 t) of own tile j, row r (0/1)
     auto V = [&](int j, int v, int r) { return vecs + ((size_t)(j * 7 + v) * 2 + r) * L; };
     SmemIO<T, P> io{W};
@@ -219,7 +213,7 @@ __global__ void __launch_bounds__(P::NT) cg_fused_kernel(const FusedArgs A)
         }
     };
     // phase C: own columns, in place: forward, spectral multiply, inverse
-    auto columns = [&](const T* spec, double* en) {      // spec: sspec or smspec (shared-memory copies); en != nullptr: *en += this CTA's share of sum spec |P|^2
+    auto columns = [&](const T* spec, double* en) {      // en != nullptr: *en += this CTA's share of sum spec |P|^2
         for (int j = 0; j < TPC; ++j) {
             const int m = cta + j * G;
             cx<T>* col = Tf + (size_t)m * L;
@@ -250,7 +244,7 @@ __global__ void __launch_bounds__(P::NT) cg_fused_kernel(const FusedArgs A)
                 __syncthreads();
             };
             if (m != 0) {
-                const T* sh = spec + (size_t)j * 2 * L;
+                const T* sh = spec + (size_t)m * L;
                 static_for_up<2, S - 1>(fwd_stage);
                 if (en) {
                     double e2 = 0.0;
@@ -263,8 +257,8 @@ __global__ void __launch_bounds__(P::NT) cg_fused_kernel(const FusedArgs A)
                 static_for_down<S - 1, 2>(inv_stage);
             } else {     // packed n = 0 / L/2 column (see col2_kernel)
                 static_for_up<2, S>(fwd_stage);
-                const T* sp_ = spec + (size_t)j * 2 * L;
-                const T* sm_ = sp_ + L;
+                const T* sp_ = spec;
+                const T* sm_ = spec + (size_t)(L / 2) * L;
                 for (int mm = lt; mm <= L / 2; mm += NT) {
                     const int e = P::pos_of(mm), e2 = P::pos_of((L - mm) % L);
                     const cx<T> Wa = io.ld(e), Wb = io.ld(e2);
@@ -369,18 +363,6 @@ __global__ void __launch_bounds__(P::NT) cg_fused_kernel(const FusedArgs A)
     bool zero_u = false;
     const T* mhat = static_cast<const T*>(A.mhat);
     const bool pcg = mhat != nullptr;
-    for (int j = 0; j < TPC; ++j) {
-        const int m = cta + j * G;
-        for (int e = lt; e < L; e += NT) {
-            sspec[(size_t)j * 2 * L + e] = shat[(size_t)m * L + e];
-            if (m == 0) sspec[(size_t)j * 2 * L + L + e] = shat[(size_t)(L / 2) * L + e];
-            if (pcg) {
-                smspec[(size_t)j * 2 * L + e] = mhat[(size_t)m * L + e];
-                if (m == 0) smspec[(size_t)j * 2 * L + L + e] = mhat[(size_t)(L / 2) * L + e];
-            }
-        }
-    }
-    __syncthreads();
 
     for (int step = 0; step < (frac ? A.nsteps : 1); ++step) {
         // ---- set up initial values: first direction from p = 0, beta = 0
@@ -436,7 +418,7 @@ __global__ void __launch_bounds__(P::NT) cg_fused_kernel(const FusedArgs A)
                 rows_forward(phase == PH_RESID ? 2 : (phase == PH_Q ? 4 : 3));
                 ok = grid_barrier(A.counter, target, G, &ok_smem) && ok;
                 double en = 0.0;
-                columns(phase == PH_Z ? smspec : sspec, (!FQ && phase == PH_Q) ? &en : nullptr);
+                columns(phase == PH_Z ? mhat : shat, (!FQ && phase == PH_Q) ? &en : nullptr);
                 double* ps = A.partial + (size_t)slot * G;
                 if (!FQ && phase == PH_Q) {                    // this CTA's share of p.Ap = sum k p^2 + sum shat |P|^2, published before the barrier
                     const double mine = cta_sum(kpp + en);
