@@ -432,7 +432,7 @@ int solve_impl(fcg_handle h, const void* k, const void* f, void* u, double tol, 
 
 template <typename T>
 int break_impl(fcg_handle h, void* k, const void* u, const void* t, long long* index, double* ratio, void* fzero = nullptr) {
-    break_argmax_kernel<T><<<h->vec_blocks(), 256, 0, h->stream>>>(
+    break_argmax_kernel<T><<<h->update_blocks(), 256, 0, h->stream>>>(      // whole unrolled trips of 4 vectors per thread
         (T*)k, (const T*)u, (const T*)t, (long long)h->N, h->at<double>(h->lay.brk_r), h->at<long long>(h->lay.brk_i),
         h->at<unsigned int>(h->lay.brk_ticket), h->at<BreakResult>(h->lay.brk_out), (T*)fzero);
     ++h->launches;
