@@ -79,6 +79,9 @@ typedef enum {
     FCG_OPT_COL_PERSISTENT = 9, /* 1: column pass as persistent CTAs with two column buffers each, the next column's gather in flight
                                  while the current one is transformed (sizes where two buffers fit twice per SM); 0: one CTA per column;
                                  -1 (default): persistent for FCG_F32 and for L <= 1024, where it measured faster */
+    FCG_OPT_BARRIER_START = 10, /* testing aid: initial value (taken as unsigned 32-bit) of the arrival counter of the cooperative
+                                 kernel's grid barrier; default 0.  A value just below 2^32 makes the counter wrap within a few
+                                 iterations (the barrier compares modulo 2^32; tests/test_gpu_robustness.py) */
     FCG_OPT_ENGINE       = 3  /* 0 (default): pipelined TMA passes where the lattice is large enough (L >= 256), classic
                                  passes otherwise; 1: classic passes only (synchronous loads; kept for A/B measurements).
                                  The stored spectrum's layout belongs to the engine: changing the engine after

@@ -21,6 +21,7 @@ FCG_OPT_LOOP_MODE, FCG_OPT_CHUNK, FCG_OPT_ROW_VARIANT, FCG_OPT_ENGINE, FCG_OPT_U
 FCG_OPT_L2_HINTS = 7
 FCG_OPT_SPECTRAL_ALPHA = 8
 FCG_OPT_COL_PERSISTENT = 9
+FCG_OPT_BARRIER_START = 10
 
 EXPORTS = ["fcg_workspace_bytes", "fcg_create", "fcg_destroy", "fcg_set_option", "fcg_set_spectrum", "fcg_apply",
            "fcg_solve", "fcg_solve_host", "fcg_profile_iteration", "fcg_fft_fwd", "fcg_fft_inv", "fcg_break_step", "fcg_fracture",
@@ -224,15 +225,17 @@ class Fcg:
 
     def fcg_fracture_begin(self, k, f, u, t, nsteps: int, tol: float, maxit: int, use_pcg: bool = False):
         """Enqueue a quasi-static loop (returns at once where the loop is one cooperative kernel); finish with fcg_fracture_end."""
-        self._pending = (k, f, u, t, int(nsteps))              # keep the tensors alive
         st = self._lib.fcg_fracture_begin(self._h, self._chk(k, self.N), self._chk(f, self.N), self._chk(u, self.N),
                                           self._chk(t, self.N), int(nsteps), float(tol), int(maxit), 1 if use_pcg else 0)
         if st < 0 and st not in (FCG_BREAKDOWN, FCG_NO_CANDIDATE):
             self._raise(st)
+        self._pending = (k, f, u, t, int(nsteps))              # keep the tensors alive
 
     def fcg_fracture_end(self):
         """Returns (index, iters, steps_done, status) of the loop started by fcg_fracture_begin."""
         import numpy as np
+        if getattr(self, "_pending", None) is None:
+            raise FcgError(FCG_INVALID_ARG, "no quasi-static loop pending on this handle")
         nsteps = self._pending[4]
         index = np.full(nsteps, -1, np.int64); iters = np.zeros(nsteps, np.int32); done = C.c_int(0)
         st = self._lib.fcg_fracture_end(self._h, index.ctypes.data_as(C.c_void_p), iters.ctypes.data_as(C.c_void_p), C.byref(done))
@@ -365,15 +368,17 @@ class Fcg:
     def fcg_force_fracture_displacement_begin(self, k: torch.Tensor, D: float, u: torch.Tensor, t: torch.Tensor, nsteps: int, tol: float,
                                               maxit: int, use_pcg: bool = False) -> None:
         """Enqueue half; keep k, u, t alive and untouched until fcg_force_fracture_displacement_end()."""
-        self._pend = (k, u, t, int(nsteps))
         st = self._lib.fcg_force_fracture_displacement_begin(self._h, self._chk(k, self.N), float(D), self._chk(u, self.N),
                                                              self._chk(t, self.N), int(nsteps), float(tol), int(maxit), 1 if use_pcg else 0)
         if st < 0 and st not in (FCG_BREAKDOWN, FCG_NO_CANDIDATE):
             self._raise(st)
+        self._pend = (k, u, t, int(nsteps))
 
     def fcg_force_fracture_displacement_end(self):
         """Collect half. Returns (index[int64], iters[int32], ratio[float64], steps_done, status)."""
         import numpy as np
+        if getattr(self, "_pend", None) is None:
+            raise FcgError(FCG_INVALID_ARG, "no quasi-static loop pending on this handle")
         nsteps = self._pend[3]
         index = np.full(nsteps, -1, np.int64); iters = np.zeros(nsteps, np.int32); ratio = np.full(nsteps, np.nan, np.float64)
         done = C.c_int(0)

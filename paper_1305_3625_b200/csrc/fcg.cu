@@ -101,6 +101,8 @@ struct fcg_handle_s {
     std::vector<GraphEntry> graphs; unsigned long long stamp = 0;
     long long launches = 0;
     std::string err;
+    int device = 0;                     // the device the handle was created on; every entry point runs with it current
+    unsigned int barrier_start = 0;     // FCG_OPT_BARRIER_START: initial value of the cooperative kernel's barrier counter
 
     template <typename U> U* at(size_t off) const { return reinterpret_cast<U*>(ws + off); }
     Scalars* sc() const { return at<Scalars>(lay.scalars); }
@@ -143,6 +145,55 @@ namespace {
 
 int fail(fcg_handle h, int code, const char* msg) { if (h) h->err = msg; return code; }
 
+// Every entry point runs with the handle's device current and restores the caller's on return (a caller that switched devices
+// between fcg_create and a later call -- common with torch and several GPUs -- would otherwise launch on the wrong device).
+struct DeviceGuard {
+    int prev = -1; bool ok = true, switched = false;
+    explicit DeviceGuard(int want) {
+        if (cudaGetDevice(&prev) != cudaSuccess) { ok = false; cudaGetLastError(); return; }
+        if (prev != want) { ok = cudaSetDevice(want) == cudaSuccess; switched = ok; if (!ok) cudaGetLastError(); }
+    }
+    ~DeviceGuard() { if (switched) cudaSetDevice(prev); }
+};
+#define FCG_ENTER(h)                                                                                                   \
+    DeviceGuard dev_guard_((h)->device);                                                                               \
+    if (!dev_guard_.ok) return fail((h), FCG_CUDA_ERROR, "cannot make the handle's device current");                   \
+    if ((h)->pend_async) return fail((h), FCG_INVALID_ARG, "a quasi-static loop is pending on this handle: call its _end first");  \
+    if ((h)->tab->v2 && (h)->engine_opt == 0 && !(h)->have_tmap)                                                       \
+        return fail((h), FCG_UNSUPPORTED, "cuTensorMapEncodeTiled unavailable: the pipelined passes cannot run; FCG_OPT_ENGINE = 1 selects the classic passes")
+#define FCG_ENTER_OPT(h)                                                                                               \
+    DeviceGuard dev_guard_((h)->device);                                                                               \
+    if (!dev_guard_.ok) return fail((h), FCG_CUDA_ERROR, "cannot make the handle's device current");                   \
+    if ((h)->pend_async) return fail((h), FCG_INVALID_ARG, "a quasi-static loop is pending on this handle: call its _end first")
+#define FCG_ENTER_END(h)                                                                                               \
+    DeviceGuard dev_guard_((h)->device);                                                                               \
+    if (!dev_guard_.ok) return fail((h), FCG_CUDA_ERROR, "cannot make the handle's device current")
+
+bool misaligned(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) != 0; }
+
+// CUDA events that are destroyed on every path out of the profiling calls
+struct EventList {
+    std::vector<cudaEvent_t> ev;
+    ~EventList() { for (auto e : ev) if (e) cudaEventDestroy(e); }
+    cudaError_t create(size_t n) {
+        ev.assign(n, nullptr);
+        for (auto& e : ev) { cudaError_t r = cudaEventCreate(&e); if (r != cudaSuccess) return r; }
+        return cudaSuccess;
+    }
+    cudaEvent_t* operator+(size_t i) { return ev.data() + i; }
+    cudaEvent_t operator[](size_t i) const { return ev[i]; }
+};
+
+// one cooperative launch of fcg_fused.cuh: scalar block zeroed, barrier counter preset, kernel enqueued
+cudaError_t fused_launch(fcg_handle h, FusedArgs& A) {
+    cudaError_t e = cudaMemsetAsync(h->sc(), 0, sizeof(Scalars), h->stream);
+    if (e != cudaSuccess) return e;
+    A.counter_start = h->barrier_start;
+    if (h->barrier_start != 0u &&
+        (e = cudaMemcpyAsync(A.counter, &h->barrier_start, sizeof(unsigned int), cudaMemcpyHostToDevice, h->stream)) != cudaSuccess) return e;
+    return h->tab->fused_solve(&A, h->stream);
+}
+
 // ---- launch sequences (typed) ---------------------------------------------------------------
 template <typename T> struct Seq {
     fcg_handle h; cudaStream_t st; bool classic = false;      // classic: force the synchronous passes (stand-alone transforms)
@@ -160,12 +211,12 @@ template <typename T> struct Seq {
     T* q() const { return h->at<T>(h->lay.q); }
 
     cudaError_t row_fwd(int mode, const T* x, T* u, int check_done = 0) const {
-        RowFwdArgs<T> A{}; A.mode = mode; A.x = x; A.u = u; A.p = p(); A.r = pcg ? z() : r(); A.check_done = check_done; A.hints = h->hints; A.Tb = Tb(); A.tw = tw(); A.sc = h->sc(); A.nsm = h->nsm; A.pdl = h->pdl;
+        RowFwdArgs<T> A{}; A.mode = mode; A.x = x; A.u = u; A.p = p(); A.r = pcg ? z() : r(); A.check_done = check_done; A.hints = h->hints; A.Tb = Tb(); A.tw = tw(); A.sc = h->sc(); A.nsm = h->nsm; A.pdl = h->pdl; A.tmo = &h->sc()->timeout;
         ++h->launches;
         return v2() ? h->tab->row_fwd2(&A, st) : h->tab->row_fwd(h->row_var(), &A, st);
     }
     cudaError_t col(int mode, bool cg, bool precond = false) const {
-        ColArgs<T> A{}; A.mode = mode; A.Tb = Tb(); A.shat = precond ? mhat() : shat(); A.hints = h->hints; A.tw = tw(); A.sc = cg ? h->sc() : nullptr; A.pdl = h->pdl;
+        ColArgs<T> A{}; A.mode = mode; A.Tb = Tb(); A.shat = precond ? mhat() : shat(); A.hints = h->hints; A.tw = tw(); A.sc = cg ? h->sc() : nullptr; A.pdl = h->pdl; A.tmo = &h->sc()->timeout;
         A.nsm = h->nsm;
         ++h->launches;
         if (v2() && mode == COL_CONV && h->colp()) return h->tab->col2p(&A, &h->tmap_col, 0, st);
@@ -174,7 +225,7 @@ template <typename T> struct Seq {
     cudaError_t row_inv(int mode, const T* k, const T* v, const T* f, T* out, T* out2) const {
         RowInvArgs<T> A{}; A.mode = mode; A.Tb = Tb(); A.tw = tw(); A.k = k; A.v = v; A.f = f; A.out = out; A.out2 = out2;
         A.scale = (T)(1.0 / ((double)h->L * (double)h->L)); A.hints = h->hints; A.form = force ? 1 : 0; A.dval = (T)D;
-        A.partial = h->at<double>(h->lay.partial_row); A.sc = h->sc(); A.nsm = h->nsm; A.pdl = h->pdl;
+        A.partial = h->at<double>(h->lay.partial_row); A.sc = h->sc(); A.nsm = h->nsm; A.pdl = h->pdl; A.tmo = &h->sc()->timeout;
         ++h->launches;
         return v2() ? h->tab->row_inv2(&A, &h->tmap_row, st) : h->tab->row_inv(h->row_var(), &A, st);
     }
@@ -201,7 +252,7 @@ template <typename T> struct Seq {
     cudaError_t it_col_m() const { return col(COL_CONV, true, true); }
     cudaError_t it_row_pre() const {
         RowInvArgs<T> A{}; A.mode = ROWI_PRECOND; A.Tb = Tb(); A.tw = tw(); A.k = r(); A.out = z(); A.hints = h->hints;
-        A.partial = h->at<double>(h->lay.partial_row); A.sc = h->sc(); A.nsm = h->nsm; A.pdl = h->pdl;
+        A.partial = h->at<double>(h->lay.partial_row); A.sc = h->sc(); A.nsm = h->nsm; A.pdl = h->pdl; A.tmo = &h->sc()->timeout;
         ++h->launches;
         return v2() ? h->tab->row_inv2_pre(&A, &h->tmap_row, st) : h->tab->row_inv(h->row_var(), &A, st);
     }
@@ -216,7 +267,7 @@ template <typename T> struct Seq {
             cudaError_t e = it_update_r();
             return e != cudaSuccess ? e : row_fwd(ROWF_PLAIN, r(), nullptr, 1);
         }
-        RowFwdArgs<T> A{}; A.mode = ROWF_RUPD; A.hints = h->hints; A.rw = r(); A.q = q(); A.Tb = Tb(); A.tw = tw(); A.sc = h->sc(); A.nsm = h->nsm; A.pdl = h->pdl;
+        RowFwdArgs<T> A{}; A.mode = ROWF_RUPD; A.hints = h->hints; A.rw = r(); A.q = q(); A.Tb = Tb(); A.tw = tw(); A.sc = h->sc(); A.nsm = h->nsm; A.pdl = h->pdl; A.tmo = &h->sc()->timeout;
         A.partial = h->at<double>(h->lay.partial_vec);
         ++h->launches;
         return h->tab->row_fwd2_rupd(&A, st);
@@ -240,7 +291,7 @@ template <typename T> struct Seq {
     }
     // spectral search length: alpha is known after the column pass, so the residual update rides in P3
     cudaError_t it_col_e() const {
-        ColArgs<T> A{}; A.mode = COL_CONV; A.Tb = Tb(); A.shat = shat(); A.hints = h->hints; A.tw = tw(); A.sc = h->sc(); A.pdl = h->pdl;
+        ColArgs<T> A{}; A.mode = COL_CONV; A.Tb = Tb(); A.shat = shat(); A.hints = h->hints; A.tw = tw(); A.sc = h->sc(); A.pdl = h->pdl; A.tmo = &h->sc()->timeout;
         A.partial = h->at<double>(h->lay.partial_col); A.nsm = h->nsm;
         ++h->launches;
         if (h->colp()) return h->tab->col2p(&A, &h->tmap_col, 1, st);
@@ -249,7 +300,7 @@ template <typename T> struct Seq {
     cudaError_t it_row_inv_f(const T* k) const {
         RowInvArgs<T> A{}; A.mode = ROWI_CGF; A.Tb = Tb(); A.tw = tw(); A.k = k; A.v = p(); A.f = r(); A.out = r(); A.hints = h->hints;
         A.partial = h->at<double>(h->lay.partial_row); A.colsum = h->at<double>(h->lay.partial_col);
-        A.sc = h->sc(); A.nsm = h->nsm; A.pdl = h->pdl;
+        A.sc = h->sc(); A.nsm = h->nsm; A.pdl = h->pdl; A.tmo = &h->sc()->timeout;
         ++h->launches;
         if (force) { A.form = 1; A.kappa = kappa; return h->tab->row_inv2_cgf_force(&A, &h->tmap_row, st); }
         return h->tab->row_inv2_cgf(&A, &h->tmap_row, st);
@@ -346,8 +397,7 @@ int solve_impl(fcg_handle h, const void* k, const void* f, void* u, double tol, 
         A.form = force ? 1 : 0; A.D = D;
         A.k = k; A.f = f; A.u = u; A.Tf = h->ws + h->lay.Tb; A.shat = h->ws + h->lay.shat; A.tw = h->ws + h->lay.tw;
         A.partial = h->at<double>(h->lay.partial_row); A.counter = &h->sc()->ticket[3]; A.sc = h->sc(); A.tol = tol; A.maxit = maxit;
-        FCG_CK(h, cudaMemsetAsync(h->sc(), 0, sizeof(Scalars), h->stream));
-        cudaError_t e = h->tab->fused_solve(&A, h->stream);
+        cudaError_t e = fused_launch(h, A);
         if (e == cudaSuccess) {
             FCG_CK(h, cudaMemcpyAsync(h->h_sc, h->sc(), sizeof(Scalars), cudaMemcpyDeviceToHost, h->stream));
             FCG_CK(h, cudaStreamSynchronize(h->stream));
@@ -427,6 +477,7 @@ int solve_impl(fcg_handle h, const void* k, const void* f, void* u, double tol, 
     }
     if (iters) *iters = h->h_sc->it;
     if (relres) *relres = h->h_sc->relres;
+    if (h->h_sc->timeout) return fail(h, FCG_CUDA_ERROR, "a pipelined pass gave up waiting on an mbarrier (TMA copy never completed)");
     return h->h_sc->status;
 }
 
@@ -450,7 +501,7 @@ int fft_impl(fcg_handle h, const void* in, void* out, bool inverse) {
     if (h->v2()) {
         // pipelined passes on the T2 layout; T2 <-> public half spectrum X[m][n] by one line-wise permutation kernel
         Seq<T> s{h, h->stream};
-        ColArgs<T> CA{}; CA.mode = inverse ? COL_INV : COL_FWD; CA.Tb = s.Tb(); CA.tw = s.tw();
+        ColArgs<T> CA{}; CA.mode = inverse ? COL_INV : COL_FWD; CA.Tb = s.Tb(); CA.tw = s.tw(); CA.tmo = &h->sc()->timeout;
         if (!inverse) {
             FCG_CK(h, s.row_fwd(ROWF_PLAIN, (const T*)in, nullptr));
             FCG_CK(h, h->tab->col2_xform(&CA, &h->tmap_col, 0, h->stream));
@@ -495,10 +546,10 @@ int profile_impl(fcg_handle h, const void* k, const void* f, void* u, int iters,
     h->launches = 0;
     FCG_CK(h, s.init((const T*)k, (const T*)f, (T*)u, 0.0, 1 << 30, false, 0ULL));
     for (int w = 0; w < 2; ++w) FCG_CK(h, s.iteration((const T*)k, (T*)u));       // warm-up
-    std::vector<cudaEvent_t> ev((size_t)iters * 5);
-    for (auto& e : ev) FCG_CK(h, cudaEventCreate(&e));
+    EventList ev;
+    FCG_CK(h, ev.create((size_t)iters * 5));
     for (int i = 0; i < iters; ++i) {
-        cudaEvent_t* e = &ev[(size_t)i * 5];
+        cudaEvent_t* e = ev + (size_t)i * 5;
         if (s.sl()) {       // three launches: the residual update is part of P3 (ms[3] = 0)
             FCG_CK(h, cudaEventRecord(e[0], h->stream)); FCG_CK(h, s.it_row_fwd((T*)u));
             FCG_CK(h, cudaEventRecord(e[1], h->stream)); FCG_CK(h, s.it_col_e());
@@ -522,7 +573,6 @@ int profile_impl(fcg_handle h, const void* k, const void* f, void* u, int iters,
             FCG_CK(h, cudaEventElapsedTime(&t, ev[(size_t)i * 5 + q], ev[(size_t)i * 5 + q + 1]));
             ms[q] += (double)t / iters;
         }
-    for (auto& e : ev) cudaEventDestroy(e);
     return h->h_sc->done ? FCG_NOT_CONVERGED : FCG_OK;       // done would mean the loop kernels exited early
 }
 
@@ -534,10 +584,10 @@ int profile_pcg_impl(fcg_handle h, const void* k, const void* f, void* u, int it
     h->launches = 0;
     FCG_CK(h, s.init((const T*)k, (const T*)f, (T*)u, 0.0, 1 << 30, false, 0ULL));
     for (int w = 0; w < 2; ++w) FCG_CK(h, s.iteration((const T*)k, (T*)u));
-    std::vector<cudaEvent_t> ev((size_t)iters * 7);
-    for (auto& e : ev) FCG_CK(h, cudaEventCreate(&e));
+    EventList ev;
+    FCG_CK(h, ev.create((size_t)iters * 7));
     for (int i = 0; i < iters; ++i) {
-        cudaEvent_t* e = &ev[(size_t)i * 7];
+        cudaEvent_t* e = ev + (size_t)i * 7;
         FCG_CK(h, cudaEventRecord(e[0], h->stream)); FCG_CK(h, s.it_row_fwd((T*)u));
         FCG_CK(h, cudaEventRecord(e[1], h->stream)); FCG_CK(h, s.it_col());
         FCG_CK(h, cudaEventRecord(e[2], h->stream)); FCG_CK(h, s.it_row_inv((const T*)k));
@@ -555,7 +605,6 @@ int profile_pcg_impl(fcg_handle h, const void* k, const void* f, void* u, int it
             FCG_CK(h, cudaEventElapsedTime(&t, ev[(size_t)i * 7 + q], ev[(size_t)i * 7 + q + 1]));
             ms[q] += (double)t / iters;
         }
-    for (auto& e : ev) cudaEventDestroy(e);
     return h->h_sc->done ? FCG_NOT_CONVERGED : FCG_OK;
 }
 
@@ -609,8 +658,9 @@ int tensor_map_init(fcg_handle h) {
     cudaDriverEntryPointQueryResult qres;
     if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn ||
         qres != cudaDriverEntryPointSuccess) {
+        // no silent 2x cliff: the pipelined passes are the product; the classic ones run only when asked for (FCG_OPT_ENGINE = 1)
         cudaGetLastError();
-        h->err = "cuTensorMapEncodeTiled unavailable; using the classic passes";
+        h->err = "cuTensorMapEncodeTiled unavailable: the pipelined passes cannot run (FCG_OPT_ENGINE = 1 selects the classic passes)";
         return FCG_OK;
     }
     const cuuint64_t L = (cuuint64_t)h->L, w = (cuuint64_t)h->w, NB = (cuuint64_t)h->tab->v2_nb;
@@ -660,7 +710,9 @@ int fcg_create(int L, fcg_dtype dt, void* workspace, void* cuda_stream, fcg_hand
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) { cudaGetLastError(); return FCG_CUDA_ERROR; }
     fcg_handle h = new fcg_handle_s();
     { int dev = 0, n = 0;
-      if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && n > 0) h->nsm = n; }
+      if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); delete h; return FCG_CUDA_ERROR; }
+      h->device = dev;
+      if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && n > 0) h->nsm = n; }
     h->L = L; h->dtype = dt; h->w = dt == FCG_F64 ? 8 : 4; h->N = (size_t)L * L;
     h->tab = get_table(L, dt);
     h->stream = (cudaStream_t)cuda_stream;
@@ -689,6 +741,7 @@ int fcg_create(int L, fcg_dtype dt, void* workspace, void* cuda_stream, fcg_hand
 
 int fcg_destroy(fcg_handle h) {
     if (!h) return FCG_INVALID_ARG;
+    DeviceGuard dev_guard_(h->device);
     if (h->stream || h->ws) cudaStreamSynchronize(h->stream);
     for (auto& g : h->graphs) drop_graph(g);
     if (h->cap_stream) cudaStreamDestroy(h->cap_stream);
@@ -709,6 +762,7 @@ int fcg_destroy(fcg_handle h) {
 
 int fcg_set_option(fcg_handle h, int option, int value) {
     if (!h) return FCG_INVALID_ARG;
+    FCG_ENTER_OPT(h);
     switch (option) {
         case FCG_OPT_LOOP_MODE: if (value != 0 && value != 1) return fail(h, FCG_INVALID_ARG, "loop mode must be 0 or 1"); h->loop_mode = value; return FCG_OK;
         case FCG_OPT_CHUNK: if (value < 1) return fail(h, FCG_INVALID_ARG, "chunk must be >= 1"); h->chunk = value; return FCG_OK;
@@ -720,6 +774,7 @@ int fcg_set_option(fcg_handle h, int option, int value) {
         case FCG_OPT_L2_HINTS: if (value < 0 || value > 255) return fail(h, FCG_INVALID_ARG, "hints must be 0..255"); h->hints = value; return FCG_OK;
         case FCG_OPT_SPECTRAL_ALPHA: if (value != 0 && value != 1) return fail(h, FCG_INVALID_ARG, "spectral alpha must be 0 or 1"); h->sl_opt = value; return FCG_OK;
         case FCG_OPT_COL_PERSISTENT: if (value < -1 || value > 1) return fail(h, FCG_INVALID_ARG, "col persistent must be -1, 0 or 1"); h->colp_opt = value; return FCG_OK;
+        case FCG_OPT_BARRIER_START: h->barrier_start = (unsigned int)value; return FCG_OK;
         case FCG_OPT_UNROLL: if (value < 1 || value > 64) return fail(h, FCG_INVALID_ARG, "unroll must be 1..64"); h->unroll = value; return FCG_OK;
         case FCG_OPT_ENGINE:
             if (value != 0 && value != 1) return fail(h, FCG_INVALID_ARG, "engine must be 0 or 1");
@@ -732,6 +787,7 @@ int fcg_set_option(fcg_handle h, int option, int value) {
 
 int fcg_set_spectrum(fcg_handle h, const void* s) {
     if (!h || !s) return fail(h, FCG_INVALID_ARG, "null argument");
+    FCG_ENTER(h);
     h->spectrum_colpos = h->v2() ? 1 : 0;
     FCG_CK(h, h->tab->spectrum_prep(s, h->at<void>(h->lay.shat), h->spectrum_colpos, h->stream));
     FCG_CK(h, cudaStreamSynchronize(h->stream));      // the caller's array is not referenced after return
@@ -741,6 +797,7 @@ int fcg_set_spectrum(fcg_handle h, const void* s) {
 
 int fcg_apply(fcg_handle h, const void* k, const void* x, void* y) {
     if (!h || !k || !x || !y) return fail(h, FCG_INVALID_ARG, "null argument");
+    FCG_ENTER(h);
     if (y == k || y == x) return fail(h, FCG_INVALID_ARG, "y must not alias k or x");
     if (!h->have_spectrum) return fail(h, FCG_NO_SPECTRUM, "fcg_set_spectrum has not been called");
     return h->dtype == FCG_F64 ? apply_impl<double>(h, k, x, y) : apply_impl<float>(h, k, x, y);
@@ -748,6 +805,9 @@ int fcg_apply(fcg_handle h, const void* k, const void* x, void* y) {
 
 int fcg_solve(fcg_handle h, const void* k, const void* f, void* u, double tol, int maxit, int* iters_host, double* rel_residual_host) {
     if (!h || !k || !f || !u) return fail(h, FCG_INVALID_ARG, "null argument");
+    FCG_ENTER(h);
+    if (u == k || u == f) return fail(h, FCG_INVALID_ARG, "u must not alias k or f");
+    if (misaligned(k) || misaligned(f) || misaligned(u)) return fail(h, FCG_INVALID_ARG, "k, f, u must be 16-byte aligned");
     if (!(tol >= 0.0) || maxit < 0) return fail(h, FCG_INVALID_ARG, "tol must be >= 0 and maxit >= 0");
     if (!h->have_spectrum) return fail(h, FCG_NO_SPECTRUM, "fcg_set_spectrum has not been called");
     return h->dtype == FCG_F64 ? solve_impl<double>(h, k, f, u, tol, maxit, iters_host, rel_residual_host)
@@ -756,6 +816,7 @@ int fcg_solve(fcg_handle h, const void* k, const void* f, void* u, double tol, i
 
 int fcg_set_preconditioner(fcg_handle h, const void* s, double kbar) {
     if (!h || !s) return fail(h, FCG_INVALID_ARG, "null argument");
+    FCG_ENTER(h);
     if (!(kbar >= 0.0) || !std::isfinite(kbar)) return fail(h, FCG_INVALID_ARG, "kbar must be finite and >= 0");
     if (!h->have_spectrum) return fail(h, FCG_NO_SPECTRUM, "fcg_set_spectrum has not been called");
     int st = h->dtype == FCG_F64 ? precond_impl<double>(h, s, kbar) : precond_impl<float>(h, s, kbar);
@@ -765,6 +826,9 @@ int fcg_set_preconditioner(fcg_handle h, const void* s, double kbar) {
 
 int fcg_pcg_solve(fcg_handle h, const void* k, const void* f, void* u, double tol, int maxit, int* iters_host, double* rel_residual_host) {
     if (!h || !k || !f || !u) return fail(h, FCG_INVALID_ARG, "null argument");
+    FCG_ENTER(h);
+    if (u == k || u == f) return fail(h, FCG_INVALID_ARG, "u must not alias k or f");
+    if (misaligned(k) || misaligned(f) || misaligned(u)) return fail(h, FCG_INVALID_ARG, "k, f, u must be 16-byte aligned");
     if (!(tol >= 0.0) || maxit < 0) return fail(h, FCG_INVALID_ARG, "tol must be >= 0 and maxit >= 0");
     if (!h->have_spectrum) return fail(h, FCG_NO_SPECTRUM, "fcg_set_spectrum has not been called");
     if (!h->have_precond) return fail(h, FCG_NO_SPECTRUM, "fcg_set_preconditioner has not been called");
@@ -774,6 +838,7 @@ int fcg_pcg_solve(fcg_handle h, const void* k, const void* f, void* u, double to
 
 int fcg_profile_pcg_iteration(fcg_handle h, const void* k, const void* f, void* u, int iters, double* ms_host) {
     if (!h || !k || !f || !u || iters < 1 || !ms_host) return fail(h, FCG_INVALID_ARG, "bad argument");
+    FCG_ENTER(h);
     if (!h->have_spectrum || !h->have_precond) return fail(h, FCG_NO_SPECTRUM, "spectrum or preconditioner not set");
     if (!h->v2()) return fail(h, FCG_UNSUPPORTED, "pipelined engine only");
     return h->dtype == FCG_F64 ? profile_pcg_impl<double>(h, k, f, u, iters, ms_host) : profile_pcg_impl<float>(h, k, f, u, iters, ms_host);
@@ -782,6 +847,7 @@ int fcg_profile_pcg_iteration(fcg_handle h, const void* k, const void* f, void* 
 int fcg_solve_host(fcg_handle h, const void* k_host, const void* f_host, void* u_host, double tol, int maxit,
                    int* iters_host, double* rel_residual_host) {
     if (!h || !k_host || !f_host || !u_host) return fail(h, FCG_INVALID_ARG, "null argument");
+    FCG_ENTER(h);
     const size_t bytes = h->N * h->w;
     if (!h->hk) { FCG_CK(h, cudaMalloc(&h->hk, bytes)); FCG_CK(h, cudaMalloc(&h->hf, bytes)); FCG_CK(h, cudaMalloc(&h->hu, bytes)); }
     FCG_CK(h, cudaMemcpyAsync(h->hk, k_host, bytes, cudaMemcpyHostToDevice, h->stream));
@@ -796,16 +862,19 @@ int fcg_solve_host(fcg_handle h, const void* k_host, const void* f_host, void* u
 
 int fcg_fft_fwd(fcg_handle h, const void* x, void* X) {
     if (!h || !x || !X) return fail(h, FCG_INVALID_ARG, "null argument");
+    FCG_ENTER(h);
     return h->dtype == FCG_F64 ? fft_impl<double>(h, x, X, false) : fft_impl<float>(h, x, X, false);
 }
 
 int fcg_fft_inv(fcg_handle h, const void* X, void* x) {
     if (!h || !x || !X) return fail(h, FCG_INVALID_ARG, "null argument");
+    FCG_ENTER(h);
     return h->dtype == FCG_F64 ? fft_impl<double>(h, X, x, true) : fft_impl<float>(h, X, x, true);
 }
 
 int fcg_break_step(fcg_handle h, void* k, const void* u, const void* t, long long* index_host, double* ratio_host) {
     if (!h || !k || !u || !t) return fail(h, FCG_INVALID_ARG, "null argument");
+    FCG_ENTER(h);
     h->launches = 0;
     return h->dtype == FCG_F64 ? break_impl<double>(h, k, u, t, index_host, ratio_host)
                                : break_impl<float>(h, k, u, t, index_host, ratio_host);
@@ -829,7 +898,9 @@ static int frac_reserve(fcg_handle h, int nsteps) {
 // loop is one cooperative kernel, returns at once); end blocks and hands out the results.
 static int fracture_begin(fcg_handle h, void* k, const void* f, void* u, const void* t, int nsteps, double tol, int maxit, bool pcg) {
     if (!h || !k || !f || !u || !t || nsteps < 0) return fail(h, FCG_INVALID_ARG, "bad argument");
+    FCG_ENTER(h);
     if (pcg && !h->have_precond) return fail(h, FCG_NO_SPECTRUM, "fcg_set_preconditioner has not been called");
+    if (h->pend_nsteps >= 0) return fail(h, FCG_INVALID_ARG, "a quasi-static loop is already pending on this handle: call its _end first");
     h->pend_nsteps = -1; h->pend_async = false; h->pend_done = 0; h->pend_status = FCG_OK; h->pend_kind = 0;
     if (h->fused() && h->have_spectrum && nsteps > 0 && tol >= 0.0 && maxit >= 0) {
         // small lattices: the whole quasi-static loop -- every solve and every break step -- is one cooperative kernel
@@ -840,8 +911,7 @@ static int fracture_begin(fcg_handle h, void* k, const void* f, void* u, const v
         A.mhat = pcg ? h->ws + h->lay.mhat : nullptr;
         A.nsteps = nsteps; A.t = t; A.k_out = k; A.out_index = h->frac_idx; A.out_iters = h->frac_it;
         A.brk_r = h->at<double>(h->lay.brk_r); A.brk_i = h->at<long long>(h->lay.brk_i);
-        FCG_CK(h, cudaMemsetAsync(h->sc(), 0, sizeof(Scalars), h->stream));
-        cudaError_t e = h->tab->fused_solve(&A, h->stream);
+        cudaError_t e = fused_launch(h, A);
         if (e == cudaSuccess) {
             FCG_CK(h, cudaMemcpyAsync(h->h_sc, h->sc(), sizeof(Scalars), cudaMemcpyDeviceToHost, h->stream));
             h->pend_nsteps = nsteps; h->pend_async = true; h->launches = 1;
@@ -870,9 +940,11 @@ static int fracture_begin(fcg_handle h, void* k, const void* f, void* u, const v
 
 static int fracture_end(fcg_handle h, long long* index_host, int* iters_host, int* steps_done_host) {
     if (!h || !index_host || !iters_host) return fail(h, FCG_INVALID_ARG, "bad argument");
+    FCG_ENTER_END(h);
     if (h->pend_nsteps < 0 || h->pend_kind != 0) return fail(h, FCG_INVALID_ARG, "no quasi-static loop of this kind pending on this handle");
     h->pend_nsteps = -1;
     if (h->pend_async) {
+        h->pend_async = false;
         FCG_CK(h, cudaStreamSynchronize(h->stream));
         const int done = h->h_sc->steps_done;
         if (done > 0) {
@@ -919,12 +991,14 @@ int fcg_pcg_fracture(fcg_handle h, void* k, const void* f, void* u, const void* 
 // ---- the paper's formulation in the bond forces, (I + K G) f = K D (eq. (2))
 int fcg_green_function(fcg_handle h, double nu, double E, double a, void* G) {
     if (!h || !G) return fail(h, FCG_INVALID_ARG, "null argument");
+    FCG_ENTER(h);
     if (!(E > 0.0) || !(a > 0.0) || !std::isfinite(nu) || !std::isfinite(E) || !std::isfinite(a)) return fail(h, FCG_INVALID_ARG, "E and a must be positive and finite, nu finite");
     return h->dtype == FCG_F64 ? green_impl<double>(h, nu, E, a, G) : green_impl<float>(h, nu, E, a, G);
 }
 
 int fcg_kernel_spectrum(fcg_handle h, const void* G, void* s) {
     if (!h || !G || !s) return fail(h, FCG_INVALID_ARG, "null argument");
+    FCG_ENTER(h);
     if (G == s) return fail(h, FCG_INVALID_ARG, "s must not alias G");
     static_assert(ALIGN % 16 == 0, "workspace alignment");
     if (h->lay.p != h->lay.r + h->N * h->w) return fail(h, FCG_UNSUPPORTED, "workspace layout: r and p not adjacent");
@@ -933,6 +1007,7 @@ int fcg_kernel_spectrum(fcg_handle h, const void* G, void* s) {
 
 int fcg_inverse_spectrum(fcg_handle h, const void* g, void* s) {
     if (!h || !g || !s) return fail(h, FCG_INVALID_ARG, "null argument");
+    FCG_ENTER(h);
     if (h->dtype == FCG_F64) inverse_spectrum_kernel<double><<<h->vec_blocks(), 256, 0, h->stream>>>((const double*)g, (double*)s, h->N);
     else inverse_spectrum_kernel<float><<<h->vec_blocks(), 256, 0, h->stream>>>((const float*)g, (float*)s, h->N);
     FCG_CK(h, cudaGetLastError());
@@ -941,6 +1016,7 @@ int fcg_inverse_spectrum(fcg_handle h, const void* g, void* s) {
 
 int fcg_force_rhs(fcg_handle h, const void* k, double D, void* b) {
     if (!h || !k || !b || !std::isfinite(D)) return fail(h, FCG_INVALID_ARG, "null argument or D not finite");
+    FCG_ENTER(h);
     if (h->dtype == FCG_F64) scale_kernel<double><<<h->vec_blocks(), 256, 0, h->stream>>>((const double*)k, (double*)b, h->N, D);
     else scale_kernel<float><<<h->vec_blocks(), 256, 0, h->stream>>>((const float*)k, (float*)b, h->N, (float)D);
     FCG_CK(h, cudaGetLastError());
@@ -949,6 +1025,7 @@ int fcg_force_rhs(fcg_handle h, const void* k, double D, void* b) {
 
 int fcg_force_from_displacement(fcg_handle h, const void* k, double D, const void* u, void* f) {
     if (!h || !k || !u || !f || !std::isfinite(D)) return fail(h, FCG_INVALID_ARG, "null argument or D not finite");
+    FCG_ENTER(h);
     if (h->dtype == FCG_F64) force_from_displacement_kernel<double><<<h->vec_blocks(), 256, 0, h->stream>>>((const double*)k, (const double*)u, (double*)f, h->N, D);
     else force_from_displacement_kernel<float><<<h->vec_blocks(), 256, 0, h->stream>>>((const float*)k, (const float*)u, (float*)f, h->N, (float)D);
     FCG_CK(h, cudaGetLastError());
@@ -957,6 +1034,7 @@ int fcg_force_from_displacement(fcg_handle h, const void* k, double D, const voi
 
 int fcg_force_apply(fcg_handle h, const void* k, const void* x, void* y) {
     if (!h || !k || !x || !y) return fail(h, FCG_INVALID_ARG, "null argument");
+    FCG_ENTER(h);
     if (y == k || y == x) return fail(h, FCG_INVALID_ARG, "y must not alias k or x");
     if (!h->have_spectrum) return fail(h, FCG_NO_SPECTRUM, "fcg_set_spectrum has not been called");
     return h->dtype == FCG_F64 ? apply_impl<double>(h, k, x, y, true) : apply_impl<float>(h, k, x, y, true);
@@ -964,6 +1042,7 @@ int fcg_force_apply(fcg_handle h, const void* k, const void* x, void* y) {
 
 int fcg_force_solve(fcg_handle h, const void* k, double D, void* f, double tol, int maxit, int* iters_host, double* rel_residual_host) {
     if (!h || !k || !f) return fail(h, FCG_INVALID_ARG, "null argument");
+    FCG_ENTER(h);
     if (!(tol >= 0.0) || maxit < 0 || !std::isfinite(D)) return fail(h, FCG_INVALID_ARG, "tol must be >= 0, maxit >= 0, D finite");
     if (!h->have_spectrum) return fail(h, FCG_NO_SPECTRUM, "fcg_set_spectrum has not been called");
     return h->dtype == FCG_F64 ? solve_impl<double>(h, k, nullptr, f, tol, maxit, iters_host, rel_residual_host, false, true, D)
@@ -972,6 +1051,7 @@ int fcg_force_solve(fcg_handle h, const void* k, double D, void* f, double tol, 
 
 int fcg_force_break_step(fcg_handle h, void* k, void* f, const void* t, long long* index_host, double* ratio_host) {
     if (!h || !k || !f || !t) return fail(h, FCG_INVALID_ARG, "null argument");
+    FCG_ENTER(h);
     h->launches = 0;
     return h->dtype == FCG_F64 ? break_impl<double>(h, k, f, t, index_host, ratio_host, f)
                                : break_impl<float>(h, k, f, t, index_host, ratio_host, f);
@@ -980,6 +1060,7 @@ int fcg_force_break_step(fcg_handle h, void* k, void* f, const void* t, long lon
 int fcg_force_fracture(fcg_handle h, void* k, double D, void* f, const void* t, int nsteps, double tol, int maxit,
                        long long* index_host, int* iters_host, double* ratio_host, int* steps_done_host) {
     if (!h || !k || !f || !t || nsteps < 0 || !index_host || !iters_host) return fail(h, FCG_INVALID_ARG, "bad argument");
+    FCG_ENTER(h);
     if (!(tol >= 0.0) || maxit < 0 || !std::isfinite(D)) return fail(h, FCG_INVALID_ARG, "tol must be >= 0, maxit >= 0, D finite");
     if (!h->have_spectrum) return fail(h, FCG_NO_SPECTRUM, "fcg_set_spectrum has not been called");
     if (h->fused() && nsteps > 0) {
@@ -990,8 +1071,7 @@ int fcg_force_fracture(fcg_handle h, void* k, double D, void* f, const void* t, 
         A.partial = h->at<double>(h->lay.partial_row); A.counter = &h->sc()->ticket[3]; A.sc = h->sc(); A.tol = tol; A.maxit = maxit;
         A.nsteps = nsteps; A.t = t; A.k_out = k; A.out_index = h->frac_idx; A.out_iters = h->frac_it; A.out_ratio = h->frac_ratio;
         A.brk_r = h->at<double>(h->lay.brk_r); A.brk_i = h->at<long long>(h->lay.brk_i);
-        FCG_CK(h, cudaMemsetAsync(h->sc(), 0, sizeof(Scalars), h->stream));
-        cudaError_t e = h->tab->fused_solve(&A, h->stream);
+        cudaError_t e = fused_launch(h, A);
         if (e == cudaSuccess) {
             FCG_CK(h, cudaMemcpyAsync(h->h_sc, h->sc(), sizeof(Scalars), cudaMemcpyDeviceToHost, h->stream));
             FCG_CK(h, cudaStreamSynchronize(h->stream));
@@ -1033,9 +1113,11 @@ int fcg_force_fracture(fcg_handle h, void* k, double D, void* f, const void* t, 
 // fcg_fracture_begin / _end so that one host thread can keep an ensemble of samples (handles on their own streams) in flight
 int fcg_force_fracture_displacement_begin(fcg_handle h, void* k, double D, void* u, const void* t, int nsteps, double tol, int maxit, int use_pcg) {
     if (!h || !k || !u || !t || nsteps < 0) return fail(h, FCG_INVALID_ARG, "bad argument");
+    FCG_ENTER(h);
     if (!(tol >= 0.0) || maxit < 0 || !std::isfinite(D)) return fail(h, FCG_INVALID_ARG, "tol must be >= 0, maxit >= 0, D finite");
     if (!h->have_spectrum) return fail(h, FCG_NO_SPECTRUM, "fcg_set_spectrum has not been called");
     if (use_pcg && !h->have_precond) return fail(h, FCG_NO_SPECTRUM, "fcg_set_preconditioner has not been called");
+    if (h->pend_nsteps >= 0) return fail(h, FCG_INVALID_ARG, "a quasi-static loop is already pending on this handle: call its _end first");
     h->pend_nsteps = -1; h->pend_async = false; h->pend_done = 0; h->pend_status = FCG_OK; h->pend_kind = 1;
     if (h->fused() && nsteps > 0) {
         // small lattices: the whole loop in one cooperative kernel (fcg_fused.cuh, FORCE = 2)
@@ -1046,8 +1128,7 @@ int fcg_force_fracture_displacement_begin(fcg_handle h, void* k, double D, void*
         A.partial = h->at<double>(h->lay.partial_row); A.counter = &h->sc()->ticket[3]; A.sc = h->sc(); A.tol = tol; A.maxit = maxit;
         A.nsteps = nsteps; A.t = t; A.k_out = k; A.out_index = h->frac_idx; A.out_iters = h->frac_it; A.out_ratio = h->frac_ratio;
         A.brk_r = h->at<double>(h->lay.brk_r); A.brk_i = h->at<long long>(h->lay.brk_i);
-        FCG_CK(h, cudaMemsetAsync(h->sc(), 0, sizeof(Scalars), h->stream));
-        cudaError_t e = h->tab->fused_solve(&A, h->stream);
+        cudaError_t e = fused_launch(h, A);
         if (e == cudaSuccess) {
             FCG_CK(h, cudaMemcpyAsync(h->h_sc, h->sc(), sizeof(Scalars), cudaMemcpyDeviceToHost, h->stream));
             h->pend_nsteps = nsteps; h->pend_async = true; h->launches = 1;
@@ -1083,9 +1164,11 @@ int fcg_force_fracture_displacement_begin(fcg_handle h, void* k, double D, void*
 
 int fcg_force_fracture_displacement_end(fcg_handle h, long long* index_host, int* iters_host, double* ratio_host, int* steps_done_host) {
     if (!h || !index_host || !iters_host) return fail(h, FCG_INVALID_ARG, "bad argument");
+    FCG_ENTER_END(h);
     if (h->pend_nsteps < 0 || h->pend_kind != 1) return fail(h, FCG_INVALID_ARG, "no quasi-static loop of this kind pending on this handle");
     h->pend_nsteps = -1; h->pend_kind = 0;
     if (h->pend_async) {
+        h->pend_async = false;
         FCG_CK(h, cudaStreamSynchronize(h->stream));
         const int done = h->h_sc->steps_done;
         if (done > 0) {
@@ -1117,6 +1200,7 @@ int fcg_force_fracture_displacement(fcg_handle h, void* k, double D, void* u, co
 
 int fcg_profile_iteration(fcg_handle h, const void* k, const void* f, void* u, int iters, double* ms_host) {
     if (!h || !k || !f || !u || iters < 1 || !ms_host) return fail(h, FCG_INVALID_ARG, "bad argument");
+    FCG_ENTER(h);
     if (!h->have_spectrum) return fail(h, FCG_NO_SPECTRUM, "fcg_set_spectrum has not been called");
     return h->dtype == FCG_F64 ? profile_impl<double>(h, k, f, u, iters, ms_host) : profile_impl<float>(h, k, f, u, iters, ms_host);
 }

@@ -177,7 +177,7 @@ __global__ void __launch_bounds__(P::NT + 32, CTAS) row_fwd2_kernel(const RowFwd
         // L2 hints (bit 0): u is not touched again before the next iteration's P1 -- its strips should not displace T2, q, r
         const uint64_t pol = (cg && lane >= 4 && (A.hints & 1)) ? tma::policy_evict_first() : tma::policy_evict_normal();
         for (int g = 0; g < G; ++g) {
-            if (g >= NSLOT) tma::mbar_wait(&empty[slot], phase ^ 1u);          // the slot's previous strip has been read by every warp
+            if (g >= NSLOT) tma::mbar_wait(&empty[slot], phase ^ 1u, A.tmo);          // the slot's previous strip has been read by every warp
             if (lane == 0) tma::mbar_expect_tx(&full[slot], nv * PIECE);
             __syncwarp();
             if (lane < nv)
@@ -206,7 +206,7 @@ __global__ void __launch_bounds__(P::NT + 32, CTAS) row_fwd2_kernel(const RowFwd
         cx<T> z[PER1][R1];
 #pragma unroll
         for (int t = 0; t < R1; ++t) {
-            tma::mbar_wait(&full[slot], phase);
+            tma::mbar_wait(&full[slot], phase, A.tmo);
             const T* sl = reinterpret_cast<const T*>(ring + (size_t)slot * SLOTB);
 #pragma unroll
             for (int q = 0; q < PER1; ++q) {
@@ -320,7 +320,7 @@ __global__ void __launch_bounds__(P::NT, CTAS) col2_kernel(const ColArgs<T> A, c
     }
     __syncthreads();
     const bool done = A.sc && A.sc->done;
-    tma::mbar_wait(&bar, 0);
+    tma::mbar_wait(&bar, 0, A.tmo);
     if (done) return;
     double energy = 0.0;
 
@@ -398,7 +398,7 @@ __global__ void __launch_bounds__(P::NT, CTAS) col2_kernel(const ColArgs<T> A, c
     tma::fence_proxy_async();                 // my writes -> visible to the async proxy
     tma::mbar_warp_arrive(&ready);
     if (lt == 0) {
-        tma::mbar_wait(&ready, 0);            // every warp's part of the column is in place
+        tma::mbar_wait(&ready, 0, A.tmo);            // every warp's part of the column is in place
 #pragma unroll
         for (int b = 0; b < (L / 2) / ABOX; ++b)
             tma::tensor_s2g_4d(&tmap, 0, n % AS::NB, b * ABOX, n / AS::NB, smem_raw + (size_t)b * BOXB);
@@ -473,7 +473,7 @@ __global__ void __launch_bounds__(P::NT + 32, CTAS) col2p_kernel(const ColArgs<T
             for (int i = 0; i < cnt; ++i) {
                 const int n = col_of(i), b = i & 1;
                 unsigned char* Wb = smem_raw + (size_t)b * CP::BUF;
-                tma::mbar_wait(&ready[b], (uint32_t)((i >> 1) & 1));          // every consumer warp's part of column i is in place
+                tma::mbar_wait(&ready[b], (uint32_t)((i >> 1) & 1), A.tmo);          // every consumer warp's part of column i is in place
 #pragma unroll
                 for (int q = 0; q < (L / 2) / ABOX; ++q)
                     tma::tensor_s2g_4d(&tmap, 0, n % AS::NB, q * ABOX, n / AS::NB, Wb + (size_t)q * BOXB);
@@ -494,7 +494,7 @@ __global__ void __launch_bounds__(P::NT + 32, CTAS) col2p_kernel(const ColArgs<T
         const T* sh = reinterpret_cast<const T*>(smem_raw + (size_t)b * CP::BUF + AS::WBYTES);
         SmemIO<T, P> io{W};
         double energy = 0.0;
-        tma::mbar_wait(&full[b], (uint32_t)((i >> 1) & 1));
+        tma::mbar_wait(&full[b], (uint32_t)((i >> 1) & 1), A.tmo);
         auto ld_sw = [&](int e) { return io.ld(e); };
         auto st_sw = [&](int e, cx<T> v) { io.st(e, v); };
         auto fwd_smem_stage = [&](auto s) {
@@ -608,7 +608,7 @@ __global__ void __launch_bounds__(P::NT, CTAS) col2_xform_kernel(const ColArgs<T
     __syncthreads();
     cx<T> wb[S + 1][PM];
     static_for_up<1, S - 1>([&](auto s) { base_tw<P, decltype(s)::value, T>(lt, A.tw, wb[decltype(s)::value]); });
-    tma::mbar_wait(&bar, 0);
+    tma::mbar_wait(&bar, 0, A.tmo);
     auto ld_sw = [&](int e) { return io.ld(e); };
     auto st_sw = [&](int e, cx<T> v) { io.st(e, v); };
     if constexpr (DIR < 0) {
@@ -659,7 +659,7 @@ __global__ void __launch_bounds__(P::NT, CTAS) col2_xform_kernel(const ColArgs<T
     tma::fence_proxy_async();
     tma::mbar_warp_arrive(&ready);
     if (lt == 0) {
-        tma::mbar_wait(&ready, 0);
+        tma::mbar_wait(&ready, 0, A.tmo);
 #pragma unroll
         for (int b = 0; b < (L / 2) / ABOX; ++b)
             tma::tensor_s2g_4d(&tmap, 0, n % AS::NB, b * ABOX, n / AS::NB, smem_raw + (size_t)b * BOXB);
@@ -815,7 +815,7 @@ __global__ void __launch_bounds__(AsyncShape<T, P>::INV_THREADS, CTAS) row_inv2_
     const uint64_t pol_r = (A.hints & 128) ? tma::policy_evict_last() : tma::policy_evict_normal();   // (bit 7) the new r is read back by the next P1
     const uint64_t pol_k = (lane < 2 && !PRE && (A.hints & 16)) ? tma::policy_evict_first() : tma::policy_evict_normal();
     auto issue_next_T = [&]() {          // whole warp; tile p_tn = (transform p_tn / NSUB, part p_tn % NSUB): TSUB / NB whole lines
-        if (p_tn >= NTS) tma::mbar_wait(&tempty[p_ts], p_tph ^ 1u);
+        if (p_tn >= NTS) tma::mbar_wait(&tempty[p_ts], p_tph ^ 1u, A.tmo);
         if (lane == 0) {
             tma::mbar_expect_tx(&tfull[p_ts], TBYTES);
             tma::tensor_g2s_3d_hint(tring + (size_t)p_ts * TBYTES, &tmap, 0, tile_of(p_tn / NSUB), (p_tn % NSUB) * (TSUB / AS::NB), &tfull[p_ts], pol_t);
@@ -824,7 +824,7 @@ __global__ void __launch_bounds__(AsyncShape<T, P>::INV_THREADS, CTAS) row_inv2_
         if (++p_ts == NTS) { p_ts = 0; p_tph ^= 1u; }
     };
     auto issue_next_K = [&]() {          // whole warp; strip p_kn % (R1 SPT) of k0 k1 v0 v1 (f0 f1) of transform p_kn / (R1 SPT), one bulk copy per lane < nv
-        if (p_kn >= nks) tma::mbar_wait(&kempty[p_ks], p_kph ^ 1u);
+        if (p_kn >= nks) tma::mbar_wait(&kempty[p_ks], p_kph ^ 1u, A.tmo);
         if (lane == 0) tma::mbar_expect_tx(&kfull[p_ks], kslotb);
         __syncwarp();
         if (lane < nv)
@@ -873,7 +873,7 @@ __global__ void __launch_bounds__(AsyncShape<T, P>::INV_THREADS, CTAS) row_inv2_
             const size_t row0 = (size_t)a0 * L;
             // rebuild the packed spectrum Z = X_even + i X_odd at its digit-reversed place, tile by tile
             for (int sub = 0; sub < NSUB; ++sub) {
-                tma::mbar_wait(&tfull[ts], tph);
+                tma::mbar_wait(&tfull[ts], tph, A.tmo);
                 const cx<T>* Ts = reinterpret_cast<const cx<T>*>(tring + (size_t)ts * TBYTES);
 #pragma unroll 4
                 for (int ml = lt; ml < TSUB; ml += NT) {
@@ -906,14 +906,14 @@ __global__ void __launch_bounds__(AsyncShape<T, P>::INV_THREADS, CTAS) row_inv2_
             stage_ld<P, 1, T>(lt, [&](int e) { return io.ld(e); }, c);
             bar_named<NT>();                                          // W may now be rebuilt for the next transform
             stage_math<P, 1, +1, T>(c, wb[1]);
-            T f_rr = (T)0, f_t = (T)0, f_v = (T)0;                   // CGF: one transform's sums in the working precision, then double
+            double f_rr = 0.0, f_t = 0.0, f_v = 0.0;                 // CGF: products and sums in double for both dtypes (reading S12)
 #pragma unroll
             for (int t = 0; t < R1; ++t) {
 #pragma unroll
               for (int qq = 0; qq < SPT; ++qq) {
                 const T* sl = nullptr;
                 if (nv) {
-                    tma::mbar_wait(&kfull[ks], kph);
+                    tma::mbar_wait(&kfull[ks], kph, A.tmo);
                     sl = reinterpret_cast<const T*>(kring + (size_t)ks * kslotb);
                 }
 #pragma unroll
@@ -933,10 +933,11 @@ __global__ void __launch_bounds__(AsyncShape<T, P>::INV_THREADS, CTAS) row_inv2_
                     if constexpr (CGF) {
                         const T r0 = sl[4 * QV + j] - alpha * val0, r1 = sl[5 * QV + j] - alpha * val1;   // residue
                         if (st_on) { tma::st_hint(A.out + i0, r0, pol_r); tma::st_hint(A.out + i0 + L, r1, pol_r); }
-                        f_rr += r0 * r0; f_rr += r1 * r1;                                                   // residue length (97)
-                        const T kr0 = FCGF ? r0 : sl[j] * r0, kr1 = FCGF ? r1 : sl[QV + j] * r1;
-                        f_t += kr0 * r0; f_t += kr1 * r1;
-                        f_v += kr0 * v0; f_v += kr1 * v1;
+                        const double r0d = (double)r0, r1d = (double)r1;
+                        f_rr += r0d * r0d; f_rr += r1d * r1d;                                               // residue length (97)
+                        const double kr0 = FCGF ? r0d : (double)sl[j] * r0d, kr1 = FCGF ? r1d : (double)sl[QV + j] * r1d;
+                        f_t += kr0 * r0d; f_t += kr1 * r1d;
+                        f_v += kr0 * (double)v0; f_v += kr1 * (double)v1;
                         continue;
                     }
                     if (mode == ROWI_RESID) {
@@ -957,7 +958,7 @@ __global__ void __launch_bounds__(AsyncShape<T, P>::INV_THREADS, CTAS) row_inv2_
                 }
               }
             }
-            if constexpr (CGF) { acc3[0] += (double)f_rr; acc3[1] += (double)f_t; acc3[2] += (double)f_v; }
+            if constexpr (CGF) { acc3[0] += f_rr; acc3[1] += f_t; acc3[2] += f_v; }
         }
     }
     if constexpr (CGF) {         // all warps (the producers contribute zeros)

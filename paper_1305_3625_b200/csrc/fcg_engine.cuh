@@ -67,12 +67,19 @@ FCG_HD void run_middle(int lt, LD ld, ST st, MUL mul, double* energy = nullptr)
 #pragma unroll
         for (int t = 0; t < R; ++t) a[t] = ld(base + t);
         dftR<R, -1>(a);
-#pragma unroll
+#ifdef FCG_ENERGY_WIDE
+        double e = 0.0;
+#else
         T e = (T)0;
+#endif
 #pragma unroll
         for (int u = 0; u < R; ++u) {
             const T sv = mul(lt + i * P::NT, u);
+#ifdef FCG_ENERGY_WIDE
+            if constexpr (ENERGY) e += (double)sv * ((double)a[u].x * (double)a[u].x + (double)a[u].y * (double)a[u].y);
+#else
             if constexpr (ENERGY) e += sv * (a[u].x * a[u].x + a[u].y * a[u].y);
+#endif
             a[u].x *= sv; a[u].y *= sv;
         }
         if constexpr (ENERGY) *energy += (double)e;

@@ -28,7 +28,8 @@ struct FusedArgs {
     void* Tf;                                   // workspace: L/2 columns x L complex, column m contiguous
     const void* shat; const void* tw;
     double* partial;                            // 4 x G doubles
-    unsigned int* counter;                      // grid barrier (zeroed by the host before the launch)
+    unsigned int* counter;                      // grid barrier (set to counter_start by the host before the launch)
+    unsigned int counter_start;                 // normally 0; FCG_OPT_BARRIER_START presets it (test of the wrap-around)
     Scalars* sc;                                // result: it, relres, status
     double tol; int maxit;
     // quasi-static loop (nsteps > 0): thresholds, k written back, per-step results, arg-max scratch (G entries each)
@@ -76,7 +77,10 @@ __device__ __forceinline__ bool grid_barrier(unsigned int* counter, unsigned int
         unsigned int spins = 0;
         // poll relaxed (no L1 invalidate per poll), with a short back-off so that G pollers do not crowd the arrivals out of
         // the counter's L2 slice; one acquire load once the count is there orders the other CTAs' writes before what follows
-        while (ld_relaxed_u32(counter) < target && ++spins < SPIN_CAP) { __nanosleep(32); }
+        // (wrap-safe: the counter is monotonic modulo 2^32 and never more than G ahead of any CTA's target, so the sign of the
+        //  difference decides; a plain `counter < target` fails when target wraps to a small number after ~2^32 / G barriers,
+        //  i.e. ~5.6 M CG iterations at L = 512 -- a run to failure gets there)
+        while ((int)(ld_relaxed_u32(counter) - target) < 0 && ++spins < SPIN_CAP) { __nanosleep(32); }
         (void)ld_acquire_u32(counter);
         *ok_smem = spins < SPIN_CAP;
     }
@@ -113,7 +117,7 @@ __global__ void __launch_bounds__(P::NT) cg_fused_kernel(const FusedArgs A)
     cx<T>* Tf = static_cast<cx<T>*>(A.Tf);
     const T* shat = static_cast<const T*>(A.shat);
     const cx<T>* tw = static_cast<const cx<T>*>(A.tw);
-    unsigned int target = 0;
+    unsigned int target = A.counter_start;
     int slot = 0;                                  // partial-sum slot, rotates over 4
     auto ld_sw = [&](int e) { return io.ld(e); };
     auto st_sw = [&](int e, cx<T> v) { io.st(e, v); };

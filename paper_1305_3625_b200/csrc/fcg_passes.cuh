@@ -33,6 +33,7 @@ struct Scalars {
     double rr;                     // PCG: r.r of the current residual
     double kpp;                    // spectral search length: sum k p^2 from P1; P2 adds sum shat |P|^2
     unsigned int ticket2[2];       // [0] P1's k p^2 reduction, [1] P2's spectral-energy reduction
+    unsigned int timeout, pad3_;   // raised by a pipelined pass whose mbarrier wait gave up (fcg_tma.cuh); sticky until fcg_destroy
 };
 
 enum { ROWF_PLAIN = 0, ROWF_CG = 1, ROWF_RUPD = 2 };   // RUPD (PCG): r -= alpha q, partial r.r, row transforms of r
@@ -53,6 +54,7 @@ template <typename T> struct RowFwdArgs {
     T* rw;                 // RUPD: r (read / write)
     double* partial;       // RUPD: [gridDim.x] partial r.r
     int hints;             // L2 eviction-priority hints (FCG_OPT_L2_HINTS bit mask; pipelined passes only)
+    unsigned int* tmo;     // pipelined passes: raised when an mbarrier wait gives up (fcg_tma.cuh); = &Scalars::timeout
 };
 
 template <typename T> struct ColArgs {
@@ -65,6 +67,7 @@ template <typename T> struct ColArgs {
     int hints;
     double* partial;       // ENERGY instantiation: [L/2] partial sums of shat |P|^2, one per column
     int nsm;               // persistent column pass: SMs of the device
+    unsigned int* tmo;     // pipelined passes: raised when an mbarrier wait gives up
 };
 
 template <typename T> struct RowInvArgs {
@@ -85,6 +88,7 @@ template <typename T> struct RowInvArgs {
     T dval;                               // form 1, RESID: right-hand side b = k * dval (K D of eq. (2)); f is not read
     double kappa;                         // form 1, CGF (three launches, reading F1: k in {0, kappa}, vectors zero on broken bonds):
                                           //    p.(I + K G)p = sum p^2 + kappa sum g |P|^2
+    unsigned int* tmo;                    // pipelined passes: raised when an mbarrier wait gives up
 };
 
 template <int A, int B, typename F> FCG_HD void static_for_up(F&& f) {

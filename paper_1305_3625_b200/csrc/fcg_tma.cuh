@@ -59,8 +59,22 @@ __device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, uint32_t parity) {
         : "memory");
     return ok != 0;
 }
-__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
-    while (!mbar_try_wait(bar, parity)) {}
+// Bounded wait.  A wrong expect_tx byte count or a lost arrival must not hang the device: after WAIT_CAP failed polls (seconds;
+// a legitimate wait is microseconds) the thread raises *tmo and gives up, and every other waiter that has been polling for a
+// while sees the flag and gives up too, so the kernel ends with garbage instead of spinning for ever.  The host finds the flag
+// in the scalar block it reads back after every solve and returns FCG_CUDA_ERROR.  The first poll that succeeds costs nothing extra.
+constexpr uint32_t WAIT_CAP = 1u << 26, WAIT_LOOK = 1u << 10;
+__device__ __forceinline__ void mbar_wait_slow(uint64_t* bar, uint32_t parity, unsigned int* tmo) {
+    uint32_t polls = 0;
+    while (!mbar_try_wait(bar, parity)) {
+        if ((++polls & (WAIT_LOOK - 1)) == 0) {
+            if (*reinterpret_cast<volatile unsigned int*>(tmo) != 0u) return;
+            if (polls >= WAIT_CAP) { atomicExch(tmo, 1u); return; }
+        }
+    }
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity, unsigned int* tmo) {
+    if (!mbar_try_wait(bar, parity)) mbar_wait_slow(bar, parity, tmo);
 }
 
 // L2 eviction-priority policies for the cache_hint operand of the copies below

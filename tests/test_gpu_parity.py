@@ -182,9 +182,12 @@ def cg_parity(B, w, **opts):
         assert it2 == ref["iters"]
         d_pin = rel(u2.cpu().numpy(), ref["u"])
     assert min(d_nat, d_pin) <= TOL_CG[dt], (d_nat, d_pin, it, ref["iters"])
-    # the recurrence residual at the stop is rounding-sensitive (~0.2 % without broken sites, tens of
-    # percent with them while u still agrees to 1e-10), so it is only checked loosely; u above is the parity criterion
-    assert rr <= w.tol and abs(rr - ref["hist"][ref["iters"]]) <= 0.6 * ref["hist"][ref["iters"]] + 1e-15
+    # the recurrence residual is rounding-sensitive (~0.2 % without broken sites, up to 28 % with them
+    # while u still agrees to 1e-10), so it is only checked loosely, against the oracle's residual AT THE SAME COUNT
+    # (residuals of different iterations are different quantities); u above is the parity criterion
+    assert rr <= w.tol
+    if it <= ref["iters"]:
+        assert abs(rr - ref["hist"][it]) <= 0.5 * ref["hist"][it] + 1e-15, (it, ref["iters"], rr, ref["hist"][it])
     if dt == np.float64 and w.L <= 512:
         tight = orc.cg(w.s, w.k, w.f, w.u0, 1e-14, 10 * w.maxit)["u"]
         assert rel(u_nat, tight) <= 2.0 * rel(ref["u"], tight) + 1e-12
@@ -365,45 +368,90 @@ def test_column_pass_persistent_and_per_column(B, L, dt):
 
 
 # ------------------------------------------------------------------------------------ full-size configs
-@pytest.mark.parametrize("dt,count", [(np.float64, 100), (np.float32, 33)])
-def test_cg_config2_full_size(B, dt, count):
-    """L=2048 in the launch configuration bench.py times.  The oracle cannot run the whole solve in seconds, so:
-    (1) pinned-count comparison after 8 iterations, element by element; (2) the finished solve satisfies
-    ||f - A_oracle u||/||f|| <= 2 tol with ONE oracle operator application; (3) indicative iteration count."""
+@pytest.mark.parametrize("dt", [np.float64, np.float32])
+def test_cg_config2_full_size(B, dt):
+    """configs[2], L=2048, in the launch configuration bench.py times, against the ORACLE'S OWN full solve (natural stop;
+    about 10 s of host time per dtype): the whole cg_parity protocol -- status, |it - it_oracle| <= 2, u element by element
+    at the natural stops or at the oracle's count -- plus (1) a pinned-count comparison after 8 iterations at a tenth of
+    the tolerance and (2) ||f - A_oracle u||/||f|| <= 2 tol with one oracle operator application."""
     w = inputs.config(2, dt)
+    it, it_or = cg_parity(B, w)
     h = handle(B, w.L, dt, w.s)
     kd, fd = dev(w.k), dev(w.f)
     ref = orc.cg(w.s, w.k, w.f, w.u0, 0.0, 8, history=True)
     u = dev(w.u0)
-    it, rr, _ = h.fcg_solve(kd, fd, u, 0.0, 8)
-    assert it == 8 and rel(u.cpu().numpy(), ref["u"]) <= TOL_CG[dt] * 0.1
+    it8, rr, _ = h.fcg_solve(kd, fd, u, 0.0, 8)
+    assert it8 == 8 and rel(u.cpu().numpy(), ref["u"]) <= TOL_CG[dt] * 0.1
     assert abs(rr - ref["hist"][8]) <= 1e-3 * ref["hist"][8]
     u = dev(w.u0)
-    it, rr, st = h.fcg_solve(kd, fd, u, w.tol, w.maxit)
-    assert st == 0 and rr <= w.tol
-    assert abs(it - count) <= 2                            # BASELINE.md section 3, survey probe (not a paper number)
+    it2, rr, st = h.fcg_solve(kd, fd, u, w.tol, w.maxit)
+    assert st == 0 and rr <= w.tol and it2 == it
     uh = u.cpu().numpy()
     true_res = np.linalg.norm((w.f - orc.apply(w.s, w.k, uh)).astype(np.float64)) / np.linalg.norm(w.f.astype(np.float64))
     assert true_res <= 2 * w.tol
     h.close()
 
 
+def load_cfg4_golden():
+    """tests/golden/cfg4_oracle.txt, written by tests/golden/make_golden_cfg4.py from oracle/ only."""
+    path = os.path.join(GOLD, "cfg4_oracle.txt")
+    meta, hist = {}, None
+    with open(path) as fh:
+        for line in fh:
+            if line.startswith("# iters="):
+                meta = dict(kv.split("=") for kv in line[2:].split())
+            elif line.startswith("# hist "):
+                hist = np.array(line[7:].split(), np.float64)
+            elif not line.startswith("#"):
+                break
+    tab = np.loadtxt(path, comments="#")
+    return meta, hist, tab[:, 0].astype(np.int64), tab[:, 1].astype(np.float32), tab[:, 2].astype(np.float32)
+
+
 def test_cg_config4_full_size(B):
-    """L=8192 fp32 (largest config): pinned count 3 vs oracle + residual property with one oracle application."""
+    """configs[4], L=8192 fp32 (the largest config), against the oracle's stored full solve (its count, its residual history,
+    u at 4096 seeded sample sites after 20 iterations and at the stop; the oracle needs minutes for it, hence the file):
+      * pinned count 20 (SURVEY.md 8(d)): samples to 1e-5 (a tenth of the tolerance), ||u|| and the residual to 1e-3;
+      * natural stop: |it - it_oracle| <= 2 (north_star).  A larger difference is accepted only when the stored history
+        classifies it as a rounding flip of the stopping decision (SURVEY.md 8(c) P14 risk note): whichever side stopped later
+        was within 1 % of tol at the other side's stop, so both stops are first crossings of the same run up to rounding;
+      * u at the stop on the samples to 1e-4, at the natural stops if the counts agree, else re-run pinned at the oracle's count;
+      * ||f - A_oracle u||/||f|| <= 2 tol with one oracle operator application (a property that needs no stored value)."""
+    meta, hist, site, u_pin, u_stop = load_cfg4_golden()
+    it_or, pin = int(meta["iters"]), int(meta["pin"])
+    assert int(meta["status"]) == 0 and len(hist) == it_or + 1 and len(site) >= 4096
     w = inputs.config(4)
     h = handle(B, w.L, np.float32, w.s)
     kd, fd = dev(w.k), dev(w.f)
-    ref = orc.cg(w.s, w.k, w.f, w.u0, 0.0, 3, history=True)
+    sd = torch.from_numpy(site).cuda()
     u = dev(w.u0)
-    it, rr, _ = h.fcg_solve(kd, fd, u, 0.0, 3)
-    assert it == 3 and rel(u.cpu().numpy(), ref["u"]) <= 1e-5
-    assert abs(rr - ref["hist"][3]) <= 1e-3 * ref["hist"][3]
+    it, rr, _ = h.fcg_solve(kd, fd, u, 0.0, pin)
+    assert it == pin and rel(u.view(-1)[sd].cpu().numpy(), u_pin) <= 1e-5
+    assert abs(float(u.double().norm()) - float(meta["norm_u_pin"])) <= 1e-5 * float(meta["norm_u_pin"])
+    assert abs(rr - hist[pin]) <= 1e-3 * hist[pin]
     u = dev(w.u0)
     it, rr, st = h.fcg_solve(kd, fd, u, w.tol, w.maxit)
     assert st == 0 and rr <= w.tol
-    assert abs(it - 175) <= 6                              # survey probe 175; rough residual history near the stop (P14 risk note)
+    if abs(it - it_or) > 2:
+        if it < it_or:
+            assert hist[it] <= 1.01 * w.tol, (it, it_or, hist[it], hist[-6:])          # the oracle all but crossed where the GPU did
+        else:
+            u2 = dev(w.u0)
+            _, rr_at, _ = h.fcg_solve(kd, fd, u2, 0.0, it_or)
+            assert rr_at <= 1.01 * w.tol, (it, it_or, rr_at, hist[-6:])                 # the GPU all but crossed where the oracle did
     true_res = np.linalg.norm((w.f - orc.apply(w.s, w.k, u.cpu().numpy())).astype(np.float64)) / np.linalg.norm(w.f.astype(np.float64))
     assert true_res <= 2 * w.tol
+    d_nat = rel(u.view(-1)[sd].cpu().numpy(), u_stop)
+    d_pin = d_nat
+    if it != it_or and d_nat > TOL_CG[np.float32]:
+        u2 = dev(w.u0)
+        it2, _, _ = h.fcg_solve(kd, fd, u2, 0.0, it_or)
+        assert it2 == it_or
+        u = u2
+        d_pin = rel(u.view(-1)[sd].cpu().numpy(), u_stop)
+    assert min(d_nat, d_pin) <= TOL_CG[np.float32], (d_nat, d_pin, it, it_or)
+    if it == it_or or d_pin < d_nat:
+        assert abs(float(u.double().norm()) - float(meta["norm_u_stop"])) <= 1e-4 * float(meta["norm_u_stop"])
     h.close()
 
 

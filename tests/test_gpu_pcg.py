@@ -39,7 +39,9 @@ def pcg_parity(B, w, **opts):
         assert it2 == ref["iters"]
         d_pin = rel(u2.cpu().numpy(), ref["u"])
     assert min(d_nat, d_pin) <= TOL_CG[dt], (d_nat, d_pin, it, ref["iters"])
-    assert rr <= w.tol and abs(rr - ref["hist"][ref["iters"]]) <= 0.6 * ref["hist"][ref["iters"]] + 1e-15
+    assert rr <= w.tol
+    if it <= ref["iters"]:      # against the oracle's residual at the same count, loosely (rounding-sensitive)
+        assert abs(rr - ref["hist"][it]) <= 0.5 * ref["hist"][it] + 1e-15, (it, ref["iters"], rr, ref["hist"][it])
     # pinned count, element by element: a few iterations in, where nothing depends on the stopping decision
     npin = min(4, ref["iters"])
     refp = orc.pcg(w.s, w.k, w.f, w.u0, kbar, 0.0, npin, history=True)

@@ -1,0 +1,145 @@
+"""Robustness of the C ABI on the GPU (ADVICE r1 / VERDICT r1 "What's weak" 11-12): the wrap-around of the cooperative
+kernel's grid-barrier counter, the pending-loop guard of the _begin/_end pairs, argument checks, and a repeated-solve stress of
+the TMA rings (bitwise repeatability at every pipelined size x dtype: any ordering slip between a ring slot's reader and its
+refill shows up as a run-to-run difference)."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import api as orc
+from paper_1305_3625_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+TDT = {np.float64: torch.float64, np.float32: torch.float32}
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_1305_3625_b200 import binding
+    assert torch.cuda.is_available()
+    binding.lib()
+    return binding
+
+
+def dev(a, dt=None):
+    return torch.from_numpy(np.ascontiguousarray(a, dtype=dt or a.dtype)).cuda()
+
+
+@pytest.mark.parametrize("L", [256, 512])
+def test_grid_barrier_counter_wraps(B, L):
+    """The one-launch kernel's barrier counter is a 32-bit monotonic count; preset just below 2^32 it wraps within the first
+    iterations.  The solve and a short quasi-static loop must be bit-identical to the runs that start at 0 (and equal the oracle)."""
+    w = inputs.config(1, L=L)
+    ref = orc.cg(w.s, w.k, w.f, w.u0, w.tol, w.maxit)
+    outs = []
+    for start in (0, -3 * (L // 2) - 7, -1, -(1 << 31)):            # as unsigned: 0, 2^32 - 3G - 7, 2^32 - 1, 2^31
+        h = B.Fcg(L, torch.float64)
+        h.fcg_set_option(B.FCG_OPT_BARRIER_START, start)
+        h.fcg_set_spectrum(dev(w.s))
+        u = dev(w.u0)
+        it, rr, st = h.fcg_solve(dev(w.k), dev(w.f), u, w.tol, w.maxit)
+        assert st == 0 and h.fcg_last_launch_count() == 1, h.last_error()
+        outs.append((it, rr, u.cpu().numpy()))
+        h.close()
+    assert abs(outs[0][0] - ref["iters"]) <= 2
+    assert np.linalg.norm(outs[0][2] - ref["u"]) / np.linalg.norm(ref["u"]) <= 1e-9
+    for o in outs[1:]:
+        assert o[:2] == outs[0][:2] and np.array_equal(o[2], outs[0][2])
+    # the whole quasi-static loop in one launch (one more barrier per break step)
+    steps = 40
+    w3 = inputs.config(3, L=L, nsteps=steps)
+    res = []
+    for start in (0, -5 * (L // 2) - 1):
+        h = B.Fcg(L, torch.float64)
+        h.fcg_set_option(B.FCG_OPT_BARRIER_START, start)
+        h.fcg_set_spectrum(dev(w3.s))
+        kd, ud = dev(w3.k), dev(w3.u0)
+        index, iters, done, st = h.fcg_fracture(kd, dev(w3.f), ud, dev(w3.t), steps, w3.tol, w3.maxit)
+        assert done == steps and st == 0 and h.fcg_last_launch_count() == 1
+        res.append((index, iters, ud.cpu().numpy()))
+        h.close()
+    assert np.array_equal(res[0][0], res[1][0]) and np.array_equal(res[0][1], res[1][1]) and np.array_equal(res[0][2], res[1][2])
+
+
+def test_pending_loop_guard(B):
+    """Between _begin and _end every other call on the handle is refused (it would reuse the scalar block of the loop in
+    flight), a second _begin too, and the pending loop's results are untouched by the refused calls."""
+    L, steps = 256, 30
+    w = inputs.config(3, L=L, nsteps=steps)
+    h = B.Fcg(L, torch.float64)
+    h.fcg_set_spectrum(dev(w.s))
+    kd, fd, ud, td = dev(w.k), dev(w.f), dev(w.u0), dev(w.t)
+    index0, iters0, done0, st0 = h.fcg_fracture(kd, fd, ud, td, steps, w.tol, w.maxit)
+    kd, ud = dev(w.k), dev(w.u0)
+    h.fcg_fracture_begin(kd, fd, ud, td, steps, w.tol, w.maxit, 0)
+    k2, u2 = dev(w.k), dev(w.u0)
+    for call in (lambda: h.fcg_solve(k2, fd, u2, w.tol, w.maxit),
+                 lambda: h.fcg_break_step(k2, u2, td),
+                 lambda: h.fcg_apply(k2, fd),
+                 lambda: h.fcg_set_spectrum(dev(w.s)),
+                 lambda: h.fcg_fracture_begin(k2, fd, u2, td, steps, w.tol, w.maxit, 0)):
+        with pytest.raises(B.FcgError) as ei:
+            call()
+        assert ei.value.status == B.FCG_INVALID_ARG
+    index, iters, done, st = h.fcg_fracture_end()
+    assert done == steps and st == 0
+    assert np.array_equal(index, index0) and np.array_equal(iters, iters0)
+    it, rr, st = h.fcg_solve(k2, fd, u2, w.tol, w.maxit)              # the handle is usable again
+    assert st == 0
+    with pytest.raises(B.FcgError):
+        h.fcg_fracture_end()                                     # nothing pending
+    h.close()
+
+
+def test_solve_argument_checks(B):
+    L = 64
+    w = inputs.config(0)
+    h = B.Fcg(L, torch.float64)
+    h.fcg_set_spectrum(dev(w.s))
+    kd, fd, ud = dev(w.k), dev(w.f), dev(w.u0)
+    for args in ((kd, fd, kd), (kd, fd, fd)):                         # u aliases k / f
+        with pytest.raises(B.FcgError) as ei:
+            h.fcg_solve(*args, w.tol, w.maxit)
+        assert ei.value.status == B.FCG_INVALID_ARG
+    big = torch.zeros(L * L + 1, dtype=torch.float64, device="cuda")
+    off = big[1:].view(L, L)                                          # 8-byte aligned only
+    with pytest.raises(B.FcgError) as ei:
+        h.fcg_solve(kd, fd, off, w.tol, w.maxit)
+    assert ei.value.status == B.FCG_INVALID_ARG
+    assert h.fcg_solve(kd, fd, ud, w.tol, w.maxit)[2] == 0
+    h.close()
+
+
+@pytest.mark.parametrize("L", [256, 512, 1024, 2048, 4096, 8192])
+@pytest.mark.parametrize("dt", [np.float64, np.float32])
+def test_ring_stress_bitwise_repeatable(B, L, dt):
+    """Every pipelined size x dtype, graph and direct-launch modes, the three- and the four-launch iteration, PCG: REPS repeated
+    solves of a few iterations each must agree bit for bit (fcg_tma.cuh releases ring slots without a proxy fence where every
+    loaded value has been consumed; a slip there gives rare wrong strips -- ~1e-4 of the warps when it was seen in round 1)."""
+    if L == 8192 and dt == np.float64:
+        reps, its = 12, 3
+    else:
+        reps, its = (200, 3) if L <= 1024 else (60, 3) if L <= 2048 else (24, 3)
+    w = inputs.config(4 if L >= 4096 else 1, dt, L=L)
+    kd, fd, sd = dev(w.k), dev(w.f), dev(w.s)
+    kbar = inputs.precond_kbar(w.k)
+    for name, opts, pcg in (("cg3", {}, False), ("cg4", {"FCG_OPT_SPECTRAL_ALPHA": 0}, False), ("direct", {"FCG_OPT_LOOP_MODE": 1}, False),
+                            ("pcg", {}, True)):
+        h = B.Fcg(L, TDT[dt])
+        h.fcg_set_option(B.FCG_OPT_FUSED, 0)
+        for k_, v in opts.items():
+            h.fcg_set_option(getattr(B, k_), v)
+        h.fcg_set_spectrum(sd)
+        if pcg:
+            h.fcg_set_preconditioner(sd, kbar)
+        u = torch.zeros((L, L), dtype=TDT[dt], device="cuda")
+        ref = None
+        n = reps if name == "cg3" else max(reps // 4, 6)
+        for rep in range(n):
+            u.zero_()
+            r = (h.fcg_pcg_solve if pcg else h.fcg_solve)(kd, fd, u, 0.0, its)
+            if ref is None:
+                ref = (r, u.clone())
+            else:
+                assert r == ref[0] and torch.equal(u, ref[1]), (name, rep)
+        h.close()
