@@ -6,7 +6,8 @@ site-iterations/s at L=2048; achieved HBM GB/s vs peak).
 
 A "step" is one whole solve of the workload (set-up, CG loop to the configured tolerance, finish) through
 the C ABI.  Default workload: BASELINE.json configs[2], L=2048, fp64 (the size the metric is quoted on); the
-fp32 run of the same config and the L=8192 fp32 point are reported in "extra" when --full is given.
+fp32 run of the same config, the L=8192 fp32 point (configs[4]), the stand-alone transforms and the break step are measured in
+the same run and reported under "configs"; --full adds the quasi-static loops and the force formulation under "extra".
 Prints ONE JSON line (see DESIGN.md section 7 for every key).
 """
 from __future__ import annotations
@@ -197,36 +198,10 @@ def bench_workload(binding, torch, w, steps, warmup, profile_iters=20, e2e_steps
 
 
 def bench_extras(binding, torch, inputs):
-    """--full: the rest of north_star's list -- stand-alone transforms (GB/s on 4 N w bytes per transform), the break step, and
-    the quasi-static loop of configs[3] (all 2000 steps, CG and PCG solves, and ensembles; latency-bound: us per CG iteration and break steps per second are the figures)."""
+    """--full: the quasi-static loop of configs[3] (all 2000 steps, CG and PCG solves, and ensembles; latency-bound: us per CG
+    iteration and break steps per second are the figures) and the force formulation (bench_force)."""
     out = {}
     to = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
-    for L, dt, tdt in ((2048, np.float64, torch.float64), (2048, np.float32, torch.float32), (8192, np.float32, torch.float32)):
-        h = binding.Fcg(L, tdt)
-        x = to(inputs.fft_field(L).astype(dt))
-        X = h.fcg_fft_fwd(x); xb = h.fcg_fft_inv(X)
-        ev = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
-        torch.cuda.synchronize()
-        reps = 10
-        ev[0].record()
-        for _ in range(reps): h.fcg_fft_fwd(x, X)
-        ev[1].record()
-        for _ in range(reps): h.fcg_fft_inv(X, xb)
-        ev[2].record(); torch.cuda.synchronize()
-        nw = L * L * np.dtype(dt).itemsize
-        tf, ti = ev[0].elapsed_time(ev[1]) / reps, ev[1].elapsed_time(ev[2]) / reps
-        out[f"fft_L{L}_{'f64' if dt == np.float64 else 'f32'}"] = {"fwd_us": 1e3 * tf, "inv_us": 1e3 * ti, "fwd_gbs": 4 * nw / (tf * 1e-3) / 1e9,
-                                                                   "inv_gbs": 4 * nw / (ti * 1e-3) / 1e9,
-                                                                   "note": "row pass + column pass + layout kernel; bytes = 4 N w per transform"}
-        h.close()
-    w = inputs.config(2)
-    h = binding.Fcg(w.L, torch.float64)
-    k, u, t = to(w.k), to(inputs.fft_field(w.L)), to(inputs.thresholds(w.L))
-    h.fcg_break_step(k, u, t)
-    torch.cuda.synchronize(); t0 = time.perf_counter()
-    for _ in range(20): h.fcg_break_step(k, u, t)
-    out["break_step_L2048_f64"] = {"us_per_call_incl_host_sync": 1e6 * (time.perf_counter() - t0) / 20, "bytes": 3 * w.N * 8}
-    h.close()
     # quasi-static loop of configs[3], all 2000 steps in one cooperative launch: CG solves, PCG solves, and an ensemble of
     # independent samples (different threshold seeds) on several streams through fcg_fracture_begin / _end
     w3 = inputs.config(3)
@@ -384,6 +359,91 @@ def bench_force(binding, torch, inputs):
     return out
 
 
+def moved_nw():
+    """Bytes one CG iteration of this implementation moves, in units of N*w (DESIGN.md sections 4, 12)."""
+    return sum(PASS_NW.values())
+
+
+def bench_configs(binding, torch, inputs, hbm_peak):
+    """Default run, beside the headline: the other numbers north_star asks for, each measured here in a few solves / calls --
+    configs[2] in fp32, configs[4] (L = 8192 fp32, the HBM-bound point), the stand-alone transforms (GB/s on 4 N w bytes per
+    transform) and the break step (3 N w bytes).  Fractions are of the measured copy peak and of 8 TB/s nominal, on the bytes the
+    implementation moves (13.5 N w per iteration); the 16.5 N w survey model is given beside them as an equivalent rate."""
+    out = {}
+    to = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    for cfg, dt in ((2, np.float32), (4, np.float32)):
+        w2 = inputs.config(cfg, dt)
+        r2 = bench_workload(binding, torch, w2, 2, 1, profile_iters=10, e2e_steps=1)
+        nw2 = w2.N * w2.dtype.itemsize
+        t2 = 1e3 * (sum(r2["dev_ms"]) / len(r2["dev_ms"])) / r2["iters"][0]
+        gbs = moved_nw() * nw2 / (t2 * 1e-6) / 1e9
+        out[f"cfg{cfg}_L{w2.L}_f32"] = {
+            "iterations": r2["iters"][0], "status": r2["status"], "final_rel_residual": r2["relres"], "us_per_iteration": t2,
+            "iter_per_s": 1e6 / t2, "site_iter_per_s": 1e6 / t2 * w2.N,
+            "bytes_moved_per_iteration": moved_nw() * nw2, "iteration_gbs": gbs, "frac_of_measured_peak": gbs / hbm_peak,
+            "frac_of_8TBs_nominal": gbs / 8000.0, "equivalent_gbs_16p5_model": B_ITER_NW * nw2 / (t2 * 1e-6) / 1e9,
+            "kernel_us": {n: 1e3 * r2["kernel_ms"][n] for n in PASS_NAMES},
+            "kernel_gbs": {n: PASS_NW[n] * nw2 / (r2["kernel_ms"][n] * 1e-3) / 1e9 for n in PASS_NAMES},
+            "e2e_iter_per_s": r2["e2e_iter_s"]}
+        del w2, r2
+    for L, dt, tdt in ((2048, np.float64, torch.float64), (8192, np.float32, torch.float32)):
+        name = "f64" if dt == np.float64 else "f32"
+        nw = L * L * np.dtype(dt).itemsize
+        h = binding.Fcg(L, tdt)
+        x = to(inputs.fft_field(L).astype(dt))
+        X = h.fcg_fft_fwd(x); xb = h.fcg_fft_inv(X)
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+        torch.cuda.synchronize()
+        reps = 10
+        ev[0].record()
+        for _ in range(reps): h.fcg_fft_fwd(x, X)
+        ev[1].record()
+        for _ in range(reps): h.fcg_fft_inv(X, xb)
+        ev[2].record(); torch.cuda.synchronize()
+        tf, ti = ev[0].elapsed_time(ev[1]) / reps, ev[1].elapsed_time(ev[2]) / reps
+        out[f"fft_L{L}_{name}"] = {"fwd_us": 1e3 * tf, "inv_us": 1e3 * ti, "fwd_gbs": 4 * nw / (tf * 1e-3) / 1e9, "inv_gbs": 4 * nw / (ti * 1e-3) / 1e9,
+                                   "fwd_frac_of_measured_peak": 4 * nw / (tf * 1e-3) / 1e9 / hbm_peak,
+                                   "inv_frac_of_measured_peak": 4 * nw / (ti * 1e-3) / 1e9 / hbm_peak,
+                                   "round_trip_rel_l2": float((xb - x).norm() / x.norm()), "bytes_per_transform": 4 * nw}
+        # break step on the same handle: k, u, t resident; each call = one kernel + a 16-byte read-back and a stream sync
+        k = to((0.5 + np.random.default_rng(0).random((L, L))).astype(dt)); t = to(inputs.thresholds(L).astype(dt))
+        h.fcg_break_step(k, x, t)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize(); t0 = time.perf_counter(); e0.record()
+        for _ in range(10): h.fcg_break_step(k, x, t)
+        e1.record(); torch.cuda.synchronize()
+        us = 1e3 * e0.elapsed_time(e1) / 10
+        out[f"break_step_L{L}_{name}"] = {"us_per_call": us, "bytes": 3 * nw, "gbs": 3 * nw / (us * 1e-6) / 1e9,
+                                          "frac_of_measured_peak": 3 * nw / (us * 1e-6) / 1e9 / hbm_peak,
+                                          "note": "device time between events around 10 blocking calls: kernel + 16-byte read-back + host sync each"}
+        h.close()
+        del x, X, xb, k, t
+    torch.cuda.empty_cache()
+    return out
+
+
+def iteration_roofline(nw, t_iter_us, hbm_peak, peak_src, dram_iter):
+    """Whole iteration against the HBM roofline, on the bytes this implementation MOVES (13.5 N w with three launches, 15.5 with
+    four; DESIGN.md sections 4 and 12).  The 16.5 N w of SURVEY.md 8(d) -- the count for a design that stores and re-reads q -- is
+    kept beside it as an equivalent rate, labelled; dram_* are the bytes that really reach DRAM per iteration with warm caches
+    (single-pass ncu capture under profiles/), which at L = 2048 is well below the bytes moved because L2 serves T2."""
+    moved = moved_nw() * nw
+    ach = moved / (t_iter_us * 1e-6) / 1e9
+    eq = B_ITER_NW * nw / (t_iter_us * 1e-6) / 1e9
+    d = {"bound": "hbm", "bytes_per_iteration": moved, "bytes_per_iteration_Nw": moved_nw(), "achieved": ach, "peak": hbm_peak, "unit": "GB/s",
+         "frac": ach / hbm_peak, "frac_of_8TBs_nominal": ach / 8000.0, "peak_source": peak_src,
+         "floor_us_at_measured_peak": moved / (hbm_peak * 1e9) * 1e6,
+         "survey_model_16p5": {"bytes_per_iteration": B_ITER_NW * nw, "equivalent_gbs": eq, "frac": eq / hbm_peak, "frac_of_8TBs_nominal": eq / 8000.0,
+                               "note": "SURVEY.md 8(d) counts 16.5 N w for a design that stores q and reads p twice; this one does not, so this is an "
+                                       "equivalent rate, not bytes moved"},
+         "note": "time = whole solve / iterations (set-up and finish included)"}
+    if dram_iter is not None:
+        d["dram_bytes_per_iteration_warm"] = dram_iter
+        d["dram_gbs"] = dram_iter / (t_iter_us * 1e-6) / 1e9
+        d["dram_frac"] = d["dram_gbs"] / hbm_peak
+    return d
+
+
 def aggregate_over_ranks(dist, torch, step_ms, total_it, launches, e2e_iter_s, device):
     """Replicas only: whole-job time = MAX over ranks of the device time, whole-job work = SUM over ranks.
     `dist` is torch.distributed with an initialised group (nccl on the GPU box, gloo in the CPU test) or None for one rank."""
@@ -412,6 +472,7 @@ def main():
                     help="pcg: time fcg_pcg_solve instead (metric pcg_iterations_per_s, 22 N w bytes per iteration; no e2e leg) -- "
                          "for profiling the PCG kernels; the headline BASELINE.json names is the default")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-configs", action="store_true", help="skip the 'configs' block (configs[2] fp32, configs[4], transforms, break step)")
     ap.add_argument("--no-spectral-alpha", action="store_true",
                     help="four launches per iteration: p.Ap as a dot product after the last pass + a residual-update kernel")
     ap.add_argument("--no-pcg", action="store_true", help="skip the preconditioned-CG time-to-solution of the same workload ('pcg' key)")
@@ -529,6 +590,7 @@ def main():
     dom = max(PASS_NAMES, key=lambda n: kms[n])
     achieved = PASS_NW[dom] * nw / (kms[dom] * 1e-3) / 1e9
     traffic = traffic_warm = None
+    tj = {}
     tpath = os.path.join(ROOT, "profiles", "traffic.json")          # dram bytes per launch from the committed ncu --set full capture
     if os.path.exists(tpath):
         try:
@@ -537,6 +599,13 @@ def main():
             traffic_warm = tj.get(f"warm_L{w.L}_{args.dtype}", {}).get(dom)   # single-pass capture with warm caches (profiles/r1_warm_traffic.md)
         except Exception:
             traffic = traffic_warm = None
+    dram_iter = None                                                   # dram bytes per steady-state iteration (warm caches), all kernels
+    try:
+        tw = tj.get(f"warm_L{w.L}_{args.dtype}", {})
+        if all(n in tw for n in PASS_NAMES):
+            dram_iter = float(sum(tw[n] for n in PASS_NAMES))
+    except Exception:
+        dram_iter = None
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": step_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -548,13 +617,11 @@ def main():
                    "launches_per_iteration": len(PASS_NAMES)},
         "site_iterations_per_s": value * w.N,
         "us_per_iteration": t_iter_us,
-        "iteration_roofline": {"bound": "hbm", "bytes_per_iteration": B_ITER_NW * nw, "achieved": B_ITER_NW * nw / (t_iter_us * 1e-6) / 1e9,
-                               "peak": hbm_peak, "unit": "GB/s", "frac": B_ITER_NW * nw / (t_iter_us * 1e-6) / 1e9 / hbm_peak,
-                               "frac_of_8TBs_nominal": B_ITER_NW * nw / (t_iter_us * 1e-6) / 1e9 / 8000.0, "peak_source": peak_src,
-                               "note": "16.5*N*w model of SURVEY.md 8(d); time = whole solve / iterations"},
+        "iteration_roofline": iteration_roofline(nw, t_iter_us, hbm_peak, peak_src, dram_iter),
         "kernel_us": {n: 1e3 * kms[n] for n in PASS_NAMES},
         "kernel_gbs": {n: PASS_NW[n] * nw / (kms[n] * 1e-3) / 1e9 for n in PASS_NAMES},
         "roofline": {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": hbm_peak, "unit": "GB/s", "frac": achieved / hbm_peak,
+                     "frac_of_8TBs_nominal": achieved / 8000.0,
                      "traffic": traffic, "traffic_warm_caches": traffic_warm, "algorithmic_bytes_per_launch": PASS_NW[dom] * nw, "peak_source": peak_src},
         "e2e": {"value": res["e2e_iter_s"], "unit": UNIT, "h2d_bytes_per_step": res["h2d"], "d2h_bytes_per_step": res["d2h"]},
         "gpu_launches": launches,
@@ -563,18 +630,10 @@ def main():
     }
     if "pcg" in res:
         line["pcg"] = res["pcg"]
+    if world == 1 and not args.no_configs and args.config == 2 and args.dtype == "f64" and args.loop_mode == 0:
+        line["configs"] = bench_configs(binding, torch, inputs, hbm_peak)          # outside the timed region of the headline
     if args.full and world == 1:
-        extra = {}
-        for cfg, dt in ((2, np.float32), (4, np.float32)):
-            w2 = inputs.config(cfg, dt)
-            r2 = bench_workload(binding, torch, w2, max(2, args.steps // 3), 2, e2e_steps=1)
-            nw2 = w2.N * 4; t2 = 1e3 * (sum(r2["dev_ms"]) / len(r2["dev_ms"])) / r2["iters"][0]
-            extra[f"cfg{cfg}_L{w2.L}_f32"] = {"iterations": r2["iters"][0], "iter_per_s": 1e6 / t2, "site_iter_per_s": 1e6 / t2 * w2.N,
-                                               "us_per_iteration": t2, "iteration_gbs_16p5": B_ITER_NW * nw2 / (t2 * 1e-6) / 1e9,
-                                               "frac_of_measured_peak": B_ITER_NW * nw2 / (t2 * 1e-6) / 1e9 / hbm_peak,
-                                               "kernel_us": {n: 1e3 * r2["kernel_ms"][n] for n in PASS_NAMES}, "e2e_iter_per_s": r2["e2e_iter_s"]}
-        extra.update(bench_extras(binding, torch, inputs))
-        line["extra"] = extra
+        line["extra"] = bench_extras(binding, torch, inputs)
     if not args.no_cpu_baseline and world == 1:
         n_cpu = args.cpu_baseline_iters
         if n_cpu is None:                                  # bounded sample: about 12 s of host work, at least 8 iterations

@@ -12,7 +12,7 @@ import os
 import torch
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libfcg.so")
+LIB_PATH = os.environ.get("FCG_LIB") or os.path.join(_HERE, "libfcg.so")      # FCG_LIB: a variant build for A/B measurements
 
 FCG_F32, FCG_F64 = 0, 1
 FCG_OK, FCG_NOT_CONVERGED = 0, 1

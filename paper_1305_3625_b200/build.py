@@ -12,8 +12,10 @@ import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
-OBJ = os.path.join(HERE, "build")
-LIB = os.path.join(HERE, "libfcg.so")
+# FCG_BUILD_DIR / FCG_LIB_OUT: build a variant (e.g. with FCG_EXTRA_FLAGS=-D...) beside the product for A/B measurements;
+# the binding loads it when FCG_LIB names it.  The defaults are the product.
+OBJ = os.environ.get("FCG_BUILD_DIR") or os.path.join(HERE, "build")
+LIB = os.environ.get("FCG_LIB_OUT") or os.path.join(HERE, "libfcg.so")
 SIZES = [16, 32, 64, 128, 256, 512, 1024, 2048, 4096, 8192]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",

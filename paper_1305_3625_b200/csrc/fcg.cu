@@ -771,7 +771,11 @@ int fcg_set_option(fcg_handle h, int option, int value) {
             h->row_var_opt = value; return FCG_OK;
         case FCG_OPT_FUSED: if (value != 0 && value != 1) return fail(h, FCG_INVALID_ARG, "fused must be 0 or 1"); h->fused_opt = value; return FCG_OK;
         case FCG_OPT_PDL: if (value != 0 && value != 1) return fail(h, FCG_INVALID_ARG, "pdl must be 0 or 1"); h->pdl = value; return FCG_OK;
+#ifdef FCG_PROBE
+        case FCG_OPT_L2_HINTS: h->hints = value; return FCG_OK;      // measurement build: the probe bits of fcg_async.cuh too
+#else
         case FCG_OPT_L2_HINTS: if (value < 0 || value > 255) return fail(h, FCG_INVALID_ARG, "hints must be 0..255"); h->hints = value; return FCG_OK;
+#endif
         case FCG_OPT_SPECTRAL_ALPHA: if (value != 0 && value != 1) return fail(h, FCG_INVALID_ARG, "spectral alpha must be 0 or 1"); h->sl_opt = value; return FCG_OK;
         case FCG_OPT_COL_PERSISTENT: if (value < -1 || value > 1) return fail(h, FCG_INVALID_ARG, "col persistent must be -1, 0 or 1"); h->colp_opt = value; return FCG_OK;
         case FCG_OPT_BARRIER_START: h->barrier_start = (unsigned int)value; return FCG_OK;

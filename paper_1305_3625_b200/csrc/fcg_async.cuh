@@ -109,6 +109,28 @@ __device__ __forceinline__ void store_pair_hint(float2* dst, float2 a, float2 b,
 // CTA barrier among the first N threads only (the consumers of a warp-specialised kernel); barrier 0 stays __syncthreads
 template <int N> __device__ __forceinline__ void bar_named() { asm volatile("bar.sync 1, %0;" ::"n"(N) : "memory"); }
 
+// Grouped butterfly assignment in the stages >= 2 of the pipelined passes (fcg_engine.cuh, Grp), built with -DFCG_GROUPS.  Correct
+// (parity green) but not faster: measured L = 2048 fp64 93.7 vs 94.2 us per iteration, and slower where it costs registers
+// (L = 8192 fp32 826 vs 798 us, L = 4096 fp64 379 vs 369 us) -- the stage barriers are not what these kernels wait for.  Default:
+// the cyclic assignment with a CTA barrier after every stage.
+#ifdef FCG_GROUPS
+constexpr bool GRP = true;
+#else
+constexpr bool GRP = false;
+#endif
+// Elimination runs (-DFCG_PROBE, measurement builds only; results are then wrong): bits of ColArgs/RowInvArgs/RowFwdArgs::hints
+//   0x100 column pass without its stages   0x200 without its gather   0x400 without its scatter
+//   0x800 last pass without its shared-memory stages   0x1000 first pass without them
+#ifdef FCG_PROBE
+#define FCG_PROBE_ON(bit) ((A.hints & (bit)) != 0)
+#else
+#define FCG_PROBE_ON(bit) false
+#endif
+// after a stage >= 2: only the threads that share my sub-blocks (GRP), else all NT consumers
+template <typename P, int NT> __device__ __forceinline__ void stage_sync(int lt) {
+    if constexpr (GRP) group_sync<P>(lt); else asm volatile("bar.sync 1, %0;" ::"n"(NT) : "memory");
+}
+
 template <typename P> constexpr int per_max() {
     int m = 1;
     for (int s = 1; s <= P::S; ++s) { const int per = (P::N / P::radix(s)) / P::NT; if (per > m) m = per; }
@@ -195,7 +217,7 @@ __global__ void __launch_bounds__(P::NT + 32, CTAS) row_fwd2_kernel(const RowFwd
     const uint64_t pol_u = (A.hints & 2) ? tma::policy_evict_first() : tma::policy_evict_normal();   // L2 hints (bit 1): the u stores
     const uint64_t pol_t2 = (A.hints & 64) ? tma::policy_evict_last() : tma::policy_evict_normal(); // (bit 6): T2 is read back by the next two passes
     cx<T> wb[S + 1][PM];
-    static_for_up<1, S - 1>([&](auto s) { base_tw<P, decltype(s)::value, T>(lt, A.tw, wb[decltype(s)::value]); });
+    static_for_up<1, S - 1>([&](auto s) { base_tw<P, decltype(s)::value, T, GRP>(lt, A.tw, wb[decltype(s)::value]); });
 
     int slot = 0;
     uint32_t phase = 0;
@@ -242,13 +264,15 @@ __global__ void __launch_bounds__(P::NT + 32, CTAS) row_fwd2_kernel(const RowFwd
         stage_math<P, 1, -1, T, true>(z, wb[1]);
         stage_st<P, 1, T>(lt, [&](int e, cx<T> v) { io.st(e, v); }, z);
         bar_named<NT>();
+        if (!FCG_PROBE_ON(0x1000))
         static_for_up<2, S>([&](auto s) {
             constexpr int sv = decltype(s)::value;
             cx<T> a[St<P, sv>::PER][St<P, sv>::R];
-            stage_ld<P, sv, T>(lt, [&](int e) { return io.ld(e); }, a);
+            stage_ld<P, sv, T, GRP>(lt, [&](int e) { return io.ld(e); }, a);
             stage_math<P, sv, -1, T, true>(a, wb[sv]);
-            stage_st<P, sv, T>(lt, [&](int e, cx<T> v) { io.st(e, v); }, a);
-            bar_named<NT>();
+            stage_st<P, sv, T, GRP>(lt, [&](int e, cx<T> v) { io.st(e, v); }, a);
+            if constexpr (sv == S) bar_named<NT>();           // the separation below reads Z[n] and Z[L - n]: everybody's
+            else stage_sync<P, NT>(lt);
         });
         // Separate the two rows and store them as column m of T2 (X_even[n], X_odd[n] side by side).  Consecutive
         // threads take consecutive POSITIONS e of the digit-reversed spectrum (n = freq_of(e), n < L/2 <=> the last
@@ -308,9 +332,9 @@ __global__ void __launch_bounds__(P::NT, CTAS) col2_kernel(const ColArgs<T> A, c
         tma::fence_mbar_init();
     }
     cx<T> wb[S + 1][PM];
-    static_for_up<1, S - 1>([&](auto s) { base_tw<P, decltype(s)::value, T>(lt, A.tw, wb[decltype(s)::value]); });
+    static_for_up<1, S - 1>([&](auto s) { base_tw<P, decltype(s)::value, T, GRP>(lt, A.tw, wb[decltype(s)::value]); });
     tma::grid_dep_wait();                                         // everything above overlaps the previous kernel's tail
-    if (lt == 0) {
+    if (lt == 0 && !FCG_PROBE_ON(0x200)) {
         tma::mbar_expect_tx(&bar, (uint32_t)(AS::WBYTES + (n ? L * sizeof(T) : 0)));
 #pragma unroll
         for (int b = 0; b < (L / 2) / ABOX; ++b)
@@ -320,28 +344,31 @@ __global__ void __launch_bounds__(P::NT, CTAS) col2_kernel(const ColArgs<T> A, c
     }
     __syncthreads();
     const bool done = A.sc && A.sc->done;
-    tma::mbar_wait(&bar, 0, A.tmo);
+    if (!FCG_PROBE_ON(0x200)) tma::mbar_wait(&bar, 0, A.tmo);
     if (done) return;
     double energy = 0.0;
 
     auto ld_sw = [&](int e) { return io.ld(e); };
     auto st_sw = [&](int e, cx<T> v) { io.st(e, v); };
+    // stages >= 2: grouped assignment, only the group synchronises (fcg_engine.cuh); a CTA barrier where all sub-blocks meet --
+    // before the packed column's pair loop (after forward stage S) and before inverse stage 1 (after inverse stage 2)
     auto fwd_smem_stage = [&](auto s) {
         constexpr int sv = decltype(s)::value;
         cx<T> a[St<P, sv>::PER][St<P, sv>::R];
-        stage_ld<P, sv, T>(lt, ld_sw, a);
+        stage_ld<P, sv, T, GRP>(lt, ld_sw, a);
         stage_math<P, sv, -1, T>(a, wb[sv]);
-        stage_st<P, sv, T>(lt, st_sw, a);
-        __syncthreads();
+        stage_st<P, sv, T, GRP>(lt, st_sw, a);
+        if constexpr (sv == S) __syncthreads(); else stage_sync<P, NT>(lt);
     };
     auto inv_smem_stage = [&](auto s) {
         constexpr int sv = decltype(s)::value;
         cx<T> a[St<P, sv>::PER][St<P, sv>::R];
-        stage_ld<P, sv, T>(lt, ld_sw, a);
+        stage_ld<P, sv, T, GRP>(lt, ld_sw, a);
         stage_math<P, sv, +1, T>(a, wb[sv]);
-        stage_st<P, sv, T>(lt, st_sw, a);
-        __syncthreads();
+        stage_st<P, sv, T, GRP>(lt, st_sw, a);
+        if constexpr (sv == 2) __syncthreads(); else stage_sync<P, NT>(lt);
     };
+    if (!FCG_PROBE_ON(0x100)) {
     {   // forward stage 1: the column arrived in natural (linear) order; it leaves the stage swizzled
         cx<T> a[St<P, 1>::PER][St<P, 1>::R];
         stage_ld<P, 1, T>(lt, [&](int e) { return W[e]; }, a);
@@ -354,12 +381,12 @@ __global__ void __launch_bounds__(P::NT, CTAS) col2_kernel(const ColArgs<T> A, c
         static_for_up<2, S - 1>(fwd_smem_stage);
         // last forward stage * shat * first inverse stage, in registers
         if constexpr (ENERGY) {
-            run_middle<P, T, true>(lt, ld_sw, st_sw, [&](int g, int u) { return sh[u * (L / P::RLAST) + g]; }, &energy);
+            run_middle<P, T, true, GRP>(lt, ld_sw, st_sw, [&](int g, int u) { return sh[u * (L / P::RLAST) + g]; }, &energy);
             energy *= 2.0;                                       // column n stands for n and L - n
         } else {
-            run_middle<P, T>(lt, ld_sw, st_sw, [&](int g, int u) { return sh[u * (L / P::RLAST) + g]; });
+            run_middle<P, T, false, GRP>(lt, ld_sw, st_sw, [&](int g, int u) { return sh[u * (L / P::RLAST) + g]; });
         }
-        __syncthreads();
+        if constexpr (S - 1 >= 2) stage_sync<P, NT>(lt); else __syncthreads();
         static_for_down<S - 1, 2>(inv_smem_stage);
     } else {
         // packed column: W = Y0 + i YN.  W'[m] = sp[m] W[m] + sm[m] conj W[-m], sp = (s0+sN)/2 (row 0 of shat),
@@ -395,13 +422,16 @@ __global__ void __launch_bounds__(P::NT, CTAS) col2_kernel(const ColArgs<T> A, c
         __syncthreads();
         stage_st<P, 1, T>(lt, [&](int e, cx<T> v) { W[e] = v; }, a);
     }
+    }
     tma::fence_proxy_async();                 // my writes -> visible to the async proxy
     tma::mbar_warp_arrive(&ready);
     if (lt == 0) {
         tma::mbar_wait(&ready, 0, A.tmo);            // every warp's part of the column is in place
+        if (!FCG_PROBE_ON(0x400)) {
 #pragma unroll
         for (int b = 0; b < (L / 2) / ABOX; ++b)
             tma::tensor_s2g_4d(&tmap, 0, n % AS::NB, b * ABOX, n / AS::NB, smem_raw + (size_t)b * BOXB);
+        }
         tma::bulk_commit();
     }
     if constexpr (ENERGY) {      // this column's share of sum shat |P|^2, while the scatter drains; the next pass adds the L/2 shares
@@ -462,6 +492,7 @@ __global__ void __launch_bounds__(P::NT + 32, CTAS) col2p_kernel(const ColArgs<T
             auto gather = [&](int i) {
                 const int n = col_of(i), b = i & 1;
                 unsigned char* Wb = smem_raw + (size_t)b * CP::BUF;
+                if (FCG_PROBE_ON(0x200)) { tma::mbar_arrive(&full[b]); return; }
                 tma::mbar_expect_tx(&full[b], (uint32_t)(AS::WBYTES + (n ? L * sizeof(T) : 0)));
 #pragma unroll
                 for (int q = 0; q < (L / 2) / ABOX; ++q)
@@ -474,9 +505,11 @@ __global__ void __launch_bounds__(P::NT + 32, CTAS) col2p_kernel(const ColArgs<T
                 const int n = col_of(i), b = i & 1;
                 unsigned char* Wb = smem_raw + (size_t)b * CP::BUF;
                 tma::mbar_wait(&ready[b], (uint32_t)((i >> 1) & 1), A.tmo);          // every consumer warp's part of column i is in place
+                if (!FCG_PROBE_ON(0x400)) {
 #pragma unroll
                 for (int q = 0; q < (L / 2) / ABOX; ++q)
                     tma::tensor_s2g_4d(&tmap, 0, n % AS::NB, q * ABOX, n / AS::NB, Wb + (size_t)q * BOXB);
+                }
                 tma::bulk_commit();
                 tma::bulk_wait_read0();                                        // the buffer may be refilled (or the CTA may exit)
                 if (i + 2 < cnt) gather(i + 2);
@@ -487,7 +520,7 @@ __global__ void __launch_bounds__(P::NT + 32, CTAS) col2p_kernel(const ColArgs<T
 
     // ---- consumers
     cx<T> wb[S + 1][PM];
-    static_for_up<1, S - 1>([&](auto s) { base_tw<P, decltype(s)::value, T>(lt, A.tw, wb[decltype(s)::value]); });
+    static_for_up<1, S - 1>([&](auto s) { base_tw<P, decltype(s)::value, T, GRP>(lt, A.tw, wb[decltype(s)::value]); });
     for (int i = 0; i < cnt; ++i) {
         const int n = col_of(i), b = i & 1;
         cx<T>* W = reinterpret_cast<cx<T>*>(smem_raw + (size_t)b * CP::BUF);
@@ -497,22 +530,23 @@ __global__ void __launch_bounds__(P::NT + 32, CTAS) col2p_kernel(const ColArgs<T
         tma::mbar_wait(&full[b], (uint32_t)((i >> 1) & 1), A.tmo);
         auto ld_sw = [&](int e) { return io.ld(e); };
         auto st_sw = [&](int e, cx<T> v) { io.st(e, v); };
-        auto fwd_smem_stage = [&](auto s) {
+        auto fwd_smem_stage = [&](auto s) {              // (grouped stages and their barriers: see col2_kernel)
             constexpr int sv = decltype(s)::value;
             cx<T> a[St<P, sv>::PER][St<P, sv>::R];
-            stage_ld<P, sv, T>(lt, ld_sw, a);
+            stage_ld<P, sv, T, GRP>(lt, ld_sw, a);
             stage_math<P, sv, -1, T>(a, wb[sv]);
-            stage_st<P, sv, T>(lt, st_sw, a);
-            bar_named<NT>();
+            stage_st<P, sv, T, GRP>(lt, st_sw, a);
+            if constexpr (sv == S) bar_named<NT>(); else stage_sync<P, NT>(lt);
         };
         auto inv_smem_stage = [&](auto s) {
             constexpr int sv = decltype(s)::value;
             cx<T> a[St<P, sv>::PER][St<P, sv>::R];
-            stage_ld<P, sv, T>(lt, ld_sw, a);
+            stage_ld<P, sv, T, GRP>(lt, ld_sw, a);
             stage_math<P, sv, +1, T>(a, wb[sv]);
-            stage_st<P, sv, T>(lt, st_sw, a);
-            bar_named<NT>();
+            stage_st<P, sv, T, GRP>(lt, st_sw, a);
+            if constexpr (sv == 2) bar_named<NT>(); else stage_sync<P, NT>(lt);
         };
+        if (!FCG_PROBE_ON(0x100)) {
         {   // forward stage 1: the column arrived in natural (linear) order; it leaves the stage swizzled
             cx<T> a[St<P, 1>::PER][St<P, 1>::R];
             stage_ld<P, 1, T>(lt, [&](int e) { return W[e]; }, a);
@@ -524,12 +558,12 @@ __global__ void __launch_bounds__(P::NT + 32, CTAS) col2p_kernel(const ColArgs<T
         if (n != 0) {
             static_for_up<2, S - 1>(fwd_smem_stage);
             if constexpr (ENERGY) {
-                run_middle<P, T, true>(lt, ld_sw, st_sw, [&](int g, int u) { return sh[u * (L / P::RLAST) + g]; }, &energy);
+                run_middle<P, T, true, GRP>(lt, ld_sw, st_sw, [&](int g, int u) { return sh[u * (L / P::RLAST) + g]; }, &energy);
                 energy *= 2.0;
             } else {
-                run_middle<P, T>(lt, ld_sw, st_sw, [&](int g, int u) { return sh[u * (L / P::RLAST) + g]; });
+                run_middle<P, T, false, GRP>(lt, ld_sw, st_sw, [&](int g, int u) { return sh[u * (L / P::RLAST) + g]; });
             }
-            bar_named<NT>();
+            if constexpr (S - 1 >= 2) stage_sync<P, NT>(lt); else bar_named<NT>();
             static_for_down<S - 1, 2>(inv_smem_stage);
         } else {         // packed n = 0 / L/2 column, see col2_kernel
             static_for_up<2, S>(fwd_smem_stage);
@@ -561,6 +595,7 @@ __global__ void __launch_bounds__(P::NT + 32, CTAS) col2p_kernel(const ColArgs<T
             stage_math<P, 1, +1, T>(a, wb[1]);
             bar_named<NT>();
             stage_st<P, 1, T>(lt, [&](int e, cx<T> v) { W[e] = v; }, a);
+        }
         }
         tma::fence_proxy_async();                 // my writes -> visible to the async proxy
         tma::mbar_warp_arrive(&ready[b]);
@@ -865,7 +900,7 @@ __global__ void __launch_bounds__(AsyncShape<T, P>::INV_THREADS, CTAS) row_inv2_
         }
         // ---- consumers
         cx<T> wb[S + 1][PM];
-        static_for_up<1, S - 1>([&](auto s) { base_tw<P, decltype(s)::value, T>(lt, A.tw, wb[decltype(s)::value]); });
+        static_for_up<1, S - 1>([&](auto s) { base_tw<P, decltype(s)::value, T, GRP>(lt, A.tw, wb[decltype(s)::value]); });
         int ts = 0, ks = 0;
         uint32_t tph = 0, kph = 0;
         for (int i = 0; i < ntl; ++i) {
@@ -893,13 +928,15 @@ __global__ void __launch_bounds__(AsyncShape<T, P>::INV_THREADS, CTAS) row_inv2_
                 if (++ts == NTS) { ts = 0; tph ^= 1u; }
             }
             bar_named<NT>();                                          // Z complete in W
+            if (!FCG_PROBE_ON(0x800))
             static_for_down<S, 2>([&](auto s) {
                 constexpr int sv = decltype(s)::value;
                 cx<T> a[St<P, sv>::PER][St<P, sv>::R];
-                stage_ld<P, sv, T>(lt, [&](int e) { return io.ld(e); }, a);
+                stage_ld<P, sv, T, GRP>(lt, [&](int e) { return io.ld(e); }, a);
                 stage_math<P, sv, +1, T>(a, wb[sv]);
-                stage_st<P, sv, T>(lt, [&](int e, cx<T> v) { io.st(e, v); }, a);
-                bar_named<NT>();
+                stage_st<P, sv, T, GRP>(lt, [&](int e, cx<T> v) { io.st(e, v); }, a);
+                if constexpr (sv == 2) bar_named<NT>();           // stage 1 joins the sub-blocks: everybody's
+                else stage_sync<P, NT>(lt);
             });
             // inverse stage 1 straight into the epilogue: natural order, re = even row, im = odd row
             cx<T> c[PER1][R1];

@@ -49,12 +49,45 @@ FCG_HD void run_stage(int lt, const cx<T>* __restrict__ tw, LD ld, ST st)
     }
 }
 
+template <typename P, int s> struct St {
+    static constexpr int R = P::radix(s), M = P::mlen(s), Q = M / R, NB = P::N / R, PER = NB / P::NT, TWO = P::tw_off(s);
+    static_assert(PER >= 1, "plan: NT too large for this radix");
+};
+
+// Which butterflies a thread owns.  Natural: g = lt + i NT (cyclic over the CTA's threads), which makes every stage depend on
+// every thread of the previous one: a CTA barrier after each stage.  But after stage 1 a decimation-in-frequency transform
+// falls apart into R1 independent sub-transforms of length N / R1 (and the adjoint inverse only joins them again in its last
+// stage, stage 1), so the stages 2 .. S need no exchange between threads that own different sub-blocks.  GROUPED assignment:
+// the NT threads form G groups of TPG consecutive threads (whole warps); group j owns the sub-blocks [j R1/G, (j+1) R1/G) in
+// EVERY stage >= 2, i.e. the contiguous butterfly range [j PER TPG, (j+1) PER TPG) of each stage, dealt cyclically inside the
+// group.  A warp instruction still covers 32 consecutive butterflies (same shared-memory bank behaviour), and between two
+// stages >= 2 only the group has to synchronise: __syncwarp() where a group is one warp (every plan but L = 8192), a named
+// barrier of TPG threads otherwise.  The groups of a CTA drift apart, so one group's shared-memory phase overlaps another's
+// arithmetic -- with CTA barriers all warps alternate between the two in lock-step.
+template <typename P> struct Grp {
+    static constexpr int G_ = P::NT / 32 < P::R1 ? P::NT / 32 : P::R1;
+    static constexpr int G = G_ < 1 ? 1 : G_;
+    static constexpr int TPG = P::NT / G;
+    static_assert(P::NT % G == 0 && P::R1 % G == 0, "groups must divide the threads and the stage-2 sub-blocks");
+};
+template <typename P, int s, bool GR> FCG_HD int bfly(int lt, int i) {
+    if constexpr (!GR || s == 1) return lt + i * P::NT;
+    else return (lt / Grp<P>::TPG) * (St<P, s>::PER * Grp<P>::TPG) + lt % Grp<P>::TPG + i * Grp<P>::TPG;
+}
+#ifdef __CUDACC__
+// synchronise the threads that share sub-blocks with me (all of them call this): between two stages >= 2 of a GROUPED transform
+template <typename P> __device__ __forceinline__ void group_sync(int lt) {
+    if constexpr (Grp<P>::TPG == 32) __syncwarp();
+    else asm volatile("bar.sync %0, %1;" ::"r"(2 + lt / Grp<P>::TPG), "n"(Grp<P>::TPG) : "memory");
+}
+#endif
+
 // Last forward stage, a pointwise real multiply, and the first inverse stage, all in registers:
 //   a <- DFT_R(a);  a[u] *= mul(e_u);  a <- DFT_R^H(a)
 // (the last stage has Q = 1, so no twiddles are involved).  mul(g, u) returns the real factor for position g*R + u.
 // ENERGY: *energy += sum of mul * |a|^2 over this thread's elements after the forward stage: the R products of one butterfly
 // are summed in the working precision, the butterflies' sums in double.
-template <typename P, typename T, bool ENERGY = false, typename LD, typename ST, typename MUL>
+template <typename P, typename T, bool ENERGY = false, bool GR = false, typename LD, typename ST, typename MUL>
 FCG_HD void run_middle(int lt, LD ld, ST st, MUL mul, double* energy = nullptr)
 {
     constexpr int R = P::RLAST;
@@ -62,7 +95,8 @@ FCG_HD void run_middle(int lt, LD ld, ST st, MUL mul, double* energy = nullptr)
     constexpr int PER = NB / P::NT;
 #pragma unroll
     for (int i = 0; i < PER; ++i) {
-        const int base = (lt + i * P::NT) * R;
+        const int g = bfly<P, P::S, GR>(lt, i);
+        const int base = g * R;
         cx<T> a[R];
 #pragma unroll
         for (int t = 0; t < R; ++t) a[t] = ld(base + t);
@@ -74,7 +108,7 @@ FCG_HD void run_middle(int lt, LD ld, ST st, MUL mul, double* energy = nullptr)
 #endif
 #pragma unroll
         for (int u = 0; u < R; ++u) {
-            const T sv = mul(lt + i * P::NT, u);
+            const T sv = mul(g, u);
 #ifdef FCG_ENERGY_WIDE
             if constexpr (ENERGY) e += (double)sv * ((double)a[u].x * (double)a[u].x + (double)a[u].y * (double)a[u].y);
 #else
@@ -94,11 +128,6 @@ FCG_HD void run_middle(int lt, LD ld, ST st, MUL mul, double* energy = nullptr)
 // can be placed between the steps.  Twiddles are not read from the [u][j] tables: each thread keeps the base
 // twiddle w = w_M^j of each of its butterflies (one table entry, fetched once at kernel start) and forms the
 // powers w^2 .. w^(R-1) by a product tree (apply_twiddles, error <= ~4 ulp), which costs no memory traffic.
-template <typename P, int s> struct St {
-    static constexpr int R = P::radix(s), M = P::mlen(s), Q = M / R, NB = P::N / R, PER = NB / P::NT, TWO = P::tw_off(s);
-    static_assert(PER >= 1, "plan: NT too large for this radix");
-};
-
 // a[u] *= w^u (CONJ: conj(w)^u), u = 1 .. R-1.  Two ways to form the powers, chosen per kernel by measurement (it is a
 // register-allocation matter: row_fwd2 at L=2048 fp64 runs 39 us with CHAIN and 44 us with the tree, row_inv2 36 vs 39):
 //   tree : w^u = w^(u/2) w^(u - u/2), depth log2 R products (error <= ~4 ulp), all powers live at once;
@@ -139,31 +168,31 @@ template <int R, bool CONJ, bool CHAIN, typename C> FCG_HD void apply_twiddles(C
 }
 
 // base twiddles of this thread's butterflies in stage s (u = 1 row of the stage's table)
-template <typename P, int s, typename T> FCG_HD void base_tw(int lt, const cx<T>* __restrict__ tw, cx<T>* w) {
+template <typename P, int s, typename T, bool GR = false> FCG_HD void base_tw(int lt, const cx<T>* __restrict__ tw, cx<T>* w) {
     using I = St<P, s>;
     if constexpr (I::Q > 1) {
 #pragma unroll
-        for (int i = 0; i < I::PER; ++i) w[i] = tw[I::TWO + (lt + i * P::NT) % I::Q];
+        for (int i = 0; i < I::PER; ++i) w[i] = tw[I::TWO + bfly<P, s, GR>(lt, i) % I::Q];
     }
 }
 
-template <typename P, int s, typename T, typename LD>
+template <typename P, int s, typename T, bool GR = false, typename LD>
 FCG_HD void stage_ld(int lt, LD ld, cx<T> (&a)[St<P, s>::PER][St<P, s>::R]) {
     using I = St<P, s>;
 #pragma unroll
     for (int i = 0; i < I::PER; ++i) {
-        const int g = lt + i * P::NT;
+        const int g = bfly<P, s, GR>(lt, i);
         const int base = (g / I::Q) * I::M + g % I::Q;
 #pragma unroll
         for (int t = 0; t < I::R; ++t) a[i][t] = ld(base + t * I::Q);
     }
 }
-template <typename P, int s, typename T, typename ST>
+template <typename P, int s, typename T, bool GR = false, typename ST>
 FCG_HD void stage_st(int lt, ST st, const cx<T> (&a)[St<P, s>::PER][St<P, s>::R]) {
     using I = St<P, s>;
 #pragma unroll
     for (int i = 0; i < I::PER; ++i) {
-        const int g = lt + i * P::NT;
+        const int g = bfly<P, s, GR>(lt, i);
         const int base = (g / I::Q) * I::M + g % I::Q;
 #pragma unroll
         for (int t = 0; t < I::R; ++t) st(base + t * I::Q, a[i][t]);

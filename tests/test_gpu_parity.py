@@ -408,27 +408,49 @@ def load_cfg4_golden():
     return meta, hist, tab[:, 0].astype(np.int64), tab[:, 1].astype(np.float32), tab[:, 2].astype(np.float32)
 
 
+def load_cfg4_drift():
+    """tests/golden/cfg4_indep.txt (make_golden_cfg4.py --indep): the same workload by a second CPU implementation (textbook CG
+    around scipy's float32 pocketfft).  Not an expected value: it measures how far two correct fp32 implementations drift apart."""
+    tab = np.loadtxt(os.path.join(GOLD, "cfg4_indep.txt"), comments="#")
+    return tab[:, 0].astype(np.int64), tab[:, 1].astype(np.float32), tab[:, 2].astype(np.float32)
+
+
 def test_cg_config4_full_size(B):
     """configs[4], L=8192 fp32 (the largest config), against the oracle's stored full solve (its count, its residual history,
     u at 4096 seeded sample sites after 20 iterations and at the stop; the oracle needs minutes for it, hence the file):
-      * pinned count 20 (SURVEY.md 8(d)): samples to 1e-5 (a tenth of the tolerance), ||u|| and the residual to 1e-3;
       * natural stop: |it - it_oracle| <= 2 (north_star).  A larger difference is accepted only when the stored history
         classifies it as a rounding flip of the stopping decision (SURVEY.md 8(c) P14 risk note): whichever side stopped later
         was within 1 % of tol at the other side's stop, so both stops are first crossings of the same run up to rounding;
-      * u at the stop on the samples to 1e-4, at the natural stops if the counts agree, else re-run pinned at the oracle's count;
-      * ||f - A_oracle u||/||f|| <= 2 tol with one oracle operator application (a property that needs no stored value)."""
+      * u at the stop on the samples to 1e-4 (north_star), at the natural stops if the counts agree, else re-run pinned at the
+        oracle's count; ||u|| to 1e-4;
+      * ||f - A_oracle u||/||f|| <= 2 tol with one oracle operator application (a property that needs no stored value);
+      * pinned count 3, the whole vector against the oracle run here: 1e-5 (a tenth of the tolerance);
+      * pinned count 20 on the samples.  Reading S19: at this size fp32 CG amplifies rounding-level
+        differences of the operator between ANY two implementations in mid-run (the residual stalls near 0.1 for ten iterations)
+        and convergence pulls the iterates together again: the oracle and a second CPU implementation (scipy pocketfft, stored by
+        make_golden_cfg4.py --indep) are 4.8e-4 apart after 20 iterations and 2.2e-6 apart at their stops.  So the bound here is
+        that drift, not 1e-5: the GPU must be no further from the oracle than three times what the second CPU implementation is."""
     meta, hist, site, u_pin, u_stop = load_cfg4_golden()
+    site2, v_pin, v_stop = load_cfg4_drift()
     it_or, pin = int(meta["iters"]), int(meta["pin"])
-    assert int(meta["status"]) == 0 and len(hist) == it_or + 1 and len(site) >= 4096
+    assert int(meta["status"]) == 0 and len(hist) == it_or + 1 and len(site) >= 4096 and np.array_equal(site, site2)
+    drift_pin, drift_stop = rel(v_pin, u_pin), rel(v_stop, u_stop)
+    assert drift_stop <= 1e-5 < drift_pin                               # what S19 says, from the two stored CPU runs alone
     w = inputs.config(4)
     h = handle(B, w.L, np.float32, w.s)
     kd, fd = dev(w.k), dev(w.f)
     sd = torch.from_numpy(site).cuda()
+    ref3 = orc.cg(w.s, w.k, w.f, w.u0, 0.0, 3, history=True)
+    u = dev(w.u0)
+    it, rr, _ = h.fcg_solve(kd, fd, u, 0.0, 3)
+    assert it == 3 and rel(u.cpu().numpy(), ref3["u"]) <= 1e-5
+    assert abs(rr - ref3["hist"][3]) <= 1e-3 * ref3["hist"][3]
     u = dev(w.u0)
     it, rr, _ = h.fcg_solve(kd, fd, u, 0.0, pin)
-    assert it == pin and rel(u.view(-1)[sd].cpu().numpy(), u_pin) <= 1e-5
-    assert abs(float(u.double().norm()) - float(meta["norm_u_pin"])) <= 1e-5 * float(meta["norm_u_pin"])
-    assert abs(rr - hist[pin]) <= 1e-3 * hist[pin]
+    d20 = rel(u.view(-1)[sd].cpu().numpy(), u_pin)
+    assert it == pin and d20 <= 3.0 * drift_pin, (d20, drift_pin)
+    assert abs(float(u.double().norm()) - float(meta["norm_u_pin"])) <= 3.0 * drift_pin * float(meta["norm_u_pin"])
+    assert abs(rr - hist[pin]) <= 0.1 * hist[pin]
     u = dev(w.u0)
     it, rr, st = h.fcg_solve(kd, fd, u, w.tol, w.maxit)
     assert st == 0 and rr <= w.tol
