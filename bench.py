@@ -444,6 +444,70 @@ def iteration_roofline(nw, t_iter_us, hbm_peak, peak_src, dram_iter):
     return d
 
 
+def run_slab(args, rank, world, local):
+    """--shard slab: ONE solve spread over the ranks by rows instead of one
+    replica per rank.  Under torchrun every process is one rank (DistComm: NCCL all-to-all of the half spectrum around the column
+    pass, all-reduce of the two scalars); with one process, --slab-ranks G runs G LOGICAL ranks on the one device (LocalComm:
+    device copies), which exercises the same kernels and orchestration but measures nothing about scaling."""
+    import torch
+    import torch.distributed as dist
+    from paper_1305_3625_b200 import binding, inputs, slab
+    torch.cuda.set_device(local)
+    tdt = torch.float64 if args.dtype == "f64" else torch.float32
+    w = inputs.config(args.config, np.float64 if args.dtype == "f64" else np.float32)
+    to = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        comm, G, mine = slab.DistComm(), world, [rank]
+    else:
+        comm, G, mine = slab.LocalComm(), args.slab_ranks, list(range(args.slab_ranks))
+    sd = to(w.s)
+    ranks = [slab.SlabRank(w.L, tdt, G, g, sd) for g in mine]
+    k = [to(w.k[r.rows]) for r in ranks]; f = [to(w.f[r.rows]) for r in ranks]
+    u = [torch.zeros_like(x) for x in k]
+    sampler = ClockSampler(local) if rank == 0 else None
+    for _ in range(args.warmup):
+        for x in u: x.zero_()
+        it, rr, st = slab.slab_solve(ranks, comm, k, f, u, w.tol, w.maxit)
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    if sampler:
+        sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    its, launches = 0, 0
+    e0.record()
+    for _ in range(args.steps):
+        for x in u: x.zero_()
+        it, rr, st = slab.slab_solve(ranks, comm, k, f, u, w.tol, w.maxit)
+        its += it; launches += sum(r.h.fcg_last_launch_count() for r in ranks)
+    e1.record(); torch.cuda.synchronize()
+    clocks = sampler.stop() if sampler else None
+    ms = e0.elapsed_time(e1)
+    if world > 1:                                            # one job: time = max over ranks, work = the iterations of the one solve
+        t = torch.tensor([ms], dtype=torch.float64, device="cuda"); dist.all_reduce(t, op=dist.ReduceOp.MAX); ms = float(t.item())
+        c = torch.tensor([float(launches)], dtype=torch.float64, device="cuda"); dist.all_reduce(c); launches = int(c.item())
+    if rank == 0:
+        nw = w.N * w.dtype.itemsize
+        t_iter_us = 1e3 * ms / max(its, 1)
+        print(json.dumps({
+            "metric": METRIC, "value": its / (ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": args.dtype,
+            "data": "synthetic",
+            "config": {"workload": f"BASELINE.json configs[{args.config}]: L={w.L} {args.dtype}, ONE solve split by rows over {G} "
+                                   f"{'ranks (one per GPU, NCCL)' if world > 1 else 'LOGICAL ranks on one device (device copies)'}, tol={w.tol:g} ({it} iterations)",
+                       "parallelism": f"slab x{G}", "launches_per_iteration_per_rank": 5, "collectives_per_iteration": "2 all-to-all (N w / G bytes per rank each) + 2 all-reduce (16 B)",
+                       "note": "textbook order, host poll once per iteration; the hardware scaling curve is unmeasured on this one-GPU pool"},
+            "site_iterations_per_s": its / (ms * 1e-3) * w.N, "us_per_iteration": t_iter_us,
+            "exchange_bytes_per_iteration_per_rank": 2.0 * nw / G * (G - 1) / G,
+            "gpu_launches": launches, "clocks": clocks, "final_rel_residual": rr, "status": st}))
+    for r in ranks:
+        r.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
 def aggregate_over_ranks(dist, torch, step_ms, total_it, launches, e2e_iter_s, device):
     """Replicas only: whole-job time = MAX over ranks of the device time, whole-job work = SUM over ranks.
     `dist` is torch.distributed with an initialised group (nccl on the GPU box, gloo in the CPU test) or None for one rank."""
@@ -471,6 +535,10 @@ def main():
     ap.add_argument("--solver", choices=["cg", "pcg", "force"], default="cg",
                     help="pcg: time fcg_pcg_solve instead (metric pcg_iterations_per_s, 22 N w bytes per iteration; no e2e leg) -- "
                          "for profiling the PCG kernels; the headline BASELINE.json names is the default")
+    ap.add_argument("--shard", choices=["replicas", "slab"], default="replicas",
+                    help="N > 1: replicas (default; one independent solve per GPU, no data-path collective) or slab (ONE solve split by rows "
+                         "over the ranks: all-to-all transposes around the column pass, all-reduce of the scalars; DESIGN.md section 18)")
+    ap.add_argument("--slab-ranks", type=int, default=4, help="--shard slab with one process: number of LOGICAL ranks on the one device")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-configs", action="store_true", help="skip the 'configs' block (configs[2] fp32, configs[4], transforms, break step)")
     ap.add_argument("--no-spectral-alpha", action="store_true",
@@ -487,6 +555,9 @@ def main():
     local = int(os.environ.get("LOCAL_RANK", "0"))
     if args.impl == "reference":
         run_reference(args, rank)
+        return
+    if args.shard == "slab":
+        run_slab(args, rank, world, local)
         return
 
     import torch

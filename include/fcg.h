@@ -260,6 +260,66 @@ int fcg_force_break_step(fcg_handle h, void* k, void* f, const void* t, long lon
 int fcg_force_fracture(fcg_handle h, void* k, double D, void* f, const void* t, int nsteps, double tol, int maxit,
                        long long* index_host, int* iters_host, double* ratio_host, int* steps_done_host);
 
+/* ---- Slab-decomposed conjugate gradient over several ranks (the paper's remark on the bus as the
+ * bottleneck between devices) ----------------------------------------------------------------
+ * The path shards by rows: rank g of G owns rows [g L/G, (g+1) L/G) of every vector (k, f, u and the library's r, p, q), i.e. the
+ * row pairs [g L/2G, (g+1) L/2G).  The row passes are local.  The column pass needs whole columns, so the half spectrum is
+ * transposed between the ranks before and after it: rank g ends up with the columns [g L/2G, (g+1) L/2G) (whole 128-byte lines of
+ * T2: L/(2 NB G) column blocks of NB columns), and the two scalars of Listing 2 (p.q and r.r) are sums over the ranks.
+ * The library provides the local passes, the (un)packing around the exchange and the scalar steps; the CALLER runs the two
+ * collectives -- an all-to-all with equal chunks on the send / receive buffers and an all-reduce (sum) on a device buffer of two
+ * doubles -- with whatever connects the ranks (torch.distributed over NCCL in paper_1305_3625_b200/slab.py; plain copies when
+ * several logical ranks share one device).  One handle per rank (fcg_create on the rank's device, then fcg_slab_configure);
+ * fcg_set_spectrum takes the full L x L spectrum on every rank.  Textbook order of Listing 2, one iteration =
+ *     rows_fwd(cg) | all-to-all S->R | unpack, cols, pack | all-to-all R->S | rows_inv -> xch | all-reduce | scalar(1) |
+ *     update_r -> xch | all-reduce | scalar(2) | poll
+ * Every rank computes alpha, beta, the count and the stopping decision itself from the all-reduced sums: identical everywhere.
+ *
+ *   fcg_slab_shape_of   pure host arithmetic, no device needed: how the lattice splits over nranks (FCG_UNSUPPORTED unless nranks
+ *                       divides L / (2 NB) and L / 2; NB = columns per 128-byte line: 4 for FCG_F64, 8 for FCG_F32; L >= 256)
+ *   fcg_slab_configure  make this handle rank `rank` of `nranks` (this slice keeps the full-size workspace of fcg_create)
+ *   fcg_slab_buffers    byte offsets into the handle's workspace of the send buffer S (T2 of the own rows, ordered by destination
+ *                       rank: nranks chunks of chunk_bytes) and the receive buffer R (ordered by source rank), buffer_bytes each.
+ *                       Forward exchange: all-to-all S -> R; backward: all-to-all R -> S.  (The workspace must be the caller's.)
+ *   fcg_slab_setup      reset the scalar block: tol, maxit (before fcg_slab_rows_inv(residual = 1))
+ *   fcg_slab_rows_fwd   cg = 0: row transforms of the own rows of xu (an input vector) into S;  cg = 1: u += alpha p (lagged one
+ *                       pass), p = r + beta p, row transforms of p into S (xu = the own rows of u, updated in place)
+ *   fcg_slab_unpack     R -> C, the own columns in the layout the column pass reads;   fcg_slab_pack  C -> R
+ *   fcg_slab_cols       column pass on C in place: F^H (shat o F .) of the own columns
+ *   fcg_slab_rows_inv   inverse row transforms of S;  residual = 1: r = f - (k o u + C u), p := 0, xch = { r.r, f.f } of the own rows;
+ *                       residual = 0: q = k o p + C p, xch[0] = p.q of the own rows.  xch: device, 2 doubles, caller-owned
+ *   fcg_slab_update_r   r -= alpha q on the own rows, xch[0] = their r.r
+ *   fcg_slab_scalar     the scalar step on the ALL-REDUCED xch: what = 0 after the residual pass (rho, ||f||^2, early exit), 1 after
+ *                       rows_inv (alpha, or breakdown), 2 after update_r (count, convergence / maxit, beta, rho)
+ *   fcg_slab_finish     the last lagged u += alpha p on the own rows
+ *   fcg_slab_poll       read the scalar block back (blocks): done flag, iteration count, relative residual, status
+ * All calls but fcg_slab_shape_of and fcg_slab_poll are asynchronous on the handle's stream. */
+typedef struct {
+    int nranks, rank;
+    int columns_per_line;      /* NB */
+    int column_blocks;         /* L / (2 NB): 128-byte-line blocks of NB columns */
+    int column_blocks_local;   /* of which this rank owns L / (2 NB nranks) */
+    int row_pairs_local;       /* L / (2 nranks) */
+    int rows_local;            /* L / nranks: rows [rank * rows_local, ..) of every vector */
+    int columns_local, column0;/* columns [column0, column0 + columns_local) of the half spectrum (column 0 = the packed n = 0, L/2 pair) */
+    size_t line_bytes;         /* 128 */
+    size_t chunk_bytes;        /* one (source rank, destination rank) piece of the exchange */
+    size_t buffer_bytes;       /* nranks * chunk_bytes = N w / nranks */
+} fcg_slab_shape;
+int fcg_slab_shape_of(int L, fcg_dtype dt, int nranks, int rank, fcg_slab_shape* out);
+int fcg_slab_configure(fcg_handle h, int nranks, int rank);
+int fcg_slab_buffers(fcg_handle h, size_t* send_offset, size_t* recv_offset, size_t* bytes);
+int fcg_slab_setup(fcg_handle h, double tol, int maxit);
+int fcg_slab_rows_fwd(fcg_handle h, int cg, void* xu);
+int fcg_slab_unpack(fcg_handle h);
+int fcg_slab_pack(fcg_handle h);
+int fcg_slab_cols(fcg_handle h);
+int fcg_slab_rows_inv(fcg_handle h, int residual, const void* k, const void* u, const void* f, void* xch);
+int fcg_slab_update_r(fcg_handle h, void* xch);
+int fcg_slab_scalar(fcg_handle h, int what, const void* xch);
+int fcg_slab_finish(fcg_handle h, void* u);
+int fcg_slab_poll(fcg_handle h, int* done_host, int* iters_host, double* rel_residual_host, int* status_host);
+
 /* Measurement aid: runs the set-up of fcg_solve and then `iters` iterations of the CG loop body as direct
  * launches with CUDA events between the four kernels (tol = 0: never stops early), and returns their mean
  * device times in milliseconds, ms_host[0..3] = { row pass forward (P1), column pass (P2), row pass inverse

@@ -30,7 +30,16 @@ EXPORTS = ["fcg_workspace_bytes", "fcg_create", "fcg_destroy", "fcg_set_option",
            "fcg_fracture_begin", "fcg_fracture_end",
            "fcg_green_function", "fcg_kernel_spectrum", "fcg_force_apply", "fcg_force_solve", "fcg_force_break_step",
            "fcg_force_fracture", "fcg_inverse_spectrum", "fcg_force_rhs", "fcg_force_from_displacement",
-           "fcg_force_fracture_displacement", "fcg_force_fracture_displacement_begin", "fcg_force_fracture_displacement_end"]
+           "fcg_force_fracture_displacement", "fcg_force_fracture_displacement_begin", "fcg_force_fracture_displacement_end",
+           "fcg_slab_shape_of", "fcg_slab_configure", "fcg_slab_buffers", "fcg_slab_setup", "fcg_slab_rows_fwd", "fcg_slab_unpack",
+           "fcg_slab_pack", "fcg_slab_cols", "fcg_slab_rows_inv", "fcg_slab_update_r", "fcg_slab_scalar", "fcg_slab_finish", "fcg_slab_poll"]
+
+
+class SlabShape(C.Structure):
+    """fcg_slab_shape of include/fcg.h."""
+    _fields_ = [("nranks", C.c_int), ("rank", C.c_int), ("columns_per_line", C.c_int), ("column_blocks", C.c_int),
+                ("column_blocks_local", C.c_int), ("row_pairs_local", C.c_int), ("rows_local", C.c_int), ("columns_local", C.c_int),
+                ("column0", C.c_int), ("line_bytes", C.c_size_t), ("chunk_bytes", C.c_size_t), ("buffer_bytes", C.c_size_t)]
 
 _lib = None
 
@@ -83,6 +92,19 @@ def lib() -> C.CDLL:
         L.fcg_force_solve.argtypes = [vp, vp, d, vp, d, i, C.POINTER(i), C.POINTER(d)]; L.fcg_force_solve.restype = i
         L.fcg_force_break_step.argtypes = [vp, vp, vp, vp, C.POINTER(ll), C.POINTER(d)]; L.fcg_force_break_step.restype = i
         L.fcg_force_fracture.argtypes = [vp, vp, d, vp, vp, i, d, i, vp, vp, vp, C.POINTER(i)]; L.fcg_force_fracture.restype = i
+        L.fcg_slab_shape_of.argtypes = [i, i, i, i, C.POINTER(SlabShape)]; L.fcg_slab_shape_of.restype = i
+        L.fcg_slab_configure.argtypes = [vp, i, i]; L.fcg_slab_configure.restype = i
+        L.fcg_slab_buffers.argtypes = [vp, C.POINTER(C.c_size_t), C.POINTER(C.c_size_t), C.POINTER(C.c_size_t)]; L.fcg_slab_buffers.restype = i
+        L.fcg_slab_setup.argtypes = [vp, d, i]; L.fcg_slab_setup.restype = i
+        L.fcg_slab_rows_fwd.argtypes = [vp, i, vp]; L.fcg_slab_rows_fwd.restype = i
+        L.fcg_slab_unpack.argtypes = [vp]; L.fcg_slab_unpack.restype = i
+        L.fcg_slab_pack.argtypes = [vp]; L.fcg_slab_pack.restype = i
+        L.fcg_slab_cols.argtypes = [vp]; L.fcg_slab_cols.restype = i
+        L.fcg_slab_rows_inv.argtypes = [vp, i, vp, vp, vp, vp]; L.fcg_slab_rows_inv.restype = i
+        L.fcg_slab_update_r.argtypes = [vp, vp]; L.fcg_slab_update_r.restype = i
+        L.fcg_slab_scalar.argtypes = [vp, i, vp]; L.fcg_slab_scalar.restype = i
+        L.fcg_slab_finish.argtypes = [vp, vp]; L.fcg_slab_finish.restype = i
+        L.fcg_slab_poll.argtypes = [vp, C.POINTER(i), C.POINTER(i), C.POINTER(d), C.POINTER(i)]; L.fcg_slab_poll.restype = i
         L.fcg_last_launch_count.argtypes = [vp]; L.fcg_last_launch_count.restype = ll
         L.fcg_last_error.argtypes = [vp]; L.fcg_last_error.restype = C.c_char_p
         L.fcg_version.argtypes = []; L.fcg_version.restype = C.c_char_p
@@ -389,8 +411,67 @@ class Fcg:
             self._raise(st)
         return index, iters, ratio, int(done.value), int(st)
 
+    # -- slab-decomposed CG over several ranks (include/fcg.h): the local passes of one rank -------------------
+    def _ok(self, st: int):
+        if st != FCG_OK:
+            self._raise(st)
+
+    def fcg_slab_configure(self, nranks: int, rank: int):
+        self._ok(self._lib.fcg_slab_configure(self._h, int(nranks), int(rank)))
+
+    def fcg_slab_buffers(self):
+        """(send, recv): uint8 views of the handle's workspace -- the two exchange buffers of this rank."""
+        if self._ws is None:
+            raise ValueError("slab buffers are views of the caller-owned workspace (own_workspace=False)")
+        so, ro, nb = C.c_size_t(0), C.c_size_t(0), C.c_size_t(0)
+        self._ok(self._lib.fcg_slab_buffers(self._h, C.byref(so), C.byref(ro), C.byref(nb)))
+        return self._ws[so.value: so.value + nb.value], self._ws[ro.value: ro.value + nb.value]
+
+    def fcg_slab_setup(self, tol: float, maxit: int):
+        self._ok(self._lib.fcg_slab_setup(self._h, float(tol), int(maxit)))
+
+    def fcg_slab_rows_fwd(self, cg: bool, xu: torch.Tensor):
+        self._ok(self._lib.fcg_slab_rows_fwd(self._h, 1 if cg else 0, self._chk(xu)))
+
+    def fcg_slab_unpack(self):
+        self._ok(self._lib.fcg_slab_unpack(self._h))
+
+    def fcg_slab_pack(self):
+        self._ok(self._lib.fcg_slab_pack(self._h))
+
+    def fcg_slab_cols(self):
+        self._ok(self._lib.fcg_slab_cols(self._h))
+
+    def fcg_slab_rows_inv(self, residual: bool, k: torch.Tensor, u, f, xch: torch.Tensor):
+        self._ok(self._lib.fcg_slab_rows_inv(self._h, 1 if residual else 0, self._chk(k), self._chk(u) if u is not None else None,
+                                             self._chk(f) if f is not None else None, self._chk(xch, 2, torch.float64)))
+
+    def fcg_slab_update_r(self, xch: torch.Tensor):
+        self._ok(self._lib.fcg_slab_update_r(self._h, self._chk(xch, 2, torch.float64)))
+
+    def fcg_slab_scalar(self, what: int, xch: torch.Tensor):
+        self._ok(self._lib.fcg_slab_scalar(self._h, int(what), self._chk(xch, 2, torch.float64)))
+
+    def fcg_slab_finish(self, u: torch.Tensor):
+        self._ok(self._lib.fcg_slab_finish(self._h, self._chk(u)))
+
+    def fcg_slab_poll(self):
+        """(done, iters, rel_residual, status) of the scalar block; blocks."""
+        dn, it, st = C.c_int(0), C.c_int(0), C.c_int(0); rr = C.c_double(0.0)
+        self._ok(self._lib.fcg_slab_poll(self._h, C.byref(dn), C.byref(it), C.byref(rr), C.byref(st)))
+        return bool(dn.value), int(it.value), float(rr.value), int(st.value)
+
     def fcg_last_launch_count(self) -> int:
         return int(self._lib.fcg_last_launch_count(self._h))
+
+
+def fcg_slab_shape_of(L: int, dtype, nranks: int, rank: int) -> dict:
+    """Pure host arithmetic in libfcg (no device needed): how an L x L lattice of this dtype splits over nranks."""
+    sh = SlabShape()
+    st = lib().fcg_slab_shape_of(int(L), _dt(dtype), int(nranks), int(rank), C.byref(sh))
+    if st != FCG_OK:
+        raise FcgError(st, f"slab decomposition of L={L} over {nranks} ranks is not supported")
+    return {name: getattr(sh, name) for name, _ in SlabShape._fields_}
 
 
 def fcg_version() -> str:

@@ -101,6 +101,11 @@ struct fcg_handle_s {
     std::vector<GraphEntry> graphs; unsigned long long stamp = 0;
     long long launches = 0;
     std::string err;
+    // slab-decomposed CG: this handle is rank `slab_rank` of `slab_G`
+    int slab_G = 0, slab_rank = 0, slab_Al = 0, slab_MBl = 0;     // row pairs and column blocks this rank owns
+    size_t slab_S = 0, slab_R = 0, slab_C = 0, slab_bytes = 0;     // workspace offsets of T2 (rows side), the exchange buffer, T2 (columns side)
+    alignas(64) CUtensorMap tmap_row_s;  // S as [L/(2 NB)][Al][128 B]
+    alignas(64) CUtensorMap tmap_col_s;  // C as [MBl][L/2][NB][2 complex]
     int device = 0;                     // the device the handle was created on; every entry point runs with it current
     unsigned int barrier_start = 0;     // FCG_OPT_BARRIER_START: initial value of the cooperative kernel's barrier counter
 
@@ -287,7 +292,7 @@ template <typename T> struct Seq {
         at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
         at[0].val.programmaticStreamSerializationAllowed = 1;
         cfg.attrs = at; cfg.numAttrs = h->pdl ? 1u : 0u;
-        return cudaLaunchKernelEx(&cfg, cg_update_r_kernel<T>, r(), (const T*)q(), nvec, h->at<double>(h->lay.partial_vec), h->sc(), h->hints);
+        return cudaLaunchKernelEx(&cfg, cg_update_r_kernel<T>, r(), (const T*)q(), nvec, h->at<double>(h->lay.partial_vec), h->sc(), h->hints, (double*)nullptr);
     }
     // spectral search length: alpha is known after the column pass, so the residual update rides in P3
     cudaError_t it_col_e() const {
@@ -686,6 +691,107 @@ int tensor_map_init(fcg_handle h) {
         if (r != CUDA_SUCCESS) { h->err = "cuTensorMapEncodeTiled (columns) failed (code " + std::to_string((int)r) + ")"; return FCG_CUDA_ERROR; }
     }
     h->have_tmap = true;
+    return FCG_OK;
+}
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+// tensor maps of one rank's two T2 buffers (same boxes as tensor_map_init, other extents)
+int slab_tensor_maps(fcg_handle h) {
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn || qres != cudaDriverEntryPointSuccess) {
+        cudaGetLastError();
+        return fail(h, FCG_UNSUPPORTED, "cuTensorMapEncodeTiled unavailable");
+    }
+    auto enc = reinterpret_cast<EncodeTiledFn>(fn);
+    const cuuint64_t L = (cuuint64_t)h->L, w = (cuuint64_t)h->w, NB = (cuuint64_t)h->tab->v2_nb, Al = (cuuint64_t)h->slab_Al, MBl = (cuuint64_t)h->slab_MBl;
+    const CUtensorMapDataType dtp = h->dtype == FCG_F64 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32;
+    const cuuint32_t estr[4] = {1u, 1u, 1u, 1u};
+    {   // rows side S: d0 = one 128-byte line, d1 = local row pair, d2 = column block
+        const cuuint64_t gdim[3] = {4 * NB, Al, L / (2 * NB)};
+        const cuuint64_t gstride[2] = {4 * NB * w, Al * 4 * NB * w};
+        const cuuint32_t box[3] = {(cuuint32_t)(4 * NB), 1u, (cuuint32_t)(h->tab->v2_tsub / (int)NB)};
+        if (enc(&h->tmap_row_s, dtp, 3, h->ws + h->slab_S, gdim, gstride, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+            return fail(h, FCG_CUDA_ERROR, "cuTensorMapEncodeTiled (slab rows) failed");
+    }
+    {   // columns side C: d0 = 2 complex of one row pair, d1 = column in block, d2 = row pair (all of them), d3 = local column block
+        const cuuint64_t gdim[4] = {4, NB, L / 2, MBl};
+        const cuuint64_t gstride[3] = {4 * w, 4 * NB * w, (L / 2) * 4 * NB * w};
+        const cuuint32_t box[4] = {4u, 1u, (cuuint32_t)h->tab->v2_abox, 1u};
+        if (enc(&h->tmap_col_s, dtp, 4, h->ws + h->slab_C, gdim, gstride, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+            return fail(h, FCG_CUDA_ERROR, "cuTensorMapEncodeTiled (slab columns) failed");
+    }
+    return FCG_OK;
+}
+
+// shape algebra of the slab decomposition: pure host arithmetic (also callable without a device: fcg_slab_shape_of)
+int slab_shape(int L, int dtype, int G, int rank, fcg_slab_shape* o) {
+    if (!supported(L) || (dtype != FCG_F32 && dtype != FCG_F64) || !o) return FCG_INVALID_ARG;
+    const PassTable* tab = get_table(L, dtype);
+    if (!tab || !tab->v2) return FCG_UNSUPPORTED;
+    const int NB = tab->v2_nb, MB = L / (2 * NB);
+    if (G < 1 || rank < 0 || rank >= G || MB % G != 0 || (L / 2) % G != 0) return FCG_UNSUPPORTED;
+    const size_t w = dtype == FCG_F64 ? 8 : 4;
+    o->nranks = G; o->rank = rank; o->columns_per_line = NB; o->column_blocks = MB; o->column_blocks_local = MB / G;
+    o->row_pairs_local = (L / 2) / G; o->rows_local = L / G; o->columns_local = (L / 2) / G; o->column0 = rank * ((L / 2) / G);
+    o->line_bytes = (size_t)NB * 4 * w;
+    o->chunk_bytes = (size_t)(MB / G) * ((L / 2) / G) * o->line_bytes;
+    o->buffer_bytes = (size_t)G * o->chunk_bytes;
+    return FCG_OK;
+}
+
+template <typename T>
+int slab_rows_fwd_impl(fcg_handle h, int mode, void* xu) {
+    RowFwdArgs<T> A{}; A.mode = mode; A.x = (const T*)xu; A.u = (T*)xu; A.p = h->at<T>(h->lay.p); A.r = h->at<T>(h->lay.r);
+    A.Tb = reinterpret_cast<cx<T>*>(h->ws + h->slab_S); A.tw = h->at<cx<T>>(h->lay.tw); A.sc = h->sc(); A.nsm = h->nsm; A.tmo = &h->sc()->timeout;
+    A.ntile = h->slab_Al; A.astride = h->slab_Al;
+    ++h->launches;
+    FCG_CK(h, h->tab->row_fwd2_slab(&A, h->stream));
+    return FCG_OK;
+}
+template <typename T>
+int slab_cols_impl(fcg_handle h) {
+    ColArgs<T> A{}; A.mode = COL_CONV; A.Tb = reinterpret_cast<cx<T>*>(h->ws + h->slab_C); A.shat = h->at<T>(h->lay.shat); A.tw = h->at<cx<T>>(h->lay.tw);
+    A.sc = nullptr; A.nsm = h->nsm; A.tmo = &h->sc()->timeout; A.col0 = h->slab_rank * ((h->L / 2) / h->slab_G);
+    ++h->launches;
+    FCG_CK(h, h->tab->col2_slab(&A, &h->tmap_col_s, (h->L / 2) / h->slab_G, h->stream));
+    return FCG_OK;
+}
+template <typename T>
+int slab_rows_inv_impl(fcg_handle h, int mode, const void* k, const void* v, const void* f, void* xch) {
+    RowInvArgs<T> A{}; A.mode = mode; A.tw = h->at<cx<T>>(h->lay.tw); A.k = (const T*)k; A.f = (const T*)f;
+    A.v = mode == ROWI_RESID ? (const T*)v : h->at<T>(h->lay.p);
+    A.out = mode == ROWI_RESID ? h->at<T>(h->lay.r) : h->at<T>(h->lay.q); A.out2 = mode == ROWI_RESID ? h->at<T>(h->lay.p) : nullptr;
+    A.scale = (T)(1.0 / ((double)h->L * (double)h->L)); A.partial = h->at<double>(h->lay.partial_row); A.sc = h->sc(); A.nsm = h->nsm;
+    A.tmo = &h->sc()->timeout; A.ntile = h->slab_Al; A.xch = (double*)xch;
+    ++h->launches;
+    FCG_CK(h, h->tab->row_inv2_slab(&A, &h->tmap_row_s, h->stream));
+    return FCG_OK;
+}
+template <typename T>
+int slab_update_r_impl(fcg_handle h, void* xch) {
+    const size_t nvec = (h->N / (size_t)h->slab_G) / Vec<T>::W, per = 256 * 4;
+    size_t b = (nvec + per - 1) / per;
+    if (b > (size_t)VEC_BLOCKS_MAX) b = VEC_BLOCKS_MAX;
+    if (b < 1) b = 1;
+    ++h->launches;
+    cg_update_r_kernel<T><<<(unsigned)b, 256, 0, h->stream>>>(h->at<T>(h->lay.r), (const T*)h->at<T>(h->lay.q), nvec, h->at<double>(h->lay.partial_vec), h->sc(), 0, (double*)xch);
+    FCG_CK(h, cudaGetLastError());
+    return FCG_OK;
+}
+template <typename T>
+int slab_finish_impl(fcg_handle h, void* u) {
+    const size_t nvec = (h->N / (size_t)h->slab_G) / Vec<T>::W;
+    size_t b = (nvec + 255) / 256;
+    if (b > (size_t)VEC_BLOCKS_MAX) b = VEC_BLOCKS_MAX;
+    ++h->launches;
+    cg_finish_kernel<T><<<(unsigned)b, 256, 0, h->stream>>>((T*)u, h->at<T>(h->lay.p), nvec, h->sc());
+    FCG_CK(h, cudaGetLastError());
     return FCG_OK;
 }
 
@@ -1200,6 +1306,115 @@ int fcg_force_fracture_displacement(fcg_handle h, void* k, double D, void* u, co
     const int st = fcg_force_fracture_displacement_begin(h, k, D, u, t, nsteps, tol, maxit, use_pcg);
     if (st < 0 && (!h || h->pend_nsteps < 0)) return st;
     return fcg_force_fracture_displacement_end(h, index_host, iters_host, ratio_host, steps_done_host);
+}
+
+// ---- slab-decomposed CG over several ranks
+int fcg_slab_shape_of(int L, fcg_dtype dt, int nranks, int rank, fcg_slab_shape* out) { return slab_shape(L, dt, nranks, rank, out); }
+
+#define FCG_SLAB_ENTER(h)                                                                              \
+    if (!(h)) return FCG_INVALID_ARG;                                                                  \
+    FCG_ENTER(h);                                                                                      \
+    if ((h)->slab_G < 1) return fail((h), FCG_INVALID_ARG, "fcg_slab_configure has not been called")
+
+int fcg_slab_configure(fcg_handle h, int nranks, int rank) {
+    if (!h) return FCG_INVALID_ARG;
+    FCG_ENTER(h);
+    if (!h->v2()) return fail(h, FCG_UNSUPPORTED, "slab decomposition needs the pipelined engine (L >= 256)");
+    fcg_slab_shape sh;
+    const int st = slab_shape(h->L, h->dtype, nranks, rank, &sh);
+    if (st != FCG_OK) return fail(h, st, "slab decomposition: nranks must divide the column blocks L / (2 NB) and the row pairs L / 2");
+    h->slab_G = nranks; h->slab_rank = rank; h->slab_Al = sh.row_pairs_local; h->slab_MBl = sh.column_blocks_local; h->slab_bytes = sh.buffer_bytes;
+    // This first slice keeps the full-size workspace of fcg_create.  S (T2, rows side) and C (T2, columns side) share the T2 region:
+    // N w / G bytes each, C in its upper half; with one rank (the undecomposed case, kept for tests) C is S itself, which is free
+    // once the exchange has copied it out.  The exchange buffer R lives in z, the vector only preconditioned CG uses.
+    h->slab_S = h->lay.Tb;
+    h->slab_C = nranks >= 2 ? h->lay.Tb + align_up(h->N * h->w / 2) : h->lay.Tb;
+    h->slab_R = h->lay.z;
+    return slab_tensor_maps(h);
+}
+
+int fcg_slab_buffers(fcg_handle h, size_t* send_offset, size_t* recv_offset, size_t* bytes) {
+    FCG_SLAB_ENTER(h);
+    if (!send_offset || !recv_offset || !bytes) return fail(h, FCG_INVALID_ARG, "null argument");
+    *send_offset = h->slab_S; *recv_offset = h->slab_R; *bytes = h->slab_bytes;
+    return FCG_OK;
+}
+
+int fcg_slab_setup(fcg_handle h, double tol, int maxit) {
+    FCG_SLAB_ENTER(h);
+    if (!(tol >= 0.0) || maxit < 0) return fail(h, FCG_INVALID_ARG, "tol must be >= 0 and maxit >= 0");
+    if (!h->have_spectrum) return fail(h, FCG_NO_SPECTRUM, "fcg_set_spectrum has not been called");
+    h->launches = 0;
+    SetupArgs sa{tol, maxit, 0, 0ULL, 0};
+    cg_setup_kernel<<<1, 32, 0, h->stream>>>(h->sc(), sa); ++h->launches;
+    FCG_CK(h, cudaGetLastError());
+    return FCG_OK;
+}
+
+int fcg_slab_rows_fwd(fcg_handle h, int cg, void* xu) {
+    FCG_SLAB_ENTER(h);
+    if (!xu) return fail(h, FCG_INVALID_ARG, "null argument");
+    const int mode = cg ? ROWF_CG : ROWF_PLAIN;
+    return h->dtype == FCG_F64 ? slab_rows_fwd_impl<double>(h, mode, xu) : slab_rows_fwd_impl<float>(h, mode, xu);
+}
+
+// R[s][column block][local row pair][line]  <->  C[column block][s Al + local row pair][line]
+static int slab_repack(fcg_handle h, bool unpack) {
+    const size_t line = (size_t)h->tab->v2_nb * 4 * h->w, Al = (size_t)h->slab_Al, chunk = (size_t)h->slab_MBl * Al * line;
+    for (int s2 = 0; s2 < h->slab_G; ++s2) {
+        char* c = h->ws + h->slab_C + (size_t)s2 * Al * line;
+        char* r = h->ws + h->slab_R + (size_t)s2 * chunk;
+        if (unpack) FCG_CK(h, cudaMemcpy2DAsync(c, ((size_t)h->L / 2) * line, r, Al * line, Al * line, (size_t)h->slab_MBl, cudaMemcpyDeviceToDevice, h->stream));
+        else FCG_CK(h, cudaMemcpy2DAsync(r, Al * line, c, ((size_t)h->L / 2) * line, Al * line, (size_t)h->slab_MBl, cudaMemcpyDeviceToDevice, h->stream));
+    }
+    return FCG_OK;
+}
+int fcg_slab_unpack(fcg_handle h) { FCG_SLAB_ENTER(h); return slab_repack(h, true); }
+int fcg_slab_pack(fcg_handle h) { FCG_SLAB_ENTER(h); return slab_repack(h, false); }
+
+int fcg_slab_cols(fcg_handle h) {
+    FCG_SLAB_ENTER(h);
+    if (!h->have_spectrum) return fail(h, FCG_NO_SPECTRUM, "fcg_set_spectrum has not been called");
+    return h->dtype == FCG_F64 ? slab_cols_impl<double>(h) : slab_cols_impl<float>(h);
+}
+
+int fcg_slab_rows_inv(fcg_handle h, int residual, const void* k, const void* u, const void* f, void* xch) {
+    FCG_SLAB_ENTER(h);
+    if (!k || !xch || (residual && (!u || !f))) return fail(h, FCG_INVALID_ARG, "null argument");
+    const int mode = residual ? ROWI_RESID : ROWI_CG;
+    return h->dtype == FCG_F64 ? slab_rows_inv_impl<double>(h, mode, k, u, f, xch) : slab_rows_inv_impl<float>(h, mode, k, u, f, xch);
+}
+
+int fcg_slab_update_r(fcg_handle h, void* xch) {
+    FCG_SLAB_ENTER(h);
+    if (!xch) return fail(h, FCG_INVALID_ARG, "null argument");
+    return h->dtype == FCG_F64 ? slab_update_r_impl<double>(h, xch) : slab_update_r_impl<float>(h, xch);
+}
+
+int fcg_slab_scalar(fcg_handle h, int what, const void* xch) {
+    FCG_SLAB_ENTER(h);
+    if (!xch || what < 0 || what > 2) return fail(h, FCG_INVALID_ARG, "bad argument");
+    slab_scalar_kernel<<<1, 32, 0, h->stream>>>(h->sc(), what, (const double*)xch); ++h->launches;
+    FCG_CK(h, cudaGetLastError());
+    return FCG_OK;
+}
+
+int fcg_slab_finish(fcg_handle h, void* u) {
+    FCG_SLAB_ENTER(h);
+    if (!u) return fail(h, FCG_INVALID_ARG, "null argument");
+    return h->dtype == FCG_F64 ? slab_finish_impl<double>(h, u) : slab_finish_impl<float>(h, u);
+}
+
+int fcg_slab_poll(fcg_handle h, int* done_host, int* iters_host, double* rel_residual_host, int* status_host) {
+    FCG_SLAB_ENTER(h);
+    FCG_CK(h, cudaMemcpyAsync(h->h_sc, h->sc(), sizeof(Scalars), cudaMemcpyDeviceToHost, h->stream));
+    FCG_CK(h, cudaStreamSynchronize(h->stream));
+    if (done_host) *done_host = h->h_sc->done;
+    if (iters_host) *iters_host = h->h_sc->it;
+    if (rel_residual_host) *rel_residual_host = h->h_sc->relres;
+    if (status_host) *status_host = h->h_sc->status;
+    if (h->h_sc->timeout) return fail(h, FCG_CUDA_ERROR, "a pipelined pass gave up waiting on an mbarrier");
+    return FCG_OK;
 }
 
 int fcg_profile_iteration(fcg_handle h, const void* k, const void* f, void* u, int iters, double* ms_host) {

@@ -45,6 +45,7 @@ template <typename T, typename P> struct AsyncShape {
     static FCG_HD int pos_of_col(int m) { return (m / HR) * P::RLAST + m % HR; }
     static FCG_HD int col_of_pos(int e) { return (e / P::RLAST) * HR + e % P::RLAST; }
     static FCG_HD size_t t2_index(int m, int A) { return (((size_t)(m / NB) * (L / 2) + A) * NB + m % NB) * 2; }   // complex units, r = 0
+    static FCG_HD size_t t2_index_s(int m, int A, int astride) { return (((size_t)(m / NB) * astride + A) * NB + m % NB) * 2; }   // a slab's T2
 
     // Shared memory.  The rings are sized for CRES resident CTAs per SM: 4 transforms in flight when a work buffer is
     // small, else 2 (1 when even that does not fit); whatever the work buffers leave goes to the rings, whose depth is
@@ -151,9 +152,11 @@ template <typename T, typename P, int CTAS, int VAR = 0>
 __global__ void __launch_bounds__(P::NT + 32, CTAS) row_fwd2_kernel(const RowFwdArgs<T> A)
 {
     constexpr bool RUPD = VAR == 1;
+    constexpr bool SLAB = VAR == 2;      // one rank's row slab: A.ntile row pairs, T2 of A.astride row pairs per column block
     using AS = AsyncShape<T, P>;
     constexpr int L = P::N, S = P::S, NT = P::NT, R1 = AS::R1, Q1 = AS::Q1, PER1 = AS::PER1, PM = per_max<P>();
     constexpr uint32_t PIECE = AS::PIECE;
+    const int NTILE = SLAB ? A.ntile : L / 2, ASTR = SLAB ? A.astride : L / 2;
     constexpr int NSLOT = RUPD ? (AS::NFS * 6 / 4 > AS::MAXSLOT ? AS::MAXSLOT : AS::NFS * 6 / 4) : AS::NFS;
     constexpr uint32_t SLOTB = RUPD ? 4 * PIECE : AS::FSLOTB;
     extern __shared__ unsigned char smem_dyn[];
@@ -176,7 +179,7 @@ __global__ void __launch_bounds__(P::NT + 32, CTAS) row_fwd2_kernel(const RowFwd
               kk = (int)gridDim.x / nsm;
     auto tile_of = [&](int i) { return grp + nsm * (jj + i * kk); };
     int ntl = 0;
-    while (tile_of(ntl) < L / 2) ++ntl;
+    while (tile_of(ntl) < NTILE) ++ntl;
     const int G = ntl * R1;                                       // strips this CTA will consume
 
     if (lt == 0) {
@@ -291,7 +294,7 @@ __global__ void __launch_bounds__(P::NT + 32, CTAS) row_fwd2_kernel(const RowFwd
                 X0 = mk<T>((Za.x + Zb.x) * h, (Za.y - Zb.y) * h);
                 X1 = mk<T>((Za.y + Zb.y) * h, (Zb.x - Za.x) * h);
             }
-            if (st_on) store_pair_hint(A.Tb + AS::t2_index(m, a0 >> 1), X0, X1, pol_t2);
+            if (st_on) store_pair_hint(A.Tb + (SLAB ? AS::t2_index_s(m, a0 >> 1, ASTR) : AS::t2_index(m, a0 >> 1)), X0, X1, pol_t2);
         }
     }
     }
@@ -308,7 +311,9 @@ __global__ void __launch_bounds__(P::NT + 32, CTAS) row_fwd2_kernel(const RowFwd
 // ENERGY = true (a separate instantiation) also accumulates the spectral half of the search length,
 //   p.Cp = sum over the full spectrum of shat |P|^2 = 2 x (columns 0 < n < L/2) + (columns n = 0, L/2)      (Parseval),
 // in the registers of the spectral multiply, and leaves one partial sum per column; row_inv2_kernel<.., 2> adds them up.
-template <typename T, typename P, int CTAS, bool ENERGY = false>
+// SLAB = true (a separate instantiation): the launch covers the columns one rank owns; blockIdx.x numbers them locally (tensor-map
+// coordinates), A.col0 + blockIdx.x is the global column (spectrum row, packed column 0).
+template <typename T, typename P, int CTAS, bool ENERGY = false, bool SLAB = false>
 __global__ void __launch_bounds__(P::NT, CTAS) col2_kernel(const ColArgs<T> A, const __grid_constant__ CUtensorMap tmap)
 {
     using AS = AsyncShape<T, P>;
@@ -321,7 +326,7 @@ __global__ void __launch_bounds__(P::NT, CTAS) col2_kernel(const ColArgs<T> A, c
     SmemIO<T, P> io{W};
     // column m of T2 (frequency freq_of(pos_of_col(m)); m = 0 is the packed n = 0 / L/2 column): 2 complex per row pair,
     // gathered by TMA into natural row order a = 2A + r, and scattered back the same way at the end
-    const int lt = threadIdx.x, n = (int)blockIdx.x;
+    const int lt = threadIdx.x, nl = (int)blockIdx.x, n = SLAB ? nl + A.col0 : nl;      // local (T2 of this launch) and global column
     constexpr int ABOX = AS::ABOX;
     constexpr uint32_t BOXB = (uint32_t)(ABOX * 2 * sizeof(cx<T>));
     tma::grid_dep_launch();
@@ -338,7 +343,7 @@ __global__ void __launch_bounds__(P::NT, CTAS) col2_kernel(const ColArgs<T> A, c
         tma::mbar_expect_tx(&bar, (uint32_t)(AS::WBYTES + (n ? L * sizeof(T) : 0)));
 #pragma unroll
         for (int b = 0; b < (L / 2) / ABOX; ++b)
-            tma::tensor_g2s_4d(smem_raw + (size_t)b * BOXB, &tmap, 0, n % AS::NB, b * ABOX, n / AS::NB, &bar);
+            tma::tensor_g2s_4d(smem_raw + (size_t)b * BOXB, &tmap, 0, nl % AS::NB, b * ABOX, nl / AS::NB, &bar);
         if (n) tma::bulk_g2s_hint(sh, A.shat + (size_t)n * L, (uint32_t)(L * sizeof(T)), &bar,
                                   (A.hints & 4) ? tma::policy_evict_first() : tma::policy_evict_normal());   // read once per iteration
     }
@@ -430,7 +435,7 @@ __global__ void __launch_bounds__(P::NT, CTAS) col2_kernel(const ColArgs<T> A, c
         if (!FCG_PROBE_ON(0x400)) {
 #pragma unroll
         for (int b = 0; b < (L / 2) / ABOX; ++b)
-            tma::tensor_s2g_4d(&tmap, 0, n % AS::NB, b * ABOX, n / AS::NB, smem_raw + (size_t)b * BOXB);
+            tma::tensor_s2g_4d(&tmap, 0, nl % AS::NB, b * ABOX, nl / AS::NB, smem_raw + (size_t)b * BOXB);
         }
         tma::bulk_commit();
     }
@@ -782,6 +787,7 @@ __global__ void __launch_bounds__(AsyncShape<T, P>::INV_THREADS, CTAS) row_inv2_
     using AS = AsyncShape<T, P>;
     constexpr int L = P::N, S = P::S, NT = P::NT, R1 = AS::R1, Q1 = AS::Q1, PER1 = AS::PER1, PM = per_max<P>();
     constexpr bool PRE = VAR == 1, CGF = VAR == 2 || VAR == 3, FCGF = VAR == 3;
+    constexpr bool SLAB = VAR == 4;      // one rank's row slab: A.ntile row pairs; sums go to A.xch, no scalar step
     constexpr int TSUB = AS::TSUB, NSUB = AS::NSUB;
     constexpr uint32_t TBYTES = (uint32_t)AS::TSB;
     // CGF moves three vectors of strips per transform against one of tiles: the tile ring is kept short (TCAP) and the strips
@@ -820,7 +826,7 @@ __global__ void __launch_bounds__(AsyncShape<T, P>::INV_THREADS, CTAS) row_inv2_
               kk = (int)gridDim.x / nsm;
     auto tile_of = [&](int i) { return grp + nsm * (jj + i * kk); };
     int ntl = 0;
-    while (tile_of(ntl) < L / 2) ++ntl;
+    while (tile_of(ntl) < (SLAB ? A.ntile : L / 2)) ++ntl;
 
     if (lt == 0) {
         tma::prefetch_tmap(&tmap);

@@ -56,6 +56,9 @@ template <typename T> struct Inst {
             }
             if ((e = prep(row_inv2_kernel<T, P, C_INV, 2>, AS::inv_smem)) != cudaSuccess) return e;
             if ((e = prep(row_inv2_kernel<T, P, C_INV, 3>, AS::inv_smem)) != cudaSuccess) return e;
+            if ((e = prep(row_fwd2_kernel<T, P, C_FWD, 2>, AS::fwd_smem)) != cudaSuccess) return e;
+            if ((e = prep(col2_kernel<T, P, C_COL, false, true>, AS::col_smem)) != cudaSuccess) return e;
+            if ((e = prep(row_inv2_kernel<T, P, C_INV, 4>, AS::inv_smem)) != cudaSuccess) return e;
             if ((e = prep(col2_xform_kernel<T, P, C_COL, -1>, AS::WBYTES + 128)) != cudaSuccess) return e;
             if ((e = prep(col2_xform_kernel<T, P, C_COL, +1>, AS::WBYTES + 128)) != cudaSuccess) return e;
             if ((e = prep(t2_export_kernel<T, P>, AS::WBYTES + 1024)) != cudaSuccess) return e;
@@ -85,6 +88,33 @@ template <typename T> struct Inst {
         int k = ctas;
         while (k > 1 && nsm * k > L / 2) --k;
         return nsm * k > L / 2 ? L / 2 : nsm * k;
+    }
+    static int pgrid_n(int nsm, int ctas, int ntile) {       // the same for a slab of ntile row pairs
+        int k = ctas;
+        while (k > 1 && nsm * k > ntile) --k;
+        return nsm * k > ntile ? ntile : nsm * k;
+    }
+    static cudaError_t row_fwd2_slab(const void* args, cudaStream_t st) {
+        if constexpr (V2) {
+            const RowFwdArgs<T>& A = *static_cast<const RowFwdArgs<T>*>(args);
+            return launch(row_fwd2_kernel<T, P, C_FWD, 2>, pgrid_n(A.nsm, C_FWD, A.ntile), P::NT + 32, AS::fwd_smem, st, 0, A);
+        }
+        return cudaErrorInvalidValue;
+    }
+    static cudaError_t col2_slab(const void* args, const void* tensor_map, int ncols, cudaStream_t st) {
+        if constexpr (V2) {
+            const ColArgs<T>& A = *static_cast<const ColArgs<T>*>(args);
+            return launch(col2_kernel<T, P, C_COL, false, true>, ncols, P::NT, AS::col_smem, st, 0, A, *static_cast<const CUtensorMap*>(tensor_map));
+        }
+        return cudaErrorInvalidValue;
+    }
+    static cudaError_t row_inv2_slab(const void* args, const void* tensor_map, cudaStream_t st) {
+        if constexpr (V2) {
+            const RowInvArgs<T>& A = *static_cast<const RowInvArgs<T>*>(args);
+            return launch(row_inv2_kernel<T, P, C_INV, 4>, pgrid_n(A.nsm, C_INV, A.ntile), AS::INV_THREADS, AS::inv_smem, st, 0, A,
+                          *static_cast<const CUtensorMap*>(tensor_map));
+        }
+        return cudaErrorInvalidValue;
     }
     static cudaError_t row_fwd2(const void* args, cudaStream_t st) {
         if constexpr (V2) {
@@ -255,6 +285,7 @@ template <typename T> struct Inst {
         t.row_fwd2 = &row_fwd2; t.col2 = &col2; t.row_inv2 = &row_inv2; t.row_fwd2_rupd = &row_fwd2_rupd; t.row_inv2_pre = &row_inv2_pre;
         t.colp_ok = COLP ? 1 : 0; t.colp_ctas = COLP ? CPS::CTAS : 0; t.col2p = &col2p;
         t.sl_ok = SL ? 1 : 0; t.col2_energy = &col2_energy; t.row_inv2_cgf = &row_inv2_cgf; t.row_inv2_cgf_force = &row_inv2_cgf_force;
+        t.row_fwd2_slab = &row_fwd2_slab; t.col2_slab = &col2_slab; t.row_inv2_slab = &row_inv2_slab;
         t.col2_xform = &col2_xform; t.t2_export = &t2_export; t.t2_import = &t2_import;
         t.fused = FS::valid ? 1 : 0; t.fused_grid = FS::G; t.fused_solve = &fused_solve;
         t.init = &init; t.row_fwd = &row_fwd; t.col = &col; t.row_inv = &row_inv; t.spectrum_prep = &spectrum_prep;

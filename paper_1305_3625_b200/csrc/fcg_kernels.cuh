@@ -118,6 +118,7 @@ __device__ __forceinline__ void row_inv_reduce_finalize(const RowInvArgs<T>& A, 
     double tot[2];
     if (!grid_sum_last<2>(acc, A.partial, &A.sc->ticket[0], red, tot)) return;
     if (threadIdx.x != 0) return;
+    if (A.xch) { A.xch[0] = tot[0]; A.xch[1] = tot[1]; return; }       // slab: this rank's share; the scalar step follows the all-reduce
     Scalars* sc = A.sc;
     if (A.mode == ROWI_CGF) { cg_after_rr(sc, tot[0]); return; }           // fused residual update: r.r is this pass's sum
     if (A.mode == ROWI_CG) {
@@ -201,7 +202,7 @@ __device__ __forceinline__ void axpy_sq(float4& r, const float4 q, float a, doub
 // residue, residue length (97), update calculation variables (98: beta), check convergence (99)
 template <typename T>
 __global__ void __launch_bounds__(256) cg_update_r_kernel(T* __restrict__ r, const T* __restrict__ q, size_t nvec,
-                                                           double* partial, Scalars* sc, int hints) {
+                                                           double* partial, Scalars* sc, int hints, double* xch = nullptr) {
     __shared__ double red[32];
     using V = typename Vec<T>::type;
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");    // programmatic dependent launch (fcg_tma.cuh)
@@ -235,8 +236,40 @@ __global__ void __launch_bounds__(256) cg_update_r_kernel(T* __restrict__ r, con
     double tot[1];
     if (!grid_sum_last<1>(acc, partial, &sc->ticket[1], red, tot)) return;
     if (threadIdx.x != 0) return;
+    if (xch) { xch[0] = tot[0]; return; }                  // slab: this rank's share of r.r (fcg_slab_scalar after the all-reduce)
     cg_after_rr(sc, tot[0]);
 }
+
+// Slab-decomposed CG: the scalar steps of Listing 2 on
+// sums that have been all-reduced over the ranks.  Every rank runs this on identical inputs, so alpha, beta, the count and
+// the stopping decision are identical everywhere and nothing is broadcast.
+//   what = 0: after the residual pass      xch = { r.r, f.f }   -> rho, ||f||^2, early exit
+//   what = 1: after the operator           xch = { p.q }        -> alpha (or breakdown)
+//   what = 2: after the residual update    xch = { r.r }        -> count, convergence / maxit, beta, rho
+#ifdef FCG_MAIN_TU   // non-template kernel: defined in fcg.cu only
+__global__ void slab_scalar_kernel(Scalars* sc, int what, const double* xch) {
+    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    if (what == 0) {
+        const double rho = xch[0], fn2 = xch[1];
+        sc->rho = rho; sc->rr = rho; sc->fn2 = fn2; sc->it = 0; sc->alpha = 0.0; sc->beta = 0.0;
+        if (fn2 == 0.0) { sc->zero_u = 1; sc->done = 1; sc->status = ST_OK; sc->rho = 0.0; sc->relres = 0.0; }
+        else {
+            sc->relres = sqrt(rho) / sqrt(fn2);
+            if (sqrt(rho) <= sc->tol * sqrt(fn2)) { sc->done = 1; sc->status = ST_OK; }
+            else if (sc->maxit <= 0) { sc->done = 1; sc->status = ST_NOT_CONVERGED; }
+        }
+    } else if (what == 1) {
+        if (sc->done) return;
+        const double pq = xch[0];
+        sc->pq = pq;
+        if (!(pq > 0.0) || !isfinite(pq)) { sc->status = ST_BREAKDOWN; sc->done = 1; sc->alpha = 0.0; }
+        else sc->alpha = sc->rho / pq;
+    } else {
+        if (sc->done) return;
+        cg_after_rr(sc, xch[0]);
+    }
+}
+#endif
 
 // spectral search length: start value of the recurrence for sum k p^2 -- the first direction is p = r
 template <typename T>

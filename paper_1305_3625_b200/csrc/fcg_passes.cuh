@@ -55,6 +55,7 @@ template <typename T> struct RowFwdArgs {
     double* partial;       // RUPD: [gridDim.x] partial r.r
     int hints;             // L2 eviction-priority hints (FCG_OPT_L2_HINTS bit mask; pipelined passes only)
     unsigned int* tmo;     // pipelined passes: raised when an mbarrier wait gives up (fcg_tma.cuh); = &Scalars::timeout
+    int ntile, astride;    // slab instantiation: row pairs of this rank, and row pairs per column block of ITS T2
 };
 
 template <typename T> struct ColArgs {
@@ -68,6 +69,7 @@ template <typename T> struct ColArgs {
     double* partial;       // ENERGY instantiation: [L/2] partial sums of shat |P|^2, one per column
     int nsm;               // persistent column pass: SMs of the device
     unsigned int* tmo;     // pipelined passes: raised when an mbarrier wait gives up
+    int col0;              // slab instantiation: global number of this launch's first column (spectrum row, packed column 0)
 };
 
 template <typename T> struct RowInvArgs {
@@ -89,6 +91,9 @@ template <typename T> struct RowInvArgs {
     double kappa;                         // form 1, CGF (three launches, reading F1: k in {0, kappa}, vectors zero on broken bonds):
                                           //    p.(I + K G)p = sum p^2 + kappa sum g |P|^2
     unsigned int* tmo;                    // pipelined passes: raised when an mbarrier wait gives up
+    int ntile;                            // slab instantiation: row pairs of this rank
+    double* xch;                          // slab: the pass's grid-wide sums go HERE (device, 2 doubles) and no scalar step follows:
+                                          //       they are this rank's share, to be all-reduced first (fcg_slab_scalar)
 };
 
 template <int A, int B, typename F> FCG_HD void static_for_up(F&& f) {

@@ -81,6 +81,11 @@ struct PassTable {
     cudaError_t (*col2_xform)(const void* args, const void* tensor_map, int inverse, cudaStream_t st);   // stand-alone transforms
     cudaError_t (*t2_export)(const void* T2, void* X, cudaStream_t st);
     cudaError_t (*t2_import)(const void* X, void* T2, cudaStream_t st);
+    // slab-decomposed CG: the three passes on one rank's share -- row pairs [0, ntile) of its own vectors,
+    // `ncols` columns starting at global column col0
+    cudaError_t (*row_fwd2_slab)(const void* args, cudaStream_t st);
+    cudaError_t (*col2_slab)(const void* args, const void* tensor_map, int ncols, cudaStream_t st);
+    cudaError_t (*row_inv2_slab)(const void* args, const void* tensor_map, cudaStream_t st);
     // whole solve as one cooperative kernel (fcg_fused.cuh); fused == 0 when the size has none
     int fused, fused_grid;
     cudaError_t (*fused_solve)(const void* fused_args, cudaStream_t st);

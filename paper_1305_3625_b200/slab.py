@@ -1,0 +1,125 @@
+"""Slab-decomposed CG over several ranks: the ORDER of the library's
+local passes and of the two collectives between them.  No arithmetic of the method happens here -- every vector update,
+transform, dot product and scalar step is a kernel of libfcg (fcg_slab_* in include/fcg.h); this module only sequences them
+and moves the exchange buffers between the ranks:
+
+  * DistComm   one process per GPU (torchrun): torch.distributed all_to_all_single / all_reduce over NCCL on the handle's
+               stream; with the gloo backend (CPU tests) the all-to-all is done with isend / irecv, which gloo does have;
+  * LocalComm  G logical ranks that share one device and one stream (parity tests on the one-GPU pool): the all-to-all is G*G
+               device copies, the all-reduce a sum of G two-element tensors.
+
+Textbook order of Listing 2 per iteration:
+    rows_fwd | all-to-all S->R | unpack, cols, pack | all-to-all R->S | rows_inv | all-reduce | scalar(1) | update_r | all-reduce |
+    scalar(2) | poll
+"""
+from __future__ import annotations
+
+import torch
+
+from . import binding
+
+
+class LocalComm:
+    """Collectives among logical ranks of ONE process: arguments are lists with one tensor per rank."""
+
+    def all_to_all(self, outs, ins):
+        G = len(ins)
+        chunk = ins[0].numel() // G
+        for dst in range(G):
+            for src in range(G):
+                outs[dst][src * chunk:(src + 1) * chunk].copy_(ins[src][dst * chunk:(dst + 1) * chunk])
+
+    def all_reduce(self, xs):
+        total = torch.stack(list(xs)).sum(dim=0)
+        for x in xs:
+            x.copy_(total)
+
+
+class DistComm:
+    """Collectives among the processes of torch.distributed's default group: lists of length one (this process's tensors)."""
+
+    def __init__(self):
+        import torch.distributed as dist
+        self.dist = dist
+        self.world, self.rank = dist.get_world_size(), dist.get_rank()
+        self.native_a2a = dist.get_backend() == "nccl"
+
+    def all_to_all(self, outs, ins):
+        out, inp = outs[0], ins[0]
+        if self.native_a2a:
+            self.dist.all_to_all_single(out, inp)
+            return
+        chunk = inp.numel() // self.world                 # gloo: no all_to_all; the same exchange from point-to-point calls
+        reqs = []
+        for peer in range(self.world):
+            if peer == self.rank:
+                out[peer * chunk:(peer + 1) * chunk].copy_(inp[peer * chunk:(peer + 1) * chunk])
+                continue
+            reqs.append(self.dist.isend(inp[peer * chunk:(peer + 1) * chunk].contiguous(), peer))
+            reqs.append(self.dist.irecv(out[peer * chunk:(peer + 1) * chunk], peer))
+        for r in reqs:
+            r.wait()
+
+    def all_reduce(self, xs):
+        self.dist.all_reduce(xs[0])
+
+
+class SlabRank:
+    """One rank's handle, its rows of k, f, u, and its exchange buffers."""
+
+    def __init__(self, L: int, dtype, nranks: int, rank: int, s_full: torch.Tensor, device="cuda"):
+        self.shape = binding.fcg_slab_shape_of(L, dtype, nranks, rank)
+        self.h = binding.Fcg(L, dtype, device=device)
+        self.h.fcg_set_spectrum(s_full)
+        self.h.fcg_slab_configure(nranks, rank)
+        self.send, self.recv = self.h.fcg_slab_buffers()
+        self.xch = torch.zeros(2, dtype=torch.float64, device=device)
+        self.rows = slice(rank * self.shape["rows_local"], (rank + 1) * self.shape["rows_local"])
+
+    def close(self):
+        self.h.close()
+
+
+def _operator_round_trip(ranks, comm):
+    """S (row transforms of the own rows) -> columns -> S (ready for the inverse row transforms), on every rank."""
+    comm.all_to_all([r.recv for r in ranks], [r.send for r in ranks])
+    for r in ranks:
+        r.h.fcg_slab_unpack(); r.h.fcg_slab_cols(); r.h.fcg_slab_pack()
+    comm.all_to_all([r.send for r in ranks], [r.recv for r in ranks])
+
+
+def slab_solve(ranks, comm, k, f, u, tol: float, maxit: int):
+    """Solve A u = f with the lattice split by rows over `ranks` (all the ranks of this process: one with DistComm, G with
+    LocalComm).  k, f, u: lists, one tensor of the rank's own rows each; u in: initial guess, out: solution.
+    Returns (iters, rel_residual, status) -- identical on every rank."""
+    xs = [r.xch for r in ranks]
+    for r, ui in zip(ranks, u):
+        r.h.fcg_slab_setup(tol, maxit)
+        r.h.fcg_slab_rows_fwd(False, ui)
+    _operator_round_trip(ranks, comm)
+    for r, ki, fi, ui in zip(ranks, k, f, u):
+        r.h.fcg_slab_rows_inv(True, ki, ui, fi, r.xch)          # r = f - A u, p := 0; xch = {r.r, f.f} of the own rows
+    comm.all_reduce(xs)
+    for r in ranks:
+        r.h.fcg_slab_scalar(0, r.xch)
+    while True:
+        done, it, rr, st = ranks[0].h.fcg_slab_poll()           # every rank holds the same scalars; one read-back per iteration
+        if done:
+            break
+        for r, ui in zip(ranks, u):
+            r.h.fcg_slab_rows_fwd(True, ui)                     # u += alpha p (lagged), p = r + beta p, row transforms of p
+        _operator_round_trip(ranks, comm)
+        for r, ki in zip(ranks, k):
+            r.h.fcg_slab_rows_inv(False, ki, None, None, r.xch) # q = k o p + C p; xch[0] = p.q of the own rows
+        comm.all_reduce(xs)
+        for r in ranks:
+            r.h.fcg_slab_scalar(1, r.xch)                       # alpha
+            r.h.fcg_slab_update_r(r.xch)                        # r -= alpha q; xch[0] = r.r of the own rows
+        comm.all_reduce(xs)
+        for r in ranks:
+            r.h.fcg_slab_scalar(2, r.xch)                       # count, convergence, beta
+    for r, ui in zip(ranks, u):
+        r.h.fcg_slab_finish(ui)
+    for r in ranks[1:]:
+        r.h.fcg_slab_poll()
+    return it, rr, st

@@ -1,0 +1,119 @@
+"""Slab-decomposed CG on the GPU: G logical ranks on one device, each with its
+own handle and its own rows of every vector, the exchanges as device copies (slab.LocalComm).  Same parity protocol as
+fcg_solve (tests/test_gpu_parity.py): status equal, count within +-2 of the ORACLE, u element by element at the natural stop or
+at the oracle's count; plus agreement with the undecomposed library solve in the same textbook order."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import api as orc
+from paper_1305_3625_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+TDT = {np.float64: torch.float64, np.float32: torch.float32}
+TOL_CG = {np.float64: 1e-9, np.float32: 1e-4}
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_1305_3625_b200 import binding
+    assert torch.cuda.is_available()
+    binding.lib()
+    return binding
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def rel(a, b):
+    a = np.asarray(a, np.float64).ravel(); b = np.asarray(b, np.float64).ravel()
+    return np.linalg.norm(a - b) / max(np.linalg.norm(b), 1e-300)
+
+
+def slab_run(w, G, tol, maxit, u0=None):
+    from paper_1305_3625_b200 import slab
+    dt = w.dtype.type
+    sd = dev(w.s)
+    ranks = [slab.SlabRank(w.L, TDT[dt], G, g, sd) for g in range(G)]
+    k = [dev(w.k[r.rows]) for r in ranks]; f = [dev(w.f[r.rows]) for r in ranks]
+    u = [dev((w.u0 if u0 is None else u0)[r.rows]) for r in ranks]
+    it, rr, st = slab.slab_solve(ranks, slab.LocalComm(), k, f, u, tol, maxit)
+    out = np.concatenate([x.cpu().numpy() for x in u], axis=0)
+    for r in ranks:
+        r.close()
+    return it, rr, st, out
+
+
+@pytest.mark.parametrize("cfg,L,dt", [(1, 256, np.float64), (2, 512, np.float64), (1, 1024, np.float64), (4, 1024, np.float32),
+                                      (2, 2048, np.float32)])
+@pytest.mark.parametrize("G", [1, 2, 4])
+def test_slab_cg_matches_oracle(B, cfg, L, dt, G):
+    w = inputs.config(cfg, dt, L=L)
+    ref = orc.cg(w.s, w.k, w.f, w.u0, w.tol, w.maxit, history=True)
+    it, rr, st, u = slab_run(w, G, w.tol, w.maxit)
+    assert st == ref["status"] and abs(it - ref["iters"]) <= 2, (it, ref["iters"])
+    d = rel(u, ref["u"])
+    if it != ref["iters"] and d > TOL_CG[dt]:
+        it2, _, _, u = slab_run(w, G, 0.0, ref["iters"])
+        assert it2 == ref["iters"]
+        d = rel(u, ref["u"])
+    assert d <= TOL_CG[dt], (d, it, ref["iters"])
+    assert rr <= w.tol
+    # pinned count a few iterations in, where nothing depends on the stopping decision: a tenth of the tolerance
+    refp = orc.cg(w.s, w.k, w.f, w.u0, 0.0, 5, history=True)
+    itp, rrp, _, up = slab_run(w, G, 0.0, 5)
+    assert itp == 5 and rel(up, refp["u"]) <= 0.1 * TOL_CG[dt]
+    assert abs(rrp - refp["hist"][5]) <= 1e-3 * refp["hist"][5]
+
+
+def test_slab_cg_equals_undecomposed_textbook_order(B):
+    """The undecomposed library solve in the same textbook order (four launches per iteration) and the slab solve with any G do
+    the same arithmetic per element; only the order of the partial sums differs, so the iterates agree to rounding."""
+    w = inputs.config(1, np.float64, L=512)
+    h = B.Fcg(w.L, torch.float64)
+    h.fcg_set_option(B.FCG_OPT_FUSED, 0); h.fcg_set_option(B.FCG_OPT_SPECTRAL_ALPHA, 0)
+    h.fcg_set_spectrum(dev(w.s))
+    u = dev(w.u0)
+    it0, rr0, st0 = h.fcg_solve(dev(w.k), dev(w.f), u, 0.0, 30)
+    u0 = u.cpu().numpy()
+    h.close()
+    for G in (1, 2, 8):
+        it, rr, st, ug = slab_run(w, G, 0.0, 30)
+        assert (it, st) == (it0, st0) and rel(ug, u0) <= 1e-12 and abs(rr - rr0) <= 1e-9 * rr0
+
+
+def test_slab_edge_cases(B):
+    from paper_1305_3625_b200 import slab
+    w = inputs.config(0, np.float64, L=256)
+    # warm start from the solution: zero iterations; maxit = 0; f = 0
+    it, rr, st, u = slab_run(w, 2, w.tol, w.maxit)
+    assert st == 0
+    it2, rr2, st2, _ = slab_run(w, 2, 10 * w.tol, w.maxit, u0=u)
+    assert (it2, st2) == (0, 0)
+    it3, _, st3, u3 = slab_run(w, 4, w.tol, 0)
+    assert (it3, st3) == (0, B.FCG_NOT_CONVERGED) and not u3.any()
+    w.f[:] = 0
+    it4, rr4, st4, u4 = slab_run(w, 2, w.tol, w.maxit, u0=np.ones_like(w.u0))
+    assert (it4, rr4, st4) == (0, 0.0, 0) and not u4.any()
+    # a split that does not divide the column blocks is refused; so is a slab call on an unconfigured handle
+    with pytest.raises(B.FcgError):
+        slab.SlabRank(256, torch.float64, 3, 0, dev(w.s))
+    h = B.Fcg(256, torch.float64)
+    with pytest.raises(B.FcgError):
+        h.fcg_slab_cols()
+    h.close()
+
+
+@pytest.mark.parametrize("dt", [np.float64, np.float32])
+def test_slab_cg_full_size_config2(B, dt):
+    """configs[2] at L = 2048 over four logical ranks: the whole solve against the oracle's own."""
+    w = inputs.config(2, dt)
+    ref = orc.cg(w.s, w.k, w.f, w.u0, w.tol, w.maxit)
+    it, rr, st, u = slab_run(w, 4, w.tol, w.maxit)
+    assert st == 0 and abs(it - ref["iters"]) <= 2
+    d = rel(u, ref["u"])
+    if it != ref["iters"] and d > TOL_CG[dt]:
+        _, _, _, u = slab_run(w, 4, 0.0, ref["iters"])
+        d = rel(u, ref["u"])
+    assert d <= TOL_CG[dt], (d, it, ref["iters"])
