@@ -114,6 +114,18 @@ template <int N> __device__ __forceinline__ void bar_named() { asm volatile("bar
 // (parity green) but not faster: measured L = 2048 fp64 93.7 vs 94.2 us per iteration, and slower where it costs registers
 // (L = 8192 fp32 826 vs 798 us, L = 4096 fp64 379 vs 369 us) -- the stage barriers are not what these kernels wait for.  Default:
 // the cyclic assignment with a CTA barrier after every stage.
+// Column gather by the LSU's asynchronous 16-byte copies (cp.async, SASS LDGSTS) instead of TMA tensor loads, the scatter staying
+// on TMA: built with -DFCG_LSU_GATHER, measured, NOT the default.  Elimination runs (-DFCG_PROBE) show the column pass without
+// its arithmetic at 0.7 ns per gathered / scattered cell whatever the cell's size (L = 2048 fp64: 32-byte cells, 18.0 of 27.1 us;
+// L = 8192 fp32: 16-byte cells, 164 of 218 us), i.e. bound by the rate of small requests, not by HBM bytes.  Moving the gather's
+// requests from the TMA engine to the load/store unit did not help -- L = 2048 fp64 28.4 vs 26.7 us, L = 8192 fp32 241 vs 220 us,
+// parity green either way -- so the limit is not the TMA engine's row rate but the L2 sector rate behind both paths (a 16-byte
+// cell still costs a 32-byte sector).  DESIGN.md section 17.
+#ifdef FCG_LSU_GATHER
+constexpr bool LSU_GATHER = true;
+#else
+constexpr bool LSU_GATHER = false;
+#endif
 #ifdef FCG_GROUPS
 constexpr bool GRP = true;
 #else
@@ -330,24 +342,37 @@ __global__ void __launch_bounds__(P::NT, CTAS) col2_kernel(const ColArgs<T> A, c
     constexpr int ABOX = AS::ABOX;
     constexpr uint32_t BOXB = (uint32_t)(ABOX * 2 * sizeof(cx<T>));
     tma::grid_dep_launch();
+    constexpr bool LG = LSU_GATHER && !SLAB;                      // (the slab instantiation keeps the TMA gather: its T2 has another extent)
     if (lt == 0) {
         tma::prefetch_tmap(&tmap);
-        tma::mbar_init(&bar, 1);
+        tma::mbar_init(&bar, LG ? NT + 1 : 1);
         tma::mbar_init(&ready, NT / 32);
         tma::fence_mbar_init();
     }
     cx<T> wb[S + 1][PM];
     static_for_up<1, S - 1>([&](auto s) { base_tw<P, decltype(s)::value, T, GRP>(lt, A.tw, wb[decltype(s)::value]); });
+    __syncthreads();                                              // the barriers exist before anybody arrives on them
     tma::grid_dep_wait();                                         // everything above overlaps the previous kernel's tail
+    if constexpr (LG) {
+        // column nl: cell (row pair a2) = 2 complex at T2[nl / NB][a2][nl % NB], CB bytes, to natural order in shared memory
+        constexpr int CB = (int)(2 * sizeof(cx<T>)), PIECES = CB / 16;
+        const unsigned char* src = reinterpret_cast<const unsigned char*>(A.Tb + AS::t2_index(nl, 0));
+        constexpr size_t ASTRIDE = (size_t)AS::NB * CB;           // bytes between consecutive row pairs of one column
+#pragma unroll 8
+        for (int i = lt; i < (L / 2) * PIECES; i += NT)
+            tma::cp_async16(smem_raw + (size_t)i * 16, src + (size_t)(i / PIECES) * ASTRIDE + (size_t)(i % PIECES) * 16);
+        tma::cp_async_arrive(&bar);
+    }
     if (lt == 0 && !FCG_PROBE_ON(0x200)) {
-        tma::mbar_expect_tx(&bar, (uint32_t)(AS::WBYTES + (n ? L * sizeof(T) : 0)));
+        tma::mbar_expect_tx(&bar, (uint32_t)((LG ? 0 : AS::WBYTES) + (n ? L * sizeof(T) : 0)));
+        if constexpr (!LG) {
 #pragma unroll
         for (int b = 0; b < (L / 2) / ABOX; ++b)
             tma::tensor_g2s_4d(smem_raw + (size_t)b * BOXB, &tmap, 0, nl % AS::NB, b * ABOX, nl / AS::NB, &bar);
+        }
         if (n) tma::bulk_g2s_hint(sh, A.shat + (size_t)n * L, (uint32_t)(L * sizeof(T)), &bar,
                                   (A.hints & 4) ? tma::policy_evict_first() : tma::policy_evict_normal());   // read once per iteration
     }
-    __syncthreads();
     const bool done = A.sc && A.sc->done;
     if (!FCG_PROBE_ON(0x200)) tma::mbar_wait(&bar, 0, A.tmo);
     if (done) return;
@@ -484,7 +509,7 @@ __global__ void __launch_bounds__(P::NT + 32, CTAS) col2p_kernel(const ColArgs<T
     tma::grid_dep_launch();
     if (lt == 0) {
         tma::prefetch_tmap(&tmap);
-        for (int b = 0; b < 2; ++b) { tma::mbar_init(&full[b], 1); tma::mbar_init(&ready[b], NT / 32); }
+        for (int b = 0; b < 2; ++b) { tma::mbar_init(&full[b], LSU_GATHER ? 33 : 1); tma::mbar_init(&ready[b], NT / 32); }
         tma::fence_mbar_init();
     }
     __syncthreads();
@@ -492,24 +517,40 @@ __global__ void __launch_bounds__(P::NT + 32, CTAS) col2p_kernel(const ColArgs<T
     if (A.sc && A.sc->done) return;                              // before any copy is issued
 
     if (warp == NT / 32) {
-        if (lane == 0) {
-            const uint64_t pol = (A.hints & 4) ? tma::policy_evict_first() : tma::policy_evict_normal();   // spectrum rows: read once per iteration
-            auto gather = [&](int i) {
-                const int n = col_of(i), b = i & 1;
-                unsigned char* Wb = smem_raw + (size_t)b * CP::BUF;
-                if (FCG_PROBE_ON(0x200)) { tma::mbar_arrive(&full[b]); return; }
-                tma::mbar_expect_tx(&full[b], (uint32_t)(AS::WBYTES + (n ? L * sizeof(T) : 0)));
+        // producer warp.  Lane 0 owns the TMA copies (spectrum row in, scatter out); with LSU_GATHER all 32 lanes gather the column
+        // itself with 16-byte asynchronous copies (one arrival each on full[b] when theirs have landed) -- see LSU_GATHER above.
+        const uint64_t pol = (A.hints & 4) ? tma::policy_evict_first() : tma::policy_evict_normal();   // spectrum rows: read once per iteration
+        auto gather = [&](int i) {
+            const int n = col_of(i), b = i & 1;
+            unsigned char* Wb = smem_raw + (size_t)b * CP::BUF;
+            if (FCG_PROBE_ON(0x200)) { if (LSU_GATHER || lane == 0) tma::mbar_arrive(&full[b]); if (LSU_GATHER && lane == 0) tma::mbar_arrive(&full[b]); return; }
+            if constexpr (LSU_GATHER) {
+                constexpr int CB = (int)(2 * sizeof(cx<T>)), PIECES = CB / 16;
+                const unsigned char* src = reinterpret_cast<const unsigned char*>(A.Tb + AS::t2_index(n, 0));
+                constexpr size_t ASTRIDE = (size_t)AS::NB * CB;
+#pragma unroll 8
+                for (int c = lane; c < (L / 2) * PIECES; c += 32)
+                    tma::cp_async16(Wb + (size_t)c * 16, src + (size_t)(c / PIECES) * ASTRIDE + (size_t)(c % PIECES) * 16);
+                tma::cp_async_arrive(&full[b]);
+            }
+            if (lane == 0) {
+                tma::mbar_expect_tx(&full[b], (uint32_t)((LSU_GATHER ? 0 : AS::WBYTES) + (n ? L * sizeof(T) : 0)));
+                if constexpr (!LSU_GATHER) {
 #pragma unroll
-                for (int q = 0; q < (L / 2) / ABOX; ++q)
-                    tma::tensor_g2s_4d(Wb + (size_t)q * BOXB, &tmap, 0, n % AS::NB, q * ABOX, n / AS::NB, &full[b]);
+                    for (int q = 0; q < (L / 2) / ABOX; ++q)
+                        tma::tensor_g2s_4d(Wb + (size_t)q * BOXB, &tmap, 0, n % AS::NB, q * ABOX, n / AS::NB, &full[b]);
+                }
                 if (n) tma::bulk_g2s_hint(Wb + AS::WBYTES, A.shat + (size_t)n * L, (uint32_t)(L * sizeof(T)), &full[b], pol);
-            };
-            if (cnt > 0) gather(0);
-            if (cnt > 1) gather(1);
-            for (int i = 0; i < cnt; ++i) {
-                const int n = col_of(i), b = i & 1;
-                unsigned char* Wb = smem_raw + (size_t)b * CP::BUF;
-                tma::mbar_wait(&ready[b], (uint32_t)((i >> 1) & 1), A.tmo);          // every consumer warp's part of column i is in place
+            }
+        };
+        if (!LSU_GATHER && lane != 0) return;
+        if (cnt > 0) gather(0);
+        if (cnt > 1) gather(1);
+        for (int i = 0; i < cnt; ++i) {
+            const int n = col_of(i), b = i & 1;
+            unsigned char* Wb = smem_raw + (size_t)b * CP::BUF;
+            tma::mbar_wait(&ready[b], (uint32_t)((i >> 1) & 1), A.tmo);          // every consumer warp's part of column i is in place
+            if (lane == 0) {
                 if (!FCG_PROBE_ON(0x400)) {
 #pragma unroll
                 for (int q = 0; q < (L / 2) / ABOX; ++q)
@@ -517,8 +558,9 @@ __global__ void __launch_bounds__(P::NT + 32, CTAS) col2p_kernel(const ColArgs<T
                 }
                 tma::bulk_commit();
                 tma::bulk_wait_read0();                                        // the buffer may be refilled (or the CTA may exit)
-                if (i + 2 < cnt) gather(i + 2);
             }
+            if constexpr (LSU_GATHER) __syncwarp();                            // .. by every lane
+            if (i + 2 < cnt) gather(i + 2);
         }
         return;
     }

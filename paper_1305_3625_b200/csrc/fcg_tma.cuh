@@ -117,6 +117,14 @@ __device__ __forceinline__ void bulk_g2s_hint(void* dst_smem, const void* src_gm
                  "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar)), "l"(policy)
                  : "memory");
 }
+// 16 bytes global -> shared by the LSU's asynchronous copy (LDGSTS): no register staging, not a TMA request.  Completion: the
+// issuing thread calls cp_async_arrive on an mbarrier whose init count includes it (.noinc), which fires once all its copies landed.
+__device__ __forceinline__ void cp_async16(void* dst_smem, const void* src_gmem) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(dst_smem)), "l"(src_gmem) : "memory");
+}
+__device__ __forceinline__ void cp_async_arrive(uint64_t* bar) {
+    asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
 // contiguous shared -> global (bulk async-group completion)
 __device__ __forceinline__ void bulk_s2g(void* dst_gmem, const void* src_smem, uint32_t bytes) {
     asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst_gmem), "r"(smem_u32(src_smem)), "r"(bytes) : "memory");
