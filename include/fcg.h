@@ -82,6 +82,12 @@ typedef enum {
     FCG_OPT_BARRIER_START = 10, /* testing aid: initial value (taken as unsigned 32-bit) of the arrival counter of the cooperative
                                  kernel's grid barrier; default 0.  A value just below 2^32 makes the counter wrap within a few
                                  iterations (the barrier compares modulo 2^32; tests/test_gpu_robustness.py) */
+    FCG_OPT_FFT_DIRECT   = 11, /* 1: fcg_fft_fwd / fcg_fft_inv are two launches, the column pass reading / writing the public layout
+                                 X[m][n] itself (a TMA tensor tile per column for FCG_F64; plain 8-byte accesses for FCG_F32, whose
+                                 row stride is not a multiple of 16 bytes); 0: three launches, a layout kernel between the internal
+                                 T2 and X; -1 (default): two launches where they measured faster -- forward while X is <= 64 MiB
+                                 (it then stays in L2 until the neighbouring columns have completed its sectors), inverse for
+                                 FCG_F64 at every size and for FCG_F32 while X is <= 64 MiB.  Pipelined engine only (L >= 256) */
     FCG_OPT_ENGINE       = 3  /* 0 (default): pipelined TMA passes where the lattice is large enough (L >= 256), classic
                                  passes otherwise; 1: classic passes only (synchronous loads; kept for A/B measurements).
                                  The stored spectrum's layout belongs to the engine: changing the engine after

@@ -106,6 +106,19 @@ struct fcg_handle_s {
     size_t slab_S = 0, slab_R = 0, slab_C = 0, slab_bytes = 0;     // workspace offsets of T2 (rows side), the exchange buffer, T2 (columns side)
     alignas(64) CUtensorMap tmap_row_s;  // S as [L/(2 NB)][Al][128 B]
     alignas(64) CUtensorMap tmap_col_s;  // C as [MBl][L/2][NB][2 complex]
+    alignas(64) CUtensorMap tmap_x;      // FCG_F64: the caller's half spectrum X[m][n] as a tensor of columns (fft_impl; re-encoded when X moves)
+    const void* tmap_x_ptr = nullptr;
+    int fft_pub = -1;                   // FCG_OPT_FFT_DIRECT (-1: automatic)
+    // Automatic rule, from measurements on one B200.  Writing X column by column leaves every 32-byte sector
+    // of X to be completed by the neighbouring column's CTA: fine while X stays in L2 until then (L = 2048 fp64: 67.8 -> 55.5 us),
+    // a read-modify-write storm once it does not (L = 4096 fp64 forward 254 -> 321 us, L = 8192 fp32 509 -> 1508 us).  Reading X
+    // column by column has no such cliff for 16-byte elements (L = 4096 fp64 inverse 241 -> 199 us) but 8-byte elements waste
+    // three quarters of every sector (L = 8192 fp32 inverse 609 -> 1273 us).
+    bool fft_direct(bool inverse) const {
+        if (fft_pub >= 0) return fft_pub != 0;
+        const bool small = N * w <= ((size_t)64 << 20);
+        return inverse ? (dtype == FCG_F64 || small) : small;
+    }
     int device = 0;                     // the device the handle was created on; every entry point runs with it current
     unsigned int barrier_start = 0;     // FCG_OPT_BARRIER_START: initial value of the cooperative kernel's barrier counter
 
@@ -500,9 +513,26 @@ int break_impl(fcg_handle h, void* k, const void* u, const void* t, long long* i
     return h->h_brk->status;
 }
 
+int x_tensor_map(fcg_handle h, const void* X);
+
 template <typename T>
 int fft_impl(fcg_handle h, const void* in, void* out, bool inverse) {
     const int L = h->L;
+    if (h->v2() && h->fft_direct(inverse)) {
+        // two launches: the column pass reads / writes the public layout X[m][n] itself (col2_xpub_kernel)
+        Seq<T> s{h, h->stream};
+        ColArgs<T> CA{}; CA.mode = inverse ? COL_INV : COL_FWD; CA.Tb = s.Tb(); CA.tw = s.tw(); CA.tmo = &h->sc()->timeout;
+        CA.X = (cx<T>*)(inverse ? const_cast<void*>(in) : out);
+        if (sizeof(T) == 8) { const int st = x_tensor_map(h, CA.X); if (st != FCG_OK) return st; }
+        if (!inverse) {
+            FCG_CK(h, s.row_fwd(ROWF_PLAIN, (const T*)in, nullptr));
+            FCG_CK(h, h->tab->col2_xpub(&CA, &h->tmap_col, &h->tmap_x, 0, h->stream)); ++h->launches;
+        } else {
+            FCG_CK(h, h->tab->col2_xpub(&CA, &h->tmap_col, &h->tmap_x, 1, h->stream)); ++h->launches;
+            FCG_CK(h, s.row_inv(ROWI_PLAIN, nullptr, nullptr, nullptr, (T*)out, nullptr));
+        }
+        return FCG_OK;
+    }
     if (h->v2()) {
         // pipelined passes on the T2 layout; T2 <-> public half spectrum X[m][n] by one line-wise permutation kernel
         Seq<T> s{h, h->stream};
@@ -698,6 +728,29 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t,
                                   const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
                                   CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
+// FCG_F64: X[m][n] (L rows of L/2+1 complex) as a 3-D tensor {re/im, n, m}: box = one complex x one column x XBOX rows
+int x_tensor_map(fcg_handle h, const void* X) {
+    if (h->tmap_x_ptr == X) return FCG_OK;
+    if ((reinterpret_cast<uintptr_t>(X) & 15u) != 0) return fail(h, FCG_INVALID_ARG, "X must be 16-byte aligned");
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn || qres != cudaDriverEntryPointSuccess) {
+        cudaGetLastError();
+        return fail(h, FCG_UNSUPPORTED, "cuTensorMapEncodeTiled unavailable");
+    }
+    const cuuint64_t L = (cuuint64_t)h->L, XW = L / 2 + 1;
+    const cuuint64_t gdim[3] = {2, XW, L};
+    const cuuint64_t gstride[2] = {16, XW * 16};
+    const cuuint32_t box[3] = {2u, 1u, (cuuint32_t)(L < 256 ? L : 256)};
+    const cuuint32_t estr[3] = {1u, 1u, 1u};
+    if (reinterpret_cast<EncodeTiledFn>(fn)(&h->tmap_x, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, const_cast<void*>(X), gdim, gstride, box, estr,
+                                            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
+                                            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+        return fail(h, FCG_CUDA_ERROR, "cuTensorMapEncodeTiled (public half spectrum) failed");
+    h->tmap_x_ptr = X;
+    return FCG_OK;
+}
+
 // tensor maps of one rank's two T2 buffers (same boxes as tensor_map_init, other extents)
 int slab_tensor_maps(fcg_handle h) {
     void* fn = nullptr;
@@ -885,6 +938,7 @@ int fcg_set_option(fcg_handle h, int option, int value) {
         case FCG_OPT_SPECTRAL_ALPHA: if (value != 0 && value != 1) return fail(h, FCG_INVALID_ARG, "spectral alpha must be 0 or 1"); h->sl_opt = value; return FCG_OK;
         case FCG_OPT_COL_PERSISTENT: if (value < -1 || value > 1) return fail(h, FCG_INVALID_ARG, "col persistent must be -1, 0 or 1"); h->colp_opt = value; return FCG_OK;
         case FCG_OPT_BARRIER_START: h->barrier_start = (unsigned int)value; return FCG_OK;
+        case FCG_OPT_FFT_DIRECT: if (value < -1 || value > 1) return fail(h, FCG_INVALID_ARG, "fft direct must be -1, 0 or 1"); h->fft_pub = value; return FCG_OK;
         case FCG_OPT_UNROLL: if (value < 1 || value > 64) return fail(h, FCG_INVALID_ARG, "unroll must be 1..64"); h->unroll = value; return FCG_OK;
         case FCG_OPT_ENGINE:
             if (value != 0 && value != 1) return fail(h, FCG_INVALID_ARG, "engine must be 0 or 1");

@@ -750,6 +750,155 @@ __global__ void __launch_bounds__(P::NT, CTAS) col2_xform_kernel(const ColArgs<T
     }
 }
 
+// Column pass of fcg_fft_fwd / fcg_fft_inv that reads / writes the PUBLIC half spectrum X[m][n] (L x (L/2+1), n fastest) itself, so
+// that a stand-alone transform is two launches (row pass + this) instead of three (+ t2_export / t2_import, 2 N w of pure layout
+// traffic).  Column c of T2 is frequency n = freq_of(pos_of_col(c)); its L outputs are the strided column X[.][n]:
+//   * FCG_F64: one complex is 16 bytes and a row of X is 16 (L/2+1) bytes, so the column is a legal TMA tensor tile (xmap: 3-D,
+//     box = 1 complex x 1 column x XBOX rows) -- stored from / loaded into the natural-order column in shared memory;
+//   * FCG_F32: 8-byte elements at a stride that is not a multiple of 16 bytes cannot be a tensor map: plain 8-byte accesses
+//     straight from / to the registers that hold the natural-order column (neighbouring columns run on neighbouring SMs at the
+//     same time, so L2 merges the pieces of a sector);
+//   * column 0 is the packed pair n = 0, L/2 (W = Y0 + i YN): unpacked / packed with its mirror element, plain accesses.
+template <typename T, typename P, int CTAS, int DIR>
+__global__ void __launch_bounds__(P::NT, CTAS) col2_xpub_kernel(const ColArgs<T> A, const __grid_constant__ CUtensorMap tmap,
+                                                                const __grid_constant__ CUtensorMap xmap)
+{
+    using AS = AsyncShape<T, P>;
+    constexpr int L = P::N, S = P::S, NT = P::NT, PM = per_max<P>(), EPT = L / NT, XW = L / 2 + 1;
+    constexpr bool XTMA = sizeof(T) == 8;
+    constexpr int XBOX = L < 256 ? L : 256;
+    extern __shared__ unsigned char smem_dyn[];
+    unsigned char* const smem_raw = align128(smem_dyn);
+    __shared__ __align__(8) uint64_t bar, ready;
+    cx<T>* W = reinterpret_cast<cx<T>*>(smem_raw);
+    SmemIO<T, P> io{W};
+    const int lt = threadIdx.x, c = (int)blockIdx.x;
+    const int n = P::freq_of(AS::pos_of_col(c));                  // 0 for the packed column
+    constexpr int ABOX = AS::ABOX;
+    constexpr uint32_t BOXB = (uint32_t)(ABOX * 2 * sizeof(cx<T>));
+    constexpr uint32_t XBOXB = (uint32_t)(XBOX * sizeof(cx<T>));
+    cx<T>* const X = A.X;
+    if (lt == 0) {
+        tma::prefetch_tmap(&tmap);
+        if (XTMA) tma::prefetch_tmap(&xmap);
+        tma::mbar_init(&bar, 1);
+        tma::mbar_init(&ready, NT / 32);
+        tma::fence_mbar_init();
+        if (DIR < 0) {
+            tma::mbar_expect_tx(&bar, (uint32_t)AS::WBYTES);
+#pragma unroll
+            for (int b = 0; b < (L / 2) / ABOX; ++b)
+                tma::tensor_g2s_4d(smem_raw + (size_t)b * BOXB, &tmap, 0, c % AS::NB, b * ABOX, c / AS::NB, &bar);
+        } else if (XTMA && c != 0) {
+            tma::mbar_expect_tx(&bar, (uint32_t)AS::WBYTES);
+#pragma unroll
+            for (int b = 0; b < L / XBOX; ++b)
+                tma::tensor_g2s_3d(smem_raw + (size_t)b * XBOXB, &xmap, 0, n, b * XBOX, &bar);
+        }
+    }
+    __syncthreads();
+    cx<T> wb[S + 1][PM];
+    static_for_up<1, S - 1>([&](auto s) { base_tw<P, decltype(s)::value, T>(lt, A.tw, wb[decltype(s)::value]); });
+    auto ld_sw = [&](int e) { return io.ld(e); };
+    auto st_sw = [&](int e, cx<T> v) { io.st(e, v); };
+    const T h = (T)0.5;
+    if constexpr (DIR < 0) {
+        tma::mbar_wait(&bar, 0, A.tmo);
+        {   // stage 1: linear in, swizzled out
+            cx<T> a[St<P, 1>::PER][St<P, 1>::R];
+            stage_ld<P, 1, T>(lt, [&](int e) { return W[e]; }, a);
+            __syncthreads();
+            stage_math<P, 1, -1, T>(a, wb[1]);
+            stage_st<P, 1, T>(lt, st_sw, a);
+            __syncthreads();
+        }
+        static_for_up<2, S>([&](auto s) {
+            constexpr int sv = decltype(s)::value;
+            cx<T> a[St<P, sv>::PER][St<P, sv>::R];
+            stage_ld<P, sv, T>(lt, ld_sw, a);
+            stage_math<P, sv, -1, T>(a, wb[sv]);
+            stage_st<P, sv, T>(lt, st_sw, a);
+            __syncthreads();
+        });
+        cx<T> v[EPT];                       // digit-reversed -> natural order m = lt + i NT, in registers
+#pragma unroll
+        for (int i = 0; i < EPT; ++i) v[i] = io.ld(P::pos_of(lt + i * NT));
+        if (c == 0) {                       // packed pair: X[m][0] and X[m][L/2] from Z[m] and its mirror Z[L - m]
+#pragma unroll
+            for (int i = 0; i < EPT; ++i) {
+                const int m = lt + i * NT;
+                const cx<T> a = v[i], b = io.ld(P::pos_of((L - m) % L));
+                X[(size_t)m * XW] = mk<T>((a.x + b.x) * h, (a.y - b.y) * h);
+                X[(size_t)m * XW + L / 2] = mk<T>((a.y + b.y) * h, (b.x - a.x) * h);
+            }
+            return;
+        }
+        if constexpr (!XTMA) {
+#pragma unroll
+            for (int i = 0; i < EPT; ++i) X[(size_t)(lt + i * NT) * XW + n] = v[i];
+            return;
+        } else {
+            __syncthreads();
+#pragma unroll
+            for (int i = 0; i < EPT; ++i) W[lt + i * NT] = v[i];
+            tma::fence_proxy_async();
+            tma::mbar_warp_arrive(&ready);
+            if (lt == 0) {
+                tma::mbar_wait(&ready, 0, A.tmo);
+#pragma unroll
+                for (int b = 0; b < L / XBOX; ++b)
+                    tma::tensor_s2g_3d(&xmap, 0, n, b * XBOX, smem_raw + (size_t)b * XBOXB);
+                tma::bulk_commit();
+                tma::bulk_wait_read0();
+            }
+        }
+    } else {
+        cx<T> v[EPT];                       // natural order in -> digit-reversed positions
+        if (c == 0) {
+#pragma unroll
+            for (int i = 0; i < EPT; ++i) {
+                const int m = lt + i * NT;
+                const cx<T> x0 = X[(size_t)m * XW], xN = X[(size_t)m * XW + L / 2];
+                v[i] = mk<T>(x0.x - xN.y, x0.y + xN.x);
+            }
+        } else if constexpr (!XTMA) {
+#pragma unroll
+            for (int i = 0; i < EPT; ++i) v[i] = X[(size_t)(lt + i * NT) * XW + n];
+        } else {
+            tma::mbar_wait(&bar, 0, A.tmo);
+#pragma unroll
+            for (int i = 0; i < EPT; ++i) v[i] = W[lt + i * NT];
+            __syncthreads();
+        }
+#pragma unroll
+        for (int i = 0; i < EPT; ++i) io.st(P::pos_of(lt + i * NT), v[i]);
+        __syncthreads();
+        static_for_down<S, 2>([&](auto s) {
+            constexpr int sv = decltype(s)::value;
+            cx<T> a[St<P, sv>::PER][St<P, sv>::R];
+            stage_ld<P, sv, T>(lt, ld_sw, a);
+            stage_math<P, sv, +1, T>(a, wb[sv]);
+            stage_st<P, sv, T>(lt, st_sw, a);
+            __syncthreads();
+        });
+        cx<T> a[St<P, 1>::PER][St<P, 1>::R];
+        stage_ld<P, 1, T>(lt, ld_sw, a);
+        stage_math<P, 1, +1, T>(a, wb[1]);
+        __syncthreads();
+        stage_st<P, 1, T>(lt, [&](int e, cx<T> x) { W[e] = x; }, a);
+        tma::fence_proxy_async();
+        tma::mbar_warp_arrive(&ready);
+        if (lt == 0) {
+            tma::mbar_wait(&ready, 0, A.tmo);
+#pragma unroll
+            for (int b = 0; b < (L / 2) / ABOX; ++b)
+                tma::tensor_s2g_4d(&tmap, 0, c % AS::NB, b * ABOX, c / AS::NB, smem_raw + (size_t)b * BOXB);
+            tma::bulk_commit();
+            tma::bulk_wait_read0();
+        }
+    }
+}
+
 // T2 (columns in position order, row frequencies m in natural order after col2_xform<-1>) -> public half spectrum
 // X[m][n], n = 0 .. L/2.  One CTA per row pair (m = 2A, 2A+1): its L complex numbers are whole 128-byte lines of T2; they are
 // permuted to frequency order through shared memory and leave as two contiguous rows.  The packed column 0 (W = Y0 + i YN)

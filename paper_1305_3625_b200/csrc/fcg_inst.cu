@@ -61,6 +61,8 @@ template <typename T> struct Inst {
             if ((e = prep(row_inv2_kernel<T, P, C_INV, 4>, AS::inv_smem)) != cudaSuccess) return e;
             if ((e = prep(col2_xform_kernel<T, P, C_COL, -1>, AS::WBYTES + 128)) != cudaSuccess) return e;
             if ((e = prep(col2_xform_kernel<T, P, C_COL, +1>, AS::WBYTES + 128)) != cudaSuccess) return e;
+            if ((e = prep(col2_xpub_kernel<T, P, C_COL, -1>, AS::WBYTES + 128)) != cudaSuccess) return e;
+            if ((e = prep(col2_xpub_kernel<T, P, C_COL, +1>, AS::WBYTES + 128)) != cudaSuccess) return e;
             if ((e = prep(t2_export_kernel<T, P>, AS::WBYTES + 1024)) != cudaSuccess) return e;
             if ((e = prep(t2_import_kernel<T, P>, AS::WBYTES + 1024)) != cudaSuccess) return e;
         }
@@ -192,6 +194,17 @@ template <typename T> struct Inst {
         }
         return cudaErrorInvalidValue;
     }
+    static cudaError_t col2_xpub(const void* args, const void* tensor_map, const void* x_map, int inverse, cudaStream_t st) {
+        if constexpr (V2) {
+            const ColArgs<T>& A = *static_cast<const ColArgs<T>*>(args);
+            const CUtensorMap& tm = *static_cast<const CUtensorMap*>(tensor_map);
+            const CUtensorMap& xm = *static_cast<const CUtensorMap*>(x_map);
+            if (inverse) col2_xpub_kernel<T, P, C_COL, +1><<<L / 2, P::NT, AS::WBYTES + 128, st>>>(A, tm, xm);
+            else col2_xpub_kernel<T, P, C_COL, -1><<<L / 2, P::NT, AS::WBYTES + 128, st>>>(A, tm, xm);
+            return cudaGetLastError();
+        }
+        return cudaErrorInvalidValue;
+    }
     static cudaError_t t2_export(const void* T2, void* X, cudaStream_t st) {
         if constexpr (V2) {
             t2_export_kernel<T, P><<<L / 2, 256, AS::WBYTES + 1024, st>>>(static_cast<const cx<T>*>(T2), static_cast<cx<T>*>(X));
@@ -286,7 +299,7 @@ template <typename T> struct Inst {
         t.colp_ok = COLP ? 1 : 0; t.colp_ctas = COLP ? CPS::CTAS : 0; t.col2p = &col2p;
         t.sl_ok = SL ? 1 : 0; t.col2_energy = &col2_energy; t.row_inv2_cgf = &row_inv2_cgf; t.row_inv2_cgf_force = &row_inv2_cgf_force;
         t.row_fwd2_slab = &row_fwd2_slab; t.col2_slab = &col2_slab; t.row_inv2_slab = &row_inv2_slab;
-        t.col2_xform = &col2_xform; t.t2_export = &t2_export; t.t2_import = &t2_import;
+        t.col2_xform = &col2_xform; t.col2_xpub = &col2_xpub; t.t2_export = &t2_export; t.t2_import = &t2_import;
         t.fused = FS::valid ? 1 : 0; t.fused_grid = FS::G; t.fused_solve = &fused_solve;
         t.init = &init; t.row_fwd = &row_fwd; t.col = &col; t.row_inv = &row_inv; t.spectrum_prep = &spectrum_prep;
         return t;

@@ -79,6 +79,7 @@ struct PassTable {
     cudaError_t (*row_fwd2_rupd)(const void* args, cudaStream_t st);                                // PCG: r update + r.r + row transforms of r
     cudaError_t (*row_inv2_pre)(const void* args, const void* tensor_map, cudaStream_t st);        // PCG: z = M^-1 r, r.z
     cudaError_t (*col2_xform)(const void* args, const void* tensor_map, int inverse, cudaStream_t st);   // stand-alone transforms
+    cudaError_t (*col2_xpub)(const void* args, const void* tensor_map, const void* x_map, int inverse, cudaStream_t st);   // .. straight to / from X[m][n]
     cudaError_t (*t2_export)(const void* T2, void* X, cudaStream_t st);
     cudaError_t (*t2_import)(const void* X, void* T2, cudaStream_t st);
     // slab-decomposed CG: the three passes on one rank's share -- row pairs [0, ntile) of its own vectors,

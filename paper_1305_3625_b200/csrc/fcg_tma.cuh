@@ -177,6 +177,11 @@ __device__ __forceinline__ void tensor_s2g_4d(const void* tmap, int c0, int c1, 
                  "r"(c2), "r"(c3), "r"(smem_u32(src_smem))
                  : "memory");
 }
+__device__ __forceinline__ void tensor_s2g_3d(const void* tmap, int c0, int c1, int c2, const void* src_smem) {
+    asm volatile("cp.async.bulk.tensor.3d.global.shared::cta.tile.bulk_group [%0, {%1, %2, %3}], [%4];" ::"l"(tmap), "r"(c0), "r"(c1), "r"(c2),
+                 "r"(smem_u32(src_smem))
+                 : "memory");
+}
 __device__ __forceinline__ void prefetch_tmap(const void* tmap) {
     asm volatile("prefetch.tensormap [%0];" ::"l"(tmap) : "memory");
 }

@@ -57,16 +57,20 @@ def handle(B, L, dt, s=None, **opts):
 @pytest.mark.parametrize("dt", [np.float64, np.float32])
 def test_fft_forward_and_round_trip(B, L, dt):
     x = inputs.fft_field(L).astype(dt)
-    h = handle(B, L, dt)
-    X = h.fcg_fft_fwd(dev(x))
     X_or = orc.fft2(x)[:, : L // 2 + 1]
-    assert rel(X.cpu().numpy(), X_or) <= TOL_FFT[dt]
-    back = h.fcg_fft_inv(X)
-    assert rel(back.cpu().numpy(), x) <= TOL_FFT[dt]
-    # the inverse alone, fed with the oracle's spectrum
-    x2 = h.fcg_fft_inv(dev(np.ascontiguousarray(X_or)))
-    assert rel(x2.cpu().numpy(), x) <= TOL_FFT[dt]
-    h.close()
+    outs = []
+    for direct in (1, 0):          # two launches (the column pass on the public layout itself) / three (layout kernel); same below L = 256
+        h = handle(B, L, dt, FCG_OPT_FFT_DIRECT=direct)
+        X = h.fcg_fft_fwd(dev(x))
+        assert rel(X.cpu().numpy(), X_or) <= TOL_FFT[dt], direct
+        back = h.fcg_fft_inv(X)
+        assert rel(back.cpu().numpy(), x) <= TOL_FFT[dt], direct
+        # the inverse alone, fed with the oracle's spectrum
+        x2 = h.fcg_fft_inv(dev(np.ascontiguousarray(X_or)))
+        assert rel(x2.cpu().numpy(), x) <= TOL_FFT[dt], direct
+        outs.append((X.cpu().numpy(), back.cpu().numpy()))
+        h.close()
+    assert np.array_equal(outs[0][0], outs[1][0]) and np.array_equal(outs[0][1], outs[1][1])     # the same arithmetic, another route to memory
 
 
 @pytest.mark.parametrize("L,dt", [(4096, np.float64), (8192, np.float32), (4096, np.float32), (8192, np.float64)])
