@@ -88,6 +88,10 @@ typedef enum {
                                  T2 and X; -1 (default): two launches where they measured faster -- forward while X is <= 64 MiB
                                  (it then stays in L2 until the neighbouring columns have completed its sectors), inverse for
                                  FCG_F64 at every size and for FCG_F32 while X is <= 64 MiB.  Pipelined engine only (L >= 256) */
+    FCG_OPT_FUSED_TWO    = 12, /* 1 (default): the one-launch kernel of FCG_OPT_FUSED runs un-preconditioned CG with TWO grid barriers per
+                                 iteration: it transforms the residual instead of the direction and carries the row-transformed
+                                 direction by the recurrence of Listing 2 (F_row p' = F_row r' + beta F_row p, exact in exact
+                                 arithmetic); 0: three barriers, the direction itself is transformed */
     FCG_OPT_ENGINE       = 3  /* 0 (default): pipelined TMA passes where the lattice is large enough (L >= 256), classic
                                  passes otherwise; 1: classic passes only (synchronous loads; kept for A/B measurements).
                                  The stored spectrum's layout belongs to the engine: changing the engine after

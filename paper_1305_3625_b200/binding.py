@@ -23,6 +23,7 @@ FCG_OPT_SPECTRAL_ALPHA = 8
 FCG_OPT_COL_PERSISTENT = 9
 FCG_OPT_BARRIER_START = 10
 FCG_OPT_FFT_DIRECT = 11
+FCG_OPT_FUSED_TWO = 12
 
 EXPORTS = ["fcg_workspace_bytes", "fcg_create", "fcg_destroy", "fcg_set_option", "fcg_set_spectrum", "fcg_apply",
            "fcg_solve", "fcg_solve_host", "fcg_profile_iteration", "fcg_fft_fwd", "fcg_fft_inv", "fcg_break_step", "fcg_fracture",

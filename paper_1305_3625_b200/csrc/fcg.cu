@@ -121,6 +121,7 @@ struct fcg_handle_s {
     }
     int device = 0;                     // the device the handle was created on; every entry point runs with it current
     unsigned int barrier_start = 0;     // FCG_OPT_BARRIER_START: initial value of the cooperative kernel's barrier counter
+    int fused_two = 1;                  // FCG_OPT_FUSED_TWO: plain CG in the one-launch kernel with two grid barriers per iteration
 
     template <typename U> U* at(size_t off) const { return reinterpret_cast<U*>(ws + off); }
     Scalars* sc() const { return at<Scalars>(lay.scalars); }
@@ -207,6 +208,7 @@ cudaError_t fused_launch(fcg_handle h, FusedArgs& A) {
     cudaError_t e = cudaMemsetAsync(h->sc(), 0, sizeof(Scalars), h->stream);
     if (e != cudaSuccess) return e;
     A.counter_start = h->barrier_start;
+    A.two = h->fused_two;
     if (h->barrier_start != 0u &&
         (e = cudaMemcpyAsync(A.counter, &h->barrier_start, sizeof(unsigned int), cudaMemcpyHostToDevice, h->stream)) != cudaSuccess) return e;
     return h->tab->fused_solve(&A, h->stream);
@@ -939,6 +941,7 @@ int fcg_set_option(fcg_handle h, int option, int value) {
         case FCG_OPT_COL_PERSISTENT: if (value < -1 || value > 1) return fail(h, FCG_INVALID_ARG, "col persistent must be -1, 0 or 1"); h->colp_opt = value; return FCG_OK;
         case FCG_OPT_BARRIER_START: h->barrier_start = (unsigned int)value; return FCG_OK;
         case FCG_OPT_FFT_DIRECT: if (value < -1 || value > 1) return fail(h, FCG_INVALID_ARG, "fft direct must be -1, 0 or 1"); h->fft_pub = value; return FCG_OK;
+        case FCG_OPT_FUSED_TWO: if (value != 0 && value != 1) return fail(h, FCG_INVALID_ARG, "fused two must be 0 or 1"); h->fused_two = value; return FCG_OK;
         case FCG_OPT_UNROLL: if (value < 1 || value > 64) return fail(h, FCG_INVALID_ARG, "unroll must be 1..64"); h->unroll = value; return FCG_OK;
         case FCG_OPT_ENGINE:
             if (value != 0 && value != 1) return fail(h, FCG_INVALID_ARG, "engine must be 0 or 1");

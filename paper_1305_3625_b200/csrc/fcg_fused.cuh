@@ -38,6 +38,7 @@ struct FusedArgs {
     // force formulation (I + K G) f = K D (eq. (2)): u holds the bond forces, f is not read
     // (b = k * D is formed in shared memory), out_ratio[step] = the winning f/t of the break step (may be nullptr)
     int form; double D; double* out_ratio;
+    int two;                                    // plain CG (mhat == nullptr, form != 1): 1 = the two-barrier iteration (TWO instantiation)
 };
 
 template <typename T, typename P> struct FusedShape {
@@ -48,6 +49,8 @@ template <typename T, typename P> struct FusedShape {
     static constexpr size_t WBYTES = (size_t)L * 2 * sizeof(T);
     static constexpr size_t VBYTES = (size_t)2 * L * sizeof(T);  // one vector's two rows
     static constexpr size_t smem = WBYTES + (size_t)TPC * 7 * VBYTES + 128;     // k f u r p q t
+    static constexpr size_t smem_two = smem;     // TWO keeps the own columns of the row-transformed direction in q's slot
+    static_assert(WBYTES == VBYTES, "a column of T is as large as a vector's two rows");
 };
 
 #ifdef __CUDACC__
@@ -94,9 +97,18 @@ __device__ __forceinline__ bool grid_barrier(unsigned int* counter, unsigned int
 // FORCE = 2: the force model through the displacements (reading F7): the arithmetic of FORCE = 0 (spectral
 // search length, optional preconditioner) on (K + G^-1) u = K D, with b = K D re-formed in shared memory at every step and the
 // break rule of the force model, f_i / t_i with f_i = k_i (D - u_i) by eq. (1a); u is not touched by the break.
-template <typename T, typename P, int FORCE = 0>
+// TWO = true (plain CG only: FORCE = 0 or 2, no preconditioner): TWO grid barriers per iteration instead of three.  The row
+// transforms are linear, so the row-transformed direction obeys the recurrence of Listing 2 itself: with p' = r' + beta p,
+//     F_row p' = F_row r' + beta F_row p.
+// Each CTA keeps its own columns of F_row p in shared memory (Pc) and transforms the RESIDUAL instead of the direction, which it
+// can do as soon as it has formed its rows of r' -- before beta is known -- so that the barrier of the r.r sum is also the
+// barrier that completes T:   .. -> rows_inverse: u, r' -> row transforms of r' -> [sum r.r | T complete] -> beta, p' (real
+// space, for k o p and u), columns: Pc = T + beta Pc, column transforms, energy -> [sum p.Ap] -> alpha -> rows_inverse ..
+// The recurrence starts afresh with every solve (p = 0), so its rounding does not accumulate over a quasi-static loop.
+template <typename T, typename P, int FORCE = 0, bool TWO = false>
 __global__ void __launch_bounds__(P::NT) cg_fused_kernel(const FusedArgs A)
 {
+    static_assert(!TWO || FORCE != 1, "the two-barrier iteration is for the displacement form");
     constexpr bool FQ = FORCE == 1, FD = FORCE == 2;
     using AS = AsyncShape<T, P>;
     using FS = FusedShape<T, P>;
@@ -109,6 +121,8 @@ __global__ void __launch_bounds__(P::NT) cg_fused_kernel(const FusedArgs A)
     __shared__ int ok_smem;
     cx<T>* W = reinterpret_cast<cx<T>*>(smem_raw);
     T* const vecs = reinterpret_cast<T*>(smem_raw + FS::WBYTES);
+    // TWO: the own columns of F_row p live in the slot of q (vector 5), which plain CG never stores: L complex = two real rows
+    auto PcOf = [&](int j) { return reinterpret_cast<cx<T>*>(vecs + ((size_t)(j * 7 + 5) * 2) * L); };
     // vector v (0 k, 1 f, 2 u, 3 r, 4 p, 5 q, 6 t) of own tile j, row r (0/1)
     auto V = [&](int j, int v, int r) { return vecs + ((size_t)(j * 7 + v) * 2 + r) * L; };
     SmemIO<T, P> io{W};
@@ -217,11 +231,24 @@ __global__ void __launch_bounds__(P::NT) cg_fused_kernel(const FusedArgs A)
         }
     };
     // phase C: own columns, in place: forward, spectral multiply, inverse
-    auto columns = [&](const T* spec, double* en) {      // en != nullptr: *en += this CTA's share of sum spec |P|^2
-        for (int j = 0; j < TPC; ++j) {
+    auto columns = [&](const T* spec, double* en, bool recur = false, T rb = (T)0) {      // en != nullptr: *en += this CTA's share of sum spec |P|^2
+        for (int j = 0; j < TPC; ++j) {                     // recur (TWO): the column is T + rb * Pc, and becomes the new Pc
             const int m = cta + j * G;
             cx<T>* col = Tf + (size_t)m * L;
-            for (int e = lt; e < L; e += NT) W[e] = __ldcg(col + e);
+            if constexpr (TWO) {
+                cx<T>* pc = PcOf(j);
+                if (recur) {
+                    for (int e = lt; e < L; e += NT) {
+                        const cx<T> t = __ldcg(col + e), o = pc[e];
+                        const cx<T> v = mk<T>(t.x + rb * o.x, t.y + rb * o.y);
+                        pc[e] = v; W[e] = v;
+                    }
+                } else {
+                    for (int e = lt; e < L; e += NT) W[e] = __ldcg(col + e);
+                }
+            } else {
+                for (int e = lt; e < L; e += NT) W[e] = __ldcg(col + e);
+            }
             __syncthreads();
             {
                 cx<T> a[St<P, 1>::PER][St<P, 1>::R];
@@ -373,6 +400,7 @@ __global__ void __launch_bounds__(P::NT) cg_fused_kernel(const FusedArgs A)
         for (int j = 0; j < TPC; ++j) {
             T* pp = V(j, 4, 0);
             for (int e = lt; e < 2 * L; e += NT) pp[e] = (T)0;
+            if constexpr (TWO) { cx<T>* pc = PcOf(j); for (int e = lt; e < L; e += NT) pc[e] = mk<T>((T)0, (T)0); }
         }
         if (FORCE != 0) {                                   // right-hand side b = K D (eq. (2)), one multiply in the working precision
             const T dv = (T)A.D;
@@ -386,6 +414,87 @@ __global__ void __launch_bounds__(P::NT) cg_fused_kernel(const FusedArgs A)
         double beta = 0.0;
         T al_u = (T)0;                                 // FORCE: the search length between phases Q and U
         int phase = (have_fn && FORCE == 0) ? PH_RESID : PH_FN;
+        if constexpr (TWO) {
+            // FN (||f||^2 where not known yet; row transforms of u) -> RESID (r = f - A u; row transforms of r) -> Q -> Q -> ..
+            // every phase ends with the row transforms of the NEXT operand and the grid-wide sum whose barrier also completes T
+            const bool need_fn = phase == PH_FN;
+            phase = PH_FN;
+            while (true) {
+                double acc = 0.0, kpp = 0.0;
+                bool bd = false;
+                if (phase == PH_FN) {
+                    if (need_fn)
+                        for (int j = 0; j < TPC; ++j) {
+                            const T* ff = V(j, 1, 0);
+                            for (int e = lt; e < 2 * L; e += NT) acc += (double)ff[e] * (double)ff[e];
+                        }
+                } else {
+                    if (phase == PH_Q) {                    // update calculation variables: new direction (98); sum k p^2 on the way
+                        for (int j = 0; j < TPC; ++j) {
+                            const T* dv = V(j, 3, 0); T* pp = V(j, 4, 0); const T* kk = V(j, 0, 0);
+                            const T b = (T)beta;
+                            for (int e = lt; e < 2 * L; e += NT) {
+                                const T pn = dv[e] + b * pp[e];
+                                pp[e] = pn;
+                                kpp += (double)kk[e] * ((double)pn * (double)pn);
+                            }
+                        }
+                        __syncthreads();
+                    }
+                    double en = 0.0;
+                    columns(shat, phase == PH_Q ? &en : nullptr, phase == PH_Q, (T)beta);
+                    double* ps = A.partial + (size_t)slot * G;
+                    if (phase == PH_Q) {                    // this CTA's share of p.Ap = sum k p^2 + sum shat |P|^2
+                        const double mine = cta_sum(kpp + en);
+                        if (lt == 0) ps[cta] = mine;
+                    }
+                    ok = grid_barrier(A.counter, target, G, &ok_smem) && ok;
+                    T al = (T)0;
+                    if (phase == PH_Q) {                    // search length (94): every CTA adds the G shares in the same order
+                        const double v = sum_partials(ps);
+                        slot = (slot + 1) & 3;
+                        const double pq = cta_sum(v);
+                        if (!(pq > 0.0) || !isfinite(pq)) bd = true;
+                        else al = (T)(rho / pq);
+                    }
+                    if (!bd) rows_inverse([&](int j, int e, T c0, T c1) {
+                        const T* kk = V(j, 0, 0); T* uu = V(j, 2, 0); T* rv = V(j, 3, 0);
+                        if (phase == PH_RESID) {                              // r = f - (k o u + C u)
+                            const T* ff = V(j, 1, 0);
+                            const T r0 = ff[e] - (kk[e] * uu[e] + c0), r1 = ff[L + e] - (kk[L + e] * uu[L + e] + c1);
+                            rv[e] = r0; rv[L + e] = r1;
+                            acc += (double)r0 * (double)r0; acc += (double)r1 * (double)r1;
+                        } else {                        // q = k o p + C p; new x (95), residue (96), residue length (97)
+                            const T* pp = V(j, 4, 0);
+                            const T p0 = pp[e], p1 = pp[L + e];
+                            const T q0 = kk[e] * p0 + c0, q1 = kk[L + e] * p1 + c1;
+                            uu[e] = uu[e] + al * p0; uu[L + e] = uu[L + e] + al * p1;
+                            const T r0 = rv[e] - al * q0, r1 = rv[L + e] - al * q1;
+                            rv[e] = r0; rv[L + e] = r1;
+                            acc += (double)r0 * (double)r0; acc += (double)r1 * (double)r1;
+                        }
+                    });
+                }
+                if (bd) { status = ST_BREAKDOWN; break; }
+                __syncthreads();                            // the epilogue's writes to r (u) are in place for every thread
+                rows_forward(phase == PH_FN ? 2 : 3);       // u for the residual pass, else the residual just formed
+                const double s0 = grid_sum(acc, okb); ok = ok && okb;
+                if (!ok) { status = -3; break; }
+                if (phase == PH_FN) { if (need_fn) { fn2 = s0; have_fn = true; } phase = PH_RESID; }
+                else if (phase == PH_RESID) {
+                    rr = s0; rho = rr;
+                    if (fn2 == 0.0) { zero_u = true; rho = 0.0; rr = 0.0; break; }
+                    if (sqrt(rr) <= A.tol * sqrt(fn2)) break;
+                    if (A.maxit <= 0) { status = ST_NOT_CONVERGED; break; }
+                    phase = PH_Q;
+                } else {
+                    rr = s0; ++it;
+                    if (sqrt(rr) <= A.tol * sqrt(fn2)) { rho = rr; break; }                         // check convergence (99)
+                    if (it >= A.maxit) { rho = rr; status = ST_NOT_CONVERGED; break; }
+                    beta = rr / rho; rho = rr;
+                }
+            }
+        } else
         while (true) {
             double acc = 0.0, kpp = 0.0;
             bool bd = false;

@@ -70,6 +70,8 @@ template <typename T> struct Inst {
             if ((e = prep(cg_fused_kernel<T, P>, FS::smem)) != cudaSuccess) return e;
             if ((e = prep(cg_fused_kernel<T, P, 1>, FS::smem)) != cudaSuccess) return e;
             if ((e = prep(cg_fused_kernel<T, P, 2>, FS::smem)) != cudaSuccess) return e;
+            if ((e = prep(cg_fused_kernel<T, P, 0, true>, FS::smem_two)) != cudaSuccess) return e;
+            if ((e = prep(cg_fused_kernel<T, P, 2, true>, FS::smem_two)) != cudaSuccess) return e;
         }
         return prep(col_kernel<T, P, CS::COLS>, CS::smem);
     }
@@ -224,9 +226,11 @@ template <typename T> struct Inst {
         if constexpr (FS::valid) {
             FusedArgs A = *static_cast<const FusedArgs*>(fused_args);
             void* params[] = {&A};
-            const void* fn = A.form == 1 ? (const void*)cg_fused_kernel<T, P, 1> : A.form == 2 ? (const void*)cg_fused_kernel<T, P, 2>
-                                                                                         : (const void*)cg_fused_kernel<T, P>;
-            return cudaLaunchCooperativeKernel(fn, dim3(FS::G), dim3(P::NT), params, FS::smem, st);
+            const bool two = A.two && A.mhat == nullptr && A.form != 1;        // plain CG: two grid barriers per iteration
+            const void* fn = A.form == 1 ? (const void*)cg_fused_kernel<T, P, 1>
+                             : A.form == 2 ? (two ? (const void*)cg_fused_kernel<T, P, 2, true> : (const void*)cg_fused_kernel<T, P, 2>)
+                                           : (two ? (const void*)cg_fused_kernel<T, P, 0, true> : (const void*)cg_fused_kernel<T, P>);
+            return cudaLaunchCooperativeKernel(fn, dim3(FS::G), dim3(P::NT), params, two ? FS::smem_two : FS::smem, st);
         }
         return cudaErrorInvalidValue;
     }
