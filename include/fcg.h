@@ -276,12 +276,12 @@ int fcg_force_fracture(fcg_handle h, void* k, double D, void* f, const void* t, 
  * row pairs [g L/2G, (g+1) L/2G).  The row passes are local.  The column pass needs whole columns, so the half spectrum is
  * transposed between the ranks before and after it: rank g ends up with the columns [g L/2G, (g+1) L/2G) (whole 128-byte lines of
  * T2: L/(2 NB G) column blocks of NB columns), and the two scalars of Listing 2 (p.q and r.r) are sums over the ranks.
- * The library provides the local passes, the (un)packing around the exchange and the scalar steps; the CALLER runs the two
+ * The library provides the local passes and the scalar steps; the CALLER runs the two
  * collectives -- an all-to-all with equal chunks on the send / receive buffers and an all-reduce (sum) on a device buffer of two
  * doubles -- with whatever connects the ranks (torch.distributed over NCCL in paper_1305_3625_b200/slab.py; plain copies when
  * several logical ranks share one device).  One handle per rank (fcg_create on the rank's device, then fcg_slab_configure);
  * fcg_set_spectrum takes the full L x L spectrum on every rank.  Textbook order of Listing 2, one iteration =
- *     rows_fwd(cg) | all-to-all S->R | unpack, cols, pack | all-to-all R->S | rows_inv -> xch | all-reduce | scalar(1) |
+ *     rows_fwd(cg) | all-to-all S->R | cols (on R, in place) | all-to-all R->S | rows_inv -> xch | all-reduce | scalar(1) |
  *     update_r -> xch | all-reduce | scalar(2) | poll
  * Every rank computes alpha, beta, the count and the stopping decision itself from the all-reduced sums: identical everywhere.
  *
@@ -294,8 +294,9 @@ int fcg_force_fracture(fcg_handle h, void* k, double D, void* f, const void* t, 
  *   fcg_slab_setup      reset the scalar block: tol, maxit (before fcg_slab_rows_inv(residual = 1))
  *   fcg_slab_rows_fwd   cg = 0: row transforms of the own rows of xu (an input vector) into S;  cg = 1: u += alpha p (lagged one
  *                       pass), p = r + beta p, row transforms of p into S (xu = the own rows of u, updated in place)
- *   fcg_slab_unpack     R -> C, the own columns in the layout the column pass reads;   fcg_slab_pack  C -> R
- *   fcg_slab_cols       column pass on C in place: F^H (shat o F .) of the own columns
+ *   fcg_slab_cols       column pass on R in place: F^H (shat o F .) of the own columns.  R is read and written where the all-to-all
+ *                       left it / will take it -- [source rank][local column block][local row pair][line] -- through a 5-D tensor map,
+ *                       so nothing is repacked around the exchange.  Returns at once when the solve has finished.
  *   fcg_slab_rows_inv   inverse row transforms of S;  residual = 1: r = f - (k o u + C u), p := 0, xch = { r.r, f.f } of the own rows;
  *                       residual = 0: q = k o p + C p, xch[0] = p.q of the own rows.  xch: device, 2 doubles, caller-owned
  *   fcg_slab_update_r   r -= alpha q on the own rows, xch[0] = their r.r
@@ -321,8 +322,6 @@ int fcg_slab_configure(fcg_handle h, int nranks, int rank);
 int fcg_slab_buffers(fcg_handle h, size_t* send_offset, size_t* recv_offset, size_t* bytes);
 int fcg_slab_setup(fcg_handle h, double tol, int maxit);
 int fcg_slab_rows_fwd(fcg_handle h, int cg, void* xu);
-int fcg_slab_unpack(fcg_handle h);
-int fcg_slab_pack(fcg_handle h);
 int fcg_slab_cols(fcg_handle h);
 int fcg_slab_rows_inv(fcg_handle h, int residual, const void* k, const void* u, const void* f, void* xch);
 int fcg_slab_update_r(fcg_handle h, void* xch);

@@ -33,8 +33,7 @@ EXPORTS = ["fcg_workspace_bytes", "fcg_create", "fcg_destroy", "fcg_set_option",
            "fcg_green_function", "fcg_kernel_spectrum", "fcg_force_apply", "fcg_force_solve", "fcg_force_break_step",
            "fcg_force_fracture", "fcg_inverse_spectrum", "fcg_force_rhs", "fcg_force_from_displacement",
            "fcg_force_fracture_displacement", "fcg_force_fracture_displacement_begin", "fcg_force_fracture_displacement_end",
-           "fcg_slab_shape_of", "fcg_slab_configure", "fcg_slab_buffers", "fcg_slab_setup", "fcg_slab_rows_fwd", "fcg_slab_unpack",
-           "fcg_slab_pack", "fcg_slab_cols", "fcg_slab_rows_inv", "fcg_slab_update_r", "fcg_slab_scalar", "fcg_slab_finish", "fcg_slab_poll"]
+           "fcg_slab_shape_of", "fcg_slab_configure", "fcg_slab_buffers", "fcg_slab_setup", "fcg_slab_rows_fwd", "fcg_slab_cols", "fcg_slab_rows_inv", "fcg_slab_update_r", "fcg_slab_scalar", "fcg_slab_finish", "fcg_slab_poll"]
 
 
 class SlabShape(C.Structure):
@@ -99,8 +98,6 @@ def lib() -> C.CDLL:
         L.fcg_slab_buffers.argtypes = [vp, C.POINTER(C.c_size_t), C.POINTER(C.c_size_t), C.POINTER(C.c_size_t)]; L.fcg_slab_buffers.restype = i
         L.fcg_slab_setup.argtypes = [vp, d, i]; L.fcg_slab_setup.restype = i
         L.fcg_slab_rows_fwd.argtypes = [vp, i, vp]; L.fcg_slab_rows_fwd.restype = i
-        L.fcg_slab_unpack.argtypes = [vp]; L.fcg_slab_unpack.restype = i
-        L.fcg_slab_pack.argtypes = [vp]; L.fcg_slab_pack.restype = i
         L.fcg_slab_cols.argtypes = [vp]; L.fcg_slab_cols.restype = i
         L.fcg_slab_rows_inv.argtypes = [vp, i, vp, vp, vp, vp]; L.fcg_slab_rows_inv.restype = i
         L.fcg_slab_update_r.argtypes = [vp, vp]; L.fcg_slab_update_r.restype = i
@@ -434,12 +431,6 @@ class Fcg:
 
     def fcg_slab_rows_fwd(self, cg: bool, xu: torch.Tensor):
         self._ok(self._lib.fcg_slab_rows_fwd(self._h, 1 if cg else 0, self._chk(xu)))
-
-    def fcg_slab_unpack(self):
-        self._ok(self._lib.fcg_slab_unpack(self._h))
-
-    def fcg_slab_pack(self):
-        self._ok(self._lib.fcg_slab_pack(self._h))
 
     def fcg_slab_cols(self):
         self._ok(self._lib.fcg_slab_cols(self._h))

@@ -102,10 +102,10 @@ struct fcg_handle_s {
     long long launches = 0;
     std::string err;
     // slab-decomposed CG: this handle is rank `slab_rank` of `slab_G`
-    int slab_G = 0, slab_rank = 0, slab_Al = 0, slab_MBl = 0;     // row pairs and column blocks this rank owns
-    size_t slab_S = 0, slab_R = 0, slab_C = 0, slab_bytes = 0;     // workspace offsets of T2 (rows side), the exchange buffer, T2 (columns side)
+    int slab_G = 0, slab_rank = 0, slab_Al = 0, slab_MBl = 0, slab_boxa = 0;     // row pairs and column blocks this rank owns; row pairs per column box
+    size_t slab_S = 0, slab_R = 0, slab_bytes = 0;                 // workspace offsets of T2 (rows side) and of the exchange buffer (= the columns side)
     alignas(64) CUtensorMap tmap_row_s;  // S as [L/(2 NB)][Al][128 B]
-    alignas(64) CUtensorMap tmap_col_s;  // C as [MBl][L/2][NB][2 complex]
+    alignas(64) CUtensorMap tmap_col_s;  // R as [source rank][MBl][Al][NB][2 complex] (5-D)
     alignas(64) CUtensorMap tmap_x;      // FCG_F64: the caller's half spectrum X[m][n] as a tensor of columns (fft_impl; re-encoded when X moves)
     const void* tmap_x_ptr = nullptr;
     int fft_pub = -1;                   // FCG_OPT_FFT_DIRECT (-1: automatic)
@@ -773,11 +773,14 @@ int slab_tensor_maps(fcg_handle h) {
                 CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
             return fail(h, FCG_CUDA_ERROR, "cuTensorMapEncodeTiled (slab rows) failed");
     }
-    {   // columns side C: d0 = 2 complex of one row pair, d1 = column in block, d2 = row pair (all of them), d3 = local column block
-        const cuuint64_t gdim[4] = {4, NB, L / 2, MBl};
-        const cuuint64_t gstride[3] = {4 * w, 4 * NB * w, (L / 2) * 4 * NB * w};
-        const cuuint32_t box[4] = {4u, 1u, (cuuint32_t)h->tab->v2_abox, 1u};
-        if (enc(&h->tmap_col_s, dtp, 4, h->ws + h->slab_C, gdim, gstride, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+    {   // columns side = the exchange buffer R itself: d0 = 2 complex of one row pair, d1 = column in block, d2 = local row pair,
+        // d3 = local column block, d4 = source rank; a box is one column x boxa row pairs of one source rank
+        const cuuint64_t G = (cuuint64_t)h->slab_G;
+        const cuuint64_t gdim[5] = {4, NB, Al, MBl, G};
+        const cuuint64_t gstride[4] = {4 * w, 4 * NB * w, Al * 4 * NB * w, MBl * Al * 4 * NB * w};
+        const cuuint32_t box[5] = {4u, 1u, (cuuint32_t)h->slab_boxa, 1u, 1u};
+        const cuuint32_t estr5[5] = {1u, 1u, 1u, 1u, 1u};
+        if (enc(&h->tmap_col_s, dtp, 5, h->ws + h->slab_R, gdim, gstride, box, estr5, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
                 CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
             return fail(h, FCG_CUDA_ERROR, "cuTensorMapEncodeTiled (slab columns) failed");
     }
@@ -811,8 +814,8 @@ int slab_rows_fwd_impl(fcg_handle h, int mode, void* xu) {
 }
 template <typename T>
 int slab_cols_impl(fcg_handle h) {
-    ColArgs<T> A{}; A.mode = COL_CONV; A.Tb = reinterpret_cast<cx<T>*>(h->ws + h->slab_C); A.shat = h->at<T>(h->lay.shat); A.tw = h->at<cx<T>>(h->lay.tw);
-    A.sc = nullptr; A.nsm = h->nsm; A.tmo = &h->sc()->timeout; A.col0 = h->slab_rank * ((h->L / 2) / h->slab_G);
+    ColArgs<T> A{}; A.mode = COL_CONV; A.Tb = reinterpret_cast<cx<T>*>(h->ws + h->slab_R); A.shat = h->at<T>(h->lay.shat); A.tw = h->at<cx<T>>(h->lay.tw);
+    A.sc = h->sc(); A.nsm = h->nsm; A.nranks = h->slab_G; A.al = h->slab_Al; A.boxa = h->slab_boxa; A.tmo = &h->sc()->timeout; A.col0 = h->slab_rank * ((h->L / 2) / h->slab_G);
     ++h->launches;
     FCG_CK(h, h->tab->col2_slab(&A, &h->tmap_col_s, (h->L / 2) / h->slab_G, h->stream));
     return FCG_OK;
@@ -1381,12 +1384,11 @@ int fcg_slab_configure(fcg_handle h, int nranks, int rank) {
     const int st = slab_shape(h->L, h->dtype, nranks, rank, &sh);
     if (st != FCG_OK) return fail(h, st, "slab decomposition: nranks must divide the column blocks L / (2 NB) and the row pairs L / 2");
     h->slab_G = nranks; h->slab_rank = rank; h->slab_Al = sh.row_pairs_local; h->slab_MBl = sh.column_blocks_local; h->slab_bytes = sh.buffer_bytes;
-    // This first slice keeps the full-size workspace of fcg_create.  S (T2, rows side) and C (T2, columns side) share the T2 region:
-    // N w / G bytes each, C in its upper half; with one rank (the undecomposed case, kept for tests) C is S itself, which is free
-    // once the exchange has copied it out.  The exchange buffer R lives in z, the vector only preconditioned CG uses.
+    // This first slice keeps the full-size workspace of fcg_create: S (T2 of the own rows, N w / G bytes) in the T2 region, the exchange
+    // buffer R in z, the vector only preconditioned CG uses.  The column pass works on R in place through a 5-D tensor map.
     h->slab_S = h->lay.Tb;
-    h->slab_C = nranks >= 2 ? h->lay.Tb + align_up(h->N * h->w / 2) : h->lay.Tb;
     h->slab_R = h->lay.z;
+    h->slab_boxa = h->tab->v2_abox < sh.row_pairs_local ? h->tab->v2_abox : sh.row_pairs_local;
     return slab_tensor_maps(h);
 }
 
@@ -1414,20 +1416,6 @@ int fcg_slab_rows_fwd(fcg_handle h, int cg, void* xu) {
     const int mode = cg ? ROWF_CG : ROWF_PLAIN;
     return h->dtype == FCG_F64 ? slab_rows_fwd_impl<double>(h, mode, xu) : slab_rows_fwd_impl<float>(h, mode, xu);
 }
-
-// R[s][column block][local row pair][line]  <->  C[column block][s Al + local row pair][line]
-static int slab_repack(fcg_handle h, bool unpack) {
-    const size_t line = (size_t)h->tab->v2_nb * 4 * h->w, Al = (size_t)h->slab_Al, chunk = (size_t)h->slab_MBl * Al * line;
-    for (int s2 = 0; s2 < h->slab_G; ++s2) {
-        char* c = h->ws + h->slab_C + (size_t)s2 * Al * line;
-        char* r = h->ws + h->slab_R + (size_t)s2 * chunk;
-        if (unpack) FCG_CK(h, cudaMemcpy2DAsync(c, ((size_t)h->L / 2) * line, r, Al * line, Al * line, (size_t)h->slab_MBl, cudaMemcpyDeviceToDevice, h->stream));
-        else FCG_CK(h, cudaMemcpy2DAsync(r, Al * line, c, ((size_t)h->L / 2) * line, Al * line, (size_t)h->slab_MBl, cudaMemcpyDeviceToDevice, h->stream));
-    }
-    return FCG_OK;
-}
-int fcg_slab_unpack(fcg_handle h) { FCG_SLAB_ENTER(h); return slab_repack(h, true); }
-int fcg_slab_pack(fcg_handle h) { FCG_SLAB_ENTER(h); return slab_repack(h, false); }
 
 int fcg_slab_cols(fcg_handle h) {
     FCG_SLAB_ENTER(h);

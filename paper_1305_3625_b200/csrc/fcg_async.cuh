@@ -365,7 +365,13 @@ __global__ void __launch_bounds__(P::NT, CTAS) col2_kernel(const ColArgs<T> A, c
     }
     if (lt == 0 && !FCG_PROBE_ON(0x200)) {
         tma::mbar_expect_tx(&bar, (uint32_t)((LG ? 0 : AS::WBYTES) + (n ? L * sizeof(T) : 0)));
-        if constexpr (!LG) {
+        if constexpr (SLAB) {
+            // straight from the exchange buffer R[source rank][local column block][local row pair][column][2 complex] (5-D map): row pair
+            // s al + a of the column lands at its natural place, so nothing has to be repacked after the all-to-all
+            for (int s2 = 0; s2 < A.nranks; ++s2)
+                for (int a = 0; a < A.al; a += A.boxa)
+                    tma::tensor_g2s_5d(smem_raw + (size_t)(s2 * A.al + a) * (2 * sizeof(cx<T>)), &tmap, 0, nl % AS::NB, a, nl / AS::NB, s2, &bar);
+        } else if constexpr (!LG) {
 #pragma unroll
         for (int b = 0; b < (L / 2) / ABOX; ++b)
             tma::tensor_g2s_4d(smem_raw + (size_t)b * BOXB, &tmap, 0, nl % AS::NB, b * ABOX, nl / AS::NB, &bar);
@@ -457,7 +463,11 @@ __global__ void __launch_bounds__(P::NT, CTAS) col2_kernel(const ColArgs<T> A, c
     tma::mbar_warp_arrive(&ready);
     if (lt == 0) {
         tma::mbar_wait(&ready, 0, A.tmo);            // every warp's part of the column is in place
-        if (!FCG_PROBE_ON(0x400)) {
+        if constexpr (SLAB) {
+            for (int s2 = 0; s2 < A.nranks; ++s2)
+                for (int a = 0; a < A.al; a += A.boxa)
+                    tma::tensor_s2g_5d(&tmap, 0, nl % AS::NB, a, nl / AS::NB, s2, smem_raw + (size_t)(s2 * A.al + a) * (2 * sizeof(cx<T>)));
+        } else if (!FCG_PROBE_ON(0x400)) {
 #pragma unroll
         for (int b = 0; b < (L / 2) / ABOX; ++b)
             tma::tensor_s2g_4d(&tmap, 0, nl % AS::NB, b * ABOX, nl / AS::NB, smem_raw + (size_t)b * BOXB);

@@ -70,6 +70,7 @@ template <typename T> struct ColArgs {
     int nsm;               // persistent column pass: SMs of the device
     unsigned int* tmo;     // pipelined passes: raised when an mbarrier wait gives up
     int col0;              // slab instantiation: global number of this launch's first column (spectrum row, packed column 0)
+    int nranks, al, boxa;  // slab: source ranks, row pairs per rank, row pairs per box of the 5-D map of the exchange buffer
     cx<T>* X;              // stand-alone transforms (col2_xpub_kernel): the public half spectrum X[m][n], L x (L/2+1)
 };
 

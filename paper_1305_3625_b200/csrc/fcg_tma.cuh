@@ -177,6 +177,18 @@ __device__ __forceinline__ void tensor_s2g_4d(const void* tmap, int c0, int c1, 
                  "r"(c2), "r"(c3), "r"(smem_u32(src_smem))
                  : "memory");
 }
+// 5-D tiles: the slab decomposition's column pass reads the exchange buffer [source rank][column block][local row pair][column][2 complex] directly
+__device__ __forceinline__ void tensor_g2s_5d(void* dst_smem, const void* tmap, int c0, int c1, int c2, int c3, int c4, uint64_t* bar) {
+    asm volatile("cp.async.bulk.tensor.5d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5, %6}], [%7];" ::"r"(
+                     smem_u32(dst_smem)),
+                 "l"(tmap), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(c4), "r"(smem_u32(bar))
+                 : "memory");
+}
+__device__ __forceinline__ void tensor_s2g_5d(const void* tmap, int c0, int c1, int c2, int c3, int c4, const void* src_smem) {
+    asm volatile("cp.async.bulk.tensor.5d.global.shared::cta.tile.bulk_group [%0, {%1, %2, %3, %4, %5}], [%6];" ::"l"(tmap), "r"(c0), "r"(c1),
+                 "r"(c2), "r"(c3), "r"(c4), "r"(smem_u32(src_smem))
+                 : "memory");
+}
 __device__ __forceinline__ void tensor_s2g_3d(const void* tmap, int c0, int c1, int c2, const void* src_smem) {
     asm volatile("cp.async.bulk.tensor.3d.global.shared::cta.tile.bulk_group [%0, {%1, %2, %3}], [%4];" ::"l"(tmap), "r"(c0), "r"(c1), "r"(c2),
                  "r"(smem_u32(src_smem))

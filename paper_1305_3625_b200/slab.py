@@ -9,8 +9,10 @@ and moves the exchange buffers between the ranks:
                device copies, the all-reduce a sum of G two-element tensors.
 
 Textbook order of Listing 2 per iteration:
-    rows_fwd | all-to-all S->R | unpack, cols, pack | all-to-all R->S | rows_inv | all-reduce | scalar(1) | update_r | all-reduce |
-    scalar(2) | poll
+    rows_fwd | all-to-all S->R | cols (on R, in place) | all-to-all R->S | rows_inv | all-reduce | scalar(1) | update_r | all-reduce |
+    scalar(2)
+with one read-back of the scalar block every `poll_every` iterations: once the device-side stopping decision has been taken
+(identically on every rank) the remaining passes of the chunk return at once without touching anything.
 """
 from __future__ import annotations
 
@@ -84,11 +86,11 @@ def _operator_round_trip(ranks, comm):
     """S (row transforms of the own rows) -> columns -> S (ready for the inverse row transforms), on every rank."""
     comm.all_to_all([r.recv for r in ranks], [r.send for r in ranks])
     for r in ranks:
-        r.h.fcg_slab_unpack(); r.h.fcg_slab_cols(); r.h.fcg_slab_pack()
+        r.h.fcg_slab_cols()                          # on R in place: a 5-D tensor map reads the all-to-all's layout as columns
     comm.all_to_all([r.send for r in ranks], [r.recv for r in ranks])
 
 
-def slab_solve(ranks, comm, k, f, u, tol: float, maxit: int):
+def slab_solve(ranks, comm, k, f, u, tol: float, maxit: int, poll_every: int = 8):
     """Solve A u = f with the lattice split by rows over `ranks` (all the ranks of this process: one with DistComm, G with
     LocalComm).  k, f, u: lists, one tensor of the rank's own rows each; u in: initial guess, out: solution.
     Returns (iters, rel_residual, status) -- identical on every rank."""
@@ -103,21 +105,22 @@ def slab_solve(ranks, comm, k, f, u, tol: float, maxit: int):
     for r in ranks:
         r.h.fcg_slab_scalar(0, r.xch)
     while True:
-        done, it, rr, st = ranks[0].h.fcg_slab_poll()           # every rank holds the same scalars; one read-back per iteration
+        done, it, rr, st = ranks[0].h.fcg_slab_poll()           # every rank holds the same scalars
         if done:
             break
-        for r, ui in zip(ranks, u):
-            r.h.fcg_slab_rows_fwd(True, ui)                     # u += alpha p (lagged), p = r + beta p, row transforms of p
-        _operator_round_trip(ranks, comm)
-        for r, ki in zip(ranks, k):
-            r.h.fcg_slab_rows_inv(False, ki, None, None, r.xch) # q = k o p + C p; xch[0] = p.q of the own rows
-        comm.all_reduce(xs)
-        for r in ranks:
-            r.h.fcg_slab_scalar(1, r.xch)                       # alpha
-            r.h.fcg_slab_update_r(r.xch)                        # r -= alpha q; xch[0] = r.r of the own rows
-        comm.all_reduce(xs)
-        for r in ranks:
-            r.h.fcg_slab_scalar(2, r.xch)                       # count, convergence, beta
+        for _ in range(max(1, int(poll_every))):
+            for r, ui in zip(ranks, u):
+                r.h.fcg_slab_rows_fwd(True, ui)                 # u += alpha p (lagged), p = r + beta p, row transforms of p
+            _operator_round_trip(ranks, comm)
+            for r, ki in zip(ranks, k):
+                r.h.fcg_slab_rows_inv(False, ki, None, None, r.xch)     # q = k o p + C p; xch[0] = p.q of the own rows
+            comm.all_reduce(xs)
+            for r in ranks:
+                r.h.fcg_slab_scalar(1, r.xch)                   # alpha
+                r.h.fcg_slab_update_r(r.xch)                    # r -= alpha q; xch[0] = r.r of the own rows
+            comm.all_reduce(xs)
+            for r in ranks:
+                r.h.fcg_slab_scalar(2, r.xch)                   # count, convergence, beta
     for r, ui in zip(ranks, u):
         r.h.fcg_slab_finish(ui)
     for r in ranks[1:]:

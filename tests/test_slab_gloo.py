@@ -2,9 +2,9 @@
 pure host arithmetic (fcg_slab_shape_of), and the exchange of paper_1305_3625_b200/slab.py's DistComm between two gloo ranks.
 
 A synthetic global half spectrum T2[column block][row pair][line] whose every byte-line encodes its own coordinates is split by
-rows (what the row passes write: S), exchanged with DistComm.all_to_all, unpacked the way fcg_slab_unpack copies (R[source][block]
-[local row pair] -> C[block][source * Al + local row pair]), and must then be exactly the columns the rank owns with ALL row pairs;
-the way back (pack, all_to_all) must restore S.  The all-reduce leg is checked with the scalar block's two doubles."""
+rows (what the row passes write: S), exchanged with DistComm.all_to_all, viewed the way fcg_slab_cols' 5-D tensor map reads it (R[source][block]
+[local row pair] as C[block][source * Al + local row pair]), and must then be exactly the columns the rank owns with ALL row pairs;
+the way back (all_to_all) must restore S.  The all-reduce leg is checked with the scalar block's two doubles."""
 import os
 import socket
 import sys
@@ -49,9 +49,9 @@ def _worker(rank, world, port, out, L):
     comm = slab.DistComm()
     comm.all_to_all([R], [S])
     Rn = R.numpy().reshape(world, MBl, Al, lb)
-    C = np.ascontiguousarray(Rn.transpose(1, 0, 2, 3)).reshape(MBl, world * Al, lb)                 # fcg_slab_unpack's copy
+    C = np.ascontiguousarray(Rn.transpose(1, 0, 2, 3)).reshape(MBl, world * Al, lb)                 # the column pass's view of R
     ok_fwd = np.array_equal(C, T2[rank * MBl:(rank + 1) * MBl])                                      # my columns, every row pair
-    R2 = torch.from_numpy(np.ascontiguousarray(C.reshape(MBl, world, Al, lb).transpose(1, 0, 2, 3)).reshape(-1))   # fcg_slab_pack's copy
+    R2 = torch.from_numpy(np.ascontiguousarray(C.reshape(MBl, world, Al, lb).transpose(1, 0, 2, 3)).reshape(-1))   # .. and what it leaves there
     S2 = torch.zeros_like(S)
     comm.all_to_all([S2], [R2])
     ok_back = torch.equal(S2, S)
