@@ -320,6 +320,17 @@ typedef struct {
 int fcg_slab_shape_of(int L, fcg_dtype dt, int nranks, int rank, fcg_slab_shape* out);
 int fcg_slab_configure(fcg_handle h, int nranks, int rank);
 int fcg_slab_buffers(fcg_handle h, size_t* send_offset, size_t* recv_offset, size_t* bytes);
+/* Peer mode: the exchange FUSED INTO THE PASSES over peer memory (NVLink / NVSwitch stores), no all-to-all at all.
+ *   peer_send_host[g], peer_recv_host[g]   HOST arrays of nranks DEVICE addresses, valid on this handle's device, of rank g's S and
+ *                       R buffers (the own ones included; 128-byte aligned): the other handles' buffers for logical ranks on one
+ *                       device, peer-enabled or cudaIpcOpenMemHandle'd mappings for one process per GPU.
+ * Afterwards fcg_slab_rows_fwd stores every 128-byte line of the row-transformed half spectrum straight into the exchange buffer
+ * of the rank that owns its column block (R[my rank][..] there), and fcg_slab_cols scatters the row pairs of source rank s
+ * straight into rank s's S (one TMA tensor map per peer), so the transfer overlaps the transforms line by line instead of
+ * following them.  The caller replaces each all-to-all by a BARRIER between the ranks (all of them have finished the pass):
+ * on one stream that is implicit, across processes any stream-ordered collective does it (slab.py uses the all-reduce).
+ * NULL, NULL returns to the all-to-all mode. */
+int fcg_slab_set_peers(fcg_handle h, void* const* peer_send_host, void* const* peer_recv_host);
 int fcg_slab_setup(fcg_handle h, double tol, int maxit);
 int fcg_slab_rows_fwd(fcg_handle h, int cg, void* xu);
 int fcg_slab_cols(fcg_handle h);

@@ -33,7 +33,7 @@ EXPORTS = ["fcg_workspace_bytes", "fcg_create", "fcg_destroy", "fcg_set_option",
            "fcg_green_function", "fcg_kernel_spectrum", "fcg_force_apply", "fcg_force_solve", "fcg_force_break_step",
            "fcg_force_fracture", "fcg_inverse_spectrum", "fcg_force_rhs", "fcg_force_from_displacement",
            "fcg_force_fracture_displacement", "fcg_force_fracture_displacement_begin", "fcg_force_fracture_displacement_end",
-           "fcg_slab_shape_of", "fcg_slab_configure", "fcg_slab_buffers", "fcg_slab_setup", "fcg_slab_rows_fwd", "fcg_slab_cols", "fcg_slab_rows_inv", "fcg_slab_update_r", "fcg_slab_scalar", "fcg_slab_finish", "fcg_slab_poll"]
+           "fcg_slab_shape_of", "fcg_slab_configure", "fcg_slab_buffers", "fcg_slab_set_peers", "fcg_slab_setup", "fcg_slab_rows_fwd", "fcg_slab_cols", "fcg_slab_rows_inv", "fcg_slab_update_r", "fcg_slab_scalar", "fcg_slab_finish", "fcg_slab_poll"]
 
 
 class SlabShape(C.Structure):
@@ -96,6 +96,7 @@ def lib() -> C.CDLL:
         L.fcg_slab_shape_of.argtypes = [i, i, i, i, C.POINTER(SlabShape)]; L.fcg_slab_shape_of.restype = i
         L.fcg_slab_configure.argtypes = [vp, i, i]; L.fcg_slab_configure.restype = i
         L.fcg_slab_buffers.argtypes = [vp, C.POINTER(C.c_size_t), C.POINTER(C.c_size_t), C.POINTER(C.c_size_t)]; L.fcg_slab_buffers.restype = i
+        L.fcg_slab_set_peers.argtypes = [vp, C.POINTER(vp), C.POINTER(vp)]; L.fcg_slab_set_peers.restype = i
         L.fcg_slab_setup.argtypes = [vp, d, i]; L.fcg_slab_setup.restype = i
         L.fcg_slab_rows_fwd.argtypes = [vp, i, vp]; L.fcg_slab_rows_fwd.restype = i
         L.fcg_slab_cols.argtypes = [vp]; L.fcg_slab_cols.restype = i
@@ -425,6 +426,15 @@ class Fcg:
         so, ro, nb = C.c_size_t(0), C.c_size_t(0), C.c_size_t(0)
         self._ok(self._lib.fcg_slab_buffers(self._h, C.byref(so), C.byref(ro), C.byref(nb)))
         return self._ws[so.value: so.value + nb.value], self._ws[ro.value: ro.value + nb.value]
+
+    def fcg_slab_set_peers(self, peer_send, peer_recv):
+        """peer_send / peer_recv: device addresses (ints) of every rank's S and R buffer, valid on this device; None, None: off."""
+        if peer_send is None:
+            self._ok(self._lib.fcg_slab_set_peers(self._h, None, None))
+            return
+        n = len(peer_send)
+        a = (C.c_void_p * n)(*[int(x) for x in peer_send]); b = (C.c_void_p * n)(*[int(x) for x in peer_recv])
+        self._ok(self._lib.fcg_slab_set_peers(self._h, a, b))
 
     def fcg_slab_setup(self, tol: float, maxit: int):
         self._ok(self._lib.fcg_slab_setup(self._h, float(tol), int(maxit)))

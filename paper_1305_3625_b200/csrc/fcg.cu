@@ -104,6 +104,8 @@ struct fcg_handle_s {
     // slab-decomposed CG: this handle is rank `slab_rank` of `slab_G`
     int slab_G = 0, slab_rank = 0, slab_Al = 0, slab_MBl = 0, slab_boxa = 0;     // row pairs and column blocks this rank owns; row pairs per column box
     size_t slab_S = 0, slab_R = 0, slab_bytes = 0;                 // workspace offsets of T2 (rows side) and of the exchange buffer (= the columns side)
+    void* slab_peerR[16] = {};           // peer mode (fcg_slab_set_peers): every rank's exchange buffer R ..
+    CUtensorMap* slab_peer_maps = nullptr;   // .. and a device array of tensor maps of every rank's T2 (rows side, S); nullptr: exchange by all-to-all
     alignas(64) CUtensorMap tmap_row_s;  // S as [L/(2 NB)][Al][128 B]
     alignas(64) CUtensorMap tmap_col_s;  // R as [source rank][MBl][Al][NB][2 complex] (5-D)
     alignas(64) CUtensorMap tmap_x;      // FCG_F64: the caller's half spectrum X[m][n] as a tensor of columns (fft_impl; re-encoded when X moves)
@@ -808,6 +810,10 @@ int slab_rows_fwd_impl(fcg_handle h, int mode, void* xu) {
     RowFwdArgs<T> A{}; A.mode = mode; A.x = (const T*)xu; A.u = (T*)xu; A.p = h->at<T>(h->lay.p); A.r = h->at<T>(h->lay.r);
     A.Tb = reinterpret_cast<cx<T>*>(h->ws + h->slab_S); A.tw = h->at<cx<T>>(h->lay.tw); A.sc = h->sc(); A.nsm = h->nsm; A.tmo = &h->sc()->timeout;
     A.ntile = h->slab_Al; A.astride = h->slab_Al;
+    if (h->slab_peer_maps) {
+        A.npeer = h->slab_G; A.prank = h->slab_rank; A.mbl = h->slab_MBl;
+        for (int g = 0; g < h->slab_G; ++g) A.peerR[g] = reinterpret_cast<cx<T>*>(h->slab_peerR[g]);
+    }
     ++h->launches;
     FCG_CK(h, h->tab->row_fwd2_slab(&A, h->stream));
     return FCG_OK;
@@ -815,7 +821,8 @@ int slab_rows_fwd_impl(fcg_handle h, int mode, void* xu) {
 template <typename T>
 int slab_cols_impl(fcg_handle h) {
     ColArgs<T> A{}; A.mode = COL_CONV; A.Tb = reinterpret_cast<cx<T>*>(h->ws + h->slab_R); A.shat = h->at<T>(h->lay.shat); A.tw = h->at<cx<T>>(h->lay.tw);
-    A.sc = h->sc(); A.nsm = h->nsm; A.nranks = h->slab_G; A.al = h->slab_Al; A.boxa = h->slab_boxa; A.tmo = &h->sc()->timeout; A.col0 = h->slab_rank * ((h->L / 2) / h->slab_G);
+    A.sc = h->sc(); A.nsm = h->nsm; A.nranks = h->slab_G; A.al = h->slab_Al; A.boxa = h->slab_boxa;
+    A.peer_maps = h->slab_peer_maps; A.prank = h->slab_rank; A.mbl = h->slab_MBl; A.tmo = &h->sc()->timeout; A.col0 = h->slab_rank * ((h->L / 2) / h->slab_G);
     ++h->launches;
     FCG_CK(h, h->tab->col2_slab(&A, &h->tmap_col_s, (h->L / 2) / h->slab_G, h->stream));
     return FCG_OK;
@@ -919,6 +926,7 @@ int fcg_destroy(fcg_handle h) {
     if (h->frac_idx) cudaFree(h->frac_idx);
     if (h->frac_it) cudaFree(h->frac_it);
     if (h->frac_ratio) cudaFree(h->frac_ratio);
+    if (h->slab_peer_maps) cudaFree(h->slab_peer_maps);
     cudaGetLastError();
     delete h;
     return FCG_OK;
@@ -1390,6 +1398,43 @@ int fcg_slab_configure(fcg_handle h, int nranks, int rank) {
     h->slab_R = h->lay.z;
     h->slab_boxa = h->tab->v2_abox < sh.row_pairs_local ? h->tab->v2_abox : sh.row_pairs_local;
     return slab_tensor_maps(h);
+}
+
+// Peer mode: the exchange fused into the passes.  peer_send[g] / peer_recv[g] = device addresses, valid on THIS device, of rank g's
+// S and R buffers (its own included): pointers of the other handles for logical ranks on one device, cudaIpcOpenMemHandle'd
+// mappings or peer-enabled addresses over NVLink for one process per GPU.
+int fcg_slab_set_peers(fcg_handle h, void* const* peer_send_host, void* const* peer_recv_host) {
+    FCG_SLAB_ENTER(h);
+    if (h->slab_peer_maps) { cudaFree(h->slab_peer_maps); h->slab_peer_maps = nullptr; }
+    if (!peer_send_host || !peer_recv_host) return FCG_OK;           // back to the all-to-all mode
+    if (h->slab_G > 16) return fail(h, FCG_UNSUPPORTED, "peer mode supports up to 16 ranks");
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn || qres != cudaDriverEntryPointSuccess) {
+        cudaGetLastError();
+        return fail(h, FCG_UNSUPPORTED, "cuTensorMapEncodeTiled unavailable");
+    }
+    auto enc = reinterpret_cast<EncodeTiledFn>(fn);
+    const cuuint64_t L = (cuuint64_t)h->L, w = (cuuint64_t)h->w, NB = (cuuint64_t)h->tab->v2_nb, Al = (cuuint64_t)h->slab_Al;
+    const CUtensorMapDataType dtp = h->dtype == FCG_F64 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32;
+    std::vector<CUtensorMap> maps((size_t)h->slab_G);
+    for (int g = 0; g < h->slab_G; ++g) {
+        if (!peer_send_host[g] || !peer_recv_host[g] || (reinterpret_cast<uintptr_t>(peer_send_host[g]) & 127u) || (reinterpret_cast<uintptr_t>(peer_recv_host[g]) & 127u))
+            return fail(h, FCG_INVALID_ARG, "peer buffers must be non-null and 128-byte aligned");
+        // rank g's T2 (rows side): d0 = 2 complex of one row pair, d1 = column in line, d2 = ITS local row pair, d3 = column block (all of them)
+        const cuuint64_t gdim[4] = {4, NB, Al, L / (2 * NB)};
+        const cuuint64_t gstride[3] = {4 * w, 4 * NB * w, Al * 4 * NB * w};
+        const cuuint32_t box[4] = {4u, 1u, (cuuint32_t)h->slab_boxa, 1u};
+        const cuuint32_t estr[4] = {1u, 1u, 1u, 1u};
+        if (enc(&maps[(size_t)g], dtp, 4, peer_send_host[g], gdim, gstride, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+            return fail(h, FCG_CUDA_ERROR, "cuTensorMapEncodeTiled (peer T2) failed");
+        h->slab_peerR[g] = peer_recv_host[g];
+    }
+    FCG_CK(h, cudaMalloc((void**)&h->slab_peer_maps, maps.size() * sizeof(CUtensorMap)));
+    FCG_CK(h, cudaMemcpyAsync(h->slab_peer_maps, maps.data(), maps.size() * sizeof(CUtensorMap), cudaMemcpyHostToDevice, h->stream));
+    FCG_CK(h, cudaStreamSynchronize(h->stream));
+    return FCG_OK;
 }
 
 int fcg_slab_buffers(fcg_handle h, size_t* send_offset, size_t* recv_offset, size_t* bytes) {

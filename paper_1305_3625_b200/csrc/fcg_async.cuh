@@ -306,7 +306,18 @@ __global__ void __launch_bounds__(P::NT + 32, CTAS) row_fwd2_kernel(const RowFwd
                 X0 = mk<T>((Za.x + Zb.x) * h, (Za.y - Zb.y) * h);
                 X1 = mk<T>((Za.y + Zb.y) * h, (Zb.x - Za.x) * h);
             }
-            if (st_on) store_pair_hint(A.Tb + (SLAB ? AS::t2_index_s(m, a0 >> 1, ASTR) : AS::t2_index(m, a0 >> 1)), X0, X1, pol_t2);
+            if constexpr (SLAB) {
+                cx<T>* dst;
+                if (A.npeer) {         // straight into the owner's exchange buffer: R[my rank][local block][row pair][column][2]
+                    const int mb = m / AS::NB;
+                    dst = A.peerR[mb / A.mbl] + ((((size_t)A.prank * A.mbl + mb % A.mbl) * ASTR + (a0 >> 1)) * AS::NB + m % AS::NB) * 2;
+                } else {
+                    dst = A.Tb + AS::t2_index_s(m, a0 >> 1, ASTR);
+                }
+                if (st_on) store_pair_hint(dst, X0, X1, pol_t2);
+            } else {
+                if (st_on) store_pair_hint(A.Tb + AS::t2_index(m, a0 >> 1), X0, X1, pol_t2);
+            }
         }
     }
     }
@@ -464,9 +475,13 @@ __global__ void __launch_bounds__(P::NT, CTAS) col2_kernel(const ColArgs<T> A, c
     if (lt == 0) {
         tma::mbar_wait(&ready, 0, A.tmo);            // every warp's part of the column is in place
         if constexpr (SLAB) {
+            const CUtensorMap* pm = static_cast<const CUtensorMap*>(A.peer_maps);
             for (int s2 = 0; s2 < A.nranks; ++s2)
-                for (int a = 0; a < A.al; a += A.boxa)
-                    tma::tensor_s2g_5d(&tmap, 0, nl % AS::NB, a, nl / AS::NB, s2, smem_raw + (size_t)(s2 * A.al + a) * (2 * sizeof(cx<T>)));
+                for (int a = 0; a < A.al; a += A.boxa) {
+                    const void* src = smem_raw + (size_t)(s2 * A.al + a) * (2 * sizeof(cx<T>));
+                    if (pm) tma::tensor_s2g_4d(pm + s2, 0, nl % AS::NB, a, A.prank * A.mbl + nl / AS::NB, src);   // rank s2's T2, over NVLink
+                    else tma::tensor_s2g_5d(&tmap, 0, nl % AS::NB, a, nl / AS::NB, s2, src);
+                }
         } else if (!FCG_PROBE_ON(0x400)) {
 #pragma unroll
         for (int b = 0; b < (L / 2) / ABOX; ++b)

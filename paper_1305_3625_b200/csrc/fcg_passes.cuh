@@ -56,6 +56,11 @@ template <typename T> struct RowFwdArgs {
     int hints;             // L2 eviction-priority hints (FCG_OPT_L2_HINTS bit mask; pipelined passes only)
     unsigned int* tmo;     // pipelined passes: raised when an mbarrier wait gives up (fcg_tma.cuh); = &Scalars::timeout
     int ntile, astride;    // slab instantiation: row pairs of this rank, and row pairs per column block of ITS T2
+    // slab, exchange fused into the pass (peer mode): the line of column block mb goes straight into the exchange buffer R of the rank
+    // that owns the block, peerR[mb / mbl], at [my rank][mb % mbl][local row pair] -- a store over NVLink (or into the same device
+    // for logical ranks).  npeer == 0: the lines stay in the own T2 (Tb) and an all-to-all moves them.
+    int npeer, prank, mbl;
+    cx<T>* peerR[16];
 };
 
 template <typename T> struct ColArgs {
@@ -71,6 +76,8 @@ template <typename T> struct ColArgs {
     unsigned int* tmo;     // pipelined passes: raised when an mbarrier wait gives up
     int col0;              // slab instantiation: global number of this launch's first column (spectrum row, packed column 0)
     int nranks, al, boxa;  // slab: source ranks, row pairs per rank, row pairs per box of the 5-D map of the exchange buffer
+    const void* peer_maps; // slab, peer mode: device array of nranks CUtensorMap, one per rank's T2 (rows side); the scatter of source
+    int prank, mbl;        //   rank s's row pairs goes straight there, to column block prank * mbl + local block.  nullptr: back into R
     cx<T>* X;              // stand-alone transforms (col2_xpub_kernel): the public half spectrum X[m][n], L x (L/2+1)
 };
 

@@ -36,6 +36,9 @@ class LocalComm:
         for x in xs:
             x.copy_(total)
 
+    def barrier(self, xs):
+        pass                                         # one stream: the launches of all logical ranks are already ordered
+
 
 class DistComm:
     """Collectives among the processes of torch.distributed's default group: lists of length one (this process's tensors)."""
@@ -65,6 +68,13 @@ class DistComm:
     def all_reduce(self, xs):
         self.dist.all_reduce(xs[0])
 
+    def barrier(self, xs):
+        """Stream-ordered barrier between the ranks: a collective on the stream completes on a rank only after every rank has
+        reached it in ITS stream, i.e. after that rank's preceding pass (whose peer stores are then visible) has finished."""
+        if not hasattr(self, "_tok"):
+            self._tok = torch.zeros(1, dtype=torch.float32, device=xs[0].device)
+        self.dist.all_reduce(self._tok)
+
 
 class SlabRank:
     """One rank's handle, its rows of k, f, u, and its exchange buffers."""
@@ -82,12 +92,28 @@ class SlabRank:
         self.h.close()
 
 
+def connect_peers_local(ranks):
+    """Logical ranks of one process on one device: every handle gets the addresses of all the others' buffers (peer mode: the
+    row pass stores, and the column pass scatters, straight into the destination rank's buffer; include/fcg.h)."""
+    send = [r.send.data_ptr() for r in ranks]; recv = [r.recv.data_ptr() for r in ranks]
+    for r in ranks:
+        r.h.fcg_slab_set_peers(send, recv)
+        r.peers = True
+
+
 def _operator_round_trip(ranks, comm):
     """S (row transforms of the own rows) -> columns -> S (ready for the inverse row transforms), on every rank."""
-    comm.all_to_all([r.recv for r in ranks], [r.send for r in ranks])
+    peers = getattr(ranks[0], "peers", False)
+    if peers:
+        comm.barrier([r.xch for r in ranks])         # every rank's row pass has delivered its lines into the owners' R
+    else:
+        comm.all_to_all([r.recv for r in ranks], [r.send for r in ranks])
     for r in ranks:
-        r.h.fcg_slab_cols()                          # on R in place: a 5-D tensor map reads the all-to-all's layout as columns
-    comm.all_to_all([r.send for r in ranks], [r.recv for r in ranks])
+        r.h.fcg_slab_cols()                          # on R in place: a 5-D tensor map reads the exchange layout as columns
+    if peers:
+        comm.barrier([r.xch for r in ranks])         # every rank's column pass has scattered into the owners' S
+    else:
+        comm.all_to_all([r.send for r in ranks], [r.recv for r in ranks])
 
 
 def slab_solve(ranks, comm, k, f, u, tol: float, maxit: int, poll_every: int = 8):

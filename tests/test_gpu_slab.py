@@ -31,11 +31,13 @@ def rel(a, b):
     return np.linalg.norm(a - b) / max(np.linalg.norm(b), 1e-300)
 
 
-def slab_run(w, G, tol, maxit, u0=None):
+def slab_run(w, G, tol, maxit, u0=None, peers=False):
     from paper_1305_3625_b200 import slab
     dt = w.dtype.type
     sd = dev(w.s)
     ranks = [slab.SlabRank(w.L, TDT[dt], G, g, sd) for g in range(G)]
+    if peers:
+        slab.connect_peers_local(ranks)
     k = [dev(w.k[r.rows]) for r in ranks]; f = [dev(w.f[r.rows]) for r in ranks]
     u = [dev((w.u0 if u0 is None else u0)[r.rows]) for r in ranks]
     it, rr, st = slab.slab_solve(ranks, slab.LocalComm(), k, f, u, tol, maxit)
@@ -117,3 +119,19 @@ def test_slab_cg_full_size_config2(B, dt):
         _, _, _, u = slab_run(w, 4, 0.0, ref["iters"])
         d = rel(u, ref["u"])
     assert d <= TOL_CG[dt], (d, it, ref["iters"])
+
+
+@pytest.mark.parametrize("cfg,L,dt", [(1, 256, np.float64), (1, 1024, np.float64), (4, 1024, np.float32), (2, 2048, np.float64)])
+@pytest.mark.parametrize("G", [2, 4, 8])
+def test_slab_peer_mode_fused_exchange(B, cfg, L, dt, G):
+    """Peer mode (fcg_slab_set_peers): no all-to-all -- the row pass stores its lines straight into the owning rank's exchange buffer
+    and the column pass scatters straight into the source ranks' T2.  The data that arrives is the same, so the solve must be
+    BITWISE the all-to-all mode's (same kernels, same arithmetic, same order of sums), and it is checked against the oracle too."""
+    w = inputs.config(cfg, dt, L=L)
+    maxit = 40 if L >= 2048 else w.maxit
+    a = slab_run(w, G, w.tol, maxit)
+    b = slab_run(w, G, w.tol, maxit, peers=True)
+    assert a[:3] == b[:3] and np.array_equal(a[3], b[3])
+    ref = orc.cg(w.s, w.k, w.f, w.u0, 0.0, 6)
+    it, _, _, u = slab_run(w, G, 0.0, 6, peers=True)
+    assert it == 6 and rel(u, ref["u"]) <= 0.1 * TOL_CG[dt]
