@@ -464,6 +464,11 @@ def run_slab(args, rank, world, local):
         comm, G, mine = slab.LocalComm(), args.slab_ranks, list(range(args.slab_ranks))
     sd = to(w.s)
     ranks = [slab.SlabRank(w.L, tdt, G, g, sd) for g in mine]
+    if args.slab_peers:          # the exchange fused into the passes: peer stores instead of all-to-alls
+        if world > 1:
+            slab.connect_peers_dist(ranks[0], comm)
+        else:
+            slab.connect_peers_local(ranks)
     k = [to(w.k[r.rows]) for r in ranks]; f = [to(w.f[r.rows]) for r in ranks]
     u = [torch.zeros_like(x) for x in k]
     sampler = ClockSampler(local) if rank == 0 else None
@@ -497,7 +502,7 @@ def run_slab(args, rank, world, local):
             "data": "synthetic",
             "config": {"workload": f"BASELINE.json configs[{args.config}]: L={w.L} {args.dtype}, ONE solve split by rows over {G} "
                                    f"{'ranks (one per GPU, NCCL)' if world > 1 else 'LOGICAL ranks on one device (device copies)'}, tol={w.tol:g} ({it} iterations)",
-                       "parallelism": f"slab x{G}", "launches_per_iteration_per_rank": 5, "collectives_per_iteration": "2 all-to-all (N w / G bytes per rank each) + 2 all-reduce (16 B)",
+                       "parallelism": f"slab x{G}" + (" peer mode" if args.slab_peers else ""), "launches_per_iteration_per_rank": 5, "collectives_per_iteration": "2 all-to-all (N w / G bytes per rank each) + 2 all-reduce (16 B)",
                        "note": "textbook order, host poll once per iteration; the hardware scaling curve is unmeasured on this one-GPU pool"},
             "site_iterations_per_s": its / (ms * 1e-3) * w.N, "us_per_iteration": t_iter_us,
             "exchange_bytes_per_iteration_per_rank": 2.0 * nw / G * (G - 1) / G,
@@ -538,6 +543,9 @@ def main():
     ap.add_argument("--shard", choices=["replicas", "slab"], default="replicas",
                     help="N > 1: replicas (default; one independent solve per GPU, no data-path collective) or slab (ONE solve split by rows "
                          "over the ranks: all-to-all transposes around the column pass, all-reduce of the scalars; DESIGN.md section 18)")
+    ap.add_argument("--slab-peers", action="store_true",
+                    help="--shard slab: peer mode -- the row pass stores straight into the owning rank's exchange buffer and the column pass "
+                         "scatters straight into the source ranks' T2 (CUDA IPC mappings over NVLink under torchrun); barriers replace the all-to-alls")
     ap.add_argument("--slab-ranks", type=int, default=4, help="--shard slab with one process: number of LOGICAL ranks on the one device")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-configs", action="store_true", help="skip the 'configs' block (configs[2] fp32, configs[4], transforms, break step)")

@@ -331,6 +331,14 @@ int fcg_slab_buffers(fcg_handle h, size_t* send_offset, size_t* recv_offset, siz
  * on one stream that is implicit, across processes any stream-ordered collective does it (slab.py uses the all-reduce).
  * NULL, NULL returns to the all-to-all mode. */
 int fcg_slab_set_peers(fcg_handle h, void* const* peer_send_host, void* const* peer_recv_host);
+/* The same for one process per GPU: fcg_slab_ipc_export fills FCG_SLAB_IPC_BYTES host bytes (the CUDA IPC handle of the allocation
+ * that holds this rank's workspace, and the offsets of S and R in it); the caller gathers the blobs of all ranks in rank order
+ * (nranks * FCG_SLAB_IPC_BYTES bytes) and hands them to fcg_slab_ipc_open on every rank, which maps the peers' buffers
+ * (cudaIpcOpenMemHandle with lazy peer access, i.e. over NVLink between GPUs) and calls fcg_slab_set_peers.  The workspace must
+ * come from cudaMalloc (torch's default allocator qualifies; expandable segments do not). */
+#define FCG_SLAB_IPC_BYTES 80
+int fcg_slab_ipc_export(fcg_handle h, void* blob_host);
+int fcg_slab_ipc_open(fcg_handle h, const void* blobs_host);
 int fcg_slab_setup(fcg_handle h, double tol, int maxit);
 int fcg_slab_rows_fwd(fcg_handle h, int cg, void* xu);
 int fcg_slab_cols(fcg_handle h);

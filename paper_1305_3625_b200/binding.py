@@ -24,6 +24,7 @@ FCG_OPT_COL_PERSISTENT = 9
 FCG_OPT_BARRIER_START = 10
 FCG_OPT_FFT_DIRECT = 11
 FCG_OPT_FUSED_TWO = 12
+FCG_SLAB_IPC_BYTES = 80
 
 EXPORTS = ["fcg_workspace_bytes", "fcg_create", "fcg_destroy", "fcg_set_option", "fcg_set_spectrum", "fcg_apply",
            "fcg_solve", "fcg_solve_host", "fcg_profile_iteration", "fcg_fft_fwd", "fcg_fft_inv", "fcg_break_step", "fcg_fracture",
@@ -33,7 +34,7 @@ EXPORTS = ["fcg_workspace_bytes", "fcg_create", "fcg_destroy", "fcg_set_option",
            "fcg_green_function", "fcg_kernel_spectrum", "fcg_force_apply", "fcg_force_solve", "fcg_force_break_step",
            "fcg_force_fracture", "fcg_inverse_spectrum", "fcg_force_rhs", "fcg_force_from_displacement",
            "fcg_force_fracture_displacement", "fcg_force_fracture_displacement_begin", "fcg_force_fracture_displacement_end",
-           "fcg_slab_shape_of", "fcg_slab_configure", "fcg_slab_buffers", "fcg_slab_set_peers", "fcg_slab_setup", "fcg_slab_rows_fwd", "fcg_slab_cols", "fcg_slab_rows_inv", "fcg_slab_update_r", "fcg_slab_scalar", "fcg_slab_finish", "fcg_slab_poll"]
+           "fcg_slab_shape_of", "fcg_slab_configure", "fcg_slab_buffers", "fcg_slab_set_peers", "fcg_slab_ipc_export", "fcg_slab_ipc_open", "fcg_slab_setup", "fcg_slab_rows_fwd", "fcg_slab_cols", "fcg_slab_rows_inv", "fcg_slab_update_r", "fcg_slab_scalar", "fcg_slab_finish", "fcg_slab_poll"]
 
 
 class SlabShape(C.Structure):
@@ -97,6 +98,8 @@ def lib() -> C.CDLL:
         L.fcg_slab_configure.argtypes = [vp, i, i]; L.fcg_slab_configure.restype = i
         L.fcg_slab_buffers.argtypes = [vp, C.POINTER(C.c_size_t), C.POINTER(C.c_size_t), C.POINTER(C.c_size_t)]; L.fcg_slab_buffers.restype = i
         L.fcg_slab_set_peers.argtypes = [vp, C.POINTER(vp), C.POINTER(vp)]; L.fcg_slab_set_peers.restype = i
+        L.fcg_slab_ipc_export.argtypes = [vp, vp]; L.fcg_slab_ipc_export.restype = i
+        L.fcg_slab_ipc_open.argtypes = [vp, vp]; L.fcg_slab_ipc_open.restype = i
         L.fcg_slab_setup.argtypes = [vp, d, i]; L.fcg_slab_setup.restype = i
         L.fcg_slab_rows_fwd.argtypes = [vp, i, vp]; L.fcg_slab_rows_fwd.restype = i
         L.fcg_slab_cols.argtypes = [vp]; L.fcg_slab_cols.restype = i
@@ -435,6 +438,15 @@ class Fcg:
         n = len(peer_send)
         a = (C.c_void_p * n)(*[int(x) for x in peer_send]); b = (C.c_void_p * n)(*[int(x) for x in peer_recv])
         self._ok(self._lib.fcg_slab_set_peers(self._h, a, b))
+
+    def fcg_slab_ipc_export(self) -> bytes:
+        buf = C.create_string_buffer(FCG_SLAB_IPC_BYTES)
+        self._ok(self._lib.fcg_slab_ipc_export(self._h, buf))
+        return buf.raw
+
+    def fcg_slab_ipc_open(self, blobs: bytes):
+        buf = C.create_string_buffer(bytes(blobs), len(blobs))
+        self._ok(self._lib.fcg_slab_ipc_open(self._h, buf))
 
     def fcg_slab_setup(self, tol: float, maxit: int):
         self._ok(self._lib.fcg_slab_setup(self._h, float(tol), int(maxit)))

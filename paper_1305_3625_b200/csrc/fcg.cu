@@ -104,6 +104,7 @@ struct fcg_handle_s {
     // slab-decomposed CG: this handle is rank `slab_rank` of `slab_G`
     int slab_G = 0, slab_rank = 0, slab_Al = 0, slab_MBl = 0, slab_boxa = 0;     // row pairs and column blocks this rank owns; row pairs per column box
     size_t slab_S = 0, slab_R = 0, slab_bytes = 0;                 // workspace offsets of T2 (rows side) and of the exchange buffer (= the columns side)
+    void* slab_ipc_base[16] = {};        // peer mode across processes: the peers' workspaces as opened by fcg_slab_ipc_open (closed in fcg_destroy)
     void* slab_peerR[16] = {};           // peer mode (fcg_slab_set_peers): every rank's exchange buffer R ..
     CUtensorMap* slab_peer_maps = nullptr;   // .. and a device array of tensor maps of every rank's T2 (rows side, S); nullptr: exchange by all-to-all
     alignas(64) CUtensorMap tmap_row_s;  // S as [L/(2 NB)][Al][128 B]
@@ -927,6 +928,7 @@ int fcg_destroy(fcg_handle h) {
     if (h->frac_it) cudaFree(h->frac_it);
     if (h->frac_ratio) cudaFree(h->frac_ratio);
     if (h->slab_peer_maps) cudaFree(h->slab_peer_maps);
+    for (void* b : h->slab_ipc_base) if (b) cudaIpcCloseMemHandle(b);
     cudaGetLastError();
     delete h;
     return FCG_OK;
@@ -1435,6 +1437,46 @@ int fcg_slab_set_peers(fcg_handle h, void* const* peer_send_host, void* const* p
     FCG_CK(h, cudaMemcpyAsync(h->slab_peer_maps, maps.data(), maps.size() * sizeof(CUtensorMap), cudaMemcpyHostToDevice, h->stream));
     FCG_CK(h, cudaStreamSynchronize(h->stream));
     return FCG_OK;
+}
+
+// One process per GPU: the exchange buffers live in the caller's workspace, possibly inside a larger allocation (torch's caching
+// allocator), so what is exported is the IPC handle of the ALLOCATION plus the two offsets into it.
+struct SlabIpcBlob { cudaIpcMemHandle_t handle; unsigned long long off_send, off_recv; };
+static_assert(sizeof(SlabIpcBlob) == FCG_SLAB_IPC_BYTES, "fcg_slab_ipc blob size");
+
+int fcg_slab_ipc_export(fcg_handle h, void* blob_host) {
+    FCG_SLAB_ENTER(h);
+    if (!blob_host) return fail(h, FCG_INVALID_ARG, "null argument");
+    typedef CUresult (*GetRange)(CUdeviceptr*, size_t*, CUdeviceptr);
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuMemGetAddressRange", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn || qres != cudaDriverEntryPointSuccess) {
+        cudaGetLastError();
+        return fail(h, FCG_UNSUPPORTED, "cuMemGetAddressRange unavailable");
+    }
+    CUdeviceptr base = 0; size_t size = 0;
+    if (reinterpret_cast<GetRange>(fn)(&base, &size, (CUdeviceptr)(uintptr_t)h->ws) != CUDA_SUCCESS) return fail(h, FCG_CUDA_ERROR, "cuMemGetAddressRange failed");
+    SlabIpcBlob b{};
+    FCG_CK(h, cudaIpcGetMemHandle(&b.handle, (void*)(uintptr_t)base));
+    const unsigned long long off = (unsigned long long)((uintptr_t)h->ws - (uintptr_t)base);
+    b.off_send = off + h->slab_S; b.off_recv = off + h->slab_R;
+    std::memcpy(blob_host, &b, sizeof(b));
+    return FCG_OK;
+}
+
+int fcg_slab_ipc_open(fcg_handle h, const void* blobs_host) {
+    FCG_SLAB_ENTER(h);
+    if (!blobs_host) return fail(h, FCG_INVALID_ARG, "null argument");
+    if (h->slab_G > 16) return fail(h, FCG_UNSUPPORTED, "peer mode supports up to 16 ranks");
+    void* send[16]; void* recv[16];
+    for (int g = 0; g < h->slab_G; ++g) {
+        if (g == h->slab_rank) { send[g] = h->ws + h->slab_S; recv[g] = h->ws + h->slab_R; continue; }
+        SlabIpcBlob b;
+        std::memcpy(&b, static_cast<const char*>(blobs_host) + (size_t)g * sizeof(SlabIpcBlob), sizeof(b));
+        if (!h->slab_ipc_base[g]) FCG_CK(h, cudaIpcOpenMemHandle(&h->slab_ipc_base[g], b.handle, cudaIpcMemLazyEnablePeerAccess));
+        send[g] = static_cast<char*>(h->slab_ipc_base[g]) + b.off_send; recv[g] = static_cast<char*>(h->slab_ipc_base[g]) + b.off_recv;
+    }
+    return fcg_slab_set_peers(h, send, recv);
 }
 
 int fcg_slab_buffers(fcg_handle h, size_t* send_offset, size_t* recv_offset, size_t* bytes) {

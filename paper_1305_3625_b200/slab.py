@@ -101,6 +101,17 @@ def connect_peers_local(ranks):
         r.peers = True
 
 
+def connect_peers_dist(rank_obj, comm):
+    """One process per GPU: exchange the CUDA IPC blobs of the workspaces (a small all-gather of bytes) and map the peers' buffers."""
+    mine = torch.frombuffer(bytearray(rank_obj.h.fcg_slab_ipc_export()), dtype=torch.uint8).clone()
+    if comm.native_a2a:
+        mine = mine.to(rank_obj.xch.device)
+    parts = [torch.empty_like(mine) for _ in range(comm.world)]
+    comm.dist.all_gather(parts, mine)
+    rank_obj.h.fcg_slab_ipc_open(b"".join(bytes(p.cpu().numpy().tobytes()) for p in parts))
+    rank_obj.peers = True
+
+
 def _operator_round_trip(ranks, comm):
     """S (row transforms of the own rows) -> columns -> S (ready for the inverse row transforms), on every rank."""
     peers = getattr(ranks[0], "peers", False)
