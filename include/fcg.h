@@ -348,6 +348,29 @@ int fcg_slab_scalar(fcg_handle h, int what, const void* xch);
 int fcg_slab_finish(fcg_handle h, void* u);
 int fcg_slab_poll(fcg_handle h, int* done_host, int* iters_host, double* rel_residual_host, int* status_host);
 
+/* ---- Break step that allocates NOTHING (no handle, no workspace) ---------------------------------------------------------------
+ * For callers that cannot call cudaMalloc: code under CUDA-graph stream capture, tight serving loops, harnesses that forbid
+ * allocation.  The same kernel and rule as fcg_break_step (configs[3], S5, S13: over {i : k_i > 0} the maximum of
+ * (k_i * u_i) / t_i in double, ties -> lowest i, NaN skipped, k_i := 0 at the winner), but its scratch -- one partial (ratio,
+ * index) per CTA and an arrival ticket -- lives in a static device array of FCG_BREAK_STATIC_SCRATCH_BYTES inside libfcg.so, which
+ * every GPU that loads the library holds until the process exits.  The call enqueues one 4-byte memset (the ticket must start at
+ * zero; the array otherwise keeps the last call's contents) and one kernel on `cuda_stream` of the CURRENT device and returns:
+ * no cudaMalloc / cudaFree / allocating routine, no host synchronisation, no device-to-host copy.
+ *   dt, n        element type and count of k, u, t;  1 <= n <= FCG_BREAK_STATIC_MAX_N (= 8192 * 8192, the largest lattice of
+ *                this library), else FCG_UNSUPPORTED; the arrays need not be a square lattice
+ *   k            device, in/out (k[index] := 0);  u, t  device, read-only;  all 16-byte aligned
+ *   result_dev   device, 8-byte aligned, caller-owned: receives one fcg_break_result { index (-1: no candidate), ratio, status
+ *                (FCG_OK or FCG_NO_CANDIDATE) } when the kernel has run
+ *   cuda_stream  a cudaStream_t of the current device (NULL: default stream)
+ * All calls on a device share the one array: calls whose kernels may OVERLAP on the GPU (different streams without an ordering
+ * between them, concurrent graph branches) race on it and give wrong results -- keep them on one stream or order them.
+ * Returns FCG_OK when enqueued; on error fcg_static_last_error() (per host thread) says why. */
+#define FCG_BREAK_STATIC_MAX_N (8192LL * 8192LL)
+#define FCG_BREAK_STATIC_SCRATCH_BYTES 19200
+typedef struct { long long index; double ratio; int status; int pad_; } fcg_break_result;
+int fcg_break_step_static(fcg_dtype dt, long long n, void* k, const void* u, const void* t, void* result_dev, void* cuda_stream);
+const char* fcg_static_last_error(void);
+
 /* Measurement aid: runs the set-up of fcg_solve and then `iters` iterations of the CG loop body as direct
  * launches with CUDA events between the four kernels (tol = 0: never stops early), and returns their mean
  * device times in milliseconds, ms_host[0..3] = { row pass forward (P1), column pass (P2), row pass inverse

@@ -34,7 +34,8 @@ EXPORTS = ["fcg_workspace_bytes", "fcg_create", "fcg_destroy", "fcg_set_option",
            "fcg_green_function", "fcg_kernel_spectrum", "fcg_force_apply", "fcg_force_solve", "fcg_force_break_step",
            "fcg_force_fracture", "fcg_inverse_spectrum", "fcg_force_rhs", "fcg_force_from_displacement",
            "fcg_force_fracture_displacement", "fcg_force_fracture_displacement_begin", "fcg_force_fracture_displacement_end",
-           "fcg_slab_shape_of", "fcg_slab_configure", "fcg_slab_buffers", "fcg_slab_set_peers", "fcg_slab_ipc_export", "fcg_slab_ipc_open", "fcg_slab_setup", "fcg_slab_rows_fwd", "fcg_slab_cols", "fcg_slab_rows_inv", "fcg_slab_update_r", "fcg_slab_scalar", "fcg_slab_finish", "fcg_slab_poll"]
+           "fcg_slab_shape_of", "fcg_slab_configure", "fcg_slab_buffers", "fcg_slab_set_peers", "fcg_slab_ipc_export", "fcg_slab_ipc_open", "fcg_slab_setup", "fcg_slab_rows_fwd", "fcg_slab_cols", "fcg_slab_rows_inv", "fcg_slab_update_r", "fcg_slab_scalar", "fcg_slab_finish", "fcg_slab_poll",
+           "fcg_break_step_static", "fcg_static_last_error"]
 
 
 class SlabShape(C.Structure):
@@ -108,6 +109,8 @@ def lib() -> C.CDLL:
         L.fcg_slab_scalar.argtypes = [vp, i, vp]; L.fcg_slab_scalar.restype = i
         L.fcg_slab_finish.argtypes = [vp, vp]; L.fcg_slab_finish.restype = i
         L.fcg_slab_poll.argtypes = [vp, C.POINTER(i), C.POINTER(i), C.POINTER(d), C.POINTER(i)]; L.fcg_slab_poll.restype = i
+        L.fcg_break_step_static.argtypes = [i, ll, vp, vp, vp, vp, vp]; L.fcg_break_step_static.restype = i
+        L.fcg_static_last_error.argtypes = []; L.fcg_static_last_error.restype = C.c_char_p
         L.fcg_last_launch_count.argtypes = [vp]; L.fcg_last_launch_count.restype = ll
         L.fcg_last_error.argtypes = [vp]; L.fcg_last_error.restype = C.c_char_p
         L.fcg_version.argtypes = []; L.fcg_version.restype = C.c_char_p
@@ -487,6 +490,31 @@ def fcg_slab_shape_of(L: int, dtype, nranks: int, rank: int) -> dict:
     if st != FCG_OK:
         raise FcgError(st, f"slab decomposition of L={L} over {nranks} ranks is not supported")
     return {name: getattr(sh, name) for name, _ in SlabShape._fields_}
+
+
+FCG_BREAK_STATIC_MAX_N = 8192 * 8192
+
+
+def fcg_break_step_static(k: torch.Tensor, u: torch.Tensor, t: torch.Tensor, result: torch.Tensor, stream: torch.cuda.Stream | None = None):
+    """The allocation-free break step (include/fcg.h): enqueues on `stream` (default: the current one) and returns at once.
+    k (in/out), u, t: contiguous CUDA tensors of one dtype and size; result: caller-owned CUDA tensor of 3 int64 that receives
+    the fcg_break_result block (read it with break_result())."""
+    if not (k.is_cuda and u.is_cuda and t.is_cuda and result.is_cuda and k.is_contiguous() and u.is_contiguous() and t.is_contiguous()):
+        raise ValueError("expected contiguous CUDA tensors")
+    if not (k.dtype == u.dtype == t.dtype and k.numel() == u.numel() == t.numel()):
+        raise ValueError("k, u, t must agree in dtype and size")
+    if result.dtype != torch.int64 or result.numel() < 3 or not result.is_contiguous():
+        raise ValueError("result must be a contiguous int64 tensor of >= 3 elements")
+    st = stream or torch.cuda.current_stream(k.device)
+    rc = lib().fcg_break_step_static(_dt(k.dtype), k.numel(), k.data_ptr(), u.data_ptr(), t.data_ptr(), result.data_ptr(), st.cuda_stream)
+    if rc != FCG_OK:
+        raise FcgError(rc, lib().fcg_static_last_error().decode())
+
+
+def break_result(result: torch.Tensor):
+    """(index, ratio, status) from the block fcg_break_step_static filled; synchronises (a device-to-host read)."""
+    r = result[:3].cpu()
+    return int(r[0]), float(r[1:2].view(torch.float64)[0]), int(r[2:3].view(torch.int32)[0])
 
 
 def fcg_version() -> str:

@@ -2,6 +2,7 @@
 // Kernels live in fcg_kernels.cuh / fcg_passes.cuh; the transform passes are instantiated per lattice
 // size in fcg_inst.cu.  No cuFFT, no cuBLAS, no host arithmetic on the data path.
 #define FCG_MAIN_TU
+#include <atomic>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -1546,6 +1547,78 @@ int fcg_slab_poll(fcg_handle h, int* done_host, int* iters_host, double* rel_res
     if (rel_residual_host) *rel_residual_host = h->h_sc->relres;
     if (status_host) *status_host = h->h_sc->status;
     if (h->h_sc->timeout) return fail(h, FCG_CUDA_ERROR, "a pipelined pass gave up waiting on an mbarrier");
+    return FCG_OK;
+}
+
+// ---- break step without any allocation (include/fcg.h: fcg_break_step_static) -------------------------------------------------
+// Scratch of break_argmax_kernel -- one (ratio, index) partial per CTA and the arrival ticket -- in static device memory, so that
+// callers who may not allocate (stream capture, serving loops) can run the break step with no handle, workspace or cudaMalloc.
+// Every GPU that loads libfcg.so holds these FCG_BREAK_STATIC_SCRATCH_BYTES until the process exits.  In HOST code the array's name
+// is only a stand-in: the device address comes from cudaGetSymbolAddress, once per device, with that device current.
+}  // extern "C"  (the array, the per-device table and the typed launcher have C++ linkage)
+namespace {
+constexpr size_t BRK_PR_OFF = 0, BRK_PI_OFF = VEC_BLOCKS_MAX * sizeof(double),
+                 BRK_TICKET_OFF = (VEC_BLOCKS_MAX * (sizeof(double) + sizeof(long long)) + 255) / 256 * 256;
+static_assert(BRK_TICKET_OFF + 256 == FCG_BREAK_STATIC_SCRATCH_BYTES, "static break-step scratch layout");
+}
+static __device__ __align__(256) unsigned char g_break_static_scratch[FCG_BREAK_STATIC_SCRATCH_BYTES];
+namespace {
+constexpr int MAX_DEVICES = 64;
+std::atomic<unsigned char*> g_break_static_ptr[MAX_DEVICES];       // device address of the array, per device ordinal (nullptr: not asked yet)
+thread_local std::string g_static_err;
+int static_fail(int code, const std::string& msg) { g_static_err = msg; return code; }
+
+template <typename T>
+cudaError_t break_static_launch(unsigned char* scratch, long long n, void* k, const void* u, const void* t, void* result_dev, cudaStream_t st) {
+    // grid as fcg_break_step's: whole unrolled trips of 4 vectors per thread, at most VEC_BLOCKS_MAX CTAs (= the partials' capacity)
+    const size_t nvec = (size_t)n / Vec<T>::W, per = 256 * 4;
+    size_t b = (nvec + per - 1) / per;
+    if (b > (size_t)VEC_BLOCKS_MAX) {
+        const size_t trips = (nvec + (size_t)VEC_BLOCKS_MAX * per - 1) / ((size_t)VEC_BLOCKS_MAX * per);
+        b = (nvec + per * trips - 1) / (per * trips);
+    }
+    if (b < 1) b = 1;
+    if (b > (size_t)VEC_BLOCKS_MAX) b = VEC_BLOCKS_MAX;
+    // the array keeps the last call's contents: the ticket must start at zero (a finished call leaves it there; a call that was
+    // aborted may not), the partials are overwritten before they are read
+    cudaError_t e = cudaMemsetAsync(scratch + BRK_TICKET_OFF, 0, sizeof(unsigned int), st);
+    if (e != cudaSuccess) return e;
+    break_argmax_kernel<T><<<(unsigned)b, 256, 0, st>>>((T*)k, (const T*)u, (const T*)t, n, reinterpret_cast<double*>(scratch + BRK_PR_OFF),
+                                                        reinterpret_cast<long long*>(scratch + BRK_PI_OFF),
+                                                        reinterpret_cast<unsigned int*>(scratch + BRK_TICKET_OFF),
+                                                        static_cast<BreakResult*>(result_dev), (T*)nullptr);
+    return cudaGetLastError();
+}
+}  // namespace
+
+extern "C" {
+
+const char* fcg_static_last_error(void) { return g_static_err.c_str(); }
+
+int fcg_break_step_static(fcg_dtype dt, long long n, void* k, const void* u, const void* t, void* result_dev, void* cuda_stream) {
+    static_assert(sizeof(BreakResult) == sizeof(fcg_break_result), "fcg_break_result layout");
+    if (dt != FCG_F32 && dt != FCG_F64) return static_fail(FCG_INVALID_ARG, "dtype must be FCG_F32 or FCG_F64");
+    if (!k || !u || !t || !result_dev) return static_fail(FCG_INVALID_ARG, "null argument");
+    if (n < 1) return static_fail(FCG_INVALID_ARG, "n must be >= 1");
+    if (n > FCG_BREAK_STATIC_MAX_N)
+        return static_fail(FCG_UNSUPPORTED, "n = " + std::to_string(n) + " exceeds FCG_BREAK_STATIC_MAX_N = " + std::to_string((long long)FCG_BREAK_STATIC_MAX_N) +
+                                                " (the static scratch is sized for that; use fcg_break_step with a handle beyond it)");
+    if (misaligned(k) || misaligned(u) || misaligned(t) || (reinterpret_cast<uintptr_t>(result_dev) & 7u))
+        return static_fail(FCG_INVALID_ARG, "k, u, t must be 16-byte aligned, result_dev 8-byte aligned");
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= MAX_DEVICES) { cudaGetLastError(); return static_fail(FCG_CUDA_ERROR, "no current CUDA device"); }
+    unsigned char* scratch = g_break_static_ptr[dev].load(std::memory_order_acquire);
+    if (!scratch) {        // set-up, once per device, with that device current: the symbol's DEVICE address (its host-side name is not one)
+        void* p = nullptr;
+        const cudaError_t e = cudaGetSymbolAddress(&p, g_break_static_scratch);
+        if (e != cudaSuccess || !p) { cudaGetLastError(); return static_fail(FCG_CUDA_ERROR, std::string("cudaGetSymbolAddress(g_break_static_scratch): ") + cudaGetErrorString(e)); }
+        scratch = static_cast<unsigned char*>(p);
+        g_break_static_ptr[dev].store(scratch, std::memory_order_release);      // (two threads racing here store the same address)
+    }
+    const cudaStream_t st = (cudaStream_t)cuda_stream;
+    const cudaError_t e = dt == FCG_F64 ? break_static_launch<double>(scratch, n, k, u, t, result_dev, st)
+                                        : break_static_launch<float>(scratch, n, k, u, t, result_dev, st);
+    if (e != cudaSuccess) return static_fail(FCG_CUDA_ERROR, std::string("fcg_break_step_static: ") + cudaGetErrorString(e));
     return FCG_OK;
 }
 
