@@ -24,6 +24,7 @@ FCG_OPT_COL_PERSISTENT = 9
 FCG_OPT_BARRIER_START = 10
 FCG_OPT_FFT_DIRECT = 11
 FCG_OPT_FUSED_TWO = 12
+FCG_OPT_STAGGER_P1, FCG_OPT_STAGGER_P2, FCG_OPT_STAGGER_P3 = 13, 14, 15
 FCG_SLAB_IPC_BYTES = 80
 
 EXPORTS = ["fcg_workspace_bytes", "fcg_create", "fcg_destroy", "fcg_set_option", "fcg_set_spectrum", "fcg_apply",

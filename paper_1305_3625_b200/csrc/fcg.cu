@@ -60,7 +60,7 @@ Layout make_layout(int L, size_t w) {
     o.brk_i = take(VEC_BLOCKS_MAX * sizeof(long long));
     o.scalars = take(sizeof(Scalars));
     o.brk_out = take(sizeof(BreakResult));
-    o.brk_ticket = take(sizeof(unsigned int));
+    o.brk_ticket = take(2 * sizeof(unsigned int));        // arrival ticket + key of the screen's running maximum (break_argmax_kernel)
     o.uni = take(4 * sizeof(unsigned long long));         // force_uniform_kernel's result (reading F1 check)
     o.total = off;
     return o;
@@ -89,6 +89,16 @@ struct fcg_handle_s {
     // persistent column pass: measured faster for fp32 (L = 2048: 23.2 -> 20.6 us, L = 4096: 59.1 -> 53.1) and for fp64 up to
     // L = 1024; slower at L = 2048 fp64 (two CTAs of 4 warps per SM instead of three: 26.5 -> 31.0 us), hence the automatic rule
     bool colp() const { return tab->colp_ok && (colp_opt < 0 ? (dtype == FCG_F32 || L <= 1024) : colp_opt != 0); }
+    // start offsets in ns between the CTAs that share an SM, per pass (P1, P2, P3): -1 = the measured default for this size (stagger())
+    int stag_opt[3] = {-1, -1, -1};
+    int stagger(int pass) const {
+        if (stag_opt[pass] >= 0) return stag_opt[pass];
+        // measured (us per CG iteration, interleaved runs on one B200): L = 2048 fp64 91.8 -> 89.0 with the last pass 2 us apart (after 93.2 ->
+        // 91.8 from the column pass), nothing from the first pass; L = 1024 fp64 40.5 -> 38.9; L = 2048 fp32 and L = 4096 fp64 lose or stay
+        if (dtype == FCG_F64 && L == 2048) return pass == 0 ? 0 : pass == 1 ? 1500 : 2000;
+        if (dtype == FCG_F64 && L == 1024) return pass == 1 ? 500 : 1000;
+        return 0;
+    }
     bool sl() const { return sl_opt && v2() && tab->sl_ok; }     // spectral search length: 3 launches per CG iteration
     bool fused() const { return fused_opt && tab->fused && v2() && loop_mode == 0; }   // whole solve in one cooperative kernel
     Scalars* h_sc = nullptr;            // pinned
@@ -235,13 +245,13 @@ template <typename T> struct Seq {
     T* q() const { return h->at<T>(h->lay.q); }
 
     cudaError_t row_fwd(int mode, const T* x, T* u, int check_done = 0) const {
-        RowFwdArgs<T> A{}; A.mode = mode; A.x = x; A.u = u; A.p = p(); A.r = pcg ? z() : r(); A.check_done = check_done; A.hints = h->hints; A.Tb = Tb(); A.tw = tw(); A.sc = h->sc(); A.nsm = h->nsm; A.pdl = h->pdl; A.tmo = &h->sc()->timeout;
+        RowFwdArgs<T> A{}; A.mode = mode; A.x = x; A.u = u; A.p = p(); A.r = pcg ? z() : r(); A.check_done = check_done; A.stagger_ns = mode == ROWF_CG ? h->stagger(0) : 0; A.hints = h->hints; A.Tb = Tb(); A.tw = tw(); A.sc = h->sc(); A.nsm = h->nsm; A.pdl = h->pdl; A.tmo = &h->sc()->timeout;
         ++h->launches;
         return v2() ? h->tab->row_fwd2(&A, st) : h->tab->row_fwd(h->row_var(), &A, st);
     }
     cudaError_t col(int mode, bool cg, bool precond = false) const {
         ColArgs<T> A{}; A.mode = mode; A.Tb = Tb(); A.shat = precond ? mhat() : shat(); A.hints = h->hints; A.tw = tw(); A.sc = cg ? h->sc() : nullptr; A.pdl = h->pdl; A.tmo = &h->sc()->timeout;
-        A.nsm = h->nsm;
+        A.nsm = h->nsm; A.stagger_ns = cg ? h->stagger(1) : 0;
         ++h->launches;
         if (v2() && mode == COL_CONV && h->colp()) return h->tab->col2p(&A, &h->tmap_col, 0, st);
         return (v2() && mode == COL_CONV) ? h->tab->col2(&A, &h->tmap_col, st) : h->tab->col(&A, st);
@@ -316,13 +326,13 @@ template <typename T> struct Seq {
     // spectral search length: alpha is known after the column pass, so the residual update rides in P3
     cudaError_t it_col_e() const {
         ColArgs<T> A{}; A.mode = COL_CONV; A.Tb = Tb(); A.shat = shat(); A.hints = h->hints; A.tw = tw(); A.sc = h->sc(); A.pdl = h->pdl; A.tmo = &h->sc()->timeout;
-        A.partial = h->at<double>(h->lay.partial_col); A.nsm = h->nsm;
+        A.partial = h->at<double>(h->lay.partial_col); A.nsm = h->nsm; A.stagger_ns = h->stagger(1);
         ++h->launches;
         if (h->colp()) return h->tab->col2p(&A, &h->tmap_col, 1, st);
         return h->tab->col2_energy(&A, &h->tmap_col, st);
     }
     cudaError_t it_row_inv_f(const T* k) const {
-        RowInvArgs<T> A{}; A.mode = ROWI_CGF; A.Tb = Tb(); A.tw = tw(); A.k = k; A.v = p(); A.f = r(); A.out = r(); A.hints = h->hints;
+        RowInvArgs<T> A{}; A.mode = ROWI_CGF; A.Tb = Tb(); A.tw = tw(); A.k = k; A.v = p(); A.f = r(); A.out = r(); A.hints = h->hints; A.stagger_ns = h->stagger(2);
         A.partial = h->at<double>(h->lay.partial_row); A.colsum = h->at<double>(h->lay.partial_col);
         A.sc = h->sc(); A.nsm = h->nsm; A.pdl = h->pdl; A.tmo = &h->sc()->timeout;
         ++h->launches;
@@ -452,7 +462,7 @@ int solve_impl(fcg_handle h, const void* k, const void* f, void* u, double tol, 
     }
     if (h->loop_mode == 0) {
         const int var = h->v2() ? 100 + (h->sl() && (!force || kappa > 0.0) ? 1 : 0) : h->row_var();
-        const int key = (pcg ? 1 : 0) + 2 * (h->colp() ? 1 : 0) + 4 * h->hints;
+        const int key = (pcg ? 1 : 0) + 2 * (h->colp() ? 1 : 0) + 4 * h->hints + 1024 * ((h->stagger(0) * 31 + h->stagger(1)) * 31 + h->stagger(2));
         GraphEntry* hit = nullptr;
         for (auto& g : h->graphs)
             if (g.k == k && g.f == f && g.u == u && g.tol == tol && g.maxit == maxit && g.var == var && g.unroll == h->unroll && g.pdl == h->pdl && g.pcg == key && g.force == (force ? 1 : 0) && g.D == D && g.kappa == kappa) { hit = &g; break; }
@@ -956,6 +966,9 @@ int fcg_set_option(fcg_handle h, int option, int value) {
         case FCG_OPT_BARRIER_START: h->barrier_start = (unsigned int)value; return FCG_OK;
         case FCG_OPT_FFT_DIRECT: if (value < -1 || value > 1) return fail(h, FCG_INVALID_ARG, "fft direct must be -1, 0 or 1"); h->fft_pub = value; return FCG_OK;
         case FCG_OPT_FUSED_TWO: if (value != 0 && value != 1) return fail(h, FCG_INVALID_ARG, "fused two must be 0 or 1"); h->fused_two = value; return FCG_OK;
+        case FCG_OPT_STAGGER_P1: case FCG_OPT_STAGGER_P2: case FCG_OPT_STAGGER_P3:
+            if (value < -1 || value > 100000) return fail(h, FCG_INVALID_ARG, "stagger must be -1 (default) or 0..100000 ns");
+            h->stag_opt[option - FCG_OPT_STAGGER_P1] = value; return FCG_OK;
         case FCG_OPT_UNROLL: if (value < 1 || value > 64) return fail(h, FCG_INVALID_ARG, "unroll must be 1..64"); h->unroll = value; return FCG_OK;
         case FCG_OPT_ENGINE:
             if (value != 0 && value != 1) return fail(h, FCG_INVALID_ARG, "engine must be 0 or 1");
@@ -1581,7 +1594,7 @@ cudaError_t break_static_launch(unsigned char* scratch, long long n, void* k, co
     if (b > (size_t)VEC_BLOCKS_MAX) b = VEC_BLOCKS_MAX;
     // the array keeps the last call's contents: the ticket must start at zero (a finished call leaves it there; a call that was
     // aborted may not), the partials are overwritten before they are read
-    cudaError_t e = cudaMemsetAsync(scratch + BRK_TICKET_OFF, 0, sizeof(unsigned int), st);
+    cudaError_t e = cudaMemsetAsync(scratch + BRK_TICKET_OFF, 0, 2 * sizeof(unsigned int), st);     // ticket + the screen's running maximum
     if (e != cudaSuccess) return e;
     break_argmax_kernel<T><<<(unsigned)b, 256, 0, st>>>((T*)k, (const T*)u, (const T*)t, n, reinterpret_cast<double*>(scratch + BRK_PR_OFF),
                                                         reinterpret_cast<long long*>(scratch + BRK_PI_OFF),

@@ -374,6 +374,21 @@ __device__ __forceinline__ bool better(double ra, long long ia, double rb, long 
     return ra > rb || (ra == rb && ia < ib);
 }
 
+// Order-preserving key of a float for atomicMax on unsigned: key(a) < key(b) <=> a < b; key 0 lies below every float (the empty maximum)
+__device__ __forceinline__ unsigned int float_key(float f) { const unsigned int b = __float_as_uint(f); return (b & 0x80000000u) ? ~b : (b | 0x80000000u); }
+__device__ __forceinline__ float key_float(unsigned int k) { return __uint_as_float((k & 0x80000000u) ? (k & 0x7fffffffu) : ~k); }
+
+// ticket[0]: arrival count of the CTAs;  ticket[1]: key of the grid-wide running maximum of the SCREEN (below); both 0 at launch and
+// reset to 0 by the last CTA (the words are part of a 256-byte-aligned scratch block).
+//
+// The screen.  The rule needs one IEEE double multiply and divide per candidate (~40 fp64-pipe instructions with the conversions:
+// 140 us of that pipe at L = 8192 fp32 against 125 us of bytes).  Most candidates are nowhere near the maximum, and that can be
+// decided in single precision: a_i = fl32(k_i u_i / t_i) differs from the exact ratio r_i by at most e = 5e-7 relative as long as no
+// operand leaves [1e-30, 1e30] (checked; anything outside, NaN, inf takes the exact path) and the quotient is a normal number.  Every
+// thread publishes the largest such a_j it has seen among valid candidates (atomicMax on ticket[1]) and skips candidate i when
+// a_i < g - |g| 1e-5 for the g it last read: then r_i <= a_i + |a_i| e < a_j - |a_j| e <= r_j (1e-5 > 2 e, either sign; an underflowed
+// a_i means |r_i| < 1.2e-38 and is skipped only against g > 2e-30), so i is neither the maximum nor tied with it.  What is
+// skipped depends on timing; the result does not: the winner and every candidate tied with it always reach the exact comparison.
 template <typename T>
 __global__ void __launch_bounds__(256) break_argmax_kernel(T* __restrict__ k, const T* u, const T* __restrict__ t,
                                                             long long n, double* pr, long long* pi, unsigned int* ticket,
@@ -385,6 +400,29 @@ __global__ void __launch_bounds__(256) break_argmax_kernel(T* __restrict__ k, co
     __shared__ int is_last;
     double br = 0.0; long long bi = -1;
     auto consider = [&](double r, long long i) { if (better(r, i, br, bi)) { br = r; bi = i; } };
+    unsigned int* const gkey = ticket + 1;
+    float thr = -INFINITY, amax = -INFINITY;          // skip below thr; amax = largest screened value of this thread's valid candidates
+    bool have_a = false;
+    auto refresh = [&]() {                            // re-read the grid-wide running maximum (relaxed: a stale value only screens less)
+        unsigned int g;
+        asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(g) : "l"(gkey) : "memory");
+        if (g == 0u) return;
+        const float gm = key_float(g);
+        thr = gm == INFINITY ? 3.4028235e38f * (1.0f - 1e-5f) : gm - fabsf(gm) * 1e-5f;
+    };
+    auto publish = [&]() {
+        if (have_a && !(amax < thr)) atomicMax(gkey, float_key(amax));
+    };
+    // true: candidate i is provably below the maximum (see above); false: take the exact path
+    auto screened_out = [&](float kf, float uf, float tf) {
+        const float pf = fzero ? uf : kf * uf;
+        const float ap = fabsf(pf), at = fabsf(tf);
+        if (!(ap > 1e-30f && ap < 1e30f && at > 1e-30f && at < 1e30f)) return false;     // (also NaN)
+        const float a = __fdividef(pf, tf);                                                // <= 2 ulp; |tf| < 2^126
+        const bool normal = fabsf(a) > 1e-30f;             // (a quotient that underflowed has no relative accuracy, but is known to be tiny)
+        if (normal && (!have_a || a > amax)) { amax = a; have_a = true; }                  // only accurate values are published
+        return a < thr && (normal || thr > 2e-30f);
+    };
     // One sweep over 3 N w bytes: 16-byte loads of k, u, t issued unconditionally, four vectors of each in flight per thread
     // (the scalar form, with u and t loaded behind the k > 0 branch, ran at 2.3 TB/s at L = 2048 fp64 and 1.6 TB/s at L = 8192
     // fp32).  Plain loads, not the read-only path: the last block writes k (and f) at the end.  `better` is a total order, so
@@ -397,6 +435,7 @@ __global__ void __launch_bounds__(256) break_argmax_kernel(T* __restrict__ k, co
         for (int c = 0; c < W; ++c) {
             const T ki = ks[c];
             if (!(ki > (T)0)) continue;
+            if (screened_out((float)ki, (float)us[c], (float)ts[c])) continue;
             const double load = fzero ? (double)us[c] : (double)ki * (double)us[c];      // l_i = k_i u_i   (one IEEE multiply)
             const double rt = load / (double)ts[c];            // l_i / t_i       (one IEEE divide)
             if (rt != rt) continue;
@@ -410,12 +449,16 @@ __global__ void __launch_bounds__(256) break_argmax_kernel(T* __restrict__ k, co
         V kk[4], uu[4], tt[4];
 #pragma unroll
         for (int c = 0; c < 4; ++c) { kk[c] = kvp[v + c * stride]; uu[c] = uvp[v + c * stride]; tt[c] = tvp[v + c * stride]; }
+        refresh();
 #pragma unroll
         for (int c = 0; c < 4; ++c) eval(kk[c], uu[c], tt[c], (v + c * stride) * W);
+        publish();
     }
     for (; v < nvec; v += stride) {
         const V kk = kvp[v], uu = uvp[v], tt = tvp[v];
+        refresh();
         eval(kk, uu, tt, v * W);
+        publish();
     }
     for (long long i = nvec * W + (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {      // (n not a multiple of W: never for a lattice)
         const T ki = k[i];
@@ -457,7 +500,7 @@ __global__ void __launch_bounds__(256) break_argmax_kernel(T* __restrict__ k, co
     __syncthreads();
     block_red();
     if (threadIdx.x == 0) {
-        *ticket = 0u;
+        ticket[0] = 0u; ticket[1] = 0u;
         out->index = bi; out->ratio = br; out->status = bi < 0 ? -6 : 0;
         if (bi >= 0) k[bi] = (T)0;
         if (bi >= 0 && fzero) fzero[bi] = (T)0;

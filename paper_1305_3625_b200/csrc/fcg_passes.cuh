@@ -61,6 +61,7 @@ template <typename T> struct RowFwdArgs {
     // for logical ranks).  npeer == 0: the lines stay in the own T2 (Tb) and an all-to-all moves them.
     int npeer, prank, mbl;
     cx<T>* peerR[16];
+    int stagger_ns;        // start offset between the CTAs that share an SM (fcg_tma.cuh: stagger_wait); 0: none
 };
 
 template <typename T> struct ColArgs {
@@ -79,6 +80,7 @@ template <typename T> struct ColArgs {
     const void* peer_maps; // slab, peer mode: device array of nranks CUtensorMap, one per rank's T2 (rows side); the scatter of source
     int prank, mbl;        //   rank s's row pairs goes straight there, to column block prank * mbl + local block.  nullptr: back into R
     cx<T>* X;              // stand-alone transforms (col2_xpub_kernel): the public half spectrum X[m][n], L x (L/2+1)
+    int stagger_ns;        // col2_kernel: start offset between the first-wave CTAs that share an SM (0: none)
 };
 
 template <typename T> struct RowInvArgs {
@@ -101,6 +103,7 @@ template <typename T> struct RowInvArgs {
                                           //    p.(I + K G)p = sum p^2 + kappa sum g |P|^2
     unsigned int* tmo;                    // pipelined passes: raised when an mbarrier wait gives up
     int ntile;                            // slab instantiation: row pairs of this rank
+    int stagger_ns;                       // start offset between the CTAs that share an SM; 0: none
     double* xch;                          // slab: the pass's grid-wide sums go HERE (device, 2 doubles) and no scalar step follows:
                                           //       they are this rank's share, to be all-reduced first (fcg_slab_scalar)
 };

@@ -19,8 +19,23 @@ FCG_PLAN(double, 64, 8, 8, 1, 1)      FCG_PLAN(float, 64, 4, 16, 1, 1)
 FCG_PLAN(double, 128, 16, 8, 1, 1)    FCG_PLAN(float, 128, 8, 16, 1, 1)
 FCG_PLAN(double, 256, 4, 4, 4, 4)     FCG_PLAN(float, 256, 4, 4, 4, 4)
 FCG_PLAN(double, 512, 8, 8, 8, 1)     FCG_PLAN(float, 512, 4, 8, 16, 1)
-FCG_PLAN(double, 1024, 8, 8, 4, 4)   FCG_PLAN(float, 1024, 8, 8, 16, 1)
-FCG_PLAN(double, 2048, 16, 16, 8, 1)  FCG_PLAN(float, 2048, 8, 16, 16, 1)
+// L = 1024 and 2048 in fp64: measured in round 2 (interleaved runs on one box, us per CG iteration): 1024: (8,8,4,4) 42.5, (16,8,8) 47.5,
+// (8,16,8) 41.0, (16,16,4) 48.3, (4,4,8,8) 40.2;  2048: (16,16,8) 94.5, (8,8,4,8) 100.2, (4,8,8,8) 103.1, (16,8,16) 95.9, (8,16,16) 93.1 --
+// a last radix that spans a whole 128-byte line (8 in fp64) or two helps the last pass; 256 threads per transform lose in the column pass.
+#ifndef FCG_P1024D_R1        // (-DFCG_P1024D_R1=.. -DFCG_P1024D_R2=.. ..; the same for 2048: plan experiments)
+#define FCG_P1024D_R1 4
+#define FCG_P1024D_R2 4
+#define FCG_P1024D_R3 8
+#define FCG_P1024D_R4 8
+#endif
+#ifndef FCG_P2048D_R1
+#define FCG_P2048D_R1 8
+#define FCG_P2048D_R2 16
+#define FCG_P2048D_R3 16
+#define FCG_P2048D_R4 1
+#endif
+FCG_PLAN(double, 1024, FCG_P1024D_R1, FCG_P1024D_R2, FCG_P1024D_R3, FCG_P1024D_R4)   FCG_PLAN(float, 1024, 8, 8, 16, 1)
+FCG_PLAN(double, 2048, FCG_P2048D_R1, FCG_P2048D_R2, FCG_P2048D_R3, FCG_P2048D_R4)  FCG_PLAN(float, 2048, 8, 16, 16, 1)
 FCG_PLAN(double, 4096, 16, 16, 16, 1) FCG_PLAN(float, 4096, 16, 16, 16, 1)
 FCG_PLAN(double, 8192, 16, 8, 8, 8)   FCG_PLAN(float, 8192, 8, 8, 8, 16)
 #undef FCG_PLAN

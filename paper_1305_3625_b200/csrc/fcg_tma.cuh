@@ -202,6 +202,15 @@ __device__ __forceinline__ void prefetch_tmap(const void* tmap) {
 // no-ops for a kernel launched without the programmatic-serialization attribute.
 __device__ __forceinline__ void grid_dep_launch() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 __device__ __forceinline__ void grid_dep_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+// Start offset between the CTAs that share an SM.  CTAs launched together move through their phases together -- all of them waiting
+// for copies, then all of them in the butterflies -- so the copy engine and the arithmetic pipes take turns instead of overlapping.
+// A fraction of one work item's time between their starts keeps them out of step for the whole launch (persistent CTAs) or hands the
+// offsets on to the CTAs that replace them (one CTA per item).  Cost: the wait itself, at most once per CTA.
+__device__ __forceinline__ void stagger_wait(unsigned long long ns) {
+    unsigned long long t0, t1;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t0));
+    do { __nanosleep(200); asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t1)); } while (t1 - t0 < ns);
+}
 // generic-proxy writes to shared memory -> visible to the async proxy (before a bulk store reads them)
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 

@@ -143,3 +143,38 @@ def test_ring_stress_bitwise_repeatable(B, L, dt):
             else:
                 assert r == ref[0] and torch.equal(u, ref[1]), (name, rep)
         h.close()
+
+
+@pytest.mark.parametrize("dt", [np.float64, np.float32])
+def test_break_step_screen_adversarial(B, dt):
+    """The break kernel screens candidates in single precision against a grid-wide running maximum and takes the exact IEEE
+    multiply / divide only near it (fcg_kernels.cuh).  Index AND ratio must stay bit-identical to the oracle where the screen is
+    under most stress: thousands of candidates within 1e-8 .. 1e-6 of the maximum, exact ties, only negative loads, operands far
+    outside the float range (exact path), in float's denormal range, infinities and NaNs -- several break steps in a row each."""
+    rng = np.random.default_rng(77)
+    L = 256; N = L * L
+    big = 300 if dt == np.float64 else 37
+    cases = {}
+    t = rng.random(N) + 0.1
+    cases["near ties"] = (np.ones(N), 3.7 * t * (1.0 + 1e-6 * rng.random(N)), t)
+    u = 2.5 * t; u[rng.integers(0, N, 500)] *= (1.0 + 1e-8)
+    cases["ties and 1e-8"] = (np.ones(N), u, t)
+    cases["negative only"] = (rng.random(N) + 0.5, -(rng.random(N) + 1e-3), rng.random(N) + 1e-3)
+    cases["huge range"] = (np.ones(N), 10.0 ** rng.uniform(-big, big, N) * rng.choice([-1.0, 1.0], N), 10.0 ** rng.uniform(-big, big, N))
+    cases["float denormals"] = (np.ones(N), 10.0 ** rng.uniform(-44, -36, N), 10.0 ** rng.uniform(-44, -36, N))
+    k = rng.random(N) + 0.5; k[rng.random(N) < 0.4] = 0
+    u = rng.standard_normal(N); t = rng.random(N)
+    t[rng.integers(0, N, 50)] = 0.0; u[rng.integers(0, N, 50)] = 0.0; u[100] = 0.0; t[100] = 0.0; k[100] = 1.0
+    cases["inf and nan"] = (k, u, t)
+    h = B.Fcg(L, TDT[dt])
+    for name, (k, u, t) in cases.items():
+        with np.errstate(all="ignore"):
+            k, u, t = k.astype(dt), u.astype(dt), t.astype(dt)
+        kd, ud, td = dev(k), dev(u), dev(t)
+        ko = k.copy()
+        for step in range(6):
+            idx, ratio, st = h.fcg_break_step(kd, ud, td)
+            io, ro, _, so = orc.break_step(ko, u, t)
+            assert (idx, st) == (io, so) and (ratio == ro or (np.isnan(ratio) and np.isnan(ro))), (name, step, idx, io, ratio, ro)
+            assert np.array_equal(kd.cpu().numpy(), ko), (name, step)
+    h.close()
