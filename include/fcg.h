@@ -89,9 +89,10 @@ typedef enum {
                                  (it then stays in L2 until the neighbouring columns have completed its sectors), inverse for
                                  FCG_F64 at every size and for FCG_F32 while X is <= 64 MiB.  Pipelined engine only (L >= 256) */
     FCG_OPT_FUSED_TWO    = 12, /* 1 (default): the one-launch kernel of FCG_OPT_FUSED runs un-preconditioned CG with TWO grid barriers per
-                                 iteration: it transforms the residual instead of the direction and carries the row-transformed
-                                 direction by the recurrence of Listing 2 (F_row p' = F_row r' + beta F_row p, exact in exact
-                                 arithmetic); 0: three barriers, the direction itself is transformed */
+                                 iteration (preconditioned CG with FOUR): it transforms the residual (and z = M^-1 r) instead of the
+                                 direction and carries the row-transformed direction by the recurrence of Listing 2 (F_row p' =
+                                 F_row r' + beta F_row p, exact in exact arithmetic); 0: three (six)
+                                 barriers, the direction itself is transformed */
     FCG_OPT_STAGGER_P1   = 13, /* start offset in ns between the CTAs that share an SM, in the loop's first / column / last pass: CTAs launched */
     FCG_OPT_STAGGER_P2   = 14, /* together otherwise move through their copy and butterfly phases in step and the two do not overlap.  -1 */
     FCG_OPT_STAGGER_P3   = 15, /* (default): the measured value for the size (FCG_F64 L = 2048: 0 / 1500 / 2000, L = 1024: 1000 / 500 / 1000; else 0); 0: none */

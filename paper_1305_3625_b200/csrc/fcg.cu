@@ -260,6 +260,7 @@ template <typename T> struct Seq {
         RowInvArgs<T> A{}; A.mode = mode; A.Tb = Tb(); A.tw = tw(); A.k = k; A.v = v; A.f = f; A.out = out; A.out2 = out2;
         A.scale = (T)(1.0 / ((double)h->L * (double)h->L)); A.hints = h->hints; A.form = force ? 1 : 0; A.dval = (T)D;
         A.partial = h->at<double>(h->lay.partial_row); A.sc = h->sc(); A.nsm = h->nsm; A.pdl = h->pdl; A.tmo = &h->sc()->timeout;
+        A.stagger_ns = mode == ROWI_CG ? h->stagger(2) : 0;
         ++h->launches;
         return v2() ? h->tab->row_inv2(&A, &h->tmap_row, st) : h->tab->row_inv(h->row_var(), &A, st);
     }
@@ -285,7 +286,7 @@ template <typename T> struct Seq {
     // PCG: column pass with the preconditioner's spectrum, then z = inverse row transforms, r.z -> rho', beta
     cudaError_t it_col_m() const { return col(COL_CONV, true, true); }
     cudaError_t it_row_pre() const {
-        RowInvArgs<T> A{}; A.mode = ROWI_PRECOND; A.Tb = Tb(); A.tw = tw(); A.k = r(); A.out = z(); A.hints = h->hints;
+        RowInvArgs<T> A{}; A.mode = ROWI_PRECOND; A.Tb = Tb(); A.tw = tw(); A.k = r(); A.out = z(); A.hints = h->hints; A.stagger_ns = h->stagger(2);
         A.partial = h->at<double>(h->lay.partial_row); A.sc = h->sc(); A.nsm = h->nsm; A.pdl = h->pdl; A.tmo = &h->sc()->timeout;
         ++h->launches;
         return v2() ? h->tab->row_inv2_pre(&A, &h->tmap_row, st) : h->tab->row_inv(h->row_var(), &A, st);
@@ -301,7 +302,7 @@ template <typename T> struct Seq {
             cudaError_t e = it_update_r();
             return e != cudaSuccess ? e : row_fwd(ROWF_PLAIN, r(), nullptr, 1);
         }
-        RowFwdArgs<T> A{}; A.mode = ROWF_RUPD; A.hints = h->hints; A.rw = r(); A.q = q(); A.Tb = Tb(); A.tw = tw(); A.sc = h->sc(); A.nsm = h->nsm; A.pdl = h->pdl; A.tmo = &h->sc()->timeout;
+        RowFwdArgs<T> A{}; A.mode = ROWF_RUPD; A.stagger_ns = h->stagger(0); A.hints = h->hints; A.rw = r(); A.q = q(); A.Tb = Tb(); A.tw = tw(); A.sc = h->sc(); A.nsm = h->nsm; A.pdl = h->pdl; A.tmo = &h->sc()->timeout;
         A.partial = h->at<double>(h->lay.partial_vec);
         ++h->launches;
         return h->tab->row_fwd2_rupd(&A, st);

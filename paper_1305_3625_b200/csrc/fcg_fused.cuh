@@ -38,7 +38,7 @@ struct FusedArgs {
     // force formulation (I + K G) f = K D (eq. (2)): u holds the bond forces, f is not read
     // (b = k * D is formed in shared memory), out_ratio[step] = the winning f/t of the break step (may be nullptr)
     int form; double D; double* out_ratio;
-    int two;                                    // plain CG (mhat == nullptr, form != 1): 1 = the two-barrier iteration (TWO instantiation)
+    int two;                                    // form != 1: 1 = fewer grid barriers per iteration (TWO instantiations: 2 for CG, 4 for PCG)
 };
 
 template <typename T, typename P> struct FusedShape {
@@ -49,7 +49,8 @@ template <typename T, typename P> struct FusedShape {
     static constexpr size_t WBYTES = (size_t)L * 2 * sizeof(T);
     static constexpr size_t VBYTES = (size_t)2 * L * sizeof(T);  // one vector's two rows
     static constexpr size_t smem = WBYTES + (size_t)TPC * 7 * VBYTES + 128;     // k f u r p q t
-    static constexpr size_t smem_two = smem;     // TWO keeps the own columns of the row-transformed direction in q's slot
+    static constexpr size_t smem_two = smem;     // TWO = 1 keeps the own columns of the row-transformed direction in q's slot
+    static constexpr size_t smem_two_pcg = smem + (size_t)TPC * VBYTES;          // TWO = 2 (PCG): q's slot holds z, an eighth slot the columns
     static_assert(WBYTES == VBYTES, "a column of T is as large as a vector's two rows");
 };
 
@@ -105,7 +106,10 @@ __device__ __forceinline__ bool grid_barrier(unsigned int* counter, unsigned int
 // barrier that completes T:   .. -> rows_inverse: u, r' -> row transforms of r' -> [sum r.r | T complete] -> beta, p' (real
 // space, for k o p and u), columns: Pc = T + beta Pc, column transforms, energy -> [sum p.Ap] -> alpha -> rows_inverse ..
 // The recurrence starts afresh with every solve (p = 0), so its rounding does not accumulate over a quasi-static loop.
-template <typename T, typename P, int FORCE = 0, bool TWO = false>
+// TWO = 2: the same for preconditioned CG, FOUR barriers instead of six: r' is transformed where the operator's last phase forms it
+// (the r.r barrier completes T for z = M^-1 r'), z where the preconditioner's last phase forms it (the r.z barrier completes T for
+// the operator, whose column phase then forms F_row p' = F_row z + beta F_row p).  z keeps q's slot, the columns get an eighth one.
+template <typename T, typename P, int FORCE = 0, int TWO = 0>
 __global__ void __launch_bounds__(P::NT) cg_fused_kernel(const FusedArgs A)
 {
     static_assert(!TWO || FORCE != 1, "the two-barrier iteration is for the displacement form");
@@ -122,9 +126,10 @@ __global__ void __launch_bounds__(P::NT) cg_fused_kernel(const FusedArgs A)
     cx<T>* W = reinterpret_cast<cx<T>*>(smem_raw);
     T* const vecs = reinterpret_cast<T*>(smem_raw + FS::WBYTES);
     // TWO: the own columns of F_row p live in the slot of q (vector 5), which plain CG never stores: L complex = two real rows
-    auto PcOf = [&](int j) { return reinterpret_cast<cx<T>*>(vecs + ((size_t)(j * 7 + 5) * 2) * L); };
+    constexpr int NVEC = TWO == 2 ? 8 : 7, PCSLOT = TWO == 2 ? 7 : 5;
+    auto PcOf = [&](int j) { return reinterpret_cast<cx<T>*>(vecs + ((size_t)(j * NVEC + PCSLOT) * 2) * L); };
     // vector v (0 k, 1 f, 2 u, 3 r, 4 p, 5 q, 6 t) of own tile j, row r (0/1)
-    auto V = [&](int j, int v, int r) { return vecs + ((size_t)(j * 7 + v) * 2 + r) * L; };
+    auto V = [&](int j, int v, int r) { return vecs + ((size_t)(j * NVEC + v) * 2 + r) * L; };
     SmemIO<T, P> io{W};
     const int lt = threadIdx.x, cta = (int)blockIdx.x;
     const T* gk = static_cast<const T*>(A.k); const T* gf = static_cast<const T*>(A.f); T* gu = static_cast<T*>(A.u);
@@ -416,6 +421,7 @@ __global__ void __launch_bounds__(P::NT) cg_fused_kernel(const FusedArgs A)
         int phase = (have_fn && FORCE == 0) ? PH_RESID : PH_FN;
         if constexpr (TWO) {
             // FN (||f||^2 where not known yet; row transforms of u) -> RESID (r = f - A u; row transforms of r) -> Q -> Q -> ..
+            // (TWO = 2, PCG: .. RESID -> Z (z = M^-1 r, r.z; row transforms of z) -> Q (.. row transforms of r') -> Z -> Q -> ..)
             // every phase ends with the row transforms of the NEXT operand and the grid-wide sum whose barrier also completes T
             const bool need_fn = phase == PH_FN;
             phase = PH_FN;
@@ -431,7 +437,7 @@ __global__ void __launch_bounds__(P::NT) cg_fused_kernel(const FusedArgs A)
                 } else {
                     if (phase == PH_Q) {                    // update calculation variables: new direction (98); sum k p^2 on the way
                         for (int j = 0; j < TPC; ++j) {
-                            const T* dv = V(j, 3, 0); T* pp = V(j, 4, 0); const T* kk = V(j, 0, 0);
+                            const T* dv = V(j, TWO == 2 ? 5 : 3, 0); T* pp = V(j, 4, 0); const T* kk = V(j, 0, 0);   // r, or z = M^-1 r
                             const T b = (T)beta;
                             for (int e = lt; e < 2 * L; e += NT) {
                                 const T pn = dv[e] + b * pp[e];
@@ -442,7 +448,7 @@ __global__ void __launch_bounds__(P::NT) cg_fused_kernel(const FusedArgs A)
                         __syncthreads();
                     }
                     double en = 0.0;
-                    columns(shat, phase == PH_Q ? &en : nullptr, phase == PH_Q, (T)beta);
+                    columns(phase == PH_Z ? mhat : shat, phase == PH_Q ? &en : nullptr, phase == PH_Q, (T)beta);
                     double* ps = A.partial + (size_t)slot * G;
                     if (phase == PH_Q) {                    // this CTA's share of p.Ap = sum k p^2 + sum shat |P|^2
                         const double mine = cta_sum(kpp + en);
@@ -464,6 +470,10 @@ __global__ void __launch_bounds__(P::NT) cg_fused_kernel(const FusedArgs A)
                             const T r0 = ff[e] - (kk[e] * uu[e] + c0), r1 = ff[L + e] - (kk[L + e] * uu[L + e] + c1);
                             rv[e] = r0; rv[L + e] = r1;
                             acc += (double)r0 * (double)r0; acc += (double)r1 * (double)r1;
+                        } else if (TWO == 2 && phase == PH_Z) {               // z = M^-1 r, r.z
+                            T* zz = V(j, 5, 0);
+                            zz[e] = c0; zz[L + e] = c1;
+                            acc += (double)rv[e] * (double)c0; acc += (double)rv[L + e] * (double)c1;
                         } else {                        // q = k o p + C p; new x (95), residue (96), residue length (97)
                             const T* pp = V(j, 4, 0);
                             const T p0 = pp[e], p1 = pp[L + e];
@@ -477,7 +487,7 @@ __global__ void __launch_bounds__(P::NT) cg_fused_kernel(const FusedArgs A)
                 }
                 if (bd) { status = ST_BREAKDOWN; break; }
                 __syncthreads();                            // the epilogue's writes to r (u) are in place for every thread
-                rows_forward(phase == PH_FN ? 2 : 3);       // u for the residual pass, else the residual just formed
+                rows_forward(phase == PH_FN ? 2 : (TWO == 2 && phase == PH_Z) ? 5 : 3);   // u for the residual pass, z for the operator, else the residual just formed
                 const double s0 = grid_sum(acc, okb); ok = ok && okb;
                 if (!ok) { status = -3; break; }
                 if (phase == PH_FN) { if (need_fn) { fn2 = s0; have_fn = true; } phase = PH_RESID; }
@@ -486,12 +496,17 @@ __global__ void __launch_bounds__(P::NT) cg_fused_kernel(const FusedArgs A)
                     if (fn2 == 0.0) { zero_u = true; rho = 0.0; rr = 0.0; break; }
                     if (sqrt(rr) <= A.tol * sqrt(fn2)) break;
                     if (A.maxit <= 0) { status = ST_NOT_CONVERGED; break; }
-                    phase = PH_Q;
+                    phase = TWO == 2 ? PH_Z : PH_Q;
+                } else if (TWO == 2 && phase == PH_Z) {
+                    if (!(s0 > 0.0) || !isfinite(s0)) { status = ST_BREAKDOWN; break; }
+                    beta = it == 0 ? 0.0 : s0 / rho;
+                    rho = s0; phase = PH_Q;
                 } else {
                     rr = s0; ++it;
-                    if (sqrt(rr) <= A.tol * sqrt(fn2)) { rho = rr; break; }                         // check convergence (99)
-                    if (it >= A.maxit) { rho = rr; status = ST_NOT_CONVERGED; break; }
-                    beta = rr / rho; rho = rr;
+                    if (sqrt(rr) <= A.tol * sqrt(fn2)) { if (TWO != 2) rho = rr; break; }            // check convergence (99)
+                    if (it >= A.maxit) { if (TWO != 2) rho = rr; status = ST_NOT_CONVERGED; break; }
+                    if (TWO == 2) phase = PH_Z;
+                    else { beta = rr / rho; rho = rr; }
                 }
             }
         } else

@@ -70,8 +70,10 @@ template <typename T> struct Inst {
             if ((e = prep(cg_fused_kernel<T, P>, FS::smem)) != cudaSuccess) return e;
             if ((e = prep(cg_fused_kernel<T, P, 1>, FS::smem)) != cudaSuccess) return e;
             if ((e = prep(cg_fused_kernel<T, P, 2>, FS::smem)) != cudaSuccess) return e;
-            if ((e = prep(cg_fused_kernel<T, P, 0, true>, FS::smem_two)) != cudaSuccess) return e;
-            if ((e = prep(cg_fused_kernel<T, P, 2, true>, FS::smem_two)) != cudaSuccess) return e;
+            if ((e = prep(cg_fused_kernel<T, P, 0, 1>, FS::smem_two)) != cudaSuccess) return e;
+            if ((e = prep(cg_fused_kernel<T, P, 2, 1>, FS::smem_two)) != cudaSuccess) return e;
+            if ((e = prep(cg_fused_kernel<T, P, 0, 2>, FS::smem_two_pcg)) != cudaSuccess) return e;
+            if ((e = prep(cg_fused_kernel<T, P, 2, 2>, FS::smem_two_pcg)) != cudaSuccess) return e;
         }
         return prep(col_kernel<T, P, CS::COLS>, CS::smem);
     }
@@ -226,11 +228,13 @@ template <typename T> struct Inst {
         if constexpr (FS::valid) {
             FusedArgs A = *static_cast<const FusedArgs*>(fused_args);
             void* params[] = {&A};
-            const bool two = A.two && A.mhat == nullptr && A.form != 1;        // plain CG: two grid barriers per iteration
-            const void* fn = A.form == 1 ? (const void*)cg_fused_kernel<T, P, 1>
-                             : A.form == 2 ? (two ? (const void*)cg_fused_kernel<T, P, 2, true> : (const void*)cg_fused_kernel<T, P, 2>)
-                                           : (two ? (const void*)cg_fused_kernel<T, P, 0, true> : (const void*)cg_fused_kernel<T, P>);
-            return cudaLaunchCooperativeKernel(fn, dim3(FS::G), dim3(P::NT), params, two ? FS::smem_two : FS::smem, st);
+            const int two = (A.two && A.form != 1) ? (A.mhat ? 2 : 1) : 0;        // fewer grid barriers per iteration (CG: 2, PCG: 4)
+            const void* fn;
+            if (A.form == 1) fn = (const void*)cg_fused_kernel<T, P, 1>;
+            else if (A.form == 2) fn = two == 2 ? (const void*)cg_fused_kernel<T, P, 2, 2> : two == 1 ? (const void*)cg_fused_kernel<T, P, 2, 1> : (const void*)cg_fused_kernel<T, P, 2>;
+            else fn = two == 2 ? (const void*)cg_fused_kernel<T, P, 0, 2> : two == 1 ? (const void*)cg_fused_kernel<T, P, 0, 1> : (const void*)cg_fused_kernel<T, P>;
+            const size_t smem = two == 2 ? FS::smem_two_pcg : two == 1 ? FS::smem_two : FS::smem;
+            return cudaLaunchCooperativeKernel(fn, dim3(FS::G), dim3(P::NT), params, smem, st);
         }
         return cudaErrorInvalidValue;
     }
