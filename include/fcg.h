@@ -95,7 +95,7 @@ typedef enum {
                                  barriers, the direction itself is transformed */
     FCG_OPT_STAGGER_P1   = 13, /* start offset in ns between the CTAs that share an SM, in the loop's first / column / last pass: CTAs launched */
     FCG_OPT_STAGGER_P2   = 14, /* together otherwise move through their copy and butterfly phases in step and the two do not overlap.  -1 */
-    FCG_OPT_STAGGER_P3   = 15, /* (default): the measured value for the size (FCG_F64 L = 2048: 0 / 1500 / 2000, L = 1024: 1000 / 500 / 1000; else 0); 0: none */
+    FCG_OPT_STAGGER_P3   = 15, /* (default): the measured value for the size (FCG_F64 L = 2048: 0 / 1500 / 2000; else 0); 0: none; <= 100000 */
     FCG_OPT_ENGINE       = 3  /* 0 (default): pipelined TMA passes where the lattice is large enough (L >= 256), classic
                                  passes otherwise; 1: classic passes only (synchronous loads; kept for A/B measurements).
                                  The stored spectrum's layout belongs to the engine: changing the engine after

@@ -94,9 +94,9 @@ struct fcg_handle_s {
     int stagger(int pass) const {
         if (stag_opt[pass] >= 0) return stag_opt[pass];
         // measured (us per CG iteration, interleaved runs on one B200): L = 2048 fp64 91.8 -> 89.0 with the last pass 2 us apart (after 93.2 ->
-        // 91.8 from the column pass), nothing from the first pass; L = 1024 fp64 40.5 -> 38.9; L = 2048 fp32 and L = 4096 fp64 lose or stay
+        // 91.8 from the column pass), nothing from the first pass; L = 2048 fp32 and L = 4096 lose or stay; L = 1024 gained (40.5 -> 38.9) only
+        // until its row passes got one CTA per transform (fcg_inst.cu pgrid: 37.9 with or without offsets)
         if (dtype == FCG_F64 && L == 2048) return pass == 0 ? 0 : pass == 1 ? 1500 : 2000;
-        if (dtype == FCG_F64 && L == 1024) return pass == 1 ? 500 : 1000;
         return 0;
     }
     bool sl() const { return sl_opt && v2() && tab->sl_ok; }     // spectral search length: 3 launches per CG iteration

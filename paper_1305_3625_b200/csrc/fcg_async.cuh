@@ -76,9 +76,21 @@ template <typename T, typename P> struct AsyncShape {
     static constexpr size_t KRB = RING_BUDGET - (size_t)NTS * TSB;
     static constexpr size_t inv_smem = WBYTES + (size_t)NTS * TSB + KRB + 128;
     static constexpr bool PRODUCER_WARPS = NT <= 256;                        // P3: dedicated TMA-issuing warps (else consumer warp 0 issues)
-    static constexpr int INV_THREADS = NT + (PRODUCER_WARPS ? 64 : 0);
-
     static constexpr int thread_cap = sizeof(T) == 8 ? 640 : 1152;           // ~104-128 / ~56-64 registers per thread
+    // P3 normally has TWO producer warps (tiles of T2 / strips of the vectors: each runs ahead across transforms on its own).  Where a
+    // second one costs a resident CTA AND with that CTA every transform of the lattice is resident at once (L = 1024 fp64: 3 x 148 = 444
+    // slots for 512 transforms with two, 4 x 148 = 592 with one), ONE producer warp issues tiles then strips of each transform in
+    // consumption order: nothing runs ahead, but nothing has to -- each CTA has a single transform -- and the pass is one round instead
+    // of two (measured 22.6 -> see DESIGN.md section 17).
+    static constexpr int NSM_DESIGN = 148;
+    static constexpr int slots_with(int extra) {
+        const int by_smem = (int)((size_t)FCG_MAX_SMEM / ((size_t)FCG_MAX_SMEM / CRES_I + 1280 - 2688 + 1024 + 128));
+        const int by_thr = thread_cap / (NT + extra) > 1 ? thread_cap / (NT + extra) : 1;
+        return (by_smem < by_thr ? by_smem : by_thr) * NSM_DESIGN;
+    }
+    static constexpr int NPW = !PRODUCER_WARPS ? 0 : (slots_with(64) < L / 2 && slots_with(32) >= L / 2) ? 1 : 2;
+    static constexpr int INV_THREADS = NT + 32 * NPW;
+
     // resident CTAs per SM to compile for: static_smem = the kernel's __shared__ barriers etc., extra = producer threads
     static constexpr int ctas(size_t smem, size_t static_smem, int extra) {
         const int by_smem = (int)((size_t)FCG_MAX_SMEM / (smem + static_smem + 1024));
@@ -187,9 +199,11 @@ __global__ void __launch_bounds__(P::NT + 32, CTAS) row_fwd2_kernel(const RowFwd
     const bool st_on = A.mode >= 0;
 
     // my transforms: tile(i) = grp + nsm * (j + i * k)
+    // (a grid that is not a whole multiple of the SM count is the one-transform-per-CTA launch: every transform resident at once)
     const int nsm = A.nsm < (int)gridDim.x ? A.nsm : (int)gridDim.x, grp = (int)blockIdx.x % nsm, jj = (int)blockIdx.x / nsm,
               kk = (int)gridDim.x / nsm;
-    auto tile_of = [&](int i) { return grp + nsm * (jj + i * kk); };
+    const bool whole = (int)gridDim.x % nsm == 0;
+    auto tile_of = [&](int i) { return whole ? grp + nsm * (jj + i * kk) : (int)blockIdx.x + i * (int)gridDim.x; };
     int ntl = 0;
     while (tile_of(ntl) < NTILE) ++ntl;
     const int G = ntl * R1;                                       // strips this CTA will consume
@@ -1049,7 +1063,8 @@ __global__ void __launch_bounds__(AsyncShape<T, P>::INV_THREADS, CTAS) row_inv2_
 
     const int nsm = A.nsm < (int)gridDim.x ? A.nsm : (int)gridDim.x, grp = (int)blockIdx.x % nsm, jj = (int)blockIdx.x / nsm,
               kk = (int)gridDim.x / nsm;
-    auto tile_of = [&](int i) { return grp + nsm * (jj + i * kk); };
+    const bool whole = (int)gridDim.x % nsm == 0;        // else: one transform per CTA, every transform resident at once
+    auto tile_of = [&](int i) { return whole ? grp + nsm * (jj + i * kk) : (int)blockIdx.x + i * (int)gridDim.x; };
     int ntl = 0;
     while (tile_of(ntl) < (SLAB ? A.ntile : L / 2)) ++ntl;
 
@@ -1123,9 +1138,14 @@ __global__ void __launch_bounds__(AsyncShape<T, P>::INV_THREADS, CTAS) row_inv2_
         alpha_d = A.sc->rho / pq_d;
         alpha = (T)alpha_d;
     }
-    if (PW && warp == NT / 32) {
+    if (PW && AS::NPW == 1 && warp == NT / 32) {       // one producer warp: tiles, then strips, of each transform in consumption order
+        for (int i = 0; i < ntl; ++i) {
+            for (int c = 0; c < NSUB; ++c) issue_next_T();
+            if (nv) for (int c = 0; c < R1 * SPT; ++c) issue_next_K();
+        }
+    } else if (PW && AS::NPW == 2 && warp == NT / 32) {
         while (p_tn < GT) issue_next_T();
-    } else if (PW && warp == NT / 32 + 1) {
+    } else if (PW && AS::NPW == 2 && warp == NT / 32 + 1) {
         while (p_kn < GK) issue_next_K();
     } else if (warp < NT / 32) {
         if (!PW && warp == 0) {

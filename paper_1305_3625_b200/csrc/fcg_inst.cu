@@ -91,6 +91,7 @@ template <typename T> struct Inst {
     }
     // persistent grid: CTAS CTAs on each of nsm SMs, but never more CTAs than transforms (whole multiples of nsm)
     static int pgrid(int nsm, int ctas) {
+        if (nsm * ctas >= L / 2 && nsm < L / 2) return L / 2;      // every transform resident at once: one CTA each, a single round
         int k = ctas;
         while (k > 1 && nsm * k > L / 2) --k;
         return nsm * k > L / 2 ? L / 2 : nsm * k;
