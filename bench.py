@@ -413,9 +413,17 @@ def bench_configs(binding, torch, inputs, hbm_peak):
         for _ in range(10): h.fcg_break_step(k, x, t)
         e1.record(); torch.cuda.synchronize()
         us = 1e3 * e0.elapsed_time(e1) / 10
-        out[f"break_step_L{L}_{name}"] = {"us_per_call": us, "bytes": 3 * nw, "gbs": 3 * nw / (us * 1e-6) / 1e9,
-                                          "frac_of_measured_peak": 3 * nw / (us * 1e-6) / 1e9 / hbm_peak,
-                                          "note": "device time between events around 10 blocking calls: kernel + 16-byte read-back + host sync each"}
+        # the same kernel through the allocation-free, asynchronous entry point (no read-back, no host sync): its device time
+        res = torch.zeros(3, dtype=torch.int64, device="cuda")
+        binding.fcg_break_step_static(k, x, t, res)
+        torch.cuda.synchronize(); e0.record()
+        for _ in range(10): binding.fcg_break_step_static(k, x, t, res)
+        e1.record(); torch.cuda.synchronize()
+        dus = 1e3 * e0.elapsed_time(e1) / 10
+        out[f"break_step_L{L}_{name}"] = {"us_per_call": us, "device_us": dus, "bytes": 3 * nw, "gbs": 3 * nw / (dus * 1e-6) / 1e9,
+                                          "frac_of_measured_peak": 3 * nw / (dus * 1e-6) / 1e9 / hbm_peak,
+                                          "note": "us_per_call: 10 blocking fcg_break_step calls (kernel + 16-byte read-back + host sync each); device_us, gbs, "
+                                                  "frac: 10 back-to-back fcg_break_step_static calls (4-byte memset + the same kernel, no host sync)"}
         h.close()
         del x, X, xb, k, t
     torch.cuda.empty_cache()
