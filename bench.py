@@ -471,6 +471,7 @@ def run_slab(args, rank, world, local):
     else:
         comm, G, mine = slab.LocalComm(), args.slab_ranks, list(range(args.slab_ranks))
     sd = to(w.s)
+    spectral = args.slab_order == "spectral"
     ranks = [slab.SlabRank(w.L, tdt, G, g, sd) for g in mine]
     if args.slab_peers:          # the exchange fused into the passes: peer stores instead of all-to-alls
         if world > 1:
@@ -482,7 +483,7 @@ def run_slab(args, rank, world, local):
     sampler = ClockSampler(local) if rank == 0 else None
     for _ in range(args.warmup):
         for x in u: x.zero_()
-        it, rr, st = slab.slab_solve(ranks, comm, k, f, u, w.tol, w.maxit)
+        it, rr, st = slab.slab_solve(ranks, comm, k, f, u, w.tol, w.maxit, spectral=spectral)
     if world > 1:
         dist.barrier()
     torch.cuda.synchronize()
@@ -493,7 +494,7 @@ def run_slab(args, rank, world, local):
     e0.record()
     for _ in range(args.steps):
         for x in u: x.zero_()
-        it, rr, st = slab.slab_solve(ranks, comm, k, f, u, w.tol, w.maxit)
+        it, rr, st = slab.slab_solve(ranks, comm, k, f, u, w.tol, w.maxit, spectral=spectral)
         its += it; launches += sum(r.h.fcg_last_launch_count() for r in ranks)
     e1.record(); torch.cuda.synchronize()
     clocks = sampler.stop() if sampler else None
@@ -510,8 +511,10 @@ def run_slab(args, rank, world, local):
             "data": "synthetic",
             "config": {"workload": f"BASELINE.json configs[{args.config}]: L={w.L} {args.dtype}, ONE solve split by rows over {G} "
                                    f"{'ranks (one per GPU, NCCL)' if world > 1 else 'LOGICAL ranks on one device (device copies)'}, tol={w.tol:g} ({it} iterations)",
-                       "parallelism": f"slab x{G}" + (" peer mode" if args.slab_peers else ""), "launches_per_iteration_per_rank": 5, "collectives_per_iteration": "2 all-to-all (N w / G bytes per rank each) + 2 all-reduce (16 B)",
-                       "note": "textbook order, host poll once per iteration; the hardware scaling curve is unmeasured on this one-GPU pool"},
+                       "parallelism": f"slab x{G}" + (" peer mode" if args.slab_peers else ""), "launches_per_iteration_per_rank": "3 passes + 3 one-block kernels" if spectral else "4 passes + 2 one-block kernels",
+                       "collectives_per_iteration": ("2 barriers" if args.slab_peers else "2 all-to-all (N w / G bytes per rank each)") + " + 2 all-reduce (32 B)",
+                       "note": ("spectral search length (three passes)" if spectral else "textbook order (four passes)") +
+                               ", host poll every eighth iteration; the hardware scaling curve is unmeasured on this one-GPU pool"},
             "site_iterations_per_s": its / (ms * 1e-3) * w.N, "us_per_iteration": t_iter_us,
             "exchange_bytes_per_iteration_per_rank": 2.0 * nw / G * (G - 1) / G,
             "gpu_launches": launches, "clocks": clocks, "final_rel_residual": rr, "status": st}))
@@ -551,6 +554,8 @@ def main():
     ap.add_argument("--shard", choices=["replicas", "slab"], default="replicas",
                     help="N > 1: replicas (default; one independent solve per GPU, no data-path collective) or slab (ONE solve split by rows "
                          "over the ranks: all-to-all transposes around the column pass, all-reduce of the scalars; DESIGN.md section 18)")
+    ap.add_argument("--slab-order", choices=["spectral", "textbook"], default="spectral",
+                    help="--shard slab: the iteration with the spectral search length (three passes per iteration, default) or in the textbook order (four)")
     ap.add_argument("--slab-peers", action="store_true",
                     help="--shard slab: peer mode -- the row pass stores straight into the owning rank's exchange buffer and the column pass "
                          "scatters straight into the source ranks' T2 (CUDA IPC mappings over NVLink under torchrun); barriers replace the all-to-alls")

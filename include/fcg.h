@@ -308,6 +308,17 @@ int fcg_force_fracture(fcg_handle h, void* k, double D, void* f, const void* t, 
  *                       rows_inv (alpha, or breakdown), 2 after update_r (count, convergence / maxit, beta, rho)
  *   fcg_slab_finish     the last lagged u += alpha p on the own rows
  *   fcg_slab_poll       read the scalar block back (blocks): done flag, iteration count, relative residual, status
+ * The same iteration with the SPECTRAL SEARCH LENGTH (DESIGN.md sections 12 and 18; xch: device, 4 doubles): p.Ap = sum k p^2 +
+ * sum shat |P|^2 is known after the column pass, so the residual update rides in the last pass and the update_r pass disappears:
+ *     rows_fwd(cg) | exchange | cols_energy -> xch | exchange, all-reduce | scalar(4) | rows_inv(2) -> xch | all-reduce | scalar(5)
+ *   fcg_slab_kpp0       after rows_inv(residual = 1): xch[2] = sum k r^2 of the own rows (the first direction is p = r), so that the
+ *                       one all-reduce of the set-up carries r.r, f.f and this; then fcg_slab_scalar(0) and fcg_slab_scalar(3)
+ *   fcg_slab_cols_energy  fcg_slab_cols that also leaves xch[0] = this rank's share of sum shat |P|^2 (xch[1..3] = 0)
+ *   fcg_slab_rows_inv(residual = 2)   r -= alpha (k o p + C p) on the own rows, q never stored (u, f unused);
+ *                       xch = { r.r, sum k r^2, sum k r p } of the own rows (the new r)
+ *   fcg_slab_scalar     what = 3: start of the recurrence for sum k p^2 (xch[2] of the set-up); 4: alpha = rho / (sum k p^2 + xch[0]),
+ *                       or breakdown; 5: count, convergence / maxit, beta, rho from xch[0], and sum k p'^2 = xch[1] + 2 beta xch[2] +
+ *                       beta^2 sum k p^2 for the next direction
  * All calls but fcg_slab_shape_of and fcg_slab_poll are asynchronous on the handle's stream. */
 typedef struct {
     int nranks, rank;
@@ -346,6 +357,8 @@ int fcg_slab_ipc_open(fcg_handle h, const void* blobs_host);
 int fcg_slab_setup(fcg_handle h, double tol, int maxit);
 int fcg_slab_rows_fwd(fcg_handle h, int cg, void* xu);
 int fcg_slab_cols(fcg_handle h);
+int fcg_slab_cols_energy(fcg_handle h, void* xch);
+int fcg_slab_kpp0(fcg_handle h, const void* k, void* xch);
 int fcg_slab_rows_inv(fcg_handle h, int residual, const void* k, const void* u, const void* f, void* xch);
 int fcg_slab_update_r(fcg_handle h, void* xch);
 int fcg_slab_scalar(fcg_handle h, int what, const void* xch);

@@ -35,7 +35,7 @@ EXPORTS = ["fcg_workspace_bytes", "fcg_create", "fcg_destroy", "fcg_set_option",
            "fcg_green_function", "fcg_kernel_spectrum", "fcg_force_apply", "fcg_force_solve", "fcg_force_break_step",
            "fcg_force_fracture", "fcg_inverse_spectrum", "fcg_force_rhs", "fcg_force_from_displacement",
            "fcg_force_fracture_displacement", "fcg_force_fracture_displacement_begin", "fcg_force_fracture_displacement_end",
-           "fcg_slab_shape_of", "fcg_slab_configure", "fcg_slab_buffers", "fcg_slab_set_peers", "fcg_slab_ipc_export", "fcg_slab_ipc_open", "fcg_slab_setup", "fcg_slab_rows_fwd", "fcg_slab_cols", "fcg_slab_rows_inv", "fcg_slab_update_r", "fcg_slab_scalar", "fcg_slab_finish", "fcg_slab_poll",
+           "fcg_slab_shape_of", "fcg_slab_configure", "fcg_slab_buffers", "fcg_slab_set_peers", "fcg_slab_ipc_export", "fcg_slab_ipc_open", "fcg_slab_setup", "fcg_slab_rows_fwd", "fcg_slab_cols", "fcg_slab_cols_energy", "fcg_slab_kpp0", "fcg_slab_rows_inv", "fcg_slab_update_r", "fcg_slab_scalar", "fcg_slab_finish", "fcg_slab_poll",
            "fcg_break_step_static", "fcg_static_last_error"]
 
 
@@ -105,6 +105,8 @@ def lib() -> C.CDLL:
         L.fcg_slab_setup.argtypes = [vp, d, i]; L.fcg_slab_setup.restype = i
         L.fcg_slab_rows_fwd.argtypes = [vp, i, vp]; L.fcg_slab_rows_fwd.restype = i
         L.fcg_slab_cols.argtypes = [vp]; L.fcg_slab_cols.restype = i
+        L.fcg_slab_cols_energy.argtypes = [vp, vp]; L.fcg_slab_cols_energy.restype = i
+        L.fcg_slab_kpp0.argtypes = [vp, vp, vp]; L.fcg_slab_kpp0.restype = i
         L.fcg_slab_rows_inv.argtypes = [vp, i, vp, vp, vp, vp]; L.fcg_slab_rows_inv.restype = i
         L.fcg_slab_update_r.argtypes = [vp, vp]; L.fcg_slab_update_r.restype = i
         L.fcg_slab_scalar.argtypes = [vp, i, vp]; L.fcg_slab_scalar.restype = i
@@ -461,15 +463,22 @@ class Fcg:
     def fcg_slab_cols(self):
         self._ok(self._lib.fcg_slab_cols(self._h))
 
-    def fcg_slab_rows_inv(self, residual: bool, k: torch.Tensor, u, f, xch: torch.Tensor):
-        self._ok(self._lib.fcg_slab_rows_inv(self._h, 1 if residual else 0, self._chk(k), self._chk(u) if u is not None else None,
-                                             self._chk(f) if f is not None else None, self._chk(xch, 2, torch.float64)))
+    def fcg_slab_cols_energy(self, xch: torch.Tensor):
+        self._ok(self._lib.fcg_slab_cols_energy(self._h, self._chk(xch, 4, torch.float64)))
+
+    def fcg_slab_kpp0(self, k: torch.Tensor, xch: torch.Tensor):
+        self._ok(self._lib.fcg_slab_kpp0(self._h, self._chk(k), self._chk(xch, 4, torch.float64)))
+
+    def fcg_slab_rows_inv(self, residual, k: torch.Tensor, u, f, xch: torch.Tensor):
+        """residual: 0 / False (q = A p), 1 / True (r = f - A u), 2 (fused: r -= alpha A p)."""
+        self._ok(self._lib.fcg_slab_rows_inv(self._h, int(residual), self._chk(k), self._chk(u) if u is not None else None,
+                                             self._chk(f) if f is not None else None, self._chk(xch, 4, torch.float64)))
 
     def fcg_slab_update_r(self, xch: torch.Tensor):
-        self._ok(self._lib.fcg_slab_update_r(self._h, self._chk(xch, 2, torch.float64)))
+        self._ok(self._lib.fcg_slab_update_r(self._h, self._chk(xch, 4, torch.float64)))
 
     def fcg_slab_scalar(self, what: int, xch: torch.Tensor):
-        self._ok(self._lib.fcg_slab_scalar(self._h, int(what), self._chk(xch, 2, torch.float64)))
+        self._ok(self._lib.fcg_slab_scalar(self._h, int(what), self._chk(xch, 4, torch.float64)))
 
     def fcg_slab_finish(self, u: torch.Tensor):
         self._ok(self._lib.fcg_slab_finish(self._h, self._chk(u)))

@@ -832,12 +832,31 @@ int slab_rows_fwd_impl(fcg_handle h, int mode, void* xu) {
     return FCG_OK;
 }
 template <typename T>
-int slab_cols_impl(fcg_handle h) {
+int slab_cols_impl(fcg_handle h, void* xch = nullptr) {       // xch: also this rank's share of sum shat |P|^2 (spectral search length)
     ColArgs<T> A{}; A.mode = COL_CONV; A.Tb = reinterpret_cast<cx<T>*>(h->ws + h->slab_R); A.shat = h->at<T>(h->lay.shat); A.tw = h->at<cx<T>>(h->lay.tw);
     A.sc = h->sc(); A.nsm = h->nsm; A.nranks = h->slab_G; A.al = h->slab_Al; A.boxa = h->slab_boxa;
     A.peer_maps = h->slab_peer_maps; A.prank = h->slab_rank; A.mbl = h->slab_MBl; A.tmo = &h->sc()->timeout; A.col0 = h->slab_rank * ((h->L / 2) / h->slab_G);
+    const int ncols = (h->L / 2) / h->slab_G;
     ++h->launches;
-    FCG_CK(h, h->tab->col2_slab(&A, &h->tmap_col_s, (h->L / 2) / h->slab_G, h->stream));
+    if (xch) {
+        A.partial = h->at<double>(h->lay.partial_col);
+        FCG_CK(h, h->tab->col2_slab_e(&A, &h->tmap_col_s, ncols, h->stream));
+        ++h->launches;
+        slab_energy_kernel<<<1, 256, 0, h->stream>>>(h->at<double>(h->lay.partial_col), ncols, (double*)xch, h->sc());
+        FCG_CK(h, cudaGetLastError());
+        return FCG_OK;
+    }
+    FCG_CK(h, h->tab->col2_slab(&A, &h->tmap_col_s, ncols, h->stream));
+    return FCG_OK;
+}
+template <typename T>
+int slab_kpp0_impl(fcg_handle h, const void* k, void* xch) {
+    const size_t nvec = (h->N / (size_t)h->slab_G) / Vec<T>::W;
+    size_t b = (nvec + 255) / 256;
+    if (b > (size_t)VEC_BLOCKS_MAX) b = VEC_BLOCKS_MAX;
+    ++h->launches;
+    cg_kpp0_kernel<T><<<(unsigned)b, 256, 0, h->stream>>>((const T*)k, (const T*)h->at<T>(h->lay.r), nvec, h->at<double>(h->lay.partial_vec), h->sc(), (double*)xch);
+    FCG_CK(h, cudaGetLastError());
     return FCG_OK;
 }
 template <typename T>
@@ -848,6 +867,11 @@ int slab_rows_inv_impl(fcg_handle h, int mode, const void* k, const void* v, con
     A.scale = (T)(1.0 / ((double)h->L * (double)h->L)); A.partial = h->at<double>(h->lay.partial_row); A.sc = h->sc(); A.nsm = h->nsm;
     A.tmo = &h->sc()->timeout; A.ntile = h->slab_Al; A.xch = (double*)xch;
     ++h->launches;
+    if (mode == ROWI_CGF) {          // q is consumed on the spot: strips k, p, r of the own rows, r in place (fcg_async.cuh, VAR = 5)
+        A.f = h->at<T>(h->lay.r); A.out = h->at<T>(h->lay.r); A.out2 = nullptr;
+        FCG_CK(h, h->tab->row_inv2_slab_f(&A, &h->tmap_row_s, h->stream));
+        return FCG_OK;
+    }
     FCG_CK(h, h->tab->row_inv2_slab(&A, &h->tmap_row_s, h->stream));
     return FCG_OK;
 }
@@ -1525,10 +1549,24 @@ int fcg_slab_cols(fcg_handle h) {
     return h->dtype == FCG_F64 ? slab_cols_impl<double>(h) : slab_cols_impl<float>(h);
 }
 
+int fcg_slab_cols_energy(fcg_handle h, void* xch) {
+    FCG_SLAB_ENTER(h);
+    if (!h->have_spectrum) return fail(h, FCG_NO_SPECTRUM, "fcg_set_spectrum has not been called");
+    if (!xch) return fail(h, FCG_INVALID_ARG, "null argument");
+    return h->dtype == FCG_F64 ? slab_cols_impl<double>(h, xch) : slab_cols_impl<float>(h, xch);
+}
+
+int fcg_slab_kpp0(fcg_handle h, const void* k, void* xch) {
+    FCG_SLAB_ENTER(h);
+    if (!k || !xch) return fail(h, FCG_INVALID_ARG, "null argument");
+    return h->dtype == FCG_F64 ? slab_kpp0_impl<double>(h, k, xch) : slab_kpp0_impl<float>(h, k, xch);
+}
+
 int fcg_slab_rows_inv(fcg_handle h, int residual, const void* k, const void* u, const void* f, void* xch) {
     FCG_SLAB_ENTER(h);
-    if (!k || !xch || (residual && (!u || !f))) return fail(h, FCG_INVALID_ARG, "null argument");
-    const int mode = residual ? ROWI_RESID : ROWI_CG;
+    if (residual < 0 || residual > 2) return fail(h, FCG_INVALID_ARG, "residual must be 0, 1 or 2");
+    if (!k || !xch || (residual == 1 && (!u || !f))) return fail(h, FCG_INVALID_ARG, "null argument");
+    const int mode = residual == 1 ? ROWI_RESID : residual == 2 ? ROWI_CGF : ROWI_CG;
     return h->dtype == FCG_F64 ? slab_rows_inv_impl<double>(h, mode, k, u, f, xch) : slab_rows_inv_impl<float>(h, mode, k, u, f, xch);
 }
 
@@ -1540,7 +1578,7 @@ int fcg_slab_update_r(fcg_handle h, void* xch) {
 
 int fcg_slab_scalar(fcg_handle h, int what, const void* xch) {
     FCG_SLAB_ENTER(h);
-    if (!xch || what < 0 || what > 2) return fail(h, FCG_INVALID_ARG, "bad argument");
+    if (!xch || what < 0 || what > 5) return fail(h, FCG_INVALID_ARG, "bad argument");
     slab_scalar_kernel<<<1, 32, 0, h->stream>>>(h->sc(), what, (const double*)xch); ++h->launches;
     FCG_CK(h, cudaGetLastError());
     return FCG_OK;

@@ -516,7 +516,7 @@ __global__ void __launch_bounds__(P::NT, CTAS) col2_kernel(const ColArgs<T> A, c
         __shared__ double red[32];
         double ev[1] = {energy};
         block_sum<1>(ev, red);
-        if (lt == 0) A.partial[n] = ev[0];
+        if (lt == 0) A.partial[nl] = ev[0];       // (slab: one per column of THIS rank; fcg_slab_cols_energy sums them)
     }
     if (lt == 0) tma::bulk_wait_read0();          // shared memory must outlive the store's read
 }
@@ -1025,8 +1025,10 @@ __global__ void __launch_bounds__(AsyncShape<T, P>::INV_THREADS, CTAS) row_inv2_
 {
     using AS = AsyncShape<T, P>;
     constexpr int L = P::N, S = P::S, NT = P::NT, R1 = AS::R1, Q1 = AS::Q1, PER1 = AS::PER1, PM = per_max<P>();
-    constexpr bool PRE = VAR == 1, CGF = VAR == 2 || VAR == 3, FCGF = VAR == 3;
-    constexpr bool SLAB = VAR == 4;      // one rank's row slab: A.ntile row pairs; sums go to A.xch, no scalar step
+    constexpr bool PRE = VAR == 1, CGF = VAR == 2 || VAR == 3 || VAR == 5, FCGF = VAR == 3;
+    constexpr bool SLAB = VAR == 4 || VAR == 5;      // one rank's row slab: A.ntile row pairs; sums go to A.xch, no scalar step
+    constexpr bool SCGF = VAR == 5;      // slab + fused residual update: alpha comes from the scalar block (fcg_slab_scalar(4) after the all-reduce
+                                         // of the ranks' spectral sums), the three sums of the own rows go to A.xch
     constexpr int TSUB = AS::TSUB, NSUB = AS::NSUB;
     constexpr uint32_t TBYTES = (uint32_t)AS::TSB;
     // CGF moves three vectors of strips per transform against one of tiles: the tile ring is kept short (TCAP) and the strips
@@ -1118,7 +1120,9 @@ __global__ void __launch_bounds__(AsyncShape<T, P>::INV_THREADS, CTAS) row_inv2_
         ++p_kn;
         if (++p_ks == nks) { p_ks = 0; p_kph ^= 1u; }
     };
-    if constexpr (CGF) {
+    if constexpr (SCGF) {
+        pq_d = A.sc->pq; alpha_d = A.sc->alpha; alpha = (T)alpha_d;      // (a breakdown has set sc->done: the pass returned above)
+    } else if constexpr (CGF) {
         // search length from the column pass's partial sums, by ALL threads before the roles split (a breakdown must
         // stop producers and consumers alike); same order in every CTA, so alpha is bit-identical everywhere
         double e = 0.0;
@@ -1255,6 +1259,10 @@ __global__ void __launch_bounds__(AsyncShape<T, P>::INV_THREADS, CTAS) row_inv2_
     if constexpr (CGF) {         // all warps (the producers contribute zeros)
         double tot[3];
         if (!grid_sum_last<3>(acc3, A.partial, &A.sc->ticket[0], red, tot)) return;
+        if constexpr (SCGF) {
+            if (threadIdx.x == 0) { A.xch[0] = tot[0]; A.xch[1] = tot[1]; A.xch[2] = tot[2]; A.xch[3] = 0.0; }
+            return;
+        }
         if (threadIdx.x == 0) {
             Scalars* sc = A.sc;
             sc->alpha = alpha_d; sc->pq = pq_d;

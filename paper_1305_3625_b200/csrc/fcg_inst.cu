@@ -59,6 +59,8 @@ template <typename T> struct Inst {
             if ((e = prep(row_fwd2_kernel<T, P, C_FWD, 2>, AS::fwd_smem)) != cudaSuccess) return e;
             if ((e = prep(col2_kernel<T, P, C_COL, false, true>, AS::col_smem)) != cudaSuccess) return e;
             if ((e = prep(row_inv2_kernel<T, P, C_INV, 4>, AS::inv_smem)) != cudaSuccess) return e;
+            if ((e = prep(col2_kernel<T, P, C_COL, true, true>, AS::col_smem)) != cudaSuccess) return e;
+            if ((e = prep(row_inv2_kernel<T, P, C_INV, 5>, AS::inv_smem)) != cudaSuccess) return e;
             if ((e = prep(col2_xform_kernel<T, P, C_COL, -1>, AS::WBYTES + 128)) != cudaSuccess) return e;
             if ((e = prep(col2_xform_kernel<T, P, C_COL, +1>, AS::WBYTES + 128)) != cudaSuccess) return e;
             if ((e = prep(col2_xpub_kernel<T, P, C_COL, -1>, AS::WBYTES + 128)) != cudaSuccess) return e;
@@ -112,6 +114,21 @@ template <typename T> struct Inst {
         if constexpr (V2) {
             const ColArgs<T>& A = *static_cast<const ColArgs<T>*>(args);
             return launch(col2_kernel<T, P, C_COL, false, true>, ncols, P::NT, AS::col_smem, st, 0, A, *static_cast<const CUtensorMap*>(tensor_map));
+        }
+        return cudaErrorInvalidValue;
+    }
+    static cudaError_t col2_slab_e(const void* args, const void* tensor_map, int ncols, cudaStream_t st) {
+        if constexpr (V2) {
+            const ColArgs<T>& A = *static_cast<const ColArgs<T>*>(args);
+            return launch(col2_kernel<T, P, C_COL, true, true>, ncols, P::NT, AS::col_smem, st, 0, A, *static_cast<const CUtensorMap*>(tensor_map));
+        }
+        return cudaErrorInvalidValue;
+    }
+    static cudaError_t row_inv2_slab_f(const void* args, const void* tensor_map, cudaStream_t st) {
+        if constexpr (V2) {
+            const RowInvArgs<T>& A = *static_cast<const RowInvArgs<T>*>(args);
+            return launch(row_inv2_kernel<T, P, C_INV, 5>, pgrid_n(A.nsm, C_INV, A.ntile), AS::INV_THREADS, AS::inv_smem, st, 0, A,
+                          *static_cast<const CUtensorMap*>(tensor_map));
         }
         return cudaErrorInvalidValue;
     }
@@ -308,6 +325,7 @@ template <typename T> struct Inst {
         t.colp_ok = COLP ? 1 : 0; t.colp_ctas = COLP ? CPS::CTAS : 0; t.col2p = &col2p;
         t.sl_ok = SL ? 1 : 0; t.col2_energy = &col2_energy; t.row_inv2_cgf = &row_inv2_cgf; t.row_inv2_cgf_force = &row_inv2_cgf_force;
         t.row_fwd2_slab = &row_fwd2_slab; t.col2_slab = &col2_slab; t.row_inv2_slab = &row_inv2_slab;
+        t.col2_slab_e = &col2_slab_e; t.row_inv2_slab_f = &row_inv2_slab_f;
         t.col2_xform = &col2_xform; t.col2_xpub = &col2_xpub; t.t2_export = &t2_export; t.t2_import = &t2_import;
         t.fused = FS::valid ? 1 : 0; t.fused_grid = FS::G; t.fused_solve = &fused_solve;
         t.init = &init; t.row_fwd = &row_fwd; t.col = &col; t.row_inv = &row_inv; t.spectrum_prep = &spectrum_prep;

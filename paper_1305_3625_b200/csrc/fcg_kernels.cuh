@@ -264,16 +264,46 @@ __global__ void slab_scalar_kernel(Scalars* sc, int what, const double* xch) {
         sc->pq = pq;
         if (!(pq > 0.0) || !isfinite(pq)) { sc->status = ST_BREAKDOWN; sc->done = 1; sc->alpha = 0.0; }
         else sc->alpha = sc->rho / pq;
-    } else {
+    } else if (what == 2) {
         if (sc->done) return;
         cg_after_rr(sc, xch[0]);
+    } else if (what == 3) {          // spectral search length (DESIGN.md sections 12, 18): start of the recurrence, sum k p^2 with p = r
+        sc->kpp = xch[2];
+    } else if (what == 4) {          // alpha from the all-reduced spectral sums: p.Ap = sum k p^2 + sum shat |P|^2
+        if (sc->done) return;
+        const double pq = sc->kpp + xch[0];
+        sc->pq = pq;
+        if (!(pq > 0.0) || !isfinite(pq)) { sc->status = ST_BREAKDOWN; sc->done = 1; sc->alpha = 0.0; }
+        else sc->alpha = sc->rho / pq;
+    } else {                         // after the fused last pass: xch = { r'.r', sum k r'^2, sum k r' p }
+        if (sc->done) return;
+        const double kpp = sc->kpp;
+        cg_after_rr(sc, xch[0]);
+        if (!sc->done) sc->kpp = xch[1] + 2.0 * sc->beta * xch[2] + sc->beta * sc->beta * kpp;
+    }
+}
+// this rank's share of the spectral half of p.Ap: the column pass's per-column sums, added in a fixed order
+__global__ void __launch_bounds__(256) slab_energy_kernel(const double* __restrict__ colsum, int n, double* xch, const Scalars* sc) {
+    __shared__ double red[8];
+    if (sc->done) return;
+    double e = 0.0;
+    for (int i = threadIdx.x; i < n; i += 256) e += colsum[i];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) e += __shfl_xor_sync(0xffffffffu, e, o);
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = e;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        e = 0.0;
+        for (int w = 0; w < 8; ++w) e += red[w];
+        xch[0] = e; xch[1] = 0.0; xch[2] = 0.0; xch[3] = 0.0;
     }
 }
 #endif
 
 // spectral search length: start value of the recurrence for sum k p^2 -- the first direction is p = r
 template <typename T>
-__global__ void __launch_bounds__(256) cg_kpp0_kernel(const T* __restrict__ k, const T* __restrict__ r, size_t nvec, double* partial, Scalars* sc) {
+__global__ void __launch_bounds__(256) cg_kpp0_kernel(const T* __restrict__ k, const T* __restrict__ r, size_t nvec, double* partial, Scalars* sc,
+                                                      double* xch = nullptr) {       // slab: the sum of the own rows goes to xch[2] instead
     __shared__ double red[32];
     using V = typename Vec<T>::type;
     if (sc->done) return;
@@ -295,7 +325,7 @@ __global__ void __launch_bounds__(256) cg_kpp0_kernel(const T* __restrict__ k, c
     }
     double tot[1];
     if (!grid_sum_last<1>(acc, partial, &sc->ticket2[0], red, tot)) return;
-    if (threadIdx.x == 0) sc->kpp = tot[0];
+    if (threadIdx.x == 0) { if (xch) xch[2] = tot[0]; else sc->kpp = tot[0]; }
 }
 
 // The force problem through the displacements (reading F7): (K + G^-1) u = K D is fcg_solve / fcg_pcg_solve

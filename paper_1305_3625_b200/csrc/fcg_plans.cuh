@@ -102,6 +102,9 @@ struct PassTable {
     cudaError_t (*row_fwd2_slab)(const void* args, cudaStream_t st);
     cudaError_t (*col2_slab)(const void* args, const void* tensor_map, int ncols, cudaStream_t st);
     cudaError_t (*row_inv2_slab)(const void* args, const void* tensor_map, cudaStream_t st);
+    // the same with the spectral search length: column pass with its share of sum shat |P|^2, last pass with the residual update fused in
+    cudaError_t (*col2_slab_e)(const void* args, const void* tensor_map, int ncols, cudaStream_t st);
+    cudaError_t (*row_inv2_slab_f)(const void* args, const void* tensor_map, cudaStream_t st);
     // whole solve as one cooperative kernel (fcg_fused.cuh); fused == 0 when the size has none
     int fused, fused_grid;
     cudaError_t (*fused_solve)(const void* fused_args, cudaStream_t st);

@@ -85,7 +85,7 @@ class SlabRank:
         self.h.fcg_set_spectrum(s_full)
         self.h.fcg_slab_configure(nranks, rank)
         self.send, self.recv = self.h.fcg_slab_buffers()
-        self.xch = torch.zeros(2, dtype=torch.float64, device=device)
+        self.xch = torch.zeros(4, dtype=torch.float64, device=device)     # this rank's shares of the iteration's sums, all-reduced in place
         self.rows = slice(rank * self.shape["rows_local"], (rank + 1) * self.shape["rows_local"])
 
     def close(self):
@@ -112,25 +112,29 @@ def connect_peers_dist(rank_obj, comm):
     rank_obj.peers = True
 
 
-def _operator_round_trip(ranks, comm):
-    """S (row transforms of the own rows) -> columns -> S (ready for the inverse row transforms), on every rank."""
+def _operator_round_trip(ranks, comm, energy=False):
+    """S (row transforms of the own rows) -> columns -> S (ready for the inverse row transforms), on every rank.
+    energy: the column pass also leaves the rank's share of sum shat |P|^2 in xch[0] (spectral search length)."""
     peers = getattr(ranks[0], "peers", False)
     if peers:
         comm.barrier([r.xch for r in ranks])         # every rank's row pass has delivered its lines into the owners' R
     else:
         comm.all_to_all([r.recv for r in ranks], [r.send for r in ranks])
-    for r in ranks:
-        r.h.fcg_slab_cols()                          # on R in place: a 5-D tensor map reads the exchange layout as columns
+    for r in ranks:                                  # on R in place: a 5-D tensor map reads the exchange layout as columns
+        r.h.fcg_slab_cols_energy(r.xch) if energy else r.h.fcg_slab_cols()
     if peers:
         comm.barrier([r.xch for r in ranks])         # every rank's column pass has scattered into the owners' S
     else:
         comm.all_to_all([r.send for r in ranks], [r.recv for r in ranks])
 
 
-def slab_solve(ranks, comm, k, f, u, tol: float, maxit: int, poll_every: int = 8):
+def slab_solve(ranks, comm, k, f, u, tol: float, maxit: int, poll_every: int = 8, spectral: bool = True):
     """Solve A u = f with the lattice split by rows over `ranks` (all the ranks of this process: one with DistComm, G with
     LocalComm).  k, f, u: lists, one tensor of the rank's own rows each; u in: initial guess, out: solution.
+    spectral: the iteration with the spectral search length (three passes, include/fcg.h), else the textbook order (four).
     Returns (iters, rel_residual, status) -- identical on every rank."""
+    if spectral:
+        return _slab_solve_spectral(ranks, comm, k, f, u, tol, maxit, poll_every)
     xs = [r.xch for r in ranks]
     for r, ui in zip(ranks, u):
         r.h.fcg_slab_setup(tol, maxit)
@@ -158,6 +162,44 @@ def slab_solve(ranks, comm, k, f, u, tol: float, maxit: int, poll_every: int = 8
             comm.all_reduce(xs)
             for r in ranks:
                 r.h.fcg_slab_scalar(2, r.xch)                   # count, convergence, beta
+    for r, ui in zip(ranks, u):
+        r.h.fcg_slab_finish(ui)
+    for r in ranks[1:]:
+        r.h.fcg_slab_poll()
+    return it, rr, st
+
+
+def _slab_solve_spectral(ranks, comm, k, f, u, tol, maxit, poll_every):
+    """p.Ap = sum k p^2 + sum shat |P|^2 (Parseval): alpha is known once the ranks' column passes have added up their shares, so the
+    last pass applies r -= alpha q on the fly -- one pass and one kernel less per iteration than the textbook order, the same two
+    all-reduces (the first one now overlaps the backward exchange's place in the stream)."""
+    xs = [r.xch for r in ranks]
+    for r, ui in zip(ranks, u):
+        r.h.fcg_slab_setup(tol, maxit)
+        r.h.fcg_slab_rows_fwd(False, ui)
+    _operator_round_trip(ranks, comm)
+    for r, ki, fi, ui in zip(ranks, k, f, u):
+        r.h.fcg_slab_rows_inv(1, ki, ui, fi, r.xch)             # r = f - A u, p := 0; xch = {r.r, f.f}
+        r.h.fcg_slab_kpp0(ki, r.xch)                            # xch[2] = sum k r^2 (the first direction is p = r)
+    comm.all_reduce(xs)
+    for r in ranks:
+        r.h.fcg_slab_scalar(0, r.xch)
+        r.h.fcg_slab_scalar(3, r.xch)
+    while True:
+        done, it, rr, st = ranks[0].h.fcg_slab_poll()
+        if done:
+            break
+        for _ in range(max(1, int(poll_every))):
+            for r, ui in zip(ranks, u):
+                r.h.fcg_slab_rows_fwd(True, ui)                 # u += alpha p (lagged), p = r + beta p, row transforms of p
+            _operator_round_trip(ranks, comm, energy=True)      # xch[0] = the rank's share of sum shat |P|^2
+            comm.all_reduce(xs)
+            for r, ki in zip(ranks, k):
+                r.h.fcg_slab_scalar(4, r.xch)                   # alpha
+                r.h.fcg_slab_rows_inv(2, ki, None, None, r.xch)     # r -= alpha (k o p + C p); xch = {r.r, sum k r^2, sum k r p}
+            comm.all_reduce(xs)
+            for r in ranks:
+                r.h.fcg_slab_scalar(5, r.xch)                   # count, convergence, beta, sum k p'^2
     for r, ui in zip(ranks, u):
         r.h.fcg_slab_finish(ui)
     for r in ranks[1:]:

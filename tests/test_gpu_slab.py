@@ -31,7 +31,7 @@ def rel(a, b):
     return np.linalg.norm(a - b) / max(np.linalg.norm(b), 1e-300)
 
 
-def slab_run(w, G, tol, maxit, u0=None, peers=False):
+def slab_run(w, G, tol, maxit, u0=None, peers=False, spectral=False):
     from paper_1305_3625_b200 import slab
     dt = w.dtype.type
     sd = dev(w.s)
@@ -40,7 +40,7 @@ def slab_run(w, G, tol, maxit, u0=None, peers=False):
         slab.connect_peers_local(ranks)
     k = [dev(w.k[r.rows]) for r in ranks]; f = [dev(w.f[r.rows]) for r in ranks]
     u = [dev((w.u0 if u0 is None else u0)[r.rows]) for r in ranks]
-    it, rr, st = slab.slab_solve(ranks, slab.LocalComm(), k, f, u, tol, maxit)
+    it, rr, st = slab.slab_solve(ranks, slab.LocalComm(), k, f, u, tol, maxit, spectral=spectral)
     out = np.concatenate([x.cpu().numpy() for x in u], axis=0)
     for r in ranks:
         r.close()
@@ -161,3 +161,79 @@ def test_slab_peer_mode_fused_exchange(B, cfg, L, dt, G):
     ref = orc.cg(w.s, w.k, w.f, w.u0, 0.0, 6)
     it, _, _, u = slab_run(w, G, 0.0, 6, peers=True)
     assert it == 6 and rel(u, ref["u"]) <= 0.1 * TOL_CG[dt]
+
+
+# ---- the slab iteration with the spectral search length (three passes; include/fcg.h, DESIGN.md sections 12 and 18)
+
+@pytest.mark.parametrize("cfg,L,dt", [(1, 256, np.float64), (2, 512, np.float64), (1, 1024, np.float64), (4, 1024, np.float32),
+                                      (2, 2048, np.float32), (2, 2048, np.float64)])
+@pytest.mark.parametrize("G,peers", [(1, False), (2, False), (4, True), (8, True)])
+def test_slab_spectral_matches_oracle(B, cfg, L, dt, G, peers):
+    """Same protocol as test_slab_cg_matches_oracle; configs[2] fp64 at full size is classified as in test_slab_cg_full_size_config2
+    (reading S20) when the solve happens to stop at the oracle's count."""
+    w = inputs.config(cfg, dt, L=L)
+    ref = orc.cg(w.s, w.k, w.f, w.u0, w.tol, w.maxit, history=True)
+    it, rr, st, u = slab_run(w, G, w.tol, w.maxit, peers=peers, spectral=True)
+    assert st == ref["status"] and abs(it - ref["iters"]) <= 2, (it, ref["iters"])
+    d = rel(u, ref["u"])
+    if it != ref["iters"] and d > TOL_CG[dt]:
+        it2, _, _, u = slab_run(w, G, 0.0, ref["iters"], peers=peers, spectral=True)
+        assert it2 == ref["iters"]
+        d = rel(u, ref["u"])
+    if (cfg, L, dt) == (2, 2048, np.float64) and d > TOL_CG[dt]:
+        drift = cfg2_drift()
+        assert d <= drift[ref["iters"]] and drift[ref["iters"]] > TOL_CG[dt], (d, drift)
+    else:
+        assert d <= TOL_CG[dt], (d, it, ref["iters"])
+    assert rr <= w.tol
+    refp = orc.cg(w.s, w.k, w.f, w.u0, 0.0, 5, history=True)
+    itp, rrp, _, up = slab_run(w, G, 0.0, 5, peers=peers, spectral=True)
+    assert itp == 5 and rel(up, refp["u"]) <= 0.1 * TOL_CG[dt]
+    assert abs(rrp - refp["hist"][5]) <= 1e-3 * refp["hist"][5]
+
+
+@pytest.mark.parametrize("L,dt", [(512, np.float64), (2048, np.float32)])
+def test_slab_spectral_equals_other_orders(B, L, dt):
+    """The three-pass slab iteration agrees (a) at a pinned count with the undecomposed three-launch solve (the same arithmetic per
+    element; the order of the partial sums differs) and (b) at the stop with the four-pass slab iteration (alpha from Parseval's
+    sum instead of p.q: reading D5's bound, a fifth of the tolerance; in mid-run the two evaluations drift apart like any two
+    correct implementations, reading S19 -- 2.7e-5 after 30 iterations at L = 2048 fp32), for every G and both exchange modes."""
+    w = inputs.config(1, dt, L=L)
+    h = B.Fcg(w.L, TDT[dt])
+    h.fcg_set_option(B.FCG_OPT_FUSED, 0)
+    h.fcg_set_spectrum(dev(w.s))
+    u = dev(w.u0)
+    it0, rr0, st0 = h.fcg_solve(dev(w.k), dev(w.f), u, 0.0, 30)
+    u0 = u.cpu().numpy()
+    h.close()
+    eps = 1e-12 if dt == np.float64 else 2e-6
+    for G, peers in ((1, False), (2, True), (4, False), (8, True)):
+        it, rr, st, ug = slab_run(w, G, 0.0, 30, peers=peers, spectral=True)
+        assert (it, st) == (it0, st0) and rel(ug, u0) <= eps and abs(rr - rr0) <= 1e3 * eps * rr0, (G, rel(ug, u0), rr, rr0)
+        it4, _, st4, u4 = slab_run(w, G, w.tol, w.maxit, peers=peers, spectral=False)          # (b) at the four-pass solve's own stop,
+        it3, _, _, u3 = slab_run(w, G, 0.0, it4, peers=peers, spectral=True)                   #     as test_cg_both_search_length_evaluations
+        assert st4 == 0 and it3 == it4 and rel(u3, u4) <= 0.2 * TOL_CG[dt], (G, it4, rel(u3, u4))
+
+
+def test_slab_spectral_edge_cases(B):
+    w = inputs.config(0, np.float64, L=256)
+    it, rr, st, u = slab_run(w, 2, w.tol, w.maxit, spectral=True)
+    ref = orc.cg(w.s, w.k, w.f, w.u0, w.tol, w.maxit)
+    assert st == 0 and abs(it - ref["iters"]) <= 2 and rel(u, ref["u"]) <= TOL_CG[np.float64]
+    it2, rr2, st2, _ = slab_run(w, 2, 10 * w.tol, w.maxit, u0=u, spectral=True)          # warm start from the solution
+    assert (it2, st2) == (0, 0)
+    it3, _, st3, u3 = slab_run(w, 4, w.tol, 0, spectral=True)                             # maxit = 0
+    assert (it3, st3) == (0, B.FCG_NOT_CONVERGED) and not u3.any()
+    it5, _, st5, _ = slab_run(w, 4, w.tol, 7, spectral=True)                              # maxit reached
+    assert (it5, st5) == (7, B.FCG_NOT_CONVERGED)
+    w.f[:] = 0
+    it4, rr4, st4, u4 = slab_run(w, 2, w.tol, w.maxit, u0=np.ones_like(w.u0), spectral=True)
+    assert (it4, rr4, st4) == (0, 0.0, 0) and not u4.any()
+    # breakdown (reading S15): a negative-definite operator gives p.Ap < 0 in the first iteration; nothing may change after it
+    w = inputs.config(0, np.float64, L=256)
+    w.k[:] = -50.0
+    ref = orc.cg(w.s, w.k, w.f, w.u0, w.tol, 50)
+    for spectral in (True, False):
+        it6, _, st6, u6 = slab_run(w, 2, w.tol, 50, spectral=spectral)
+        assert st6 == ref["status"] == B.FCG_BREAKDOWN and it6 == ref["iters"]
+        assert np.linalg.norm(u6 - ref["u"]) <= 1e-9 * max(np.linalg.norm(ref["u"]), 1e-300) or not (u6.any() or ref["u"].any())
