@@ -472,6 +472,7 @@ def run_slab(args, rank, world, local):
         comm, G, mine = slab.LocalComm(), args.slab_ranks, list(range(args.slab_ranks))
     sd = to(w.s)
     spectral = args.slab_order == "spectral"
+    graph = {"auto": None, "on": True, "off": False}[args.slab_graph]
     ranks = [slab.SlabRank(w.L, tdt, G, g, sd) for g in mine]
     if args.slab_peers:          # the exchange fused into the passes: peer stores instead of all-to-alls
         if world > 1:
@@ -483,7 +484,7 @@ def run_slab(args, rank, world, local):
     sampler = ClockSampler(local) if rank == 0 else None
     for _ in range(args.warmup):
         for x in u: x.zero_()
-        it, rr, st = slab.slab_solve(ranks, comm, k, f, u, w.tol, w.maxit, spectral=spectral)
+        it, rr, st = slab.slab_solve(ranks, comm, k, f, u, w.tol, w.maxit, spectral=spectral, graph=graph)
     if world > 1:
         dist.barrier()
     torch.cuda.synchronize()
@@ -494,8 +495,8 @@ def run_slab(args, rank, world, local):
     e0.record()
     for _ in range(args.steps):
         for x in u: x.zero_()
-        it, rr, st = slab.slab_solve(ranks, comm, k, f, u, w.tol, w.maxit, spectral=spectral)
-        its += it; launches += sum(r.h.fcg_last_launch_count() for r in ranks)
+        it, rr, st = slab.slab_solve(ranks, comm, k, f, u, w.tol, w.maxit, spectral=spectral, graph=graph)
+        its += it; launches += sum(slab.launch_count(r) for r in ranks)
     e1.record(); torch.cuda.synchronize()
     clocks = sampler.stop() if sampler else None
     ms = e0.elapsed_time(e1)
@@ -514,7 +515,7 @@ def run_slab(args, rank, world, local):
                        "parallelism": f"slab x{G}" + (" peer mode" if args.slab_peers else ""), "launches_per_iteration_per_rank": "3 passes + 3 one-block kernels" if spectral else "4 passes + 2 one-block kernels",
                        "collectives_per_iteration": ("2 barriers" if args.slab_peers else "2 all-to-all (N w / G bytes per rank each)") + " + 2 all-reduce (32 B)",
                        "note": ("spectral search length (three passes)" if spectral else "textbook order (four passes)") +
-                               ", host poll every eighth iteration; the hardware scaling curve is unmeasured on this one-GPU pool"},
+                               ", host poll every eighth iteration" + ("" if graph is False or (graph is None and world > 1) else ", blocks of eight iterations replayed from a CUDA graph") + "; the hardware scaling curve is unmeasured on this one-GPU pool"},
             "site_iterations_per_s": its / (ms * 1e-3) * w.N, "us_per_iteration": t_iter_us,
             "exchange_bytes_per_iteration_per_rank": 2.0 * nw / G * (G - 1) / G,
             "gpu_launches": launches, "clocks": clocks, "final_rel_residual": rr, "status": st}))
@@ -556,6 +557,8 @@ def main():
                          "over the ranks: all-to-all transposes around the column pass, all-reduce of the scalars; DESIGN.md section 18)")
     ap.add_argument("--slab-order", choices=["spectral", "textbook"], default="spectral",
                     help="--shard slab: the iteration with the spectral search length (three passes per iteration, default) or in the textbook order (four)")
+    ap.add_argument("--slab-graph", choices=["auto", "on", "off"], default="auto",
+                    help="--shard slab: replay blocks of iterations from a CUDA graph (auto: on for logical ranks, off under torchrun)")
     ap.add_argument("--slab-peers", action="store_true",
                     help="--shard slab: peer mode -- the row pass stores straight into the owning rank's exchange buffer and the column pass "
                          "scatters straight into the source ranks' T2 (CUDA IPC mappings over NVLink under torchrun); barriers replace the all-to-alls")

@@ -113,6 +113,11 @@ size_t fcg_workspace_bytes(int L, fcg_dtype dt);
 int fcg_create(int L, fcg_dtype dt, void* workspace, void* cuda_stream, fcg_handle* out);
 int fcg_destroy(fcg_handle h);
 int fcg_set_option(fcg_handle h, int option, int value);
+/* Later calls enqueue on `cuda_stream` instead of the one given to fcg_create.  The caller orders the two streams (work already
+ * enqueued stays where it is); refused (FCG_INVALID_ARG) while a quasi-static loop is pending.  This is what lets a caller
+ * record the asynchronous calls (the fcg_slab_* passes, fcg_break_step_static aside) into a CUDA graph of its own: stream
+ * capture runs on a stream other than the legacy default one (paper_1305_3625_b200/slab.py does exactly that). */
+int fcg_set_stream(fcg_handle h, void* cuda_stream);
 
 /* Static spectrum ("the FFT of G is static and performed during initialization").
  *   s  device, L x L reals, row-major [m][n].  Copied into an internal layout (even part, scaled by

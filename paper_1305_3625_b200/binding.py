@@ -35,7 +35,7 @@ EXPORTS = ["fcg_workspace_bytes", "fcg_create", "fcg_destroy", "fcg_set_option",
            "fcg_green_function", "fcg_kernel_spectrum", "fcg_force_apply", "fcg_force_solve", "fcg_force_break_step",
            "fcg_force_fracture", "fcg_inverse_spectrum", "fcg_force_rhs", "fcg_force_from_displacement",
            "fcg_force_fracture_displacement", "fcg_force_fracture_displacement_begin", "fcg_force_fracture_displacement_end",
-           "fcg_slab_shape_of", "fcg_slab_configure", "fcg_slab_buffers", "fcg_slab_set_peers", "fcg_slab_ipc_export", "fcg_slab_ipc_open", "fcg_slab_setup", "fcg_slab_rows_fwd", "fcg_slab_cols", "fcg_slab_cols_energy", "fcg_slab_kpp0", "fcg_slab_rows_inv", "fcg_slab_update_r", "fcg_slab_scalar", "fcg_slab_finish", "fcg_slab_poll",
+           "fcg_set_stream", "fcg_slab_shape_of", "fcg_slab_configure", "fcg_slab_buffers", "fcg_slab_set_peers", "fcg_slab_ipc_export", "fcg_slab_ipc_open", "fcg_slab_setup", "fcg_slab_rows_fwd", "fcg_slab_cols", "fcg_slab_cols_energy", "fcg_slab_kpp0", "fcg_slab_rows_inv", "fcg_slab_update_r", "fcg_slab_scalar", "fcg_slab_finish", "fcg_slab_poll",
            "fcg_break_step_static", "fcg_static_last_error"]
 
 
@@ -104,6 +104,7 @@ def lib() -> C.CDLL:
         L.fcg_slab_ipc_open.argtypes = [vp, vp]; L.fcg_slab_ipc_open.restype = i
         L.fcg_slab_setup.argtypes = [vp, d, i]; L.fcg_slab_setup.restype = i
         L.fcg_slab_rows_fwd.argtypes = [vp, i, vp]; L.fcg_slab_rows_fwd.restype = i
+        L.fcg_set_stream.argtypes = [vp, vp]; L.fcg_set_stream.restype = i
         L.fcg_slab_cols.argtypes = [vp]; L.fcg_slab_cols.restype = i
         L.fcg_slab_cols_energy.argtypes = [vp, vp]; L.fcg_slab_cols_energy.restype = i
         L.fcg_slab_kpp0.argtypes = [vp, vp, vp]; L.fcg_slab_kpp0.restype = i
@@ -453,6 +454,10 @@ class Fcg:
     def fcg_slab_ipc_open(self, blobs: bytes):
         buf = C.create_string_buffer(bytes(blobs), len(blobs))
         self._ok(self._lib.fcg_slab_ipc_open(self._h, buf))
+
+    def fcg_set_stream(self, stream: torch.cuda.Stream):
+        self._ok(self._lib.fcg_set_stream(self._h, stream.cuda_stream))
+        self.stream = stream
 
     def fcg_slab_setup(self, tol: float, maxit: int):
         self._ok(self._lib.fcg_slab_setup(self._h, float(tol), int(maxit)))

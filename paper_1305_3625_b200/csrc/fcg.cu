@@ -970,6 +970,13 @@ int fcg_destroy(fcg_handle h) {
     return FCG_OK;
 }
 
+int fcg_set_stream(fcg_handle h, void* cuda_stream) {
+    if (!h) return FCG_INVALID_ARG;
+    FCG_ENTER_OPT(h);                    // refused while a quasi-static loop is pending: its work is in flight on the old stream
+    h->stream = (cudaStream_t)cuda_stream;
+    return FCG_OK;
+}
+
 int fcg_set_option(fcg_handle h, int option, int value) {
     if (!h) return FCG_INVALID_ARG;
     FCG_ENTER_OPT(h);

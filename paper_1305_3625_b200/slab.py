@@ -8,10 +8,11 @@ and moves the exchange buffers between the ranks:
   * LocalComm  G logical ranks that share one device and one stream (parity tests on the one-GPU pool): the all-to-all is G*G
                device copies, the all-reduce a sum of G two-element tensors.
 
-Textbook order of Listing 2 per iteration:
-    rows_fwd | all-to-all S->R | cols (on R, in place) | all-to-all R->S | rows_inv | all-reduce | scalar(1) | update_r | all-reduce |
-    scalar(2)
-with one read-back of the scalar block every `poll_every` iterations: once the device-side stopping decision has been taken
+Per iteration, with the spectral search length (default; DESIGN.md sections 12 and 18):
+    rows_fwd | all-to-all S->R | cols_energy (on R, in place) | all-to-all R->S | all-reduce | scalar(4) | rows_inv(2) | all-reduce | scalar(5)
+or in the textbook order of Listing 2:
+    rows_fwd | all-to-all S->R | cols | all-to-all R->S | rows_inv | all-reduce | scalar(1) | update_r | all-reduce | scalar(2)
+(peer mode: the all-to-alls are barriers, the passes store straight into the peers' buffers), with one read-back of the scalar block every `poll_every` iterations: once the device-side stopping decision has been taken
 (identically on every rank) the remaining passes of the chunk return at once without touching anything.
 """
 from __future__ import annotations
@@ -128,78 +129,115 @@ def _operator_round_trip(ranks, comm, energy=False):
         comm.all_to_all([r.send for r in ranks], [r.recv for r in ranks])
 
 
-def slab_solve(ranks, comm, k, f, u, tol: float, maxit: int, poll_every: int = 8, spectral: bool = True):
-    """Solve A u = f with the lattice split by rows over `ranks` (all the ranks of this process: one with DistComm, G with
-    LocalComm).  k, f, u: lists, one tensor of the rank's own rows each; u in: initial guess, out: solution.
-    spectral: the iteration with the spectral search length (three passes, include/fcg.h), else the textbook order (four).
-    Returns (iters, rel_residual, status) -- identical on every rank."""
-    if spectral:
-        return _slab_solve_spectral(ranks, comm, k, f, u, tol, maxit, poll_every)
+def _set_up(ranks, comm, k, f, u, tol, maxit, spectral):
     xs = [r.xch for r in ranks]
     for r, ui in zip(ranks, u):
         r.h.fcg_slab_setup(tol, maxit)
         r.h.fcg_slab_rows_fwd(False, ui)
     _operator_round_trip(ranks, comm)
     for r, ki, fi, ui in zip(ranks, k, f, u):
-        r.h.fcg_slab_rows_inv(True, ki, ui, fi, r.xch)          # r = f - A u, p := 0; xch = {r.r, f.f} of the own rows
+        r.h.fcg_slab_rows_inv(1, ki, ui, fi, r.xch)             # r = f - A u, p := 0; xch = {r.r, f.f} of the own rows
+        if spectral:
+            r.h.fcg_slab_kpp0(ki, r.xch)                        # xch[2] = sum k r^2 (the first direction is p = r)
     comm.all_reduce(xs)
     for r in ranks:
         r.h.fcg_slab_scalar(0, r.xch)
+        if spectral:
+            r.h.fcg_slab_scalar(3, r.xch)
+
+
+def _iteration(ranks, comm, k, u, spectral):
+    """One CG iteration on every rank of this process.  Every kernel returns at once when the stopping decision has been taken."""
+    xs = [r.xch for r in ranks]
+    for r, ui in zip(ranks, u):
+        r.h.fcg_slab_rows_fwd(True, ui)                         # u += alpha p (lagged), p = r + beta p, row transforms of p
+    if spectral:
+        # p.Ap = sum k p^2 + sum shat |P|^2 (Parseval): alpha is known once the ranks' column passes have added up their shares, so
+        # the last pass applies r -= alpha q on the fly -- one pass less than the textbook order, the same two all-reduces
+        _operator_round_trip(ranks, comm, energy=True)          # xch[0] = the rank's share of sum shat |P|^2
+        comm.all_reduce(xs)
+        for r, ki in zip(ranks, k):
+            r.h.fcg_slab_scalar(4, r.xch)                       # alpha
+            r.h.fcg_slab_rows_inv(2, ki, None, None, r.xch)     # r -= alpha (k o p + C p); xch = {r.r, sum k r^2, sum k r p}
+        comm.all_reduce(xs)
+        for r in ranks:
+            r.h.fcg_slab_scalar(5, r.xch)                       # count, convergence, beta, sum k p'^2
+        return
+    _operator_round_trip(ranks, comm)
+    for r, ki in zip(ranks, k):
+        r.h.fcg_slab_rows_inv(0, ki, None, None, r.xch)         # q = k o p + C p; xch[0] = p.q of the own rows
+    comm.all_reduce(xs)
+    for r in ranks:
+        r.h.fcg_slab_scalar(1, r.xch)                           # alpha
+        r.h.fcg_slab_update_r(r.xch)                            # r -= alpha q; xch[0] = r.r of the own rows
+    comm.all_reduce(xs)
+    for r in ranks:
+        r.h.fcg_slab_scalar(2, r.xch)                           # count, convergence, beta
+
+
+def _captured_block(ranks, comm, k, u, spectral, n):
+    """n iterations recorded once into a CUDA graph (stream capture on a side stream: fcg_set_stream) and kept on the first rank
+    object, keyed by the buffers it was recorded for: replaying it costs one launch instead of ~10 n host calls per rank."""
+    key = (tuple(x.data_ptr() for x in list(k) + list(u)), n, bool(spectral), bool(getattr(ranks[0], "peers", False)), len(ranks))
+    cache = ranks[0].__dict__.setdefault("_graphs", {})
+    if key in cache:
+        return cache[key]
+    main = torch.cuda.current_stream()
+    side = torch.cuda.Stream()
+    side.wait_stream(main)
+    old = [r.h.stream for r in ranks]
+    g = torch.cuda.CUDAGraph()
+    c0 = [r.h.fcg_last_launch_count() for r in ranks]
+    try:
+        for r in ranks:
+            r.h.fcg_set_stream(side)
+        with torch.cuda.graph(g, stream=side):
+            for _ in range(n):
+                _iteration(ranks, comm, k, u, spectral)
+    finally:
+        for r, st in zip(ranks, old):
+            r.h.fcg_set_stream(st)
+    main.wait_stream(side)
+    # the library counted the recorded launches once, as if they had run: take them off again; every replay adds them back
+    per = [r.h.fcg_last_launch_count() - c for r, c in zip(ranks, c0)]
+    for r, d in zip(ranks, per):
+        r.replayed_launches = getattr(r, "replayed_launches", 0) - d
+    cache[key] = (g, per)
+    return cache[key]
+
+
+def launch_count(rank_obj) -> int:
+    """Kernels of libfcg that ran for this rank's last solve: the library's own count plus those inside replayed graphs."""
+    return rank_obj.h.fcg_last_launch_count() + getattr(rank_obj, "replayed_launches", 0)
+
+
+def slab_solve(ranks, comm, k, f, u, tol: float, maxit: int, poll_every: int = 8, spectral: bool = True, graph=None):
+    """Solve A u = f with the lattice split by rows over `ranks` (all the ranks of this process: one with DistComm, G with
+    LocalComm).  k, f, u: lists, one tensor of the rank's own rows each; u in: initial guess, out: solution.
+    spectral: the iteration with the spectral search length (three passes, include/fcg.h), else the textbook order (four).
+    graph: replay blocks of poll_every iterations from a CUDA graph recorded at the first use with these buffers (default: on
+    for LocalComm; with DistComm it needs capturable collectives -- NCCL -- and is off unless asked for: not measurable on
+    this one-GPU pool).  Returns (iters, rel_residual, status) -- identical on every rank."""
+    if graph is None:
+        graph = isinstance(comm, LocalComm)
+    n = max(1, int(poll_every))
+    for r in ranks:
+        r.replayed_launches = 0
+    _set_up(ranks, comm, k, f, u, tol, maxit, spectral)
+    blocks = 0
     while True:
         done, it, rr, st = ranks[0].h.fcg_slab_poll()           # every rank holds the same scalars
         if done:
             break
-        for _ in range(max(1, int(poll_every))):
-            for r, ui in zip(ranks, u):
-                r.h.fcg_slab_rows_fwd(True, ui)                 # u += alpha p (lagged), p = r + beta p, row transforms of p
-            _operator_round_trip(ranks, comm)
-            for r, ki in zip(ranks, k):
-                r.h.fcg_slab_rows_inv(False, ki, None, None, r.xch)     # q = k o p + C p; xch[0] = p.q of the own rows
-            comm.all_reduce(xs)
-            for r in ranks:
-                r.h.fcg_slab_scalar(1, r.xch)                   # alpha
-                r.h.fcg_slab_update_r(r.xch)                    # r -= alpha q; xch[0] = r.r of the own rows
-            comm.all_reduce(xs)
-            for r in ranks:
-                r.h.fcg_slab_scalar(2, r.xch)                   # count, convergence, beta
-    for r, ui in zip(ranks, u):
-        r.h.fcg_slab_finish(ui)
-    for r in ranks[1:]:
-        r.h.fcg_slab_poll()
-    return it, rr, st
-
-
-def _slab_solve_spectral(ranks, comm, k, f, u, tol, maxit, poll_every):
-    """p.Ap = sum k p^2 + sum shat |P|^2 (Parseval): alpha is known once the ranks' column passes have added up their shares, so the
-    last pass applies r -= alpha q on the fly -- one pass and one kernel less per iteration than the textbook order, the same two
-    all-reduces (the first one now overlaps the backward exchange's place in the stream)."""
-    xs = [r.xch for r in ranks]
-    for r, ui in zip(ranks, u):
-        r.h.fcg_slab_setup(tol, maxit)
-        r.h.fcg_slab_rows_fwd(False, ui)
-    _operator_round_trip(ranks, comm)
-    for r, ki, fi, ui in zip(ranks, k, f, u):
-        r.h.fcg_slab_rows_inv(1, ki, ui, fi, r.xch)             # r = f - A u, p := 0; xch = {r.r, f.f}
-        r.h.fcg_slab_kpp0(ki, r.xch)                            # xch[2] = sum k r^2 (the first direction is p = r)
-    comm.all_reduce(xs)
-    for r in ranks:
-        r.h.fcg_slab_scalar(0, r.xch)
-        r.h.fcg_slab_scalar(3, r.xch)
-    while True:
-        done, it, rr, st = ranks[0].h.fcg_slab_poll()
-        if done:
-            break
-        for _ in range(max(1, int(poll_every))):
-            for r, ui in zip(ranks, u):
-                r.h.fcg_slab_rows_fwd(True, ui)                 # u += alpha p (lagged), p = r + beta p, row transforms of p
-            _operator_round_trip(ranks, comm, energy=True)      # xch[0] = the rank's share of sum shat |P|^2
-            comm.all_reduce(xs)
-            for r, ki in zip(ranks, k):
-                r.h.fcg_slab_scalar(4, r.xch)                   # alpha
-                r.h.fcg_slab_rows_inv(2, ki, None, None, r.xch)     # r -= alpha (k o p + C p); xch = {r.r, sum k r^2, sum k r p}
-            comm.all_reduce(xs)
-            for r in ranks:
-                r.h.fcg_slab_scalar(5, r.xch)                   # count, convergence, beta, sum k p'^2
+        if graph and blocks >= 1:                               # (the first block runs eagerly: short solves never pay for a capture)
+            g, per = _captured_block(ranks, comm, k, u, spectral, n)
+            g.replay()
+            for r, d in zip(ranks, per):
+                r.replayed_launches += d
+        else:
+            for _ in range(n):
+                _iteration(ranks, comm, k, u, spectral)
+        blocks += 1
     for r, ui in zip(ranks, u):
         r.h.fcg_slab_finish(ui)
     for r in ranks[1:]:

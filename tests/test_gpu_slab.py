@@ -31,7 +31,7 @@ def rel(a, b):
     return np.linalg.norm(a - b) / max(np.linalg.norm(b), 1e-300)
 
 
-def slab_run(w, G, tol, maxit, u0=None, peers=False, spectral=False):
+def slab_run(w, G, tol, maxit, u0=None, peers=False, spectral=False, graph=None):
     from paper_1305_3625_b200 import slab
     dt = w.dtype.type
     sd = dev(w.s)
@@ -40,7 +40,7 @@ def slab_run(w, G, tol, maxit, u0=None, peers=False, spectral=False):
         slab.connect_peers_local(ranks)
     k = [dev(w.k[r.rows]) for r in ranks]; f = [dev(w.f[r.rows]) for r in ranks]
     u = [dev((w.u0 if u0 is None else u0)[r.rows]) for r in ranks]
-    it, rr, st = slab.slab_solve(ranks, slab.LocalComm(), k, f, u, tol, maxit, spectral=spectral)
+    it, rr, st = slab.slab_solve(ranks, slab.LocalComm(), k, f, u, tol, maxit, spectral=spectral, graph=graph)
     out = np.concatenate([x.cpu().numpy() for x in u], axis=0)
     for r in ranks:
         r.close()
@@ -237,3 +237,34 @@ def test_slab_spectral_edge_cases(B):
         it6, _, st6, u6 = slab_run(w, 2, w.tol, 50, spectral=spectral)
         assert st6 == ref["status"] == B.FCG_BREAKDOWN and it6 == ref["iters"]
         assert np.linalg.norm(u6 - ref["u"]) <= 1e-9 * max(np.linalg.norm(ref["u"]), 1e-300) or not (u6.any() or ref["u"].any())
+
+
+@pytest.mark.parametrize("spectral", [True, False])
+@pytest.mark.parametrize("G,peers", [(1, False), (4, False), (4, True)])
+def test_slab_graph_replay_is_bitwise_the_eager_loop(B, G, peers, spectral):
+    """slab_solve replays blocks of eight iterations from a CUDA graph recorded through fcg_set_stream (first block eager, the graph
+    cached on the rank objects per set of buffers).  The same kernels in the same order: count, residual and u bit-identical to
+    the eager loop, the same number of kernels accounted for; a second solve on the same buffers reuses the graph."""
+    from paper_1305_3625_b200 import slab
+    w = inputs.config(1, np.float64, L=512)
+    sd = dev(w.s)
+    ranks = [slab.SlabRank(w.L, torch.float64, G, g, sd) for g in range(G)]
+    if peers:
+        slab.connect_peers_local(ranks)
+    k = [dev(w.k[r.rows]) for r in ranks]; f = [dev(w.f[r.rows]) for r in ranks]
+    u = [dev(w.u0[r.rows]) for r in ranks]
+    res = []
+    for graph in (False, True, True):
+        for x, r in zip(u, ranks):
+            x.copy_(dev(w.u0[r.rows]))
+        out = slab.slab_solve(ranks, slab.LocalComm(), k, f, u, w.tol, w.maxit, spectral=spectral, graph=graph)
+        res.append((out, [x.clone() for x in u], [slab.launch_count(r) for r in ranks]))
+    assert len(ranks[0]._graphs) == 1                                  # recorded once, replayed by the third solve too
+    assert res[0][0][0] > 16 and res[0][0][2] == 0                     # several replayed blocks
+    for other in res[1:]:
+        assert other[0] == res[0][0] and other[2] == res[0][2]
+        assert all(torch.equal(a, b) for a, b in zip(other[1], res[0][1]))
+    ref = orc.cg(w.s, w.k, w.f, w.u0, w.tol, w.maxit)
+    assert rel(np.concatenate([x.cpu().numpy() for x in u], axis=0), ref["u"]) <= TOL_CG[np.float64]
+    for r in ranks:
+        r.close()
