@@ -822,7 +822,7 @@ template <typename T>
 int slab_rows_fwd_impl(fcg_handle h, int mode, void* xu) {
     RowFwdArgs<T> A{}; A.mode = mode; A.x = (const T*)xu; A.u = (T*)xu; A.p = h->at<T>(h->lay.p); A.r = h->at<T>(h->lay.r);
     A.Tb = reinterpret_cast<cx<T>*>(h->ws + h->slab_S); A.tw = h->at<cx<T>>(h->lay.tw); A.sc = h->sc(); A.nsm = h->nsm; A.tmo = &h->sc()->timeout;
-    A.ntile = h->slab_Al; A.astride = h->slab_Al;
+    A.ntile = h->slab_Al; A.astride = h->slab_Al; A.hints = h->hints; A.stagger_ns = h->stagger(0);
     if (h->slab_peer_maps) {
         A.npeer = h->slab_G; A.prank = h->slab_rank; A.mbl = h->slab_MBl;
         for (int g = 0; g < h->slab_G; ++g) A.peerR[g] = reinterpret_cast<cx<T>*>(h->slab_peerR[g]);
@@ -837,6 +837,7 @@ int slab_cols_impl(fcg_handle h, void* xch = nullptr) {       // xch: also this 
     A.sc = h->sc(); A.nsm = h->nsm; A.nranks = h->slab_G; A.al = h->slab_Al; A.boxa = h->slab_boxa;
     A.peer_maps = h->slab_peer_maps; A.prank = h->slab_rank; A.mbl = h->slab_MBl; A.tmo = &h->sc()->timeout; A.col0 = h->slab_rank * ((h->L / 2) / h->slab_G);
     const int ncols = (h->L / 2) / h->slab_G;
+    A.hints = h->hints; A.stagger_ns = h->stagger(1);
     ++h->launches;
     if (xch) {
         A.partial = h->at<double>(h->lay.partial_col);
@@ -865,7 +866,7 @@ int slab_rows_inv_impl(fcg_handle h, int mode, const void* k, const void* v, con
     A.v = mode == ROWI_RESID ? (const T*)v : h->at<T>(h->lay.p);
     A.out = mode == ROWI_RESID ? h->at<T>(h->lay.r) : h->at<T>(h->lay.q); A.out2 = mode == ROWI_RESID ? h->at<T>(h->lay.p) : nullptr;
     A.scale = (T)(1.0 / ((double)h->L * (double)h->L)); A.partial = h->at<double>(h->lay.partial_row); A.sc = h->sc(); A.nsm = h->nsm;
-    A.tmo = &h->sc()->timeout; A.ntile = h->slab_Al; A.xch = (double*)xch;
+    A.tmo = &h->sc()->timeout; A.ntile = h->slab_Al; A.xch = (double*)xch; A.hints = h->hints; A.stagger_ns = h->stagger(2);
     ++h->launches;
     if (mode == ROWI_CGF) {          // q is consumed on the spot: strips k, p, r of the own rows, r in place (fcg_async.cuh, VAR = 5)
         A.f = h->at<T>(h->lay.r); A.out = h->at<T>(h->lay.r); A.out2 = nullptr;
