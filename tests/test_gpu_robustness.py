@@ -91,6 +91,44 @@ def test_pending_loop_guard(B):
     h.close()
 
 
+def test_set_stream_moves_the_work(B):
+    """fcg_set_stream: later calls run on the new stream (checked by recording the solve into a CUDA graph on it: capture fails if
+    any launch went to another stream, and nothing runs until the replay); results identical; refused while a loop is pending."""
+    L = 512
+    w = inputs.config(1, L=L)
+    h = B.Fcg(L, torch.float64)
+    h.fcg_set_option(B.FCG_OPT_FUSED, 0); h.fcg_set_option(B.FCG_OPT_LOOP_MODE, 1)      # direct launches: nothing but kernels and async memsets
+    h.fcg_set_spectrum(dev(w.s))
+    kd, fd, u0, u1 = dev(w.k), dev(w.f), dev(w.u0), dev(w.u0)
+    h.fcg_slab_configure(1, 0)
+    xch = torch.zeros(4, dtype=torch.float64, device="cuda")
+    def passes(u):                                   # the asynchronous slab calls: one operator round trip and the residual
+        h.fcg_slab_setup(1e-10, 5); h.fcg_slab_rows_fwd(False, u); h.fcg_slab_cols(); h.fcg_slab_rows_inv(1, kd, u, fd, xch)
+    passes(u0)
+    torch.cuda.synchronize()
+    want = xch.clone(); xch.zero_()
+    side = torch.cuda.Stream()
+    old = h.stream
+    h.fcg_set_stream(side)
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g, stream=side):
+        passes(u1)
+    torch.cuda.synchronize()
+    assert not xch.any()                             # recorded, not run
+    g.replay(); torch.cuda.synchronize()
+    assert torch.equal(xch, want) and want[0] > 0
+    h.fcg_set_stream(old)
+    w3 = inputs.config(3, L=L, nsteps=4)
+    h2 = B.Fcg(L, torch.float64)
+    h2.fcg_set_spectrum(dev(w3.s))
+    h2.fcg_fracture_begin(dev(w3.k), dev(w3.f), dev(w3.u0), dev(w3.t), 4, w3.tol, w3.maxit, 0)
+    with pytest.raises(B.FcgError) as ei:
+        h2.fcg_set_stream(side)
+    assert ei.value.status == B.FCG_INVALID_ARG
+    h2.fcg_fracture_end()
+    h.close(); h2.close()
+
+
 def test_solve_argument_checks(B):
     L = 64
     w = inputs.config(0)
