@@ -131,8 +131,8 @@ template <int N> __device__ __forceinline__ void bar_named() { asm volatile("bar
 // its arithmetic at 0.7 ns per gathered / scattered cell whatever the cell's size (L = 2048 fp64: 32-byte cells, 18.0 of 27.1 us;
 // L = 8192 fp32: 16-byte cells, 164 of 218 us), i.e. bound by the rate of small requests, not by HBM bytes.  Moving the gather's
 // requests from the TMA engine to the load/store unit did not help -- L = 2048 fp64 28.4 vs 26.7 us, L = 8192 fp32 241 vs 220 us,
-// parity green either way -- so the limit is not the TMA engine's row rate but the L2 sector rate behind both paths (a 16-byte
-// cell still costs a 32-byte sector).  DESIGN.md section 17.
+// parity green either way.  (A later timing probe with every column contiguous in T2 -- one bulk copy per column -- ran the pass
+// only 1.5 us / 4 us faster: the number and size of the copy requests is not what limits it at all.  DESIGN.md section 17.)
 #ifdef FCG_LSU_GATHER
 constexpr bool LSU_GATHER = true;
 #else
