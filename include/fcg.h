@@ -61,8 +61,13 @@ typedef enum {
     FCG_OPT_ROW_VARIANT  = 2, /* -1 (default): tuned rows-per-CTA of the classic row passes; 0,1,..: force variant */
     FCG_OPT_UNROLL       = 4, /* loop mode 0: CG iterations per evaluation of the graph's WHILE condition (default 4, 1..64);
                                  iterations after the stop are no-op launches, results do not depend on it */
-    FCG_OPT_PDL          = 5, /* 1: launch the loop kernels with programmatic stream serialization (the next kernel's
-                                 prologue overlaps the current kernel's tail); 0: plain stream order */
+    FCG_OPT_PDL          = 5, /* programmatic dependent launch of the loop kernels.  0: plain stream order; 1: every loop kernel may
+                                 start under its predecessor's tail (prologue only: nothing the predecessor writes is read before
+                                 griddepcontrol.wait); 2: only the fused last pass starts early and fills its ring of k, p, r strips
+                                 (which the column pass does not write) while the column pass drains -- the column pass triggers its
+                                 dependents after its own wait, so the early section never runs ahead of the previous iteration;
+                                 -1 (default): the measured choice per size (1 at L = 1024 fp64, 2 at L = 1024 fp32, else 0).
+                                 Results do not depend on it */
     FCG_OPT_FUSED        = 6, /* 1 (default): for L = 256 and 512 (pipelined engine, loop mode 0) a whole solve is ONE cooperative
                                  kernel with the vectors resident in shared memory and grid barriers between the phases;
                                  0: the graph of four kernels per iteration at every size */

@@ -80,7 +80,7 @@ struct fcg_handle_s {
     char* ws = nullptr; bool own_ws = false;
     Layout lay{};
     bool have_spectrum = false, have_precond = false;
-    int loop_mode = 0, chunk = 16, row_var_opt = -1, engine_opt = 0, nsm = 148, unroll = 4, pdl = 0, fused_opt = 1, hints = 63, sl_opt = 1, colp_opt = -1;
+    int loop_mode = 0, chunk = 16, row_var_opt = -1, engine_opt = 0, nsm = 148, unroll = 4, pdl_opt = -1, fused_opt = 1, hints = 63, sl_opt = 1, colp_opt = -1;
     alignas(64) CUtensorMap tmap_row;   // T2 as [L/(2 NB)][L/2][128 B]: box = v2_tsub/NB lines of one row pair (row_inv2 tiles)
     alignas(64) CUtensorMap tmap_col;   // T2 as [L/(2 NB)][L/2][NB][2 complex]: box = one column x v2_abox row pairs (col2 gather / scatter)
     bool have_tmap = false;
@@ -89,6 +89,12 @@ struct fcg_handle_s {
     // persistent column pass: measured faster for fp32 (L = 2048: 23.2 -> 20.6 us, L = 4096: 59.1 -> 53.1) and for fp64 up to
     // L = 1024; slower at L = 2048 fp64 (two CTAs of 4 warps per SM instead of three: 26.5 -> 31.0 us), hence the automatic rule
     bool colp() const { return tab->colp_ok && (colp_opt < 0 ? (dtype == FCG_F32 || L <= 1024) : colp_opt != 0); }
+    // programmatic dependent launch of the loop kernels (FCG_OPT_PDL).  Measured per CG iteration, interleaved runs on one B200:
+    // mode 1 (every kernel may start under its predecessor's tail) L = 1024 fp64 37.9 -> 36.2 us, but 2048 fp64 89.1 -> 96.1, 2048 fp32
+    // 57.4 -> 60.2, 4096 fp32 201 -> 218, 8192 fp32 807 -> 839, 1024 fp32 30.4 -> 32.0; mode 2 (only the fused last pass starts early and
+    // fills its strip ring during the column pass's tail) 1024 fp32 30.4 -> 29.9, 1024 fp64 36.7, 2048 fp64 89.4, 4096 fp64 387 -> 385,
+    // others within noise.  Hence the automatic rule: L = 1024 only.
+    int pdl() const { return pdl_opt >= 0 ? pdl_opt : (L == 1024 && v2() ? (dtype == FCG_F64 ? 1 : 2) : 0); }
     // start offsets in ns between the CTAs that share an SM, per pass (P1, P2, P3): -1 = the measured default for this size (stagger())
     int stag_opt[3] = {-1, -1, -1};
     int stagger(int pass) const {
@@ -245,12 +251,12 @@ template <typename T> struct Seq {
     T* q() const { return h->at<T>(h->lay.q); }
 
     cudaError_t row_fwd(int mode, const T* x, T* u, int check_done = 0) const {
-        RowFwdArgs<T> A{}; A.mode = mode; A.x = x; A.u = u; A.p = p(); A.r = pcg ? z() : r(); A.check_done = check_done; A.stagger_ns = mode == ROWF_CG ? h->stagger(0) : 0; A.hints = h->hints; A.Tb = Tb(); A.tw = tw(); A.sc = h->sc(); A.nsm = h->nsm; A.pdl = h->pdl; A.tmo = &h->sc()->timeout;
+        RowFwdArgs<T> A{}; A.mode = mode; A.x = x; A.u = u; A.p = p(); A.r = pcg ? z() : r(); A.check_done = check_done; A.stagger_ns = mode == ROWF_CG ? h->stagger(0) : 0; A.hints = h->hints; A.Tb = Tb(); A.tw = tw(); A.sc = h->sc(); A.nsm = h->nsm; A.pdl = h->pdl(); A.tmo = &h->sc()->timeout;
         ++h->launches;
         return v2() ? h->tab->row_fwd2(&A, st) : h->tab->row_fwd(h->row_var(), &A, st);
     }
     cudaError_t col(int mode, bool cg, bool precond = false) const {
-        ColArgs<T> A{}; A.mode = mode; A.Tb = Tb(); A.shat = precond ? mhat() : shat(); A.hints = h->hints; A.tw = tw(); A.sc = cg ? h->sc() : nullptr; A.pdl = h->pdl; A.tmo = &h->sc()->timeout;
+        ColArgs<T> A{}; A.mode = mode; A.Tb = Tb(); A.shat = precond ? mhat() : shat(); A.hints = h->hints; A.tw = tw(); A.sc = cg ? h->sc() : nullptr; A.pdl = h->pdl(); A.tmo = &h->sc()->timeout;
         A.nsm = h->nsm; A.stagger_ns = cg ? h->stagger(1) : 0;
         ++h->launches;
         if (v2() && mode == COL_CONV && h->colp()) return h->tab->col2p(&A, &h->tmap_col, 0, st);
@@ -259,7 +265,7 @@ template <typename T> struct Seq {
     cudaError_t row_inv(int mode, const T* k, const T* v, const T* f, T* out, T* out2) const {
         RowInvArgs<T> A{}; A.mode = mode; A.Tb = Tb(); A.tw = tw(); A.k = k; A.v = v; A.f = f; A.out = out; A.out2 = out2;
         A.scale = (T)(1.0 / ((double)h->L * (double)h->L)); A.hints = h->hints; A.form = force ? 1 : 0; A.dval = (T)D;
-        A.partial = h->at<double>(h->lay.partial_row); A.sc = h->sc(); A.nsm = h->nsm; A.pdl = h->pdl; A.tmo = &h->sc()->timeout;
+        A.partial = h->at<double>(h->lay.partial_row); A.sc = h->sc(); A.nsm = h->nsm; A.pdl = h->pdl(); A.tmo = &h->sc()->timeout;
         A.stagger_ns = mode == ROWI_CG ? h->stagger(2) : 0;
         ++h->launches;
         return v2() ? h->tab->row_inv2(&A, &h->tmap_row, st) : h->tab->row_inv(h->row_var(), &A, st);
@@ -287,7 +293,7 @@ template <typename T> struct Seq {
     cudaError_t it_col_m() const { return col(COL_CONV, true, true); }
     cudaError_t it_row_pre() const {
         RowInvArgs<T> A{}; A.mode = ROWI_PRECOND; A.Tb = Tb(); A.tw = tw(); A.k = r(); A.out = z(); A.hints = h->hints; A.stagger_ns = h->stagger(2);
-        A.partial = h->at<double>(h->lay.partial_row); A.sc = h->sc(); A.nsm = h->nsm; A.pdl = h->pdl; A.tmo = &h->sc()->timeout;
+        A.partial = h->at<double>(h->lay.partial_row); A.sc = h->sc(); A.nsm = h->nsm; A.pdl = h->pdl(); A.tmo = &h->sc()->timeout;
         ++h->launches;
         return v2() ? h->tab->row_inv2_pre(&A, &h->tmap_row, st) : h->tab->row_inv(h->row_var(), &A, st);
     }
@@ -302,7 +308,7 @@ template <typename T> struct Seq {
             cudaError_t e = it_update_r();
             return e != cudaSuccess ? e : row_fwd(ROWF_PLAIN, r(), nullptr, 1);
         }
-        RowFwdArgs<T> A{}; A.mode = ROWF_RUPD; A.stagger_ns = h->stagger(0); A.hints = h->hints; A.rw = r(); A.q = q(); A.Tb = Tb(); A.tw = tw(); A.sc = h->sc(); A.nsm = h->nsm; A.pdl = h->pdl; A.tmo = &h->sc()->timeout;
+        RowFwdArgs<T> A{}; A.mode = ROWF_RUPD; A.stagger_ns = h->stagger(0); A.hints = h->hints; A.rw = r(); A.q = q(); A.Tb = Tb(); A.tw = tw(); A.sc = h->sc(); A.nsm = h->nsm; A.pdl = h->pdl(); A.tmo = &h->sc()->timeout;
         A.partial = h->at<double>(h->lay.partial_vec);
         ++h->launches;
         return h->tab->row_fwd2_rupd(&A, st);
@@ -321,12 +327,12 @@ template <typename T> struct Seq {
         cudaLaunchAttribute at[1];
         at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
         at[0].val.programmaticStreamSerializationAllowed = 1;
-        cfg.attrs = at; cfg.numAttrs = h->pdl ? 1u : 0u;
+        cfg.attrs = at; cfg.numAttrs = h->pdl() == 1 ? 1u : 0u;
         return cudaLaunchKernelEx(&cfg, cg_update_r_kernel<T>, r(), (const T*)q(), nvec, h->at<double>(h->lay.partial_vec), h->sc(), h->hints, (double*)nullptr);
     }
     // spectral search length: alpha is known after the column pass, so the residual update rides in P3
     cudaError_t it_col_e() const {
-        ColArgs<T> A{}; A.mode = COL_CONV; A.Tb = Tb(); A.shat = shat(); A.hints = h->hints; A.tw = tw(); A.sc = h->sc(); A.pdl = h->pdl; A.tmo = &h->sc()->timeout;
+        ColArgs<T> A{}; A.mode = COL_CONV; A.Tb = Tb(); A.shat = shat(); A.hints = h->hints; A.tw = tw(); A.sc = h->sc(); A.pdl = h->pdl(); A.tmo = &h->sc()->timeout;
         A.partial = h->at<double>(h->lay.partial_col); A.nsm = h->nsm; A.stagger_ns = h->stagger(1);
         ++h->launches;
         if (h->colp()) return h->tab->col2p(&A, &h->tmap_col, 1, st);
@@ -335,7 +341,7 @@ template <typename T> struct Seq {
     cudaError_t it_row_inv_f(const T* k) const {
         RowInvArgs<T> A{}; A.mode = ROWI_CGF; A.Tb = Tb(); A.tw = tw(); A.k = k; A.v = p(); A.f = r(); A.out = r(); A.hints = h->hints; A.stagger_ns = h->stagger(2);
         A.partial = h->at<double>(h->lay.partial_row); A.colsum = h->at<double>(h->lay.partial_col);
-        A.sc = h->sc(); A.nsm = h->nsm; A.pdl = h->pdl; A.tmo = &h->sc()->timeout;
+        A.sc = h->sc(); A.nsm = h->nsm; A.pdl = h->pdl(); A.tmo = &h->sc()->timeout;
         ++h->launches;
         if (force) { A.form = 1; A.kappa = kappa; return h->tab->row_inv2_cgf_force(&A, &h->tmap_row, st); }
         return h->tab->row_inv2_cgf(&A, &h->tmap_row, st);
@@ -466,14 +472,14 @@ int solve_impl(fcg_handle h, const void* k, const void* f, void* u, double tol, 
         const int key = (pcg ? 1 : 0) + 2 * (h->colp() ? 1 : 0) + 4 * h->hints + 1024 * ((h->stagger(0) * 31 + h->stagger(1)) * 31 + h->stagger(2));
         GraphEntry* hit = nullptr;
         for (auto& g : h->graphs)
-            if (g.k == k && g.f == f && g.u == u && g.tol == tol && g.maxit == maxit && g.var == var && g.unroll == h->unroll && g.pdl == h->pdl && g.pcg == key && g.force == (force ? 1 : 0) && g.D == D && g.kappa == kappa) { hit = &g; break; }
+            if (g.k == k && g.f == f && g.u == u && g.tol == tol && g.maxit == maxit && g.var == var && g.unroll == h->unroll && g.pdl == h->pdl() && g.pcg == key && g.force == (force ? 1 : 0) && g.D == D && g.kappa == kappa) { hit = &g; break; }
         if (!hit) {
             if (h->graphs.size() >= 8) {
                 size_t lru = 0;
                 for (size_t i = 1; i < h->graphs.size(); ++i) if (h->graphs[i].stamp < h->graphs[lru].stamp) lru = i;
                 drop_graph(h->graphs[lru]); h->graphs.erase(h->graphs.begin() + lru);
             }
-            GraphEntry ge{k, f, u, tol, maxit, var, h->unroll, h->pdl, key, force ? 1 : 0, D, kappa, nullptr, nullptr, 0};
+            GraphEntry ge{k, f, u, tol, maxit, var, h->unroll, h->pdl(), key, force ? 1 : 0, D, kappa, nullptr, nullptr, 0};
             cudaError_t e = build_graph<T>(h, ge);
             if (e != cudaSuccess) {
                 // conditional graph nodes unavailable: fall back to direct launches for the rest of this handle's life
@@ -988,7 +994,7 @@ int fcg_set_option(fcg_handle h, int option, int value) {
             if (value >= FCG_NROWVAR || (value >= 0 && !h->tab->row_valid[value])) return fail(h, FCG_INVALID_ARG, "row variant not available for this size");
             h->row_var_opt = value; return FCG_OK;
         case FCG_OPT_FUSED: if (value != 0 && value != 1) return fail(h, FCG_INVALID_ARG, "fused must be 0 or 1"); h->fused_opt = value; return FCG_OK;
-        case FCG_OPT_PDL: if (value != 0 && value != 1) return fail(h, FCG_INVALID_ARG, "pdl must be 0 or 1"); h->pdl = value; return FCG_OK;
+        case FCG_OPT_PDL: if (value < -1 || value > 2) return fail(h, FCG_INVALID_ARG, "pdl must be -1, 0, 1 or 2"); h->pdl_opt = value; return FCG_OK;
 #ifdef FCG_PROBE
         case FCG_OPT_L2_HINTS: h->hints = value; return FCG_OK;      // measurement build: the probe bits of fcg_async.cuh too
 #else

@@ -369,7 +369,7 @@ __global__ void __launch_bounds__(P::NT, CTAS) col2_kernel(const ColArgs<T> A, c
     const int lt = threadIdx.x, nl = (int)blockIdx.x, n = SLAB ? nl + A.col0 : nl;      // local (T2 of this launch) and global column
     constexpr int ABOX = AS::ABOX;
     constexpr uint32_t BOXB = (uint32_t)(ABOX * 2 * sizeof(cx<T>));
-    tma::grid_dep_launch();
+    if (A.pdl != 2) tma::grid_dep_launch();                 // pdl == 2: triggered after this kernel's own wait (below), see row_inv2_kernel
     constexpr bool LG = LSU_GATHER && !SLAB;                      // (the slab instantiation keeps the TMA gather: its T2 has another extent)
     if (lt == 0) {
         tma::prefetch_tmap(&tmap);
@@ -381,6 +381,7 @@ __global__ void __launch_bounds__(P::NT, CTAS) col2_kernel(const ColArgs<T> A, c
     static_for_up<1, S - 1>([&](auto s) { base_tw<P, decltype(s)::value, T, GRP>(lt, A.tw, wb[decltype(s)::value]); });
     __syncthreads();                                              // the barriers exist before anybody arrives on them
     tma::grid_dep_wait();                                         // everything above overlaps the previous kernel's tail
+    if (A.pdl == 2) tma::grid_dep_launch();
     // The CTAs that share an SM in the FIRST wave start a fraction of a column time apart (later waves inherit the offsets), so that one's
     // gather overlaps another's arithmetic instead of all of them moving through the same phase together.  Measured at L = 2048 fp64
     // (3 CTAs per SM): 1.5 us apart 93.2 -> 91.7 us per iteration, 0.8 us 91.9, 2 us 92.1, 3 us no gain.
@@ -554,7 +555,7 @@ __global__ void __launch_bounds__(P::NT + 32, CTAS) col2p_kernel(const ColArgs<T
     int cnt = 0;
     while ((int)blockIdx.x + cnt * (int)gridDim.x < L / 2) ++cnt;
     auto col_of = [&](int i) { return (int)blockIdx.x + i * (int)gridDim.x; };
-    tma::grid_dep_launch();
+    if (A.pdl != 2) tma::grid_dep_launch();                 // pdl == 2: triggered after this kernel's own wait (below), see row_inv2_kernel
     if (lt == 0) {
         tma::prefetch_tmap(&tmap);
         for (int b = 0; b < 2; ++b) { tma::mbar_init(&full[b], LSU_GATHER ? 33 : 1); tma::mbar_init(&ready[b], NT / 32); }
@@ -562,6 +563,7 @@ __global__ void __launch_bounds__(P::NT + 32, CTAS) col2p_kernel(const ColArgs<T
     }
     __syncthreads();
     tma::grid_dep_wait();
+    if (A.pdl == 2) tma::grid_dep_launch();
     if (A.sc && A.sc->done) return;                              // before any copy is issued
 
     if (warp == NT / 32) {
@@ -1077,11 +1079,6 @@ __global__ void __launch_bounds__(AsyncShape<T, P>::INV_THREADS, CTAS) row_inv2_
         tma::fence_mbar_init();
     }
     __syncthreads();
-    tma::grid_dep_wait();                                         // everything above overlaps the previous kernel's tail
-    if ((mode == ROWI_CG || PRE || CGF) && A.sc->done) return;
-    if (jj > 0 && A.stagger_ns > 0) {      // the later CTAs of an SM start a fraction of a transform time after the first (see stagger_wait)
-        tma::stagger_wait((unsigned long long)jj * (unsigned long long)A.stagger_ns);
-    }
 
     double acc[2] = {0.0, 0.0};
     double acc3[3] = {0.0, 0.0, 0.0};            // CGF: r'.r', sum k r'^2, sum k r' p
@@ -1120,6 +1117,19 @@ __global__ void __launch_bounds__(AsyncShape<T, P>::INV_THREADS, CTAS) row_inv2_
         ++p_kn;
         if (++p_ks == nks) { p_ks = 0; p_kph ^= 1u; }
     };
+    // pdl == 2 (programmatic dependent launch with the column pass triggering after ITS wait, so that this section never runs before the
+    // previous iteration has completed): the strips k, p, r depend on nothing the column pass writes -- the strip producer fills its
+    // ring during the column pass's tail.
+    constexpr bool EARLY = CGF && !SLAB && PW && AS::NPW == 2;
+    if constexpr (EARLY) {
+        if (A.pdl == 2 && warp == NT / 32 + 1 && !*reinterpret_cast<const volatile int*>(&A.sc->done))
+            while (p_kn < GK && p_kn < nks) issue_next_K();
+    }
+    tma::grid_dep_wait();                                         // everything above overlaps the previous kernel's tail
+    if ((mode == ROWI_CG || PRE || CGF) && A.sc->done) return;
+    if (jj > 0 && A.stagger_ns > 0) {      // the later CTAs of an SM start a fraction of a transform time after the first (see stagger_wait)
+        tma::stagger_wait((unsigned long long)jj * (unsigned long long)A.stagger_ns);
+    }
     if constexpr (SCGF) {
         pq_d = A.sc->pq; alpha_d = A.sc->alpha; alpha = (T)alpha_d;      // (a breakdown has set sc->done: the pass returned above)
     } else if constexpr (CGF) {
@@ -1137,6 +1147,9 @@ __global__ void __launch_bounds__(AsyncShape<T, P>::INV_THREADS, CTAS) row_inv2_
         pq_d = A.sc->kpp + (FCGF ? A.kappa * e : e);
         if (!(pq_d > 0.0) || !isfinite(pq_d)) {                   // breakdown: nothing may change; CTA 0 reports it
             if (blockIdx.x == 0 && lt == 0) { A.sc->pq = pq_d; A.sc->status = ST_BREAKDOWN; A.sc->done = 1; A.sc->alpha = 0.0; set_cond(A.sc, false); }
+            if constexpr (EARLY) {                                // strips issued before the wait must have landed before the CTA leaves
+                if (warp == NT / 32 + 1) for (int s2 = 0; s2 < p_kn; ++s2) tma::mbar_wait(&kfull[s2], 0u, A.tmo);
+            }
             return;
         }
         alpha_d = A.sc->rho / pq_d;

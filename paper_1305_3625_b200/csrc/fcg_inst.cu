@@ -143,14 +143,14 @@ template <typename T> struct Inst {
     static cudaError_t row_fwd2(const void* args, cudaStream_t st) {
         if constexpr (V2) {
             const RowFwdArgs<T>& A = *static_cast<const RowFwdArgs<T>*>(args);
-            return launch(row_fwd2_kernel<T, P, C_FWD>, pgrid(A.nsm, C_FWD), P::NT + 32, AS::fwd_smem, st, A.pdl, A);
+            return launch(row_fwd2_kernel<T, P, C_FWD>, pgrid(A.nsm, C_FWD), P::NT + 32, AS::fwd_smem, st, A.pdl == 1, A);
         }
         return cudaErrorInvalidValue;
     }
     static cudaError_t row_fwd2_rupd(const void* args, cudaStream_t st) {
         if constexpr (V2) {
             const RowFwdArgs<T>& A = *static_cast<const RowFwdArgs<T>*>(args);
-            return launch(row_fwd2_kernel<T, P, C_FWD, 1>, pgrid(A.nsm, C_FWD), P::NT + 32, AS::fwd_smem, st, A.pdl, A);
+            return launch(row_fwd2_kernel<T, P, C_FWD, 1>, pgrid(A.nsm, C_FWD), P::NT + 32, AS::fwd_smem, st, A.pdl == 1, A);
         }
         return cudaErrorInvalidValue;
     }
@@ -163,15 +163,15 @@ template <typename T> struct Inst {
             int grid = A.nsm * CPS::CTAS;
             if (grid > L / 2) grid = L / 2;
             const CUtensorMap& tm = *static_cast<const CUtensorMap*>(tensor_map);
-            if (energy) return launch(col2p_kernel<T, P, CPS::CTAS, true>, grid, P::NT + 32, CPS::smem, st, A.pdl, A, tm);
-            return launch(col2p_kernel<T, P, CPS::CTAS, false>, grid, P::NT + 32, CPS::smem, st, A.pdl, A, tm);
+            if (energy) return launch(col2p_kernel<T, P, CPS::CTAS, true>, grid, P::NT + 32, CPS::smem, st, A.pdl == 1, A, tm);
+            return launch(col2p_kernel<T, P, CPS::CTAS, false>, grid, P::NT + 32, CPS::smem, st, A.pdl == 1, A, tm);
         }
         return cudaErrorInvalidValue;
     }
     static cudaError_t col2_energy(const void* args, const void* tensor_map, cudaStream_t st) {
         if constexpr (SL) {
             const ColArgs<T>& A = *static_cast<const ColArgs<T>*>(args);
-            return launch(col2_kernel<T, P, C_COL, true>, L / 2, P::NT, AS::col_smem, st, A.pdl, A, *static_cast<const CUtensorMap*>(tensor_map));
+            return launch(col2_kernel<T, P, C_COL, true>, L / 2, P::NT, AS::col_smem, st, A.pdl == 1, A, *static_cast<const CUtensorMap*>(tensor_map));
         }
         return cudaErrorInvalidValue;
     }
@@ -202,7 +202,7 @@ template <typename T> struct Inst {
     static cudaError_t col2(const void* args, const void* tensor_map, cudaStream_t st) {
         if constexpr (V2) {
             const ColArgs<T>& A = *static_cast<const ColArgs<T>*>(args);
-            return launch(col2_kernel<T, P, C_COL>, L / 2, P::NT, AS::col_smem, st, A.pdl, A, *static_cast<const CUtensorMap*>(tensor_map));
+            return launch(col2_kernel<T, P, C_COL>, L / 2, P::NT, AS::col_smem, st, A.pdl == 1, A, *static_cast<const CUtensorMap*>(tensor_map));
         }
         return cudaErrorInvalidValue;
     }

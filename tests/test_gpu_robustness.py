@@ -216,3 +216,37 @@ def test_break_step_screen_adversarial(B, dt):
             assert (idx, st) == (io, so) and (ratio == ro or (np.isnan(ratio) and np.isnan(ro))), (name, step, idx, io, ratio, ro)
             assert np.array_equal(kd.cpu().numpy(), ko), (name, step)
     h.close()
+
+
+@pytest.mark.parametrize("L,dt", [(1024, np.float64), (1024, np.float32), (2048, np.float64), (2048, np.float32)])
+def test_programmatic_dependent_launch_modes_bitwise(B, L, dt):
+    """FCG_OPT_PDL 0 / 1 / 2 (include/fcg.h) change only WHEN a loop kernel's prologue runs -- and, in mode 2, when the fused last pass
+    issues its first k, p, r strips -- never what is computed: the three-launch and four-launch CG and PCG, graph and direct-launch
+    loops, must give bit-identical counts, residuals and u in every mode, repeatedly (an early section that ran ahead of the data
+    it reads would show up as a run-to-run or mode-to-mode difference).  The default (-1) is one of the three."""
+    w = inputs.config(2, dt, L=L)
+    kd, fd, sd = dev(w.k), dev(w.f), dev(w.s)
+    kbar = inputs.precond_kbar(w.k)
+    for name, opts, pcg in (("cg3", {}, False), ("cg4", {"FCG_OPT_SPECTRAL_ALPHA": 0}, False), ("direct", {"FCG_OPT_LOOP_MODE": 1}, False),
+                            ("pcg", {}, True)):
+        ref = None
+        for mode in (0, 1, 2, -1):
+            h = B.Fcg(L, TDT[dt])
+            h.fcg_set_option(B.FCG_OPT_FUSED, 0)
+            h.fcg_set_option(B.FCG_OPT_PDL, mode)
+            for k_, v in opts.items():
+                h.fcg_set_option(getattr(B, k_), v)
+            h.fcg_set_spectrum(sd)
+            if pcg:
+                h.fcg_set_preconditioner(sd, kbar)
+            u = torch.zeros((L, L), dtype=TDT[dt], device="cuda")
+            for rep in range(8):
+                u.zero_()
+                r = (h.fcg_pcg_solve if pcg else h.fcg_solve)(kd, fd, u, 0.0, 12)
+                if ref is None:
+                    ref = (r, u.clone())
+                else:
+                    assert r == ref[0] and torch.equal(u, ref[1]), (name, mode, rep)
+            h.close()
+    with pytest.raises(B.FcgError):
+        B.Fcg(L, TDT[dt]).fcg_set_option(B.FCG_OPT_PDL, 3)
