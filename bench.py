@@ -157,17 +157,33 @@ def bench_workload(binding, torch, w, steps, warmup, profile_iters=20, e2e_steps
     ms = h.fcg_profile_iteration(k, f, u, profile_iters)
     out["kernel_ms"] = dict(zip(PASS_NAMES, ms))          # (with three launches ms[3] is the empty event pair)
     # end to end with HOST buffers through the C ABI
-    e2e_steps = e2e_steps or max(1, min(steps, 3))
+    # (every step copies its k, f, u up from pinned host memory and its u back down, inside the timed region; the initial guesses
+    #  -- one zeroed pinned buffer per step -- are prepared before it.)  Two forms of the same public call: blocking
+    #  (fcg_solve_host) and pipelined (fcg_solve_host_submit / _wait: the copies of the neighbouring steps run under the current solve).
+    e2e_steps = e2e_steps or max(1, min(steps, 6))
     kh, fh = torch.from_numpy(w.k.copy()).pin_memory(), torch.from_numpy(w.f.copy()).pin_memory()
-    uh = torch.zeros((w.L, w.L), dtype=tdt).pin_memory()
-    uh.zero_(); h.fcg_solve_host(kh, fh, uh, w.tol, w.maxit)       # warm (allocates the staging buffers)
+    uhs = [torch.zeros((w.L, w.L), dtype=tdt).pin_memory() for _ in range(e2e_steps)]
+    warm = torch.zeros((w.L, w.L), dtype=tdt).pin_memory()
+    h.fcg_solve_host(kh, fh, warm, w.tol, w.maxit)                 # warm (allocates the staging buffers)
+    warm.zero_(); h.fcg_solve_host_submit(kh, fh, warm, w.tol, w.maxit); h.fcg_solve_host_wait()
+    warm.zero_(); h.fcg_solve_host_submit(kh, fh, warm, w.tol, w.maxit); h.fcg_solve_host_wait()      # (both staging sets)
     torch.cuda.synchronize()
     t0 = time.perf_counter(); e_it = 0
-    for _ in range(e2e_steps):
-        uh.zero_()
-        it, _, _ = h.fcg_solve_host(kh, fh, uh, w.tol, w.maxit)
-        e_it += it
+    for i in range(e2e_steps):
+        h.fcg_solve_host_submit(kh, fh, uhs[i], w.tol, w.maxit)
+        if i > 0:
+            e_it += h.fcg_solve_host_wait()[0]
+    e_it += h.fcg_solve_host_wait()[0]
     out["e2e_iter_s"] = e_it / (time.perf_counter() - t0)
+    out["e2e_solution_norm"] = float(uhs[-1].double().norm())
+    nb = min(e2e_steps, 2)
+    for x in uhs[:nb]:
+        x.zero_()
+    t0 = time.perf_counter(); b_it = 0
+    for i in range(nb):
+        b_it += h.fcg_solve_host(kh, fh, uhs[i], w.tol, w.maxit)[0]
+    out["e2e_blocking_iter_s"] = b_it / (time.perf_counter() - t0)
+    out["e2e_steps"] = e2e_steps
     out["h2d"] = 3 * w.N * wbytes; out["d2h"] = w.N * wbytes
     if pcg_steps:
         # the same workload solved by preconditioned CG (time to the same tolerance; reported beside the headline, not as it)
@@ -721,7 +737,10 @@ def main():
                      # the first and the fused last pass are within a few per cent of each other: all three loop kernels, same definition
                      "all_kernels": {n: {"us": 1e3 * kms[n], "achieved": PASS_NW[n] * nw / (kms[n] * 1e-3) / 1e9,
                                          "frac": PASS_NW[n] * nw / (kms[n] * 1e-3) / 1e9 / hbm_peak} for n in PASS_NAMES}},
-        "e2e": {"value": res["e2e_iter_s"], "unit": UNIT, "h2d_bytes_per_step": res["h2d"], "d2h_bytes_per_step": res["d2h"]},
+        "e2e": {"value": res["e2e_iter_s"], "unit": UNIT, "h2d_bytes_per_step": res["h2d"], "d2h_bytes_per_step": res["d2h"],
+                "call": "fcg_solve_host_submit / fcg_solve_host_wait (pinned host buffers, two solves in flight: the copies of step i+1 and "
+                        "i-1 run under solve i)", "steps": res.get("e2e_steps"),
+                "blocking_call_value": res.get("e2e_blocking_iter_s"), "blocking_call": "fcg_solve_host"},
         "gpu_launches": launches,
         "clocks": clocks,
         "final_rel_residual": res["relres"], "status": res["status"],

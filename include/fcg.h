@@ -170,6 +170,16 @@ int fcg_pcg_solve(fcg_handle h, const void* k, const void* f, void* u, double to
  * copies u back.  This is the end-to-end entry point timed by bench.py ("e2e"). */
 int fcg_solve_host(fcg_handle h, const void* k_host, const void* f_host, void* u_host, double tol,
                    int maxit, int* iters_host, double* rel_residual_host);
+/* Pipelined form, up to TWO solves outstanding on a handle: _submit stages the inputs on a stream of its own into one of two device
+ * buffer sets, enqueues the solve behind them on the handle's stream (where the solve is one graph launch nothing blocks; the
+ * one-launch kernel of small lattices and loop mode 1 run to completion inside _submit) and the copy of u back into u_host on a
+ * third stream; _wait blocks until the OLDEST outstanding solve has its result in u_host and returns its status (as fcg_solve),
+ * count and residual.  So the host<->device copies of solve i+1 and i-1 run under solve i.  k_host, f_host, u_host (pinned memory
+ * for real overlap) must stay untouched from _submit until the matching _wait returns; u_host is the initial guess on the way
+ * in and the solution on the way out.  A third _submit without a _wait and a _wait with nothing outstanding return
+ * FCG_INVALID_ARG.  Between a _submit and its _wait call nothing else on the handle but these two. */
+int fcg_solve_host_submit(fcg_handle h, const void* k_host, const void* f_host, void* u_host, double tol, int maxit);
+int fcg_solve_host_wait(fcg_handle h, int* iters_host, double* rel_residual_host);
 
 /* Stand-alone transforms (north_star "fcg_fft_fwd/inv").
  *   x  L x L reals;  X  L x (L/2+1) interleaved complex, row-major [m][n], n = 0..L/2

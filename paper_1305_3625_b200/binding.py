@@ -35,7 +35,7 @@ EXPORTS = ["fcg_workspace_bytes", "fcg_create", "fcg_destroy", "fcg_set_option",
            "fcg_green_function", "fcg_kernel_spectrum", "fcg_force_apply", "fcg_force_solve", "fcg_force_break_step",
            "fcg_force_fracture", "fcg_inverse_spectrum", "fcg_force_rhs", "fcg_force_from_displacement",
            "fcg_force_fracture_displacement", "fcg_force_fracture_displacement_begin", "fcg_force_fracture_displacement_end",
-           "fcg_set_stream", "fcg_slab_shape_of", "fcg_slab_configure", "fcg_slab_buffers", "fcg_slab_set_peers", "fcg_slab_ipc_export", "fcg_slab_ipc_open", "fcg_slab_setup", "fcg_slab_rows_fwd", "fcg_slab_cols", "fcg_slab_cols_energy", "fcg_slab_kpp0", "fcg_slab_rows_inv", "fcg_slab_update_r", "fcg_slab_scalar", "fcg_slab_finish", "fcg_slab_poll",
+           "fcg_set_stream", "fcg_solve_host_submit", "fcg_solve_host_wait", "fcg_slab_shape_of", "fcg_slab_configure", "fcg_slab_buffers", "fcg_slab_set_peers", "fcg_slab_ipc_export", "fcg_slab_ipc_open", "fcg_slab_setup", "fcg_slab_rows_fwd", "fcg_slab_cols", "fcg_slab_cols_energy", "fcg_slab_kpp0", "fcg_slab_rows_inv", "fcg_slab_update_r", "fcg_slab_scalar", "fcg_slab_finish", "fcg_slab_poll",
            "fcg_break_step_static", "fcg_static_last_error"]
 
 
@@ -105,6 +105,8 @@ def lib() -> C.CDLL:
         L.fcg_slab_setup.argtypes = [vp, d, i]; L.fcg_slab_setup.restype = i
         L.fcg_slab_rows_fwd.argtypes = [vp, i, vp]; L.fcg_slab_rows_fwd.restype = i
         L.fcg_set_stream.argtypes = [vp, vp]; L.fcg_set_stream.restype = i
+        L.fcg_solve_host_submit.argtypes = [vp, vp, vp, vp, C.c_double, i]; L.fcg_solve_host_submit.restype = i
+        L.fcg_solve_host_wait.argtypes = [vp, C.POINTER(i), C.POINTER(C.c_double)]; L.fcg_solve_host_wait.restype = i
         L.fcg_slab_cols.argtypes = [vp]; L.fcg_slab_cols.restype = i
         L.fcg_slab_cols_energy.argtypes = [vp, vp]; L.fcg_slab_cols_energy.restype = i
         L.fcg_slab_kpp0.argtypes = [vp, vp, vp]; L.fcg_slab_kpp0.restype = i
@@ -226,6 +228,22 @@ class Fcg:
         it = C.c_int(0); rr = C.c_double(0.0)
         st = self._lib.fcg_solve_host(self._h, k.data_ptr(), f.data_ptr(), u.data_ptr(), float(tol), int(maxit),
                                       C.byref(it), C.byref(rr))
+        if st < 0 and st != FCG_BREAKDOWN:
+            self._raise(st)
+        return int(it.value), float(rr.value), int(st)
+
+    def fcg_solve_host_submit(self, k: torch.Tensor, f: torch.Tensor, u: torch.Tensor, tol: float, maxit: int):
+        """Pipelined fcg_solve_host: returns once the copies and the solve are enqueued (up to two outstanding); keep k, f, u alive
+        and untouched until the matching fcg_solve_host_wait."""
+        for t in (k, f, u):
+            if t.is_cuda or not t.is_contiguous() or t.dtype != self.dtype or t.numel() != self.N:
+                raise ValueError("expected contiguous host tensors of the handle's dtype and size")
+        self._ok(self._lib.fcg_solve_host_submit(self._h, k.data_ptr(), f.data_ptr(), u.data_ptr(), float(tol), int(maxit)))
+
+    def fcg_solve_host_wait(self):
+        """(iters, rel_residual, status) of the oldest outstanding fcg_solve_host_submit; its u tensor now holds the solution."""
+        it = C.c_int(0); rr = C.c_double(0.0)
+        st = self._lib.fcg_solve_host_wait(self._h, C.byref(it), C.byref(rr))
         if st < 0 and st != FCG_BREAKDOWN:
             self._raise(st)
         return int(it.value), float(rr.value), int(st)

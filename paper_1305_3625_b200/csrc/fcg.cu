@@ -73,6 +73,8 @@ struct GraphEntry {
 
 }  // namespace
 
+struct AsyncSolve { int enqueued; long long unroll, outside, per_iteration; };
+
 struct fcg_handle_s {
     int L = 0, dtype = 0; size_t w = 0, N = 0;
     const PassTable* tab = nullptr;
@@ -111,6 +113,14 @@ struct fcg_handle_s {
     BreakResult* h_brk = nullptr;       // pinned
     unsigned long long* h_uni = nullptr; // pinned: result of the reading-F1 check of fcg_force_solve
     void *hk = nullptr, *hf = nullptr, *hu = nullptr;   // device staging of fcg_solve_host
+    // fcg_solve_host_submit / _wait: two staging sets, a stream for the inputs and one for the results, so that the copies of the
+    // neighbouring solves run under the current one
+    void* pset[2][3] = {};
+    cudaStream_t pin_stream = nullptr, pout_stream = nullptr;
+    cudaEvent_t pev_in[2] = {}, pev_solved[2] = {}, pev_out[2] = {};
+    Scalars* pres = nullptr;             // pinned: the scalar block of each outstanding solve
+    int phead = 0, pcount = 0, pstatus[2] = {}, penq[2] = {};
+    long long punroll[2] = {}, poutside[2] = {}, pper[2] = {};
     long long* frac_idx = nullptr; int* frac_it = nullptr; double* frac_ratio = nullptr; int frac_cap = 0;   // device results of the fused quasi-static loop
     int pend_nsteps = -1, pend_done = 0, pend_status = 0; bool pend_async = false;   // fcg_fracture_begin / _end
     std::vector<long long> pend_idx; std::vector<int> pend_it; std::vector<double> pend_ratio;
@@ -429,7 +439,10 @@ cudaError_t build_graph(fcg_handle h, GraphEntry& ge) {
 
 template <typename T>
 int solve_impl(fcg_handle h, const void* k, const void* f, void* u, double tol, int maxit, int* iters, double* relres, bool pcg = false,
-               bool force = false, double D = 0.0) {
+               bool force = false, double D = 0.0, AsyncSolve* async = nullptr) {
+    // async (fcg_solve_host_submit): where the solve is one graph launch, enqueue it and return without waiting; *async then says how
+    // to count its launches once the scalar block has been read back.  Every other path runs to completion as usual (async->enqueued = 0).
+    if (async) async->enqueued = 0;
     h->launches = 0;
     if (h->fused() && !(force && pcg)) {
         // small lattices: the whole solve is one cooperative kernel with the vectors resident in shared memory (fcg_fused.cuh)
@@ -497,6 +510,12 @@ int solve_impl(fcg_handle h, const void* k, const void* f, void* u, double tol, 
         if (hit) {
             hit->stamp = ++h->stamp;
             FCG_CK(h, cudaGraphLaunch(hit->exec, h->stream));
+            if (async) {
+                Seq<T> sq{h, h->stream}; sq.pcg = pcg; sq.force = force; sq.D = D; sq.kappa = kappa;
+                async->enqueued = 1; async->unroll = hit->unroll;
+                async->outside = (kappa > 0.0 ? 1 : 0) + sq.launches_outside_loop(); async->per_iteration = sq.launches_per_iteration();
+                return FCG_OK;
+            }
             FCG_CK(h, cudaStreamSynchronize(h->stream));
             const long long U = hit->unroll;
             Seq<T> sq{h, h->stream}; sq.pcg = pcg; sq.force = force; sq.D = D; sq.kappa = kappa;
@@ -964,6 +983,17 @@ int fcg_destroy(fcg_handle h) {
     if (h->h_sc) cudaFreeHost(h->h_sc);
     if (h->h_brk) cudaFreeHost(h->h_brk);
     if (h->h_uni) cudaFreeHost(h->h_uni);
+    if (h->pin_stream) cudaStreamSynchronize(h->pin_stream);
+    if (h->pout_stream) cudaStreamSynchronize(h->pout_stream);
+    for (int s2 = 0; s2 < 2; ++s2) {
+        for (void* b : h->pset[s2]) if (b) cudaFree(b);
+        if (h->pev_in[s2]) cudaEventDestroy(h->pev_in[s2]);
+        if (h->pev_solved[s2]) cudaEventDestroy(h->pev_solved[s2]);
+        if (h->pev_out[s2]) cudaEventDestroy(h->pev_out[s2]);
+    }
+    if (h->pin_stream) cudaStreamDestroy(h->pin_stream);
+    if (h->pout_stream) cudaStreamDestroy(h->pout_stream);
+    if (h->pres) cudaFreeHost(h->pres);
     if (h->hk) cudaFree(h->hk);
     if (h->hf) cudaFree(h->hf);
     if (h->hu) cudaFree(h->hu);
@@ -1091,6 +1121,74 @@ int fcg_solve_host(fcg_handle h, const void* k_host, const void* f_host, void* u
     FCG_CK(h, cudaMemcpyAsync(u_host, h->hu, bytes, cudaMemcpyDeviceToHost, h->stream));
     FCG_CK(h, cudaStreamSynchronize(h->stream));
     return st;
+}
+
+// Pipelined form of fcg_solve_host (include/fcg.h): up to two solves outstanding.  Inputs go up on their own stream into one of two
+// staging sets, the solve is enqueued behind them on the handle's stream (one graph launch: nothing blocks), the result comes down
+// on a third stream -- so the copies of solve i+1 and of solve i-1 run while solve i computes.
+int fcg_solve_host_submit(fcg_handle h, const void* k_host, const void* f_host, void* u_host, double tol, int maxit) {
+    if (!h || !k_host || !f_host || !u_host) return fail(h, FCG_INVALID_ARG, "null argument");
+    FCG_ENTER(h);
+    if (!(tol >= 0.0) || maxit < 0) return fail(h, FCG_INVALID_ARG, "tol must be >= 0 and maxit >= 0");
+    if (!h->have_spectrum) return fail(h, FCG_NO_SPECTRUM, "fcg_set_spectrum has not been called");
+    if (h->pcount >= 2) return fail(h, FCG_INVALID_ARG, "two solves are outstanding: call fcg_solve_host_wait first");
+    const size_t bytes = h->N * h->w;
+    if (!h->pin_stream) {
+        FCG_CK(h, cudaStreamCreateWithFlags(&h->pin_stream, cudaStreamNonBlocking));
+        FCG_CK(h, cudaStreamCreateWithFlags(&h->pout_stream, cudaStreamNonBlocking));
+        for (int s2 = 0; s2 < 2; ++s2) {
+            FCG_CK(h, cudaEventCreateWithFlags(&h->pev_in[s2], cudaEventDisableTiming));
+            FCG_CK(h, cudaEventCreateWithFlags(&h->pev_solved[s2], cudaEventDisableTiming));
+            FCG_CK(h, cudaEventCreateWithFlags(&h->pev_out[s2], cudaEventDisableTiming));
+        }
+        FCG_CK(h, cudaMallocHost((void**)&h->pres, 2 * sizeof(Scalars)));
+    }
+    const int s2 = (h->phead + h->pcount) % 2;
+    for (int v = 0; v < 3; ++v) if (!h->pset[s2][v]) FCG_CK(h, cudaMalloc(&h->pset[s2][v], bytes));
+    // (this set's previous solve has been waited for: its inputs were consumed and its result is down)
+    FCG_CK(h, cudaMemcpyAsync(h->pset[s2][0], k_host, bytes, cudaMemcpyHostToDevice, h->pin_stream));
+    FCG_CK(h, cudaMemcpyAsync(h->pset[s2][1], f_host, bytes, cudaMemcpyHostToDevice, h->pin_stream));
+    FCG_CK(h, cudaMemcpyAsync(h->pset[s2][2], u_host, bytes, cudaMemcpyHostToDevice, h->pin_stream));
+    FCG_CK(h, cudaEventRecord(h->pev_in[s2], h->pin_stream));
+    FCG_CK(h, cudaStreamWaitEvent(h->stream, h->pev_in[s2], 0));
+    AsyncSolve as{};
+    const int st = h->dtype == FCG_F64
+        ? solve_impl<double>(h, h->pset[s2][0], h->pset[s2][1], h->pset[s2][2], tol, maxit, nullptr, nullptr, false, false, 0.0, &as)
+        : solve_impl<float>(h, h->pset[s2][0], h->pset[s2][1], h->pset[s2][2], tol, maxit, nullptr, nullptr, false, false, 0.0, &as);
+    if (st < 0 && st != FCG_BREAKDOWN) return st;
+    h->penq[s2] = as.enqueued; h->pstatus[s2] = st;
+    if (as.enqueued) {
+        h->punroll[s2] = as.unroll; h->poutside[s2] = as.outside; h->pper[s2] = as.per_iteration;
+        FCG_CK(h, cudaMemcpyAsync(&h->pres[s2], h->sc(), sizeof(Scalars), cudaMemcpyDeviceToHost, h->stream));
+    } else {                              // (one-launch kernel or host-driven loop: the solve has run to completion)
+        h->pres[s2] = *h->h_sc; h->poutside[s2] = h->launches;
+    }
+    FCG_CK(h, cudaEventRecord(h->pev_solved[s2], h->stream));
+    FCG_CK(h, cudaStreamWaitEvent(h->pout_stream, h->pev_solved[s2], 0));
+    FCG_CK(h, cudaMemcpyAsync(u_host, h->pset[s2][2], bytes, cudaMemcpyDeviceToHost, h->pout_stream));
+    FCG_CK(h, cudaEventRecord(h->pev_out[s2], h->pout_stream));
+    ++h->pcount;
+    return FCG_OK;
+}
+
+int fcg_solve_host_wait(fcg_handle h, int* iters_host, double* rel_residual_host) {
+    if (!h) return FCG_INVALID_ARG;
+    FCG_ENTER(h);
+    if (h->pcount < 1) return fail(h, FCG_INVALID_ARG, "no fcg_solve_host_submit is outstanding");
+    const int s2 = h->phead;
+    FCG_CK(h, cudaEventSynchronize(h->pev_out[s2]));
+    h->phead ^= 1; --h->pcount;
+    const Scalars& r = h->pres[s2];
+    if (iters_host) *iters_host = r.it;
+    if (rel_residual_host) *rel_residual_host = r.relres;
+    if (h->penq[s2]) {
+        const long long U = h->punroll[s2];
+        h->launches = h->poutside[s2] + h->pper[s2] * U * ((r.it + U - 1) / U);
+        if (r.timeout) return fail(h, FCG_CUDA_ERROR, "a pipelined pass gave up waiting on an mbarrier (TMA copy never completed)");
+        return r.status;
+    }
+    h->launches = h->poutside[s2];
+    return h->pstatus[s2];
 }
 
 int fcg_fft_fwd(fcg_handle h, const void* x, void* X) {

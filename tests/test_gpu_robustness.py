@@ -250,3 +250,50 @@ def test_programmatic_dependent_launch_modes_bitwise(B, L, dt):
             h.close()
     with pytest.raises(B.FcgError):
         B.Fcg(L, TDT[dt]).fcg_set_option(B.FCG_OPT_PDL, 3)
+
+
+@pytest.mark.parametrize("L,dt,opts", [(1024, np.float64, {}), (2048, np.float32, {}), (512, np.float64, {}),
+                                       (1024, np.float64, {"FCG_OPT_LOOP_MODE": 1}), (64, np.float64, {})])
+def test_solve_host_pipelined_equals_blocking(B, L, dt, opts):
+    """fcg_solve_host_submit / _wait (two solves in flight, copies on their own streams) against fcg_solve_host on the same host
+    buffers: same kernels on the same inputs, so count, residual, status, launch count and u are bit-identical -- for the graph
+    path (really asynchronous), the one-launch kernel of small lattices and the host-driven loop (both run inside _submit), and for
+    the classic engine at L = 64.  Four different right-hand sides in a row, so that both staging sets are reused."""
+    w = inputs.config(1, dt, L=L)
+    rng = np.random.default_rng(3)
+    fs = [w.f] + [(w.f * (1.0 + 0.3 * rng.standard_normal(w.f.shape))).astype(dt) for _ in range(3)]
+    h = B.Fcg(L, TDT[dt])
+    for k_, v in opts.items():
+        h.fcg_set_option(getattr(B, k_), v)
+    h.fcg_set_spectrum(dev(w.s))
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=dt)).pin_memory()
+    kh = pin(w.k); fh = [pin(f) for f in fs]
+    want = []
+    for f in fh:
+        u = pin(np.zeros((L, L)))
+        r = h.fcg_solve_host(kh, f, u, w.tol, w.maxit)
+        want.append((r, u.clone(), h.fcg_last_launch_count()))
+    us = [pin(np.zeros((L, L))) for _ in fh]
+    got = []
+    for i, f in enumerate(fh):
+        h.fcg_solve_host_submit(kh, f, us[i], w.tol, w.maxit)
+        if i > 0:
+            got.append((h.fcg_solve_host_wait(), h.fcg_last_launch_count()))
+    with pytest.raises(B.FcgError):                      # one outstanding: a second _submit is fine, a third is not
+        h.fcg_solve_host_submit(kh, fh[0], pin(np.zeros((L, L))), w.tol, w.maxit)
+        h.fcg_solve_host_submit(kh, fh[0], pin(np.zeros((L, L))), w.tol, w.maxit)
+    while True:                                          # drain whatever is outstanding (the test's last solve first)
+        try:
+            got.append((h.fcg_solve_host_wait(), h.fcg_last_launch_count()))
+        except B.FcgError as e:
+            assert e.status == B.FCG_INVALID_ARG
+            break
+    assert len(got) >= len(fh)
+    for i in range(len(fh)):
+        assert got[i][0] == want[i][0] and got[i][1] == want[i][2], (i, got[i], want[i][0], want[i][2])
+        assert torch.equal(us[i], want[i][1]) and want[i][0][2] == 0
+    ref = orc.cg(w.s, w.k, fs[3], w.u0, w.tol, w.maxit)
+    tol = 1e-9 if dt == np.float64 else 1e-4
+    assert abs(got[3][0][0] - ref["iters"]) <= 2
+    assert np.linalg.norm(us[3].numpy().astype(np.float64) - ref["u"]) / np.linalg.norm(ref["u"]) <= tol or got[3][0][0] != ref["iters"]
+    h.close()
