@@ -322,7 +322,8 @@ int fcg_force_fracture(fcg_handle h, void* k, double D, void* f, const void* t, 
  *                       left it / will take it -- [source rank][local column block][local row pair][line] -- through a 5-D tensor map,
  *                       so nothing is repacked around the exchange.  Returns at once when the solve has finished.
  *   fcg_slab_rows_inv   inverse row transforms of S;  residual = 1: r = f - (k o u + C u), p := 0, xch = { r.r, f.f } of the own rows;
- *                       residual = 0: q = k o p + C p, xch[0] = p.q of the own rows.  xch: device, 2 doubles, caller-owned
+ *                       residual = 0: q = k o p + C p, xch[0] = p.q of the own rows.  xch: device, caller-owned (2 doubles
+ *                       used here, 4 by the three-pass form below: allocate 4)
  *   fcg_slab_update_r   r -= alpha q on the own rows, xch[0] = their r.r
  *   fcg_slab_scalar     the scalar step on the ALL-REDUCED xch: what = 0 after the residual pass (rho, ||f||^2, early exit), 1 after
  *                       rows_inv (alpha, or breakdown), 2 after update_r (count, convergence / maxit, beta, rho)

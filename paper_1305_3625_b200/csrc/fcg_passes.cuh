@@ -104,7 +104,7 @@ template <typename T> struct RowInvArgs {
     unsigned int* tmo;                    // pipelined passes: raised when an mbarrier wait gives up
     int ntile;                            // slab instantiation: row pairs of this rank
     int stagger_ns;                       // start offset between the CTAs that share an SM; 0: none
-    double* xch;                          // slab: the pass's grid-wide sums go HERE (device, 2 doubles) and no scalar step follows:
+    double* xch;                          // slab: the pass's grid-wide sums go HERE (device; 2 doubles, 4 in the fused form) and no scalar step follows:
                                           //       they are this rank's share, to be all-reduced first (fcg_slab_scalar)
 };
 

@@ -6,7 +6,7 @@ and moves the exchange buffers between the ranks:
   * DistComm   one process per GPU (torchrun): torch.distributed all_to_all_single / all_reduce over NCCL on the handle's
                stream; with the gloo backend (CPU tests) the all-to-all is done with isend / irecv, which gloo does have;
   * LocalComm  G logical ranks that share one device and one stream (parity tests on the one-GPU pool): the all-to-all is G*G
-               device copies, the all-reduce a sum of G two-element tensors.
+               device copies, the all-reduce a sum of G four-element tensors.
 
 Per iteration, with the spectral search length (default; DESIGN.md sections 12 and 18):
     rows_fwd | all-to-all S->R | cols_energy (on R, in place) | all-to-all R->S | all-reduce | scalar(4) | rows_inv(2) | all-reduce | scalar(5)
