@@ -59,7 +59,8 @@ typedef enum {
                                     exit early on the device flag, host polls once per chunk */
     FCG_OPT_CHUNK        = 1, /* iterations per chunk in loop mode 1 (default 16) */
     FCG_OPT_ROW_VARIANT  = 2, /* -1 (default): tuned rows-per-CTA of the classic row passes; 0,1,..: force variant */
-    FCG_OPT_UNROLL       = 4, /* loop mode 0: CG iterations per evaluation of the graph's WHILE condition (default 4, 1..64);
+    FCG_OPT_UNROLL       = 4, /* loop mode 0: CG iterations per evaluation of the graph's WHILE condition (1..64; -1, the default: the
+                                 measured choice -- 8 for un-preconditioned fp64 solves at L = 1024 and 2048, 4 otherwise);
                                  iterations after the stop are no-op launches, results do not depend on it */
     FCG_OPT_PDL          = 5, /* programmatic dependent launch of the loop kernels.  0: plain stream order; 1: every loop kernel may
                                  start under its predecessor's tail (prologue only: nothing the predecessor writes is read before
@@ -118,6 +119,9 @@ size_t fcg_workspace_bytes(int L, fcg_dtype dt);
 int fcg_create(int L, fcg_dtype dt, void* workspace, void* cuda_stream, fcg_handle* out);
 int fcg_destroy(fcg_handle h);
 int fcg_set_option(fcg_handle h, int option, int value);
+/* The EFFECTIVE value of an option on this handle, automatic (-1) choices resolved: FCG_OPT_LOOP_MODE, _UNROLL (as an
+ * un-preconditioned solve would use it), _PDL, _FUSED, _SPECTRAL_ALPHA, _COL_PERSISTENT, _STAGGER_P1..P3; FCG_INVALID_ARG for the others. */
+int fcg_get_option(fcg_handle h, int option, int* value);
 /* Later calls enqueue on `cuda_stream` instead of the one given to fcg_create.  The caller orders the two streams (work already
  * enqueued stays where it is); refused (FCG_INVALID_ARG) while a quasi-static loop is pending.  This is what lets a caller
  * record the asynchronous calls (the fcg_slab_* passes, fcg_break_step_static aside) into a CUDA graph of its own: stream

@@ -35,7 +35,7 @@ EXPORTS = ["fcg_workspace_bytes", "fcg_create", "fcg_destroy", "fcg_set_option",
            "fcg_green_function", "fcg_kernel_spectrum", "fcg_force_apply", "fcg_force_solve", "fcg_force_break_step",
            "fcg_force_fracture", "fcg_inverse_spectrum", "fcg_force_rhs", "fcg_force_from_displacement",
            "fcg_force_fracture_displacement", "fcg_force_fracture_displacement_begin", "fcg_force_fracture_displacement_end",
-           "fcg_set_stream", "fcg_solve_host_submit", "fcg_solve_host_wait", "fcg_slab_shape_of", "fcg_slab_configure", "fcg_slab_buffers", "fcg_slab_set_peers", "fcg_slab_ipc_export", "fcg_slab_ipc_open", "fcg_slab_setup", "fcg_slab_rows_fwd", "fcg_slab_cols", "fcg_slab_cols_energy", "fcg_slab_kpp0", "fcg_slab_rows_inv", "fcg_slab_update_r", "fcg_slab_scalar", "fcg_slab_finish", "fcg_slab_poll",
+           "fcg_set_stream", "fcg_get_option", "fcg_solve_host_submit", "fcg_solve_host_wait", "fcg_slab_shape_of", "fcg_slab_configure", "fcg_slab_buffers", "fcg_slab_set_peers", "fcg_slab_ipc_export", "fcg_slab_ipc_open", "fcg_slab_setup", "fcg_slab_rows_fwd", "fcg_slab_cols", "fcg_slab_cols_energy", "fcg_slab_kpp0", "fcg_slab_rows_inv", "fcg_slab_update_r", "fcg_slab_scalar", "fcg_slab_finish", "fcg_slab_poll",
            "fcg_break_step_static", "fcg_static_last_error"]
 
 
@@ -105,6 +105,7 @@ def lib() -> C.CDLL:
         L.fcg_slab_setup.argtypes = [vp, d, i]; L.fcg_slab_setup.restype = i
         L.fcg_slab_rows_fwd.argtypes = [vp, i, vp]; L.fcg_slab_rows_fwd.restype = i
         L.fcg_set_stream.argtypes = [vp, vp]; L.fcg_set_stream.restype = i
+        L.fcg_get_option.argtypes = [vp, i, C.POINTER(i)]; L.fcg_get_option.restype = i
         L.fcg_solve_host_submit.argtypes = [vp, vp, vp, vp, C.c_double, i]; L.fcg_solve_host_submit.restype = i
         L.fcg_solve_host_wait.argtypes = [vp, C.POINTER(i), C.POINTER(C.c_double)]; L.fcg_solve_host_wait.restype = i
         L.fcg_slab_cols.argtypes = [vp]; L.fcg_slab_cols.restype = i
@@ -472,6 +473,12 @@ class Fcg:
     def fcg_slab_ipc_open(self, blobs: bytes):
         buf = C.create_string_buffer(bytes(blobs), len(blobs))
         self._ok(self._lib.fcg_slab_ipc_open(self._h, buf))
+
+    def fcg_get_option(self, option: int) -> int:
+        """The effective value of an option (automatic choices resolved for this size and dtype)."""
+        v = C.c_int(0)
+        self._ok(self._lib.fcg_get_option(self._h, int(option), C.byref(v)))
+        return int(v.value)
 
     def fcg_set_stream(self, stream: torch.cuda.Stream):
         self._ok(self._lib.fcg_set_stream(self._h, stream.cuda_stream))

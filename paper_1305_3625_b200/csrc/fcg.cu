@@ -82,7 +82,7 @@ struct fcg_handle_s {
     char* ws = nullptr; bool own_ws = false;
     Layout lay{};
     bool have_spectrum = false, have_precond = false;
-    int loop_mode = 0, chunk = 16, row_var_opt = -1, engine_opt = 0, nsm = 148, unroll = 4, pdl_opt = -1, fused_opt = 1, hints = 63, sl_opt = 1, colp_opt = -1;
+    int loop_mode = 0, chunk = 16, row_var_opt = -1, engine_opt = 0, nsm = 148, unroll_opt = -1, pdl_opt = -1, fused_opt = 1, hints = 63, sl_opt = 1, colp_opt = -1;
     alignas(64) CUtensorMap tmap_row;   // T2 as [L/(2 NB)][L/2][128 B]: box = v2_tsub/NB lines of one row pair (row_inv2 tiles)
     alignas(64) CUtensorMap tmap_col;   // T2 as [L/(2 NB)][L/2][NB][2 complex]: box = one column x v2_abox row pairs (col2 gather / scatter)
     bool have_tmap = false;
@@ -96,6 +96,12 @@ struct fcg_handle_s {
     // 57.4 -> 60.2, 4096 fp32 201 -> 218, 8192 fp32 807 -> 839, 1024 fp32 30.4 -> 32.0; mode 2 (only the fused last pass starts early and
     // fills its strip ring during the column pass's tail) 1024 fp32 30.4 -> 29.9, 1024 fp64 36.7, 2048 fp64 89.4, 4096 fp64 387 -> 385,
     // others within noise.  Hence the automatic rule: L = 1024 only.
+    // CG iterations per evaluation of the graph's WHILE condition (FCG_OPT_UNROLL; -1 = automatic).  Iterations after the stop are no-op
+    // launches (each kernel returns before it issues anything), an evaluation costs a node boundary.  Measured, whole solves to the
+    // configs' tolerances, us per iteration with 4 / 8 / 16 / 32: L = 2048 fp64 (100 iterations) 87.3 / 85.2 / 87.1 / 86.0, L = 1024 fp64 (77)
+    // 35.6 / 34.5 / 34.8 / 34.7; L = 2048 fp32 (33) 57.5 / 58.5 / 58.5 / 61.6, PCG at L = 2048 fp64 (10) 166 / 170 / 169 / 186, L = 4096 and
+    // 8192: within noise.  Hence 8 for un-preconditioned fp64 solves at L = 1024 and 2048, 4 otherwise.
+    int unroll(bool pcg) const { return unroll_opt > 0 ? unroll_opt : (!pcg && dtype == FCG_F64 && (L == 1024 || L == 2048) ? 8 : 4); }
     int pdl() const { return pdl_opt >= 0 ? pdl_opt : (L == 1024 && v2() ? (dtype == FCG_F64 ? 1 : 2) : 0); }
     // start offsets in ns between the CTAs that share an SM, per pass (P1, P2, P3): -1 = the measured default for this size (stagger())
     int stag_opt[3] = {-1, -1, -1};
@@ -485,14 +491,14 @@ int solve_impl(fcg_handle h, const void* k, const void* f, void* u, double tol, 
         const int key = (pcg ? 1 : 0) + 2 * (h->colp() ? 1 : 0) + 4 * h->hints + 1024 * ((h->stagger(0) * 31 + h->stagger(1)) * 31 + h->stagger(2));
         GraphEntry* hit = nullptr;
         for (auto& g : h->graphs)
-            if (g.k == k && g.f == f && g.u == u && g.tol == tol && g.maxit == maxit && g.var == var && g.unroll == h->unroll && g.pdl == h->pdl() && g.pcg == key && g.force == (force ? 1 : 0) && g.D == D && g.kappa == kappa) { hit = &g; break; }
+            if (g.k == k && g.f == f && g.u == u && g.tol == tol && g.maxit == maxit && g.var == var && g.unroll == h->unroll(pcg) && g.pdl == h->pdl() && g.pcg == key && g.force == (force ? 1 : 0) && g.D == D && g.kappa == kappa) { hit = &g; break; }
         if (!hit) {
             if (h->graphs.size() >= 8) {
                 size_t lru = 0;
                 for (size_t i = 1; i < h->graphs.size(); ++i) if (h->graphs[i].stamp < h->graphs[lru].stamp) lru = i;
                 drop_graph(h->graphs[lru]); h->graphs.erase(h->graphs.begin() + lru);
             }
-            GraphEntry ge{k, f, u, tol, maxit, var, h->unroll, h->pdl(), key, force ? 1 : 0, D, kappa, nullptr, nullptr, 0};
+            GraphEntry ge{k, f, u, tol, maxit, var, h->unroll(pcg), h->pdl(), key, force ? 1 : 0, D, kappa, nullptr, nullptr, 0};
             cudaError_t e = build_graph<T>(h, ge);
             if (e != cudaSuccess) {
                 // conditional graph nodes unavailable: fall back to direct launches for the rest of this handle's life
@@ -1014,6 +1020,22 @@ int fcg_set_stream(fcg_handle h, void* cuda_stream) {
     return FCG_OK;
 }
 
+int fcg_get_option(fcg_handle h, int option, int* value) {
+    if (!h || !value) return FCG_INVALID_ARG;
+    switch (option) {                                  // the EFFECTIVE value: automatic choices resolved for this handle's size and dtype
+        case FCG_OPT_LOOP_MODE: *value = h->loop_mode; return FCG_OK;
+        case FCG_OPT_UNROLL: *value = h->unroll(false); return FCG_OK;
+        case FCG_OPT_PDL: *value = h->pdl(); return FCG_OK;
+        case FCG_OPT_FUSED: *value = h->fused() ? 1 : 0; return FCG_OK;
+        case FCG_OPT_SPECTRAL_ALPHA: *value = h->sl() ? 1 : 0; return FCG_OK;
+        case FCG_OPT_COL_PERSISTENT: *value = h->colp() ? 1 : 0; return FCG_OK;
+        case FCG_OPT_STAGGER_P1: *value = h->stagger(0); return FCG_OK;
+        case FCG_OPT_STAGGER_P2: *value = h->stagger(1); return FCG_OK;
+        case FCG_OPT_STAGGER_P3: *value = h->stagger(2); return FCG_OK;
+        default: return fail(h, FCG_INVALID_ARG, "fcg_get_option: option has no readable value");
+    }
+}
+
 int fcg_set_option(fcg_handle h, int option, int value) {
     if (!h) return FCG_INVALID_ARG;
     FCG_ENTER_OPT(h);
@@ -1038,7 +1060,7 @@ int fcg_set_option(fcg_handle h, int option, int value) {
         case FCG_OPT_STAGGER_P1: case FCG_OPT_STAGGER_P2: case FCG_OPT_STAGGER_P3:
             if (value < -1 || value > 100000) return fail(h, FCG_INVALID_ARG, "stagger must be -1 (default) or 0..100000 ns");
             h->stag_opt[option - FCG_OPT_STAGGER_P1] = value; return FCG_OK;
-        case FCG_OPT_UNROLL: if (value < 1 || value > 64) return fail(h, FCG_INVALID_ARG, "unroll must be 1..64"); h->unroll = value; return FCG_OK;
+        case FCG_OPT_UNROLL: if ((value < 1 && value != -1) || value > 64) return fail(h, FCG_INVALID_ARG, "unroll must be 1..64 or -1"); h->unroll_opt = value; return FCG_OK;
         case FCG_OPT_ENGINE:
             if (value != 0 && value != 1) return fail(h, FCG_INVALID_ARG, "engine must be 0 or 1");
             h->engine_opt = value;

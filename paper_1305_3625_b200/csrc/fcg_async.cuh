@@ -385,6 +385,7 @@ __global__ void __launch_bounds__(P::NT, CTAS) col2_kernel(const ColArgs<T> A, c
     // The CTAs that share an SM in the FIRST wave start a fraction of a column time apart (later waves inherit the offsets), so that one's
     // gather overlaps another's arithmetic instead of all of them moving through the same phase together.  Measured at L = 2048 fp64
     // (3 CTAs per SM): 1.5 us apart 93.2 -> 91.7 us per iteration, 0.8 us 91.9, 2 us 92.1, 3 us no gain.
+    if (A.sc && A.sc->done) return;                               // after the stop: before any copy is issued (a no-op launch costs its launch only)
     if (A.stagger_ns > 0 && blockIdx.x >= (unsigned)A.nsm && blockIdx.x < (unsigned)(CTAS * A.nsm)) {
         tma::stagger_wait((unsigned long long)(blockIdx.x / (unsigned)A.nsm) * (unsigned long long)A.stagger_ns);
     }
@@ -414,9 +415,7 @@ __global__ void __launch_bounds__(P::NT, CTAS) col2_kernel(const ColArgs<T> A, c
         if (n) tma::bulk_g2s_hint(sh, A.shat + (size_t)n * L, (uint32_t)(L * sizeof(T)), &bar,
                                   (A.hints & 4) ? tma::policy_evict_first() : tma::policy_evict_normal());   // read once per iteration
     }
-    const bool done = A.sc && A.sc->done;
     if (!FCG_PROBE_ON(0x200)) tma::mbar_wait(&bar, 0, A.tmo);
-    if (done) return;
     double energy = 0.0;
 
     auto ld_sw = [&](int e) { return io.ld(e); };

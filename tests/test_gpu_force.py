@@ -340,7 +340,8 @@ def test_force_three_launch_iteration(B, L, dt):
     force_parity(B, L, dt, 10, FCG_OPT_FUSED=0, FCG_OPT_SPECTRAL_ALPHA=0)           # four
     _, g = green_spectrum_oracle(L, dt)
     k = inputs.force_k(L, 7, 2.5 if dt == np.float64 else 1.0).astype(dt)           # (another elastic constant: kappa must reach the pass)
-    count = lambda it, per, extra: extra + per * 4 * ((it + 3) // 4)
+    hU = handle(B, L, dt, g, FCG_OPT_FUSED=0); U = hU.fcg_get_option(B.FCG_OPT_UNROLL); hU.close()    # WHILE body: 4, or 8 (include/fcg.h)
+    count = lambda it, per, extra: extra + per * U * ((it + U - 1) // U)
     sols = []
     for sa in (1, 0):
         h = handle(B, L, dt, g, FCG_OPT_FUSED=0, FCG_OPT_SPECTRAL_ALPHA=sa)

@@ -176,7 +176,8 @@ def cg_parity(B, w, **opts):
     assert abs(it - ref["iters"]) <= 2, (it, ref["iters"], ref["hist"][-4:])
     # graph path: set-up 4 + finish 1 + 4 kernels x (iterations rounded up to the WHILE body's 4); fused path (L = 256, 512): 1
     # spectral search length (default): set-up 5 + finish 1 + 3 kernels x ...
-    assert h.fcg_last_launch_count() in (1, 5 + 16 * ((it + 3) // 4), 6 + 12 * ((it + 3) // 4)) or opts
+    U = h.fcg_get_option(B.FCG_OPT_UNROLL)                                # (4, or 8 for fp64 at L = 1024 / 2048: include/fcg.h)
+    assert h.fcg_last_launch_count() in (1, 5 + 4 * U * ((it + U - 1) // U), 6 + 3 * U * ((it + U - 1) // U)) or opts
     u_nat = u.cpu().numpy()
     d_nat = rel(u_nat, ref["u"])
     d_pin = d_nat
@@ -263,7 +264,8 @@ def test_cg_fused_kernel(B, cfg, L):
         h = handle(B, L, np.float64, w.s, FCG_OPT_FUSED=fused)
         u = dev(w.u0)
         it, rr, st = h.fcg_solve(dev(w.k), dev(w.f), u, w.tol, w.maxit)
-        assert st == 0 and h.fcg_last_launch_count() == (1 if fused else 6 + 12 * ((it + 3) // 4))
+        U = h.fcg_get_option(B.FCG_OPT_UNROLL)
+        assert st == 0 and h.fcg_last_launch_count() == (1 if fused else 6 + 3 * U * ((it + U - 1) // U))
         us.append((it, u.cpu().numpy()))
         h.close()
     assert us[0][0] == us[1][0] and np.array_equal(us[0][1], us[1][1])          # repeatable
@@ -338,10 +340,11 @@ def test_cg_both_search_length_evaluations(B, cfg, L, dt):
         h = handle(B, L, dt, w.s, FCG_OPT_FUSED=0, FCG_OPT_SPECTRAL_ALPHA=sl)
         u = dev(w.u0)
         r = h.fcg_solve(dev(w.k), dev(w.f), u, 0.0, it_or)          # pinned count
-        c = (it_or + 3) // 4                                        # the classic engine (small transforms) always takes 4 launches
-        assert h.fcg_last_launch_count() == 5 + 16 * c or (sl == 1 and h.fcg_last_launch_count() == 6 + 12 * c)
+        U = h.fcg_get_option(B.FCG_OPT_UNROLL)
+        c = U * ((it_or + U - 1) // U)                              # the classic engine (small transforms) always takes 4 launches
+        assert h.fcg_last_launch_count() == 5 + 4 * c or (sl == 1 and h.fcg_last_launch_count() == 6 + 3 * c)
         if sl == 1 and (L >= 1024 or dt == np.float64 and L >= 256):
-            assert h.fcg_last_launch_count() == 6 + 12 * c
+            assert h.fcg_last_launch_count() == 6 + 3 * c
         outs.append((it, r, u.cpu().numpy()))
         h.close()
     assert abs(outs[0][0] - outs[1][0]) <= 1
