@@ -147,6 +147,9 @@ def bench_workload(binding, torch, w, steps, warmup, profile_iters=20, e2e_steps
     wall = time.perf_counter() - t0
     dev_ms = [a.elapsed_time(b) for a, b in ev]
     out = {"iters": iters, "status": st, "relres": rr, "dev_ms": dev_ms, "wall_s": wall, "launches": launches}
+    # the library's automatic choices for this size and dtype (include/fcg.h: fcg_get_option)
+    out["options"] = {n: h.fcg_get_option(getattr(binding, "FCG_OPT_" + n)) for n in
+                      ("LOOP_MODE", "UNROLL", "PDL", "FUSED", "SPECTRAL_ALPHA", "COL_PERSISTENT", "STAGGER_P1", "STAGGER_P2", "STAGGER_P3")}
     # per-kernel times, in loop order, CUDA events on the library's stream
     u.zero_()
     if solver == "pcg":
@@ -725,7 +728,7 @@ def main():
                                f"({it_per_solve} iterations)", "L": w.L, "iterations_per_solve": it_per_solve,
                    "l2_policy": f"inputs larger than L2: working set {7.5 * nw / 2**20:.0f} MiB per solve vs 126 MB L2; no flush",
                    "parallelism": "replicas only" if world > 1 else "single GPU",
-                   "launches_per_iteration": len(PASS_NAMES)},
+                   "launches_per_iteration": len(PASS_NAMES), "library_options": res.get("options")},
         "site_iterations_per_s": value * w.N,
         "us_per_iteration": t_iter_us,
         "iteration_roofline": iteration_roofline(nw, t_iter_us, hbm_peak, peak_src, dram_iter),
