@@ -297,3 +297,31 @@ def test_solve_host_pipelined_equals_blocking(B, L, dt, opts):
     assert abs(got[3][0][0] - ref["iters"]) <= 2
     assert np.linalg.norm(us[3].numpy().astype(np.float64) - ref["u"]) / np.linalg.norm(ref["u"]) <= tol or got[3][0][0] != ref["iters"]
     h.close()
+
+
+@pytest.mark.parametrize("dt", [np.float64, np.float32])
+def test_fracture_loop_with_automatic_launch_options(B, dt):
+    """The quasi-static loop (solve, break, warm-started solve, ..) as a graph of pipelined kernels at L = 1024, where the library
+    chooses programmatic dependent launch and a WHILE body of 8 by itself: break indices, iteration counts, k and u must be
+    bit-identical to the same loop with plain launches and a body of 4, and to the direct-launch loop."""
+    L, steps = 1024, 10
+    w = inputs.config(3, dt, L=L, nsteps=steps)
+    tol = w.tol if dt == np.float64 else 1e-5
+    res = []
+    for opts in ({}, {"FCG_OPT_PDL": 0, "FCG_OPT_UNROLL": 4}, {"FCG_OPT_PDL": 0, "FCG_OPT_LOOP_MODE": 1}):
+        h = B.Fcg(L, TDT[dt])
+        for k_, v in opts.items():
+            h.fcg_set_option(getattr(B, k_), v)
+        if not opts:
+            assert h.fcg_get_option(B.FCG_OPT_PDL) == (1 if dt == np.float64 else 2)
+            assert h.fcg_get_option(B.FCG_OPT_UNROLL) == (8 if dt == np.float64 else 4)
+        h.fcg_set_spectrum(dev(w.s))
+        kd, ud = dev(w.k), dev(w.u0)
+        index, iters, done, st = h.fcg_fracture(kd, dev(w.f), ud, dev(w.t), steps, tol, w.maxit)
+        assert done == steps and st == 0
+        res.append((index, iters, kd.cpu().numpy(), ud.cpu().numpy()))
+        h.close()
+    for other in res[1:]:
+        assert np.array_equal(other[0], res[0][0]) and np.array_equal(other[1], res[0][1])
+        assert np.array_equal(other[2], res[0][2]) and np.array_equal(other[3], res[0][3])
+    assert res[0][0][0] == int(np.argmin(w.t)) and len(set(res[0][0].tolist())) == steps
