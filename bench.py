@@ -92,7 +92,7 @@ def run_reference(args, rank: int):
     if rank != 0:
         return
     from paper_1305_3625_b200 import inputs
-    w = inputs.config(args.config, np.float64 if args.dtype == "f64" else np.float32)
+    w = workload_of(inputs, args)
     sample = args.ref_iters
     for _ in range(args.warmup):
         oracle_sample(w, 1)
@@ -471,6 +471,13 @@ def iteration_roofline(nw, t_iter_us, hbm_peak, peak_src, dram_iter):
     return d
 
 
+def workload_of(inputs, args):
+    """BASELINE.json configs[args.config] in args.dtype; --L: the same recipe at another lattice size (a parity-test case of the
+    suite, e.g. L = 1024, the largest size of the paper -- never the headline: the JSON line's workload string says so)."""
+    dt = np.float64 if args.dtype == "f64" else np.float32
+    return inputs.config(args.config, dt) if args.L is None else inputs.config(args.config, dt, L=args.L)
+
+
 def run_slab(args, rank, world, local):
     """--shard slab: ONE solve spread over the ranks by rows instead of one
     replica per rank.  Under torchrun every process is one rank (DistComm: NCCL all-to-all of the half spectrum around the column
@@ -481,7 +488,7 @@ def run_slab(args, rank, world, local):
     from paper_1305_3625_b200 import binding, inputs, slab
     torch.cuda.set_device(local)
     tdt = torch.float64 if args.dtype == "f64" else torch.float32
-    w = inputs.config(args.config, np.float64 if args.dtype == "f64" else np.float32)
+    w = workload_of(inputs, args)
     to = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
     if world > 1:
         os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
@@ -563,6 +570,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--dtype", choices=["f64", "f32"], default="f64")
     ap.add_argument("--config", type=int, default=2, choices=[0, 1, 2, 4])
+    ap.add_argument("--L", type=int, default=None, choices=[256, 512, 1024, 2048, 4096, 8192],
+                    help="the config's recipe at another lattice size (default: the config's own L)")
     ap.add_argument("--impl", choices=["fcg", "reference"], default="fcg")
     ap.add_argument("--ref-iters", type=int, default=8, help="oracle CG iterations per step of --impl reference")
     ap.add_argument("--cpu-baseline-iters", type=int, default=None,
@@ -612,7 +621,7 @@ def main():
     if world > 1:
         os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-    w = inputs.config(args.config, np.float64 if args.dtype == "f64" else np.float32)
+    w = workload_of(inputs, args)
     wbytes = w.dtype.itemsize
     hbm_peak, peak_src = peaks()
 
@@ -724,7 +733,7 @@ def main():
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": step_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": args.dtype, "data": "synthetic",
-        "config": {"workload": f"BASELINE.json configs[{args.config}]: L={w.L} {args.dtype}, tol={w.tol:g}, one step = one full CG solve from u0=0 "
+        "config": {"workload": f"BASELINE.json configs[{args.config}]{'' if args.L is None else ' recipe at another size'}: L={w.L} {args.dtype}, tol={w.tol:g}, one step = one full CG solve from u0=0 "
                                f"({it_per_solve} iterations)", "L": w.L, "iterations_per_solve": it_per_solve,
                    "l2_policy": f"inputs larger than L2: working set {7.5 * nw / 2**20:.0f} MiB per solve vs 126 MB L2; no flush",
                    "parallelism": "replicas only" if world > 1 else "single GPU",
@@ -750,7 +759,7 @@ def main():
     }
     if "pcg" in res:
         line["pcg"] = res["pcg"]
-    if world == 1 and not args.no_configs and args.config == 2 and args.dtype == "f64" and args.loop_mode == 0:
+    if world == 1 and not args.no_configs and args.config == 2 and args.dtype == "f64" and args.loop_mode == 0 and args.L is None:
         line["configs"] = bench_configs(binding, torch, inputs, hbm_peak)          # outside the timed region of the headline
     if args.full and world == 1:
         line["extra"] = bench_extras(binding, torch, inputs)
